@@ -1,0 +1,158 @@
+/* mtp_b200.h -- C ABI of the B200-native Moment Tensor Potential hot path.
+ *
+ * What is computed (BASELINE.json north_star; "Inference computes energies,
+ * forces, and stresses"; PAPER.md:35,46 configuration-/neighbourhood-mode grades;
+ * PAPER.md:62,76 chunked evaluation).  PAPER.md prints no formula; the definitions below
+ * restate north_star with the readings G1-G24 listed in DESIGN.md:
+ *
+ *   r_ij = x_j - x_i + s.H                       (s: image shift, H rows = lattice vectors)
+ *   Q_b(r) = T_b(xi(r)) (R_cut - r)^2,  xi = (2r - R_min - R_cut)/(R_cut - R_min), b < n_beta
+ *   f_mu(r) = sum_b c[z_i][z_j][mu][b] Q_b(r)
+ *   M_{mu,(a,b,c)} = sum_j f_mu(|r_ij|) x^a y^b z^c          (packed symmetric components)
+ *   node[dst] += mult * node[src0] * node[src1]              (contraction table, in order)
+ *   B_alpha = node[basis_node[alpha]],  E_i = xi0[z_i] + sum_alpha xi[alpha] B_alpha
+ *   d_ij = dE_i/dr_ij (reverse pass),  F_k = sum_j d_kj - sum_{i: k in N(i)} d_ik
+ *   W_ab = -sum_i sum_j r_ij,a d_ij,b ;  E = sum_i E_i
+ *   gamma_i = max_k | sum_alpha B_alpha(n_i) Ainv[alpha][k] |     (neighbourhood mode)
+ *   gamma   = max_k | sum_alpha (sum_i B_alpha(n_i)) Ainv[alpha][k] |  (configuration mode)
+ *
+ * Conventions: every pointer named d_* is a DEVICE pointer owned by the caller; every
+ * other pointer is a HOST pointer.  All floating point is IEEE fp64.  Calls enqueue work
+ * on `cuda_stream` (a cudaStream_t passed as void*; NULL = legacy default stream) and
+ * return without synchronising the host.  Outputs are overwritten, never accumulated.
+ * Return value: 0 on success, a negative MTP_E* code otherwise; nothing aborts or throws.
+ * There is no CPU fallback: without a CUDA device mtp_create fails with MTP_ECUDA.
+ */
+#ifndef MTP_B200_H
+#define MTP_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MTP_OK 0
+#define MTP_EINVAL (-1)   /* bad argument / malformed table                              */
+#define MTP_ESIZE (-2)    /* workspace too small (see mtp_workspace_bytes)               */
+#define MTP_EBOX (-3)     /* d_shift == NULL but a box height is < 2 R_cut               */
+#define MTP_ECUDA (-4)    /* CUDA runtime error; text in mtp_last_error                  */
+#define MTP_EUNSUP (-5)   /* table outside the compiled kernel family (level > 28, ...)  */
+#define MTP_ENOMEM (-6)
+
+typedef struct mtp_handle mtp_handle;
+
+/* Potential description.  HOST pointers, copied at mtp_create.
+ * The table fields (basic .. basis_desc) are what mtp_enumerate emits (row a0 of
+ * "host-side basis enumerator that emits the contraction table"). */
+typedef struct {
+  int32_t n_species;        /* S                                                         */
+  int32_t n_radial_basis;   /* n_beta (8 in every BASELINE config), 1..16                */
+  int32_t n_radial_funcs;   /* n_mu                                                       */
+  double r_min, r_cut;      /* Angstrom                                                   */
+  int32_t lev_max;          /* informational                                              */
+  int32_t n_basic;          /* number of packed moment components                         */
+  const int32_t *basic;     /* [n_basic][4] = mu, a, b, c  (a+b+c = nu)                   */
+  int32_t n_nodes;          /* n_basic + intermediate components; node k<n_basic = basic k*/
+  int32_t n_prod;
+  const int32_t *prod;      /* [n_prod][4] = src0, src1, mult, dst; evaluation order;
+                               a node is final after the last op that writes it and may
+                               only be read after that; dst >= n_basic                    */
+  int32_t n_basis;
+  const int32_t *basis_node;/* [n_basis] node id of B_alpha, canonical alpha order (G11)  */
+  const double *c;          /* [S][S][n_mu][n_beta]  index z_i, z_j, mu, beta (G6)        */
+  const double *xi0;        /* [S]                                                        */
+  const double *xi;         /* [n_basis]                                                  */
+  /* description of each basis function as a multigraph, for cross-checking the order:
+     per function: n_components, then per component n_vertices, (mu,nu) per vertex,
+     upper-triangular adjacency (row-major).  Ignored by mtp_create; may be NULL.         */
+  int32_t n_desc;
+  const int32_t *basis_desc;
+  const int32_t *basis_desc_off; /* [n_basis+1] offsets into basis_desc                   */
+} mtp_params;
+
+/* a0.  Enumerate every scalar contraction with total level <= lev_max (lev(M_{mu,nu}) =
+ * 2+4mu+nu; readings G8, G9, G11, G12, G22) and emit the packed-component contraction
+ * table.  Fills the table fields of *out (n_radial_funcs, lev_max, n_basic .. basis_desc_off)
+ * with malloc'ed arrays; release with mtp_table_free.  lev_max in [2, 28]. */
+int mtp_enumerate(int32_t lev_max, mtp_params *out);
+void mtp_table_free(mtp_params *table);
+
+/* Create / destroy.  Validates the table, compiles it into the kernels' schedules and
+ * copies c, xi0, xi and the schedules to the current CUDA device. */
+int mtp_create(mtp_handle **out, const mtp_params *p);
+void mtp_destroy(mtp_handle *h);
+const char *mtp_last_error(const mtp_handle *h); /* h may be NULL: last create error     */
+
+/* Options (a10 chunk scheduler PAPER.md:62,76; a8 force mode; a12 variant PAPER.md:35). */
+#define MTP_OPT_CHUNK_ATOMS 1   /* atoms per chunk; 0 = automatic (L2-sized)               */
+#define MTP_OPT_FORCE_MODE 2    /* MTP_FORCE_GATHER (needs d_rev) | MTP_FORCE_ATOMIC       */
+#define MTP_OPT_VARIANT 3       /* MTP_VARIANT_AUTO | _THREAD | _BLOCK                     */
+#define MTP_FORCE_GATHER 0
+#define MTP_FORCE_ATOMIC 1
+#define MTP_VARIANT_AUTO 0
+#define MTP_VARIANT_THREAD 1    /* one thread group per atom walks all neighbours (large N) */
+#define MTP_VARIANT_BLOCK 2     /* neighbours split across lanes, shuffle-reduced (small N) */
+int mtp_set_option(mtp_handle *h, int key, int64_t value);
+int mtp_get_option(const mtp_handle *h, int key, int64_t *value);
+
+/* Bytes of device workspace mtp_compute / mtp_grade need for this input size under the
+ * current options. */
+int mtp_workspace_bytes(const mtp_handle *h, int64_t n_atoms, int64_t nnz, int want_grade,
+                        size_t *out_bytes);
+
+/* a1-a8, a10.  Energy, per-atom energy, forces, virial over a full CSR neighbour list.
+ *   d_pos   [N][3] f64      d_type [N] i32 in [0,S)
+ *   box     [9] HOST, rows = lattice vectors
+ *   d_off   [N+1] i64       d_idx [nnz] i32  (entries with r >= R_cut contribute nothing)
+ *   d_shift [nnz][3] i8 image shifts, or NULL = minimum image (needs heights > 2 R_cut)
+ *   d_rev   [nnz] i32 position of the reverse pair, required in MTP_FORCE_GATHER mode
+ *   d_E [1], d_Ei [N] or NULL, d_F [N][3], d_virial [6] = xx,yy,zz,xy,xz,yz (eV) or NULL
+ *   d_ws / ws_bytes: scratch of at least mtp_workspace_bytes(...). */
+int mtp_compute(mtp_handle *h, int64_t n_atoms, const double *d_pos, const int32_t *d_type,
+                const double *box, const int64_t *d_off, const int32_t *d_idx,
+                const int8_t *d_shift, const int32_t *d_rev, int64_t nnz, double *d_E,
+                double *d_Ei, double *d_F, double *d_virial, void *d_ws, size_t ws_bytes,
+                void *cuda_stream);
+
+/* a9.  Extrapolation grades (values are produced only by this call, so
+ * there is no stale state as in PAPER.md:100,125).
+ *   d_Ainv [n_basis][n_basis] row-major [alpha][k]
+ *   mode: 0 neighbourhood (d_gamma_atom [N]), 1 configuration (d_gamma_cfg [1]), 2 both
+ *   d_Bsum [n_basis] or NULL: sum_i B(n_i);  d_B [N][n_basis] or NULL: the basis values */
+int mtp_grade(mtp_handle *h, int64_t n_atoms, const double *d_pos, const int32_t *d_type,
+              const double *box, const int64_t *d_off, const int32_t *d_idx,
+              const int8_t *d_shift, int64_t nnz, const double *d_Ainv, int mode,
+              double *d_gamma_atom, double *d_gamma_cfg, double *d_Bsum, double *d_B,
+              void *d_ws, size_t ws_bytes, void *cuda_stream);
+
+/* Host-buffer convenience path (the end-to-end call bench.py's `e2e` times): same
+ * arguments as mtp_compute but every array is a HOST pointer; the library stages them
+ * through its own pinned + device buffers, runs mtp_compute and copies E, E_i, F, virial
+ * back, synchronising before it returns. */
+int mtp_compute_host(mtp_handle *h, int64_t n_atoms, const double *pos, const int32_t *type,
+                     const double *box, const int64_t *off, const int32_t *idx,
+                     const int8_t *shift, const int32_t *rev, int64_t nnz, double *E,
+                     double *Ei, double *F, double *virial);
+
+/* Diagnostics (parity bring-up and roofline denominators; not part of the hot path). */
+/* Copy the last chunk-0 intermediate arrays of the most recent mtp_compute: moments
+ * M [n][n_basic], adjoints G [n][n_basic] for the first n atoms (device buffers). */
+int mtp_debug_moments(mtp_handle *h, int64_t n_atoms, const double *d_pos,
+                      const int32_t *d_type, const double *box, const int64_t *d_off,
+                      const int32_t *d_idx, const int8_t *d_shift, double *d_M, double *d_G,
+                      double *d_B, void *d_ws, size_t ws_bytes, void *cuda_stream);
+/* Number of kernels this library has launched since load (bench.py gpu_launches). */
+int64_t mtp_launch_count(void);
+/* fp64 FMA throughput microbenchmark: runs `iters` dependent-chain DFMA batches on every
+ * SM and returns the useful flop count; time it with CUDA events on `cuda_stream`. */
+int mtp_peak_dfma(int64_t iters, double *d_sink, double *out_flops, void *cuda_stream);
+/* static facts for reporting: flops per pair / per atom of the compiled schedules */
+int mtp_cost_model(const mtp_handle *h, double *flop_per_pair, double *flop_per_atom_tree,
+                   double *flop_per_atom_grade);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MTP_B200_H */
