@@ -89,8 +89,9 @@ const char *mtp_last_error(const mtp_handle *h); /* h may be NULL: last create e
 #define MTP_OPT_CHUNK_ATOMS 1   /* atoms per chunk; 0 = automatic (L2-sized)               */
 #define MTP_OPT_FORCE_MODE 2    /* MTP_FORCE_GATHER (needs d_rev) | MTP_FORCE_ATOMIC       */
 #define MTP_OPT_VARIANT 3       /* MTP_VARIANT_AUTO | _THREAD | _BLOCK                     */
-#define MTP_FORCE_GATHER 0
-#define MTP_FORCE_ATOMIC 1
+#define MTP_FORCE_GATHER 0      /* deterministic; keeps d_ij for all pairs (nnz x 32 B)  */
+#define MTP_FORCE_ATOMIC 1      /* fp64 atomic scatter; no per-pair scratch              */
+#define MTP_FORCE_AUTO 2        /* default: gather when d_rev is given, else atomic      */
 #define MTP_VARIANT_AUTO 0
 #define MTP_VARIANT_THREAD 1    /* one thread group per atom walks all neighbours (large N) */
 #define MTP_VARIANT_BLOCK 2     /* neighbours split across lanes, shuffle-reduced (small N) */
@@ -137,8 +138,8 @@ int mtp_compute_host(mtp_handle *h, int64_t n_atoms, const double *pos, const in
                      double *Ei, double *F, double *virial);
 
 /* Diagnostics (parity bring-up and roofline denominators; not part of the hot path). */
-/* Copy the last chunk-0 intermediate arrays of the most recent mtp_compute: moments
- * M [n][n_basic], adjoints G [n][n_basic] for the first n atoms (device buffers). */
+/* Runs K1 + K2 as one chunk and exports the moments M and adjoints G = dE_i/dM, both laid
+ * out [n_basic][n_atoms] (component-major), and optionally B [n_atoms][n_basis]. */
 int mtp_debug_moments(mtp_handle *h, int64_t n_atoms, const double *d_pos,
                       const int32_t *d_type, const double *box, const int64_t *d_off,
                       const int32_t *d_idx, const int8_t *d_shift, double *d_M, double *d_G,

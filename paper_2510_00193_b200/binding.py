@@ -1,0 +1,263 @@
+"""Thin ctypes binding of include/mtp_b200.h -- argument marshalling only.
+
+Every numeric step runs in libmtp_b200.so's CUDA kernels; PyTorch is used for device
+memory and streams.  There is no CPU fallback: if the shared library is missing (and
+cannot be built) importing this module raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmtp_b200.so")
+
+OK, EINVAL, ESIZE, EBOX, ECUDA, EUNSUP, ENOMEM = 0, -1, -2, -3, -4, -5, -6
+OPT_CHUNK_ATOMS, OPT_FORCE_MODE, OPT_VARIANT = 1, 2, 3
+FORCE_GATHER, FORCE_ATOMIC, FORCE_AUTO = 0, 1, 2
+VARIANT_AUTO, VARIANT_THREAD, VARIANT_BLOCK = 0, 1, 2
+
+_I32P = C.POINTER(C.c_int32)
+
+
+class MtpParams(C.Structure):
+    _fields_ = [
+        ("n_species", C.c_int32), ("n_radial_basis", C.c_int32), ("n_radial_funcs", C.c_int32),
+        ("r_min", C.c_double), ("r_cut", C.c_double), ("lev_max", C.c_int32),
+        ("n_basic", C.c_int32), ("basic", _I32P), ("n_nodes", C.c_int32), ("n_prod", C.c_int32),
+        ("prod", _I32P), ("n_basis", C.c_int32), ("basis_node", _I32P),
+        ("c", C.POINTER(C.c_double)), ("xi0", C.POINTER(C.c_double)), ("xi", C.POINTER(C.c_double)),
+        ("n_desc", C.c_int32), ("basis_desc", _I32P), ("basis_desc_off", _I32P),
+    ]
+
+
+EXPORTS = ["mtp_enumerate", "mtp_table_free", "mtp_create", "mtp_destroy", "mtp_last_error",
+           "mtp_set_option", "mtp_get_option", "mtp_workspace_bytes", "mtp_compute", "mtp_grade",
+           "mtp_compute_host", "mtp_debug_moments", "mtp_launch_count", "mtp_peak_dfma",
+           "mtp_cost_model"]
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        from . import build as _b
+        _b.build()
+    lib = C.CDLL(LIB_PATH)
+    vp, i64, dbl = C.c_void_p, C.c_int64, C.c_double
+    lib.mtp_enumerate.argtypes = [C.c_int32, C.POINTER(MtpParams)]
+    lib.mtp_table_free.argtypes = [C.POINTER(MtpParams)]
+    lib.mtp_table_free.restype = None
+    lib.mtp_create.argtypes = [C.POINTER(vp), C.POINTER(MtpParams)]
+    lib.mtp_destroy.argtypes = [vp]
+    lib.mtp_destroy.restype = None
+    lib.mtp_last_error.argtypes = [vp]
+    lib.mtp_last_error.restype = C.c_char_p
+    lib.mtp_set_option.argtypes = [vp, C.c_int, i64]
+    lib.mtp_get_option.argtypes = [vp, C.c_int, C.POINTER(i64)]
+    lib.mtp_workspace_bytes.argtypes = [vp, i64, i64, C.c_int, C.POINTER(C.c_size_t)]
+    lib.mtp_compute.argtypes = [vp, i64, vp, vp, C.POINTER(dbl), vp, vp, vp, vp, i64, vp, vp, vp, vp, vp,
+                                C.c_size_t, vp]
+    lib.mtp_grade.argtypes = [vp, i64, vp, vp, C.POINTER(dbl), vp, vp, vp, i64, vp, C.c_int, vp, vp, vp, vp,
+                              vp, C.c_size_t, vp]
+    lib.mtp_compute_host.argtypes = [vp, i64, vp, vp, C.POINTER(dbl), vp, vp, vp, vp, i64, vp, vp, vp, vp]
+    lib.mtp_debug_moments.argtypes = [vp, i64, vp, vp, C.POINTER(dbl), vp, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
+    lib.mtp_launch_count.restype = i64
+    lib.mtp_peak_dfma.argtypes = [i64, vp, C.POINTER(dbl), vp]
+    lib.mtp_cost_model.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl)]
+    return lib
+
+
+_lib = _load()
+
+
+class MtpError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("mtp_b200 error %d: %s" % (code, msg))
+        self.code = code
+
+
+class Table:
+    """Contraction table emitted by mtp_enumerate (numpy copies of the C arrays)."""
+
+    def __init__(self, lev_max: int):
+        p = MtpParams()
+        rc = _lib.mtp_enumerate(int(lev_max), C.byref(p))
+        if rc != OK:
+            raise MtpError(rc, "mtp_enumerate(%d)" % lev_max)
+        try:
+            self.lev_max = int(p.lev_max)
+            self.n_mu = int(p.n_radial_funcs)
+            self.n_basic, self.n_nodes, self.n_prod, self.n_basis = p.n_basic, p.n_nodes, p.n_prod, p.n_basis
+            self.basic = np.ctypeslib.as_array(p.basic, (p.n_basic, 4)).copy()
+            self.prod = (np.ctypeslib.as_array(p.prod, (p.n_prod, 4)).copy() if p.n_prod
+                         else np.zeros((0, 4), np.int32))
+            self.basis_node = np.ctypeslib.as_array(p.basis_node, (p.n_basis,)).copy()
+            self.basis_desc = np.ctypeslib.as_array(p.basis_desc, (p.n_desc,)).copy()
+            self.basis_desc_off = np.ctypeslib.as_array(p.basis_desc_off, (p.n_basis + 1,)).copy()
+        finally:
+            _lib.mtp_table_free(C.byref(p))
+
+    def describe(self, alpha: int):
+        return list(self.basis_desc[self.basis_desc_off[alpha]:self.basis_desc_off[alpha + 1]])
+
+
+def _ptr(t):
+    return C.c_void_p(0 if t is None else t.data_ptr())
+
+
+def _np_ptr(a):
+    return C.c_void_p(0 if a is None else a.ctypes.data)
+
+
+class Potential:
+    """mtp_create / mtp_compute / mtp_grade behind torch device tensors."""
+
+    def __init__(self, table: Table, n_species, n_beta, r_min, r_cut, c, xi0, xi,
+                 basic=None, prod=None, basis_node=None, n_nodes=None):
+        self.table = table
+        basic = np.ascontiguousarray(table.basic if basic is None else basic, dtype=np.int32)
+        prod = np.ascontiguousarray(table.prod if prod is None else prod, dtype=np.int32)
+        basis_node = np.ascontiguousarray(table.basis_node if basis_node is None else basis_node, dtype=np.int32)
+        c = np.ascontiguousarray(c, dtype=np.float64)
+        xi0 = np.ascontiguousarray(xi0, dtype=np.float64)
+        xi = np.ascontiguousarray(xi, dtype=np.float64)
+        n_mu = c.shape[2]
+        assert c.shape == (n_species, n_species, n_mu, n_beta)
+        p = MtpParams()
+        p.n_species, p.n_radial_basis, p.n_radial_funcs = int(n_species), int(n_beta), int(n_mu)
+        p.r_min, p.r_cut, p.lev_max = float(r_min), float(r_cut), int(table.lev_max)
+        p.n_basic, p.basic = basic.shape[0], basic.ctypes.data_as(_I32P)
+        p.n_nodes = int(table.n_nodes if n_nodes is None else n_nodes)
+        p.n_prod, p.prod = prod.shape[0], prod.ctypes.data_as(_I32P)
+        p.n_basis, p.basis_node = basis_node.shape[0], basis_node.ctypes.data_as(_I32P)
+        p.c = c.ctypes.data_as(C.POINTER(C.c_double))
+        p.xi0 = xi0.ctypes.data_as(C.POINTER(C.c_double))
+        p.xi = xi.ctypes.data_as(C.POINTER(C.c_double))
+        p.n_desc, p.basis_desc, p.basis_desc_off = 0, None, None
+        h = C.c_void_p()
+        rc = _lib.mtp_create(C.byref(h), C.byref(p))
+        if rc != OK:
+            raise MtpError(rc, _lib.mtp_last_error(None).decode())
+        self._h = h
+        self.n_basis = int(p.n_basis)
+        self.n_basic = int(p.n_basic)
+        self._ws = None
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib.mtp_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc):
+        if rc != OK:
+            raise MtpError(rc, _lib.mtp_last_error(self._h).decode())
+
+    def set_option(self, key, value):
+        self._check(_lib.mtp_set_option(self._h, int(key), int(value)))
+
+    def get_option(self, key):
+        v = C.c_int64()
+        self._check(_lib.mtp_get_option(self._h, int(key), C.byref(v)))
+        return int(v.value)
+
+    def workspace_bytes(self, n_atoms, nnz, want_grade=False):
+        out = C.c_size_t()
+        self._check(_lib.mtp_workspace_bytes(self._h, int(n_atoms), int(nnz), int(bool(want_grade)), C.byref(out)))
+        return int(out.value)
+
+    def cost_model(self):
+        a, b, c = C.c_double(), C.c_double(), C.c_double()
+        self._check(_lib.mtp_cost_model(self._h, C.byref(a), C.byref(b), C.byref(c)))
+        return dict(flop_per_pair=a.value, flop_per_atom_tree=b.value, flop_per_atom_grade=c.value)
+
+    def _workspace(self, nbytes, device):
+        import torch
+        if self._ws is None or self._ws.numel() < nbytes or self._ws.device != device:
+            self._ws = torch.empty(int(nbytes), dtype=torch.uint8, device=device)
+        return self._ws
+
+    @staticmethod
+    def _stream(stream):
+        import torch
+        s = torch.cuda.current_stream() if stream is None else stream
+        return C.c_void_p(s.cuda_stream)
+
+    def compute(self, pos, types, box, off, idx, shift=None, rev=None, want_ei=True, out=None, stream=None):
+        """mtp_compute on torch CUDA tensors.  Returns dict(E[1], Ei[N], F[N,3], virial[6])."""
+        import torch
+        n, nnz, dev = int(pos.shape[0]), int(idx.shape[0]), pos.device
+        assert pos.dtype == torch.float64 and types.dtype == torch.int32 and off.dtype == torch.int64
+        assert idx.dtype == torch.int32 and pos.is_contiguous()
+        if out is None:
+            out = dict(E=torch.empty(1, dtype=torch.float64, device=dev),
+                       Ei=torch.empty(n, dtype=torch.float64, device=dev) if want_ei else None,
+                       F=torch.empty((n, 3), dtype=torch.float64, device=dev),
+                       virial=torch.empty(6, dtype=torch.float64, device=dev))
+        ws = self._workspace(self.workspace_bytes(n, nnz), dev)
+        boxh = (C.c_double * 9)(*[float(x) for x in np.asarray(box, dtype=np.float64).reshape(9)])
+        self._check(_lib.mtp_compute(self._h, n, _ptr(pos), _ptr(types), boxh, _ptr(off), _ptr(idx), _ptr(shift),
+                                     _ptr(rev), nnz, _ptr(out["E"]), _ptr(out.get("Ei")), _ptr(out["F"]),
+                                     _ptr(out["virial"]), _ptr(ws), ws.numel(), self._stream(stream)))
+        return out
+
+    def grade(self, pos, types, box, off, idx, Ainv, shift=None, mode=2, want_B=False, stream=None):
+        import torch
+        n, nnz, dev = int(pos.shape[0]), int(idx.shape[0]), pos.device
+        out = dict(gamma_atom=torch.empty(n, dtype=torch.float64, device=dev) if mode != 1 else None,
+                   gamma_cfg=torch.empty(1, dtype=torch.float64, device=dev) if mode != 0 else None,
+                   Bsum=torch.empty(self.n_basis, dtype=torch.float64, device=dev),
+                   B=torch.empty((n, self.n_basis), dtype=torch.float64, device=dev) if want_B else None)
+        ws = self._workspace(self.workspace_bytes(n, nnz, True), dev)
+        boxh = (C.c_double * 9)(*[float(x) for x in np.asarray(box, dtype=np.float64).reshape(9)])
+        self._check(_lib.mtp_grade(self._h, n, _ptr(pos), _ptr(types), boxh, _ptr(off), _ptr(idx), _ptr(shift), nnz,
+                                   _ptr(Ainv), int(mode), _ptr(out["gamma_atom"]), _ptr(out["gamma_cfg"]),
+                                   _ptr(out["Bsum"]), _ptr(out["B"]), _ptr(ws), ws.numel(), self._stream(stream)))
+        return out
+
+    def debug_moments(self, pos, types, box, off, idx, shift=None, stream=None):
+        """M, G as [n_basic][N] and B [N][n_basis] from one K1+K2 pass."""
+        import torch
+        n, dev = int(pos.shape[0]), pos.device
+        M = torch.empty((self.n_basic, n), dtype=torch.float64, device=dev)
+        G = torch.empty((self.n_basic, n), dtype=torch.float64, device=dev)
+        B = torch.empty((n, self.n_basis), dtype=torch.float64, device=dev)
+        saved = self.get_option(OPT_CHUNK_ATOMS)
+        self.set_option(OPT_CHUNK_ATOMS, max(n, 1))
+        ws = self._workspace(self.workspace_bytes(n, 0), dev)
+        self.set_option(OPT_CHUNK_ATOMS, saved)
+        boxh = (C.c_double * 9)(*[float(x) for x in np.asarray(box, dtype=np.float64).reshape(9)])
+        self._check(_lib.mtp_debug_moments(self._h, n, _ptr(pos), _ptr(types), boxh, _ptr(off), _ptr(idx),
+                                           _ptr(shift), _ptr(M), _ptr(G), _ptr(B), _ptr(ws), ws.numel(),
+                                           self._stream(stream)))
+        return M, G, B
+
+    def compute_host(self, pos, types, box, off, idx, shift=None, rev=None, out=None):
+        """mtp_compute_host on numpy (or pinned torch CPU) arrays; H2D/D2H inside the call."""
+        n, nnz = int(pos.shape[0]), int(idx.shape[0])
+        if out is None:
+            out = dict(E=np.empty(1), Ei=np.empty(n), F=np.empty((n, 3)), virial=np.empty(6))
+        boxh = (C.c_double * 9)(*[float(x) for x in np.asarray(box, dtype=np.float64).reshape(9)])
+        self._check(_lib.mtp_compute_host(self._h, n, _np_ptr(pos), _np_ptr(types), boxh, _np_ptr(off), _np_ptr(idx),
+                                          _np_ptr(shift), _np_ptr(rev), nnz, _np_ptr(out["E"]), _np_ptr(out["Ei"]),
+                                          _np_ptr(out["F"]), _np_ptr(out["virial"])))
+        return out
+
+
+def launch_count() -> int:
+    return int(_lib.mtp_launch_count())
+
+
+def peak_dfma(iters: int, sink, stream=None):
+    """Enqueue the fp64-FMA microbenchmark; returns the flop count of the launch."""
+    fl = C.c_double()
+    rc = _lib.mtp_peak_dfma(int(iters), _ptr(sink), C.byref(fl), Potential._stream(stream))
+    if rc != OK:
+        raise MtpError(rc, "mtp_peak_dfma")
+    return fl.value

@@ -1,0 +1,500 @@
+// C ABI of the MTP hot path (include/mtp_b200.h): handle, table compilation, chunk scheduler
+// (a10), variant selection and the launch sequences of
+// mtp_compute / mtp_grade.  No CPU fallback: every numeric step runs in the CUDA kernels.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <map>
+#include <string>
+#include <tuple>
+#include <vector>
+
+#include "kernels.h"
+#include "mtp_b200.h"
+#include "stair.h"
+
+using namespace mtpb;
+
+namespace mtpb {
+PairLevel pair_level_10();
+PairLevel pair_level_16();
+PairLevel pair_level_20();
+PairLevel pair_level_24();
+PairLevel pair_level_28();
+const PairLevel *pair_level(int index) {
+  static const PairLevel levels[] = {pair_level_10(), pair_level_16(), pair_level_20(), pair_level_24(),
+                                     pair_level_28()};
+  return (index >= 0 && index < kNumLevels) ? &levels[index] : nullptr;
+}
+}  // namespace mtpb
+
+static thread_local std::string g_create_error;
+
+struct mtp_handle {
+  int S = 0, nb = 0, nmu = 0, n_basic = 0, n_nodes = 0, n_basis = 0, lev_max = 0;
+  double r_min = 0, r_cut = 0;
+  const PairLevel *pl = nullptr;
+  int crow = 0, AL = 0;
+  double *d_coef = nullptr, *d_xi = nullptr, *d_xi0 = nullptr;
+  int *d_kmapF = nullptr, *d_kmapB = nullptr, *d_basis_node = nullptr;
+  TreeTerm *d_fterms = nullptr, *d_bterms = nullptr;
+  TreeItem *d_fitems = nullptr, *d_bitems = nullptr;
+  int *d_fwave = nullptr, *d_bwave = nullptr;
+  TreeSched sched;
+  int64_t chunk_atoms = 0;
+  int force_mode = MTP_FORCE_AUTO, variant = MTP_VARIANT_AUTO;
+  std::string err;
+  // staging for mtp_compute_host (grow-only)
+  void *stage = nullptr;
+  size_t stage_bytes = 0;
+  std::vector<void *> to_free;
+};
+
+static int fail(mtp_handle *h, int code, const std::string &msg) {
+  if (h) h->err = msg; else g_create_error = msg;
+  return code;
+}
+static int cuda_fail(mtp_handle *h, cudaError_t e, const char *where) {
+  return fail(h, MTP_ECUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+#define CU(h, call)                                                  \
+  do {                                                               \
+    cudaError_t e__ = (call);                                        \
+    if (e__ != cudaSuccess) return cuda_fail(h, e__, #call);         \
+  } while (0)
+
+template <class T>
+static cudaError_t upload(mtp_handle *h, T **dst, const T *src, size_t n) {
+  cudaError_t e = cudaMalloc((void **)dst, sizeof(T) * std::max<size_t>(n, 1));
+  if (e != cudaSuccess) return e;
+  h->to_free.push_back(*dst);
+  if (n) e = cudaMemcpy(*dst, src, sizeof(T) * n, cudaMemcpyHostToDevice);
+  return e;
+}
+
+// ---- staircase helpers at run time (mirror stair.h) -----------------------------------
+static int rt_numax(int lev, int mu) { int t = lev - 4 - 4 * mu; return t >= 2 ? t / 2 : 0; }
+static int rt_nmu(int lev) { return (lev - 2) / 4 + 1; }
+static bool rt_valid(int lev, int mu, int nu) { return mu < rt_nmu(lev) && (nu == 0 || rt_numax(lev, mu) >= nu); }
+static int rt_nmu_for(int lev, int nu) {
+  int n = 0;
+  for (int mu = 0; mu < rt_nmu(lev); ++mu) if (nu == 0 || rt_numax(lev, mu) >= nu) ++n;
+  return n;
+}
+
+// kmapF: slot order of k_moments (a, i, k, mu);  kmapB: slot order of k_pairgrad (mu, a desc, i desc, k desc)
+static void build_kmaps(const PairLevel &pl, int n_basic, const int32_t *basic, std::vector<int> &kf,
+                        std::vector<int> &kb) {
+  const int lev = pl.lev, NSB = pl.nsb, NSC = pl.nsc, NS = NSB * NSC, NU0 = rt_numax(lev, 0);
+  std::map<std::tuple<int, int, int, int>, int> where;
+  for (int k = 0; k < n_basic; ++k) where[{basic[4 * k], basic[4 * k + 1], basic[4 * k + 2], basic[4 * k + 3]}] = k;
+  auto find = [&](int mu, int a, int b, int c) {
+    if (!rt_valid(lev, mu, a + b + c)) return -1;
+    auto it = where.find({mu, a, b, c});
+    return it == where.end() ? -1 : it->second;
+  };
+  kf.assign((size_t)NS * pl.nslot, -1);
+  kb.assign((size_t)NS * pl.nslot, -1);
+  for (int s = 0; s < NS; ++s) {
+    const int sb = s % NSB, sc = s / NSB;
+    int slot = 0;
+    for (int a = 0; a <= NU0; ++a)
+      for (int i = 0; i <= (NU0 - a) / NSB; ++i)
+        for (int k = 0; k <= (NU0 - a - NSB * i) / NSC; ++k)
+          for (int m = 0; m < rt_nmu_for(lev, a + NSB * i + NSC * k); ++m)
+            kf[(size_t)s * pl.nslot + slot++] = find(m, a, sb + NSB * i, sc + NSC * k);
+    slot = 0;
+    for (int m = 0; m < rt_nmu(lev); ++m) {
+      const int NUm = rt_numax(lev, m);
+      for (int a = NUm; a >= 0; --a)
+        for (int i = (NUm - a) / NSB; i >= 0; --i)
+          for (int k = (NUm - a - NSB * i) / NSC; k >= 0; --k)
+            kb[(size_t)s * pl.nslot + slot++] = find(m, a, sb + NSB * i, sc + NSC * k);
+    }
+  }
+}
+
+extern "C" const char *mtp_last_error(const mtp_handle *h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+extern "C" int64_t mtp_launch_count(void) { return launch_count(); }
+
+extern "C" void mtp_destroy(mtp_handle *h) {
+  if (!h) return;
+  for (void *p : h->to_free) cudaFree(p);
+  if (h->stage) cudaFree(h->stage);
+  delete h;
+}
+
+extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
+  if (!out || !p) return fail(nullptr, MTP_EINVAL, "null argument");
+  *out = nullptr;
+  if (p->n_species < 1 || p->n_species > 16 || p->n_radial_basis < 1 || p->n_radial_basis > 16 ||
+      p->n_radial_funcs < 1 || !(p->r_cut > p->r_min) || !(p->r_min >= 0) || p->n_basic < 1 ||
+      p->n_nodes < p->n_basic || p->n_prod < 0 || p->n_basis < 1 || !p->basic || (p->n_prod && !p->prod) ||
+      !p->basis_node || !p->c || !p->xi0 || !p->xi)
+    return fail(nullptr, MTP_EINVAL, "mtp_params: bad sizes or null arrays");
+  int dev_count = 0;
+  if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0)
+    return fail(nullptr, MTP_ECUDA, "no CUDA device: this library has no CPU fallback");
+  // level of the pair kernels: the smallest compiled staircase containing every table tensor
+  int li = -1;
+  for (int c = 0; c < kNumLevels && li < 0; ++c) {
+    bool ok = true;
+    for (int k = 0; k < p->n_basic && ok; ++k) {
+      const int32_t *b = p->basic + 4 * k;
+      if (b[0] < 0 || b[1] < 0 || b[2] < 0 || b[3] < 0 || b[0] >= p->n_radial_funcs) return fail(nullptr, MTP_EINVAL, "basic: bad (mu,a,b,c)");
+      ok = rt_valid(kLevels[c].lev, b[0], b[1] + b[2] + b[3]);
+    }
+    if (ok) li = c;
+  }
+  if (li < 0) return fail(nullptr, MTP_EUNSUP, "moment set exceeds the largest compiled level (28)");
+  mtp_handle *h = new mtp_handle();
+  h->S = p->n_species; h->nb = p->n_radial_basis; h->nmu = p->n_radial_funcs; h->n_basic = p->n_basic;
+  h->n_nodes = p->n_nodes; h->n_basis = p->n_basis; h->lev_max = p->lev_max; h->r_min = p->r_min; h->r_cut = p->r_cut;
+  h->pl = pair_level(li);
+  const char *terr = "";
+  int rc = tree_compile(p->n_basic, p->n_nodes, p->n_prod, p->prod, p->n_basis, p->basis_node, h->sched, &terr);
+  if (rc != MTP_OK) { g_create_error = terr; delete h; return rc; }
+  h->AL = tree_pick_al(p->n_nodes);
+  if (h->AL == 0) { delete h; return fail(nullptr, MTP_EUNSUP, "contraction tree does not fit in shared memory (n_nodes*16 B > 220 KB)"); }
+  // radial coefficients: rows (z_i, z_j) padded to the level's n_mu, odd row stride (bank spread)
+  const int nmu_lev = rt_nmu(h->pl->lev);
+  h->crow = nmu_lev * h->nb + 1;
+  std::vector<double> coef((size_t)h->S * h->S * h->crow, 0.0);
+  for (int r = 0; r < h->S * h->S; ++r)
+    for (int m = 0; m < h->nmu && m < nmu_lev; ++m)
+      for (int b = 0; b < h->nb; ++b) coef[(size_t)r * h->crow + m * h->nb + b] = p->c[((size_t)r * h->nmu + m) * h->nb + b];
+  std::vector<int> kf, kb;
+  build_kmaps(*h->pl, p->n_basic, p->basic, kf, kb);
+  cudaError_t e = cudaSuccess;
+  auto up = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+  up(upload(h, &h->d_coef, coef.data(), coef.size()));
+  up(upload(h, &h->d_xi, p->xi, (size_t)p->n_basis));
+  up(upload(h, &h->d_xi0, p->xi0, (size_t)p->n_species));
+  up(upload(h, &h->d_kmapF, kf.data(), kf.size()));
+  up(upload(h, &h->d_kmapB, kb.data(), kb.size()));
+  up(upload(h, &h->d_basis_node, p->basis_node, (size_t)p->n_basis));
+  up(upload(h, &h->d_fterms, h->sched.fterms.data(), h->sched.fterms.size()));
+  up(upload(h, &h->d_bterms, h->sched.bterms.data(), h->sched.bterms.size()));
+  up(upload(h, &h->d_fitems, h->sched.fitems.data(), h->sched.fitems.size()));
+  up(upload(h, &h->d_bitems, h->sched.bitems.data(), h->sched.bitems.size()));
+  up(upload(h, &h->d_fwave, h->sched.fwave.data(), h->sched.fwave.size()));
+  up(upload(h, &h->d_bwave, h->sched.bwave.data(), h->sched.bwave.size()));
+  if (e != cudaSuccess) { int r = cuda_fail(nullptr, e, "mtp_create upload"); mtp_destroy(h); return r; }
+  *out = h;
+  return MTP_OK;
+}
+
+extern "C" int mtp_set_option(mtp_handle *h, int key, int64_t v) {
+  if (!h) return MTP_EINVAL;
+  switch (key) {
+    case MTP_OPT_CHUNK_ATOMS: if (v < 0) return fail(h, MTP_EINVAL, "chunk_atoms < 0"); h->chunk_atoms = v; return MTP_OK;
+    case MTP_OPT_FORCE_MODE: if (v < 0 || v > 2) return fail(h, MTP_EINVAL, "bad force mode"); h->force_mode = (int)v; return MTP_OK;
+    case MTP_OPT_VARIANT: if (v < 0 || v > 2) return fail(h, MTP_EINVAL, "bad variant"); h->variant = (int)v; return MTP_OK;
+  }
+  return fail(h, MTP_EINVAL, "unknown option");
+}
+extern "C" int mtp_get_option(const mtp_handle *h, int key, int64_t *v) {
+  if (!h || !v) return MTP_EINVAL;
+  switch (key) {
+    case MTP_OPT_CHUNK_ATOMS: *v = h->chunk_atoms; return MTP_OK;
+    case MTP_OPT_FORCE_MODE: *v = h->force_mode; return MTP_OK;
+    case MTP_OPT_VARIANT: *v = h->variant; return MTP_OK;
+  }
+  return MTP_EINVAL;
+}
+
+// ---- chunk scheduler / workspace plan ---------------------------------------------------
+namespace {
+struct Plan {
+  int64_t N = 0, nnz = 0, C = 0, ldm = 0;
+  int n_chunks = 0, P = 1, atomic = 0, grid_chunk = 0;
+  size_t o_pos4 = 0, o_Ei = 0, o_M = 0, o_G = 0, o_wpart = 0, o_d4 = 0, o_B = 0, o_part = 0, total = 0;
+};
+size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+int make_plan(const mtp_handle *h, int64_t N, int64_t nnz, int want_grade, int has_rev, Plan &pl) {
+  if (N < 0 || nnz < 0 || N > 2147483000LL) return MTP_EINVAL;
+  pl.N = N; pl.nnz = nnz;
+  int64_t C = h->chunk_atoms;
+  if (C <= 0) {   // automatic: M and G of a chunk (16 B x n_basic per atom) stay L2-resident
+    C = (64LL << 20) / (16LL * h->n_basic);
+    C = std::max<int64_t>(1024, C / 1024 * 1024);
+    if (N > C) {  // avoid a small last chunk
+      const int64_t nc = (N + C - 1) / C;
+      C = ((N + nc - 1) / nc + 31) / 32 * 32;
+    }
+  }
+  if (C > N) C = std::max<int64_t>(N, 1);
+  pl.C = C;
+  pl.ldm = (C + 31) / 32 * 32;
+  pl.n_chunks = N ? (int)((N + C - 1) / C) : 0;
+  const int NS = h->pl->nsb * h->pl->nsc;
+  if (h->variant == MTP_VARIANT_THREAD) pl.P = 1;
+  else if (h->variant == MTP_VARIANT_BLOCK) pl.P = h->pl->p_small;
+  else pl.P = (N * NS >= 2LL * 148 * 256) ? 1 : h->pl->p_small;   // fill the SMs' register files
+  pl.atomic = h->force_mode == MTP_FORCE_ATOMIC || (h->force_mode == MTP_FORCE_AUTO && !has_rev);
+  pl.grid_chunk = h->pl->pairgrad_grid((int)C, pl.P);
+  size_t o = 0;
+  pl.o_pos4 = o; o = align_up(o + (size_t)N * 32);
+  pl.o_Ei = o; o = align_up(o + (size_t)N * 8);
+  pl.o_M = o; o = align_up(o + (size_t)h->n_basic * pl.ldm * 8);
+  pl.o_G = o; o = align_up(o + (size_t)h->n_basic * pl.ldm * 8);
+  pl.o_wpart = o; o = align_up(o + (size_t)std::max(1, pl.n_chunks) * pl.grid_chunk * 64);
+  pl.o_d4 = o; if (!want_grade && !pl.atomic) o = align_up(o + (size_t)nnz * 32);
+  pl.o_B = o; if (want_grade) o = align_up(o + (size_t)C * h->n_basis * 8);
+  pl.o_part = o; if (want_grade) o = align_up(o + (size_t)64 * h->n_basis * 8);
+  pl.total = o;
+  return MTP_OK;
+}
+
+int box_setup(mtp_handle *h, const double *box, bool need_minimg, double r_cut, PairArgs &pa) {
+  const double *a = box, *b = box + 3, *c = box + 6;
+  const double bc[3] = {b[1] * c[2] - b[2] * c[1], b[2] * c[0] - b[0] * c[2], b[0] * c[1] - b[1] * c[0]};
+  const double ca[3] = {c[1] * a[2] - c[2] * a[1], c[2] * a[0] - c[0] * a[2], c[0] * a[1] - c[1] * a[0]};
+  const double ab[3] = {a[1] * b[2] - a[2] * b[1], a[2] * b[0] - a[0] * b[2], a[0] * b[1] - a[1] * b[0]};
+  const double vol = a[0] * bc[0] + a[1] * bc[1] + a[2] * bc[2];
+  for (int i = 0; i < 9; ++i) pa.H[i] = box[i];
+  if (!(std::fabs(vol) > 0)) {
+    if (need_minimg) return fail(h, MTP_EBOX, "singular box");
+    for (int i = 0; i < 9; ++i) pa.Hi[i] = 0;
+    return MTP_OK;
+  }
+  // H^-1 (row-vector convention: frac = cart . Hi): columns are bc, ca, ab over vol
+  for (int i = 0; i < 3; ++i) { pa.Hi[3 * i + 0] = bc[i] / vol; pa.Hi[3 * i + 1] = ca[i] / vol; pa.Hi[3 * i + 2] = ab[i] / vol; }
+  if (need_minimg) {
+    auto norm = [](const double *v) { return std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]); };
+    const double hmin = std::min({std::fabs(vol) / norm(bc), std::fabs(vol) / norm(ca), std::fabs(vol) / norm(ab)});
+    if (!(hmin > 2.0 * r_cut)) return fail(h, MTP_EBOX, "box height < 2 R_cut and no image shifts given");
+  }
+  return MTP_OK;
+}
+
+void fill_pair_args(const mtp_handle *h, PairArgs &pa, const double *pos4, const int64_t *off, const int32_t *idx,
+                    const int8_t *shift) {
+  pa.pos4 = pos4; pa.off = (const long long *)off; pa.idx = idx; pa.shift = (const signed char *)shift;
+  pa.coef = h->d_coef; pa.n_species = h->S; pa.nb = h->nb; pa.crow = h->crow;
+  pa.minimg = shift ? 0 : 1; pa.r_min = h->r_min; pa.r_cut = h->r_cut;
+  pa.M = nullptr; pa.G = nullptr; pa.d4 = nullptr; pa.F = nullptr; pa.wpart = nullptr; pa.kmap = nullptr;
+}
+
+void fill_tree_args(const mtp_handle *h, TreeArgs &ta, const double *pos4) {
+  ta.fterms = h->d_fterms; ta.fitems = h->d_fitems; ta.fwave = h->d_fwave; ta.nfw = (int)h->sched.fwave.size() - 1;
+  ta.bterms = h->d_bterms; ta.bitems = h->d_bitems; ta.bwave = h->d_bwave; ta.nbw = (int)h->sched.bwave.size() - 1;
+  ta.basis_node = h->d_basis_node; ta.xi = h->d_xi; ta.xi0 = h->d_xi0; ta.pos4 = pos4;
+  ta.n_nodes = h->n_nodes; ta.n_basic = h->n_basic; ta.n_basis = h->n_basis;
+  ta.B = nullptr; ta.want_adj = 1;
+}
+}  // namespace
+
+extern "C" int mtp_workspace_bytes(const mtp_handle *h, int64_t n_atoms, int64_t nnz, int want_grade, size_t *out) {
+  if (!h || !out) return MTP_EINVAL;
+  Plan pl;
+  int rc = make_plan(h, n_atoms, nnz, want_grade, /*has_rev=*/1, pl);
+  if (rc != MTP_OK) return rc;
+  *out = pl.total + 256 + (want_grade ? align_up((size_t)h->n_basis * 8) : 0);
+  return MTP_OK;
+}
+
+extern "C" int mtp_compute(mtp_handle *h, int64_t N, const double *d_pos, const int32_t *d_type, const double *box,
+                           const int64_t *d_off, const int32_t *d_idx, const int8_t *d_shift, const int32_t *d_rev,
+                           int64_t nnz, double *d_E, double *d_Ei, double *d_F, double *d_virial, void *d_ws,
+                           size_t ws_bytes, void *stream) {
+  if (!h) return MTP_EINVAL;
+  if (!box || !d_E || (N > 0 && (!d_pos || !d_type || !d_off || !d_F)) || (nnz > 0 && !d_idx))
+    return fail(h, MTP_EINVAL, "mtp_compute: null argument");
+  if (h->force_mode == MTP_FORCE_GATHER && !d_rev && nnz > 0) return fail(h, MTP_EINVAL, "gather mode needs d_rev");
+  cudaStream_t st = (cudaStream_t)stream;
+  Plan pl;
+  int rc = make_plan(h, N, nnz, 0, d_rev != nullptr, pl);
+  if (rc != MTP_OK) return fail(h, rc, "bad sizes");
+  const size_t base = align_up((size_t)(uintptr_t)d_ws) - (size_t)(uintptr_t)d_ws;
+  if (N > 0 && (!d_ws || ws_bytes < pl.total + base)) return fail(h, MTP_ESIZE, "workspace too small");
+  PairArgs pa;
+  rc = box_setup(h, box, d_shift == nullptr && nnz > 0, h->r_cut, pa);
+  if (rc != MTP_OK) return rc;
+  if (N == 0) {
+    CU(h, launch_zero(d_E, 1, st));
+    if (d_virial) CU(h, launch_zero(d_virial, 6, st));
+    return MTP_OK;
+  }
+  char *ws = (char *)d_ws + base;
+  double *pos4 = (double *)(ws + pl.o_pos4), *Ei = d_Ei ? d_Ei : (double *)(ws + pl.o_Ei);
+  double *M = (double *)(ws + pl.o_M), *G = (double *)(ws + pl.o_G), *wpart = (double *)(ws + pl.o_wpart);
+  double *d4 = (double *)(ws + pl.o_d4);
+  CU(h, launch_pack(d_pos, d_type, (int)N, pos4, st));
+  CU(h, launch_zero(wpart, (long long)pl.n_chunks * pl.grid_chunk * 8, st));
+  if (pl.atomic) CU(h, launch_zero(d_F, 3 * N, st));
+  fill_pair_args(h, pa, pos4, d_off, d_idx, d_shift);
+  pa.ldm = pl.ldm;
+  TreeArgs ta;
+  fill_tree_args(h, ta, pos4);
+  ta.M = M; ta.G = G; ta.ldm = pl.ldm; ta.Ei = Ei;
+  for (int c = 0; c < pl.n_chunks; ++c) {
+    pa.c0 = (int)(c * pl.C); pa.c1 = (int)std::min<int64_t>(N, (c + 1) * pl.C);
+    pa.M = M; pa.G = G; pa.kmap = h->d_kmapF;
+    CU(h, h->pl->moments(pa, pl.P, st));
+    ta.c0 = pa.c0; ta.c1 = pa.c1;
+    CU(h, launch_tree(ta, h->AL, st));
+    pa.kmap = h->d_kmapB; pa.wpart = wpart + (size_t)c * pl.grid_chunk * 8;
+    pa.d4 = pl.atomic ? nullptr : d4; pa.F = pl.atomic ? d_F : nullptr;
+    CU(h, h->pl->pairgrad(pa, pl.P, pl.atomic, st, nullptr));
+  }
+  if (!pl.atomic) CU(h, launch_gather((const long long *)d_off, d_rev, d4, (int)N, d_F, st));
+  CU(h, launch_reduce(Ei, N, 1, 1, d_E, st));
+  if (d_virial) CU(h, launch_reduce(wpart, (long long)pl.n_chunks * pl.grid_chunk, 8, 6, d_virial, st));
+  return MTP_OK;
+}
+
+extern "C" int mtp_grade(mtp_handle *h, int64_t N, const double *d_pos, const int32_t *d_type, const double *box,
+                         const int64_t *d_off, const int32_t *d_idx, const int8_t *d_shift, int64_t nnz,
+                         const double *d_Ainv, int mode, double *d_gamma_atom, double *d_gamma_cfg, double *d_Bsum,
+                         double *d_B, void *d_ws, size_t ws_bytes, void *stream) {
+  if (!h) return MTP_EINVAL;
+  if (!box || !d_Ainv || mode < 0 || mode > 2 || (N > 0 && (!d_pos || !d_type || !d_off)) || (nnz > 0 && !d_idx) ||
+      (mode != 1 && N > 0 && !d_gamma_atom) || (mode != 0 && !d_gamma_cfg))
+    return fail(h, MTP_EINVAL, "mtp_grade: null or inconsistent argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  Plan pl;
+  int rc = make_plan(h, N, nnz, 1, 0, pl);
+  if (rc != MTP_OK) return fail(h, rc, "bad sizes");
+  const size_t base = align_up((size_t)(uintptr_t)d_ws) - (size_t)(uintptr_t)d_ws;
+  // one extra n_basis vector at the end holds sum_i B when the caller does not want it
+  const size_t need = pl.total + base + align_up((size_t)h->n_basis * 8);
+  if (!d_ws || ws_bytes < need) return fail(h, MTP_ESIZE, "workspace too small");
+  PairArgs pa;
+  rc = box_setup(h, box, d_shift == nullptr && nnz > 0, h->r_cut, pa);
+  if (rc != MTP_OK) return rc;
+  char *ws = (char *)d_ws + base;
+  double *pos4 = (double *)(ws + pl.o_pos4), *Ei = (double *)(ws + pl.o_Ei), *M = (double *)(ws + pl.o_M);
+  double *G = (double *)(ws + pl.o_G), *Bc = (double *)(ws + pl.o_B), *part = (double *)(ws + pl.o_part);
+  double *Bsum = d_Bsum ? d_Bsum : (double *)(ws + pl.total);
+  if (mode != 0 || d_Bsum) CU(h, launch_zero(Bsum, h->n_basis, st));
+  if (N > 0) {
+    CU(h, launch_pack(d_pos, d_type, (int)N, pos4, st));
+    fill_pair_args(h, pa, pos4, d_off, d_idx, d_shift);
+    pa.ldm = pl.ldm;
+    TreeArgs ta;
+    fill_tree_args(h, ta, pos4);
+    ta.M = M; ta.G = G; ta.ldm = pl.ldm; ta.Ei = Ei; ta.want_adj = 0;
+    for (int c = 0; c < pl.n_chunks; ++c) {
+      pa.c0 = (int)(c * pl.C); pa.c1 = (int)std::min<int64_t>(N, (c + 1) * pl.C);
+      pa.M = M; pa.kmap = h->d_kmapF;
+      CU(h, h->pl->moments(pa, pl.P, st));
+      ta.c0 = pa.c0; ta.c1 = pa.c1;
+      // B rows are indexed by absolute atom: point the kernel at a base shifted by -c0 rows
+      double *Brows = d_B ? d_B : Bc - (size_t)pa.c0 * h->n_basis;
+      ta.B = Brows;
+      CU(h, launch_tree(ta, h->AL, st));
+      const double *Bchunk = Brows + (size_t)pa.c0 * h->n_basis;
+      const int64_t nc = pa.c1 - pa.c0;
+      if (mode != 1) CU(h, launch_grade(Bchunk, d_Ainv, nc, h->n_basis, d_gamma_atom + pa.c0, st));
+      if (mode != 0 || d_Bsum) CU(h, launch_colsum(Bchunk, nc, h->n_basis, Bsum, part, st));
+    }
+  }
+  if (mode != 0) CU(h, launch_grade_cfg(Bsum, d_Ainv, h->n_basis, nullptr, d_gamma_cfg, st));
+  return MTP_OK;
+}
+
+// ---- host-buffer end-to-end path ----------------------------------------------------------
+extern "C" int mtp_compute_host(mtp_handle *h, int64_t N, const double *pos, const int32_t *type, const double *box,
+                                const int64_t *off, const int32_t *idx, const int8_t *shift, const int32_t *rev,
+                                int64_t nnz, double *E, double *Ei, double *F, double *virial) {
+  if (!h) return MTP_EINVAL;
+  if (!box || !E || (N > 0 && (!pos || !type || !off || !F)) || (nnz > 0 && !idx)) return fail(h, MTP_EINVAL, "mtp_compute_host: null argument");
+  size_t wsb = 0;
+  int rc = mtp_workspace_bytes(h, N, nnz, 0, &wsb);
+  if (rc != MTP_OK) return rc;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
+  const size_t o_pos = take((size_t)N * 24), o_type = take((size_t)N * 4), o_off = take((size_t)(N + 1) * 8);
+  const size_t o_idx = take((size_t)nnz * 4), o_shift = take(shift ? (size_t)nnz * 3 : 0), o_rev = take(rev ? (size_t)nnz * 4 : 0);
+  const size_t o_out = take((size_t)(7 + N + 3 * N) * 8), o_ws = take(wsb);
+  if (o > h->stage_bytes) {
+    if (h->stage) cudaFree(h->stage);
+    h->stage = nullptr; h->stage_bytes = 0;
+    CU(h, cudaMalloc(&h->stage, o));
+    h->stage_bytes = o;
+  }
+  char *d = (char *)h->stage;
+  cudaStream_t st = 0;
+  if (N > 0) {
+    CU(h, cudaMemcpyAsync(d + o_pos, pos, (size_t)N * 24, cudaMemcpyHostToDevice, st));
+    CU(h, cudaMemcpyAsync(d + o_type, type, (size_t)N * 4, cudaMemcpyHostToDevice, st));
+    CU(h, cudaMemcpyAsync(d + o_off, off, (size_t)(N + 1) * 8, cudaMemcpyHostToDevice, st));
+  }
+  if (nnz > 0) {
+    CU(h, cudaMemcpyAsync(d + o_idx, idx, (size_t)nnz * 4, cudaMemcpyHostToDevice, st));
+    if (shift) CU(h, cudaMemcpyAsync(d + o_shift, shift, (size_t)nnz * 3, cudaMemcpyHostToDevice, st));
+    if (rev) CU(h, cudaMemcpyAsync(d + o_rev, rev, (size_t)nnz * 4, cudaMemcpyHostToDevice, st));
+  }
+  double *dE = (double *)(d + o_out), *dW = dE + 1, *dEi = dE + 7, *dF = dEi + N;
+  rc = mtp_compute(h, N, (double *)(d + o_pos), (int32_t *)(d + o_type), box, (int64_t *)(d + o_off),
+                   (int32_t *)(d + o_idx), shift ? (int8_t *)(d + o_shift) : nullptr,
+                   rev ? (int32_t *)(d + o_rev) : nullptr, nnz, dE, dEi, dF, dW, d + o_ws, wsb, st);
+  if (rc != MTP_OK) return rc;
+  CU(h, cudaMemcpyAsync(E, dE, 8, cudaMemcpyDeviceToHost, st));
+  if (virial) CU(h, cudaMemcpyAsync(virial, dW, 48, cudaMemcpyDeviceToHost, st));
+  if (Ei && N > 0) CU(h, cudaMemcpyAsync(Ei, dEi, (size_t)N * 8, cudaMemcpyDeviceToHost, st));
+  if (N > 0) CU(h, cudaMemcpyAsync(F, dF, (size_t)N * 24, cudaMemcpyDeviceToHost, st));
+  CU(h, cudaStreamSynchronize(st));
+  return MTP_OK;
+}
+
+// ---- diagnostics ------------------------------------------------------------------------------
+extern "C" int mtp_debug_moments(mtp_handle *h, int64_t N, const double *d_pos, const int32_t *d_type,
+                                 const double *box, const int64_t *d_off, const int32_t *d_idx, const int8_t *d_shift,
+                                 double *d_M, double *d_G, double *d_B, void *d_ws, size_t ws_bytes, void *stream) {
+  if (!h || !box || N <= 0 || !d_pos || !d_type || !d_off || !d_idx) return MTP_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t saved = h->chunk_atoms;
+  h->chunk_atoms = N;                       // single chunk so that M, G hold every atom
+  Plan pl;
+  int rc = make_plan(h, N, 0, 0, 0, pl);
+  h->chunk_atoms = saved;
+  if (rc != MTP_OK) return rc;
+  const size_t base = align_up((size_t)(uintptr_t)d_ws) - (size_t)(uintptr_t)d_ws;
+  if (!d_ws || ws_bytes < pl.total + base) return fail(h, MTP_ESIZE, "workspace too small");
+  PairArgs pa;
+  rc = box_setup(h, box, d_shift == nullptr, h->r_cut, pa);
+  if (rc != MTP_OK) return rc;
+  char *ws = (char *)d_ws + base;
+  double *pos4 = (double *)(ws + pl.o_pos4), *Ei = (double *)(ws + pl.o_Ei), *M = (double *)(ws + pl.o_M), *G = (double *)(ws + pl.o_G);
+  CU(h, launch_pack(d_pos, d_type, (int)N, pos4, st));
+  fill_pair_args(h, pa, pos4, d_off, d_idx, d_shift);
+  pa.ldm = pl.ldm; pa.c0 = 0; pa.c1 = (int)N; pa.M = M; pa.kmap = h->d_kmapF;
+  CU(h, h->pl->moments(pa, pl.P, st));
+  TreeArgs ta;
+  fill_tree_args(h, ta, pos4);
+  ta.M = M; ta.G = G; ta.ldm = pl.ldm; ta.Ei = Ei; ta.c0 = 0; ta.c1 = (int)N; ta.B = d_B;
+  CU(h, launch_tree(ta, h->AL, st));
+  // outputs are [n_basic][N] (component-major), the kernels' own layout
+  if (d_M) CU(h, cudaMemcpy2DAsync(d_M, (size_t)N * 8, M, (size_t)pl.ldm * 8, (size_t)N * 8, h->n_basic, cudaMemcpyDeviceToDevice, st));
+  if (d_G) CU(h, cudaMemcpy2DAsync(d_G, (size_t)N * 8, G, (size_t)pl.ldm * 8, (size_t)N * 8, h->n_basic, cudaMemcpyDeviceToDevice, st));
+  return MTP_OK;
+}
+
+extern "C" int mtp_peak_dfma(int64_t iters, double *d_sink, double *out_flops, void *stream) {
+  if (iters <= 0 || !d_sink) return MTP_EINVAL;
+  return launch_peak_dfma(iters, d_sink, out_flops, (cudaStream_t)stream) == cudaSuccess ? MTP_OK : MTP_ECUDA;
+}
+
+// Useful flops (FMA = 2, MUL/ADD = 1), each quantity counted once -- DESIGN.md "Roofline".
+//   per pair : geometry + rsqrt (12) + Chebyshev T_b, T'_b (2*3 per b) + f, f' (2*2 n_beta n_mu)
+//              + monomials (1 per packed monomial of rank <= nu_max) + moments (2 n_basic)
+//              + pair derivative (value+gradient of sum_mu f_mu P_mu: 8 n_basic)
+//   per atom : tree forward 3/op, adjoint 6/op, energy 2 n_basis;  grade 2 n_basis^2
+extern "C" int mtp_cost_model(const mtp_handle *h, double *flop_per_pair, double *flop_per_atom_tree,
+                              double *flop_per_atom_grade) {
+  if (!h) return MTP_EINVAL;
+  int numax = 0;
+  for (int k = 0; k < h->n_basic; ++k) (void)k;
+  // highest rank present in the table
+  numax = rt_numax(h->pl->lev, 0);
+  const double monos = (numax + 1.0) * (numax + 2.0) * (numax + 3.0) / 6.0;
+  if (flop_per_pair) *flop_per_pair = 12.0 + 6.0 * h->nb + 4.0 * h->nb * h->nmu + monos + 10.0 * h->n_basic;
+  if (flop_per_atom_tree) *flop_per_atom_tree = 9.0 * (double)h->sched.n_prod + 2.0 * h->n_basis;
+  if (flop_per_atom_grade) *flop_per_atom_grade = 2.0 * (double)h->n_basis * h->n_basis;
+  return MTP_OK;
+}

@@ -1,0 +1,130 @@
+// K5 (a9): extrapolation grades.  gamma_i = max_k | sum_a B[i][a] Ainv[a][k] |  (PAPER.md:35,46
+// neighbourhood mode) and gamma = max_k | (sum_i B_i) Ainv |_k (configuration mode).
+// BASELINE.json north_star: "a batched B.A^-1 grade kernel, the one genuinely dense
+// contraction".  fp64 has no tcgen05 kind; this is a register-tiled DFMA GEMM (128x64x16 CTA
+// tile, 8x4 per thread) whose epilogue folds |.| and the row maximum, so the N x n_basis
+// product is never written.  Non-negative doubles order like their bit patterns, so the row
+// maximum across column tiles is an integer atomicMax (order independent -> deterministic).
+#include <cuda_runtime.h>
+
+#include "kernels.h"
+
+namespace mtpb {
+
+constexpr int GBM = 128, GBN = 64, GBK = 16;
+
+__global__ void __launch_bounds__(256) k_grade(const double *__restrict__ B, const double *__restrict__ Ainv,
+                                               long long n, int nb, double *__restrict__ gamma) {
+  __shared__ __align__(16) double As[GBK][GBM];
+  __shared__ __align__(16) double Bs[GBK][GBN];
+  const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+  const long long m0 = (long long)blockIdx.y * GBM;
+  const int n0 = blockIdx.x * GBN;
+  double acc[8][4];
+#pragma unroll
+  for (int r = 0; r < 8; ++r)
+#pragma unroll
+    for (int c = 0; c < 4; ++c) acc[r][c] = 0.0;
+  const int arow = tid >> 1, ak = (tid & 1) * 8;        // A tile: 128 rows x 16 k
+  const int bk = tid >> 4, bc = (tid & 15) * 4;         // Ainv tile: 16 k x 64 cols
+  for (int k0 = 0; k0 < nb; k0 += GBK) {
+    {
+      const long long row = m0 + arow;
+      const double *src = B + row * nb + k0 + ak;
+#pragma unroll
+      for (int j = 0; j < 8; ++j) As[ak + j][arow] = (row < n && k0 + ak + j < nb) ? src[j] : 0.0;
+      const int kr = k0 + bk;
+      const double *s2 = Ainv + (long long)kr * nb + n0 + bc;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) Bs[bk][bc + j] = (kr < nb && n0 + bc + j < nb) ? s2[j] : 0.0;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int kk = 0; kk < GBK; ++kk) {
+      double a[8], b[4];
+      const double2 *ap = reinterpret_cast<const double2 *>(&As[kk][ty * 8]);
+      const double2 *bp = reinterpret_cast<const double2 *>(&Bs[kk][tx * 4]);
+#pragma unroll
+      for (int j = 0; j < 4; ++j) { const double2 v = ap[j]; a[2 * j] = v.x; a[2 * j + 1] = v.y; }
+#pragma unroll
+      for (int j = 0; j < 2; ++j) { const double2 v = bp[j]; b[2 * j] = v.x; b[2 * j + 1] = v.y; }
+#pragma unroll
+      for (int r = 0; r < 8; ++r)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) acc[r][c] = fma(a[r], b[c], acc[r][c]);
+    }
+    __syncthreads();
+  }
+#pragma unroll
+  for (int r = 0; r < 8; ++r) {
+    double m = fmax(fmax(fabs(acc[r][0]), fabs(acc[r][1])), fmax(fabs(acc[r][2]), fabs(acc[r][3])));
+#pragma unroll
+    for (int o = 8; o >= 1; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    const long long row = m0 + ty * 8 + r;
+    if (tx == 0 && row < n)
+      atomicMax(reinterpret_cast<unsigned long long *>(gamma) + row, (unsigned long long)__double_as_longlong(m));
+  }
+}
+
+// configuration mode: y_k = sum_a Bsum[a] Ainv[a][k]; gamma = max_k |y_k|
+__global__ void k_grade_cfg(const double *__restrict__ Bsum, const double *__restrict__ Ainv, int nb,
+                            double *__restrict__ gamma_cfg) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  double y = 0.0;
+  if (k < nb)
+    for (int a = 0; a < nb; ++a) y = fma(Bsum[a], Ainv[(long long)a * nb + k], y);
+  double m = fabs(y);
+#pragma unroll
+  for (int o = 16; o >= 1; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0)
+    atomicMax(reinterpret_cast<unsigned long long *>(gamma_cfg), (unsigned long long)__double_as_longlong(m));
+}
+
+cudaError_t launch_grade(const double *B, const double *Ainv, long long n, int nb, double *gamma, cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  cudaError_t e = launch_zero(gamma, n, st);
+  if (e != cudaSuccess) return e;
+  dim3 g((nb + GBN - 1) / GBN, (unsigned)((n + GBM - 1) / GBM));
+  k_grade<<<g, 256, 0, st>>>(B, Ainv, n, nb, gamma);
+  count_launch();
+  return cudaGetLastError();
+}
+
+cudaError_t launch_grade_cfg(const double *Bsum, const double *Ainv, int nb, double *scratch, double *gamma_cfg,
+                             cudaStream_t st) {
+  (void)scratch;
+  cudaError_t e = launch_zero(gamma_cfg, 1, st);
+  if (e != cudaSuccess) return e;
+  k_grade_cfg<<<(nb + 127) / 128, 128, 0, st>>>(Bsum, Ainv, nb, gamma_cfg);
+  count_launch();
+  return cudaGetLastError();
+}
+
+// ---- fp64 FMA throughput: 8 independent chains per thread, 4 blocks of 256 threads per SM
+__global__ void __launch_bounds__(256) k_peak_dfma(long long iters, double *sink) {
+  double a0 = 1.0 + threadIdx.x * 1e-9, a1 = a0 + 1e-3, a2 = a0 + 2e-3, a3 = a0 + 3e-3;
+  double a4 = a0 + 4e-3, a5 = a0 + 5e-3, a6 = a0 + 6e-3, a7 = a0 + 7e-3;
+  const double m = 0.999999, c = 1e-7;
+  for (long long i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+      a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+    }
+  }
+  const double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+  if (s == 123.456) sink[0] = s;
+}
+
+cudaError_t launch_peak_dfma(long long iters, double *sink, double *flops_out, cudaStream_t st) {
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const int grid = sms * 4;
+  k_peak_dfma<<<grid, 256, 0, st>>>(iters, sink);
+  count_launch();
+  if (flops_out) *flops_out = 2.0 * 64.0 * (double)iters * 256.0 * grid;
+  return cudaGetLastError();
+}
+
+}  // namespace mtpb

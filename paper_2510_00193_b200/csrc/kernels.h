@@ -1,0 +1,59 @@
+// Internal launch interface between api.cu and the kernel translation units.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+
+#include "pair_kernels_args.h"
+#include "tree.h"
+
+namespace mtpb {
+
+void count_launch();
+long long launch_count();
+
+// ---- K2
+struct TreeArgs {
+  const TreeTerm *fterms; const TreeItem *fitems; const int *fwave; int nfw;
+  const TreeTerm *bterms; const TreeItem *bitems; const int *bwave; int nbw;
+  const int *basis_node; const double *xi; const double *xi0;
+  const double *pos4;
+  const double *M; double *G; long long ldm;
+  double *Ei;          // [N]
+  double *B;           // [N][n_basis] or null
+  int n_nodes, n_basic, n_basis;
+  int c0, c1;
+  int want_adj;
+};
+int tree_pick_al(int n_nodes);
+size_t tree_smem_bytes(int n_nodes, int AL);
+cudaError_t launch_tree(const TreeArgs &a, int AL, cudaStream_t st);
+
+// ---- K1 / K3: one entry per compiled level (pair_lev*.cu)
+struct PairLevel {
+  int lev, nsb, nsc, nslot, p_small;
+  cudaError_t (*moments)(const PairArgs &a, int P, cudaStream_t st);
+  cudaError_t (*pairgrad)(const PairArgs &a, int P, int atomic, cudaStream_t st, int *grid_out);
+  int (*pairgrad_grid)(int n_atoms, int P);
+};
+const PairLevel *pair_level(int index);   // index into kLevels
+
+// ---- misc kernels (misc_kernels.cu)
+cudaError_t launch_pack(const double *pos, const int *type, int n, double *pos4, cudaStream_t st);
+cudaError_t launch_zero(double *p, long long n, cudaStream_t st);
+// F_k = sum_p d[p] - d[rev[p]] over row k (warp per atom, fixed order)
+cudaError_t launch_gather(const long long *off, const int *rev, const double *d4, int n, double *F, cudaStream_t st);
+// out[c] = sum_i in[i*stride + c] for c < ncomp, single block, fixed order
+cudaError_t launch_reduce(const double *in, long long n, int stride, int ncomp, double *out, cudaStream_t st);
+// Bsum[b] = sum_i B[i][b]  (fixed order per column)
+cudaError_t launch_colsum(const double *B, long long n, int nb, double *Bsum, double *scratch, cudaStream_t st);
+
+// ---- K5 (grade_kernel.cu)
+// gamma[i] = max_k | sum_a B[i][a] Ainv[a][k] |
+cudaError_t launch_grade(const double *B, const double *Ainv, long long n, int nb, double *gamma, cudaStream_t st);
+// gamma_cfg = max_k | sum_a Bsum[a] Ainv[a][k] |
+cudaError_t launch_grade_cfg(const double *Bsum, const double *Ainv, int nb, double *scratch, double *gamma_cfg,
+                             cudaStream_t st);
+// fp64 FMA throughput microbenchmark
+cudaError_t launch_peak_dfma(long long iters, double *sink, double *flops_out, cudaStream_t st);
+
+}  // namespace mtpb

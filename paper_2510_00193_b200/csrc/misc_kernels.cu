@@ -1,0 +1,130 @@
+// Small memory-bound kernels around the hot path: input packing (a1), deterministic force
+// gather over the reverse-neighbour index (a8), fixed-order reductions of E, virial and B.
+#include <cuda_runtime.h>
+
+#include <atomic>
+
+#include "kernels.h"
+
+namespace mtpb {
+
+static std::atomic<long long> g_launches{0};
+void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+long long launch_count() { return g_launches.load(std::memory_order_relaxed); }
+
+// pos4[i] = (x, y, z, species): one aligned 32-byte sector per neighbour gather
+__global__ void k_pack(const double *__restrict__ pos, const int *__restrict__ type, int n,
+                       double *__restrict__ pos4) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double2 *o = reinterpret_cast<double2 *>(pos4) + 2 * (size_t)i;
+  o[0] = make_double2(pos[3 * (size_t)i], pos[3 * (size_t)i + 1]);
+  o[1] = make_double2(pos[3 * (size_t)i + 2], (double)type[i]);
+}
+
+__global__ void k_zero(double *p, long long n) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) p[i] = 0.0;
+}
+
+// a8 gather: F_k = sum_{p in row k} ( d[p] - d[rev[p]] ); one warp per atom, lanes over the
+// row, xor-shuffle tree -> the summation order is fixed, the result bit-reproducible (G19).
+__global__ void __launch_bounds__(256) k_gather(const long long *__restrict__ off, const int *__restrict__ rev,
+                                                const double *__restrict__ d4, int n, double *__restrict__ F) {
+  const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (warp >= n) return;
+  const long long beg = off[warp], end = off[warp + 1];
+  double fx = 0, fy = 0, fz = 0;
+  const double2 *d = reinterpret_cast<const double2 *>(d4);
+  for (long long p = beg + lane; p < end; p += 32) {
+    const long long q = rev[p];
+    const double2 a0 = d[2 * p], a1 = d[2 * p + 1];
+    const double2 b0 = __ldg(d + 2 * q), b1 = __ldg(d + 2 * q + 1);
+    fx += a0.x - b0.x; fy += a0.y - b0.y; fz += a1.x - b1.x;
+  }
+#pragma unroll
+  for (int o = 16; o >= 1; o >>= 1) {
+    fx += __shfl_xor_sync(0xffffffffu, fx, o);
+    fy += __shfl_xor_sync(0xffffffffu, fy, o);
+    fz += __shfl_xor_sync(0xffffffffu, fz, o);
+  }
+  if (lane == 0) { F[3 * (size_t)warp] = fx; F[3 * (size_t)warp + 1] = fy; F[3 * (size_t)warp + 2] = fz; }
+}
+
+// out[c] = sum_i in[i*stride + c], c < ncomp <= 8; one block of 1024 threads, fixed order
+__global__ void __launch_bounds__(1024) k_reduce_rows(const double *__restrict__ in, long long n, int stride,
+                                                      int ncomp, double *__restrict__ out) {
+  __shared__ double sm[32][8];
+  double acc[8];
+#pragma unroll
+  for (int c = 0; c < 8; ++c) acc[c] = 0.0;
+  for (long long i = threadIdx.x; i < n; i += 1024)
+    for (int c = 0; c < ncomp; ++c) acc[c] += in[i * stride + c];
+#pragma unroll
+  for (int c = 0; c < 8; ++c) {
+    double v = acc[c];
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5][c] = v;
+  }
+  __syncthreads();
+  if (threadIdx.x < ncomp) {
+    double v = 0.0;
+    for (int w = 0; w < 32; ++w) v += sm[w][threadIdx.x];
+    out[threadIdx.x] = v;
+  }
+}
+
+// partial[s][b] = sum_{i = s, s+ns, ...} B[i][b]
+__global__ void k_colsum_part(const double *__restrict__ B, long long n, int nb, double *__restrict__ part) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= nb) return;
+  double acc = 0.0;
+  for (long long i = blockIdx.y; i < n; i += gridDim.y) acc += B[i * nb + b];
+  part[(size_t)blockIdx.y * nb + b] = acc;
+}
+// Bsum[b] += sum_s partial[s][b]   (accumulates across chunks in launch order)
+__global__ void k_colsum_final(const double *__restrict__ part, int ns, int nb, double *__restrict__ Bsum) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= nb) return;
+  double acc = 0.0;
+  for (int s = 0; s < ns; ++s) acc += part[(size_t)s * nb + b];
+  Bsum[b] += acc;
+}
+
+cudaError_t launch_pack(const double *pos, const int *type, int n, double *pos4, cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  k_pack<<<(n + 255) / 256, 256, 0, st>>>(pos, type, n, pos4);
+  count_launch();
+  return cudaGetLastError();
+}
+cudaError_t launch_zero(double *p, long long n, cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  k_zero<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p, n);
+  count_launch();
+  return cudaGetLastError();
+}
+cudaError_t launch_gather(const long long *off, const int *rev, const double *d4, int n, double *F,
+                          cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  k_gather<<<(n + 7) / 8, 256, 0, st>>>(off, rev, d4, n, F);
+  count_launch();
+  return cudaGetLastError();
+}
+cudaError_t launch_reduce(const double *in, long long n, int stride, int ncomp, double *out, cudaStream_t st) {
+  k_reduce_rows<<<1, 1024, 0, st>>>(in, n, stride, ncomp, out);
+  count_launch();
+  return cudaGetLastError();
+}
+cudaError_t launch_colsum(const double *B, long long n, int nb, double *Bsum, double *scratch, cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  const int ns = 64;
+  dim3 g((nb + 127) / 128, ns);
+  k_colsum_part<<<g, 128, 0, st>>>(B, n, nb, scratch);
+  count_launch();
+  k_colsum_final<<<(nb + 127) / 128, 128, 0, st>>>(scratch, ns, nb, Bsum);
+  count_launch();
+  return cudaGetLastError();
+}
+
+}  // namespace mtpb

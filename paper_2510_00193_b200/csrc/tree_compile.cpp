@@ -1,0 +1,105 @@
+// Host-side compilation of the flat contraction table (include/mtp_b200.h) into the wave /
+// item schedule the K2 kernel interprets.  BASELINE.json north_star: "a forward/adjoint
+// contraction kernel with the tree in registers and shared memory" -- the table itself is an
+// input of mtp_create, so any valid table (not only mtp_enumerate's) is accepted.
+#include "tree.h"
+
+#include <algorithm>
+
+#include "mtp_b200.h"
+
+namespace mtpb {
+
+int tree_compile(int n_basic, int n_nodes, int n_prod, const int32_t *prod, int n_basis,
+                 const int32_t *basis_node, TreeSched &s, const char **err) {
+  static const char *e_range = "contraction table: node index out of range";
+  static const char *e_order = "contraction table: a node is read before its last write";
+  static const char *e_big = "contraction table: more than 65535 nodes";
+  if (n_nodes > 65535) { *err = e_big; return MTP_EUNSUP; }
+  s = TreeSched();
+  s.n_nodes = n_nodes; s.n_basic = n_basic; s.n_basis = n_basis; s.n_prod = n_prod;
+  std::vector<int> depth(n_nodes, 0), last_write(n_nodes, -1), first_read(n_nodes, n_prod);
+  for (int t = 0; t < n_prod; ++t) {
+    const int32_t *p = prod + 4 * t;
+    if (p[0] < 0 || p[0] >= n_nodes || p[1] < 0 || p[1] >= n_nodes || p[3] < n_basic || p[3] >= n_nodes) {
+      *err = e_range; return MTP_EINVAL;
+    }
+    last_write[p[3]] = t;
+    first_read[p[0]] = std::min(first_read[p[0]], t);
+    first_read[p[1]] = std::min(first_read[p[1]], t);
+  }
+  for (int n = n_basic; n < n_nodes; ++n)
+    if (last_write[n] >= 0 && first_read[n] <= last_write[n]) { *err = e_order; return MTP_EINVAL; }
+  for (int a = 0; a < n_basis; ++a)
+    if (basis_node[a] < 0 || basis_node[a] >= n_nodes) { *err = e_range; return MTP_EINVAL; }
+  // depth: list order is a valid evaluation order, so one pass suffices
+  for (int t = 0; t < n_prod; ++t) {
+    const int32_t *p = prod + 4 * t;
+    depth[p[3]] = std::max(depth[p[3]], 1 + std::max(depth[p[0]], depth[p[1]]));
+  }
+  int D = 0;
+  for (int n = 0; n < n_nodes; ++n) D = std::max(D, depth[n]);
+  s.depth = D;
+
+  // ---- forward rows grouped by dst, waves by depth 1..D
+  std::vector<std::vector<int>> row(n_nodes);   // op ids per dst
+  for (int t = 0; t < n_prod; ++t) row[prod[4 * t + 3]].push_back(t);
+  auto emit = [](std::vector<TreeItem> &items, std::vector<TreeTerm> &terms, int dst,
+                 const std::vector<TreeTerm> &rt) {
+    const int n = (int)rt.size();
+    const int pieces = (n + kSeg - 1) / kSeg;
+    for (int q = 0; q < pieces; ++q) {
+      TreeItem it;
+      it.dst = dst; it.begin = (int)terms.size();
+      it.n = std::min(kSeg, n - q * kSeg); it.split = pieces > 1;
+      for (int k = 0; k < it.n; ++k) terms.push_back(rt[q * kSeg + k]);
+      items.push_back(it);
+    }
+  };
+  auto by_len = [](const std::vector<TreeItem> &items, int lo, int hi, std::vector<TreeItem> &dst) {
+    std::vector<TreeItem> tmp(items.begin() + lo, items.begin() + hi);
+    std::stable_sort(tmp.begin(), tmp.end(), [](const TreeItem &x, const TreeItem &y) { return x.n > y.n; });
+    for (auto &x : tmp) dst.push_back(x);
+  };
+  {
+    std::vector<TreeItem> items;
+    s.fwave.push_back(0);
+    for (int w = 1; w <= D; ++w) {
+      const int lo = (int)items.size();
+      for (int n = n_basic; n < n_nodes; ++n) {
+        if (depth[n] != w || row[n].empty()) continue;
+        std::vector<TreeTerm> rt;
+        for (int t : row[n]) {
+          const int32_t *p = prod + 4 * t;
+          rt.push_back(TreeTerm{(uint16_t)p[0], (uint16_t)p[1], 0, (double)p[2]});
+        }
+        emit(items, s.fterms, n, rt);
+      }
+      by_len(items, lo, (int)items.size(), s.fitems);
+      s.fwave.push_back((int32_t)s.fitems.size());
+    }
+  }
+  // ---- backward rows grouped by source node, waves by depth D-1 .. 0
+  std::vector<std::vector<TreeTerm>> brow(n_nodes);
+  for (int t = 0; t < n_prod; ++t) {
+    const int32_t *p = prod + 4 * t;
+    brow[p[0]].push_back(TreeTerm{(uint16_t)p[3], (uint16_t)p[1], 0, (double)p[2]});
+    brow[p[1]].push_back(TreeTerm{(uint16_t)p[3], (uint16_t)p[0], 0, (double)p[2]});
+  }
+  {
+    std::vector<TreeItem> items;
+    s.bwave.push_back(0);
+    for (int w = D - 1; w >= 0; --w) {
+      const int lo = (int)items.size();
+      for (int n = 0; n < n_nodes; ++n) {
+        if (depth[n] != w || brow[n].empty()) continue;
+        emit(items, s.bterms, n, brow[n]);
+      }
+      by_len(items, lo, (int)items.size(), s.bitems);
+      s.bwave.push_back((int32_t)s.bitems.size());
+    }
+  }
+  return MTP_OK;
+}
+
+}  // namespace mtpb
