@@ -1,0 +1,332 @@
+#!/usr/bin/env python
+"""bench.py -- MTP energy+force atom-evaluations/s on one B200 (or N replicas, weak scaling).
+
+A "step" is one pass of the whole hot path (rows a1-a8, a10 of SURVEY.md 8(a)) over the
+BASELINE.json configs[3] workload: 1,048,576 atoms, 3 species, FCC 64^3, level 16, fp64,
+chunked evaluation.  `value` is device-resident throughput (CUDA events), `e2e` the same
+metric through mtp_compute_host with pinned HOST buffers (H2D + D2H inside the timed region).
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                  [--config I] [--cells C] [--grade]        (the last three: profiling aids)
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+LEVELS = [10, 16, 20, 16, 24]
+METRIC = "MTP energy+force atom-evals/s at ~1M atoms lev16 fp64"
+UNIT = "atom-evals/s"
+
+
+def survey_flops(lev, n_mu, n_basic, n_prod, n_basis, nu_max):
+    """Useful flops (FMA = 2): F_pair = 60 + 32 n_mu + 2 C(nu_max+3,3) + 10 n_basic,
+    split K1 (moments) / K3 (pair derivative); tree 6 n_prod + 2 n_basis per atom."""
+    mono = (nu_max + 1) * (nu_max + 2) * (nu_max + 3) // 6
+    k1 = 30 + 16 * n_mu + 2 * mono + 2 * n_basic
+    k3 = 30 + 16 * n_mu + 8 * n_basic
+    tree = 6 * n_prod + 2 * n_basis
+    return dict(k1_per_pair=k1, k3_per_pair=k3, tree_per_atom=tree)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.path = tempfile.mktemp(prefix="mtp_clocks_", suffix=".csv")
+        self.gpu = gpu_index
+        self.proc = None
+
+    def start(self):
+        try:
+            self.f = open(self.path, "w")
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[])
+        if self.proc is None:
+            return out
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.f.close()
+        sm, mx, reasons = [], [], set()
+        for line in open(self.path):
+            p = [x.strip() for x in line.split(",")]
+            if len(p) < 9:
+                continue
+            try:
+                sm.append(float(p[1])); mx.append(float(p[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), p[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        os.unlink(self.path)
+        if sm:
+            out = dict(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons),
+                       samples=len(sm))
+        return out
+
+
+def build_workload(config, cells, seed_shift=0):
+    from workloads import make_workload, CONFIGS
+    import paper_2510_00193_b200 as lib
+    table = lib.Table(LEVELS[config])
+    from workloads.lattice import BASE_SEED
+    w = make_workload(config, table.n_basis, cells=cells, with_ainv=None,
+                      seed=BASE_SEED + config + 1000 * seed_shift)
+    return w, table, CONFIGS[config]
+
+
+def oracle_rate(w, n_sample, want_grad=True):
+    """atom-evals/s of the CPU oracle on the first n_sample atoms of the workload."""
+    from oracle import mtp as omtp
+    pot = omtp.Potential(w.lev_max, w.n_mu, w.n_beta, w.r_min, w.r_cut, w.c, w.xi0, w.xi)
+    atoms = range(min(n_sample, w.n_atoms))
+    t0 = time.perf_counter()
+    omtp.evaluate(pot, w.pos, w.types, w.box, w.off, w.idx, w.shift, atoms=atoms, want_grad=want_grad)
+    dt = time.perf_counter() - t0
+    return len(atoms) / dt, dt, len(atoms)
+
+
+def run_reference(args):
+    """--impl reference: the oracle timed on host cores; each step is a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    try:
+        from threadpoolctl import threadpool_limits
+        ctx = threadpool_limits(limits=1)
+    except Exception:
+        ctx = None
+    w, table, cfg = build_workload(args.config, args.cells)
+    n_sample = args.ref_atoms
+    for _ in range(args.warmup):
+        oracle_rate(w, n_sample)
+    t = 0.0
+    n = 0
+    for _ in range(args.steps):
+        r, dt, k = oracle_rate(w, n_sample)
+        t += dt
+        n += k
+    value = n / t
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"], "n_atoms": w.n_atoms, "nnz": w.nnz, "lev_max": w.lev_max,
+                   "n_species": w.n_species},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
+                         "sample": "first %d atoms of the workload per step, E_i + d_ij + force scatter" % n_sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import torch
+    import paper_2510_00193_b200 as lib
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_
+        dist = dist_
+        dist.init_process_group("nccl", device_id=dev)
+
+    w, table, cfg = build_workload(args.config, args.cells, seed_shift=rank)
+    pot = lib.Potential(table, w.n_species, w.n_beta, w.r_min, w.r_cut, w.c, w.xi0, w.xi)
+    if args.chunk >= 0:
+        pot.set_option(lib.OPT_CHUNK_ATOMS, args.chunk)
+    if args.force_mode >= 0:
+        pot.set_option(lib.OPT_FORCE_MODE, args.force_mode)
+    pot.set_option(lib.OPT_PROFILE, 1)
+    t = lambda a, dt: torch.as_tensor(np.ascontiguousarray(a), dtype=dt).to(dev)
+    pos, types, off, idx = t(w.pos, torch.float64), t(w.types, torch.int32), t(w.off, torch.int64), t(w.idx, torch.int32)
+    shift, rev = t(w.shift, torch.int8), t(w.rev, torch.int32)
+    Ainv = t(w.Ainv, torch.float64) if (args.grade and w.Ainv is not None) else None
+
+    def step(out=None):
+        o = pot.compute(pos, types, w.box, off, idx, shift, rev, out=out)
+        if Ainv is not None:
+            pot.grade(pos, types, w.box, off, idx, Ainv, shift, mode=2)
+        return o
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    out = None
+    for _ in range(max(args.warmup, 0)):
+        out = step(out)
+    torch.cuda.synchronize()
+    pot.profile_read()
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    n0 = lib.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        out = step(out)
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    launches = lib.launch_count() - n0
+    ms = e0.elapsed_time(e1)
+    prof = pot.profile_read()
+    if dist is not None:
+        tt = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms = float(tt.item())
+    value = world * w.n_atoms * args.steps / (ms * 1e-3)
+
+    # ---- end to end through the host-buffer entry point (pinned inputs, results read back)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+    hp = dict(pos=pin(w.pos), types=pin(w.types), off=pin(w.off), idx=pin(w.idx), shift=pin(w.shift), rev=pin(w.rev))
+    hout = dict(E=pin(np.zeros(1)), Ei=pin(np.zeros(w.n_atoms)), F=pin(np.zeros((w.n_atoms, 3))), virial=pin(np.zeros(6)))
+    e2e_steps = max(1, min(args.steps, 3))
+    pot.compute_host(hp["pos"], hp["types"], w.box, hp["off"], hp["idx"], hp["shift"], hp["rev"], out=hout)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        pot.compute_host(hp["pos"], hp["types"], w.box, hp["off"], hp["idx"], hp["shift"], hp["rev"], out=hout)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        tt = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_s = float(tt.item())
+    h2d = sum(hp[k].nbytes for k in hp)
+    d2h = sum(hout[k].nbytes for k in hout)
+    e2e_value = world * w.n_atoms * e2e_steps / e2e_s
+    pot.profile_read()
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (fp64 ALU bound)
+    nu_max = int(table.basic[:, 1:].sum(axis=1).max())
+    fl = survey_flops(w.lev_max, w.n_mu, table.n_basic, table.n_prod, table.n_basis, nu_max)
+    per_step = {"moments": fl["k1_per_pair"] * w.nnz, "pairgrad": fl["k3_per_pair"] * w.nnz,
+                "tree": fl["tree_per_atom"] * w.n_atoms}
+    timed = {k: prof[k] for k in ("moments", "tree", "pairgrad")}
+    dom = max(timed, key=lambda k: timed[k][0])
+    dom_ms, dom_n = timed[dom]
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    peak_tf = sms * 64 * 2 * 1.965e9 / 1e12          # 64 fp64 FMA / clk / SM at clocks.max.sm
+    achieved_tf = per_step[dom] * args.steps / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
+    step_tf = sum(per_step.values()) * args.steps / (ms * 1e-3) / 1e12
+    # measured DFMA throughput of this box (own microbenchmark, reported beside the derived peak)
+    sink = torch.zeros(8, dtype=torch.float64, device=dev)
+    lib.peak_dfma(2000, sink)
+    torch.cuda.synchronize()
+    a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a0.record()
+    pk = lib.peak_dfma(20000, sink)
+    a1.record()
+    torch.cuda.synchronize()
+    measured_tf = pk / (a0.elapsed_time(a1) * 1e-3) / 1e12
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get(dom)
+        except Exception:
+            traffic = None
+
+    # ---- CPU baseline: the oracle on a bounded sample of the same workload
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        try:
+            from threadpoolctl import threadpool_limits
+            lim = threadpool_limits(limits=1)
+        except Exception:
+            lim = None
+        rate, dt, k = oracle_rate(w, args.ref_atoms)
+        cpu = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": "first %d atoms of the workload (E_i, d_ij, force scatter), %.1f s" % (k, dt)}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"], "n_atoms": w.n_atoms, "nnz": w.nnz, "lev_max": w.lev_max,
+                   "n_species": w.n_species, "n_basis": table.n_basis, "chunk_atoms": pot.get_option(lib.OPT_CHUNK_ATOMS),
+                   "force_mode": pot.get_option(lib.OPT_FORCE_MODE), "grade": bool(Ainv is not None),
+                   "l2": "inputs larger than L2 (neighbour list %.0f MB + per-pair scratch), no flush" % (w.nnz * 11 / 1e6),
+                   "parallelism": "replicas x%d" % world},
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                "steps": e2e_steps},
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                     "frac": achieved_tf / peak_tf, "traffic": traffic,
+                     "peak_source": "derived: %d SMs x 64 fp64 FMA/clk x 2 x 1.965 GHz; measured DFMA microbenchmark %.1f TF/s" % (sms, measured_tf),
+                     "flops_per_launch": per_step[dom] / max(dom_n / args.steps, 1), "launches": dom_n,
+                     "avg_launch_ms": dom_ms / max(dom_n, 1),
+                     "step_achieved": step_tf, "step_frac": step_tf / peak_tf,
+                     "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()}},
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="0-based index into BASELINE.json configs")
+    ap.add_argument("--cells", type=int, default=None, help="override the lattice repeat (scaled-down instance)")
+    ap.add_argument("--chunk", type=int, default=-1)
+    ap.add_argument("--force-mode", type=int, default=-1)
+    ap.add_argument("--grade", action="store_true", help="also run mtp_grade each step (config 4)")
+    ap.add_argument("--ref-atoms", type=int, default=1024, help="atoms per oracle sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -89,6 +89,7 @@ const char *mtp_last_error(const mtp_handle *h); /* h may be NULL: last create e
 #define MTP_OPT_CHUNK_ATOMS 1   /* atoms per chunk; 0 = automatic (L2-sized)               */
 #define MTP_OPT_FORCE_MODE 2    /* MTP_FORCE_GATHER (needs d_rev) | MTP_FORCE_ATOMIC       */
 #define MTP_OPT_VARIANT 3       /* MTP_VARIANT_AUTO | _THREAD | _BLOCK                     */
+#define MTP_OPT_PROFILE 4       /* 1: record CUDA events around every kernel launch        */
 #define MTP_FORCE_GATHER 0      /* deterministic; keeps d_ij for all pairs (nnz x 32 B)  */
 #define MTP_FORCE_ATOMIC 1      /* fp64 atomic scatter; no per-pair scratch              */
 #define MTP_FORCE_AUTO 2        /* default: gather when d_rev is given, else atomic      */
@@ -144,6 +145,10 @@ int mtp_debug_moments(mtp_handle *h, int64_t n_atoms, const double *d_pos,
                       const int32_t *d_type, const double *box, const int64_t *d_off,
                       const int32_t *d_idx, const int8_t *d_shift, double *d_M, double *d_G,
                       double *d_B, void *d_ws, size_t ws_bytes, void *cuda_stream);
+/* With MTP_OPT_PROFILE on: device time (ms, CUDA events on the launching stream) and launch
+ * count per kernel class since the last read; classes: 0 moments (K1), 1 tree (K2),
+ * 2 pair gradient (K3), 3 force gather, 4 grade (K5).  Synchronises on the recorded events. */
+int mtp_profile_read(mtp_handle *h, double *ms /*[5]*/, int64_t *launches /*[5]*/);
 /* Number of kernels this library has launched since load (bench.py gpu_launches). */
 int64_t mtp_launch_count(void);
 /* fp64 FMA throughput microbenchmark: runs `iters` dependent-chain DFMA batches on every

@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmtp_b200.so")
 
 OK, EINVAL, ESIZE, EBOX, ECUDA, EUNSUP, ENOMEM = 0, -1, -2, -3, -4, -5, -6
-OPT_CHUNK_ATOMS, OPT_FORCE_MODE, OPT_VARIANT = 1, 2, 3
+OPT_CHUNK_ATOMS, OPT_FORCE_MODE, OPT_VARIANT, OPT_PROFILE = 1, 2, 3, 4
 FORCE_GATHER, FORCE_ATOMIC, FORCE_AUTO = 0, 1, 2
 VARIANT_AUTO, VARIANT_THREAD, VARIANT_BLOCK = 0, 1, 2
 
@@ -36,14 +36,23 @@ class MtpParams(C.Structure):
 EXPORTS = ["mtp_enumerate", "mtp_table_free", "mtp_create", "mtp_destroy", "mtp_last_error",
            "mtp_set_option", "mtp_get_option", "mtp_workspace_bytes", "mtp_compute", "mtp_grade",
            "mtp_compute_host", "mtp_debug_moments", "mtp_launch_count", "mtp_peak_dfma",
-           "mtp_cost_model"]
+           "mtp_cost_model", "mtp_profile_read"]
+
+
+def _build():
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("_mtp_b200_build", os.path.join(_HERE, "build.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    mod.build()
 
 
 def _load():
     if not os.path.exists(LIB_PATH):
-        from . import build as _b
-        _b.build()
+        _build()
     lib = C.CDLL(LIB_PATH)
+    if not all(hasattr(lib, name) for name in EXPORTS):
+        raise ImportError("%s is stale (missing exports): run `python paper_2510_00193_b200/build.py`" % LIB_PATH)
     vp, i64, dbl = C.c_void_p, C.c_int64, C.c_double
     lib.mtp_enumerate.argtypes = [C.c_int32, C.POINTER(MtpParams)]
     lib.mtp_table_free.argtypes = [C.POINTER(MtpParams)]
@@ -65,6 +74,7 @@ def _load():
     lib.mtp_launch_count.restype = i64
     lib.mtp_peak_dfma.argtypes = [i64, vp, C.POINTER(dbl), vp]
     lib.mtp_cost_model.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl)]
+    lib.mtp_profile_read.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
     return lib
 
 
@@ -176,6 +186,14 @@ class Potential:
         a, b, c = C.c_double(), C.c_double(), C.c_double()
         self._check(_lib.mtp_cost_model(self._h, C.byref(a), C.byref(b), C.byref(c)))
         return dict(flop_per_pair=a.value, flop_per_atom_tree=b.value, flop_per_atom_grade=c.value)
+
+    def profile_read(self):
+        """dict class -> (ms, launches) since the last read (needs OPT_PROFILE = 1)."""
+        ms = (C.c_double * 5)()
+        n = (C.c_int64 * 5)()
+        self._check(_lib.mtp_profile_read(self._h, ms, n))
+        names = ["moments", "tree", "pairgrad", "gather", "grade"]
+        return {k: (ms[i], int(n[i])) for i, k in enumerate(names)}
 
     def _workspace(self, nbytes, device):
         import torch

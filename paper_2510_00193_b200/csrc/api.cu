@@ -41,7 +41,8 @@ struct mtp_handle {
   int *d_kmapF = nullptr, *d_kmapB = nullptr, *d_basis_node = nullptr;
   TreeTerm *d_fterms = nullptr, *d_bterms = nullptr;
   TreeItem *d_fitems = nullptr, *d_bitems = nullptr;
-  int *d_fwave = nullptr, *d_bwave = nullptr;
+  int *d_fwave = nullptr, *d_bwave = nullptr, *d_seed_node = nullptr;
+  double *d_seed_val = nullptr;
   TreeSched sched;
   int64_t chunk_atoms = 0;
   int force_mode = MTP_FORCE_AUTO, variant = MTP_VARIANT_AUTO;
@@ -50,7 +51,31 @@ struct mtp_handle {
   void *stage = nullptr;
   size_t stage_bytes = 0;
   std::vector<void *> to_free;
+  // per-kernel-class device timing (MTP_OPT_PROFILE): event pairs recorded around each launch
+  int profile = 0;
+  struct Span { cudaEvent_t a, b; int cls; };
+  std::vector<Span> spans;
+  std::vector<cudaEvent_t> pool;
 };
+
+namespace {
+enum { CLS_MOMENTS = 0, CLS_TREE = 1, CLS_PAIRGRAD = 2, CLS_OTHER = 3, CLS_GRADE = 4, N_CLS = 5 };
+cudaEvent_t prof_event(mtp_handle *h) {
+  if (!h->pool.empty()) { cudaEvent_t e = h->pool.back(); h->pool.pop_back(); return e; }
+  cudaEvent_t e = nullptr;
+  cudaEventCreate(&e);
+  return e;
+}
+struct ProfScope {
+  mtp_handle *h; cudaStream_t st; mtp_handle::Span s; bool on;
+  ProfScope(mtp_handle *h_, int cls, cudaStream_t st_) : h(h_), st(st_), on(h_->profile != 0) {
+    if (on) { s.a = prof_event(h); s.b = prof_event(h); s.cls = cls; cudaEventRecord(s.a, st); }
+  }
+  ~ProfScope() { if (on) { cudaEventRecord(s.b, st); h->spans.push_back(s); } }
+};
+}  // namespace
+#define TIMED(h, cls, st, call) do { ProfScope ps__(h, cls, st); CU(h, call); } while (0)
+
 
 static int fail(mtp_handle *h, int code, const std::string &msg) {
   if (h) h->err = msg; else g_create_error = msg;
@@ -119,8 +144,24 @@ static void build_kmaps(const PairLevel &pl, int n_basic, const int32_t *basic, 
 extern "C" const char *mtp_last_error(const mtp_handle *h) { return h ? h->err.c_str() : g_create_error.c_str(); }
 extern "C" int64_t mtp_launch_count(void) { return launch_count(); }
 
+extern "C" int mtp_profile_read(mtp_handle *h, double *ms, int64_t *launches) {
+  if (!h || !ms || !launches) return MTP_EINVAL;
+  for (int c = 0; c < N_CLS; ++c) { ms[c] = 0.0; launches[c] = 0; }
+  for (auto &s : h->spans) {
+    if (cudaEventSynchronize(s.b) != cudaSuccess) return cuda_fail(h, cudaGetLastError(), "mtp_profile_read");
+    float t = 0.f;
+    cudaEventElapsedTime(&t, s.a, s.b);
+    ms[s.cls] += t; launches[s.cls] += 1;
+    h->pool.push_back(s.a); h->pool.push_back(s.b);
+  }
+  h->spans.clear();
+  return MTP_OK;
+}
+
 extern "C" void mtp_destroy(mtp_handle *h) {
   if (!h) return;
+  for (auto &s : h->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
+  for (auto e : h->pool) cudaEventDestroy(e);
   for (void *p : h->to_free) cudaFree(p);
   if (h->stage) cudaFree(h->stage);
   delete h;
@@ -154,10 +195,11 @@ extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
   h->n_nodes = p->n_nodes; h->n_basis = p->n_basis; h->lev_max = p->lev_max; h->r_min = p->r_min; h->r_cut = p->r_cut;
   h->pl = pair_level(li);
   const char *terr = "";
-  int rc = tree_compile(p->n_basic, p->n_nodes, p->n_prod, p->prod, p->n_basis, p->basis_node, h->sched, &terr);
-  if (rc != MTP_OK) { g_create_error = terr; delete h; return rc; }
   h->AL = tree_pick_al(p->n_nodes);
   if (h->AL == 0) { delete h; return fail(nullptr, MTP_EUNSUP, "contraction tree does not fit in shared memory (n_nodes*16 B > 220 KB)"); }
+  int rc = tree_compile(p->n_basic, p->n_nodes, p->n_prod, p->prod, p->n_basis, p->basis_node, p->xi, 128 / h->AL,
+                        h->sched, &terr);
+  if (rc != MTP_OK) { g_create_error = terr; delete h; return rc; }
   // radial coefficients: rows (z_i, z_j) padded to the level's n_mu, odd row stride (bank spread)
   const int nmu_lev = rt_nmu(h->pl->lev);
   h->crow = nmu_lev * h->nb + 1;
@@ -181,6 +223,8 @@ extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
   up(upload(h, &h->d_bitems, h->sched.bitems.data(), h->sched.bitems.size()));
   up(upload(h, &h->d_fwave, h->sched.fwave.data(), h->sched.fwave.size()));
   up(upload(h, &h->d_bwave, h->sched.bwave.data(), h->sched.bwave.size()));
+  up(upload(h, &h->d_seed_node, h->sched.seed_node.data(), h->sched.seed_node.size()));
+  up(upload(h, &h->d_seed_val, h->sched.seed_val.data(), h->sched.seed_val.size()));
   if (e != cudaSuccess) { int r = cuda_fail(nullptr, e, "mtp_create upload"); mtp_destroy(h); return r; }
   *out = h;
   return MTP_OK;
@@ -192,6 +236,7 @@ extern "C" int mtp_set_option(mtp_handle *h, int key, int64_t v) {
     case MTP_OPT_CHUNK_ATOMS: if (v < 0) return fail(h, MTP_EINVAL, "chunk_atoms < 0"); h->chunk_atoms = v; return MTP_OK;
     case MTP_OPT_FORCE_MODE: if (v < 0 || v > 2) return fail(h, MTP_EINVAL, "bad force mode"); h->force_mode = (int)v; return MTP_OK;
     case MTP_OPT_VARIANT: if (v < 0 || v > 2) return fail(h, MTP_EINVAL, "bad variant"); h->variant = (int)v; return MTP_OK;
+    case MTP_OPT_PROFILE: h->profile = v != 0; return MTP_OK;
   }
   return fail(h, MTP_EINVAL, "unknown option");
 }
@@ -201,6 +246,7 @@ extern "C" int mtp_get_option(const mtp_handle *h, int key, int64_t *v) {
     case MTP_OPT_CHUNK_ATOMS: *v = h->chunk_atoms; return MTP_OK;
     case MTP_OPT_FORCE_MODE: *v = h->force_mode; return MTP_OK;
     case MTP_OPT_VARIANT: *v = h->variant; return MTP_OK;
+    case MTP_OPT_PROFILE: *v = h->profile; return MTP_OK;
   }
   return MTP_EINVAL;
 }
@@ -283,6 +329,7 @@ void fill_tree_args(const mtp_handle *h, TreeArgs &ta, const double *pos4) {
   ta.fterms = h->d_fterms; ta.fitems = h->d_fitems; ta.fwave = h->d_fwave; ta.nfw = (int)h->sched.fwave.size() - 1;
   ta.bterms = h->d_bterms; ta.bitems = h->d_bitems; ta.bwave = h->d_bwave; ta.nbw = (int)h->sched.bwave.size() - 1;
   ta.basis_node = h->d_basis_node; ta.xi = h->d_xi; ta.xi0 = h->d_xi0; ta.pos4 = pos4;
+  ta.seed_node = h->d_seed_node; ta.seed_val = h->d_seed_val; ta.n_seed = (int)h->sched.seed_node.size();
   ta.n_nodes = h->n_nodes; ta.n_basic = h->n_basic; ta.n_basis = h->n_basis;
   ta.B = nullptr; ta.want_adj = 1;
 }
@@ -334,14 +381,14 @@ extern "C" int mtp_compute(mtp_handle *h, int64_t N, const double *d_pos, const 
   for (int c = 0; c < pl.n_chunks; ++c) {
     pa.c0 = (int)(c * pl.C); pa.c1 = (int)std::min<int64_t>(N, (c + 1) * pl.C);
     pa.M = M; pa.G = G; pa.kmap = h->d_kmapF;
-    CU(h, h->pl->moments(pa, pl.P, st));
+    TIMED(h, CLS_MOMENTS, st, h->pl->moments(pa, pl.P, st));
     ta.c0 = pa.c0; ta.c1 = pa.c1;
-    CU(h, launch_tree(ta, h->AL, st));
+    TIMED(h, CLS_TREE, st, launch_tree(ta, h->AL, st));
     pa.kmap = h->d_kmapB; pa.wpart = wpart + (size_t)c * pl.grid_chunk * 8;
     pa.d4 = pl.atomic ? nullptr : d4; pa.F = pl.atomic ? d_F : nullptr;
-    CU(h, h->pl->pairgrad(pa, pl.P, pl.atomic, st, nullptr));
+    TIMED(h, CLS_PAIRGRAD, st, h->pl->pairgrad(pa, pl.P, pl.atomic, st, nullptr));
   }
-  if (!pl.atomic) CU(h, launch_gather((const long long *)d_off, d_rev, d4, (int)N, d_F, st));
+  if (!pl.atomic) TIMED(h, CLS_OTHER, st, launch_gather((const long long *)d_off, d_rev, d4, (int)N, d_F, st));
   CU(h, launch_reduce(Ei, N, 1, 1, d_E, st));
   if (d_virial) CU(h, launch_reduce(wpart, (long long)pl.n_chunks * pl.grid_chunk, 8, 6, d_virial, st));
   return MTP_OK;
@@ -381,15 +428,15 @@ extern "C" int mtp_grade(mtp_handle *h, int64_t N, const double *d_pos, const in
     for (int c = 0; c < pl.n_chunks; ++c) {
       pa.c0 = (int)(c * pl.C); pa.c1 = (int)std::min<int64_t>(N, (c + 1) * pl.C);
       pa.M = M; pa.kmap = h->d_kmapF;
-      CU(h, h->pl->moments(pa, pl.P, st));
+      TIMED(h, CLS_MOMENTS, st, h->pl->moments(pa, pl.P, st));
       ta.c0 = pa.c0; ta.c1 = pa.c1;
       // B rows are indexed by absolute atom: point the kernel at a base shifted by -c0 rows
       double *Brows = d_B ? d_B : Bc - (size_t)pa.c0 * h->n_basis;
       ta.B = Brows;
-      CU(h, launch_tree(ta, h->AL, st));
+      TIMED(h, CLS_TREE, st, launch_tree(ta, h->AL, st));
       const double *Bchunk = Brows + (size_t)pa.c0 * h->n_basis;
       const int64_t nc = pa.c1 - pa.c0;
-      if (mode != 1) CU(h, launch_grade(Bchunk, d_Ainv, nc, h->n_basis, d_gamma_atom + pa.c0, st));
+      if (mode != 1) TIMED(h, CLS_GRADE, st, launch_grade(Bchunk, d_Ainv, nc, h->n_basis, d_gamma_atom + pa.c0, st));
       if (mode != 0 || d_Bsum) CU(h, launch_colsum(Bchunk, nc, h->n_basis, Bsum, part, st));
     }
   }

@@ -16,6 +16,7 @@ struct TreeArgs {
   const TreeTerm *fterms; const TreeItem *fitems; const int *fwave; int nfw;
   const TreeTerm *bterms; const TreeItem *bitems; const int *bwave; int nbw;
   const int *basis_node; const double *xi; const double *xi0;
+  const int *seed_node; const double *seed_val; int n_seed;
   const double *pos4;
   const double *M; double *G; long long ldm;
   double *Ei;          // [N]

@@ -1,7 +1,9 @@
 // Compiled form of the contraction table for the K2 kernel (rows a5, a6 of SURVEY.md 8(a)):
 // forward rows  node[dst] = sum_t mult_t node[a_t] node[b_t]           (waves by depth)
 // backward rows adj[n]   += sum_t mult_t adj[dst_t] node[other_t]     (waves by depth, deepest first)
-// Rows are cut into items of at most kSeg terms so that the row-lanes of a CTA stay balanced.
+// A row is never split (no atomics -> bit-reproducible); the host deals the rows of a wave to
+// the R row-lanes of a CTA by longest-processing-time-first and pads the lanes to equal item
+// counts, so item (k, rl) of a wave sits at wave_begin + k*R + rl.
 #pragma once
 #include <cstdint>
 #include <vector>
@@ -17,21 +19,22 @@ struct TreeItem {      // 16 bytes
   int32_t dst;         // fwd: node written; bwd: node whose adjoint is accumulated
   int32_t begin;       // first term
   int32_t n;           // number of terms
-  int32_t split;       // 1: row is cut into several items -> accumulate atomically
+  int32_t pad;
 };
-
-constexpr int kSeg = 8;
 
 struct TreeSched {
   int n_nodes = 0, n_basic = 0, n_basis = 0, depth = 0;
   std::vector<TreeTerm> fterms, bterms;
   std::vector<TreeItem> fitems, bitems;
   std::vector<int32_t> fwave, bwave;   // item offsets per wave, size n_waves + 1
+  std::vector<int32_t> seed_node;      // adjoint seeds: adj[seed_node[s]] = seed_val[s] (unique nodes)
+  std::vector<double> seed_val;        // = sum of xi over the basis functions that live on that node
+  int R = 0;                           // row-lanes the schedule was dealt for
   long long n_prod = 0;
 };
 
 // returns 0 or a negative MTP_E* code; err receives a message
 int tree_compile(int n_basic, int n_nodes, int n_prod, const int32_t *prod, int n_basis,
-                 const int32_t *basis_node, TreeSched &out, const char **err);
+                 const int32_t *basis_node, const double *xi, int R, TreeSched &out, const char **err);
 
 }  // namespace mtpb

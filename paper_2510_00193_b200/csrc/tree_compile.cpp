@@ -11,7 +11,7 @@
 namespace mtpb {
 
 int tree_compile(int n_basic, int n_nodes, int n_prod, const int32_t *prod, int n_basis,
-                 const int32_t *basis_node, TreeSched &s, const char **err) {
+                 const int32_t *basis_node, const double *xi, int R, TreeSched &s, const char **err) {
   static const char *e_range = "contraction table: node index out of range";
   static const char *e_order = "contraction table: a node is read before its last write";
   static const char *e_big = "contraction table: more than 65535 nodes";
@@ -44,40 +44,45 @@ int tree_compile(int n_basic, int n_nodes, int n_prod, const int32_t *prod, int 
   // ---- forward rows grouped by dst, waves by depth 1..D
   std::vector<std::vector<int>> row(n_nodes);   // op ids per dst
   for (int t = 0; t < n_prod; ++t) row[prod[4 * t + 3]].push_back(t);
-  auto emit = [](std::vector<TreeItem> &items, std::vector<TreeTerm> &terms, int dst,
-                 const std::vector<TreeTerm> &rt) {
-    const int n = (int)rt.size();
-    const int pieces = (n + kSeg - 1) / kSeg;
-    for (int q = 0; q < pieces; ++q) {
-      TreeItem it;
-      it.dst = dst; it.begin = (int)terms.size();
-      it.n = std::min(kSeg, n - q * kSeg); it.split = pieces > 1;
-      for (int k = 0; k < it.n; ++k) terms.push_back(rt[q * kSeg + k]);
-      items.push_back(it);
+  // deal the rows of one wave to R lanes: longest first, always to the least-loaded lane
+  struct Row { int dst; std::vector<TreeTerm> terms; };
+  auto deal = [R](std::vector<Row> &rows, std::vector<TreeItem> &items, std::vector<TreeTerm> &terms) {
+    std::stable_sort(rows.begin(), rows.end(), [](const Row &x, const Row &y) { return x.terms.size() > y.terms.size(); });
+    std::vector<long long> load(R, 0);
+    std::vector<std::vector<int>> mine(R);
+    for (int r = 0; r < (int)rows.size(); ++r) {
+      int best = 0;
+      for (int l = 1; l < R; ++l) if (load[l] < load[best]) best = l;
+      load[best] += (long long)rows[r].terms.size() + 2;   // +2: per-row overhead (item load, store)
+      mine[best].push_back(r);
     }
-  };
-  auto by_len = [](const std::vector<TreeItem> &items, int lo, int hi, std::vector<TreeItem> &dst) {
-    std::vector<TreeItem> tmp(items.begin() + lo, items.begin() + hi);
-    std::stable_sort(tmp.begin(), tmp.end(), [](const TreeItem &x, const TreeItem &y) { return x.n > y.n; });
-    for (auto &x : tmp) dst.push_back(x);
-  };
-  {
-    std::vector<TreeItem> items;
-    s.fwave.push_back(0);
-    for (int w = 1; w <= D; ++w) {
-      const int lo = (int)items.size();
-      for (int n = n_basic; n < n_nodes; ++n) {
-        if (depth[n] != w || row[n].empty()) continue;
-        std::vector<TreeTerm> rt;
-        for (int t : row[n]) {
-          const int32_t *p = prod + 4 * t;
-          rt.push_back(TreeTerm{(uint16_t)p[0], (uint16_t)p[1], 0, (double)p[2]});
-        }
-        emit(items, s.fterms, n, rt);
+    size_t K = 0;
+    for (int l = 0; l < R; ++l) K = std::max(K, mine[l].size());
+    const size_t base = items.size();
+    items.resize(base + K * R, TreeItem{-1, 0, 0, 0});
+    for (int l = 0; l < R; ++l)
+      for (size_t k = 0; k < mine[l].size(); ++k) {
+        const Row &row = rows[mine[l][k]];
+        TreeItem it{row.dst, (int32_t)terms.size(), (int32_t)row.terms.size(), 0};
+        terms.insert(terms.end(), row.terms.begin(), row.terms.end());
+        items[base + k * R + l] = it;
       }
-      by_len(items, lo, (int)items.size(), s.fitems);
-      s.fwave.push_back((int32_t)s.fitems.size());
+  };
+  s.R = R;
+  s.fwave.push_back(0);
+  for (int w = 1; w <= D; ++w) {
+    std::vector<Row> rows;
+    for (int n = n_basic; n < n_nodes; ++n) {
+      if (depth[n] != w || row[n].empty()) continue;
+      Row r; r.dst = n;
+      for (int t : row[n]) {
+        const int32_t *p = prod + 4 * t;
+        r.terms.push_back(TreeTerm{(uint16_t)p[0], (uint16_t)p[1], 0, (double)p[2]});
+      }
+      rows.push_back(std::move(r));
     }
+    deal(rows, s.fitems, s.fterms);
+    s.fwave.push_back((int32_t)s.fitems.size());
   }
   // ---- backward rows grouped by source node, waves by depth D-1 .. 0
   std::vector<std::vector<TreeTerm>> brow(n_nodes);
@@ -86,18 +91,22 @@ int tree_compile(int n_basic, int n_nodes, int n_prod, const int32_t *prod, int 
     brow[p[0]].push_back(TreeTerm{(uint16_t)p[3], (uint16_t)p[1], 0, (double)p[2]});
     brow[p[1]].push_back(TreeTerm{(uint16_t)p[3], (uint16_t)p[0], 0, (double)p[2]});
   }
-  {
-    std::vector<TreeItem> items;
-    s.bwave.push_back(0);
-    for (int w = D - 1; w >= 0; --w) {
-      const int lo = (int)items.size();
-      for (int n = 0; n < n_nodes; ++n) {
-        if (depth[n] != w || brow[n].empty()) continue;
-        emit(items, s.bterms, n, brow[n]);
-      }
-      by_len(items, lo, (int)items.size(), s.bitems);
-      s.bwave.push_back((int32_t)s.bitems.size());
+  s.bwave.push_back(0);
+  for (int w = D - 1; w >= 0; --w) {
+    std::vector<Row> rows;
+    for (int n = 0; n < n_nodes; ++n) {
+      if (depth[n] != w || brow[n].empty()) continue;
+      rows.push_back(Row{n, brow[n]});
     }
+    deal(rows, s.bitems, s.bterms);
+    s.bwave.push_back((int32_t)s.bitems.size());
+  }
+  // ---- adjoint seeds: dE_i/dB_alpha = xi_alpha, summed per node in alpha order
+  {
+    std::vector<double> sv(n_nodes, 0.0);
+    std::vector<char> has(n_nodes, 0);
+    for (int a = 0; a < n_basis; ++a) { sv[basis_node[a]] += xi[a]; has[basis_node[a]] = 1; }
+    for (int n = 0; n < n_nodes; ++n) if (has[n]) { s.seed_node.push_back(n); s.seed_val.push_back(sv[n]); }
   }
   return MTP_OK;
 }

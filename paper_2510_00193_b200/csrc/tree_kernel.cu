@@ -32,19 +32,17 @@ __global__ void __launch_bounds__(128) k_tree(const TreeArgs a) {
     const int lo = a.fwave[w], hi = a.fwave[w + 1];
     for (int it = lo + rl; it < hi; it += R) {
       const int4 I = __ldg(reinterpret_cast<const int4 *>(a.fitems) + it);
+      if (I.z <= 0) continue;
       const int4 *tp = reinterpret_cast<const int4 *>(a.fterms) + I.y;
       double acc = 0.0;
-#pragma unroll
-      for (int k = 0; k < kSeg; ++k) {
-        if (k < I.z) {
-          const int4 T = __ldg(tp + k);
-          const double m = __hiloint2double(T.w, T.z);
-          const int na = T.x & 0xffff, nb = (unsigned)T.x >> 16;
-          acc = fma(m * val[na * AL + al], val[nb * AL + al], acc);
-        }
+#pragma unroll 4
+      for (int k = 0; k < I.z; ++k) {
+        const int4 T = __ldg(tp + k);
+        const double m = __hiloint2double(T.w, T.z);
+        const int na = T.x & 0xffff, nb = (unsigned)T.x >> 16;
+        acc = fma(m * val[na * AL + al], val[nb * AL + al], acc);
       }
-      if (I.w) atomicAdd(&val[I.x * AL + al], acc);
-      else val[I.x * AL + al] = acc;
+      val[I.x * AL + al] = acc;
     }
     __syncthreads();
   }
@@ -56,7 +54,6 @@ __global__ void __launch_bounds__(128) k_tree(const TreeArgs a) {
       const double v = val[n * AL + al], x = a.xi[b];
       e = fma(x, v, e);
       if (a.B && act) a.B[(long long)atom * a.n_basis + b] = v;
-      if (a.want_adj) atomicAdd(&adj[n * AL + al], x);
     }
     // reduce e over the R row-lanes of this atom through shared memory, fixed order
     __shared__ double esm[128];
@@ -70,25 +67,24 @@ __global__ void __launch_bounds__(128) k_tree(const TreeArgs a) {
     }
   }
   if (!a.want_adj) return;
+  for (int q = rl; q < a.n_seed; q += R) adj[a.seed_node[q] * AL + al] = a.seed_val[q];
   __syncthreads();
   // ---- backward
   for (int w = 0; w < a.nbw; ++w) {
     const int lo = a.bwave[w], hi = a.bwave[w + 1];
     for (int it = lo + rl; it < hi; it += R) {
       const int4 I = __ldg(reinterpret_cast<const int4 *>(a.bitems) + it);
+      if (I.z <= 0) continue;
       const int4 *tp = reinterpret_cast<const int4 *>(a.bterms) + I.y;
       double acc = 0.0;
-#pragma unroll
-      for (int k = 0; k < kSeg; ++k) {
-        if (k < I.z) {
-          const int4 T = __ldg(tp + k);
-          const double m = __hiloint2double(T.w, T.z);
-          const int nd = T.x & 0xffff, no = (unsigned)T.x >> 16;
-          acc = fma(m * adj[nd * AL + al], val[no * AL + al], acc);
-        }
+#pragma unroll 4
+      for (int k = 0; k < I.z; ++k) {
+        const int4 T = __ldg(tp + k);
+        const double m = __hiloint2double(T.w, T.z);
+        const int nd = T.x & 0xffff, no = (unsigned)T.x >> 16;
+        acc = fma(m * adj[nd * AL + al], val[no * AL + al], acc);
       }
-      if (I.w) atomicAdd(&adj[I.x * AL + al], acc);
-      else adj[I.x * AL + al] += acc;
+      adj[I.x * AL + al] += acc;
     }
     __syncthreads();
   }

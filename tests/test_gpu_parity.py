@@ -21,9 +21,9 @@ def torch():
     return t
 
 
-def run_gpu(lib, torch, w, pot=None, **opts):
+def run_gpu(lib, torch, w, pot=None, opts=None):
     pot = gpu_pot(lib, w) if pot is None else pot
-    for k, v in opts.items():
+    for k, v in (opts or {}).items():
         pot.set_option(k, v)
     d = to_dev(w, torch)
     out = pot.compute(d["pos"], d["types"], w.box, d["off"], d["idx"], d["shift"], d["rev"])
@@ -52,17 +52,17 @@ def test_energy_force_virial_parity(lib, torch, ci, cells):
     ref = omtp.evaluate(opot, w.pos, w.types, w.box, w.off, w.idx, w.shift)
     for variant in (lib.VARIANT_THREAD, lib.VARIANT_BLOCK):
         for mode in (lib.FORCE_GATHER, lib.FORCE_ATOMIC):
-            got, pot, _ = run_gpu(lib, torch, w, **{lib.OPT_VARIANT: variant, lib.OPT_FORCE_MODE: mode})
+            got, pot, _ = run_gpu(lib, torch, w, opts={lib.OPT_VARIANT: variant, lib.OPT_FORCE_MODE: mode})
             check(w, ref, got, opot)
             pot.close()
 
 
 def test_chunked_equals_unchunked_and_gather_is_deterministic(lib, torch):
     w = make_workload(1, n_basis_of(16), cells=5)
-    a, pot, d = run_gpu(lib, torch, w, **{lib.OPT_FORCE_MODE: lib.FORCE_GATHER})
+    a, pot, d = run_gpu(lib, torch, w, opts={lib.OPT_FORCE_MODE: lib.FORCE_GATHER})
     b, _, _ = run_gpu(lib, torch, w, pot=pot)
     assert np.array_equal(a["F"], b["F"]) and np.array_equal(a["Ei"], b["Ei"]) and np.array_equal(a["virial"], b["virial"])
-    c, _, _ = run_gpu(lib, torch, w, pot=pot, **{lib.OPT_CHUNK_ATOMS: 77})   # ragged last chunk
+    c, _, _ = run_gpu(lib, torch, w, pot=pot, opts={lib.OPT_CHUNK_ATOMS: 77})   # ragged last chunk
     assert np.array_equal(a["Ei"], c["Ei"])
     assert np.array_equal(a["F"], c["F"])          # gather: same per-pair values, same order
     assert np.allclose(a["virial"], c["virial"], rtol=1e-12)
