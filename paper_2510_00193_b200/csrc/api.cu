@@ -39,8 +39,7 @@ struct mtp_handle {
   int crow = 0, AL = 0;
   double *d_coef = nullptr, *d_xi = nullptr, *d_xi0 = nullptr;
   int *d_kmapF = nullptr, *d_kmapB = nullptr, *d_basis_node = nullptr;
-  TreeTerm *d_fterms = nullptr, *d_bterms = nullptr;
-  TreeItem *d_fitems = nullptr, *d_bitems = nullptr;
+  TreeTerm *d_fprog = nullptr, *d_bprog = nullptr;
   int *d_fwave = nullptr, *d_bwave = nullptr, *d_seed_node = nullptr;
   double *d_seed_val = nullptr;
   TreeSched sched;
@@ -197,7 +196,7 @@ extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
   const char *terr = "";
   h->AL = tree_pick_al(p->n_nodes);
   if (h->AL == 0) { delete h; return fail(nullptr, MTP_EUNSUP, "contraction tree does not fit in shared memory (n_nodes*16 B > 220 KB)"); }
-  int rc = tree_compile(p->n_basic, p->n_nodes, p->n_prod, p->prod, p->n_basis, p->basis_node, p->xi, 128 / h->AL,
+  int rc = tree_compile(p->n_basic, p->n_nodes, p->n_prod, p->prod, p->n_basis, p->basis_node, p->xi, tree_row_lanes(h->AL),
                         h->sched, &terr);
   if (rc != MTP_OK) { g_create_error = terr; delete h; return rc; }
   // radial coefficients: rows (z_i, z_j) padded to the level's n_mu, odd row stride (bank spread)
@@ -217,10 +216,8 @@ extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
   up(upload(h, &h->d_kmapF, kf.data(), kf.size()));
   up(upload(h, &h->d_kmapB, kb.data(), kb.size()));
   up(upload(h, &h->d_basis_node, p->basis_node, (size_t)p->n_basis));
-  up(upload(h, &h->d_fterms, h->sched.fterms.data(), h->sched.fterms.size()));
-  up(upload(h, &h->d_bterms, h->sched.bterms.data(), h->sched.bterms.size()));
-  up(upload(h, &h->d_fitems, h->sched.fitems.data(), h->sched.fitems.size()));
-  up(upload(h, &h->d_bitems, h->sched.bitems.data(), h->sched.bitems.size()));
+  up(upload(h, &h->d_fprog, h->sched.fprog.data(), h->sched.fprog.size()));
+  up(upload(h, &h->d_bprog, h->sched.bprog.data(), h->sched.bprog.size()));
   up(upload(h, &h->d_fwave, h->sched.fwave.data(), h->sched.fwave.size()));
   up(upload(h, &h->d_bwave, h->sched.bwave.data(), h->sched.bwave.size()));
   up(upload(h, &h->d_seed_node, h->sched.seed_node.data(), h->sched.seed_node.size()));
@@ -264,10 +261,10 @@ int make_plan(const mtp_handle *h, int64_t N, int64_t nnz, int want_grade, int h
   if (N < 0 || nnz < 0 || N > 2147483000LL) return MTP_EINVAL;
   pl.N = N; pl.nnz = nnz;
   int64_t C = h->chunk_atoms;
-  if (C <= 0) {   // automatic: M and G of a chunk (16 B x n_basic per atom) stay L2-resident
-    C = (64LL << 20) / (16LL * h->n_basic);
+  if (C <= 0) {   // automatic: many waves per launch (no tail), M + G scratch (16 B x n_basic per atom) <= 1 GB
+    C = std::min<int64_t>(262144, (1LL << 30) / (16LL * h->n_basic));
     C = std::max<int64_t>(1024, C / 1024 * 1024);
-    if (N > C) {  // avoid a small last chunk
+    if (N > C) {  // equal chunks: no small last chunk
       const int64_t nc = (N + C - 1) / C;
       C = ((N + nc - 1) / nc + 31) / 32 * 32;
     }
@@ -326,8 +323,8 @@ void fill_pair_args(const mtp_handle *h, PairArgs &pa, const double *pos4, const
 }
 
 void fill_tree_args(const mtp_handle *h, TreeArgs &ta, const double *pos4) {
-  ta.fterms = h->d_fterms; ta.fitems = h->d_fitems; ta.fwave = h->d_fwave; ta.nfw = (int)h->sched.fwave.size() - 1;
-  ta.bterms = h->d_bterms; ta.bitems = h->d_bitems; ta.bwave = h->d_bwave; ta.nbw = (int)h->sched.bwave.size() - 1;
+  ta.fprog = h->d_fprog; ta.fwave = h->d_fwave; ta.nfw = (int)h->sched.fwave.size() - 1;
+  ta.bprog = h->d_bprog; ta.bwave = h->d_bwave; ta.nbw = (int)h->sched.bwave.size() - 1;
   ta.basis_node = h->d_basis_node; ta.xi = h->d_xi; ta.xi0 = h->d_xi0; ta.pos4 = pos4;
   ta.seed_node = h->d_seed_node; ta.seed_val = h->d_seed_val; ta.n_seed = (int)h->sched.seed_node.size();
   ta.n_nodes = h->n_nodes; ta.n_basic = h->n_basic; ta.n_basis = h->n_basis;

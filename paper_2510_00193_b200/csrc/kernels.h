@@ -13,8 +13,8 @@ long long launch_count();
 
 // ---- K2
 struct TreeArgs {
-  const TreeTerm *fterms; const TreeItem *fitems; const int *fwave; int nfw;
-  const TreeTerm *bterms; const TreeItem *bitems; const int *bwave; int nbw;
+  const TreeTerm *fprog; const int *fwave; int nfw;
+  const TreeTerm *bprog; const int *bwave; int nbw;
   const int *basis_node; const double *xi; const double *xi0;
   const int *seed_node; const double *seed_val; int n_seed;
   const double *pos4;
@@ -25,7 +25,8 @@ struct TreeArgs {
   int c0, c1;
   int want_adj;
 };
-int tree_pick_al(int n_nodes);
+int tree_pick_al(int n_nodes);          // atoms per CTA (A)
+int tree_row_lanes(int A);              // row-lanes R the schedule must be dealt for
 size_t tree_smem_bytes(int n_nodes, int AL);
 cudaError_t launch_tree(const TreeArgs &a, int AL, cudaStream_t st);
 

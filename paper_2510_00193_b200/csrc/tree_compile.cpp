@@ -44,29 +44,30 @@ int tree_compile(int n_basic, int n_nodes, int n_prod, const int32_t *prod, int 
   // ---- forward rows grouped by dst, waves by depth 1..D
   std::vector<std::vector<int>> row(n_nodes);   // op ids per dst
   for (int t = 0; t < n_prod; ++t) row[prod[4 * t + 3]].push_back(t);
-  // deal the rows of one wave to R lanes: longest first, always to the least-loaded lane
+  // deal the rows of one wave to R lanes: longest first, always to the least-loaded lane;
+  // emit the lane-major program of the wave and return its number of steps
   struct Row { int dst; std::vector<TreeTerm> terms; };
-  auto deal = [R](std::vector<Row> &rows, std::vector<TreeItem> &items, std::vector<TreeTerm> &terms) {
+  auto deal = [R](std::vector<Row> &rows, std::vector<TreeTerm> &prog) {
     std::stable_sort(rows.begin(), rows.end(), [](const Row &x, const Row &y) { return x.terms.size() > y.terms.size(); });
-    std::vector<long long> load(R, 0);
-    std::vector<std::vector<int>> mine(R);
-    for (int r = 0; r < (int)rows.size(); ++r) {
+    std::vector<std::vector<TreeTerm>> lane(R);
+    for (auto &row : rows) {
       int best = 0;
-      for (int l = 1; l < R; ++l) if (load[l] < load[best]) best = l;
-      load[best] += (long long)rows[r].terms.size() + 2;   // +2: per-row overhead (item load, store)
-      mine[best].push_back(r);
-    }
-    size_t K = 0;
-    for (int l = 0; l < R; ++l) K = std::max(K, mine[l].size());
-    const size_t base = items.size();
-    items.resize(base + K * R, TreeItem{-1, 0, 0, 0});
-    for (int l = 0; l < R; ++l)
-      for (size_t k = 0; k < mine[l].size(); ++k) {
-        const Row &row = rows[mine[l][k]];
-        TreeItem it{row.dst, (int32_t)terms.size(), (int32_t)row.terms.size(), 0};
-        terms.insert(terms.end(), row.terms.begin(), row.terms.end());
-        items[base + k * R + l] = it;
+      for (int l = 1; l < R; ++l) if (lane[l].size() < lane[best].size()) best = l;
+      for (size_t k = 0; k < row.terms.size(); ++k) {
+        TreeTerm t = row.terms[k];
+        t.dst = (uint16_t)row.dst;
+        t.last = (k + 1 == row.terms.size());
+        lane[best].push_back(t);
       }
+    }
+    size_t S = 0;
+    for (int l = 0; l < R; ++l) S = std::max(S, lane[l].size());
+    S = (S + kTreePrefetch - 1) / kTreePrefetch * kTreePrefetch;
+    const size_t base = prog.size();
+    prog.resize(base + S * R, TreeTerm{0, 0, 0, 0, 0.0});
+    for (int l = 0; l < R; ++l)
+      for (size_t k = 0; k < lane[l].size(); ++k) prog[base + k * R + l] = lane[l][k];
+    return (int)S;
   };
   s.R = R;
   s.fwave.push_back(0);
@@ -77,19 +78,18 @@ int tree_compile(int n_basic, int n_nodes, int n_prod, const int32_t *prod, int 
       Row r; r.dst = n;
       for (int t : row[n]) {
         const int32_t *p = prod + 4 * t;
-        r.terms.push_back(TreeTerm{(uint16_t)p[0], (uint16_t)p[1], 0, (double)p[2]});
+        r.terms.push_back(TreeTerm{(uint16_t)p[0], (uint16_t)p[1], 0, 0, (double)p[2]});
       }
       rows.push_back(std::move(r));
     }
-    deal(rows, s.fitems, s.fterms);
-    s.fwave.push_back((int32_t)s.fitems.size());
+    s.fwave.push_back(s.fwave.back() + deal(rows, s.fprog));
   }
   // ---- backward rows grouped by source node, waves by depth D-1 .. 0
   std::vector<std::vector<TreeTerm>> brow(n_nodes);
   for (int t = 0; t < n_prod; ++t) {
     const int32_t *p = prod + 4 * t;
-    brow[p[0]].push_back(TreeTerm{(uint16_t)p[3], (uint16_t)p[1], 0, (double)p[2]});
-    brow[p[1]].push_back(TreeTerm{(uint16_t)p[3], (uint16_t)p[0], 0, (double)p[2]});
+    brow[p[0]].push_back(TreeTerm{(uint16_t)p[3], (uint16_t)p[1], 0, 0, (double)p[2]});
+    brow[p[1]].push_back(TreeTerm{(uint16_t)p[3], (uint16_t)p[0], 0, 0, (double)p[2]});
   }
   s.bwave.push_back(0);
   for (int w = D - 1; w >= 0; --w) {
@@ -98,9 +98,10 @@ int tree_compile(int n_basic, int n_nodes, int n_prod, const int32_t *prod, int 
       if (depth[n] != w || brow[n].empty()) continue;
       rows.push_back(Row{n, brow[n]});
     }
-    deal(rows, s.bitems, s.bterms);
-    s.bwave.push_back((int32_t)s.bitems.size());
+    s.bwave.push_back(s.bwave.back() + deal(rows, s.bprog));
   }
+  // the kernel prefetches kTreePrefetch steps ahead: pad so that those reads stay in bounds
+  for (int q = 0; q < kTreePrefetch * R; ++q) { s.fprog.push_back(TreeTerm{0, 0, 0, 0, 0.0}); s.bprog.push_back(TreeTerm{0, 0, 0, 0, 0.0}); }
   // ---- adjoint seeds: dE_i/dB_alpha = xi_alpha, summed per node in alpha order
   {
     std::vector<double> sv(n_nodes, 0.0);
