@@ -36,13 +36,22 @@ struct mtp_handle {
   int S = 0, nb = 0, nmu = 0, n_basic = 0, n_nodes = 0, n_basis = 0, lev_max = 0;
   double r_min = 0, r_cut = 0;
   const PairLevel *pl = nullptr;
-  int crow = 0, AL = 0;
+  int crow = 0;
   double *d_coef = nullptr, *d_xi = nullptr, *d_xi0 = nullptr;
   int *d_kmapF = nullptr, *d_kmapB = nullptr, *d_basis_node = nullptr;
-  TreeTerm *d_fprog = nullptr, *d_bprog = nullptr;
-  int *d_fwave = nullptr, *d_bwave = nullptr, *d_seed_node = nullptr;
-  double *d_seed_val = nullptr;
-  TreeSched sched;
+  // K2 schedules, one per atom-lane count AL (compiled on first use; the large-N one at create)
+  struct TreeDev {
+    TreeSched sched;
+    TreeTerm *d_fprog = nullptr, *d_bprog = nullptr;
+    int *d_fwave = nullptr, *d_bwave = nullptr, *d_gseed_k = nullptr, *d_gzero_k = nullptr;
+    int *d_eseed_slot = nullptr, *d_basis_slot = nullptr;
+    double *d_adj_init = nullptr, *d_gseed_val = nullptr, *d_leaf_seed = nullptr, *d_eseed_val = nullptr;
+  };
+  std::map<int, TreeDev> trees;                // key: AL * 8 + AR * 2 + elide
+  int slots[2][2] = {{0, 0}, {0, 0}};          // [elide][n_val, n_adj]
+  std::vector<int32_t> t_prod, t_basis_node;   // host copy of the table for those compilations
+  std::vector<double> t_xi;
+  long long n_prod = 0;
   int64_t chunk_atoms = 0;
   int force_mode = MTP_FORCE_AUTO, variant = MTP_VARIANT_AUTO;
   std::string err;
@@ -140,6 +149,39 @@ static void build_kmaps(const PairLevel &pl, int n_basic, const int32_t *basic, 
   }
 }
 
+// K2 schedule for a CTA shape (AL, AR) and leaf elision on/off: compiled from the host copy of the
+// table and uploaded on first use
+static int get_tree(mtp_handle *h, int AL, int AR, bool elide, const mtp_handle::TreeDev **out) {
+  if (AL <= 0) return fail(h, MTP_EUNSUP, "contraction tree does not fit in shared memory");
+  const int key = AL * 8 + AR * 2 + (elide ? 1 : 0);
+  auto it = h->trees.find(key);
+  if (it != h->trees.end()) { *out = &it->second; return MTP_OK; }
+  mtp_handle::TreeDev td;
+  const char *terr = "";
+  int rc = tree_compile(h->n_basic, h->n_nodes, (int)h->n_prod, h->t_prod.data(), h->n_basis, h->t_basis_node.data(),
+                        h->t_xi.data(), AL * AR, tree_row_lanes(AL), elide, td.sched, &terr);
+  if (rc != MTP_OK) return fail(h, rc, terr);
+  cudaError_t e = cudaSuccess;
+  auto up = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+  const TreeSched &sc = td.sched;
+  up(upload(h, &td.d_fprog, sc.fprog.data(), sc.fprog.size()));
+  up(upload(h, &td.d_bprog, sc.bprog.data(), sc.bprog.size()));
+  up(upload(h, &td.d_fwave, sc.fwave.data(), sc.fwave.size()));
+  up(upload(h, &td.d_bwave, sc.bwave.data(), sc.bwave.size()));
+  up(upload(h, &td.d_adj_init, sc.adj_init.data(), sc.adj_init.size()));
+  up(upload(h, &td.d_leaf_seed, sc.leaf_seed.data(), sc.leaf_seed.size()));
+  up(upload(h, &td.d_eseed_slot, sc.eseed_slot.data(), sc.eseed_slot.size()));
+  up(upload(h, &td.d_eseed_val, sc.eseed_val.data(), sc.eseed_val.size()));
+  up(upload(h, &td.d_basis_slot, sc.basis_slot.data(), sc.basis_slot.size()));
+  up(upload(h, &td.d_gseed_k, sc.gseed_k.data(), sc.gseed_k.size()));
+  up(upload(h, &td.d_gseed_val, sc.gseed_val.data(), sc.gseed_val.size()));
+  up(upload(h, &td.d_gzero_k, sc.gzero_k.data(), sc.gzero_k.size()));
+  if (e != cudaSuccess) return cuda_fail(h, e, "tree schedule upload");
+  auto ins = h->trees.emplace(key, std::move(td));
+  *out = &ins.first->second;
+  return MTP_OK;
+}
+
 extern "C" const char *mtp_last_error(const mtp_handle *h) { return h ? h->err.c_str() : g_create_error.c_str(); }
 extern "C" int64_t mtp_launch_count(void) { return launch_count(); }
 
@@ -193,12 +235,19 @@ extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
   h->S = p->n_species; h->nb = p->n_radial_basis; h->nmu = p->n_radial_funcs; h->n_basic = p->n_basic;
   h->n_nodes = p->n_nodes; h->n_basis = p->n_basis; h->lev_max = p->lev_max; h->r_min = p->r_min; h->r_cut = p->r_cut;
   h->pl = pair_level(li);
-  const char *terr = "";
-  h->AL = tree_pick_al(p->n_nodes);
-  if (h->AL == 0) { delete h; return fail(nullptr, MTP_EUNSUP, "contraction tree does not fit in shared memory (n_nodes*16 B > 220 KB)"); }
-  int rc = tree_compile(p->n_basic, p->n_nodes, p->n_prod, p->prod, p->n_basis, p->basis_node, p->xi, tree_row_lanes(h->AL),
-                        h->sched, &terr);
-  if (rc != MTP_OK) { g_create_error = terr; delete h; return rc; }
+  h->n_prod = p->n_prod;
+  h->t_prod.assign(p->prod, p->prod + 4 * (size_t)p->n_prod);
+  h->t_basis_node.assign(p->basis_node, p->basis_node + p->n_basis);
+  h->t_xi.assign(p->xi, p->xi + p->n_basis);
+  for (int el = 0; el < 2; ++el) {
+    tree_count_slots(p->n_basic, p->n_nodes, p->n_prod, p->prod, el != 0, &h->slots[el][0], &h->slots[el][1]);
+    int AL = 0, AR = 1;
+    tree_pick_shape(h->slots[el][0], h->slots[el][1], 0, &AL, &AR);
+    if (AL == 0) {
+      delete h;
+      return fail(nullptr, MTP_EUNSUP, "contraction tree does not fit in shared memory (one atom's node values and adjoints > 225 KB)");
+    }
+  }
   // radial coefficients: rows (z_i, z_j) padded to the level's n_mu, odd row stride (bank spread)
   const int nmu_lev = rt_nmu(h->pl->lev);
   h->crow = nmu_lev * h->nb + 1;
@@ -216,13 +265,14 @@ extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
   up(upload(h, &h->d_kmapF, kf.data(), kf.size()));
   up(upload(h, &h->d_kmapB, kb.data(), kb.size()));
   up(upload(h, &h->d_basis_node, p->basis_node, (size_t)p->n_basis));
-  up(upload(h, &h->d_fprog, h->sched.fprog.data(), h->sched.fprog.size()));
-  up(upload(h, &h->d_bprog, h->sched.bprog.data(), h->sched.bprog.size()));
-  up(upload(h, &h->d_fwave, h->sched.fwave.data(), h->sched.fwave.size()));
-  up(upload(h, &h->d_bwave, h->sched.bwave.data(), h->sched.bwave.size()));
-  up(upload(h, &h->d_seed_node, h->sched.seed_node.data(), h->sched.seed_node.size()));
-  up(upload(h, &h->d_seed_val, h->sched.seed_val.data(), h->sched.seed_val.size()));
   if (e != cudaSuccess) { int r = cuda_fail(nullptr, e, "mtp_create upload"); mtp_destroy(h); return r; }
+  {   // validate the table and build the large-system schedule now, so that errors surface at create
+    const mtp_handle::TreeDev *td = nullptr;
+    int AL = 0, AR = 1;
+    tree_pick_shape(h->slots[1][0], h->slots[1][1], 0, &AL, &AR);
+    int rc = get_tree(h, AL, AR, true, &td);
+    if (rc != MTP_OK) { g_create_error = h->err; mtp_destroy(h); return rc; }
+  }
   *out = h;
   return MTP_OK;
 }
@@ -252,8 +302,8 @@ extern "C" int mtp_get_option(const mtp_handle *h, int key, int64_t *v) {
 namespace {
 struct Plan {
   int64_t N = 0, nnz = 0, C = 0, ldm = 0;
-  int n_chunks = 0, P = 1, atomic = 0, grid_chunk = 0;
-  size_t o_pos4 = 0, o_Ei = 0, o_M = 0, o_G = 0, o_wpart = 0, o_d4 = 0, o_B = 0, o_part = 0, total = 0;
+  int n_chunks = 0, P = 1, atomic = 0, grid_chunk = 0, AL = 0, AR = 1, elide = 1;
+  size_t o_pos4 = 0, o_Ei = 0, o_M = 0, o_G = 0, o_wpart = 0, o_d4 = 0, o_B = 0, o_part = 0, o_red = 0, total = 0;
 };
 size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
@@ -277,6 +327,8 @@ int make_plan(const mtp_handle *h, int64_t N, int64_t nnz, int want_grade, int h
   if (h->variant == MTP_VARIANT_THREAD) pl.P = 1;
   else if (h->variant == MTP_VARIANT_BLOCK) pl.P = h->pl->p_small;
   else pl.P = (N * NS >= 2LL * 148 * 256) ? 1 : h->pl->p_small;   // fill the SMs' register files
+  pl.elide = want_grade ? 0 : 1;           // grades need every B_alpha stored
+  tree_pick_shape(h->slots[pl.elide][0], h->slots[pl.elide][1], N, &pl.AL, &pl.AR);
   pl.atomic = h->force_mode == MTP_FORCE_ATOMIC || (h->force_mode == MTP_FORCE_AUTO && !has_rev);
   pl.grid_chunk = h->pl->pairgrad_grid((int)C, pl.P);
   size_t o = 0;
@@ -284,6 +336,7 @@ int make_plan(const mtp_handle *h, int64_t N, int64_t nnz, int want_grade, int h
   pl.o_Ei = o; o = align_up(o + (size_t)N * 8);
   pl.o_M = o; o = align_up(o + (size_t)h->n_basic * pl.ldm * 8);
   pl.o_G = o; o = align_up(o + (size_t)h->n_basic * pl.ldm * 8);
+  pl.o_red = o; o = align_up(o + 256 * 8 * 8);
   pl.o_wpart = o; o = align_up(o + (size_t)std::max(1, pl.n_chunks) * pl.grid_chunk * 64);
   pl.o_d4 = o; if (!want_grade && !pl.atomic) o = align_up(o + (size_t)nnz * 32);
   pl.o_B = o; if (want_grade) o = align_up(o + (size_t)C * h->n_basis * 8);
@@ -322,13 +375,23 @@ void fill_pair_args(const mtp_handle *h, PairArgs &pa, const double *pos4, const
   pa.M = nullptr; pa.G = nullptr; pa.d4 = nullptr; pa.F = nullptr; pa.wpart = nullptr; pa.kmap = nullptr;
 }
 
-void fill_tree_args(const mtp_handle *h, TreeArgs &ta, const double *pos4) {
-  ta.fprog = h->d_fprog; ta.fwave = h->d_fwave; ta.nfw = (int)h->sched.fwave.size() - 1;
-  ta.bprog = h->d_bprog; ta.bwave = h->d_bwave; ta.nbw = (int)h->sched.bwave.size() - 1;
-  ta.basis_node = h->d_basis_node; ta.xi = h->d_xi; ta.xi0 = h->d_xi0; ta.pos4 = pos4;
-  ta.seed_node = h->d_seed_node; ta.seed_val = h->d_seed_val; ta.n_seed = (int)h->sched.seed_node.size();
-  ta.n_nodes = h->n_nodes; ta.n_basic = h->n_basic; ta.n_basis = h->n_basis;
+int fill_tree_args(mtp_handle *h, TreeArgs &ta, const double *pos4, const Plan &pl) {
+  const mtp_handle::TreeDev *td = nullptr;
+  int rc = get_tree(h, pl.AL, pl.AR, pl.elide != 0, &td);
+  if (rc != MTP_OK) return rc;
+  const TreeSched &sc = td->sched;
+  ta.fprog = td->d_fprog; ta.fwave = td->d_fwave; ta.nfw = (int)sc.fwave.size() - 1;
+  ta.bprog = td->d_bprog; ta.bwave = td->d_bwave; ta.nbw = (int)sc.bwave.size() - 1;
+  ta.n_fprog = (int)sc.fprog.size(); ta.n_bprog = (int)sc.bprog.size(); ta.prog_smem_off = 0;
+  ta.xi0 = h->d_xi0; ta.pos4 = pos4;
+  ta.adj_init = td->d_adj_init; ta.leaf_seed = td->d_leaf_seed;
+  ta.eseed_slot = td->d_eseed_slot; ta.eseed_val = td->d_eseed_val; ta.n_eseed = (int)sc.eseed_slot.size();
+  ta.basis_slot = td->d_basis_slot;
+  ta.gseed_k = td->d_gseed_k; ta.gseed_val = td->d_gseed_val; ta.n_gseed = (int)sc.gseed_k.size();
+  ta.gzero_k = td->d_gzero_k; ta.n_gzero = (int)sc.gzero_k.size();
+  ta.n_val = sc.n_val; ta.n_adj = sc.n_adj; ta.n_basic = h->n_basic; ta.n_basis = h->n_basis;
   ta.B = nullptr; ta.want_adj = 1;
+  return MTP_OK;
 }
 }  // namespace
 
@@ -373,21 +436,23 @@ extern "C" int mtp_compute(mtp_handle *h, int64_t N, const double *d_pos, const 
   fill_pair_args(h, pa, pos4, d_off, d_idx, d_shift);
   pa.ldm = pl.ldm;
   TreeArgs ta;
-  fill_tree_args(h, ta, pos4);
+  rc = fill_tree_args(h, ta, pos4, pl);
+  if (rc != MTP_OK) return rc;
   ta.M = M; ta.G = G; ta.ldm = pl.ldm; ta.Ei = Ei;
   for (int c = 0; c < pl.n_chunks; ++c) {
     pa.c0 = (int)(c * pl.C); pa.c1 = (int)std::min<int64_t>(N, (c + 1) * pl.C);
     pa.M = M; pa.G = G; pa.kmap = h->d_kmapF;
     TIMED(h, CLS_MOMENTS, st, h->pl->moments(pa, pl.P, st));
     ta.c0 = pa.c0; ta.c1 = pa.c1;
-    TIMED(h, CLS_TREE, st, launch_tree(ta, h->AL, st));
+    TIMED(h, CLS_TREE, st, launch_tree(ta, pl.AL, pl.AR, st));
     pa.kmap = h->d_kmapB; pa.wpart = wpart + (size_t)c * pl.grid_chunk * 8;
     pa.d4 = pl.atomic ? nullptr : d4; pa.F = pl.atomic ? d_F : nullptr;
     TIMED(h, CLS_PAIRGRAD, st, h->pl->pairgrad(pa, pl.P, pl.atomic, st, nullptr));
   }
   if (!pl.atomic) TIMED(h, CLS_OTHER, st, launch_gather((const long long *)d_off, d_rev, d4, (int)N, d_F, st));
-  CU(h, launch_reduce(Ei, N, 1, 1, d_E, st));
-  if (d_virial) CU(h, launch_reduce(wpart, (long long)pl.n_chunks * pl.grid_chunk, 8, 6, d_virial, st));
+  double *red = (double *)(ws + pl.o_red);
+  CU(h, launch_reduce(Ei, N, 1, 1, d_E, red, st));
+  if (d_virial) CU(h, launch_reduce(wpart, (long long)pl.n_chunks * pl.grid_chunk, 8, 6, d_virial, red, st));
   return MTP_OK;
 }
 
@@ -420,7 +485,8 @@ extern "C" int mtp_grade(mtp_handle *h, int64_t N, const double *d_pos, const in
     fill_pair_args(h, pa, pos4, d_off, d_idx, d_shift);
     pa.ldm = pl.ldm;
     TreeArgs ta;
-    fill_tree_args(h, ta, pos4);
+    rc = fill_tree_args(h, ta, pos4, pl);
+    if (rc != MTP_OK) return rc;
     ta.M = M; ta.G = G; ta.ldm = pl.ldm; ta.Ei = Ei; ta.want_adj = 0;
     for (int c = 0; c < pl.n_chunks; ++c) {
       pa.c0 = (int)(c * pl.C); pa.c1 = (int)std::min<int64_t>(N, (c + 1) * pl.C);
@@ -430,7 +496,7 @@ extern "C" int mtp_grade(mtp_handle *h, int64_t N, const double *d_pos, const in
       // B rows are indexed by absolute atom: point the kernel at a base shifted by -c0 rows
       double *Brows = d_B ? d_B : Bc - (size_t)pa.c0 * h->n_basis;
       ta.B = Brows;
-      TIMED(h, CLS_TREE, st, launch_tree(ta, h->AL, st));
+      TIMED(h, CLS_TREE, st, launch_tree(ta, pl.AL, pl.AR, st));
       const double *Bchunk = Brows + (size_t)pa.c0 * h->n_basis;
       const int64_t nc = pa.c1 - pa.c0;
       if (mode != 1) TIMED(h, CLS_GRADE, st, launch_grade(Bchunk, d_Ainv, nc, h->n_basis, d_gamma_atom + pa.c0, st));
@@ -498,6 +564,8 @@ extern "C" int mtp_debug_moments(mtp_handle *h, int64_t N, const double *d_pos, 
   int rc = make_plan(h, N, 0, 0, 0, pl);
   h->chunk_atoms = saved;
   if (rc != MTP_OK) return rc;
+  pl.elide = 0;                             // B is exported: every basis value must be stored
+  tree_pick_shape(h->slots[0][0], h->slots[0][1], N, &pl.AL, &pl.AR);
   const size_t base = align_up((size_t)(uintptr_t)d_ws) - (size_t)(uintptr_t)d_ws;
   if (!d_ws || ws_bytes < pl.total + base) return fail(h, MTP_ESIZE, "workspace too small");
   PairArgs pa;
@@ -510,9 +578,10 @@ extern "C" int mtp_debug_moments(mtp_handle *h, int64_t N, const double *d_pos, 
   pa.ldm = pl.ldm; pa.c0 = 0; pa.c1 = (int)N; pa.M = M; pa.kmap = h->d_kmapF;
   CU(h, h->pl->moments(pa, pl.P, st));
   TreeArgs ta;
-  fill_tree_args(h, ta, pos4);
+  rc = fill_tree_args(h, ta, pos4, pl);
+  if (rc != MTP_OK) return rc;
   ta.M = M; ta.G = G; ta.ldm = pl.ldm; ta.Ei = Ei; ta.c0 = 0; ta.c1 = (int)N; ta.B = d_B;
-  CU(h, launch_tree(ta, h->AL, st));
+  CU(h, launch_tree(ta, pl.AL, pl.AR, st));
   // outputs are [n_basic][N] (component-major), the kernels' own layout
   if (d_M) CU(h, cudaMemcpy2DAsync(d_M, (size_t)N * 8, M, (size_t)pl.ldm * 8, (size_t)N * 8, h->n_basic, cudaMemcpyDeviceToDevice, st));
   if (d_G) CU(h, cudaMemcpy2DAsync(d_G, (size_t)N * 8, G, (size_t)pl.ldm * 8, (size_t)N * 8, h->n_basic, cudaMemcpyDeviceToDevice, st));
@@ -538,7 +607,7 @@ extern "C" int mtp_cost_model(const mtp_handle *h, double *flop_per_pair, double
   numax = rt_numax(h->pl->lev, 0);
   const double monos = (numax + 1.0) * (numax + 2.0) * (numax + 3.0) / 6.0;
   if (flop_per_pair) *flop_per_pair = 12.0 + 6.0 * h->nb + 4.0 * h->nb * h->nmu + monos + 10.0 * h->n_basic;
-  if (flop_per_atom_tree) *flop_per_atom_tree = 9.0 * (double)h->sched.n_prod + 2.0 * h->n_basis;
+  if (flop_per_atom_tree) *flop_per_atom_tree = 9.0 * (double)h->n_prod + 2.0 * h->n_basis;
   if (flop_per_atom_grade) *flop_per_atom_grade = 2.0 * (double)h->n_basis * h->n_basis;
   return MTP_OK;
 }

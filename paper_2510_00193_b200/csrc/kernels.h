@@ -15,20 +15,28 @@ long long launch_count();
 struct TreeArgs {
   const TreeTerm *fprog; const int *fwave; int nfw;
   const TreeTerm *bprog; const int *bwave; int nbw;
-  const int *basis_node; const double *xi; const double *xi0;
-  const int *seed_node; const double *seed_val; int n_seed;
+  int n_fprog, n_bprog;                    // entries incl. the prefetch padding
+  int prog_smem_off;                       // byte offset of the staged program in shared memory (set by launch_tree)
+  const double *xi0;
+  const double *adj_init;                  // [n_adj] initial adjoints (slot 0 = 1, else the node's seed)
+  const double *leaf_seed;                 // [n_leaf] seeds of the elided leaves
+  const int *eseed_slot; const double *eseed_val; int n_eseed;   // stored nodes that are basis functions
+  const int *basis_slot;                   // [n_basis] val slot of B_alpha (schedules compiled without elision)
+  const int *gseed_k; const double *gseed_val; int n_gseed;   // packed moments that are basis functions
+  const int *gzero_k; int n_gzero;         // packed moments no op reads
   const double *pos4;
   const double *M; double *G; long long ldm;
   double *Ei;          // [N]
   double *B;           // [N][n_basis] or null
-  int n_nodes, n_basic, n_basis;
+  int n_val, n_adj, n_basic, n_basis;
   int c0, c1;
   int want_adj;
 };
-int tree_pick_al(int n_nodes);          // atoms per CTA (A)
-int tree_row_lanes(int A);              // row-lanes R the schedule must be dealt for
-size_t tree_smem_bytes(int n_nodes, int AL);
-cudaError_t launch_tree(const TreeArgs &a, int AL, cudaStream_t st);
+void tree_pick_shape(int n_val, int n_adj, long long n_atoms, int *AL, int *AR);   // AL = 0: does not fit
+int tree_threads(int AL);               // CTA size used with AL atom-lanes
+int tree_row_lanes(int AL);             // row-lanes R = threads / AL the schedule must be dealt for
+size_t tree_smem_bytes(int n_val, int n_adj, int AL, int AR);
+cudaError_t launch_tree(const TreeArgs &a, int AL, int AR, cudaStream_t st);
 
 // ---- K1 / K3: one entry per compiled level (pair_lev*.cu)
 struct PairLevel {
@@ -44,8 +52,9 @@ cudaError_t launch_pack(const double *pos, const int *type, int n, double *pos4,
 cudaError_t launch_zero(double *p, long long n, cudaStream_t st);
 // F_k = sum_p d[p] - d[rev[p]] over row k (warp per atom, fixed order)
 cudaError_t launch_gather(const long long *off, const int *rev, const double *d4, int n, double *F, cudaStream_t st);
-// out[c] = sum_i in[i*stride + c] for c < ncomp, single block, fixed order
-cudaError_t launch_reduce(const double *in, long long n, int stride, int ncomp, double *out, cudaStream_t st);
+// out[c] = sum_i in[i*stride + c] for c < ncomp <= 8, fixed order; scratch: 256 x 8 doubles (or null)
+cudaError_t launch_reduce(const double *in, long long n, int stride, int ncomp, double *out, double *scratch,
+                          cudaStream_t st);
 // Bsum[b] = sum_i B[i][b]  (fixed order per column)
 cudaError_t launch_colsum(const double *B, long long n, int nb, double *Bsum, double *scratch, cudaStream_t st);
 

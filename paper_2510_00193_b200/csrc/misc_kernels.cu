@@ -51,14 +51,17 @@ __global__ void __launch_bounds__(256) k_gather(const long long *__restrict__ of
   if (lane == 0) { F[3 * (size_t)warp] = fx; F[3 * (size_t)warp + 1] = fy; F[3 * (size_t)warp + 2] = fz; }
 }
 
-// out[c] = sum_i in[i*stride + c], c < ncomp <= 8; one block of 1024 threads, fixed order
+// out[blockIdx.x][c] = sum over this block's share of i of in[i*stride + c], c < ncomp <= 8.
+// Fixed grid, fixed order -> bit-reproducible.  Two launches reduce any n: kReduceBlocks partial rows
+// of stride 8, then one block over those.
+constexpr int kReduceBlocks = 256;
 __global__ void __launch_bounds__(1024) k_reduce_rows(const double *__restrict__ in, long long n, int stride,
                                                       int ncomp, double *__restrict__ out) {
   __shared__ double sm[32][8];
   double acc[8];
 #pragma unroll
   for (int c = 0; c < 8; ++c) acc[c] = 0.0;
-  for (long long i = threadIdx.x; i < n; i += 1024)
+  for (long long i = (long long)blockIdx.x * 1024 + threadIdx.x; i < n; i += 1024LL * gridDim.x)
     for (int c = 0; c < ncomp; ++c) acc[c] += in[i * stride + c];
 #pragma unroll
   for (int c = 0; c < 8; ++c) {
@@ -68,10 +71,12 @@ __global__ void __launch_bounds__(1024) k_reduce_rows(const double *__restrict__
     if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5][c] = v;
   }
   __syncthreads();
-  if (threadIdx.x < ncomp) {
+  if (threadIdx.x < 8) {
     double v = 0.0;
-    for (int w = 0; w < 32; ++w) v += sm[w][threadIdx.x];
-    out[threadIdx.x] = v;
+    if (threadIdx.x < ncomp)
+      for (int w = 0; w < 32; ++w) v += sm[w][threadIdx.x];
+    if (gridDim.x > 1) out[(size_t)blockIdx.x * 8 + threadIdx.x] = v;
+    else if (threadIdx.x < ncomp) out[threadIdx.x] = v;
   }
 }
 
@@ -111,8 +116,15 @@ cudaError_t launch_gather(const long long *off, const int *rev, const double *d4
   count_launch();
   return cudaGetLastError();
 }
-cudaError_t launch_reduce(const double *in, long long n, int stride, int ncomp, double *out, cudaStream_t st) {
-  k_reduce_rows<<<1, 1024, 0, st>>>(in, n, stride, ncomp, out);
+cudaError_t launch_reduce(const double *in, long long n, int stride, int ncomp, double *out, double *scratch,
+                          cudaStream_t st) {
+  if (n > 64 * 1024 && scratch) {
+    k_reduce_rows<<<kReduceBlocks, 1024, 0, st>>>(in, n, stride, ncomp, scratch);
+    count_launch();
+    k_reduce_rows<<<1, 1024, 0, st>>>(scratch, kReduceBlocks, 8, ncomp, out);
+  } else {
+    k_reduce_rows<<<1, 1024, 0, st>>>(in, n, stride, ncomp, out);
+  }
   count_launch();
   return cudaGetLastError();
 }

@@ -1,195 +1,278 @@
 // K2: forward contraction tree (a5: B_alpha, E_i) and its adjoint sweep (a6: G = dE_i/dM).
 // BASELINE.json north_star: "forward/adjoint contraction kernel with the tree in registers and
-// shared memory".  A CTA of 128 threads owns AL atoms; node values and adjoints of those atoms
-// live in shared memory as [node][AL]; thread (rl, al) walks the items rl, rl+R, ... of each
-// wave for its AR atoms (R = 128/AL row-lanes, A = AL*AR atoms per CTA).  The table is read once per CTA per wave through
-// L1/L2 (identical for all atoms).
+// shared memory".  Persistent CTAs loop over groups of A = AL*AR atoms.  Thread (rl, al) owns
+// the AR atoms of atom-lane al and is row-lane rl of R = NT/AL; node values val[slot][A] and
+// the adjoints of the intermediate nodes adj[slot][A] live in shared memory (tree.h explains
+// which nodes get a slot).  Row-lane rl executes entry [s][rl] of every step s of the
+// lane-major program.  With AL = 32 a warp is one row-lane: the 16-byte entry is warp-uniform,
+// every shared access is a conflict-free full row, M is read and G written as full lines; AR = 2
+// halves the decode work per atom.  The adjoints of the packed moments (the last backward
+// wave) go straight to global memory.  The program is staged in shared memory once per CTA when
+// it fits, else streamed through L1/L2 (it is identical for all CTAs).
 #include <cuda_runtime.h>
 
 #include "kernels.h"
 
 namespace mtpb {
 
-// row stride (doubles) of the [node][atom] arrays: +2 spreads rows of different nodes over the banks
-__host__ __device__ constexpr int tree_ld(int A) { return A >= 4 ? A + 2 : A; }
-
 template <int AR>
-__device__ __forceinline__ void ldv(const double *p, double (&v)[AR]) {
-  if (AR == 1) { v[0] = p[0]; }
-  else {
-#pragma unroll
-    for (int j = 0; j < AR; j += 2) { const double2 t = *reinterpret_cast<const double2 *>(p + j); v[j] = t.x; v[j + 1] = t.y; }
-  }
+struct Vec { double v[AR]; };
+template <int AR>
+__device__ __forceinline__ Vec<AR> lds(const char *p) {
+  Vec<AR> r;
+  if (AR == 1) r.v[0] = *reinterpret_cast<const double *>(p);
+  else { const double2 t = *reinterpret_cast<const double2 *>(p); r.v[0] = t.x; r.v[AR - 1] = t.y; }
+  return r;
 }
 template <int AR>
-__device__ __forceinline__ void stv(double *p, const double (&v)[AR]) {
-  if (AR == 1) { p[0] = v[0]; }
-  else {
-#pragma unroll
-    for (int j = 0; j < AR; j += 2) *reinterpret_cast<double2 *>(p + j) = make_double2(v[j], v[j + 1]);
-  }
+__device__ __forceinline__ void sts(char *p, const Vec<AR> &x) {
+  if (AR == 1) *reinterpret_cast<double *>(p) = x.v[0];
+  else *reinterpret_cast<double2 *>(p) = make_double2(x.v[0], x.v[AR - 1]);
 }
 
-// One wave of the lane-major program (tree.h): thread (rl, al) executes entry [s][rl] of every
-// step s for its AR atoms (register blocking: one table read and one decode serve AR atoms).
-// Entries are prefetched kTreePrefetch steps ahead; a warp's reads of one step are contiguous.
-template <int LD, int AR, int R, bool BWD>
-__device__ __forceinline__ void run_wave(const TreeTerm *__restrict__ prog, int lo, int hi, int rl,
-                                         const double *__restrict__ val, double *adj, double *valw, int cb) {
-  constexpr int PF = kTreePrefetch;
-  const double *src0 = BWD ? adj : val;
-  const int4 *p = reinterpret_cast<const int4 *>(prog) + (size_t)lo * R + rl;
+// One pass (all forward waves, or all backward waves) of the lane-major program.  The entries of a
+// row-lane form one contiguous strided stream across the waves, so a PF-deep register queue of
+// entries is kept full over the whole pass (from the shared-memory copy of the program when PS,
+// else through L1/L2); waves end on multiples of kTreePrefetch steps, where the CTA barrier sits.
+//   fwd: acc += val[a] * val[b];        bwd: acc += adj[a] * val[b]
+//   group close: tot += mult * acc;     row close: store / accumulate tot (tree.h kTreeAlt)
+template <int AL, int AR, int R, bool BWD, bool PS>
+__device__ __forceinline__ void run_pass(const int4 *__restrict__ prog, const int *__restrict__ wave, int n_waves,
+                                         int rl, const char *__restrict__ val, char *adj, char *valw,
+                                         const double *__restrict__ leaf_seed, Vec<AR> &e,
+                                         double *__restrict__ Gcol, long long ldm, int n_ok) {
+  constexpr int BL = kTreePrefetch;            // block: entries between two wave-boundary checks
+  constexpr int NB = PS ? 1 : 4;               // blocks in the queue: 4 entries ahead from shared memory, 16 from L2
+  constexpr int PF = BL * NB;
+  constexpr unsigned ROW = AL * AR * 8;
+  if (n_waves <= 0) return;
+  const char *src0 = BWD ? adj : val;
+  const int4 *p = prog + rl;                   // entry of step 0
   int4 T[PF];
 #pragma unroll
-  for (int u = 0; u < PF; ++u) T[u] = __ldg(p + (size_t)u * R);
-  double acc[AR];
+  for (int u = 0; u < PF; ++u) T[u] = PS ? p[(size_t)u * R] : __ldg(p + (size_t)u * R);
+  Vec<AR> acc, tot;
 #pragma unroll
-  for (int r = 0; r < AR; ++r) acc[r] = 0.0;
-  for (int s = lo; s < hi; s += PF) {
-    p += (size_t)PF * R;
+  for (int r = 0; r < AR; ++r) { acc.v[r] = 0.0; tot.v[r] = 0.0; }
+  int s = 0, w = 0, hi = wave[1];
+  while (true) {
 #pragma unroll
-    for (int u = 0; u < PF; ++u) {
-      const int4 t = T[u];
-      T[u] = __ldg(p + (size_t)u * R);          // padded past the end of the program
-      const double m = __hiloint2double(t.w, t.z);
-      const int na = t.x & 0xffff, nb = (unsigned)t.x >> 16;
-      double x[AR], y[AR];
-      ldv<AR>(src0 + na * LD + cb, x);
-      ldv<AR>(val + nb * LD + cb, y);
+    for (int q = 0; q < NB; ++q) {
+      while (s >= hi) {                        // wave boundary (uniform over the CTA)
+        __syncthreads();
+        if (++w == n_waves) return;
+        hi = wave[w + 1];
 #pragma unroll
-      for (int r = 0; r < AR; ++r) acc[r] = fma(m * x[r], y[r], acc[r]);
-      if ((unsigned)t.y >> 16) {                 // entry closes a row
-        double *dst = (BWD ? adj : valw) + (t.y & 0xffff) * LD + cb;
-        if (BWD) {
-          double old[AR];
-          ldv<AR>(dst, old);
+        for (int r = 0; r < AR; ++r) { acc.v[r] = 0.0; tot.v[r] = 0.0; }   // drop what the no-op padding added
+      }
 #pragma unroll
-          for (int r = 0; r < AR; ++r) acc[r] += old[r];
+      for (int v = 0; v < BL; ++v) {
+        const int u = q * BL + v;
+        const int4 t = T[u];
+        const Vec<AR> x = lds<AR>(src0 + ((unsigned)t.x & ~7u));
+        const Vec<AR> y = lds<AR>(val + ((unsigned)t.y & ((1u << kTreeDstShift) - 1)));
+#pragma unroll
+        for (int r = 0; r < AR; ++r) acc.v[r] = fma(x.v[r], y.v[r], acc.v[r]);
+        if (t.x & (int)kTreeGroup) {
+          const double m = __hiloint2double(t.w, t.z);
+#pragma unroll
+          for (int r = 0; r < AR; ++r) { tot.v[r] = fma(m, acc.v[r], tot.v[r]); acc.v[r] = 0.0; }
+          if (t.x & (int)kTreeRow) {
+            const unsigned d = (unsigned)t.y >> kTreeDstShift;
+            if (!BWD) {
+              if (t.x & (int)kTreeAlt) {
+                const double sd = __ldg(leaf_seed + d);
+#pragma unroll
+                for (int r = 0; r < AR; ++r) e.v[r] = fma(sd, tot.v[r], e.v[r]);
+              } else {
+                sts<AR>(valw + d * ROW, tot);
+              }
+            } else if (t.x & (int)kTreeAlt) {
+#pragma unroll
+              for (int r = 0; r < AR; ++r)
+                if (r < n_ok) Gcol[(long long)d * ldm + r] = tot.v[r];
+            } else {
+              char *qd = adj + d * ROW;               // adj was initialised with the node's seed
+              Vec<AR> old = lds<AR>(qd);
+#pragma unroll
+              for (int r = 0; r < AR; ++r) old.v[r] += tot.v[r];
+              sts<AR>(qd, old);
+            }
+#pragma unroll
+            for (int r = 0; r < AR; ++r) tot.v[r] = 0.0;
+          }
         }
-        stv<AR>(dst, acc);
-#pragma unroll
-        for (int r = 0; r < AR; ++r) acc[r] = 0.0;
+        // refill the slot PF steps ahead (the program is padded past its end)
+        T[u] = PS ? p[(size_t)(s + v + PF) * R] : __ldg(p + (size_t)(s + v + PF) * R);
       }
+      s += BL;
     }
   }
 }
 
-template <int AL, int AR>
-__global__ void __launch_bounds__(128) k_tree(const TreeArgs a) {
-  extern __shared__ __align__(16) double sm[];
-  constexpr int A = AL * AR, R = 128 / AL, LD = tree_ld(A);
-  double *val = sm;
-  double *adj = sm + (size_t)a.n_nodes * LD;
-  const int al = threadIdx.x % AL, rl = threadIdx.x / AL, cb = al * AR;
-  const int atom0 = a.c0 + blockIdx.x * A + cb;       // this thread's first atom
-  const long long col0 = atom0 - a.c0;
-  for (int k = rl; k < a.n_nodes; k += R) {
-    double v[AR], z[AR];
+template <int AL, int AR, int NT, bool PS>
+__global__ void __launch_bounds__(NT) k_tree(const TreeArgs a) {
+  extern __shared__ __align__(16) char smraw[];
+  constexpr int R = NT / AL, A = AL * AR;
+  double *val = reinterpret_cast<double *>(smraw);
+  double *adj = val + (size_t)a.n_val * A;
+  double *esm = adj + (size_t)a.n_adj * A;            // [NT][AR] energy partials
+  int *wsm = reinterpret_cast<int *>(esm + NT * AR);  // wave offsets: fwave [nfw+1], bwave [nbw+1]
+  const int4 *fprog = reinterpret_cast<const int4 *>(a.fprog), *bprog = reinterpret_cast<const int4 *>(a.bprog);
+  for (int i = threadIdx.x; i <= a.nfw; i += NT) wsm[i] = a.fwave[i];
+  for (int i = threadIdx.x; i <= a.nbw; i += NT) wsm[a.nfw + 1 + i] = a.bwave[i];
+  if (PS) {
+    int4 *psm = reinterpret_cast<int4 *>(smraw + a.prog_smem_off);
+    for (int i = threadIdx.x; i < a.n_fprog; i += NT) psm[i] = __ldg(fprog + i);
+    for (int i = threadIdx.x; i < a.n_bprog; i += NT) psm[a.n_fprog + i] = __ldg(bprog + i);
+    fprog = psm; bprog = psm + a.n_fprog;
+  }
+  const int *fw = wsm, *bw = wsm + a.nfw + 1;
+  const int al = threadIdx.x % AL, rl = threadIdx.x / AL;
+  const char *valc = smraw + al * AR * 8;                          // this atom-lane's column
+  char *adjc = reinterpret_cast<char *>(adj) + al * AR * 8;
+  const int n_groups = (a.c1 - a.c0 + A - 1) / A;
+  for (int g = blockIdx.x; g < n_groups; g += gridDim.x) {
+    const int atom0 = a.c0 + g * A + al * AR;                      // this thread's first atom
+    const int n_ok = min(AR, max(0, a.c1 - atom0));                // how many of its atoms exist
+    const long long col = atom0 - a.c0;
+    __syncthreads();                         // previous group's reads are done (and wsm / psm are filled)
+    for (int k = rl; k < a.n_basic; k += R) {
+      Vec<AR> m;
 #pragma unroll
-    for (int r = 0; r < AR; ++r) {
-      v[r] = (k < a.n_basic && atom0 + r < a.c1) ? a.M[(long long)k * a.ldm + col0 + r] : 0.0;
-      z[r] = 0.0;
+      for (int r = 0; r < AR; ++r) m.v[r] = r < n_ok ? a.M[(long long)k * a.ldm + col + r] : 0.0;
+      sts<AR>(const_cast<char *>(valc) + (size_t)k * A * 8, m);
     }
-    stv<AR>(val + k * LD + cb, v);
-    stv<AR>(adj + k * LD + cb, z);
-  }
-  __syncthreads();
-  for (int w = 0; w < a.nfw; ++w) {
-    run_wave<LD, AR, R, false>(a.fprog, a.fwave[w], a.fwave[w + 1], rl, val, adj, val, cb);
-    __syncthreads();
-  }
-  // ---- energy and basis values
-  {
-    double e[AR];
+    if (a.want_adj)
+      for (int k = rl; k < a.n_adj; k += R) {
+        Vec<AR> s;
 #pragma unroll
-    for (int r = 0; r < AR; ++r) e[r] = 0.0;
-    for (int b = rl; b < a.n_basis; b += R) {
-      const int n = a.basis_node[b];
-      const double x = a.xi[b];
-      double v[AR];
-      ldv<AR>(val + n * LD + cb, v);
-#pragma unroll
-      for (int r = 0; r < AR; ++r) {
-        e[r] = fma(x, v[r], e[r]);
-        if (a.B && atom0 + r < a.c1) a.B[(long long)(atom0 + r) * a.n_basis + b] = v[r];
+        for (int r = 0; r < AR; ++r) s.v[r] = a.adj_init[k];
+        sts<AR>(adjc + (size_t)k * A * 8, s);
       }
-    }
-    __shared__ double esm[128 * AR];       // fixed-order reduction over the R row-lanes
-#pragma unroll
-    for (int r = 0; r < AR; ++r) esm[threadIdx.x * AR + r] = e[r];
     __syncthreads();
-    if (rl == 0) {
+    Vec<AR> e;
 #pragma unroll
-      for (int r = 0; r < AR; ++r) {
-        if (atom0 + r < a.c1) {
-          double s = 0.0;
-          for (int q = 0; q < R; ++q) s += esm[(q * AL + al) * AR + r];
-          const int z = (int)a.pos4[4 * (size_t)(atom0 + r) + 3];
-          a.Ei[atom0 + r] = a.xi0[z] + s;
+    for (int r = 0; r < AR; ++r) e.v[r] = 0.0;
+    run_pass<AL, AR, R, false, PS>(fprog, fw, a.nfw, rl, valc, nullptr, const_cast<char *>(valc), a.leaf_seed, e, nullptr,
+                                   0, n_ok);
+    // ---- energy (stored basis nodes here, elided leaves were added inside the waves) and basis values
+    {
+      for (int q = rl; q < a.n_eseed; q += R) {
+        const Vec<AR> v = lds<AR>(valc + (size_t)a.eseed_slot[q] * A * 8);
+        const double sd = a.eseed_val[q];
+#pragma unroll
+        for (int r = 0; r < AR; ++r) e.v[r] = fma(sd, v.v[r], e.v[r]);
+      }
+#pragma unroll
+      for (int r = 0; r < AR; ++r) esm[(rl * A) + al * AR + r] = e.v[r];
+      if (a.B) {        // B[atom][b]: consecutive threads write consecutive b of one atom
+        const int na = min(A, a.c1 - (a.c0 + g * A));
+        for (int i = threadIdx.x; i < na * a.n_basis; i += NT) {
+          const int at = i / a.n_basis, b = i - at * a.n_basis;
+          a.B[(long long)(a.c0 + g * A + at) * a.n_basis + b] = val[a.basis_slot[b] * A + at];
+        }
+      }
+      __syncthreads();
+      if (rl == 0) {                             // fixed-order reduction over the R row-lanes
+#pragma unroll
+        for (int r = 0; r < AR; ++r) {
+          if (r < n_ok) {
+            double s = 0.0;
+            for (int q = 0; q < R; ++q) s += esm[q * A + al * AR + r];
+            const int z = (int)a.pos4[4 * (size_t)(atom0 + r) + 3];
+            a.Ei[atom0 + r] = a.xi0[z] + s;
+          }
         }
       }
     }
-  }
-  if (!a.want_adj) return;
-  for (int q = rl; q < a.n_seed; q += R) {
-    double v[AR];
+    if (!a.want_adj) continue;
+    double *Gcol = a.G + col;
+    for (int q = rl; q < a.n_gzero; q += R)
 #pragma unroll
-    for (int r = 0; r < AR; ++r) v[r] = a.seed_val[q];
-    stv<AR>(adj + a.seed_node[q] * LD + cb, v);
-  }
-  __syncthreads();
-  for (int w = 0; w < a.nbw; ++w) {
-    run_wave<LD, AR, R, true>(a.bprog, a.bwave[w], a.bwave[w + 1], rl, val, adj, val, cb);
+      for (int r = 0; r < AR; ++r)
+        if (r < n_ok) Gcol[(long long)a.gzero_k[q] * a.ldm + r] = 0.0;
+    run_pass<AL, AR, R, true, PS>(bprog, bw, a.nbw, rl, valc, adjc, nullptr, nullptr, e, Gcol, a.ldm, n_ok);
     __syncthreads();
-  }
-  for (int k = rl; k < a.n_basic; k += R) {
-    double g[AR];
-    ldv<AR>(adj + k * LD + cb, g);
+    // packed moments that are basis functions themselves (M_{mu,0}): G += xi
+    for (int q = rl; q < a.n_gseed; q += R)
 #pragma unroll
-    for (int r = 0; r < AR; ++r)
-      if (atom0 + r < a.c1) a.G[(long long)k * a.ldm + col0 + r] = g[r];
+      for (int r = 0; r < AR; ++r)
+        if (r < n_ok) Gcol[(long long)a.gseed_k[q] * a.ldm + r] += a.gseed_val[q];
   }
 }
 
-size_t tree_smem_bytes(int n_nodes, int A) { return (size_t)n_nodes * tree_ld(A) * 16; }
+// shared memory: val [n_val][A] + adj [n_adj][A] + energy partials [NT][AR] + wave offsets (<= 1 KB)
+// [+ the program when it is staged]
+int tree_threads(int AL) { return AL >= 16 ? 512 : (AL == 8 ? 256 : 128); }
+int tree_row_lanes(int AL) { return tree_threads(AL) / AL; }
+size_t tree_smem_bytes(int n_val, int n_adj, int AL, int AR) {
+  return (((size_t)n_val + (size_t)n_adj) * AL * AR * 8 + (size_t)tree_threads(AL) * AR * 8 + 1024 + 15) & ~(size_t)15;
+}
+constexpr size_t kTreeSmemMax = 225 * 1024;
 
-int tree_pick_al(int n_nodes) {
-  // largest AL <= 16 that lets two CTAs share an SM, else the largest that fits at all
-  for (int al = 16; al >= 1; al >>= 1)
-    if (tree_smem_bytes(n_nodes, al) <= 100 * 1024) return al;
-  for (int al = 16; al >= 1; al >>= 1)
-    if (tree_smem_bytes(n_nodes, al) <= 220 * 1024) return al;
-  return 0;
+// Atoms per CTA as (AL, AR): the largest that fits in shared memory, reduced for small systems so
+// that the grid still covers the SMs (PAPER.md:35,182 small-system regime).
+void tree_pick_shape(int n_val, int n_adj, long long n_atoms, int *AL, int *AR) {
+  *AL = 0; *AR = 1;
+  static const int shapes[][2] = {{32, 2}, {32, 1}, {16, 1}, {8, 1}, {4, 1}, {2, 1}, {1, 1}};
+  for (auto &sh : shapes) {
+    if (tree_smem_bytes(n_val, n_adj, sh[0], sh[1]) > kTreeSmemMax) continue;
+    const long long A = sh[0] * sh[1];
+    if (n_atoms > 0 && A > 4 && (n_atoms + A - 1) / A < 296) continue;   // too few CTAs for 148 SMs
+    *AL = sh[0]; *AR = sh[1];
+    return;
+  }
 }
 
-template <int AL, int AR>
-static cudaError_t launch_al(const TreeArgs &a, cudaStream_t st) {
-  constexpr int A = AL * AR;
-  const size_t smem = tree_smem_bytes(a.n_nodes, A);
+template <int AL, int AR, int NT, bool PS>
+static cudaError_t launch_al(const TreeArgs &a0, size_t smem, cudaStream_t st) {
   static bool attr_done = false;
+  static int sms = 148;
   if (!attr_done) {
-    cudaError_t e = cudaFuncSetAttribute(k_tree<AL, AR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
+    cudaError_t e = cudaFuncSetAttribute(k_tree<AL, AR, NT, PS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTreeSmemMax);
     if (e != cudaSuccess) return e;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     attr_done = true;
   }
-  const int n = a.c1 - a.c0;
-  const int grid = (n + A - 1) / A;
-  if (grid <= 0) return cudaSuccess;
-  k_tree<AL, AR><<<grid, 128, smem, st>>>(a);
+  const int n = a0.c1 - a0.c0;
+  const int groups = (n + AL * AR - 1) / (AL * AR);
+  if (groups <= 0) return cudaSuccess;
+  int per_sm = 1;
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_tree<AL, AR, NT, PS>, NT, smem);
+  if (per_sm < 1) per_sm = 1;
+  const int grid = groups < sms * per_sm ? groups : sms * per_sm;
+  k_tree<AL, AR, NT, PS><<<grid, NT, smem, st>>>(a0);
   count_launch();
   return cudaGetLastError();
 }
 
-// A = atoms per CTA; AR = min(4, A) atoms per thread, AL = A / AR atom-lanes, R = 128 / AL row-lanes
-int tree_row_lanes(int A) { const int AR = A < 4 ? A : 4; return 128 / (A / AR); }
+template <int AL, int AR, int NT>
+static cudaError_t launch_ps(TreeArgs a, cudaStream_t st) {
+  // stage the program in shared memory when it fits beside the node arrays and the CTA has
+  // enough atom groups to amortise the copy
+  const size_t base = tree_smem_bytes(a.n_val, a.n_adj, AL, AR);
+  const size_t pbytes = ((size_t)a.n_fprog + a.n_bprog) * sizeof(TreeTerm);
+  const long long groups = (a.c1 - a.c0 + AL * AR - 1) / (AL * AR);
+  if (base + pbytes <= kTreeSmemMax && groups >= 4 * 148) {
+    a.prog_smem_off = (int)base;
+    return launch_al<AL, AR, NT, true>(a, base + pbytes, st);
+  }
+  a.prog_smem_off = 0;
+  return launch_al<AL, AR, NT, false>(a, base, st);
+}
 
-cudaError_t launch_tree(const TreeArgs &a, int A, cudaStream_t st) {
-  switch (A) {
-    case 1: return launch_al<1, 1>(a, st);
-    case 2: return launch_al<1, 2>(a, st);
-    case 4: return launch_al<1, 4>(a, st);
-    case 8: return launch_al<2, 4>(a, st);
-    case 16: return launch_al<4, 4>(a, st);
+cudaError_t launch_tree(const TreeArgs &a, int AL, int AR, cudaStream_t st) {
+  switch (AL * 4 + AR) {
+    case 1 * 4 + 1: return launch_ps<1, 1, 128>(a, st);
+    case 2 * 4 + 1: return launch_ps<2, 1, 128>(a, st);
+    case 4 * 4 + 1: return launch_ps<4, 1, 128>(a, st);
+    case 8 * 4 + 1: return launch_ps<8, 1, 256>(a, st);
+    case 16 * 4 + 1: return launch_ps<16, 1, 512>(a, st);
+    case 32 * 4 + 1: return launch_ps<32, 1, 512>(a, st);
+    case 32 * 4 + 2: return launch_ps<32, 2, 512>(a, st);
     default: return cudaErrorInvalidValue;
   }
 }
