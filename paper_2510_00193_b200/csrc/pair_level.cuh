@@ -1,42 +1,57 @@
-// Instantiates K1 / K3 for one compiled level and exposes them through a PairLevel record.
+// Instantiates K1 / K3 (tiled, pair_tiled.cuh) for one compiled level and exposes them through a
+// PairLevel record.  P = 1 is the large-system mapping ("thread-parallel" regime), P = PS
+// splits each atom's neighbours over PS lanes (the small-system / "block-parallel" regime).
 #pragma once
 #include "kernels.h"
-#include "pair_kernels.cuh"
+#include "pair_tiled.cuh"
 
 namespace mtpb {
 
 template <int LEV, int NSB, int NSC, int PS>
 struct PairLevelImpl {
   using Sl = Slices<LEV, NSB, NSC>;
-  static int grid_for(int n_atoms, int P) {
-    const long long threads = (long long)n_atoms * Sl::NS * P;
-    return (int)((threads + 127) / 128);
+  static constexpr int kWarps = 4;                      // 128 threads per CTA
+  template <int P>
+  static int grid_for(int n_atoms) {
+    const int per_cta = Tile<LEV, NSB, NSC, P>::NA * kWarps;
+    return (n_atoms + per_cta - 1) / per_cta;
   }
-  static size_t smem(const PairArgs &a) { return sizeof(double) * a.n_species * a.n_species * a.crow; }
+  static size_t coef_doubles(const PairArgs &a) { return (size_t)((a.n_species * a.n_species * a.crow + 1) & ~1); }
+  template <class K>
+  static cudaError_t prep(K kernel, size_t smem) {
+    return smem > 48 * 1024 ? cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) : cudaSuccess;
+  }
+  template <int P>
+  static cudaError_t moments_p(const PairArgs &a, int n, cudaStream_t st) {
+    const size_t smem = 8 * (coef_doubles(a) + (size_t)kWarps * Tile<LEV, NSB, NSC, P>::WARP1);
+    cudaError_t e = prep(k_moments_t<LEV, NSB, NSC, P>, smem);
+    if (e != cudaSuccess) return e;
+    k_moments_t<LEV, NSB, NSC, P><<<grid_for<P>(n), 32 * kWarps, smem, st>>>(a);
+    count_launch();
+    return cudaGetLastError();
+  }
+  template <int P, bool ATOMIC>
+  static cudaError_t pairgrad_p(const PairArgs &a, int n, cudaStream_t st) {
+    const size_t smem = 8 * (coef_doubles(a) + (size_t)kWarps * Tile<LEV, NSB, NSC, P>::WARP3);
+    cudaError_t e = prep(k_pairgrad_t<LEV, NSB, NSC, P, ATOMIC>, smem);
+    if (e != cudaSuccess) return e;
+    k_pairgrad_t<LEV, NSB, NSC, P, ATOMIC><<<grid_for<P>(n), 32 * kWarps, smem, st>>>(a);
+    count_launch();
+    return cudaGetLastError();
+  }
   static cudaError_t moments(const PairArgs &a, int P, cudaStream_t st) {
     const int n = a.c1 - a.c0;
     if (n <= 0) return cudaSuccess;
-    if (P == 1) k_moments<LEV, NSB, NSC, 1><<<grid_for(n, 1), 128, smem(a), st>>>(a);
-    else k_moments<LEV, NSB, NSC, PS><<<grid_for(n, PS), 128, smem(a), st>>>(a);
-    count_launch();
-    return cudaGetLastError();
+    return P == 1 ? moments_p<1>(a, n, st) : moments_p<PS>(a, n, st);
   }
   static cudaError_t pairgrad(const PairArgs &a, int P, int atomic, cudaStream_t st, int *grid_out) {
     const int n = a.c1 - a.c0;
-    if (n <= 0) { if (grid_out) *grid_out = 0; return cudaSuccess; }
-    const int g = grid_for(n, P == 1 ? 1 : PS);
-    if (grid_out) *grid_out = g;
-    if (P == 1) {
-      if (atomic) k_pairgrad<LEV, NSB, NSC, 1, true><<<g, 128, smem(a), st>>>(a);
-      else k_pairgrad<LEV, NSB, NSC, 1, false><<<g, 128, smem(a), st>>>(a);
-    } else {
-      if (atomic) k_pairgrad<LEV, NSB, NSC, PS, true><<<g, 128, smem(a), st>>>(a);
-      else k_pairgrad<LEV, NSB, NSC, PS, false><<<g, 128, smem(a), st>>>(a);
-    }
-    count_launch();
-    return cudaGetLastError();
+    if (grid_out) *grid_out = n > 0 ? pairgrad_grid(n, P) : 0;
+    if (n <= 0) return cudaSuccess;
+    if (P == 1) return atomic ? pairgrad_p<1, true>(a, n, st) : pairgrad_p<1, false>(a, n, st);
+    return atomic ? pairgrad_p<PS, true>(a, n, st) : pairgrad_p<PS, false>(a, n, st);
   }
-  static int pairgrad_grid(int n_atoms, int P) { return grid_for(n_atoms, P == 1 ? 1 : PS); }
+  static int pairgrad_grid(int n_atoms, int P) { return P == 1 ? grid_for<1>(n_atoms) : grid_for<PS>(n_atoms); }
   static PairLevel record() {
     return PairLevel{LEV, NSB, NSC, Sl::NSLOT, PS, &moments, &pairgrad, &pairgrad_grid};
   }

@@ -1,0 +1,340 @@
+// Tiled pair kernels (K1 moments, K3 pair gradient): each warp alternates between two lane
+// mappings over a tile of 128 pairs staged in shared memory.
+//
+//   phase A  lanes = pairs.  A warp owns NA = 32/(NS*P) atoms whose CSR rows are contiguous; a tile
+//            holds neighbours [t*TN, (t+1)*TN) of each of them (TN = 4*NS*P, NA*TN = 128), four
+//            consecutive pairs per lane.  a1-a3 are done ONCE per pair here: coalesced loads of
+//            idx / shift, position gather, r, Chebyshev recurrence, f_mu (and f'_mu for K3); the
+//            result (x, y, z, f[, f']) goes to the warp's shared-memory tile.  Pairs past the end
+//            of a row or with r >= R_cut are stored as zeros, so that phase B needs no predicates.
+//   phase B  lanes = (atom, slice, part) as in stair.h: every lane walks the TN staged pairs of its
+//            atom (parts split them) and does only the part that scales with n_basic -- monomials
+//            and moment FMAs (K1) or the nested Horner sweeps over G (K3).
+//   phase C  (K3) lanes = pairs again: d_ij from the tile is written as full 32-byte records to
+//            d4 (or scattered with fp64 atomics), virial and own-atom force partials accumulate.
+// Only __syncwarp() separates the phases; warps of a CTA drift apart, so one warp's gathers
+// overlap another's FMA stream.  BASELINE.json north_star rows a1-a4, a7; readings G1-G7, G17.
+#pragma once
+#include <cuda_runtime.h>
+#include "pair_kernels.cuh"
+
+namespace mtpb {
+
+template <int LEV, int NSB, int NSC, int P>
+struct Tile {
+  using St = Stair<LEV>;
+  using Sl = Slices<LEV, NSB, NSC>;
+  static constexpr int NMU = St::NMU, NS = Sl::NS, LPA = NS * P, NA = 32 / LPA, TN = 4 * LPA;
+  static_assert(LPA <= 32 && 32 % LPA == 0, "lanes per atom must divide the warp");
+  static constexpr int PD1 = (3 + NMU + 1) & ~1;        // doubles per staged pair, K1: x y z f[NMU]
+  static constexpr int PD3 = (3 + 2 * NMU + 1) & ~1;    // K3: x y z f[NMU] f'[NMU]
+  static constexpr int ROW1 = TN * PD1 + 2, ROW3 = TN * PD3 + 2;   // +16 B: rows of different atoms spread over the banks
+  static constexpr int WARP1 = NA * ROW1;                // doubles per warp
+  static constexpr int WARP3 = NA * ROW3 + 128 * 4;      // + d_ij of the tile (x y z pad)
+};
+
+// Phase A for one pair: geometry + radial functions; writes PD doubles (zeros when the pair does not contribute).
+template <int NMU, bool DERIV, int PD>
+__device__ __forceinline__ void stage_pair(const PairArgs &a, const double *__restrict__ csm, bool valid, long long p,
+                                           double xi, double yi, double zi, int zi_s, double rc2, double *__restrict__ out) {
+  double x = 0.0, y = 0.0, z = 0.0, f[NMU], df[NMU];
+#pragma unroll
+  for (int m = 0; m < NMU; ++m) { f[m] = 0.0; df[m] = 0.0; }
+  if (valid) {
+    const int j = a.idx[p];
+    double xj, yj, zj, tj;
+    load_pos4(a.pos4, j, xj, yj, zj, tj);
+    pair_vector(a, p, xi, yi, zi, xj, yj, zj, x, y, z);
+    const double r2 = x * x + y * y + z * z;
+    if (r2 < rc2) {
+      const double r = r2 * rsqrt(r2);
+      radial<NMU, DERIV>(csm + (zi_s * a.n_species + (int)tj) * a.crow, a.nb, r, a.r_min, a.r_cut, f, df);
+    }
+  }
+  double2 *o = reinterpret_cast<double2 *>(out);
+  double buf[PD];
+  buf[0] = x; buf[1] = y; buf[2] = z;
+#pragma unroll
+  for (int m = 0; m < NMU; ++m) buf[3 + m] = f[m];
+  if (DERIV) {
+#pragma unroll
+    for (int m = 0; m < NMU; ++m) buf[3 + NMU + m] = df[m];
+  }
+#pragma unroll
+  for (int q = 3 + (DERIV ? 2 : 1) * NMU; q < PD; ++q) buf[q] = 0.0;
+#pragma unroll
+  for (int q = 0; q < PD / 2; ++q) o[q] = make_double2(buf[2 * q], buf[2 * q + 1]);
+}
+
+// ------------------------------------------------------------------------------ K1
+template <int LEV, int NSB, int NSC, int P>
+__global__ void __launch_bounds__(128) k_moments_t(const PairArgs a) {
+  using St = Stair<LEV>;
+  using Sl = Slices<LEV, NSB, NSC>;
+  using Tl = Tile<LEV, NSB, NSC, P>;
+  constexpr int NMU = St::NMU, NU0 = St::NU0, NS = Sl::NS, NSLOT = Sl::NSLOT, LPA = Tl::LPA, NA = Tl::NA, TN = Tl::TN;
+  constexpr int PD = Tl::PD1, ROW = Tl::ROW1;
+  extern __shared__ __align__(16) double csm[];
+  stage_coef(a, csm);
+  const int ncoef = (a.n_species * a.n_species * a.crow + 1) & ~1;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  double *tile = csm + ncoef + wib * Tl::WARP1;
+  const int warp = blockIdx.x * (blockDim.x >> 5) + wib;
+  const int sa = lane / LPA, q = lane % LPA, slice = q % NS, part = q / NS, sb = slice % NSB, sc = slice / NSB;
+  const int atom = a.c0 + warp * NA + sa;
+  const bool act = atom < a.c1;
+  double xi = 0, yi = 0, zi = 0, ti = 0;
+  long long beg = 0;
+  int n_nb = 0;
+  if (act) {
+    load_pos4(a.pos4, atom, xi, yi, zi, ti);
+    beg = a.off[atom];
+    n_nb = (int)(a.off[atom + 1] - beg);
+  }
+  const int zi_s = (int)ti;
+  const double rc2 = a.r_cut * a.r_cut;
+  const int n_max = __reduce_max_sync(0xffffffffu, n_nb);
+  double acc[NSLOT];
+#pragma unroll
+  for (int s = 0; s < NSLOT; ++s) acc[s] = 0.0;
+  const int ka = (4 * lane) % TN;                  // phase A: this lane stages neighbours t0 + ka .. + 3 of atom slot sa
+  double *mine = tile + sa * ROW;
+  for (int t0 = 0; t0 < n_max; t0 += TN) {
+    __syncwarp();
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int k = t0 + ka + u;
+      stage_pair<NMU, false, PD>(a, csm, k < n_nb, beg + k, xi, yi, zi, zi_s, rc2, mine + (ka + u) * PD);
+    }
+    __syncwarp();
+    const int kend = min(TN, n_max - t0);
+    for (int k = part; k < kend; k += P) {
+      const double2 *src = reinterpret_cast<const double2 *>(mine + k * PD);
+      double buf[PD];
+#pragma unroll
+      for (int w = 0; w < PD / 2; ++w) { const double2 v = src[w]; buf[2 * w] = v.x; buf[2 * w + 1] = v.y; }
+      const double x = buf[0], y = buf[1], z = buf[2];
+      double ysb, zs, yN, zN, dump;
+      pow_small(sb, y, ysb, dump);
+      pow_small(sc, z, zs, dump);
+      pow_fixed<NSB>(y, yN, dump);
+      pow_fixed<NSC>(z, zN, dump);
+      double xa = zs;              // x^a * z^sc
+      int slot = 0;
+#pragma unroll
+      for (int aa = 0; aa <= NU0; ++aa) {
+        double col = xa * ysb;     // x^a y^(sb + NSB i) z^sc
+#pragma unroll
+        for (int i = 0; i < Sl::ncol(aa); ++i) {
+          double tt = col;
+#pragma unroll
+          for (int kk = 0; kk < Sl::nstep(aa, i); ++kk) {
+#pragma unroll
+            for (int m = 0; m < Sl::nmu_at(aa, i, kk); ++m) { acc[slot] = fma(buf[3 + m], tt, acc[slot]); ++slot; }
+            if (kk + 1 < Sl::nstep(aa, i)) tt *= zN;
+          }
+          if (i + 1 < Sl::ncol(aa)) col *= yN;
+        }
+        if (aa < NU0) xa *= x;
+      }
+    }
+  }
+  if (P > 1) {
+#pragma unroll
+    for (int s = 0; s < NSLOT; ++s)
+#pragma unroll
+      for (int o = NS; o < LPA; o <<= 1) acc[s] += __shfl_xor_sync(0xffffffffu, acc[s], o);
+  }
+  if (act && part == 0) {
+    const int *km = a.kmap + slice * NSLOT;
+    double *Mc = a.M + (atom - a.c0);
+#pragma unroll
+    for (int s = 0; s < NSLOT; ++s) {
+      const int k = km[s];
+      if (k >= 0) Mc[(long long)k * a.ldm] = acc[s];
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------ K3
+// d_ij = sum_mu [ f'_mu P_mu rhat + f_mu grad P_mu ],  P_mu(x,y,z) = sum_{abc} G_{mu,abc} x^a y^b z^c.
+// Phase B evaluates each lane's share of P_mu and its gradient by nested Horner sweeps (z innermost,
+// then y, then x); slot order (mu, a desc, i desc, k desc) -- kmapB on the host.
+template <int LEV, int NSB, int NSC, int P, bool ATOMIC>
+__global__ void __launch_bounds__(128) k_pairgrad_t(const PairArgs a) {
+  using St = Stair<LEV>;
+  using Sl = Slices<LEV, NSB, NSC>;
+  using Tl = Tile<LEV, NSB, NSC, P>;
+  constexpr int NMU = St::NMU, NS = Sl::NS, NSLOT = Sl::NSLOT, LPA = Tl::LPA, NA = Tl::NA, TN = Tl::TN;
+  constexpr int PD = Tl::PD3, ROW = Tl::ROW3;
+  extern __shared__ __align__(16) double csm[];
+  stage_coef(a, csm);
+  const int ncoef = (a.n_species * a.n_species * a.crow + 1) & ~1;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  double *tile = csm + ncoef + wib * Tl::WARP3;
+  double *dtile = tile + NA * ROW;                  // [128][4]
+  const int warp = blockIdx.x * (blockDim.x >> 5) + wib;
+  const int sa = lane / LPA, q = lane % LPA, slice = q % NS, part = q / NS, sb = slice % NSB, sc = slice / NSB;
+  const int atom = a.c0 + warp * NA + sa;
+  const bool act = atom < a.c1;
+  double g[NSLOT];
+  double xi = 0, yi = 0, zi = 0, ti = 0;
+  long long beg = 0;
+  int n_nb = 0;
+  if (act) {
+    const int *km = a.kmap + slice * NSLOT;
+    const double *Gc = a.G + (atom - a.c0);
+#pragma unroll
+    for (int s = 0; s < NSLOT; ++s) {
+      const int k = km[s];
+      g[s] = k >= 0 ? Gc[(long long)k * a.ldm] : 0.0;
+    }
+    load_pos4(a.pos4, atom, xi, yi, zi, ti);
+    beg = a.off[atom];
+    n_nb = (int)(a.off[atom + 1] - beg);
+  } else {
+#pragma unroll
+    for (int s = 0; s < NSLOT; ++s) g[s] = 0.0;
+  }
+  const int zi_s = (int)ti;
+  const double rc2 = a.r_cut * a.r_cut;
+  const int n_max = __reduce_max_sync(0xffffffffu, n_nb);
+  double Fx = 0, Fy = 0, Fz = 0, W[6] = {0, 0, 0, 0, 0, 0};
+  const int ka = (4 * lane) % TN;
+  double *mine = tile + sa * ROW;
+  for (int t0 = 0; t0 < n_max; t0 += TN) {
+    __syncwarp();
+    // ---- phase A
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int k = t0 + ka + u;
+      stage_pair<NMU, true, PD>(a, csm, k < n_nb, beg + k, xi, yi, zi, zi_s, rc2, mine + (ka + u) * PD);
+    }
+    __syncwarp();
+    // ---- phase B
+    const int kend = min(TN, n_max - t0);
+    for (int k0 = 0; k0 < kend; k0 += P) {
+      const int k = k0 + part;                      // < TN; slots past a row's end hold zeros
+      const double2 *src = reinterpret_cast<const double2 *>(mine + k * PD);
+      double buf[PD];
+#pragma unroll
+      for (int w = 0; w < PD / 2; ++w) { const double2 v = src[w]; buf[2 * w] = v.x; buf[2 * w + 1] = v.y; }
+      const double x = buf[0], y = buf[1], z = buf[2];
+      const double *f = buf + 3, *df = buf + 3 + NMU;
+      double dx = 0, dy = 0, dz = 0;
+      double ysb, dysb, zs, dzs, yN, dyN, zN, dzN;
+      pow_small(sb, y, ysb, dysb);
+      pow_small(sc, z, zs, dzs);
+      pow_fixed<NSB>(y, yN, dyN);
+      pow_fixed<NSC>(z, zN, dzN);
+      double radial_sum = 0.0;   // sum_mu f'_mu P_mu
+      int slot = 0;
+#pragma unroll
+      for (int m = 0; m < NMU; ++m) {
+        const int NUm = St::numax(m);
+        double V = 0, Vx = 0, VY = 0, Vw = 0;
+#pragma unroll
+        for (int aa = NUm; aa >= 0; --aa) {
+          double R = 0, RY = 0, Rw = 0;
+#pragma unroll
+          for (int i = (NUm - aa) / NSB; i >= 0; --i) {
+            double qv = 0, qw = 0;
+            const int kmax = (NUm - aa - NSB * i) / NSC;
+#pragma unroll
+            for (int kk = kmax; kk >= 0; --kk) {
+              if (kk == kmax) { qv = g[slot]; }
+              else { qw = (kk == kmax - 1) ? qv : fma(qw, zN, qv); qv = fma(qv, zN, g[slot]); }
+              ++slot;
+            }
+            if (i == (NUm - aa) / NSB) { R = qv; Rw = qw; }
+            else { RY = (i == (NUm - aa) / NSB - 1) ? R : fma(RY, yN, R); R = fma(R, yN, qv); Rw = fma(Rw, yN, qw); }
+          }
+          if (aa == NUm) { V = R; VY = RY; Vw = Rw; }
+          else { Vx = (aa == NUm - 1) ? V : fma(Vx, x, V); V = fma(V, x, R); VY = fma(VY, x, RY); Vw = fma(Vw, x, Rw); }
+        }
+        // P = ysb zs V ; Px = ysb zs Vx ; Py = zs (dysb V + ysb dyN VY) ; Pz = ysb (dzs V + zs dzN Vw)
+        const double yz = ysb * zs;
+        radial_sum = fma(df[m], yz * V, radial_sum);
+        dx = fma(f[m], yz * Vx, dx);
+        dy = fma(f[m], zs * fma(dysb, V, ysb * dyN * VY), dy);
+        dz = fma(f[m], ysb * fma(dzs, V, zs * dzN * Vw), dz);
+      }
+      const double r2 = x * x + y * y + z * z;
+      const double rs = r2 > 0.0 ? radial_sum * rsqrt(r2) : 0.0;
+      dx = fma(rs, x, dx); dy = fma(rs, y, dy); dz = fma(rs, z, dz);
+      if (NS > 1) {
+#pragma unroll
+        for (int o = 1; o < NS; o <<= 1) {
+          dx += __shfl_xor_sync(0xffffffffu, dx, o);
+          dy += __shfl_xor_sync(0xffffffffu, dy, o);
+          dz += __shfl_xor_sync(0xffffffffu, dz, o);
+        }
+      }
+      if (slice == 0) {
+        double2 *o = reinterpret_cast<double2 *>(dtile + (sa * TN + k) * 4);
+        o[0] = make_double2(dx, dy);
+        o[1] = make_double2(dz, 0.0);
+      }
+    }
+    __syncwarp();
+    // ---- phase C
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int kl = ka + u, k = t0 + kl;
+      if (k < n_nb && kl < kend) {
+        const double2 *dd = reinterpret_cast<const double2 *>(dtile + (sa * TN + kl) * 4);
+        const double2 d0 = dd[0], d1 = dd[1];
+        const double dx = d0.x, dy = d0.y, dz = d1.x;
+        const double2 *xy = reinterpret_cast<const double2 *>(mine + kl * PD);
+        const double2 p0 = xy[0], p1 = xy[1];
+        const double x = p0.x, y = p0.y, z = p1.x;
+        const long long p = beg + k;
+        if (ATOMIC) {
+          if (dx != 0.0 || dy != 0.0 || dz != 0.0) {
+            const int j = a.idx[p];
+            atomicAdd(a.F + 3 * (size_t)j, -dx);
+            atomicAdd(a.F + 3 * (size_t)j + 1, -dy);
+            atomicAdd(a.F + 3 * (size_t)j + 2, -dz);
+          }
+          Fx += dx; Fy += dy; Fz += dz;
+        } else {
+          double2 *o = reinterpret_cast<double2 *>(a.d4) + 2 * (size_t)p;
+          o[0] = d0;
+          o[1] = make_double2(dz, 0.0);
+        }
+        W[0] = fma(-x, dx, W[0]); W[1] = fma(-y, dy, W[1]); W[2] = fma(-z, dz, W[2]);
+        W[3] = fma(-x, dy, W[3]); W[4] = fma(-x, dz, W[4]); W[5] = fma(-y, dz, W[5]);
+      }
+    }
+  }
+  if (ATOMIC) {
+#pragma unroll
+    for (int o = 1; o < LPA; o <<= 1) {
+      Fx += __shfl_xor_sync(0xffffffffu, Fx, o);
+      Fy += __shfl_xor_sync(0xffffffffu, Fy, o);
+      Fz += __shfl_xor_sync(0xffffffffu, Fz, o);
+    }
+    if (act && q == 0) {
+      atomicAdd(a.F + 3 * (size_t)atom, Fx);
+      atomicAdd(a.F + 3 * (size_t)atom + 1, Fy);
+      atomicAdd(a.F + 3 * (size_t)atom + 2, Fz);
+    }
+  }
+  // virial partial of this block, fixed reduction order (deterministic)
+  __shared__ double wsm[4][6];
+#pragma unroll
+  for (int c = 0; c < 6; ++c) {
+    double v = W[c];
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (lane == 0) wsm[wib][c] = v;
+  }
+  __syncthreads();
+  if (threadIdx.x < 6) {
+    double v = 0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) v += wsm[w][threadIdx.x];
+    a.wpart[(size_t)blockIdx.x * 8 + threadIdx.x] = v;
+  }
+}
+
+}  // namespace mtpb
