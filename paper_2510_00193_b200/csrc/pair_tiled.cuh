@@ -33,15 +33,30 @@ struct Tile {
   static constexpr int WARP3 = NA * ROW3 + 128 * 4;      // + d_ij of the tile (x y z pad)
 };
 
+__device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
+// Neighbour indices of the four pairs a lane stages in the tile starting at neighbour t0 (-1: past the row's
+// end), fetched one tile ahead; once they have arrived, the positions (and shifts) they point to are pulled
+// into L1 so that the next phase A finds them there.
+__device__ __forceinline__ void fetch_idx(const PairArgs &a, long long beg, int n_nb, int k0, int (&j)[4]) {
+#pragma unroll
+  for (int u = 0; u < 4; ++u) j[u] = (k0 + u < n_nb) ? __ldg(a.idx + beg + k0 + u) : -1;
+}
+__device__ __forceinline__ void prefetch_pairs(const PairArgs &a, long long beg, int k0, const int (&j)[4]) {
+#pragma unroll
+  for (int u = 0; u < 4; ++u)
+    if (j[u] >= 0) prefetch_l1(a.pos4 + 4 * (size_t)j[u]);
+  if (a.shift && j[0] >= 0) prefetch_l1(a.shift + 3 * (beg + k0));
+}
+
 // Phase A for one pair: geometry + radial functions; writes PD doubles (zeros when the pair does not contribute).
 template <int NMU, bool DERIV, int PD>
-__device__ __forceinline__ void stage_pair(const PairArgs &a, const double *__restrict__ csm, bool valid, long long p,
+__device__ __forceinline__ void stage_pair(const PairArgs &a, const double *__restrict__ csm, int j, long long p,
                                            double xi, double yi, double zi, int zi_s, double rc2, double *__restrict__ out) {
   double x = 0.0, y = 0.0, z = 0.0, f[NMU], df[NMU];
 #pragma unroll
   for (int m = 0; m < NMU; ++m) { f[m] = 0.0; df[m] = 0.0; }
-  if (valid) {
-    const int j = a.idx[p];
+  if (j >= 0) {
     double xj, yj, zj, tj;
     load_pos4(a.pos4, j, xj, yj, zj, tj);
     pair_vector(a, p, xi, yi, zi, xj, yj, zj, x, y, z);
@@ -99,13 +114,18 @@ __global__ void __launch_bounds__(128) k_moments_t(const PairArgs a) {
   for (int s = 0; s < NSLOT; ++s) acc[s] = 0.0;
   const int ka = (4 * lane) % TN;                  // phase A: this lane stages neighbours t0 + ka .. + 3 of atom slot sa
   double *mine = tile + sa * ROW;
+  int jn[4];
+  fetch_idx(a, beg, n_nb, ka, jn);
   for (int t0 = 0; t0 < n_max; t0 += TN) {
+    int jc[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) jc[u] = jn[u];
+    fetch_idx(a, beg, n_nb, t0 + TN + ka, jn);
     __syncwarp();
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const int k = t0 + ka + u;
-      stage_pair<NMU, false, PD>(a, csm, k < n_nb, beg + k, xi, yi, zi, zi_s, rc2, mine + (ka + u) * PD);
-    }
+    for (int u = 0; u < 4; ++u)
+      stage_pair<NMU, false, PD>(a, csm, jc[u], beg + t0 + ka + u, xi, yi, zi, zi_s, rc2, mine + (ka + u) * PD);
+    prefetch_pairs(a, beg, t0 + TN + ka, jn);
     __syncwarp();
     const int kend = min(TN, n_max - t0);
     for (int k = part; k < kend; k += P) {
@@ -202,14 +222,19 @@ __global__ void __launch_bounds__(128) k_pairgrad_t(const PairArgs a) {
   double Fx = 0, Fy = 0, Fz = 0, W[6] = {0, 0, 0, 0, 0, 0};
   const int ka = (4 * lane) % TN;
   double *mine = tile + sa * ROW;
+  int jn[4];
+  fetch_idx(a, beg, n_nb, ka, jn);
   for (int t0 = 0; t0 < n_max; t0 += TN) {
+    int jc[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) jc[u] = jn[u];
+    fetch_idx(a, beg, n_nb, t0 + TN + ka, jn);
     __syncwarp();
     // ---- phase A
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const int k = t0 + ka + u;
-      stage_pair<NMU, true, PD>(a, csm, k < n_nb, beg + k, xi, yi, zi, zi_s, rc2, mine + (ka + u) * PD);
-    }
+    for (int u = 0; u < 4; ++u)
+      stage_pair<NMU, true, PD>(a, csm, jc[u], beg + t0 + ka + u, xi, yi, zi, zi_s, rc2, mine + (ka + u) * PD);
+    prefetch_pairs(a, beg, t0 + TN + ka, jn);
     __syncwarp();
     // ---- phase B
     const int kend = min(TN, n_max - t0);
@@ -270,10 +295,10 @@ __global__ void __launch_bounds__(128) k_pairgrad_t(const PairArgs a) {
           dz += __shfl_xor_sync(0xffffffffu, dz, o);
         }
       }
-      if (slice == 0) {
-        double2 *o = reinterpret_cast<double2 *>(dtile + (sa * TN + k) * 4);
-        o[0] = make_double2(dx, dy);
-        o[1] = make_double2(dz, 0.0);
+      if (slice == 0) {                           // d of the tile: three arrays [TN][NA], conflict-free here
+        dtile[k * NA + sa] = dx;
+        dtile[128 + k * NA + sa] = dy;
+        dtile[256 + k * NA + sa] = dz;
       }
     }
     __syncwarp();
@@ -282,16 +307,14 @@ __global__ void __launch_bounds__(128) k_pairgrad_t(const PairArgs a) {
     for (int u = 0; u < 4; ++u) {
       const int kl = ka + u, k = t0 + kl;
       if (k < n_nb && kl < kend) {
-        const double2 *dd = reinterpret_cast<const double2 *>(dtile + (sa * TN + kl) * 4);
-        const double2 d0 = dd[0], d1 = dd[1];
-        const double dx = d0.x, dy = d0.y, dz = d1.x;
+        const double dx = dtile[kl * NA + sa], dy = dtile[128 + kl * NA + sa], dz = dtile[256 + kl * NA + sa];
         const double2 *xy = reinterpret_cast<const double2 *>(mine + kl * PD);
         const double2 p0 = xy[0], p1 = xy[1];
         const double x = p0.x, y = p0.y, z = p1.x;
         const long long p = beg + k;
         if (ATOMIC) {
           if (dx != 0.0 || dy != 0.0 || dz != 0.0) {
-            const int j = a.idx[p];
+            const int j = jc[u];
             atomicAdd(a.F + 3 * (size_t)j, -dx);
             atomicAdd(a.F + 3 * (size_t)j + 1, -dy);
             atomicAdd(a.F + 3 * (size_t)j + 2, -dz);
@@ -299,7 +322,7 @@ __global__ void __launch_bounds__(128) k_pairgrad_t(const PairArgs a) {
           Fx += dx; Fy += dy; Fz += dz;
         } else {
           double2 *o = reinterpret_cast<double2 *>(a.d4) + 2 * (size_t)p;
-          o[0] = d0;
+          o[0] = make_double2(dx, dy);
           o[1] = make_double2(dz, 0.0);
         }
         W[0] = fma(-x, dx, W[0]); W[1] = fma(-y, dy, W[1]); W[2] = fma(-z, dz, W[2]);
