@@ -248,13 +248,14 @@ extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
       return fail(nullptr, MTP_EUNSUP, "contraction tree does not fit in shared memory (one atom's node values and adjoints > 225 KB)");
     }
   }
-  // radial coefficients: rows (z_i, z_j) padded to the level's n_mu, odd row stride (bank spread)
-  const int nmu_lev = rt_nmu(h->pl->lev);
-  h->crow = nmu_lev * h->nb + 1;
+  // radial coefficients: blocks (z_i, z_j) laid out [beta][NMUP], NMUP = the level's n_mu rounded up to even
+  // (16-byte pairs); +2 doubles per block spread the blocks over the banks
+  const int nmu_lev = rt_nmu(h->pl->lev), nmup = (nmu_lev + 1) & ~1;
+  h->crow = nmup * h->nb + 2;
   std::vector<double> coef((size_t)h->S * h->S * h->crow, 0.0);
   for (int r = 0; r < h->S * h->S; ++r)
     for (int m = 0; m < h->nmu && m < nmu_lev; ++m)
-      for (int b = 0; b < h->nb; ++b) coef[(size_t)r * h->crow + m * h->nb + b] = p->c[((size_t)r * h->nmu + m) * h->nb + b];
+      for (int b = 0; b < h->nb; ++b) coef[(size_t)r * h->crow + b * nmup + m] = p->c[((size_t)r * h->nmu + m) * h->nb + b];
   std::vector<int> kf, kb;
   build_kmaps(*h->pl, p->n_basic, p->basic, kf, kb);
   cudaError_t e = cudaSuccess;

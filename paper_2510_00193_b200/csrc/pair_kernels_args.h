@@ -8,7 +8,7 @@ struct PairArgs {
   const long long *off;      // [N+1]
   const int *idx;            // [nnz]
   const signed char *shift;  // [nnz][3] or null (minimum image)
-  const double *coef;        // [S*S][crow] radial coefficients, row = (z_i*S + z_j), [mu][beta]
+  const double *coef;        // [S*S][crow] radial coefficients, block = (z_i*S + z_j), [beta][NMUP]
   const int *kmap;           // [NS][NSLOT] slot -> packed component of the table, or -1
   double *M;                 // K1 out: [n_basic][ldm], column = atom - c0
   const double *G;           // K3 in : [n_basic][ldm]

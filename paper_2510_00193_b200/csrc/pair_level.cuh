@@ -16,7 +16,10 @@ struct PairLevelImpl {
     const int per_cta = Tile<LEV, NSB, NSC, P>::NA * kWarps;
     return (n_atoms + per_cta - 1) / per_cta;
   }
-  static size_t coef_doubles(const PairArgs &a) { return (size_t)((a.n_species * a.n_species * a.crow + 1) & ~1); }
+  // shared-memory prologue: coefficients + slot map (pair_kernels.cuh stage_coef)
+  static size_t coef_doubles(const PairArgs &a) {
+    return (size_t)(a.n_species * a.n_species * a.crow) + (size_t)((Sl::NS * Sl::NSLOT + 3) / 4) * 2;
+  }
   template <class K>
   static cudaError_t prep(K kernel, size_t smem) {
     return smem > 48 * 1024 ? cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) : cudaSuccess;
@@ -24,18 +27,20 @@ struct PairLevelImpl {
   template <int P>
   static cudaError_t moments_p(const PairArgs &a, int n, cudaStream_t st) {
     const size_t smem = 8 * (coef_doubles(a) + (size_t)kWarps * Tile<LEV, NSB, NSC, P>::WARP1);
-    cudaError_t e = prep(k_moments_t<LEV, NSB, NSC, P>, smem);
+    cudaError_t e = a.nb == 8 ? prep(k_moments_t<LEV, NSB, NSC, P, 8>, smem) : prep(k_moments_t<LEV, NSB, NSC, P, 0>, smem);
     if (e != cudaSuccess) return e;
-    k_moments_t<LEV, NSB, NSC, P><<<grid_for<P>(n), 32 * kWarps, smem, st>>>(a);
+    if (a.nb == 8) k_moments_t<LEV, NSB, NSC, P, 8><<<grid_for<P>(n), 32 * kWarps, smem, st>>>(a);
+    else k_moments_t<LEV, NSB, NSC, P, 0><<<grid_for<P>(n), 32 * kWarps, smem, st>>>(a);
     count_launch();
     return cudaGetLastError();
   }
   template <int P, bool ATOMIC>
   static cudaError_t pairgrad_p(const PairArgs &a, int n, cudaStream_t st) {
     const size_t smem = 8 * (coef_doubles(a) + (size_t)kWarps * Tile<LEV, NSB, NSC, P>::WARP3);
-    cudaError_t e = prep(k_pairgrad_t<LEV, NSB, NSC, P, ATOMIC>, smem);
+    cudaError_t e = a.nb == 8 ? prep(k_pairgrad_t<LEV, NSB, NSC, P, ATOMIC, 8>, smem) : prep(k_pairgrad_t<LEV, NSB, NSC, P, ATOMIC, 0>, smem);
     if (e != cudaSuccess) return e;
-    k_pairgrad_t<LEV, NSB, NSC, P, ATOMIC><<<grid_for<P>(n), 32 * kWarps, smem, st>>>(a);
+    if (a.nb == 8) k_pairgrad_t<LEV, NSB, NSC, P, ATOMIC, 8><<<grid_for<P>(n), 32 * kWarps, smem, st>>>(a);
+    else k_pairgrad_t<LEV, NSB, NSC, P, ATOMIC, 0><<<grid_for<P>(n), 32 * kWarps, smem, st>>>(a);
     count_launch();
     return cudaGetLastError();
   }

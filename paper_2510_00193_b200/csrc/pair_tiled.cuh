@@ -31,6 +31,8 @@ struct Tile {
   static constexpr int ROW1 = TN * PD1 + 2, ROW3 = TN * PD3 + 2;   // +16 B: rows of different atoms spread over the banks
   static constexpr int WARP1 = NA * ROW1;                // doubles per warp
   static constexpr int WARP3 = NA * ROW3 + 128 * 4;      // + d_ij of the tile (x y z pad)
+  // CTAs per SM the register allocation aims at: small per-lane slot counts leave room for more warps
+  static constexpr int MINB1 = Sl::NSLOT <= 30 ? 4 : (Sl::NSLOT <= 56 ? 3 : 2), MINB3 = Sl::NSLOT <= 56 ? 3 : 2;
 };
 
 __device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
@@ -49,22 +51,30 @@ __device__ __forceinline__ void prefetch_pairs(const PairArgs &a, long long beg,
   if (a.shift && j[0] >= 0) prefetch_l1(a.shift + 3 * (beg + k0));
 }
 
-// Phase A for one pair: geometry + radial functions; writes PD doubles (zeros when the pair does not contribute).
-template <int NMU, bool DERIV, int PD>
-__device__ __forceinline__ void stage_pair(const PairArgs &a, const double *__restrict__ csm, int j, long long p,
-                                           double xi, double yi, double zi, int zi_s, double rc2, double *__restrict__ out) {
-  double x = 0.0, y = 0.0, z = 0.0, f[NMU], df[NMU];
-#pragma unroll
-  for (int m = 0; m < NMU; ++m) { f[m] = 0.0; df[m] = 0.0; }
+// Phase A, step 1: the pair vector of one staged pair (loads issued for all four pairs before any is used).
+struct PairGeo { double x, y, z; int zj; };
+__device__ __forceinline__ PairGeo load_pair(const PairArgs &a, int j, long long p, double xi, double yi, double zi) {
+  PairGeo g{0.0, 0.0, 0.0, -1};
   if (j >= 0) {
     double xj, yj, zj, tj;
     load_pos4(a.pos4, j, xj, yj, zj, tj);
-    pair_vector(a, p, xi, yi, zi, xj, yj, zj, x, y, z);
-    const double r2 = x * x + y * y + z * z;
-    if (r2 < rc2) {
-      const double r = r2 * rsqrt(r2);
-      radial<NMU, DERIV>(csm + (zi_s * a.n_species + (int)tj) * a.crow, a.nb, r, a.r_min, a.r_cut, f, df);
-    }
+    pair_vector(a, p, xi, yi, zi, xj, yj, zj, g.x, g.y, g.z);
+    g.zj = (int)tj;
+  }
+  return g;
+}
+// Phase A, step 2: radial functions; writes PD doubles (zeros when the pair does not contribute).
+template <int NMU, bool DERIV, int PD, int NB>
+__device__ __forceinline__ void stage_pair(const PairArgs &a, const double *__restrict__ csm, const PairGeo &g, int zi_s,
+                                           double rc2, double *__restrict__ out) {
+  double x = 0.0, y = 0.0, z = 0.0, f[NMU], df[NMU];
+#pragma unroll
+  for (int m = 0; m < NMU; ++m) { f[m] = 0.0; df[m] = 0.0; }
+  const double r2 = g.x * g.x + g.y * g.y + g.z * g.z;
+  if (g.zj >= 0 && r2 < rc2) {
+    x = g.x; y = g.y; z = g.z;
+    const double r = r2 * rsqrt(r2);
+    radial<NMU, DERIV, NB>(csm + (zi_s * a.n_species + g.zj) * a.crow, a.nb, r, a.r_min, a.r_cut, f, df);
   }
   double2 *o = reinterpret_cast<double2 *>(out);
   double buf[PD];
@@ -82,16 +92,16 @@ __device__ __forceinline__ void stage_pair(const PairArgs &a, const double *__re
 }
 
 // ------------------------------------------------------------------------------ K1
-template <int LEV, int NSB, int NSC, int P>
-__global__ void __launch_bounds__(128) k_moments_t(const PairArgs a) {
+template <int LEV, int NSB, int NSC, int P, int NB>
+__global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB1) k_moments_t(const PairArgs a) {
   using St = Stair<LEV>;
   using Sl = Slices<LEV, NSB, NSC>;
   using Tl = Tile<LEV, NSB, NSC, P>;
   constexpr int NMU = St::NMU, NU0 = St::NU0, NS = Sl::NS, NSLOT = Sl::NSLOT, LPA = Tl::LPA, NA = Tl::NA, TN = Tl::TN;
   constexpr int PD = Tl::PD1, ROW = Tl::ROW1;
   extern __shared__ __align__(16) double csm[];
-  stage_coef(a, csm);
-  const int ncoef = (a.n_species * a.n_species * a.crow + 1) & ~1;
+  const int ncoef = stage_coef(a, csm, NS * NSLOT);
+  const int *kmsm = reinterpret_cast<const int *>(csm + a.n_species * a.n_species * a.crow);
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   double *tile = csm + ncoef + wib * Tl::WARP1;
   const int warp = blockIdx.x * (blockDim.x >> 5) + wib;
@@ -122,9 +132,11 @@ __global__ void __launch_bounds__(128) k_moments_t(const PairArgs a) {
     for (int u = 0; u < 4; ++u) jc[u] = jn[u];
     fetch_idx(a, beg, n_nb, t0 + TN + ka, jn);
     __syncwarp();
+    PairGeo geo[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u)
-      stage_pair<NMU, false, PD>(a, csm, jc[u], beg + t0 + ka + u, xi, yi, zi, zi_s, rc2, mine + (ka + u) * PD);
+    for (int u = 0; u < 4; ++u) geo[u] = load_pair(a, jc[u], beg + t0 + ka + u, xi, yi, zi);
+#pragma unroll
+    for (int u = 0; u < 4; ++u) stage_pair<NMU, false, PD, NB>(a, csm, geo[u], zi_s, rc2, mine + (ka + u) * PD);
     prefetch_pairs(a, beg, t0 + TN + ka, jn);
     __syncwarp();
     const int kend = min(TN, n_max - t0);
@@ -166,7 +178,7 @@ __global__ void __launch_bounds__(128) k_moments_t(const PairArgs a) {
       for (int o = NS; o < LPA; o <<= 1) acc[s] += __shfl_xor_sync(0xffffffffu, acc[s], o);
   }
   if (act && part == 0) {
-    const int *km = a.kmap + slice * NSLOT;
+    const int *km = kmsm + slice * NSLOT;
     double *Mc = a.M + (atom - a.c0);
 #pragma unroll
     for (int s = 0; s < NSLOT; ++s) {
@@ -180,16 +192,16 @@ __global__ void __launch_bounds__(128) k_moments_t(const PairArgs a) {
 // d_ij = sum_mu [ f'_mu P_mu rhat + f_mu grad P_mu ],  P_mu(x,y,z) = sum_{abc} G_{mu,abc} x^a y^b z^c.
 // Phase B evaluates each lane's share of P_mu and its gradient by nested Horner sweeps (z innermost,
 // then y, then x); slot order (mu, a desc, i desc, k desc) -- kmapB on the host.
-template <int LEV, int NSB, int NSC, int P, bool ATOMIC>
-__global__ void __launch_bounds__(128) k_pairgrad_t(const PairArgs a) {
+template <int LEV, int NSB, int NSC, int P, bool ATOMIC, int NB>
+__global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB3) k_pairgrad_t(const PairArgs a) {
   using St = Stair<LEV>;
   using Sl = Slices<LEV, NSB, NSC>;
   using Tl = Tile<LEV, NSB, NSC, P>;
   constexpr int NMU = St::NMU, NS = Sl::NS, NSLOT = Sl::NSLOT, LPA = Tl::LPA, NA = Tl::NA, TN = Tl::TN;
   constexpr int PD = Tl::PD3, ROW = Tl::ROW3;
   extern __shared__ __align__(16) double csm[];
-  stage_coef(a, csm);
-  const int ncoef = (a.n_species * a.n_species * a.crow + 1) & ~1;
+  const int ncoef = stage_coef(a, csm, NS * NSLOT);
+  const int *kmsm = reinterpret_cast<const int *>(csm + a.n_species * a.n_species * a.crow);
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   double *tile = csm + ncoef + wib * Tl::WARP3;
   double *dtile = tile + NA * ROW;                  // [128][4]
@@ -202,7 +214,7 @@ __global__ void __launch_bounds__(128) k_pairgrad_t(const PairArgs a) {
   long long beg = 0;
   int n_nb = 0;
   if (act) {
-    const int *km = a.kmap + slice * NSLOT;
+    const int *km = kmsm + slice * NSLOT;
     const double *Gc = a.G + (atom - a.c0);
 #pragma unroll
     for (int s = 0; s < NSLOT; ++s) {
@@ -231,9 +243,11 @@ __global__ void __launch_bounds__(128) k_pairgrad_t(const PairArgs a) {
     fetch_idx(a, beg, n_nb, t0 + TN + ka, jn);
     __syncwarp();
     // ---- phase A
+    PairGeo geo[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u)
-      stage_pair<NMU, true, PD>(a, csm, jc[u], beg + t0 + ka + u, xi, yi, zi, zi_s, rc2, mine + (ka + u) * PD);
+    for (int u = 0; u < 4; ++u) geo[u] = load_pair(a, jc[u], beg + t0 + ka + u, xi, yi, zi);
+#pragma unroll
+    for (int u = 0; u < 4; ++u) stage_pair<NMU, true, PD, NB>(a, csm, geo[u], zi_s, rc2, mine + (ka + u) * PD);
     prefetch_pairs(a, beg, t0 + TN + ka, jn);
     __syncwarp();
     // ---- phase B
