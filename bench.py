@@ -92,6 +92,22 @@ class ClockSampler:
         return out
 
 
+def max_over_ranks(x, dist, device):
+    """Time of the slowest rank (the contract's max-over-ranks); identity for a single process."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(n_atoms_per_rank, steps, seconds_local, world, dist, device):
+    """Weak scaling over replicas: every rank evaluates its own n_atoms_per_rank atoms per step;
+    value = atoms all ranks processed / time of the slowest rank."""
+    return world * n_atoms_per_rank * steps / max_over_ranks(seconds_local, dist, device)
+
+
 def build_workload(config, cells, seed_shift=0):
     from workloads import make_workload, CONFIGS
     import paper_2510_00193_b200 as lib
@@ -207,11 +223,8 @@ def run_ours(args):
     launches = lib.launch_count() - n0
     ms = e0.elapsed_time(e1)
     prof = pot.profile_read()
-    if dist is not None:
-        tt = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms = float(tt.item())
-    value = world * w.n_atoms * args.steps / (ms * 1e-3)
+    ms = max_over_ranks(ms, dist, dev)
+    value = whole_job_rate(w.n_atoms, args.steps, ms * 1e-3, world, None, dev)
 
     # ---- end to end through the host-buffer entry point (pinned inputs, results read back)
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
@@ -225,13 +238,9 @@ def run_ours(args):
         pot.compute_host(hp["pos"], hp["types"], w.box, hp["off"], hp["idx"], hp["shift"], hp["rev"], out=hout)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    if dist is not None:
-        tt = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e_s = float(tt.item())
     h2d = sum(hp[k].nbytes for k in hp)
     d2h = sum(hout[k].nbytes for k in hout)
-    e2e_value = world * w.n_atoms * e2e_steps / e2e_s
+    e2e_value = whole_job_rate(w.n_atoms, e2e_steps, e2e_s, world, dist, dev)
     pot.profile_read()
 
     if rank != 0:
