@@ -304,12 +304,13 @@ namespace {
 struct Plan {
   int64_t N = 0, nnz = 0, C = 0, ldm = 0;
   int n_chunks = 0, P = 1, atomic = 0, grid_chunk = 0, AL = 0, AR = 1, elide = 1;
-  size_t o_pos4 = 0, o_Ei = 0, o_M = 0, o_G = 0, o_wpart = 0, o_d4 = 0, o_B = 0, o_part = 0, o_red = 0, total = 0;
+  size_t o_pos4 = 0, o_Ei = 0, o_M = 0, o_G = 0, o_wpart = 0, o_d4 = 0, o_B = 0, o_part = 0, o_red = 0, o_idxp = 0, total = 0;
 };
 size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
 int make_plan(const mtp_handle *h, int64_t N, int64_t nnz, int want_grade, int has_rev, Plan &pl) {
-  if (N < 0 || nnz < 0 || N > 2147483000LL) return MTP_EINVAL;
+  if (N < 0 || nnz < 0) return MTP_EINVAL;
+  if (N > (1LL << 27)) return MTP_EUNSUP;      // neighbour words carry 27 index bits (pair_kernels.cuh)
   pl.N = N; pl.nnz = nnz;
   int64_t C = h->chunk_atoms;
   if (C <= 0) {   // automatic: many waves per launch (no tail), M + G scratch (16 B x n_basic per atom) <= 1 GB
@@ -338,6 +339,7 @@ int make_plan(const mtp_handle *h, int64_t N, int64_t nnz, int want_grade, int h
   pl.o_M = o; o = align_up(o + (size_t)h->n_basic * pl.ldm * 8);
   pl.o_G = o; o = align_up(o + (size_t)h->n_basic * pl.ldm * 8);
   pl.o_red = o; o = align_up(o + 256 * 8 * 8);
+  pl.o_idxp = o; o = align_up(o + (size_t)nnz * 4);          // packed neighbour words (used when shifts are given)
   pl.o_wpart = o; o = align_up(o + (size_t)std::max(1, pl.n_chunks) * pl.grid_chunk * 64);
   pl.o_d4 = o; if (!want_grade && !pl.atomic) o = align_up(o + (size_t)nnz * 32);
   pl.o_B = o; if (want_grade) o = align_up(o + (size_t)C * h->n_basis * 8);
@@ -368,9 +370,10 @@ int box_setup(mtp_handle *h, const double *box, bool need_minimg, double r_cut, 
   return MTP_OK;
 }
 
+// idx: the packed neighbour words when shifts were given (launch_pack_pairs), else the caller's plain indices
 void fill_pair_args(const mtp_handle *h, PairArgs &pa, const double *pos4, const int64_t *off, const int32_t *idx,
                     const int8_t *shift) {
-  pa.pos4 = pos4; pa.off = (const long long *)off; pa.idx = idx; pa.shift = (const signed char *)shift;
+  pa.pos4 = pos4; pa.off = (const long long *)off; pa.idx = idx;
   pa.coef = h->d_coef; pa.n_species = h->S; pa.nb = h->nb; pa.crow = h->crow;
   pa.minimg = shift ? 0 : 1; pa.r_min = h->r_min; pa.r_cut = h->r_cut;
   pa.M = nullptr; pa.G = nullptr; pa.d4 = nullptr; pa.F = nullptr; pa.wpart = nullptr; pa.kmap = nullptr;
@@ -434,7 +437,12 @@ extern "C" int mtp_compute(mtp_handle *h, int64_t N, const double *d_pos, const 
   CU(h, launch_pack(d_pos, d_type, (int)N, pos4, st));
   CU(h, launch_zero(wpart, (long long)pl.n_chunks * pl.grid_chunk * 8, st));
   if (pl.atomic) CU(h, launch_zero(d_F, 3 * N, st));
-  fill_pair_args(h, pa, pos4, d_off, d_idx, d_shift);
+  const int32_t *idxp = d_idx;
+  if (d_shift && nnz > 0) {
+    CU(h, launch_pack_pairs(d_idx, (const signed char *)d_shift, nnz, (int *)(ws + pl.o_idxp), st));
+    idxp = (const int32_t *)(ws + pl.o_idxp);
+  }
+  fill_pair_args(h, pa, pos4, d_off, idxp, d_shift);
   pa.ldm = pl.ldm;
   TreeArgs ta;
   rc = fill_tree_args(h, ta, pos4, pl);
@@ -483,7 +491,12 @@ extern "C" int mtp_grade(mtp_handle *h, int64_t N, const double *d_pos, const in
   if (mode != 0 || d_Bsum) CU(h, launch_zero(Bsum, h->n_basis, st));
   if (N > 0) {
     CU(h, launch_pack(d_pos, d_type, (int)N, pos4, st));
-    fill_pair_args(h, pa, pos4, d_off, d_idx, d_shift);
+    const int32_t *idxp = d_idx;
+    if (d_shift && nnz > 0) {
+      CU(h, launch_pack_pairs(d_idx, (const signed char *)d_shift, nnz, (int *)(ws + pl.o_idxp), st));
+      idxp = (const int32_t *)(ws + pl.o_idxp);
+    }
+    fill_pair_args(h, pa, pos4, d_off, idxp, d_shift);
     pa.ldm = pl.ldm;
     TreeArgs ta;
     rc = fill_tree_args(h, ta, pos4, pl);
@@ -575,9 +588,22 @@ extern "C" int mtp_debug_moments(mtp_handle *h, int64_t N, const double *d_pos, 
   char *ws = (char *)d_ws + base;
   double *pos4 = (double *)(ws + pl.o_pos4), *Ei = (double *)(ws + pl.o_Ei), *M = (double *)(ws + pl.o_M), *G = (double *)(ws + pl.o_G);
   CU(h, launch_pack(d_pos, d_type, (int)N, pos4, st));
-  fill_pair_args(h, pa, pos4, d_off, d_idx, d_shift);
+  int *tmp_idxp = nullptr;                  // diagnostics only: this entry point has no nnz argument
+  if (d_shift) {
+    long long nnz = 0;
+    CU(h, cudaMemcpyAsync(&nnz, d_off + N, 8, cudaMemcpyDeviceToHost, st));
+    CU(h, cudaStreamSynchronize(st));
+    CU(h, cudaMalloc((void **)&tmp_idxp, (size_t)std::max<long long>(nnz, 1) * 4));
+    cudaError_t e = launch_pack_pairs(d_idx, (const signed char *)d_shift, nnz, tmp_idxp, st);
+    if (e != cudaSuccess) { cudaFree(tmp_idxp); return cuda_fail(h, e, "launch_pack_pairs"); }
+  }
+  fill_pair_args(h, pa, pos4, d_off, tmp_idxp ? tmp_idxp : d_idx, d_shift);
   pa.ldm = pl.ldm; pa.c0 = 0; pa.c1 = (int)N; pa.M = M; pa.kmap = h->d_kmapF;
-  CU(h, h->pl->moments(pa, pl.P, st));
+  {
+    cudaError_t e = h->pl->moments(pa, pl.P, st);
+    if (tmp_idxp) { cudaStreamSynchronize(st); cudaFree(tmp_idxp); }
+    if (e != cudaSuccess) return cuda_fail(h, e, "moments");
+  }
   TreeArgs ta;
   rc = fill_tree_args(h, ta, pos4, pl);
   if (rc != MTP_OK) return rc;

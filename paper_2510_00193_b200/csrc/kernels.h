@@ -50,6 +50,8 @@ const PairLevel *pair_level(int index);   // index into kLevels
 // ---- misc kernels (misc_kernels.cu)
 cudaError_t launch_pack(const double *pos, const int *type, int n, double *pos4, cudaStream_t st);
 cudaError_t launch_zero(double *p, long long n, cudaStream_t st);
+// out[p] = idx[p] | image_code(shift[p]) << 27
+cudaError_t launch_pack_pairs(const int *idx, const signed char *shift, long long nnz, int *out, cudaStream_t st);
 // F_k = sum_p d[p] - d[rev[p]] over row k (warp per atom, fixed order)
 cudaError_t launch_gather(const long long *off, const int *rev, const double *d4, int n, double *F, cudaStream_t st);
 // out[c] = sum_i in[i*stride + c] for c < ncomp <= 8, fixed order; scratch: 256 x 8 doubles (or null)

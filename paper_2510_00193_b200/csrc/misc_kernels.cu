@@ -5,6 +5,7 @@
 #include <atomic>
 
 #include "kernels.h"
+#include "pair_kernels.cuh"
 
 namespace mtpb {
 
@@ -20,6 +21,16 @@ __global__ void k_pack(const double *__restrict__ pos, const int *__restrict__ t
   double2 *o = reinterpret_cast<double2 *>(pos4) + 2 * (size_t)i;
   o[0] = make_double2(pos[3 * (size_t)i], pos[3 * (size_t)i + 1]);
   o[1] = make_double2(pos[3 * (size_t)i + 2], (double)type[i]);
+}
+
+// packed neighbour word j | code << 27 (pair_kernels.cuh): one 4-byte load per pair in K1 / K3 instead of
+// an index and three shift bytes, and the shift vector becomes a table lookup
+__global__ void k_pack_pairs(const int *__restrict__ idx, const signed char *__restrict__ shift, long long nnz,
+                             int *__restrict__ out) {
+  const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= nnz) return;
+  const int code = shift_code(shift[3 * p], shift[3 * p + 1], shift[3 * p + 2]);
+  out[p] = idx[p] | (code << kIdxBits);
 }
 
 __global__ void k_zero(double *p, long long n) {
@@ -100,6 +111,12 @@ __global__ void k_colsum_final(const double *__restrict__ part, int ns, int nb, 
 cudaError_t launch_pack(const double *pos, const int *type, int n, double *pos4, cudaStream_t st) {
   if (n <= 0) return cudaSuccess;
   k_pack<<<(n + 255) / 256, 256, 0, st>>>(pos, type, n, pos4);
+  count_launch();
+  return cudaGetLastError();
+}
+cudaError_t launch_pack_pairs(const int *idx, const signed char *shift, long long nnz, int *out, cudaStream_t st) {
+  if (nnz <= 0) return cudaSuccess;
+  k_pack_pairs<<<(unsigned)((nnz + 255) / 256), 256, 0, st>>>(idx, shift, nnz, out);
   count_launch();
   return cudaGetLastError();
 }

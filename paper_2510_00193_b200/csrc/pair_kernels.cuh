@@ -59,16 +59,22 @@ __device__ __forceinline__ void radial(const double *__restrict__ crow, int nb_r
   }
 }
 
-// a1: r_ij = x_j - x_i + s.H, or the minimum image when no shifts are given
-__device__ __forceinline__ void pair_vector(const PairArgs &a, long long p, double xi, double yi, double zi,
-                                            double xj, double yj, double zj, double &x, double &y, double &z) {
-  x = xj - xi; y = yj - yi; z = zj - zi;
-  if (a.shift) {
-    const double s0 = a.shift[3 * p], s1 = a.shift[3 * p + 1], s2 = a.shift[3 * p + 2];
-    x += s0 * a.H[0] + s1 * a.H[3] + s2 * a.H[6];
-    y += s0 * a.H[1] + s1 * a.H[4] + s2 * a.H[7];
-    z += s0 * a.H[2] + s1 * a.H[5] + s2 * a.H[8];
-  } else if (a.minimg) {
+// Packed neighbour word (k_pack_pairs): bits 0..26 the neighbour index j, bits 27..31 the image code:
+// 0 = no shift, c > 0 = shift number (c + 12) mod 27 of the list s = (q/9 - 1, (q/3)%3 - 1, q%3 - 1).
+constexpr int kIdxBits = 27;
+constexpr int kIdxMask = (1 << kIdxBits) - 1;
+__host__ __device__ __forceinline__ int shift_code(int s0, int s1, int s2) {
+  return ((s0 + 1) * 9 + (s1 + 1) * 3 + (s2 + 1) + 27 - 13) % 27;
+}
+
+// a1: r_ij = x_j - x_i + s.H (s.H from the 27-entry table in shared memory), then the minimum image
+// when the caller gave no shifts
+__device__ __forceinline__ void pair_vector(const PairArgs &a, const double *__restrict__ slut, int code, double xi,
+                                            double yi, double zi, double xj, double yj, double zj, double &x, double &y,
+                                            double &z) {
+  const double2 s01 = *reinterpret_cast<const double2 *>(slut + 4 * code);
+  x = (xj - xi) + s01.x; y = (yj - yi) + s01.y; z = (zj - zi) + slut[4 * code + 2];
+  if (a.minimg) {
     const double f0 = rint(x * a.Hi[0] + y * a.Hi[3] + z * a.Hi[6]);
     const double f1 = rint(x * a.Hi[1] + y * a.Hi[4] + z * a.Hi[7]);
     const double f2 = rint(x * a.Hi[2] + y * a.Hi[5] + z * a.Hi[8]);
@@ -84,15 +90,25 @@ __device__ __forceinline__ void load_pos4(const double *pos4, int j, double &x, 
   x = u.x; y = u.y; z = v.x; t = v.y;
 }
 
-// Shared-memory prologue of a pair kernel: radial coefficients, then the slot -> packed-component map
-// of this kernel (ints, after the coefficients); returns the number of doubles used.
+// Shared-memory prologue of a pair kernel: radial coefficients, the image-shift table s.H [27][4], then
+// the slot -> packed-component map of this kernel (ints); returns the number of doubles used.
+constexpr int kShiftLut = 27 * 4;
 __device__ __forceinline__ int stage_coef(const PairArgs &a, double *csm, int n_kmap) {
   const int n = a.n_species * a.n_species * a.crow;        // crow is even
   for (int i = threadIdx.x; i < n; i += blockDim.x) csm[i] = a.coef[i];
-  int *km = reinterpret_cast<int *>(csm + n);
+  if (threadIdx.x < 27) {
+    const int q = (threadIdx.x + 13) % 27;                  // code -> position in the {-1,0,1}^3 list
+    const double s0 = q / 9 - 1, s1 = (q / 3) % 3 - 1, s2 = q % 3 - 1;
+    double *o = csm + n + 4 * threadIdx.x;
+    o[0] = s0 * a.H[0] + s1 * a.H[3] + s2 * a.H[6];
+    o[1] = s0 * a.H[1] + s1 * a.H[4] + s2 * a.H[7];
+    o[2] = s0 * a.H[2] + s1 * a.H[5] + s2 * a.H[8];
+    o[3] = 0.0;
+  }
+  int *km = reinterpret_cast<int *>(csm + n + kShiftLut);
   for (int i = threadIdx.x; i < n_kmap; i += blockDim.x) km[i] = a.kmap[i];
   __syncthreads();
-  return n + ((n_kmap + 3) / 4) * 2;                        // keep 16-byte alignment
+  return n + kShiftLut + ((n_kmap + 3) / 4) * 2;            // keep 16-byte alignment
 }
 
 }  // namespace mtpb

@@ -6,8 +6,8 @@ namespace mtpb {
 struct PairArgs {
   const double *pos4;        // [N][4] x, y, z, species (as double)
   const long long *off;      // [N+1]
-  const int *idx;            // [nnz]
-  const signed char *shift;  // [nnz][3] or null (minimum image)
+  const int *idx;            // [nnz] packed neighbour words: j | code << 27 (k_pack_pairs); code 0 = no shift,
+                             // else 1 + the index of the image shift in {-1,0,1}^3 order with 0,0,0 moved to the front
   const double *coef;        // [S*S][crow] radial coefficients, block = (z_i*S + z_j), [beta][NMUP]
   const int *kmap;           // [NS][NSLOT] slot -> packed component of the table, or -1
   double *M;                 // K1 out: [n_basic][ldm], column = atom - c0

@@ -18,7 +18,7 @@ struct PairLevelImpl {
   }
   // shared-memory prologue: coefficients + slot map (pair_kernels.cuh stage_coef)
   static size_t coef_doubles(const PairArgs &a) {
-    return (size_t)(a.n_species * a.n_species * a.crow) + (size_t)((Sl::NS * Sl::NSLOT + 3) / 4) * 2;
+    return (size_t)(a.n_species * a.n_species * a.crow) + kShiftLut + (size_t)((Sl::NS * Sl::NSLOT + 3) / 4) * 2;
   }
   template <class K>
   static cudaError_t prep(K kernel, size_t smem) {

@@ -3,9 +3,11 @@
 //
 //   phase A  lanes = pairs.  A warp owns NA = 32/(NS*P) atoms whose CSR rows are contiguous; a tile
 //            holds neighbours [t*TN, (t+1)*TN) of each of them (TN = 4*NS*P, NA*TN = 128), four
-//            consecutive pairs per lane.  a1-a3 are done ONCE per pair here: coalesced loads of
-//            idx / shift, position gather, r, Chebyshev recurrence, f_mu (and f'_mu for K3); the
-//            result (x, y, z, f[, f']) goes to the warp's shared-memory tile.  Pairs past the end
+//            consecutive pairs per lane.  a1-a3 are done ONCE per pair here: r, Chebyshev recurrence,
+//            f_mu (and f'_mu for K3); the result (x, y, z, f[, f']) goes to the warp's shared-memory
+//            tile.  The packed neighbour words (index + image code) are fetched two tiles ahead into
+//            registers and the 32-byte position records they point to are copied one tile ahead into a
+//            double-buffered shared-memory staging area with cp.async, so phase A never waits on L2/HBM.  Pairs past the end
 //            of a row or with r >= R_cut are stored as zeros, so that phase B needs no predicates.
 //   phase B  lanes = (atom, slice, part) as in stair.h: every lane walks the TN staged pairs of its
 //            atom (parts split them) and does only the part that scales with n_basic -- monomials
@@ -29,37 +31,49 @@ struct Tile {
   static constexpr int PD1 = (3 + NMU + 1) & ~1;        // doubles per staged pair, K1: x y z f[NMU]
   static constexpr int PD3 = (3 + 2 * NMU + 1) & ~1;    // K3: x y z f[NMU] f'[NMU]
   static constexpr int ROW1 = TN * PD1 + 2, ROW3 = TN * PD3 + 2;   // +16 B: rows of different atoms spread over the banks
-  static constexpr int WARP1 = NA * ROW1;                // doubles per warp
-  static constexpr int WARP3 = NA * ROW3 + 128 * 4;      // + d_ij of the tile (x y z pad)
+  // staging per warp: two buffers of 128 position records (x y z species) + three of 128 neighbour words
+  static constexpr int STAGE = 2 * 128 * 4 + 3 * 128 / 2;
+  static constexpr int WARP1 = NA * ROW1 + STAGE;        // doubles per warp
+  static constexpr int WARP3 = NA * ROW3 + 128 * 4 + STAGE;   // + d_ij of the tile (three arrays of 128)
   // CTAs per SM the register allocation aims at: small per-lane slot counts leave room for more warps
   static constexpr int MINB1 = Sl::NSLOT <= 30 ? 4 : (Sl::NSLOT <= 56 ? 3 : 2), MINB3 = Sl::NSLOT <= 56 ? 3 : 2;
 };
 
-__device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
-
-// Neighbour indices of the four pairs a lane stages in the tile starting at neighbour t0 (-1: past the row's
-// end), fetched one tile ahead; once they have arrived, the positions (and shifts) they point to are pulled
-// into L1 so that the next phase A finds them there.
-__device__ __forceinline__ void fetch_idx(const PairArgs &a, long long beg, int n_nb, int k0, int (&j)[4]) {
+// Asynchronous copy (cp.async) of the packed neighbour words of the four pairs a lane stages in the tile
+// starting at neighbour k0 into its four staging slots; -1 (an impossible word) past the row's end.
+__device__ __forceinline__ void stage_words(const PairArgs &a, long long beg, int n_nb, int k0, int *slots) {
+  const unsigned s0 = (unsigned)__cvta_generic_to_shared(slots);
 #pragma unroll
-  for (int u = 0; u < 4; ++u) j[u] = (k0 + u < n_nb) ? __ldg(a.idx + beg + k0 + u) : -1;
+  for (int u = 0; u < 4; ++u) {
+    if (k0 + u < n_nb) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(s0 + 4 * u), "l"(a.idx + beg + k0 + u));
+    else slots[u] = -1;
+  }
 }
-__device__ __forceinline__ void prefetch_pairs(const PairArgs &a, long long beg, int k0, const int (&j)[4]) {
+// Asynchronous copy of the position records of those four neighbours into this lane's staging slots.
+__device__ __forceinline__ void stage_positions(const PairArgs &a, const int4 w, double *slots) {
+  const unsigned s0 = (unsigned)__cvta_generic_to_shared(slots);
+  const int ww[4] = {w.x, w.y, w.z, w.w};
 #pragma unroll
-  for (int u = 0; u < 4; ++u)
-    if (j[u] >= 0) prefetch_l1(a.pos4 + 4 * (size_t)j[u]);
-  if (a.shift && j[0] >= 0) prefetch_l1(a.shift + 3 * (beg + k0));
+  for (int u = 0; u < 4; ++u) {
+    if (ww[u] != -1) {
+      const double *g = a.pos4 + 4 * (size_t)(ww[u] & kIdxMask);
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s0 + 32 * u), "l"(g));
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s0 + 32 * u + 16), "l"(g + 2));
+    }
+  }
 }
+__device__ __forceinline__ void commit_copies() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void wait_positions() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-// Phase A, step 1: the pair vector of one staged pair (loads issued for all four pairs before any is used).
+// Phase A, step 1: the pair vector of one staged pair from its position record and image code.
 struct PairGeo { double x, y, z; int zj; };
-__device__ __forceinline__ PairGeo load_pair(const PairArgs &a, int j, long long p, double xi, double yi, double zi) {
+__device__ __forceinline__ PairGeo load_pair(const PairArgs &a, const double *__restrict__ slut, int w, const double *rec, 
+                                             double xi, double yi, double zi) {
   PairGeo g{0.0, 0.0, 0.0, -1};
-  if (j >= 0) {
-    double xj, yj, zj, tj;
-    load_pos4(a.pos4, j, xj, yj, zj, tj);
-    pair_vector(a, p, xi, yi, zi, xj, yj, zj, g.x, g.y, g.z);
-    g.zj = (int)tj;
+  if (w != -1) {
+    const double2 p0 = *reinterpret_cast<const double2 *>(rec), p1 = *reinterpret_cast<const double2 *>(rec + 2);
+    pair_vector(a, slut, (unsigned)w >> kIdxBits, xi, yi, zi, p0.x, p0.y, p1.x, g.x, g.y, g.z);
+    g.zj = (int)p1.y;
   }
   return g;
 }
@@ -101,7 +115,7 @@ __global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB1) k_moments_
   constexpr int PD = Tl::PD1, ROW = Tl::ROW1;
   extern __shared__ __align__(16) double csm[];
   const int ncoef = stage_coef(a, csm, NS * NSLOT);
-  const int *kmsm = reinterpret_cast<const int *>(csm + a.n_species * a.n_species * a.crow);
+  const int *kmsm = reinterpret_cast<const int *>(csm + a.n_species * a.n_species * a.crow + kShiftLut);
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   double *tile = csm + ncoef + wib * Tl::WARP1;
   const int warp = blockIdx.x * (blockDim.x >> 5) + wib;
@@ -124,20 +138,32 @@ __global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB1) k_moments_
   for (int s = 0; s < NSLOT; ++s) acc[s] = 0.0;
   const int ka = (4 * lane) % TN;                  // phase A: this lane stages neighbours t0 + ka .. + 3 of atom slot sa
   double *mine = tile + sa * ROW;
-  int jn[4];
-  fetch_idx(a, beg, n_nb, ka, jn);
+  const double *slut = csm + a.n_species * a.n_species * a.crow;
+  double *pst = tile + NA * ROW + 4 * (4 * lane);            // this lane's four position slots (buffer 0)
+  int *wst = reinterpret_cast<int *>(tile + NA * ROW + 2 * 512) + 4 * lane;   // its four word slots (buffer 0)
+  stage_words(a, beg, n_nb, ka, wst);
+  stage_words(a, beg, n_nb, TN + ka, wst + 128);
+  commit_copies();
+  wait_positions();
+  stage_positions(a, *reinterpret_cast<const int4 *>(wst), pst);
+  commit_copies();
+  int wb = 0, pb = 0;                                       // buffers holding the current tile's words / positions
   for (int t0 = 0; t0 < n_max; t0 += TN) {
-    int jc[4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u) jc[u] = jn[u];
-    fetch_idx(a, beg, n_nb, t0 + TN + ka, jn);
+    wait_positions();                                       // positions of this tile and words of the next have landed
+    const int4 jc4 = *reinterpret_cast<const int4 *>(wst + 128 * wb);
+    const int jc[4] = {jc4.x, jc4.y, jc4.z, jc4.w};
+    const double *rec = pst + 512 * pb;
+    const int wn = wb == 2 ? 0 : wb + 1, wnn = wn == 2 ? 0 : wn + 1;
+    stage_positions(a, *reinterpret_cast<const int4 *>(wst + 128 * wn), pst + 512 * (pb ^ 1));
+    stage_words(a, beg, n_nb, t0 + 2 * TN + ka, wst + 128 * wnn);
+    commit_copies();
+    wb = wn; pb ^= 1;
     __syncwarp();
     PairGeo geo[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) geo[u] = load_pair(a, jc[u], beg + t0 + ka + u, xi, yi, zi);
+    for (int u = 0; u < 4; ++u) geo[u] = load_pair(a, slut, jc[u], rec + 4 * u, xi, yi, zi);
 #pragma unroll
     for (int u = 0; u < 4; ++u) stage_pair<NMU, false, PD, NB>(a, csm, geo[u], zi_s, rc2, mine + (ka + u) * PD);
-    prefetch_pairs(a, beg, t0 + TN + ka, jn);
     __syncwarp();
     const int kend = min(TN, n_max - t0);
     for (int k = part; k < kend; k += P) {
@@ -201,7 +227,7 @@ __global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB3) k_pairgrad
   constexpr int PD = Tl::PD3, ROW = Tl::ROW3;
   extern __shared__ __align__(16) double csm[];
   const int ncoef = stage_coef(a, csm, NS * NSLOT);
-  const int *kmsm = reinterpret_cast<const int *>(csm + a.n_species * a.n_species * a.crow);
+  const int *kmsm = reinterpret_cast<const int *>(csm + a.n_species * a.n_species * a.crow + kShiftLut);
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   double *tile = csm + ncoef + wib * Tl::WARP3;
   double *dtile = tile + NA * ROW;                  // [128][4]
@@ -234,21 +260,33 @@ __global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB3) k_pairgrad
   double Fx = 0, Fy = 0, Fz = 0, W[6] = {0, 0, 0, 0, 0, 0};
   const int ka = (4 * lane) % TN;
   double *mine = tile + sa * ROW;
-  int jn[4];
-  fetch_idx(a, beg, n_nb, ka, jn);
+  const double *slut = csm + a.n_species * a.n_species * a.crow;
+  double *pst = dtile + 128 * 4 + 4 * (4 * lane);            // this lane's four position slots (buffer 0)
+  int *wst = reinterpret_cast<int *>(dtile + 128 * 4 + 2 * 512) + 4 * lane;   // its four word slots (buffer 0)
+  stage_words(a, beg, n_nb, ka, wst);
+  stage_words(a, beg, n_nb, TN + ka, wst + 128);
+  commit_copies();
+  wait_positions();
+  stage_positions(a, *reinterpret_cast<const int4 *>(wst), pst);
+  commit_copies();
+  int wb = 0, pb = 0;                                       // buffers holding the current tile's words / positions
   for (int t0 = 0; t0 < n_max; t0 += TN) {
-    int jc[4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u) jc[u] = jn[u];
-    fetch_idx(a, beg, n_nb, t0 + TN + ka, jn);
+    wait_positions();                                       // positions of this tile and words of the next have landed
+    const int4 jc4 = *reinterpret_cast<const int4 *>(wst + 128 * wb);
+    const int jc[4] = {jc4.x, jc4.y, jc4.z, jc4.w};
+    const double *rec = pst + 512 * pb;
+    const int wn = wb == 2 ? 0 : wb + 1, wnn = wn == 2 ? 0 : wn + 1;
+    stage_positions(a, *reinterpret_cast<const int4 *>(wst + 128 * wn), pst + 512 * (pb ^ 1));
+    stage_words(a, beg, n_nb, t0 + 2 * TN + ka, wst + 128 * wnn);
+    commit_copies();
+    wb = wn; pb ^= 1;
     __syncwarp();
     // ---- phase A
     PairGeo geo[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) geo[u] = load_pair(a, jc[u], beg + t0 + ka + u, xi, yi, zi);
+    for (int u = 0; u < 4; ++u) geo[u] = load_pair(a, slut, jc[u], rec + 4 * u, xi, yi, zi);
 #pragma unroll
     for (int u = 0; u < 4; ++u) stage_pair<NMU, true, PD, NB>(a, csm, geo[u], zi_s, rc2, mine + (ka + u) * PD);
-    prefetch_pairs(a, beg, t0 + TN + ka, jn);
     __syncwarp();
     // ---- phase B
     const int kend = min(TN, n_max - t0);
@@ -328,7 +366,7 @@ __global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB3) k_pairgrad
         const long long p = beg + k;
         if (ATOMIC) {
           if (dx != 0.0 || dy != 0.0 || dz != 0.0) {
-            const int j = jc[u];
+            const int j = jc[u] & kIdxMask;
             atomicAdd(a.F + 3 * (size_t)j, -dx);
             atomicAdd(a.F + 3 * (size_t)j + 1, -dy);
             atomicAdd(a.F + 3 * (size_t)j + 2, -dz);
