@@ -90,6 +90,10 @@ const char *mtp_last_error(const mtp_handle *h); /* h may be NULL: last create e
 #define MTP_OPT_FORCE_MODE 2    /* MTP_FORCE_GATHER (needs d_rev) | MTP_FORCE_ATOMIC       */
 #define MTP_OPT_VARIANT 3       /* MTP_VARIANT_AUTO | _THREAD | _BLOCK                     */
 #define MTP_OPT_PROFILE 4       /* 1: record CUDA events around every kernel launch        */
+#define MTP_OPT_TREE_CODEGEN 5  /* 1 (default): specialise the contraction kernel for the table with NVRTC at
+                                   first use when the table is short enough; 0: always interpret the table.
+                                   Same arithmetic order either way (bit-identical results).             */
+#define MTP_INFO_TREE_KERNELS 100 /* mtp_get_option only: number of NVRTC-specialised contraction kernels in use */
 #define MTP_FORCE_GATHER 0      /* deterministic; keeps d_ij for all pairs (nnz x 32 B)  */
 #define MTP_FORCE_ATOMIC 1      /* fp64 atomic scatter; no per-pair scratch              */
 #define MTP_FORCE_AUTO 2        /* default: gather when d_rev is given, else atomic      */

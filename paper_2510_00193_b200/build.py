@@ -57,7 +57,7 @@ def build(verbose: bool = False, force: bool = False) -> str:
         for r in res:
             sys.stderr.write(r[1])
     if (not os.path.exists(OUT)) or any(os.path.getmtime(o) > os.path.getmtime(OUT) for o in objs):
-        cmd = [NVCC] + ARCH + ["-shared", "-o", OUT] + objs
+        cmd = [NVCC] + ARCH + ["-shared", "-o", OUT] + objs + ["-ldl"]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError("link failed:\n%s\n%s" % (r.stdout, r.stderr))

@@ -5,6 +5,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <string>
@@ -46,7 +47,10 @@ struct mtp_handle {
     int *d_fwave = nullptr, *d_bwave = nullptr, *d_gseed_k = nullptr, *d_gzero_k = nullptr;
     int *d_eseed_slot = nullptr, *d_basis_slot = nullptr;
     double *d_adj_init = nullptr, *d_gseed_val = nullptr, *d_leaf_seed = nullptr, *d_eseed_val = nullptr;
+    TreeJit *jit = nullptr;                    // specialised kernel (tree_jit.cpp), null = interpreter
+    std::string jit_note;
   };
+  int codegen = 1;                             // MTP_OPT_TREE_CODEGEN
   std::map<int, TreeDev> trees;                // key: AL * 8 + AR * 2 + elide
   int slots[2][2] = {{0, 0}, {0, 0}};          // [elide][n_val, n_adj]
   std::vector<int32_t> t_prod, t_basis_node;   // host copy of the table for those compilations
@@ -177,6 +181,10 @@ static int get_tree(mtp_handle *h, int AL, int AR, bool elide, const mtp_handle:
   up(upload(h, &td.d_gseed_val, sc.gseed_val.data(), sc.gseed_val.size()));
   up(upload(h, &td.d_gzero_k, sc.gzero_k.data(), sc.gzero_k.size()));
   if (e != cudaSuccess) return cuda_fail(h, e, "tree schedule upload");
+  // specialise the kernel for this schedule when it is short enough to be worth compiling
+  const char *env = getenv("MTP_TREE_CODEGEN");
+  const long long entries = (sc.fsteps + sc.bsteps) * (long long)sc.R;
+  if (h->codegen && !(env && env[0] == '0') && AL == 32 && entries <= 60000) td.jit = tree_jit_build(sc, AL, AR, &td.jit_note);
   auto ins = h->trees.emplace(key, std::move(td));
   *out = &ins.first->second;
   return MTP_OK;
@@ -203,6 +211,7 @@ extern "C" void mtp_destroy(mtp_handle *h) {
   if (!h) return;
   for (auto &s : h->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
   for (auto e : h->pool) cudaEventDestroy(e);
+  for (auto &kv : h->trees) tree_jit_destroy(kv.second.jit);
   for (void *p : h->to_free) cudaFree(p);
   if (h->stage) cudaFree(h->stage);
   delete h;
@@ -285,6 +294,12 @@ extern "C" int mtp_set_option(mtp_handle *h, int key, int64_t v) {
     case MTP_OPT_FORCE_MODE: if (v < 0 || v > 2) return fail(h, MTP_EINVAL, "bad force mode"); h->force_mode = (int)v; return MTP_OK;
     case MTP_OPT_VARIANT: if (v < 0 || v > 2) return fail(h, MTP_EINVAL, "bad variant"); h->variant = (int)v; return MTP_OK;
     case MTP_OPT_PROFILE: h->profile = v != 0; return MTP_OK;
+    case MTP_OPT_TREE_CODEGEN:
+      if (h->codegen != (v != 0)) {          // schedules are cached with or without their specialised kernel
+        for (auto &kv : h->trees) { tree_jit_destroy(kv.second.jit); kv.second.jit = nullptr; }
+        if (v != 0) h->trees.clear();        // device arrays stay owned by the handle (to_free)
+      }
+      h->codegen = v != 0; return MTP_OK;
   }
   return fail(h, MTP_EINVAL, "unknown option");
 }
@@ -295,6 +310,12 @@ extern "C" int mtp_get_option(const mtp_handle *h, int key, int64_t *v) {
     case MTP_OPT_FORCE_MODE: *v = h->force_mode; return MTP_OK;
     case MTP_OPT_VARIANT: *v = h->variant; return MTP_OK;
     case MTP_OPT_PROFILE: *v = h->profile; return MTP_OK;
+    case MTP_OPT_TREE_CODEGEN: *v = h->codegen; return MTP_OK;
+    case MTP_INFO_TREE_KERNELS: {             // specialised K2 kernels in use
+      int n = 0;
+      for (auto &kv : h->trees) n += kv.second.jit != nullptr;
+      *v = n; return MTP_OK;
+    }
   }
   return MTP_EINVAL;
 }
@@ -379,11 +400,12 @@ void fill_pair_args(const mtp_handle *h, PairArgs &pa, const double *pos4, const
   pa.M = nullptr; pa.G = nullptr; pa.d4 = nullptr; pa.F = nullptr; pa.wpart = nullptr; pa.kmap = nullptr;
 }
 
-int fill_tree_args(mtp_handle *h, TreeArgs &ta, const double *pos4, const Plan &pl) {
+int fill_tree_args(mtp_handle *h, TreeArgs &ta, const double *pos4, const Plan &pl, const TreeJit **jit) {
   const mtp_handle::TreeDev *td = nullptr;
   int rc = get_tree(h, pl.AL, pl.AR, pl.elide != 0, &td);
   if (rc != MTP_OK) return rc;
   const TreeSched &sc = td->sched;
+  *jit = td->jit;
   ta.fprog = td->d_fprog; ta.fwave = td->d_fwave; ta.nfw = (int)sc.fwave.size() - 1;
   ta.bprog = td->d_bprog; ta.bwave = td->d_bwave; ta.nbw = (int)sc.bwave.size() - 1;
   ta.n_fprog = (int)sc.fprog.size(); ta.n_bprog = (int)sc.bprog.size(); ta.prog_smem_off = 0;
@@ -445,7 +467,8 @@ extern "C" int mtp_compute(mtp_handle *h, int64_t N, const double *d_pos, const 
   fill_pair_args(h, pa, pos4, d_off, idxp, d_shift);
   pa.ldm = pl.ldm;
   TreeArgs ta;
-  rc = fill_tree_args(h, ta, pos4, pl);
+  const TreeJit *jit = nullptr;
+  rc = fill_tree_args(h, ta, pos4, pl, &jit);
   if (rc != MTP_OK) return rc;
   ta.M = M; ta.G = G; ta.ldm = pl.ldm; ta.Ei = Ei;
   for (int c = 0; c < pl.n_chunks; ++c) {
@@ -453,7 +476,7 @@ extern "C" int mtp_compute(mtp_handle *h, int64_t N, const double *d_pos, const 
     pa.M = M; pa.G = G; pa.kmap = h->d_kmapF;
     TIMED(h, CLS_MOMENTS, st, h->pl->moments(pa, pl.P, st));
     ta.c0 = pa.c0; ta.c1 = pa.c1;
-    TIMED(h, CLS_TREE, st, launch_tree(ta, pl.AL, pl.AR, st));
+    TIMED(h, CLS_TREE, st, (jit ? tree_jit_launch(jit, ta, st) : launch_tree(ta, pl.AL, pl.AR, st)));
     pa.kmap = h->d_kmapB; pa.wpart = wpart + (size_t)c * pl.grid_chunk * 8;
     pa.d4 = pl.atomic ? nullptr : d4; pa.F = pl.atomic ? d_F : nullptr;
     TIMED(h, CLS_PAIRGRAD, st, h->pl->pairgrad(pa, pl.P, pl.atomic, st, nullptr));
@@ -499,7 +522,8 @@ extern "C" int mtp_grade(mtp_handle *h, int64_t N, const double *d_pos, const in
     fill_pair_args(h, pa, pos4, d_off, idxp, d_shift);
     pa.ldm = pl.ldm;
     TreeArgs ta;
-    rc = fill_tree_args(h, ta, pos4, pl);
+    const TreeJit *jit = nullptr;
+    rc = fill_tree_args(h, ta, pos4, pl, &jit);
     if (rc != MTP_OK) return rc;
     ta.M = M; ta.G = G; ta.ldm = pl.ldm; ta.Ei = Ei; ta.want_adj = 0;
     for (int c = 0; c < pl.n_chunks; ++c) {
@@ -510,7 +534,7 @@ extern "C" int mtp_grade(mtp_handle *h, int64_t N, const double *d_pos, const in
       // B rows are indexed by absolute atom: point the kernel at a base shifted by -c0 rows
       double *Brows = d_B ? d_B : Bc - (size_t)pa.c0 * h->n_basis;
       ta.B = Brows;
-      TIMED(h, CLS_TREE, st, launch_tree(ta, pl.AL, pl.AR, st));
+      TIMED(h, CLS_TREE, st, (jit ? tree_jit_launch(jit, ta, st) : launch_tree(ta, pl.AL, pl.AR, st)));
       const double *Bchunk = Brows + (size_t)pa.c0 * h->n_basis;
       const int64_t nc = pa.c1 - pa.c0;
       if (mode != 1) TIMED(h, CLS_GRADE, st, launch_grade(Bchunk, d_Ainv, nc, h->n_basis, d_gamma_atom + pa.c0, st));
@@ -605,10 +629,11 @@ extern "C" int mtp_debug_moments(mtp_handle *h, int64_t N, const double *d_pos, 
     if (e != cudaSuccess) return cuda_fail(h, e, "moments");
   }
   TreeArgs ta;
-  rc = fill_tree_args(h, ta, pos4, pl);
+  const TreeJit *jit = nullptr;
+  rc = fill_tree_args(h, ta, pos4, pl, &jit);
   if (rc != MTP_OK) return rc;
   ta.M = M; ta.G = G; ta.ldm = pl.ldm; ta.Ei = Ei; ta.c0 = 0; ta.c1 = (int)N; ta.B = d_B;
-  CU(h, launch_tree(ta, pl.AL, pl.AR, st));
+  CU(h, (jit ? tree_jit_launch(jit, ta, st) : launch_tree(ta, pl.AL, pl.AR, st)));
   // outputs are [n_basic][N] (component-major), the kernels' own layout
   if (d_M) CU(h, cudaMemcpy2DAsync(d_M, (size_t)N * 8, M, (size_t)pl.ldm * 8, (size_t)N * 8, h->n_basic, cudaMemcpyDeviceToDevice, st));
   if (d_G) CU(h, cudaMemcpy2DAsync(d_G, (size_t)N * 8, G, (size_t)pl.ldm * 8, (size_t)N * 8, h->n_basic, cudaMemcpyDeviceToDevice, st));

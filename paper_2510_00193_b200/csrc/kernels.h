@@ -2,6 +2,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <cstdint>
+#include <string>
 
 #include "pair_kernels_args.h"
 #include "tree.h"
@@ -37,6 +38,11 @@ int tree_threads(int AL);               // CTA size used with AL atom-lanes
 int tree_row_lanes(int AL);             // row-lanes R = threads / AL the schedule must be dealt for
 size_t tree_smem_bytes(int n_val, int n_adj, int AL, int AR);
 cudaError_t launch_tree(const TreeArgs &a, int AL, int AR, cudaStream_t st);
+// K2 specialised for one schedule with NVRTC (tree_jit.cpp); null when unavailable (reason in *why)
+struct TreeJit;
+TreeJit *tree_jit_build(const TreeSched &sc, int AL, int AR, std::string *why);
+cudaError_t tree_jit_launch(const TreeJit *j, const TreeArgs &a, cudaStream_t st);
+void tree_jit_destroy(TreeJit *j);
 
 // ---- K1 / K3: one entry per compiled level (pair_lev*.cu)
 struct PairLevel {

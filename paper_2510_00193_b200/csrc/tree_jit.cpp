@@ -1,0 +1,301 @@
+// K2 specialised at mtp_create time: the lane programs of tree.h are turned into straight-line CUDA
+// source (one code region per wave and row-lane warp, shared-memory operands at immediate offsets,
+// multipliers as literals), compiled with NVRTC for sm_100a and loaded through the runtime's library
+// API.  Same mapping and same arithmetic order as the interpreter in tree_kernel.cu (atoms across
+// lanes, AL = 32, AR atoms per lane, warps = row-lanes), so results are bit-identical; what goes away
+// is the per-entry fetch / decode / branch work (~20 instructions per entry -> 2 loads + AR FMAs).
+// NVRTC is dlopen'ed: without it (or when a program is too long to be worth compiling) the
+// interpreter runs instead -- both are CUDA paths.  BASELINE.json north_star: "forward/adjoint
+// contraction kernel with the tree in registers and shared memory".
+#include <cuda_runtime.h>
+#include <dlfcn.h>
+
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "kernels.h"
+
+namespace mtpb {
+
+namespace {
+// ---- the few NVRTC entry points we need, resolved at run time
+typedef struct _nvrtcProgram *nvrtcProgram;
+struct Nvrtc {
+  int (*CreateProgram)(nvrtcProgram *, const char *, const char *, int, const char *const *, const char *const *) = nullptr;
+  int (*CompileProgram)(nvrtcProgram, int, const char *const *) = nullptr;
+  int (*GetCUBINSize)(nvrtcProgram, size_t *) = nullptr;
+  int (*GetCUBIN)(nvrtcProgram, char *) = nullptr;
+  int (*GetProgramLogSize)(nvrtcProgram, size_t *) = nullptr;
+  int (*GetProgramLog)(nvrtcProgram, char *) = nullptr;
+  int (*DestroyProgram)(nvrtcProgram *) = nullptr;
+  bool ok = false;
+};
+const Nvrtc &nvrtc() {
+  static Nvrtc n = [] {
+    Nvrtc r;
+    void *h = nullptr;
+    for (const char *name : {"libnvrtc.so.12", "libnvrtc.so", "/usr/local/cuda/lib64/libnvrtc.so.12"})
+      if ((h = dlopen(name, RTLD_NOW | RTLD_LOCAL))) break;
+    if (!h) return r;
+    auto sym = [&](const char *s) { return dlsym(h, s); };
+    r.CreateProgram = (decltype(r.CreateProgram))sym("nvrtcCreateProgram");
+    r.CompileProgram = (decltype(r.CompileProgram))sym("nvrtcCompileProgram");
+    r.GetCUBINSize = (decltype(r.GetCUBINSize))sym("nvrtcGetCUBINSize");
+    r.GetCUBIN = (decltype(r.GetCUBIN))sym("nvrtcGetCUBIN");
+    r.GetProgramLogSize = (decltype(r.GetProgramLogSize))sym("nvrtcGetProgramLogSize");
+    r.GetProgramLog = (decltype(r.GetProgramLog))sym("nvrtcGetProgramLog");
+    r.DestroyProgram = (decltype(r.DestroyProgram))sym("nvrtcDestroyProgram");
+    r.ok = r.CreateProgram && r.CompileProgram && r.GetCUBINSize && r.GetCUBIN && r.DestroyProgram;
+    return r;
+  }();
+  return n;
+}
+
+// Kernel frame: prologue / epilogue as in tree_kernel.cu; @FWD@ / @BWD@ receive the generated passes.
+const char *kFrame = R"SRC(
+struct TreeTerm;
+struct TreeArgs {
+  const TreeTerm *fprog; const int *fwave; int nfw;
+  const TreeTerm *bprog; const int *bwave; int nbw;
+  int n_fprog, n_bprog;
+  int prog_smem_off;
+  const double *xi0;
+  const double *adj_init;
+  const double *leaf_seed;
+  const int *eseed_slot; const double *eseed_val; int n_eseed;
+  const int *basis_slot;
+  const int *gseed_k; const double *gseed_val; int n_gseed;
+  const int *gzero_k; int n_gzero;
+  const double *pos4;
+  const double *M; double *G; long long ldm;
+  double *Ei;
+  double *B;
+  int n_val, n_adj, n_basic, n_basis;
+  int c0, c1;
+  int want_adj;
+};
+#define AR @AR@
+#define NT @NT@
+#define AL 32
+#define A (AL * AR)
+#define R (NT / AL)
+#if AR == 2
+#define LD(p) (*(const double2 *)(p))
+#define E(OA, OB) { const double2 X = LD(s0 + OA), Y = LD(vc + OB); ax = fma(X.x, Y.x, ax); ay = fma(X.y, Y.y, ay); }
+#define GC(M) { tx = fma(M, ax, tx); ty = fma(M, ay, ty); ax = 0.0; ay = 0.0; }
+#define RV(D) { *(double2 *)(vw + D) = make_double2(tx, ty); tx = 0.0; ty = 0.0; }
+#define RL(S) { ex = fma(S, tx, ex); ey = fma(S, ty, ey); tx = 0.0; ty = 0.0; }
+#define RA(D) { double2 o = LD(ac + D); o.x += tx; o.y += ty; *(double2 *)(ac + D) = o; tx = 0.0; ty = 0.0; }
+#define RG(K) { if (n_ok > 0) Gcol[(long long)K * ldm] = tx; if (n_ok > 1) Gcol[(long long)K * ldm + 1] = ty; tx = 0.0; ty = 0.0; }
+#else
+#define LD(p) (*(const double *)(p))
+#define E(OA, OB) { ax = fma(LD(s0 + OA), LD(vc + OB), ax); }
+#define GC(M) { tx = fma(M, ax, tx); ax = 0.0; }
+#define RV(D) { *(double *)(vw + D) = tx; tx = 0.0; }
+#define RL(S) { ex = fma(S, tx, ex); tx = 0.0; }
+#define RA(D) { *(double *)(ac + D) += tx; tx = 0.0; }
+#define RG(K) { if (n_ok > 0) Gcol[(long long)K * ldm] = tx; tx = 0.0; }
+#endif
+
+extern "C" __global__ void __launch_bounds__(NT) k_tree_gen(const TreeArgs a) {
+  extern __shared__ __align__(16) char smraw[];
+  double *val = (double *)smraw;
+  double *adj = val + (size_t)a.n_val * A;
+  double *esm = adj + (size_t)a.n_adj * A;
+  const int al = threadIdx.x % AL, rl = threadIdx.x / AL;
+  const char *vc = smraw + al * AR * 8;
+  char *vw = smraw + al * AR * 8;
+  char *ac = (char *)adj + al * AR * 8;
+  const long long ldm = a.ldm;
+  const int n_groups = (a.c1 - a.c0 + A - 1) / A;
+  for (int g = blockIdx.x; g < n_groups; g += gridDim.x) {
+    const int atom0 = a.c0 + g * A + al * AR;
+    const int n_ok = min(AR, max(0, a.c1 - atom0));
+    const long long col = atom0 - a.c0;
+    __syncthreads();
+    for (int k = rl; k < a.n_basic; k += R)
+      for (int r = 0; r < AR; ++r) val[(size_t)k * A + al * AR + r] = r < n_ok ? a.M[(long long)k * ldm + col + r] : 0.0;
+    if (a.want_adj)
+      for (int k = rl; k < a.n_adj; k += R)
+        for (int r = 0; r < AR; ++r) adj[(size_t)k * A + al * AR + r] = a.adj_init[k];
+    __syncthreads();
+    double ex = 0.0, ey = 0.0, ax = 0.0, ay = 0.0, tx = 0.0, ty = 0.0;
+    (void)ey; (void)ay; (void)ty;
+    {
+      const char *s0 = vc;
+@FWD@
+    }
+    {
+      for (int q = rl; q < a.n_eseed; q += R) {
+        const double sd = a.eseed_val[q];
+        const double *v = val + (size_t)a.eseed_slot[q] * A + al * AR;
+        ex = fma(sd, v[0], ex);
+#if AR == 2
+        ey = fma(sd, v[1], ey);
+#endif
+      }
+      esm[rl * A + al * AR] = ex;
+#if AR == 2
+      esm[rl * A + al * AR + 1] = ey;
+#endif
+      if (a.B) {
+        const int na = min(A, a.c1 - (a.c0 + g * A));
+        for (int i = threadIdx.x; i < na * a.n_basis; i += NT) {
+          const int at = i / a.n_basis, b = i - at * a.n_basis;
+          a.B[(long long)(a.c0 + g * A + at) * a.n_basis + b] = val[(size_t)a.basis_slot[b] * A + at];
+        }
+      }
+      __syncthreads();
+      if (rl == 0) {
+        for (int r = 0; r < AR; ++r) {
+          if (r < n_ok) {
+            double s = 0.0;
+            for (int q = 0; q < R; ++q) s += esm[q * A + al * AR + r];
+            const int z = (int)a.pos4[4 * (size_t)(atom0 + r) + 3];
+            a.Ei[atom0 + r] = a.xi0[z] + s;
+          }
+        }
+      }
+    }
+    if (!a.want_adj) continue;
+    double *Gcol = a.G + col;
+    for (int q = rl; q < a.n_gzero; q += R)
+      for (int r = 0; r < AR; ++r)
+        if (r < n_ok) Gcol[(long long)a.gzero_k[q] * ldm + r] = 0.0;
+    {
+      const char *s0 = ac;
+      ax = 0.0; ay = 0.0; tx = 0.0; ty = 0.0;
+@BWD@
+    }
+    __syncthreads();
+    for (int q = rl; q < a.n_gseed; q += R)
+      for (int r = 0; r < AR; ++r)
+        if (r < n_ok) Gcol[(long long)a.gseed_k[q] * ldm + r] += a.gseed_val[q];
+  }
+}
+)SRC";
+
+void replace_all(std::string &s, const std::string &key, const std::string &val) {
+  for (size_t p = s.find(key); p != std::string::npos; p = s.find(key, p + val.size())) s.replace(p, key.size(), val);
+}
+
+// straight-line source of one pass: per wave a switch over the row-lane, then the CTA barrier
+std::string gen_pass(const std::vector<TreeTerm> &prog, const std::vector<int32_t> &wave, int R, bool bwd,
+                     const std::vector<double> &leaf_seed, int A) {
+  std::string out;
+  out.reserve(prog.size() * 24);
+  char buf[160];
+  const unsigned row = (unsigned)A * 8u;
+  for (size_t w = 0; w + 1 < wave.size(); ++w) {
+    out += "      switch (rl) {\n";
+    for (int l = 0; l < R; ++l) {
+      int last = -1;
+      for (int s = wave[w]; s < wave[w + 1]; ++s)
+        if (prog[(size_t)s * R + l].a & kTreeRow) last = s;
+      if (last < 0) continue;
+      snprintf(buf, sizeof buf, "      case %d: {\n", l);
+      out += buf;
+      for (int s = wave[w]; s <= last; ++s) {
+        const TreeTerm &t = prog[(size_t)s * R + l];
+        snprintf(buf, sizeof buf, "E(%u,%u)", t.a & ~7u, t.b & ((1u << kTreeDstShift) - 1));
+        out += buf;
+        if (t.a & kTreeGroup) {
+          snprintf(buf, sizeof buf, "GC(%a)", t.mult);
+          out += buf;
+          if (t.a & kTreeRow) {
+            const unsigned d = t.b >> kTreeDstShift;
+            if (!bwd) {
+              if (t.a & kTreeAlt) snprintf(buf, sizeof buf, "RL(%a)", leaf_seed[d]);
+              else snprintf(buf, sizeof buf, "RV(%u)", d * row);
+            } else {
+              if (t.a & kTreeAlt) snprintf(buf, sizeof buf, "RG(%u)", d);
+              else snprintf(buf, sizeof buf, "RA(%u)", d * row);
+            }
+            out += buf;
+          }
+        }
+        out += "\n";
+      }
+      out += "      } break;\n";
+    }
+    out += "      default: break;\n      }\n      __syncthreads();\n";
+  }
+  return out;
+}
+}  // namespace
+
+struct TreeJit {
+  cudaLibrary_t lib = nullptr;
+  cudaKernel_t kernel = nullptr;
+  int AR = 1, NT = 512;
+};
+
+void tree_jit_destroy(TreeJit *j) {
+  if (!j) return;
+  if (j->lib) cudaLibraryUnload(j->lib);
+  delete j;
+}
+
+// Returns null (and a reason in *why) when the specialised kernel is not available.
+TreeJit *tree_jit_build(const TreeSched &sc, int AL, int AR, std::string *why) {
+  if (AL != 32) { *why = "codegen needs 32 atom-lanes"; return nullptr; }
+  const Nvrtc &rt = nvrtc();
+  if (!rt.ok) { *why = "NVRTC not found"; return nullptr; }
+  const int NT = tree_threads(AL), R = NT / AL;
+  if (sc.R != R || sc.A != AL * AR) { *why = "schedule shape mismatch"; return nullptr; }
+  std::string src = kFrame;
+  replace_all(src, "@AR@", std::to_string(AR));
+  replace_all(src, "@NT@", std::to_string(NT));
+  replace_all(src, "@FWD@", gen_pass(sc.fprog, sc.fwave, R, false, sc.leaf_seed, AL * AR));
+  replace_all(src, "@BWD@", gen_pass(sc.bprog, sc.bwave, R, true, sc.leaf_seed, AL * AR));
+  nvrtcProgram prog = nullptr;
+  if (rt.CreateProgram(&prog, src.c_str(), "k_tree_gen.cu", 0, nullptr, nullptr) != 0) { *why = "nvrtcCreateProgram failed"; return nullptr; }
+  const char *opts[] = {"--gpu-architecture=sm_100a", "--std=c++17", "-lineinfo", "-default-device"};
+  const int rc = rt.CompileProgram(prog, 4, opts);
+  if (rc != 0) {
+    size_t n = 0;
+    std::string log;
+    if (rt.GetProgramLogSize && rt.GetProgramLog && rt.GetProgramLogSize(prog, &n) == 0 && n > 1) { log.resize(n); rt.GetProgramLog(prog, &log[0]); }
+    *why = "NVRTC compile failed: " + log.substr(0, 400);
+    rt.DestroyProgram(&prog);
+    return nullptr;
+  }
+  size_t nbin = 0;
+  rt.GetCUBINSize(prog, &nbin);
+  std::vector<char> cubin(nbin);
+  rt.GetCUBIN(prog, cubin.data());
+  rt.DestroyProgram(&prog);
+  TreeJit *j = new TreeJit();
+  j->AR = AR; j->NT = NT;
+  cudaError_t e = cudaLibraryLoadData(&j->lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
+  if (e == cudaSuccess) e = cudaLibraryGetKernel(&j->kernel, j->lib, "k_tree_gen");
+  if (e == cudaSuccess) e = cudaFuncSetAttribute((const void *)j->kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024);
+  if (e != cudaSuccess) {
+    *why = std::string("loading the generated kernel failed: ") + cudaGetErrorString(e);
+    cudaGetLastError();
+    tree_jit_destroy(j);
+    return nullptr;
+  }
+  return j;
+}
+
+cudaError_t tree_jit_launch(const TreeJit *j, const TreeArgs &a, cudaStream_t st) {
+  const int Aat = 32 * j->AR;
+  const int groups = (a.c1 - a.c0 + Aat - 1) / Aat;
+  if (groups <= 0) return cudaSuccess;
+  static int sms = 0;
+  if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
+  const size_t smem = tree_smem_bytes(a.n_val, a.n_adj, 32, j->AR);
+  int per_sm = (int)((227 * 1024) / (smem + 1024));
+  per_sm = per_sm < 1 ? 1 : (per_sm > 2048 / j->NT ? 2048 / j->NT : per_sm);
+  const int grid = groups < sms * per_sm ? groups : sms * per_sm;
+  TreeArgs args = a;
+  void *params[] = {&args};
+  cudaError_t e = cudaLaunchKernel((const void *)j->kernel, dim3(grid), dim3(j->NT), params, smem, st);
+  count_launch();
+  return e;
+}
+
+}  // namespace mtpb

@@ -168,3 +168,42 @@ def test_host_path_matches_device_path(lib, torch):
     h = pot.compute_host(w.pos, w.types, w.box, w.off, w.idx, w.shift, w.rev)
     assert np.array_equal(h["F"], got["F"]) and np.array_equal(h["Ei"], got["Ei"]) and h["E"][0] == got["E"][0]
     pot.close()
+
+
+def test_specialised_tree_kernel_is_bit_identical_to_the_interpreter(lib, torch):
+    """MTP_OPT_TREE_CODEGEN: the NVRTC-specialised K2 keeps the interpreter's arithmetic order."""
+    w = make_workload(3, n_basis_of(16), cells=18)            # 23 328 atoms: the AL = 32, AR = 2 shape
+    a, pot, d = run_gpu(lib, torch, w, opts={lib.OPT_TREE_CODEGEN: 0, lib.OPT_VARIANT: lib.VARIANT_THREAD})
+    assert pot.get_option(lib.INFO_TREE_KERNELS) == 0
+    pot.close()
+    b, pot, _ = run_gpu(lib, torch, w, opts={lib.OPT_TREE_CODEGEN: 1, lib.OPT_VARIANT: lib.VARIANT_THREAD})
+    used = pot.get_option(lib.INFO_TREE_KERNELS)
+    pot.close()
+    for k in ("Ei", "F", "virial", "E"):
+        assert np.array_equal(a[k], b[k]), k
+    print("specialised tree kernels in use:", used)
+
+
+def test_large_launch_configuration_on_sampled_atoms(lib, torch):
+    """The launch configuration bench.py times (config 4 structure, thread-parallel pair kernels, 64-atom
+    tree CTAs, specialised K2, several chunks): E_i, F_k on sampled atoms against the oracle, sum F = 0."""
+    w = make_workload(3, n_basis_of(16), cells=22)            # 42 592 atoms, 3 species, level 16
+    got, pot, _ = run_gpu(lib, torch, w, opts={lib.OPT_CHUNK_ATOMS: 16384})
+    assert pot.get_option(lib.OPT_VARIANT) == lib.VARIANT_AUTO
+    pot.close()
+    opot = oracle_pot(w)
+    rng = np.random.default_rng(5)
+    sample = [int(x) for x in rng.choice(w.n_atoms, 5, replace=False)]
+    need = set(sample)
+    for k in sample:
+        need.update(int(j) for j in w.idx[w.off[k]:w.off[k + 1]])
+    ref = omtp.evaluate(opot, w.pos, w.types, w.box, w.off, w.idx, w.shift, atoms=sorted(need))
+    d = ref["d"]
+    for k in sample:
+        sE = max(1.0, np.abs(ref["B"][k] * w.xi).sum())
+        assert abs(got["Ei"][k] - ref["E_i"][k]) <= TOL_E * sE
+        rows = np.arange(w.off[k], w.off[k + 1])
+        Fk = d[rows].sum(axis=0) - d[w.rev[rows]].sum(axis=0)
+        sF = max(1.0, np.abs(d[rows]).sum() + np.abs(d[w.rev[rows]]).sum())
+        assert np.all(np.abs(got["F"][k] - Fk) <= TOL_F * sF)
+    assert np.all(np.abs(got["F"].sum(axis=0)) <= 1e-9 * np.abs(got["F"]).sum())
