@@ -162,9 +162,24 @@ static int get_tree(mtp_handle *h, int AL, int AR, bool elide, const mtp_handle:
   if (it != h->trees.end()) { *out = &it->second; return MTP_OK; }
   mtp_handle::TreeDev td;
   const char *terr = "";
-  int rc = tree_compile(h->n_basic, h->n_nodes, (int)h->n_prod, h->t_prod.data(), h->n_basis, h->t_basis_node.data(),
-                        h->t_xi.data(), AL * AR, tree_row_lanes(AL), elide, td.sched, &terr);
-  if (rc != MTP_OK) return fail(h, rc, terr);
+  int rc = MTP_OK;
+  // First choice: the kernel specialised for this table (tree_jit.cpp), same schedule as the interpreter
+  // (so the two are bit-identical), when the table is short enough to be worth compiling and the shape has
+  // 32 atom-lanes.  (32 row-lane warps instead of 16 were measured slower: the generated code is bound by
+  // instruction fetch, not by per-warp latency.)
+  const char *env = getenv("MTP_TREE_CODEGEN");
+  if (h->codegen && !(env && env[0] == '0') && AL == 32 && 3LL * h->n_prod <= 60000 &&
+      tree_jit_smem_bytes(h->slots[elide][0], h->slots[elide][1], AR, tree_threads(AL)) <= 225 * 1024) {
+    rc = tree_compile(h->n_basic, h->n_nodes, (int)h->n_prod, h->t_prod.data(), h->n_basis, h->t_basis_node.data(),
+                      h->t_xi.data(), AL * AR, tree_row_lanes(AL), elide, td.sched, &terr);
+    if (rc != MTP_OK) return fail(h, rc, terr);
+    td.jit = tree_jit_build(td.sched, AL, AR, &td.jit_note);
+  }
+  if (!td.jit) {
+    rc = tree_compile(h->n_basic, h->n_nodes, (int)h->n_prod, h->t_prod.data(), h->n_basis, h->t_basis_node.data(),
+                      h->t_xi.data(), AL * AR, tree_row_lanes(AL), elide, td.sched, &terr);
+    if (rc != MTP_OK) return fail(h, rc, terr);
+  }
   cudaError_t e = cudaSuccess;
   auto up = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
   const TreeSched &sc = td.sched;
@@ -181,10 +196,6 @@ static int get_tree(mtp_handle *h, int AL, int AR, bool elide, const mtp_handle:
   up(upload(h, &td.d_gseed_val, sc.gseed_val.data(), sc.gseed_val.size()));
   up(upload(h, &td.d_gzero_k, sc.gzero_k.data(), sc.gzero_k.size()));
   if (e != cudaSuccess) return cuda_fail(h, e, "tree schedule upload");
-  // specialise the kernel for this schedule when it is short enough to be worth compiling
-  const char *env = getenv("MTP_TREE_CODEGEN");
-  const long long entries = (sc.fsteps + sc.bsteps) * (long long)sc.R;
-  if (h->codegen && !(env && env[0] == '0') && AL == 32 && entries <= 60000) td.jit = tree_jit_build(sc, AL, AR, &td.jit_note);
   auto ins = h->trees.emplace(key, std::move(td));
   *out = &ins.first->second;
   return MTP_OK;

@@ -43,6 +43,7 @@ struct TreeJit;
 TreeJit *tree_jit_build(const TreeSched &sc, int AL, int AR, std::string *why);
 cudaError_t tree_jit_launch(const TreeJit *j, const TreeArgs &a, cudaStream_t st);
 void tree_jit_destroy(TreeJit *j);
+size_t tree_jit_smem_bytes(int n_val, int n_adj, int AR, int NT);
 
 // ---- K1 / K3: one entry per compiled level (pair_lev*.cu)
 struct PairLevel {

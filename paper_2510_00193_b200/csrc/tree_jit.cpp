@@ -83,23 +83,29 @@ struct TreeArgs {
 #define R (NT / AL)
 #if AR == 2
 #define LD(p) (*(const double2 *)(p))
+// E0 / G0 open a group / row with a multiply (== fma onto an exact zero, without the zeroing instructions;
+// __dmul_rn keeps the compiler from contracting it with a later add)
+#define E0(OA, OB) { const double2 X = LD(s0 + OA), Y = LD(vc + OB); ax = __dmul_rn(X.x, Y.x); ay = __dmul_rn(X.y, Y.y); }
 #define E(OA, OB) { const double2 X = LD(s0 + OA), Y = LD(vc + OB); ax = fma(X.x, Y.x, ax); ay = fma(X.y, Y.y, ay); }
-#define GC(M) { tx = fma(M, ax, tx); ty = fma(M, ay, ty); ax = 0.0; ay = 0.0; }
-#define RV(D) { *(double2 *)(vw + D) = make_double2(tx, ty); tx = 0.0; ty = 0.0; }
-#define RL(S) { ex = fma(S, tx, ex); ey = fma(S, ty, ey); tx = 0.0; ty = 0.0; }
-#define RA(D) { double2 o = LD(ac + D); o.x += tx; o.y += ty; *(double2 *)(ac + D) = o; tx = 0.0; ty = 0.0; }
-#define RG(K) { if (n_ok > 0) Gcol[(long long)K * ldm] = tx; if (n_ok > 1) Gcol[(long long)K * ldm + 1] = ty; tx = 0.0; ty = 0.0; }
+#define G0(M) { tx = __dmul_rn(M, ax); ty = __dmul_rn(M, ay); }
+#define GC(M) { tx = fma(M, ax, tx); ty = fma(M, ay, ty); }
+#define RV(D) { *(double2 *)(vw + D) = make_double2(tx, ty); }
+#define RL(S) { ex = fma(S, tx, ex); ey = fma(S, ty, ey); }
+#define RA(D) { double2 o = LD(ac + D); o.x += tx; o.y += ty; *(double2 *)(ac + D) = o; }
+#define RG(K) { if (n_ok > 0) Gcol[(long long)K * ldm] = tx; if (n_ok > 1) Gcol[(long long)K * ldm + 1] = ty; }
 #else
 #define LD(p) (*(const double *)(p))
+#define E0(OA, OB) { ax = __dmul_rn(LD(s0 + OA), LD(vc + OB)); }
 #define E(OA, OB) { ax = fma(LD(s0 + OA), LD(vc + OB), ax); }
-#define GC(M) { tx = fma(M, ax, tx); ax = 0.0; }
-#define RV(D) { *(double *)(vw + D) = tx; tx = 0.0; }
-#define RL(S) { ex = fma(S, tx, ex); tx = 0.0; }
-#define RA(D) { *(double *)(ac + D) += tx; tx = 0.0; }
-#define RG(K) { if (n_ok > 0) Gcol[(long long)K * ldm] = tx; tx = 0.0; }
+#define G0(M) { tx = __dmul_rn(M, ax); }
+#define GC(M) { tx = fma(M, ax, tx); }
+#define RV(D) { *(double *)(vw + D) = tx; }
+#define RL(S) { ex = fma(S, tx, ex); }
+#define RA(D) { *(double *)(ac + D) += tx; }
+#define RG(K) { if (n_ok > 0) Gcol[(long long)K * ldm] = tx; }
 #endif
 
-extern "C" __global__ void __launch_bounds__(NT) k_tree_gen(const TreeArgs a) {
+extern "C" __global__ void __launch_bounds__(NT, 1) k_tree_gen(const TreeArgs a) {
   extern __shared__ __align__(16) char smraw[];
   double *val = (double *)smraw;
   double *adj = val + (size_t)a.n_val * A;
@@ -166,7 +172,6 @@ extern "C" __global__ void __launch_bounds__(NT) k_tree_gen(const TreeArgs a) {
         if (r < n_ok) Gcol[(long long)a.gzero_k[q] * ldm + r] = 0.0;
     {
       const char *s0 = ac;
-      ax = 0.0; ay = 0.0; tx = 0.0; ty = 0.0;
 @BWD@
     }
     __syncthreads();
@@ -197,13 +202,16 @@ std::string gen_pass(const std::vector<TreeTerm> &prog, const std::vector<int32_
       if (last < 0) continue;
       snprintf(buf, sizeof buf, "      case %d: {\n", l);
       out += buf;
+      bool acc_open = false, tot_open = false;      // does acc / tot hold a partial sum?
       for (int s = wave[w]; s <= last; ++s) {
         const TreeTerm &t = prog[(size_t)s * R + l];
-        snprintf(buf, sizeof buf, "E(%u,%u)", t.a & ~7u, t.b & ((1u << kTreeDstShift) - 1));
+        snprintf(buf, sizeof buf, "%s(%u,%u)", acc_open ? "E" : "E0", t.a & ~7u, t.b & ((1u << kTreeDstShift) - 1));
         out += buf;
+        acc_open = true;
         if (t.a & kTreeGroup) {
-          snprintf(buf, sizeof buf, "GC(%a)", t.mult);
+          snprintf(buf, sizeof buf, "%s(%a)", tot_open ? "GC" : "G0", t.mult);
           out += buf;
+          acc_open = false; tot_open = true;
           if (t.a & kTreeRow) {
             const unsigned d = t.b >> kTreeDstShift;
             if (!bwd) {
@@ -214,6 +222,7 @@ std::string gen_pass(const std::vector<TreeTerm> &prog, const std::vector<int32_
               else snprintf(buf, sizeof buf, "RA(%u)", d * row);
             }
             out += buf;
+            tot_open = false;
           }
         }
         out += "\n";
@@ -225,6 +234,11 @@ std::string gen_pass(const std::vector<TreeTerm> &prog, const std::vector<int32_
   return out;
 }
 }  // namespace
+
+// shared memory of the generated kernel: val + adj + energy partials [NT][AR]
+size_t tree_jit_smem_bytes(int n_val, int n_adj, int AR, int NT) {
+  return (((size_t)n_val + (size_t)n_adj) * 32 * AR * 8 + (size_t)NT * AR * 8 + 15) & ~(size_t)15;
+}
 
 struct TreeJit {
   cudaLibrary_t lib = nullptr;
@@ -243,8 +257,8 @@ TreeJit *tree_jit_build(const TreeSched &sc, int AL, int AR, std::string *why) {
   if (AL != 32) { *why = "codegen needs 32 atom-lanes"; return nullptr; }
   const Nvrtc &rt = nvrtc();
   if (!rt.ok) { *why = "NVRTC not found"; return nullptr; }
-  const int NT = tree_threads(AL), R = NT / AL;
-  if (sc.R != R || sc.A != AL * AR) { *why = "schedule shape mismatch"; return nullptr; }
+  const int R = sc.R, NT = R * AL;            // the schedule's row-lanes are this kernel's warps
+  if (NT > 1024 || sc.A != AL * AR) { *why = "schedule shape mismatch"; return nullptr; }
   std::string src = kFrame;
   replace_all(src, "@AR@", std::to_string(AR));
   replace_all(src, "@NT@", std::to_string(NT));
@@ -287,7 +301,7 @@ cudaError_t tree_jit_launch(const TreeJit *j, const TreeArgs &a, cudaStream_t st
   if (groups <= 0) return cudaSuccess;
   static int sms = 0;
   if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
-  const size_t smem = tree_smem_bytes(a.n_val, a.n_adj, 32, j->AR);
+  const size_t smem = tree_jit_smem_bytes(a.n_val, a.n_adj, j->AR, j->NT);
   int per_sm = (int)((227 * 1024) / (smem + 1024));
   per_sm = per_sm < 1 ? 1 : (per_sm > 2048 / j->NT ? 2048 / j->NT : per_sm);
   const int grid = groups < sms * per_sm ? groups : sms * per_sm;
