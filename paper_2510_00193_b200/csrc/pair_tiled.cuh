@@ -57,8 +57,8 @@ __device__ __forceinline__ void stage_positions(const PairArgs &a, const int4 w,
   for (int u = 0; u < 4; ++u) {
     if (ww[u] != -1) {
       const double *g = a.pos4 + 4 * (size_t)(ww[u] & kIdxMask);
-      asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s0 + 32 * u), "l"(g));
-      asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s0 + 32 * u + 16), "l"(g + 2));
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s0 + 1024 * u), "l"(g));           // slot (u, lane):
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s0 + 1024 * u + 16), "l"(g + 2));  // lanes 32 B apart
     }
   }
 }
@@ -139,7 +139,7 @@ __global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB1) k_moments_
   const int ka = (4 * lane) % TN;                  // phase A: this lane stages neighbours t0 + ka .. + 3 of atom slot sa
   double *mine = tile + sa * ROW;
   const double *slut = csm + a.n_species * a.n_species * a.crow;
-  double *pst = tile + NA * ROW + 4 * (4 * lane);            // this lane's four position slots (buffer 0)
+  double *pst = tile + NA * ROW + 4 * lane;                  // this lane's position slots: (u, lane) at + 128 u doubles
   int *wst = reinterpret_cast<int *>(tile + NA * ROW + 2 * 512) + 4 * lane;   // its four word slots (buffer 0)
   stage_words(a, beg, n_nb, ka, wst);
   stage_words(a, beg, n_nb, TN + ka, wst + 128);
@@ -161,7 +161,7 @@ __global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB1) k_moments_
     __syncwarp();
     PairGeo geo[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) geo[u] = load_pair(a, slut, jc[u], rec + 4 * u, xi, yi, zi);
+    for (int u = 0; u < 4; ++u) geo[u] = load_pair(a, slut, jc[u], rec + 128 * u, xi, yi, zi);
 #pragma unroll
     for (int u = 0; u < 4; ++u) stage_pair<NMU, false, PD, NB>(a, csm, geo[u], zi_s, rc2, mine + (ka + u) * PD);
     __syncwarp();
@@ -261,7 +261,7 @@ __global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB3) k_pairgrad
   const int ka = (4 * lane) % TN;
   double *mine = tile + sa * ROW;
   const double *slut = csm + a.n_species * a.n_species * a.crow;
-  double *pst = dtile + 128 * 4 + 4 * (4 * lane);            // this lane's four position slots (buffer 0)
+  double *pst = dtile + 128 * 4 + 4 * lane;                  // this lane's position slots: (u, lane) at + 128 u doubles
   int *wst = reinterpret_cast<int *>(dtile + 128 * 4 + 2 * 512) + 4 * lane;   // its four word slots (buffer 0)
   stage_words(a, beg, n_nb, ka, wst);
   stage_words(a, beg, n_nb, TN + ka, wst + 128);
@@ -284,7 +284,7 @@ __global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB3) k_pairgrad
     // ---- phase A
     PairGeo geo[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) geo[u] = load_pair(a, slut, jc[u], rec + 4 * u, xi, yi, zi);
+    for (int u = 0; u < 4; ++u) geo[u] = load_pair(a, slut, jc[u], rec + 128 * u, xi, yi, zi);
 #pragma unroll
     for (int u = 0; u < 4; ++u) stage_pair<NMU, true, PD, NB>(a, csm, geo[u], zi_s, rc2, mine + (ka + u) * PD);
     __syncwarp();
