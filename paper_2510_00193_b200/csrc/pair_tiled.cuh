@@ -57,8 +57,8 @@ __device__ __forceinline__ void stage_positions(const PairArgs &a, const int4 w,
   for (int u = 0; u < 4; ++u) {
     if (ww[u] != -1) {
       const double *g = a.pos4 + 4 * (size_t)(ww[u] & kIdxMask);
-      asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s0 + 1024 * u), "l"(g));           // slot (u, lane):
-      asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s0 + 1024 * u + 16), "l"(g + 2));  // lanes 32 B apart
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s0 + 1024 * u), "l"(g));            // slot (u, half, lane):
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s0 + 1024 * u + 512), "l"(g + 2));  // lanes 16 B apart
     }
   }
 }
@@ -71,7 +71,7 @@ __device__ __forceinline__ PairGeo load_pair(const PairArgs &a, const double *__
                                              double xi, double yi, double zi) {
   PairGeo g{0.0, 0.0, 0.0, -1};
   if (w != -1) {
-    const double2 p0 = *reinterpret_cast<const double2 *>(rec), p1 = *reinterpret_cast<const double2 *>(rec + 2);
+    const double2 p0 = *reinterpret_cast<const double2 *>(rec), p1 = *reinterpret_cast<const double2 *>(rec + 64);
     pair_vector(a, slut, (unsigned)w >> kIdxBits, xi, yi, zi, p0.x, p0.y, p1.x, g.x, g.y, g.z);
     g.zj = (int)p1.y;
   }
@@ -139,7 +139,7 @@ __global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB1) k_moments_
   const int ka = (4 * lane) % TN;                  // phase A: this lane stages neighbours t0 + ka .. + 3 of atom slot sa
   double *mine = tile + sa * ROW;
   const double *slut = csm + a.n_species * a.n_species * a.crow;
-  double *pst = tile + NA * ROW + 4 * lane;                  // this lane's position slots: (u, lane) at + 128 u doubles
+  double *pst = tile + NA * ROW + 2 * lane;                  // this lane's position slots: (u, half) at + 128 u + 64 half doubles
   int *wst = reinterpret_cast<int *>(tile + NA * ROW + 2 * 512) + 4 * lane;   // its four word slots (buffer 0)
   stage_words(a, beg, n_nb, ka, wst);
   stage_words(a, beg, n_nb, TN + ka, wst + 128);
@@ -261,7 +261,7 @@ __global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB3) k_pairgrad
   const int ka = (4 * lane) % TN;
   double *mine = tile + sa * ROW;
   const double *slut = csm + a.n_species * a.n_species * a.crow;
-  double *pst = dtile + 128 * 4 + 4 * lane;                  // this lane's position slots: (u, lane) at + 128 u doubles
+  double *pst = dtile + 128 * 4 + 2 * lane;                  // this lane's position slots: (u, half) at + 128 u + 64 half doubles
   int *wst = reinterpret_cast<int *>(dtile + 128 * 4 + 2 * 512) + 4 * lane;   // its four word slots (buffer 0)
   stage_words(a, beg, n_nb, ka, wst);
   stage_words(a, beg, n_nb, TN + ka, wst + 128);
