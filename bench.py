@@ -328,7 +328,7 @@ def main():
     ap.add_argument("--chunk", type=int, default=-1)
     ap.add_argument("--force-mode", type=int, default=-1)
     ap.add_argument("--grade", action="store_true", help="also run mtp_grade each step (config 4)")
-    ap.add_argument("--ref-atoms", type=int, default=1024, help="atoms per oracle sample")
+    ap.add_argument("--ref-atoms", type=int, default=8192, help="atoms per oracle sample (about 12 s of CPU work)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -207,3 +207,70 @@ def test_large_launch_configuration_on_sampled_atoms(lib, torch):
         sF = max(1.0, np.abs(d[rows]).sum() + np.abs(d[w.rev[rows]]).sum())
         assert np.all(np.abs(got["F"][k] - Fk) <= TOL_F * sF)
     assert np.all(np.abs(got["F"].sum(axis=0)) <= 1e-9 * np.abs(got["F"]).sum())
+
+
+def _check_sampled(w, got, n_sample, seed):
+    """E_i and F_k of sampled atoms against the oracle (the oracle evaluates the sampled atoms and their neighbours)."""
+    opot = oracle_pot(w)
+    rng = np.random.default_rng(seed)
+    sample = [int(x) for x in rng.choice(w.n_atoms, n_sample, replace=False)]
+    need = set(sample)
+    for k in sample:
+        need.update(int(j) for j in w.idx[w.off[k]:w.off[k + 1]])
+    ref = omtp.evaluate(opot, w.pos, w.types, w.box, w.off, w.idx, w.shift, atoms=sorted(need))
+    d = ref["d"]
+    for k in sample:
+        sE = max(1.0, np.abs(ref["B"][k] * w.xi).sum())
+        assert abs(got["Ei"][k] - ref["E_i"][k]) <= TOL_E * sE
+        rows = np.arange(w.off[k], w.off[k + 1])
+        Fk = d[rows].sum(axis=0) - d[w.rev[rows]].sum(axis=0)
+        sF = max(1.0, np.abs(d[rows]).sum() + np.abs(d[w.rev[rows]]).sum())
+        assert np.all(np.abs(got["F"][k] - Fk) <= TOL_F * sF)
+    assert np.all(np.abs(got["F"].sum(axis=0)) <= 1e-9 * np.abs(got["F"]).sum())
+
+
+def test_full_size_config4_sampled(lib, torch):
+    """BASELINE.json configs[3] at full size (1,048,576 atoms, level 16), default options = what bench.py times."""
+    w = make_workload(3, n_basis_of(16))
+    got, pot, _ = run_gpu(lib, torch, w)
+    pot.close()
+    assert w.n_atoms == 1048576
+    _check_sampled(w, got, 4, 11)
+
+
+def test_full_size_config3_sampled(lib, torch):
+    """BASELINE.json configs[2] at full size (54,000 atoms, 2 species, level 20)."""
+    w = make_workload(2, n_basis_of(20))
+    got, pot, _ = run_gpu(lib, torch, w)
+    pot.close()
+    assert w.n_atoms == 54000
+    _check_sampled(w, got, 2, 12)
+
+
+def test_full_size_config5_sampled_energy_and_grades(lib, torch):
+    """BASELINE.json configs[4] at full size (250,000 atoms, level 24): E_i, B and both grade modes on sampled atoms."""
+    nb = n_basis_of(24)
+    w = make_workload(4, nb)
+    assert w.n_atoms == 250000 and w.Ainv is not None
+    opot = oracle_pot(w)
+    sample = [3, 124999, 249998]
+    ref = omtp.evaluate(opot, w.pos, w.types, w.box, w.off, w.idx, w.shift, atoms=sample, want_grad=False)
+    pot = gpu_pot(lib, w)
+    d = to_dev(w, torch)
+    out = pot.compute(d["pos"], d["types"], w.box, d["off"], d["idx"], d["shift"], d["rev"])
+    Ainv = torch.as_tensor(w.Ainv).cuda()
+    g = pot.grade(d["pos"], d["types"], w.box, d["off"], d["idx"], Ainv, d["shift"], mode=2)
+    torch.cuda.synchronize()
+    Ei = out["Ei"].cpu().numpy()
+    ga = g["gamma_atom"].cpu().numpy()
+    want = omtp.grade_neighbourhood(ref["B"][sample], w.Ainv)
+    for q, k in enumerate(sample):
+        sE = max(1.0, np.abs(ref["B"][k] * w.xi).sum())
+        assert abs(Ei[k] - ref["E_i"][k]) <= TOL_E * sE
+        assert ga[k] == pytest.approx(want[q], rel=TOL_G)
+    F = out["F"].cpu().numpy()
+    assert np.all(np.abs(F.sum(axis=0)) <= 1e-9 * np.abs(F).sum())
+    # configuration mode: property that holds at any size -- gamma_cfg = max_k |Bsum . Ainv[:, k]| of the returned Bsum
+    Bsum = g["Bsum"].cpu().numpy()
+    assert g["gamma_cfg"].cpu().numpy()[0] == pytest.approx(np.abs(Bsum @ w.Ainv).max(), rel=TOL_G)
+    pot.close()
