@@ -428,6 +428,8 @@ int fill_tree_args(mtp_handle *h, TreeArgs &ta, const double *pos4, const Plan &
   ta.gzero_k = td->d_gzero_k; ta.n_gzero = (int)sc.gzero_k.size();
   ta.n_val = sc.n_val; ta.n_adj = sc.n_adj; ta.n_basic = h->n_basic; ta.n_basis = h->n_basis;
   ta.B = nullptr; ta.want_adj = 1;
+  ta.mload_k = nullptr; ta.cut_row = ta.cut_vslot = ta.cut_aslot = nullptr; ta.n_cut = 0;
+  ta.S = nullptr; ta.Sbar = nullptr; ta.g_accum = 0; ta.write_energy = 1;
   return MTP_OK;
 }
 }  // namespace

@@ -32,6 +32,13 @@ struct TreeArgs {
   int n_val, n_adj, n_basic, n_basis;
   int c0, c1;
   int want_adj;
+  // sub-programs of a partitioned tree (tree_partition.cpp); all null / 0 / 1 for a whole table
+  const int *mload_k;                      // [n_basic] row of M / G per local packed moment, or null = identity
+  const int *cut_row, *cut_vslot, *cut_aslot; int n_cut;   // the group's cut nodes: row in S / Sbar, val slot, adj slot
+  double *S;                               // [n_cut_rows][ldm] cut values out (after the forward pass), or null
+  const double *Sbar;                      // [n_cut_rows][ldm] dE_i/d(cut) in (seeds of the backward pass), or null
+  int g_accum;                             // 1: G[k] += (groups accumulate), 0: G[k] =
+  int write_energy;                        // 0: group programs leave E_i alone
 };
 void tree_pick_shape(int n_val, int n_adj, long long n_atoms, int *AL, int *AR);   // AL = 0: does not fit
 int tree_threads(int AL);               // CTA size used with AL atom-lanes

@@ -55,14 +55,19 @@ struct TreeSched {
   std::vector<int32_t> gseed_k;        // packed moments that are basis functions: G[k] += gseed_val
   std::vector<double> gseed_val;
   std::vector<int32_t> gzero_k;        // packed moments no op reads: G[k] = 0
+  // sub-programs of a partitioned tree (tree_partition.cpp)
+  std::vector<int32_t> mload_k;        // [n_basic] row of M / G each local packed moment stands for (empty: identity)
+  std::vector<int32_t> cut_val_slot, cut_adj_slot;   // storage of the cut nodes, in the caller's order
   long long n_prod = 0;
   long long fsteps = 0, bsteps = 0;    // schedule length (steps per row-lane), for the cost report
 };
 
-void tree_count_slots(int n_basic, int n_nodes, int n_prod, const int32_t *prod, bool elide, int *n_val, int *n_adj);
-// returns 0 or a negative MTP_E* code; err receives a message
+void tree_count_slots(int n_basic, int n_nodes, int n_prod, const int32_t *prod, bool elide, int *n_val, int *n_adj,
+                      const int32_t *cut_nodes = nullptr, int n_cut = 0);
+// returns 0 or a negative MTP_E* code; err receives a message.  basic_map / cut_nodes describe a sub-program of a
+// partitioned tree: local packed moment n stands for row basic_map[n] of M and G, cut_nodes are its outputs.
 int tree_compile(int n_basic, int n_nodes, int n_prod, const int32_t *prod, int n_basis,
                  const int32_t *basis_node, const double *xi, int A, int R, bool elide, TreeSched &out,
-                 const char **err);
+                 const char **err, const int32_t *basic_map = nullptr, const int32_t *cut_nodes = nullptr, int n_cut = 0);
 
 }  // namespace mtpb

@@ -16,8 +16,10 @@ constexpr int kTinyWaveTerms = 16;               // a wave this small may join a
 constexpr int kTinyChainTerms = 48;              // upper bound on a merged chain
 }  // namespace
 
-void tree_count_slots(int n_basic, int n_nodes, int n_prod, const int32_t *prod, bool elide, int *n_val, int *n_adj) {
+void tree_count_slots(int n_basic, int n_nodes, int n_prod, const int32_t *prod, bool elide, int *n_val, int *n_adj,
+                      const int32_t *cut_nodes, int n_cut) {
   std::vector<char> is_read(n_nodes, 0);
+  for (int q = 0; q < n_cut; ++q) is_read[cut_nodes[q]] = 1;      // a cut node is stored like a node some op reads
   for (int t = 0; t < n_prod; ++t)
     for (int q = 0; q < 2; ++q) { const int n = prod[4 * t + q]; if (n >= 0 && n < n_nodes) is_read[n] = 1; }
   int nv = 0, na = 1;
@@ -31,7 +33,8 @@ void tree_count_slots(int n_basic, int n_nodes, int n_prod, const int32_t *prod,
 
 int tree_compile(int n_basic, int n_nodes, int n_prod, const int32_t *prod, int n_basis,
                  const int32_t *basis_node, const double *xi, int A, int R, bool elide, TreeSched &s,
-                 const char **err) {
+                 const char **err, const int32_t *basic_map, const int32_t *cut_nodes, int n_cut) {
+  const bool group = n_cut > 0;       // sub-program of a partitioned tree (tree_partition.cpp): no constant seeds
   static const char *e_range = "contraction table: node index out of range";
   static const char *e_order = "contraction table: a node is read before its last write";
   static const char *e_mult = "contraction table: negative multiplicity";
@@ -68,6 +71,12 @@ int tree_compile(int n_basic, int n_nodes, int n_prod, const int32_t *prod, int 
   // ---- storage slots.  is_read[n]: some op has n as a factor.
   std::vector<char> is_read(n_nodes, 0);
   for (int t = 0; t < n_prod; ++t) { is_read[prod[4 * t]] = 1; is_read[prod[4 * t + 1]] = 1; }
+  // cut nodes of a group are its outputs: their values are exported and their adjoints come in per atom,
+  // so they are stored exactly like nodes some op reads
+  for (int q = 0; q < n_cut; ++q) {
+    if (cut_nodes[q] < n_basic || cut_nodes[q] >= n_nodes) { *err = e_range; return MTP_EINVAL; }
+    is_read[cut_nodes[q]] = 1;
+  }
   s.val_slot.assign(n_nodes, -1);
   std::vector<int> adj_slot(n_nodes, -1), leaf_id(n_nodes, -1);
   int nv = 0, na = 1;                                   // adj slot 0 holds the constant 1
@@ -184,7 +193,7 @@ int tree_compile(int n_basic, int n_nodes, int n_prod, const int32_t *prod, int 
     for (int n = 0; n < n_nodes; ++n) {
       if (brow[n].terms.empty()) continue;
       has_brow[n] = 1;
-      if (n < n_basic) { brow[n].dst = (uint32_t)n; brow[n].alt = 1; }
+      if (n < n_basic) { brow[n].dst = (uint32_t)(basic_map ? basic_map[n] : n); brow[n].alt = 1; }
       else { brow[n].dst = (uint32_t)adj_slot[n]; brow[n].alt = 0; }
       waves[D - depth[n]].push_back(std::move(brow[n]));   // deepest sources first
     }
@@ -193,10 +202,13 @@ int tree_compile(int n_basic, int n_nodes, int n_prod, const int32_t *prod, int 
   s.fsteps = s.fwave.back(); s.bsteps = s.bwave.back();
   // the kernel prefetches up to 4 * kTreePrefetch steps ahead: pad so that those reads stay in bounds
   for (int q = 0; q < 4 * kTreePrefetch * R; ++q) { s.fprog.push_back(TreeTerm{0, 0, 0.0}); s.bprog.push_back(TreeTerm{0, 0, 0.0}); }
-  for (int k = 0; k < n_basic; ++k) {
-    if (seeded[k]) { s.gseed_k.push_back(k); s.gseed_val.push_back(seed[k]); }
-    if (!has_brow[k]) s.gzero_k.push_back(k);
-  }
+  if (!group)
+    for (int k = 0; k < n_basic; ++k) {
+      if (seeded[k]) { s.gseed_k.push_back(k); s.gseed_val.push_back(seed[k]); }
+      if (!has_brow[k]) s.gzero_k.push_back(k);
+    }
+  if (basic_map) s.mload_k.assign(basic_map, basic_map + n_basic);
+  for (int q = 0; q < n_cut; ++q) { s.cut_val_slot.push_back(s.val_slot[cut_nodes[q]]); s.cut_adj_slot.push_back(adj_slot[cut_nodes[q]]); }
   return MTP_OK;
 }
 

@@ -75,6 +75,12 @@ struct TreeArgs {
   int n_val, n_adj, n_basic, n_basis;
   int c0, c1;
   int want_adj;
+  const int *mload_k;                      // the fields below serve group sub-programs, which are interpreted
+  const int *cut_row, *cut_vslot, *cut_aslot; int n_cut;
+  double *S;
+  const double *Sbar;
+  int g_accum;
+  int write_energy;
 };
 #define AR @AR@
 #define NT @NT@

@@ -40,7 +40,7 @@ template <int AL, int AR, int R, bool BWD, bool PS>
 __device__ __forceinline__ void run_pass(const int4 *__restrict__ prog, const int *__restrict__ wave, int n_waves,
                                          int rl, const char *__restrict__ val, char *adj, char *valw,
                                          const double *__restrict__ leaf_seed, Vec<AR> &e,
-                                         double *__restrict__ Gcol, long long ldm, int n_ok) {
+                                         double *__restrict__ Gcol, long long ldm, int n_ok, bool g_accum) {
   constexpr int BL = kTreePrefetch;            // block: entries between two wave-boundary checks
   constexpr int NB = PS ? 1 : 4;               // blocks in the queue: 4 entries ahead from shared memory, 16 from L2
   constexpr int PF = BL * NB;
@@ -90,7 +90,10 @@ __device__ __forceinline__ void run_pass(const int4 *__restrict__ prog, const in
             } else if (t.x & (int)kTreeAlt) {
 #pragma unroll
               for (int r = 0; r < AR; ++r)
-                if (r < n_ok) Gcol[(long long)d * ldm + r] = tot.v[r];
+                if (r < n_ok) {
+                  double *gp = Gcol + (long long)d * ldm + r;
+                  *gp = g_accum ? *gp + tot.v[r] : tot.v[r];
+                }
             } else {
               char *qd = adj + d * ROW;               // adj was initialised with the node's seed
               Vec<AR> old = lds<AR>(qd);
@@ -140,7 +143,7 @@ __global__ void __launch_bounds__(NT) k_tree(const TreeArgs a) {
     for (int k = rl; k < a.n_basic; k += R) {
       Vec<AR> m;
 #pragma unroll
-      for (int r = 0; r < AR; ++r) m.v[r] = r < n_ok ? a.M[(long long)k * a.ldm + col + r] : 0.0;
+      for (int r = 0; r < AR; ++r) m.v[r] = r < n_ok ? a.M[(long long)(a.mload_k ? a.mload_k[k] : k) * a.ldm + col + r] : 0.0;
       sts<AR>(const_cast<char *>(valc) + (size_t)k * A * 8, m);
     }
     if (a.want_adj)
@@ -150,12 +153,21 @@ __global__ void __launch_bounds__(NT) k_tree(const TreeArgs a) {
         for (int r = 0; r < AR; ++r) s.v[r] = a.adj_init[k];
         sts<AR>(adjc + (size_t)k * A * 8, s);
       }
+    if (a.want_adj && a.Sbar) {              // per-atom seeds of a group's cut nodes (after the constant init)
+      __syncthreads();
+      for (int q = rl; q < a.n_cut; q += R) {
+        Vec<AR> s;
+#pragma unroll
+        for (int r = 0; r < AR; ++r) s.v[r] = r < n_ok ? a.Sbar[(long long)a.cut_row[q] * a.ldm + col + r] : 0.0;
+        sts<AR>(adjc + (size_t)a.cut_aslot[q] * A * 8, s);
+      }
+    }
     __syncthreads();
     Vec<AR> e;
 #pragma unroll
     for (int r = 0; r < AR; ++r) e.v[r] = 0.0;
     run_pass<AL, AR, R, false, PS>(fprog, fw, a.nfw, rl, valc, nullptr, const_cast<char *>(valc), a.leaf_seed, e, nullptr,
-                                   0, n_ok);
+                                   0, n_ok, false);
     // ---- energy (stored basis nodes here, elided leaves were added inside the waves) and basis values
     {
       for (int q = rl; q < a.n_eseed; q += R) {
@@ -174,7 +186,14 @@ __global__ void __launch_bounds__(NT) k_tree(const TreeArgs a) {
         }
       }
       __syncthreads();
-      if (rl == 0) {                             // fixed-order reduction over the R row-lanes
+      if (a.S)                                   // cut values of a group: exported for the top program
+        for (int q = rl; q < a.n_cut; q += R) {
+          const Vec<AR> v = lds<AR>(valc + (size_t)a.cut_vslot[q] * A * 8);
+#pragma unroll
+          for (int r = 0; r < AR; ++r)
+            if (r < n_ok) a.S[(long long)a.cut_row[q] * a.ldm + col + r] = v.v[r];
+        }
+      if (rl == 0 && a.write_energy) {           // fixed-order reduction over the R row-lanes
 #pragma unroll
         for (int r = 0; r < AR; ++r) {
           if (r < n_ok) {
@@ -192,7 +211,7 @@ __global__ void __launch_bounds__(NT) k_tree(const TreeArgs a) {
 #pragma unroll
       for (int r = 0; r < AR; ++r)
         if (r < n_ok) Gcol[(long long)a.gzero_k[q] * a.ldm + r] = 0.0;
-    run_pass<AL, AR, R, true, PS>(bprog, bw, a.nbw, rl, valc, adjc, nullptr, nullptr, e, Gcol, a.ldm, n_ok);
+    run_pass<AL, AR, R, true, PS>(bprog, bw, a.nbw, rl, valc, adjc, nullptr, nullptr, e, Gcol, a.ldm, n_ok, a.g_accum != 0);
     __syncthreads();
     // packed moments that are basis functions themselves (M_{mu,0}): G += xi
     for (int q = rl; q < a.n_gseed; q += R)
