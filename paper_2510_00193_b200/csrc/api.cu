@@ -15,6 +15,7 @@
 #include "kernels.h"
 #include "mtp_b200.h"
 #include "stair.h"
+#include "tree_partition.h"
 
 using namespace mtpb;
 
@@ -47,14 +48,27 @@ struct mtp_handle {
     int *d_fwave = nullptr, *d_bwave = nullptr, *d_gseed_k = nullptr, *d_gzero_k = nullptr;
     int *d_eseed_slot = nullptr, *d_basis_slot = nullptr;
     double *d_adj_init = nullptr, *d_gseed_val = nullptr, *d_leaf_seed = nullptr, *d_eseed_val = nullptr;
+    int *d_mload_k = nullptr, *d_cut_row = nullptr, *d_cut_vslot = nullptr, *d_cut_aslot = nullptr;
     TreeJit *jit = nullptr;                    // specialised kernel (tree_jit.cpp), null = interpreter
     std::string jit_note;
   };
+  // A table the K2 kernels can run: the whole table, or -- when that leaves too few atoms per CTA -- the top
+  // program and the group programs of its partition (tree_partition.cpp).  Host copies feed the compilations.
+  struct Prog {
+    int n_basic = 0, n_nodes = 0, n_basis = 0;
+    std::vector<int32_t> prod, basis_node;
+    std::vector<double> xi;
+    std::vector<int32_t> basic_map, cut_local, cut_row;   // group programs only
+    int slots[2][2] = {{0, 0}, {0, 0}};        // [elide][n_val, n_adj]
+    std::map<int, TreeDev> trees;              // key: AL * 8 + AR * 2 + elide
+    int n_prod() const { return (int)(prod.size() / 4); }
+    bool is_group() const { return !cut_local.empty(); }
+  };
   int codegen = 1;                             // MTP_OPT_TREE_CODEGEN
-  std::map<int, TreeDev> trees;                // key: AL * 8 + AR * 2 + elide
-  int slots[2][2] = {{0, 0}, {0, 0}};          // [elide][n_val, n_adj]
-  std::vector<int32_t> t_prod, t_basis_node;   // host copy of the table for those compilations
-  std::vector<double> t_xi;
+  std::vector<Prog> progs;                     // [0] whole table; partitioned: [1] top, [2..] groups
+  bool partitioned = false;
+  int n_cut_rows = 0;                          // rows of the cut-value arrays S / dE/dS
+  int *d_gmap = nullptr;                       // [n_basic] cut row of a packed moment that is a cut node itself, else -1
   long long n_prod = 0;
   int64_t chunk_atoms = 0;
   int force_mode = MTP_FORCE_AUTO, variant = MTP_VARIANT_AUTO;
@@ -153,33 +167,31 @@ static void build_kmaps(const PairLevel &pl, int n_basic, const int32_t *basic, 
   }
 }
 
-// K2 schedule for a CTA shape (AL, AR) and leaf elision on/off: compiled from the host copy of the
-// table and uploaded on first use
-static int get_tree(mtp_handle *h, int AL, int AR, bool elide, const mtp_handle::TreeDev **out) {
+// K2 schedule of one program for a CTA shape (AL, AR) and leaf elision on/off: compiled from the host copy
+// of its table and uploaded on first use
+static int get_tree(mtp_handle *h, mtp_handle::Prog &pg, int AL, int AR, bool elide, const mtp_handle::TreeDev **out) {
   if (AL <= 0) return fail(h, MTP_EUNSUP, "contraction tree does not fit in shared memory");
   const int key = AL * 8 + AR * 2 + (elide ? 1 : 0);
-  auto it = h->trees.find(key);
-  if (it != h->trees.end()) { *out = &it->second; return MTP_OK; }
+  auto it = pg.trees.find(key);
+  if (it != pg.trees.end()) { *out = &it->second; return MTP_OK; }
   mtp_handle::TreeDev td;
   const char *terr = "";
-  int rc = MTP_OK;
-  // First choice: the kernel specialised for this table (tree_jit.cpp), same schedule as the interpreter
-  // (so the two are bit-identical), when the table is short enough to be worth compiling and the shape has
-  // 32 atom-lanes.  (32 row-lane warps instead of 16 were measured slower: the generated code is bound by
-  // instruction fetch, not by per-warp latency.)
+  const bool group = pg.is_group();
+  auto compile = [&]() {
+    return tree_compile(pg.n_basic, pg.n_nodes, pg.n_prod(), pg.prod.data(), pg.n_basis, pg.basis_node.data(), pg.xi.data(),
+                        AL * AR, tree_row_lanes(AL), elide, td.sched, &terr, group ? pg.basic_map.data() : nullptr,
+                        group ? pg.cut_local.data() : nullptr, (int)pg.cut_local.size());
+  };
+  int rc = compile();
+  if (rc != MTP_OK) return fail(h, rc, terr);
+  // The kernel specialised for this table (tree_jit.cpp) runs the same schedule as the interpreter (so the two
+  // are bit-identical); built when the table is short enough to be worth compiling and the shape has 32
+  // atom-lanes.  (32 row-lane warps instead of 16 were measured slower: the generated code is bound by
+  // instruction fetch, not by per-warp latency.)  Group programs are interpreted.
   const char *env = getenv("MTP_TREE_CODEGEN");
-  if (h->codegen && !(env && env[0] == '0') && AL == 32 && 3LL * h->n_prod <= 60000 &&
-      tree_jit_smem_bytes(h->slots[elide][0], h->slots[elide][1], AR, tree_threads(AL)) <= 225 * 1024) {
-    rc = tree_compile(h->n_basic, h->n_nodes, (int)h->n_prod, h->t_prod.data(), h->n_basis, h->t_basis_node.data(),
-                      h->t_xi.data(), AL * AR, tree_row_lanes(AL), elide, td.sched, &terr);
-    if (rc != MTP_OK) return fail(h, rc, terr);
+  if (h->codegen && !(env && env[0] == '0') && !group && AL == 32 && 3LL * pg.n_prod() <= 60000 &&
+      tree_jit_smem_bytes(td.sched.n_val, td.sched.n_adj, AR, tree_threads(AL)) <= 225 * 1024)
     td.jit = tree_jit_build(td.sched, AL, AR, &td.jit_note);
-  }
-  if (!td.jit) {
-    rc = tree_compile(h->n_basic, h->n_nodes, (int)h->n_prod, h->t_prod.data(), h->n_basis, h->t_basis_node.data(),
-                      h->t_xi.data(), AL * AR, tree_row_lanes(AL), elide, td.sched, &terr);
-    if (rc != MTP_OK) return fail(h, rc, terr);
-  }
   cudaError_t e = cudaSuccess;
   auto up = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
   const TreeSched &sc = td.sched;
@@ -195,8 +207,14 @@ static int get_tree(mtp_handle *h, int AL, int AR, bool elide, const mtp_handle:
   up(upload(h, &td.d_gseed_k, sc.gseed_k.data(), sc.gseed_k.size()));
   up(upload(h, &td.d_gseed_val, sc.gseed_val.data(), sc.gseed_val.size()));
   up(upload(h, &td.d_gzero_k, sc.gzero_k.data(), sc.gzero_k.size()));
+  if (group) {
+    up(upload(h, &td.d_mload_k, sc.mload_k.data(), sc.mload_k.size()));
+    up(upload(h, &td.d_cut_row, pg.cut_row.data(), pg.cut_row.size()));
+    up(upload(h, &td.d_cut_vslot, sc.cut_val_slot.data(), sc.cut_val_slot.size()));
+    up(upload(h, &td.d_cut_aslot, sc.cut_adj_slot.data(), sc.cut_adj_slot.size()));
+  }
   if (e != cudaSuccess) return cuda_fail(h, e, "tree schedule upload");
-  auto ins = h->trees.emplace(key, std::move(td));
+  auto ins = pg.trees.emplace(key, std::move(td));
   *out = &ins.first->second;
   return MTP_OK;
 }
@@ -222,7 +240,7 @@ extern "C" void mtp_destroy(mtp_handle *h) {
   if (!h) return;
   for (auto &s : h->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
   for (auto e : h->pool) cudaEventDestroy(e);
-  for (auto &kv : h->trees) tree_jit_destroy(kv.second.jit);
+  for (auto &pg : h->progs) for (auto &kv : pg.trees) tree_jit_destroy(kv.second.jit);
   for (void *p : h->to_free) cudaFree(p);
   if (h->stage) cudaFree(h->stage);
   delete h;
@@ -256,17 +274,60 @@ extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
   h->n_nodes = p->n_nodes; h->n_basis = p->n_basis; h->lev_max = p->lev_max; h->r_min = p->r_min; h->r_cut = p->r_cut;
   h->pl = pair_level(li);
   h->n_prod = p->n_prod;
-  h->t_prod.assign(p->prod, p->prod + 4 * (size_t)p->n_prod);
-  h->t_basis_node.assign(p->basis_node, p->basis_node + p->n_basis);
-  h->t_xi.assign(p->xi, p->xi + p->n_basis);
-  for (int el = 0; el < 2; ++el) {
-    tree_count_slots(p->n_basic, p->n_nodes, p->n_prod, p->prod, el != 0, &h->slots[el][0], &h->slots[el][1]);
+  {
+    auto slots_of = [](mtp_handle::Prog &g) {
+      for (int el = 0; el < 2; ++el)
+        tree_count_slots(g.n_basic, g.n_nodes, g.n_prod(), g.prod.data(), el != 0, &g.slots[el][0], &g.slots[el][1],
+                         g.cut_local.data(), (int)g.cut_local.size());
+    };
+    h->progs.emplace_back();
+    mtp_handle::Prog &whole = h->progs.back();
+    whole.n_basic = p->n_basic; whole.n_nodes = p->n_nodes; whole.n_basis = p->n_basis;
+    whole.prod.assign(p->prod, p->prod + 4 * (size_t)p->n_prod);
+    whole.basis_node.assign(p->basis_node, p->basis_node + p->n_basis);
+    whole.xi.assign(p->xi, p->xi + p->n_basis);
+    slots_of(whole);
     int AL = 0, AR = 1;
-    tree_pick_shape(h->slots[el][0], h->slots[el][1], 0, &AL, &AR);
-    if (AL == 0) {
-      delete h;
-      return fail(nullptr, MTP_EUNSUP, "contraction tree does not fit in shared memory (one atom's node values and adjoints > 225 KB)");
+    tree_pick_shape(whole.slots[1][0], whole.slots[1][1], 0, &AL, &AR);
+    // Too few atoms per CTA (lev_max >= 20): cut the table into a top program and group programs that each fit
+    // 64 (else 32) atoms per CTA.  Budgets = shared-memory slots per atom left beside the energy partials.
+    const char *penv = getenv("MTP_TREE_PARTITION");
+    if (AL < 32 && !(penv && penv[0] == '0')) {
+      TreePartition part;
+      bool ok = tree_partition(p->n_basic, p->n_nodes, p->n_prod, p->prod, p->n_basis, p->basis_node, 430, part);
+      if (!ok || part.groups.size() > 24)
+        ok = tree_partition(p->n_basic, p->n_nodes, p->n_prod, p->prod, p->n_basis, p->basis_node, 870, part);
+      if (ok) {
+        h->partitioned = true;
+        h->n_cut_rows = (int)part.cut_node.size();
+        h->progs.emplace_back();
+        {
+          mtp_handle::Prog &top = h->progs.back();
+          top.n_basic = part.top.n_basic; top.n_nodes = part.top.n_nodes; top.n_basis = p->n_basis;
+          top.prod = part.top.prod; top.basis_node = part.top.basis_node;
+          top.xi.assign(p->xi, p->xi + p->n_basis);
+          slots_of(top);
+        }
+        for (auto &g : part.groups) {
+          h->progs.emplace_back();
+          mtp_handle::Prog &pg = h->progs.back();
+          pg.n_basic = g.table.n_basic; pg.n_nodes = g.table.n_nodes; pg.n_basis = 0;
+          pg.prod = g.table.prod; pg.basic_map = g.basic_map; pg.cut_local = g.cut_local; pg.cut_row = g.cut_row;
+          slots_of(pg);
+        }
+        std::vector<int> gmap(p->n_basic, -1);
+        for (size_t q = 0; q < part.cut_basic_k.size(); ++q) gmap[part.cut_basic_k[q]] = part.cut_basic_row[q];
+        if (upload(h, &h->d_gmap, gmap.data(), gmap.size()) != cudaSuccess) { mtp_destroy(h); return fail(nullptr, MTP_ECUDA, "mtp_create upload"); }
+      }
     }
+    for (size_t q = h->partitioned ? 1 : 0; q < h->progs.size(); ++q)
+      for (int el = 0; el < 2; ++el) {
+        tree_pick_shape(h->progs[q].slots[el][0], h->progs[q].slots[el][1], 0, &AL, &AR);
+        if (AL == 0) {
+          mtp_destroy(h);
+          return fail(nullptr, MTP_EUNSUP, "contraction tree does not fit in shared memory (one atom's node values and adjoints > 225 KB)");
+        }
+      }
   }
   // radial coefficients: blocks (z_i, z_j) laid out [beta][NMUP], NMUP = the level's n_mu rounded up to even
   // (16-byte pairs); +2 doubles per block spread the blocks over the banks
@@ -287,11 +348,12 @@ extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
   up(upload(h, &h->d_kmapB, kb.data(), kb.size()));
   up(upload(h, &h->d_basis_node, p->basis_node, (size_t)p->n_basis));
   if (e != cudaSuccess) { int r = cuda_fail(nullptr, e, "mtp_create upload"); mtp_destroy(h); return r; }
-  {   // validate the table and build the large-system schedule now, so that errors surface at create
+  // validate the table(s) and build the large-system schedules now, so that errors surface at create
+  for (size_t q = h->partitioned ? 1 : 0; q < h->progs.size(); ++q) {
     const mtp_handle::TreeDev *td = nullptr;
     int AL = 0, AR = 1;
-    tree_pick_shape(h->slots[1][0], h->slots[1][1], 0, &AL, &AR);
-    int rc = get_tree(h, AL, AR, true, &td);
+    tree_pick_shape(h->progs[q].slots[1][0], h->progs[q].slots[1][1], 0, &AL, &AR);
+    int rc = get_tree(h, h->progs[q], AL, AR, true, &td);
     if (rc != MTP_OK) { g_create_error = h->err; mtp_destroy(h); return rc; }
   }
   *out = h;
@@ -307,8 +369,10 @@ extern "C" int mtp_set_option(mtp_handle *h, int key, int64_t v) {
     case MTP_OPT_PROFILE: h->profile = v != 0; return MTP_OK;
     case MTP_OPT_TREE_CODEGEN:
       if (h->codegen != (v != 0)) {          // schedules are cached with or without their specialised kernel
-        for (auto &kv : h->trees) { tree_jit_destroy(kv.second.jit); kv.second.jit = nullptr; }
-        if (v != 0) h->trees.clear();        // device arrays stay owned by the handle (to_free)
+        for (auto &pg : h->progs) {
+          for (auto &kv : pg.trees) { tree_jit_destroy(kv.second.jit); kv.second.jit = nullptr; }
+          if (v != 0) pg.trees.clear();      // device arrays stay owned by the handle (to_free)
+        }
       }
       h->codegen = v != 0; return MTP_OK;
   }
@@ -324,7 +388,7 @@ extern "C" int mtp_get_option(const mtp_handle *h, int key, int64_t *v) {
     case MTP_OPT_TREE_CODEGEN: *v = h->codegen; return MTP_OK;
     case MTP_INFO_TREE_KERNELS: {             // specialised K2 kernels in use
       int n = 0;
-      for (auto &kv : h->trees) n += kv.second.jit != nullptr;
+      for (auto &pg : h->progs) for (auto &kv : pg.trees) n += kv.second.jit != nullptr;
       *v = n; return MTP_OK;
     }
   }
@@ -336,7 +400,7 @@ namespace {
 struct Plan {
   int64_t N = 0, nnz = 0, C = 0, ldm = 0;
   int n_chunks = 0, P = 1, atomic = 0, grid_chunk = 0, AL = 0, AR = 1, elide = 1;
-  size_t o_pos4 = 0, o_Ei = 0, o_M = 0, o_G = 0, o_wpart = 0, o_d4 = 0, o_B = 0, o_part = 0, o_red = 0, o_idxp = 0, total = 0;
+  size_t o_pos4 = 0, o_Ei = 0, o_M = 0, o_G = 0, o_wpart = 0, o_d4 = 0, o_B = 0, o_part = 0, o_red = 0, o_idxp = 0, o_S = 0, o_Sbar = 0, total = 0;
 };
 size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
@@ -362,7 +426,7 @@ int make_plan(const mtp_handle *h, int64_t N, int64_t nnz, int want_grade, int h
   else if (h->variant == MTP_VARIANT_BLOCK) pl.P = h->pl->p_small;
   else pl.P = (N * NS >= 2LL * 148 * 256) ? 1 : h->pl->p_small;   // fill the SMs' register files
   pl.elide = want_grade ? 0 : 1;           // grades need every B_alpha stored
-  tree_pick_shape(h->slots[pl.elide][0], h->slots[pl.elide][1], N, &pl.AL, &pl.AR);
+  tree_pick_shape(h->progs[0].slots[pl.elide][0], h->progs[0].slots[pl.elide][1], N, &pl.AL, &pl.AR);
   pl.atomic = h->force_mode == MTP_FORCE_ATOMIC || (h->force_mode == MTP_FORCE_AUTO && !has_rev);
   pl.grid_chunk = h->pl->pairgrad_grid((int)C, pl.P);
   size_t o = 0;
@@ -371,6 +435,10 @@ int make_plan(const mtp_handle *h, int64_t N, int64_t nnz, int want_grade, int h
   pl.o_M = o; o = align_up(o + (size_t)h->n_basic * pl.ldm * 8);
   pl.o_G = o; o = align_up(o + (size_t)h->n_basic * pl.ldm * 8);
   pl.o_red = o; o = align_up(o + 256 * 8 * 8);
+  if (h->partitioned) {                      // cut values and their adjoints of one chunk (tree_partition.cpp)
+    pl.o_S = o; o = align_up(o + (size_t)h->n_cut_rows * pl.ldm * 8);
+    pl.o_Sbar = o; o = align_up(o + (size_t)h->n_cut_rows * pl.ldm * 8);
+  }
   pl.o_idxp = o; o = align_up(o + (size_t)nnz * 4);          // packed neighbour words (used when shifts are given)
   pl.o_wpart = o; o = align_up(o + (size_t)std::max(1, pl.n_chunks) * pl.grid_chunk * 64);
   pl.o_d4 = o; if (!want_grade && !pl.atomic) o = align_up(o + (size_t)nnz * 32);
@@ -411,26 +479,56 @@ void fill_pair_args(const mtp_handle *h, PairArgs &pa, const double *pos4, const
   pa.M = nullptr; pa.G = nullptr; pa.d4 = nullptr; pa.F = nullptr; pa.wpart = nullptr; pa.kmap = nullptr;
 }
 
-int fill_tree_args(mtp_handle *h, TreeArgs &ta, const double *pos4, const Plan &pl, const TreeJit **jit) {
+// One K2 launch of program pg over the chunk [c0, c1).
+struct K2Io {
+  const double *pos4; const double *M; double *G; long long ldm; double *Ei; double *B;
+  int c0, c1; int want_adj; int64_t N; double *S; double *Sbar;
+};
+int launch_prog(mtp_handle *h, mtp_handle::Prog &pg, const K2Io &io, bool elide, const double *M, double *G, int want_adj,
+                double *S, const double *Sbar, int g_accum, int write_energy, double *B, cudaStream_t st) {
+  int AL = 0, AR = 1;
+  tree_pick_shape(pg.slots[elide][0], pg.slots[elide][1], io.N, &AL, &AR);
   const mtp_handle::TreeDev *td = nullptr;
-  int rc = get_tree(h, pl.AL, pl.AR, pl.elide != 0, &td);
+  int rc = get_tree(h, pg, AL, AR, elide, &td);
   if (rc != MTP_OK) return rc;
   const TreeSched &sc = td->sched;
-  *jit = td->jit;
+  TreeArgs ta;
   ta.fprog = td->d_fprog; ta.fwave = td->d_fwave; ta.nfw = (int)sc.fwave.size() - 1;
   ta.bprog = td->d_bprog; ta.bwave = td->d_bwave; ta.nbw = (int)sc.bwave.size() - 1;
   ta.n_fprog = (int)sc.fprog.size(); ta.n_bprog = (int)sc.bprog.size(); ta.prog_smem_off = 0;
-  ta.xi0 = h->d_xi0; ta.pos4 = pos4;
+  ta.xi0 = h->d_xi0; ta.pos4 = io.pos4;
   ta.adj_init = td->d_adj_init; ta.leaf_seed = td->d_leaf_seed;
   ta.eseed_slot = td->d_eseed_slot; ta.eseed_val = td->d_eseed_val; ta.n_eseed = (int)sc.eseed_slot.size();
   ta.basis_slot = td->d_basis_slot;
   ta.gseed_k = td->d_gseed_k; ta.gseed_val = td->d_gseed_val; ta.n_gseed = (int)sc.gseed_k.size();
   ta.gzero_k = td->d_gzero_k; ta.n_gzero = (int)sc.gzero_k.size();
-  ta.n_val = sc.n_val; ta.n_adj = sc.n_adj; ta.n_basic = h->n_basic; ta.n_basis = h->n_basis;
-  ta.B = nullptr; ta.want_adj = 1;
-  ta.mload_k = nullptr; ta.cut_row = ta.cut_vslot = ta.cut_aslot = nullptr; ta.n_cut = 0;
-  ta.S = nullptr; ta.Sbar = nullptr; ta.g_accum = 0; ta.write_energy = 1;
+  ta.n_val = sc.n_val; ta.n_adj = sc.n_adj; ta.n_basic = pg.n_basic; ta.n_basis = pg.n_basis;
+  ta.M = M; ta.G = G; ta.ldm = io.ldm; ta.Ei = io.Ei; ta.B = B; ta.c0 = io.c0; ta.c1 = io.c1; ta.want_adj = want_adj;
+  ta.mload_k = td->d_mload_k; ta.cut_row = td->d_cut_row; ta.cut_vslot = td->d_cut_vslot; ta.cut_aslot = td->d_cut_aslot;
+  ta.n_cut = (int)pg.cut_local.size();
+  ta.S = S; ta.Sbar = Sbar; ta.g_accum = g_accum; ta.write_energy = write_energy;
+  TIMED(h, CLS_TREE, st, (td->jit ? tree_jit_launch(td->jit, ta, st) : launch_tree(ta, AL, AR, st)));
   return MTP_OK;
+}
+
+// K2 over one chunk: B_alpha / E_i (forward) and, when io.want_adj, G = dE_i/dM.  io.B != null keeps every basis
+// value (no leaf elision).  A partitioned table runs its group programs forward, the top program, and the
+// group programs again forward + backward seeded with the top program's adjoints (tree_partition.cpp).
+int run_k2(mtp_handle *h, const K2Io &io, cudaStream_t st) {
+  const bool elide = io.B == nullptr;
+  if (!h->partitioned)
+    return launch_prog(h, h->progs[0], io, elide, io.M, io.G, io.want_adj, nullptr, nullptr, 0, 1, io.B, st);
+  int rc = MTP_OK;
+  CU(h, launch_scopy(io.S, io.ldm, h->n_basic, io.c1 - io.c0, h->d_gmap, io.M, st));
+  for (size_t q = 2; q < h->progs.size() && rc == MTP_OK; ++q)
+    rc = launch_prog(h, h->progs[q], io, true, io.M, nullptr, 0, io.S, nullptr, 0, 0, nullptr, st);
+  if (rc != MTP_OK) return rc;
+  rc = launch_prog(h, h->progs[1], io, elide, io.S, io.Sbar, io.want_adj, nullptr, nullptr, 0, 1, io.B, st);
+  if (rc != MTP_OK || !io.want_adj) return rc;
+  CU(h, launch_ginit(io.G, io.ldm, h->n_basic, io.c1 - io.c0, h->d_gmap, io.Sbar, st));
+  for (size_t q = 2; q < h->progs.size() && rc == MTP_OK; ++q)
+    rc = launch_prog(h, h->progs[q], io, true, io.M, io.G, 1, nullptr, io.Sbar, 1, 0, nullptr, st);
+  return rc;
 }
 }  // namespace
 
@@ -479,17 +577,14 @@ extern "C" int mtp_compute(mtp_handle *h, int64_t N, const double *d_pos, const 
   }
   fill_pair_args(h, pa, pos4, d_off, idxp, d_shift);
   pa.ldm = pl.ldm;
-  TreeArgs ta;
-  const TreeJit *jit = nullptr;
-  rc = fill_tree_args(h, ta, pos4, pl, &jit);
-  if (rc != MTP_OK) return rc;
-  ta.M = M; ta.G = G; ta.ldm = pl.ldm; ta.Ei = Ei;
+  K2Io io{pos4, M, G, pl.ldm, Ei, nullptr, 0, 0, 1, N, (double *)(ws + pl.o_S), (double *)(ws + pl.o_Sbar)};
   for (int c = 0; c < pl.n_chunks; ++c) {
     pa.c0 = (int)(c * pl.C); pa.c1 = (int)std::min<int64_t>(N, (c + 1) * pl.C);
     pa.M = M; pa.G = G; pa.kmap = h->d_kmapF;
     TIMED(h, CLS_MOMENTS, st, h->pl->moments(pa, pl.P, st));
-    ta.c0 = pa.c0; ta.c1 = pa.c1;
-    TIMED(h, CLS_TREE, st, (jit ? tree_jit_launch(jit, ta, st) : launch_tree(ta, pl.AL, pl.AR, st)));
+    io.c0 = pa.c0; io.c1 = pa.c1;
+    rc = run_k2(h, io, st);
+    if (rc != MTP_OK) return rc;
     pa.kmap = h->d_kmapB; pa.wpart = wpart + (size_t)c * pl.grid_chunk * 8;
     pa.d4 = pl.atomic ? nullptr : d4; pa.F = pl.atomic ? d_F : nullptr;
     TIMED(h, CLS_PAIRGRAD, st, h->pl->pairgrad(pa, pl.P, pl.atomic, st, nullptr));
@@ -534,20 +629,17 @@ extern "C" int mtp_grade(mtp_handle *h, int64_t N, const double *d_pos, const in
     }
     fill_pair_args(h, pa, pos4, d_off, idxp, d_shift);
     pa.ldm = pl.ldm;
-    TreeArgs ta;
-    const TreeJit *jit = nullptr;
-    rc = fill_tree_args(h, ta, pos4, pl, &jit);
-    if (rc != MTP_OK) return rc;
-    ta.M = M; ta.G = G; ta.ldm = pl.ldm; ta.Ei = Ei; ta.want_adj = 0;
+    K2Io io{pos4, M, G, pl.ldm, Ei, nullptr, 0, 0, 0, N, (double *)(ws + pl.o_S), (double *)(ws + pl.o_Sbar)};
     for (int c = 0; c < pl.n_chunks; ++c) {
       pa.c0 = (int)(c * pl.C); pa.c1 = (int)std::min<int64_t>(N, (c + 1) * pl.C);
       pa.M = M; pa.kmap = h->d_kmapF;
       TIMED(h, CLS_MOMENTS, st, h->pl->moments(pa, pl.P, st));
-      ta.c0 = pa.c0; ta.c1 = pa.c1;
+      io.c0 = pa.c0; io.c1 = pa.c1;
       // B rows are indexed by absolute atom: point the kernel at a base shifted by -c0 rows
       double *Brows = d_B ? d_B : Bc - (size_t)pa.c0 * h->n_basis;
-      ta.B = Brows;
-      TIMED(h, CLS_TREE, st, (jit ? tree_jit_launch(jit, ta, st) : launch_tree(ta, pl.AL, pl.AR, st)));
+      io.B = Brows;
+      rc = run_k2(h, io, st);
+      if (rc != MTP_OK) return rc;
       const double *Bchunk = Brows + (size_t)pa.c0 * h->n_basis;
       const int64_t nc = pa.c1 - pa.c0;
       if (mode != 1) TIMED(h, CLS_GRADE, st, launch_grade(Bchunk, d_Ainv, nc, h->n_basis, d_gamma_atom + pa.c0, st));
@@ -615,8 +707,6 @@ extern "C" int mtp_debug_moments(mtp_handle *h, int64_t N, const double *d_pos, 
   int rc = make_plan(h, N, 0, 0, 0, pl);
   h->chunk_atoms = saved;
   if (rc != MTP_OK) return rc;
-  pl.elide = 0;                             // B is exported: every basis value must be stored
-  tree_pick_shape(h->slots[0][0], h->slots[0][1], N, &pl.AL, &pl.AR);
   const size_t base = align_up((size_t)(uintptr_t)d_ws) - (size_t)(uintptr_t)d_ws;
   if (!d_ws || ws_bytes < pl.total + base) return fail(h, MTP_ESIZE, "workspace too small");
   PairArgs pa;
@@ -641,12 +731,12 @@ extern "C" int mtp_debug_moments(mtp_handle *h, int64_t N, const double *d_pos, 
     if (tmp_idxp) { cudaStreamSynchronize(st); cudaFree(tmp_idxp); }
     if (e != cudaSuccess) return cuda_fail(h, e, "moments");
   }
-  TreeArgs ta;
-  const TreeJit *jit = nullptr;
-  rc = fill_tree_args(h, ta, pos4, pl, &jit);
+  // B is exported, so every basis value is stored (no leaf elision).  When the caller does not want B the
+  // scratch chunk of the workspace cannot be assumed (this entry point sizes it without grades): require d_B.
+  if (!d_B) return fail(h, MTP_EINVAL, "mtp_debug_moments: d_B is required");
+  K2Io io{pos4, M, G, pl.ldm, Ei, d_B, 0, (int)N, 1, N, (double *)(ws + pl.o_S), (double *)(ws + pl.o_Sbar)};
+  rc = run_k2(h, io, st);
   if (rc != MTP_OK) return rc;
-  ta.M = M; ta.G = G; ta.ldm = pl.ldm; ta.Ei = Ei; ta.c0 = 0; ta.c1 = (int)N; ta.B = d_B;
-  CU(h, (jit ? tree_jit_launch(jit, ta, st) : launch_tree(ta, pl.AL, pl.AR, st)));
   // outputs are [n_basic][N] (component-major), the kernels' own layout
   if (d_M) CU(h, cudaMemcpy2DAsync(d_M, (size_t)N * 8, M, (size_t)pl.ldm * 8, (size_t)N * 8, h->n_basic, cudaMemcpyDeviceToDevice, st));
   if (d_G) CU(h, cudaMemcpy2DAsync(d_G, (size_t)N * 8, G, (size_t)pl.ldm * 8, (size_t)N * 8, h->n_basic, cudaMemcpyDeviceToDevice, st));

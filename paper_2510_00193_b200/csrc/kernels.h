@@ -64,6 +64,11 @@ const PairLevel *pair_level(int index);   // index into kLevels
 // ---- misc kernels (misc_kernels.cu)
 cudaError_t launch_pack(const double *pos, const int *type, int n, double *pos4, cudaStream_t st);
 cudaError_t launch_zero(double *p, long long n, cudaStream_t st);
+// G[k][:] = gmap[k] >= 0 ? Sbar[gmap[k]][:] : 0  (partitioned K2, before the group programs accumulate)
+// S[gmap[k]][:] = M[k][:] for the packed moments that are cut nodes themselves
+cudaError_t launch_scopy(double *S, long long ldm, int n_basic, int ncol, const int *gmap, const double *M, cudaStream_t st);
+cudaError_t launch_ginit(double *G, long long ldm, int n_basic, int ncol, const int *gmap, const double *Sbar,
+                         cudaStream_t st);
 // out[p] = idx[p] | image_code(shift[p]) << 27
 cudaError_t launch_pack_pairs(const int *idx, const signed char *shift, long long nnz, int *out, cudaStream_t st);
 // F_k = sum_p d[p] - d[rev[p]] over row k (warp per atom, fixed order)

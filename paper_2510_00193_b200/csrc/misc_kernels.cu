@@ -33,6 +33,25 @@ __global__ void k_pack_pairs(const int *__restrict__ idx, const signed char *__r
   out[p] = idx[p] | (code << kIdxBits);
 }
 
+// G of a partitioned table before the group programs accumulate into it: dE_i/d(cut) for the packed moments
+// that are cut nodes themselves (gmap[k] = their cut row), 0 for the others
+__global__ void k_ginit(double *__restrict__ G, long long ldm, int n_basic, int ncol, const int *__restrict__ gmap,
+                        const double *__restrict__ Sbar) {
+  const int col = blockIdx.x * blockDim.x + threadIdx.x, k = blockIdx.y;
+  if (col >= ncol || k >= n_basic) return;
+  const int r = gmap[k];
+  G[(long long)k * ldm + col] = r >= 0 ? Sbar[(long long)r * ldm + col] : 0.0;
+}
+
+// cut values of the packed moments that are cut nodes themselves: S[gmap[k]][:] = M[k][:]
+__global__ void k_scopy(double *__restrict__ S, long long ldm, int n_basic, int ncol, const int *__restrict__ gmap,
+                        const double *__restrict__ M) {
+  const int col = blockIdx.x * blockDim.x + threadIdx.x, k = blockIdx.y;
+  if (col >= ncol || k >= n_basic) return;
+  const int r = gmap[k];
+  if (r >= 0) S[(long long)r * ldm + col] = M[(long long)k * ldm + col];
+}
+
 __global__ void k_zero(double *p, long long n) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) p[i] = 0.0;
@@ -117,6 +136,19 @@ cudaError_t launch_pack(const double *pos, const int *type, int n, double *pos4,
 cudaError_t launch_pack_pairs(const int *idx, const signed char *shift, long long nnz, int *out, cudaStream_t st) {
   if (nnz <= 0) return cudaSuccess;
   k_pack_pairs<<<(unsigned)((nnz + 255) / 256), 256, 0, st>>>(idx, shift, nnz, out);
+  count_launch();
+  return cudaGetLastError();
+}
+cudaError_t launch_ginit(double *G, long long ldm, int n_basic, int ncol, const int *gmap, const double *Sbar,
+                         cudaStream_t st) {
+  if (ncol <= 0 || n_basic <= 0) return cudaSuccess;
+  k_ginit<<<dim3((ncol + 255) / 256, n_basic), 256, 0, st>>>(G, ldm, n_basic, ncol, gmap, Sbar);
+  count_launch();
+  return cudaGetLastError();
+}
+cudaError_t launch_scopy(double *S, long long ldm, int n_basic, int ncol, const int *gmap, const double *M, cudaStream_t st) {
+  if (ncol <= 0 || n_basic <= 0) return cudaSuccess;
+  k_scopy<<<dim3((ncol + 255) / 256, n_basic), 256, 0, st>>>(S, ldm, n_basic, ncol, gmap, M);
   count_launch();
   return cudaGetLastError();
 }
