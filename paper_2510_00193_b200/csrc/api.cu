@@ -9,6 +9,7 @@
 #include <cstring>
 #include <map>
 #include <string>
+#include <thread>
 #include <tuple>
 #include <vector>
 
@@ -61,6 +62,7 @@ struct mtp_handle {
     std::vector<int32_t> basic_map, cut_local, cut_row;   // group programs only
     int slots[2][2] = {{0, 0}, {0, 0}};        // [elide][n_val, n_adj]
     std::map<int, TreeDev> trees;              // key: AL * 8 + AR * 2 + elide
+    std::map<int, std::vector<char>> cubin;    // same key: kernels compiled ahead in parallel at create
     int n_prod() const { return (int)(prod.size() / 4); }
     bool is_group() const { return !cut_local.empty(); }
   };
@@ -187,11 +189,15 @@ static int get_tree(mtp_handle *h, mtp_handle::Prog &pg, int AL, int AR, bool el
   // The kernel specialised for this table (tree_jit.cpp) runs the same schedule as the interpreter (so the two
   // are bit-identical); built when the table is short enough to be worth compiling and the shape has 32
   // atom-lanes.  (32 row-lane warps instead of 16 were measured slower: the generated code is bound by
-  // instruction fetch, not by per-warp latency.)  Group programs are interpreted.
+  // instruction fetch, not by per-warp latency.)
   const char *env = getenv("MTP_TREE_CODEGEN");
-  if (h->codegen && !(env && env[0] == '0') && !group && AL == 32 && 3LL * pg.n_prod() <= 60000 &&
+  if (h->codegen && !(env && env[0] == '0') && AL == 32 && 3LL * pg.n_prod() <= 60000 &&
       tree_jit_smem_bytes(td.sched.n_val, td.sched.n_adj, AR, tree_threads(AL)) <= 225 * 1024)
-    td.jit = tree_jit_build(td.sched, AL, AR, &td.jit_note);
+  {
+    auto pre = pg.cubin.find(key);
+    if (pre != pg.cubin.end()) { td.jit = tree_jit_load(pre->second, AR, td.sched.R * AL, &td.jit_note); pg.cubin.erase(pre); }
+    else td.jit = tree_jit_build(td.sched, AL, AR, &td.jit_note);
+  }
   cudaError_t e = cudaSuccess;
   auto up = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
   const TreeSched &sc = td.sched;
@@ -348,6 +354,33 @@ extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
   up(upload(h, &h->d_kmapB, kb.data(), kb.size()));
   up(upload(h, &h->d_basis_node, p->basis_node, (size_t)p->n_basis));
   if (e != cudaSuccess) { int r = cuda_fail(nullptr, e, "mtp_create upload"); mtp_destroy(h); return r; }
+  // the programs of a partitioned table are specialised in parallel (NVRTC takes seconds per program)
+  {
+    const char *env = getenv("MTP_TREE_CODEGEN");
+    std::vector<std::thread> workers;
+    for (size_t q = h->partitioned ? 1 : 0; h->partitioned && h->codegen && !(env && env[0] == '0') && q < h->progs.size(); ++q) {
+      mtp_handle::Prog *pg = &h->progs[q];
+      int AL = 0, AR = 1;
+      tree_pick_shape(pg->slots[1][0], pg->slots[1][1], 0, &AL, &AR);
+      if (AL != 32 || 3LL * pg->n_prod() > 60000) continue;
+      const int key = AL * 8 + AR * 2 + 1;
+      pg->cubin[key];                          // created here: the workers only assign to existing entries
+      workers.emplace_back([pg, AL, AR, key]() {
+        TreeSched sc;
+        const char *terr = "";
+        const bool group = pg->is_group();
+        if (tree_compile(pg->n_basic, pg->n_nodes, pg->n_prod(), pg->prod.data(), pg->n_basis, pg->basis_node.data(),
+                         pg->xi.data(), AL * AR, tree_row_lanes(AL), true, sc, &terr, group ? pg->basic_map.data() : nullptr,
+                         group ? pg->cut_local.data() : nullptr, (int)pg->cut_local.size()) != MTP_OK) return;
+        if (tree_jit_smem_bytes(sc.n_val, sc.n_adj, AR, tree_threads(AL)) > 225 * 1024) return;
+        std::string why;
+        pg->cubin[key] = tree_jit_compile(sc, AL, AR, &why);
+      });
+    }
+    for (auto &w : workers) w.join();
+    for (auto &pg : h->progs)                  // drop failed compilations: get_tree then decides on its own
+      for (auto it = pg.cubin.begin(); it != pg.cubin.end();) it = it->second.empty() ? pg.cubin.erase(it) : std::next(it);
+  }
   // validate the table(s) and build the large-system schedules now, so that errors surface at create
   for (size_t q = h->partitioned ? 1 : 0; q < h->progs.size(); ++q) {
     const mtp_handle::TreeDev *td = nullptr;

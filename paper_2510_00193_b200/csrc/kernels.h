@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <cstdint>
 #include <string>
+#include <vector>
 
 #include "pair_kernels_args.h"
 #include "tree.h"
@@ -48,6 +49,8 @@ cudaError_t launch_tree(const TreeArgs &a, int AL, int AR, cudaStream_t st);
 // K2 specialised for one schedule with NVRTC (tree_jit.cpp); null when unavailable (reason in *why)
 struct TreeJit;
 TreeJit *tree_jit_build(const TreeSched &sc, int AL, int AR, std::string *why);
+std::vector<char> tree_jit_compile(const TreeSched &sc, int AL, int AR, std::string *why);   // host only, thread-safe
+TreeJit *tree_jit_load(const std::vector<char> &cubin, int AR, int NT, std::string *why);
 cudaError_t tree_jit_launch(const TreeJit *j, const TreeArgs &a, cudaStream_t st);
 void tree_jit_destroy(TreeJit *j);
 size_t tree_jit_smem_bytes(int n_val, int n_adj, int AR, int NT);

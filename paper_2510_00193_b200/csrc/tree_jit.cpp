@@ -75,7 +75,7 @@ struct TreeArgs {
   int n_val, n_adj, n_basic, n_basis;
   int c0, c1;
   int want_adj;
-  const int *mload_k;                      // the fields below serve group sub-programs, which are interpreted
+  const int *mload_k;                      // the fields below serve the group sub-programs of a partitioned tree
   const int *cut_row, *cut_vslot, *cut_aslot; int n_cut;
   double *S;
   const double *Sbar;
@@ -98,7 +98,7 @@ struct TreeArgs {
 #define RV(D) { *(double2 *)(vw + D) = make_double2(tx, ty); }
 #define RL(S) { ex = fma(S, tx, ex); ey = fma(S, ty, ey); }
 #define RA(D) { double2 o = LD(ac + D); o.x += tx; o.y += ty; *(double2 *)(ac + D) = o; }
-#define RG(K) { if (n_ok > 0) Gcol[(long long)K * ldm] = tx; if (n_ok > 1) Gcol[(long long)K * ldm + 1] = ty; }
+#define RG(K) { double *gp = Gcol + (long long)K * ldm; if (n_ok > 0) gp[0] = ga ? gp[0] + tx : tx; if (n_ok > 1) gp[1] = ga ? gp[1] + ty : ty; }
 #else
 #define LD(p) (*(const double *)(p))
 #define E0(OA, OB) { ax = __dmul_rn(LD(s0 + OA), LD(vc + OB)); }
@@ -108,7 +108,7 @@ struct TreeArgs {
 #define RV(D) { *(double *)(vw + D) = tx; }
 #define RL(S) { ex = fma(S, tx, ex); }
 #define RA(D) { *(double *)(ac + D) += tx; }
-#define RG(K) { if (n_ok > 0) Gcol[(long long)K * ldm] = tx; }
+#define RG(K) { double *gp = Gcol + (long long)K * ldm; if (n_ok > 0) gp[0] = ga ? gp[0] + tx : tx; }
 #endif
 
 extern "C" __global__ void __launch_bounds__(NT, 1) k_tree_gen(const TreeArgs a) {
@@ -128,10 +128,17 @@ extern "C" __global__ void __launch_bounds__(NT, 1) k_tree_gen(const TreeArgs a)
     const long long col = atom0 - a.c0;
     __syncthreads();
     for (int k = rl; k < a.n_basic; k += R)
-      for (int r = 0; r < AR; ++r) val[(size_t)k * A + al * AR + r] = r < n_ok ? a.M[(long long)k * ldm + col + r] : 0.0;
+      for (int r = 0; r < AR; ++r)
+        val[(size_t)k * A + al * AR + r] = r < n_ok ? a.M[(long long)(a.mload_k ? a.mload_k[k] : k) * ldm + col + r] : 0.0;
     if (a.want_adj)
       for (int k = rl; k < a.n_adj; k += R)
         for (int r = 0; r < AR; ++r) adj[(size_t)k * A + al * AR + r] = a.adj_init[k];
+    if (a.want_adj && a.Sbar) {              // per-atom seeds of a group's cut nodes
+      __syncthreads();
+      for (int q = rl; q < a.n_cut; q += R)
+        for (int r = 0; r < AR; ++r)
+          adj[(size_t)a.cut_aslot[q] * A + al * AR + r] = r < n_ok ? a.Sbar[(long long)a.cut_row[q] * ldm + col + r] : 0.0;
+    }
     __syncthreads();
     double ex = 0.0, ey = 0.0, ax = 0.0, ay = 0.0, tx = 0.0, ty = 0.0;
     (void)ey; (void)ay; (void)ty;
@@ -160,7 +167,11 @@ extern "C" __global__ void __launch_bounds__(NT, 1) k_tree_gen(const TreeArgs a)
         }
       }
       __syncthreads();
-      if (rl == 0) {
+      if (a.S)                                 // cut values of a group, exported for the top program
+        for (int q = rl; q < a.n_cut; q += R)
+          for (int r = 0; r < AR; ++r)
+            if (r < n_ok) a.S[(long long)a.cut_row[q] * ldm + col + r] = val[(size_t)a.cut_vslot[q] * A + al * AR + r];
+      if (rl == 0 && a.write_energy) {
         for (int r = 0; r < AR; ++r) {
           if (r < n_ok) {
             double s = 0.0;
@@ -173,6 +184,7 @@ extern "C" __global__ void __launch_bounds__(NT, 1) k_tree_gen(const TreeArgs a)
     }
     if (!a.want_adj) continue;
     double *Gcol = a.G + col;
+    const bool ga = a.g_accum != 0;
     for (int q = rl; q < a.n_gzero; q += R)
       for (int r = 0; r < AR; ++r)
         if (r < n_ok) Gcol[(long long)a.gzero_k[q] * ldm + r] = 0.0;
@@ -259,19 +271,22 @@ void tree_jit_destroy(TreeJit *j) {
 }
 
 // Returns null (and a reason in *why) when the specialised kernel is not available.
-TreeJit *tree_jit_build(const TreeSched &sc, int AL, int AR, std::string *why) {
-  if (AL != 32) { *why = "codegen needs 32 atom-lanes"; return nullptr; }
+// Host-only half: generate and compile the source of one schedule (thread-safe; mtp_create runs the
+// programs of a partitioned table in parallel).  Empty result + reason when unavailable.
+std::vector<char> tree_jit_compile(const TreeSched &sc, int AL, int AR, std::string *why) {
+  std::vector<char> cubin;
+  if (AL != 32) { *why = "codegen needs 32 atom-lanes"; return cubin; }
   const Nvrtc &rt = nvrtc();
-  if (!rt.ok) { *why = "NVRTC not found"; return nullptr; }
+  if (!rt.ok) { *why = "NVRTC not found"; return cubin; }
   const int R = sc.R, NT = R * AL;            // the schedule's row-lanes are this kernel's warps
-  if (NT > 1024 || sc.A != AL * AR) { *why = "schedule shape mismatch"; return nullptr; }
+  if (NT > 1024 || sc.A != AL * AR) { *why = "schedule shape mismatch"; return cubin; }
   std::string src = kFrame;
   replace_all(src, "@AR@", std::to_string(AR));
   replace_all(src, "@NT@", std::to_string(NT));
   replace_all(src, "@FWD@", gen_pass(sc.fprog, sc.fwave, R, false, sc.leaf_seed, AL * AR));
   replace_all(src, "@BWD@", gen_pass(sc.bprog, sc.bwave, R, true, sc.leaf_seed, AL * AR));
   nvrtcProgram prog = nullptr;
-  if (rt.CreateProgram(&prog, src.c_str(), "k_tree_gen.cu", 0, nullptr, nullptr) != 0) { *why = "nvrtcCreateProgram failed"; return nullptr; }
+  if (rt.CreateProgram(&prog, src.c_str(), "k_tree_gen.cu", 0, nullptr, nullptr) != 0) { *why = "nvrtcCreateProgram failed"; return cubin; }
   const char *opts[] = {"--gpu-architecture=sm_100a", "--std=c++17", "-lineinfo", "-default-device"};
   const int rc = rt.CompileProgram(prog, 4, opts);
   if (rc != 0) {
@@ -280,13 +295,19 @@ TreeJit *tree_jit_build(const TreeSched &sc, int AL, int AR, std::string *why) {
     if (rt.GetProgramLogSize && rt.GetProgramLog && rt.GetProgramLogSize(prog, &n) == 0 && n > 1) { log.resize(n); rt.GetProgramLog(prog, &log[0]); }
     *why = "NVRTC compile failed: " + log.substr(0, 400);
     rt.DestroyProgram(&prog);
-    return nullptr;
+    return cubin;
   }
   size_t nbin = 0;
   rt.GetCUBINSize(prog, &nbin);
-  std::vector<char> cubin(nbin);
+  cubin.resize(nbin);
   rt.GetCUBIN(prog, cubin.data());
   rt.DestroyProgram(&prog);
+  return cubin;
+}
+
+// Device half: load a compiled schedule.
+TreeJit *tree_jit_load(const std::vector<char> &cubin, int AR, int NT, std::string *why) {
+  if (cubin.empty()) return nullptr;
   TreeJit *j = new TreeJit();
   j->AR = AR; j->NT = NT;
   cudaError_t e = cudaLibraryLoadData(&j->lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
@@ -299,6 +320,10 @@ TreeJit *tree_jit_build(const TreeSched &sc, int AL, int AR, std::string *why) {
     return nullptr;
   }
   return j;
+}
+
+TreeJit *tree_jit_build(const TreeSched &sc, int AL, int AR, std::string *why) {
+  return tree_jit_load(tree_jit_compile(sc, AL, AR, why), AR, sc.R * AL, why);
 }
 
 cudaError_t tree_jit_launch(const TreeJit *j, const TreeArgs &a, cudaStream_t st) {
