@@ -83,6 +83,7 @@ struct TreeArgs {
   int write_energy;
 };
 #define AR @AR@
+#define GRP @GRP@        // 1: group sub-program of a partitioned tree (subset loads, per-atom seeds, G accumulates)
 #define NT @NT@
 #define AL 32
 #define A (AL * AR)
@@ -98,7 +99,11 @@ struct TreeArgs {
 #define RV(D) { *(double2 *)(vw + D) = make_double2(tx, ty); }
 #define RL(S) { ex = fma(S, tx, ex); ey = fma(S, ty, ey); }
 #define RA(D) { double2 o = LD(ac + D); o.x += tx; o.y += ty; *(double2 *)(ac + D) = o; }
+#if GRP
 #define RG(K) { double *gp = Gcol + (long long)K * ldm; if (n_ok > 0) gp[0] = ga ? gp[0] + tx : tx; if (n_ok > 1) gp[1] = ga ? gp[1] + ty : ty; }
+#else
+#define RG(K) { if (n_ok > 0) Gcol[(long long)K * ldm] = tx; if (n_ok > 1) Gcol[(long long)K * ldm + 1] = ty; }
+#endif
 #else
 #define LD(p) (*(const double *)(p))
 #define E0(OA, OB) { ax = __dmul_rn(LD(s0 + OA), LD(vc + OB)); }
@@ -108,7 +113,11 @@ struct TreeArgs {
 #define RV(D) { *(double *)(vw + D) = tx; }
 #define RL(S) { ex = fma(S, tx, ex); }
 #define RA(D) { *(double *)(ac + D) += tx; }
+#if GRP
 #define RG(K) { double *gp = Gcol + (long long)K * ldm; if (n_ok > 0) gp[0] = ga ? gp[0] + tx : tx; }
+#else
+#define RG(K) { if (n_ok > 0) Gcol[(long long)K * ldm] = tx; }
+#endif
 #endif
 
 extern "C" __global__ void __launch_bounds__(NT, 1) k_tree_gen(const TreeArgs a) {
@@ -129,11 +138,11 @@ extern "C" __global__ void __launch_bounds__(NT, 1) k_tree_gen(const TreeArgs a)
     __syncthreads();
     for (int k = rl; k < a.n_basic; k += R)
       for (int r = 0; r < AR; ++r)
-        val[(size_t)k * A + al * AR + r] = r < n_ok ? a.M[(long long)(a.mload_k ? a.mload_k[k] : k) * ldm + col + r] : 0.0;
+        val[(size_t)k * A + al * AR + r] = r < n_ok ? a.M[(long long)(GRP ? a.mload_k[k] : k) * ldm + col + r] : 0.0;
     if (a.want_adj)
       for (int k = rl; k < a.n_adj; k += R)
         for (int r = 0; r < AR; ++r) adj[(size_t)k * A + al * AR + r] = a.adj_init[k];
-    if (a.want_adj && a.Sbar) {              // per-atom seeds of a group's cut nodes
+    if (GRP && a.want_adj && a.Sbar) {       // per-atom seeds of a group's cut nodes
       __syncthreads();
       for (int q = rl; q < a.n_cut; q += R)
         for (int r = 0; r < AR; ++r)
@@ -167,7 +176,7 @@ extern "C" __global__ void __launch_bounds__(NT, 1) k_tree_gen(const TreeArgs a)
         }
       }
       __syncthreads();
-      if (a.S)                                 // cut values of a group, exported for the top program
+      if (GRP && a.S)                          // cut values of a group, exported for the top program
         for (int q = rl; q < a.n_cut; q += R)
           for (int r = 0; r < AR; ++r)
             if (r < n_ok) a.S[(long long)a.cut_row[q] * ldm + col + r] = val[(size_t)a.cut_vslot[q] * A + al * AR + r];
@@ -184,7 +193,7 @@ extern "C" __global__ void __launch_bounds__(NT, 1) k_tree_gen(const TreeArgs a)
     }
     if (!a.want_adj) continue;
     double *Gcol = a.G + col;
-    const bool ga = a.g_accum != 0;
+    const bool ga = a.g_accum != 0; (void)ga;
     for (int q = rl; q < a.n_gzero; q += R)
       for (int r = 0; r < AR; ++r)
         if (r < n_ok) Gcol[(long long)a.gzero_k[q] * ldm + r] = 0.0;
@@ -283,6 +292,7 @@ std::vector<char> tree_jit_compile(const TreeSched &sc, int AL, int AR, std::str
   std::string src = kFrame;
   replace_all(src, "@AR@", std::to_string(AR));
   replace_all(src, "@NT@", std::to_string(NT));
+  replace_all(src, "@GRP@", sc.mload_k.empty() ? "0" : "1");
   replace_all(src, "@FWD@", gen_pass(sc.fprog, sc.fwave, R, false, sc.leaf_seed, AL * AR));
   replace_all(src, "@BWD@", gen_pass(sc.bprog, sc.bwave, R, true, sc.leaf_seed, AL * AR));
   nvrtcProgram prog = nullptr;
