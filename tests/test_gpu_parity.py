@@ -274,3 +274,38 @@ def test_full_size_config5_sampled_energy_and_grades(lib, torch):
     Bsum = g["Bsum"].cpu().numpy()
     assert g["gamma_cfg"].cpu().numpy()[0] == pytest.approx(np.abs(Bsum @ w.Ainv).max(), rel=TOL_G)
     pot.close()
+
+
+def test_error_codes_for_bad_tables_and_small_workspace(lib, torch):
+    """Errors are codes, never aborts: malformed contraction tables (MTP_EINVAL) and a short workspace (MTP_ESIZE)."""
+    import ctypes as C
+    from paper_2510_00193_b200 import binding as bnd
+    t = lib.Table(10)
+    rng = np.random.default_rng(3)
+    c = rng.uniform(-0.1, 0.1, (1, 1, t.n_mu, 8))
+    xi0, xi = np.zeros(1), rng.uniform(-0.1, 0.1, t.n_basis)
+    bad = t.prod.copy()
+    bad[0, 0] = t.n_nodes + 5                                  # source index out of range
+    with pytest.raises(lib.MtpError) as e:
+        lib.Potential(t, 1, 8, 2.0, 5.0, c, xi0, xi, prod=bad)
+    assert e.value.code == lib.EINVAL
+    bad = t.prod.copy()
+    last = bad[-1].copy()                                      # a node is read before it is written
+    bad[1:] = t.prod[:-1]
+    bad[0] = last
+    if last[0] >= t.n_basic or last[1] >= t.n_basic:
+        with pytest.raises(lib.MtpError) as e:
+            lib.Potential(t, 1, 8, 2.0, 5.0, c, xi0, xi, prod=bad)
+        assert e.value.code == lib.EINVAL
+    w = make_workload(0, t.n_basis)
+    pot = gpu_pot(lib, w)
+    d = to_dev(w, torch)
+    n, nnz = w.n_atoms, w.nnz
+    out = [torch.empty(s, dtype=torch.float64, device="cuda") for s in (1, n, (n, 3), 6)]
+    ws = torch.empty(1024, dtype=torch.uint8, device="cuda")   # far too small
+    boxh = (C.c_double * 9)(*[float(x) for x in np.asarray(w.box).reshape(9)])
+    p = lambda x: C.c_void_p(x.data_ptr())
+    rc = bnd._lib.mtp_compute(pot._h, n, p(d["pos"]), p(d["types"]), boxh, p(d["off"]), p(d["idx"]), p(d["shift"]),
+                              p(d["rev"]), nnz, p(out[0]), p(out[1]), p(out[2]), p(out[3]), p(ws), ws.numel(), C.c_void_p(0))
+    assert rc == lib.ESIZE
+    pot.close()
