@@ -34,6 +34,11 @@ constexpr uint32_t kTreeGroup = 1u;    // entry closes a group: tot += mult * ac
 constexpr uint32_t kTreeRow = 2u;      // entry closes a row: dispose of tot, tot = 0
 constexpr uint32_t kTreeAlt = 4u;      // row disposal: fwd 0 = store val[slot], 1 = leaf: e += leaf_seed[idx] * tot
                                        //               bwd 0 = adj[slot] += tot, 1 = G[k] = tot (global memory)
+constexpr uint32_t kTreeAcc = 1u;      // in b (bit 0), backward rows without kTreeAlt: the row is a piece of a split row and
+                                       // stores its partial sum into val[slot] (a spare slot) instead of adding to adj[slot]
+// val slots reserved for such partial sums: 16 .. 64, growing with the number of packed inputs
+inline int tree_spare_slots(int n_basic) { const int s = n_basic / 8; return s < 16 ? 16 : (s > 64 ? 64 : s); }
+constexpr uint32_t kTreeBMask = ((1u << 18) - 1u) & ~7u;   // byte offset of factor 1 inside b
 constexpr int kTreeDstShift = 18;
 constexpr int kTreeMaxDst = 1 << 14;
 

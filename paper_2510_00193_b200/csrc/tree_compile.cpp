@@ -28,7 +28,7 @@ void tree_count_slots(int n_basic, int n_nodes, int n_prod, const int32_t *prod,
     if (!inter || is_read[n] || !elide) ++nv;
     if (inter && is_read[n]) ++na;
   }
-  *n_val = nv; *n_adj = na;
+  *n_val = nv + (n_cut > 0 ? 0 : tree_spare_slots(n_basic)); *n_adj = na;   // (group programs do not split rows)   // room for the partial sums of split backward rows
 }
 
 int tree_compile(int n_basic, int n_nodes, int n_prod, const int32_t *prod, int n_basis,
@@ -99,7 +99,7 @@ int tree_compile(int n_basic, int n_nodes, int n_prod, const int32_t *prod, int 
     if (seeded[n] && s.val_slot[n] >= 0) { s.eseed_slot.push_back(s.val_slot[n]); s.eseed_val.push_back(seed[n]); }
   if (!elide) for (int a = 0; a < n_basis; ++a) s.basis_slot.push_back(s.val_slot[basis_node[a]]);
 
-  struct Row { uint32_t dst, alt; std::vector<RawTerm> terms; };
+  struct Row { uint32_t dst, alt; std::vector<RawTerm> terms; bool acc = false; };
   // Emit one wave.  `single`: all rows go to row-lane 0 in the given order (dependent chain).
   auto emit = [&](std::vector<Row> &rows, bool single, std::vector<TreeTerm> &prog) {
     if (!single)
@@ -116,7 +116,7 @@ int tree_compile(int n_basic, int n_nodes, int n_prod, const int32_t *prod, int 
         t.a = r.a; t.b = r.b; t.mult = r.mult;
         const bool lastk = k + 1 == row.terms.size();
         if (lastk || row.terms[k + 1].mult != r.mult) t.a |= kTreeGroup;
-        if (lastk) { t.a |= kTreeRow | (row.alt ? kTreeAlt : 0u); t.b |= row.dst << kTreeDstShift; }
+        if (lastk) { t.a |= kTreeRow | (row.alt ? kTreeAlt : 0u); t.b |= (row.dst << kTreeDstShift) | (row.acc ? kTreeAcc : 0u); }
         lane[best].push_back(t);
       }
     }
@@ -197,7 +197,38 @@ int tree_compile(int n_basic, int n_nodes, int n_prod, const int32_t *prod, int 
       else { brow[n].dst = (uint32_t)adj_slot[n]; brow[n].alt = 0; }
       waves[D - depth[n]].push_back(std::move(brow[n]));   // deepest sources first
     }
-    emit_all(waves, s.bprog, s.bwave);
+    // A backward row much longer than its wave's share per row-lane (the adjoint of M_{0,0} collects a term from
+    // every product that contains it) would serialise the wave: its terms are dealt to several pieces that run
+    // concurrently in the wave and store their partial sums in spare val slots; a short row in an extra wave
+    // right after adds the partials in fixed order (first factor = adj slot 0 = 1) into the real destination.
+    std::vector<std::vector<Row>> split;
+    int spare = 0;
+    for (auto &wave : waves) {
+      size_t terms = 0;
+      for (auto &r : wave) terms += r.terms.size();
+      const size_t lmax = std::max<size_t>(48, (terms * 5 / 4 + R - 1) / R);
+      std::vector<Row> first, combine;
+      for (auto &r : wave) {
+        const size_t np = (r.terms.size() + lmax - 1) / lmax;
+        if (r.terms.size() <= lmax + lmax / 2 || group || spare + (int)np > tree_spare_slots(n_basic)) { first.push_back(std::move(r)); continue; }
+        std::stable_sort(r.terms.begin(), r.terms.end(), [](const RawTerm &x, const RawTerm &y) { return x.mult < y.mult; });
+        const size_t per = (r.terms.size() + np - 1) / np;
+        Row sum; sum.dst = r.dst; sum.alt = r.alt;
+        for (size_t q = 0; q < np; ++q) {
+          Row piece; piece.dst = (uint32_t)(nv + spare); piece.alt = 0; piece.acc = true;   // bwd + !alt + acc: store to val
+          piece.terms.assign(r.terms.begin() + q * per, r.terms.begin() + std::min(r.terms.size(), (q + 1) * per));
+          first.push_back(std::move(piece));
+          sum.terms.push_back(RawTerm{0u, (uint32_t)(nv + spare) * row_bytes, 1.0});
+          ++spare;
+        }
+        combine.push_back(std::move(sum));
+      }
+      split.push_back(std::move(first));
+      if (!combine.empty()) split.push_back(std::move(combine));
+    }
+    s.n_val = nv + spare;
+    if ((unsigned long long)s.n_val * row_bytes >= (1ull << kTreeDstShift)) { *err = e_big; return MTP_EUNSUP; }
+    emit_all(split, s.bprog, s.bwave);
   }
   s.fsteps = s.fwave.back(); s.bsteps = s.bwave.back();
   // the kernel prefetches up to 4 * kTreePrefetch steps ahead: pad so that those reads stay in bounds

@@ -99,6 +99,7 @@ struct TreeArgs {
 #define RV(D) { *(double2 *)(vw + D) = make_double2(tx, ty); }
 #define RL(S) { ex = fma(S, tx, ex); ey = fma(S, ty, ey); }
 #define RA(D) { double2 o = LD(ac + D); o.x += tx; o.y += ty; *(double2 *)(ac + D) = o; }
+#define RGA(K) { double *gp = Gcol + (long long)K * ldm; if (n_ok > 0) gp[0] += tx; if (n_ok > 1) gp[1] += ty; }   // later piece of a split row
 #if GRP
 #define RG(K) { double *gp = Gcol + (long long)K * ldm; if (n_ok > 0) gp[0] = ga ? gp[0] + tx : tx; if (n_ok > 1) gp[1] = ga ? gp[1] + ty : ty; }
 #else
@@ -113,6 +114,7 @@ struct TreeArgs {
 #define RV(D) { *(double *)(vw + D) = tx; }
 #define RL(S) { ex = fma(S, tx, ex); }
 #define RA(D) { *(double *)(ac + D) += tx; }
+#define RGA(K) { double *gp = Gcol + (long long)K * ldm; if (n_ok > 0) gp[0] += tx; }
 #if GRP
 #define RG(K) { double *gp = Gcol + (long long)K * ldm; if (n_ok > 0) gp[0] = ga ? gp[0] + tx : tx; }
 #else
@@ -232,7 +234,7 @@ std::string gen_pass(const std::vector<TreeTerm> &prog, const std::vector<int32_
       bool acc_open = false, tot_open = false;      // does acc / tot hold a partial sum?
       for (int s = wave[w]; s <= last; ++s) {
         const TreeTerm &t = prog[(size_t)s * R + l];
-        snprintf(buf, sizeof buf, "%s(%u,%u)", acc_open ? "E" : "E0", t.a & ~7u, t.b & ((1u << kTreeDstShift) - 1));
+        snprintf(buf, sizeof buf, "%s(%u,%u)", acc_open ? "E" : "E0", t.a & ~7u, t.b & kTreeBMask);
         out += buf;
         acc_open = true;
         if (t.a & kTreeGroup) {
@@ -246,6 +248,7 @@ std::string gen_pass(const std::vector<TreeTerm> &prog, const std::vector<int32_
               else snprintf(buf, sizeof buf, "RV(%u)", d * row);
             } else {
               if (t.a & kTreeAlt) snprintf(buf, sizeof buf, "RG(%u)", d);
+              else if (t.b & kTreeAcc) snprintf(buf, sizeof buf, "RV(%u)", d * row);     // partial sum of a split row
               else snprintf(buf, sizeof buf, "RA(%u)", d * row);
             }
             out += buf;

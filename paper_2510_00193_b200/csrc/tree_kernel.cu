@@ -70,7 +70,7 @@ __device__ __forceinline__ void run_pass(const int4 *__restrict__ prog, const in
         const int u = q * BL + v;
         const int4 t = T[u];
         const Vec<AR> x = lds<AR>(src0 + ((unsigned)t.x & ~7u));
-        const Vec<AR> y = lds<AR>(val + ((unsigned)t.y & ((1u << kTreeDstShift) - 1)));
+        const Vec<AR> y = lds<AR>(val + ((unsigned)t.y & kTreeBMask));
 #pragma unroll
         for (int r = 0; r < AR; ++r) acc.v[r] = fma(x.v[r], y.v[r], acc.v[r]);
         if (t.x & (int)kTreeGroup) {
@@ -94,6 +94,8 @@ __device__ __forceinline__ void run_pass(const int4 *__restrict__ prog, const in
                   double *gp = Gcol + (long long)d * ldm + r;
                   *gp = g_accum ? *gp + tot.v[r] : tot.v[r];
                 }
+            } else if (t.y & (int)kTreeAcc) {          // piece of a split row: partial sum into a spare val slot
+              sts<AR>(valw + d * ROW, tot);
             } else {
               char *qd = adj + d * ROW;               // adj was initialised with the node's seed
               Vec<AR> old = lds<AR>(qd);
@@ -211,7 +213,7 @@ __global__ void __launch_bounds__(NT) k_tree(const TreeArgs a) {
 #pragma unroll
       for (int r = 0; r < AR; ++r)
         if (r < n_ok) Gcol[(long long)a.gzero_k[q] * a.ldm + r] = 0.0;
-    run_pass<AL, AR, R, true, PS>(bprog, bw, a.nbw, rl, valc, adjc, nullptr, nullptr, e, Gcol, a.ldm, n_ok, a.g_accum != 0);
+    run_pass<AL, AR, R, true, PS>(bprog, bw, a.nbw, rl, valc, adjc, const_cast<char *>(valc), nullptr, e, Gcol, a.ldm, n_ok, a.g_accum != 0);
     __syncthreads();
     // packed moments that are basis functions themselves (M_{mu,0}): G += xi
     for (int q = rl; q < a.n_gseed; q += R)
