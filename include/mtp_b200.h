@@ -79,8 +79,10 @@ typedef struct {
 int mtp_enumerate(int32_t lev_max, mtp_params *out);
 void mtp_table_free(mtp_params *table);
 
-/* Create / destroy.  Validates the table, compiles it into the kernels' schedules and
- * copies c, xi0, xi and the schedules to the current CUDA device. */
+/* Create / destroy.  Validates the table, compiles it into the kernels' schedules (large tables are first cut
+ * into a top program and group programs that fit shared memory; short programs are additionally specialised
+ * with NVRTC when libnvrtc is present -- seconds of one-time work) and copies c, xi0, xi and the schedules to
+ * the current CUDA device. */
 int mtp_create(mtp_handle **out, const mtp_params *p);
 void mtp_destroy(mtp_handle *h);
 const char *mtp_last_error(const mtp_handle *h); /* h may be NULL: last create error     */
@@ -109,6 +111,7 @@ int mtp_workspace_bytes(const mtp_handle *h, int64_t n_atoms, int64_t nnz, int w
                         size_t *out_bytes);
 
 /* a1-a8, a10.  Energy, per-atom energy, forces, virial over a full CSR neighbour list.
+ *   N <= 2^27 atoms (the kernels pack a neighbour index and its image code into one 32-bit word; MTP_EUNSUP beyond)
  *   d_pos   [N][3] f64      d_type [N] i32 in [0,S)
  *   box     [9] HOST, rows = lattice vectors
  *   d_off   [N+1] i64       d_idx [nnz] i32  (entries with r >= R_cut contribute nothing)

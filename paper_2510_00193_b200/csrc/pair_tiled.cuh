@@ -5,10 +5,11 @@
 //            holds neighbours [t*TN, (t+1)*TN) of each of them (TN = 4*NS*P, NA*TN = 128), four
 //            consecutive pairs per lane.  a1-a3 are done ONCE per pair here: r, Chebyshev recurrence,
 //            f_mu (and f'_mu for K3); the result (x, y, z, f[, f']) goes to the warp's shared-memory
-//            tile.  The packed neighbour words (index + image code) are fetched two tiles ahead into
-//            registers and the 32-byte position records they point to are copied one tile ahead into a
-//            double-buffered shared-memory staging area with cp.async, so phase A never waits on L2/HBM.  Pairs past the end
-//            of a row or with r >= R_cut are stored as zeros, so that phase B needs no predicates.
+//            tile.  The packed neighbour words (index + image code) are copied two tiles ahead and the
+//            32-byte position records they point to one tile ahead into per-lane shared-memory staging
+//            slots with cp.async (no registers held across phase B), so phase A does not wait on L2/HBM.
+//            Pairs past the end of a row or with r >= R_cut are stored as zeros, so that phase B needs
+//            no predicates.
 //   phase B  lanes = (atom, slice, part) as in stair.h: every lane walks the TN staged pairs of its
 //            atom (parts split them) and does only the part that scales with n_basic -- monomials
 //            and moment FMAs (K1) or the nested Horner sweeps over G (K3).
