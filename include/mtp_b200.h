@@ -137,9 +137,11 @@ int mtp_grade(mtp_handle *h, int64_t n_atoms, const double *d_pos, const int32_t
               void *d_ws, size_t ws_bytes, void *cuda_stream);
 
 /* Host-buffer convenience path (the end-to-end call bench.py's `e2e` times): same
- * arguments as mtp_compute but every array is a HOST pointer; the library stages them
- * through its own pinned + device buffers, runs mtp_compute and copies E, E_i, F, virial
- * back, synchronising before it returns. */
+ * arguments as mtp_compute but every array is a HOST pointer; the library copies them to its own
+ * device buffers on a copy stream -- the neighbour list chunk by chunk, so that the evaluation of the
+ * first chunks overlaps the transfer of the later ones (pinned host buffers are needed for that
+ * overlap) --, runs the same kernels as mtp_compute and copies E, E_i, F, virial back, synchronising
+ * before it returns. */
 int mtp_compute_host(mtp_handle *h, int64_t n_atoms, const double *pos, const int32_t *type,
                      const double *box, const int64_t *off, const int32_t *idx,
                      const int8_t *shift, const int32_t *rev, int64_t nnz, double *E,

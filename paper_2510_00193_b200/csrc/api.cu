@@ -75,9 +75,11 @@ struct mtp_handle {
   int64_t chunk_atoms = 0;
   int force_mode = MTP_FORCE_AUTO, variant = MTP_VARIANT_AUTO;
   std::string err;
-  // staging for mtp_compute_host (grow-only)
+  // staging for mtp_compute_host (grow-only), its copy / compute streams and chunk events
   void *stage = nullptr;
   size_t stage_bytes = 0;
+  cudaStream_t s_copy = nullptr, s_comp = nullptr;
+  std::vector<cudaEvent_t> ev;
   std::vector<void *> to_free;
   // per-kernel-class device timing (MTP_OPT_PROFILE): event pairs recorded around each launch
   int profile = 0;
@@ -249,6 +251,9 @@ extern "C" void mtp_destroy(mtp_handle *h) {
   for (auto &pg : h->progs) for (auto &kv : pg.trees) tree_jit_destroy(kv.second.jit);
   for (void *p : h->to_free) cudaFree(p);
   if (h->stage) cudaFree(h->stage);
+  for (auto e : h->ev) cudaEventDestroy(e);
+  if (h->s_copy) cudaStreamDestroy(h->s_copy);
+  if (h->s_comp) cudaStreamDestroy(h->s_comp);
   delete h;
 }
 
@@ -574,10 +579,19 @@ extern "C" int mtp_workspace_bytes(const mtp_handle *h, int64_t n_atoms, int64_t
   return MTP_OK;
 }
 
-extern "C" int mtp_compute(mtp_handle *h, int64_t N, const double *d_pos, const int32_t *d_type, const double *box,
-                           const int64_t *d_off, const int32_t *d_idx, const int8_t *d_shift, const int32_t *d_rev,
-                           int64_t nnz, double *d_E, double *d_Ei, double *d_F, double *d_virial, void *d_ws,
-                           size_t ws_bytes, void *stream) {
+// Pipelining hooks of mtp_compute_host: the pairs of chunk c (device arrays idx / shift, filled by an asynchronous
+// copy on another stream) are ready when chunk_ready[c] has fired, rev when rev_ready has; chunk_pair0[c] is the
+// CSR offset of the chunk's first atom (host copy), so that the neighbour words are packed chunk by chunk.
+struct HostPipe {
+  const std::vector<cudaEvent_t> *chunk_ready = nullptr;
+  const std::vector<long long> *chunk_pair0 = nullptr;    // n_chunks + 1 entries
+  cudaEvent_t rev_ready = nullptr;
+};
+
+static int compute_impl(mtp_handle *h, int64_t N, const double *d_pos, const int32_t *d_type, const double *box,
+                        const int64_t *d_off, const int32_t *d_idx, const int8_t *d_shift, const int32_t *d_rev,
+                        int64_t nnz, double *d_E, double *d_Ei, double *d_F, double *d_virial, void *d_ws,
+                        size_t ws_bytes, void *stream, const HostPipe *pipe) {
   if (!h) return MTP_EINVAL;
   if (!box || !d_E || (N > 0 && (!d_pos || !d_type || !d_off || !d_F)) || (nnz > 0 && !d_idx))
     return fail(h, MTP_EINVAL, "mtp_compute: null argument");
@@ -605,7 +619,7 @@ extern "C" int mtp_compute(mtp_handle *h, int64_t N, const double *d_pos, const 
   if (pl.atomic) CU(h, launch_zero(d_F, 3 * N, st));
   const int32_t *idxp = d_idx;
   if (d_shift && nnz > 0) {
-    CU(h, launch_pack_pairs(d_idx, (const signed char *)d_shift, nnz, (int *)(ws + pl.o_idxp), st));
+    if (!pipe) CU(h, launch_pack_pairs(d_idx, (const signed char *)d_shift, nnz, (int *)(ws + pl.o_idxp), st));
     idxp = (const int32_t *)(ws + pl.o_idxp);
   }
   fill_pair_args(h, pa, pos4, d_off, idxp, d_shift);
@@ -613,6 +627,12 @@ extern "C" int mtp_compute(mtp_handle *h, int64_t N, const double *d_pos, const 
   K2Io io{pos4, M, G, pl.ldm, Ei, nullptr, 0, 0, 1, N, (double *)(ws + pl.o_S), (double *)(ws + pl.o_Sbar)};
   for (int c = 0; c < pl.n_chunks; ++c) {
     pa.c0 = (int)(c * pl.C); pa.c1 = (int)std::min<int64_t>(N, (c + 1) * pl.C);
+    if (pipe) {                                  // this chunk's pairs have just arrived: pack their neighbour words
+      CU(h, cudaStreamWaitEvent(st, (*pipe->chunk_ready)[c], 0));
+      const long long p0 = (*pipe->chunk_pair0)[c], p1 = (*pipe->chunk_pair0)[c + 1];
+      if (d_shift && p1 > p0)
+        CU(h, launch_pack_pairs(d_idx + p0, (const signed char *)d_shift + 3 * p0, p1 - p0, (int *)(ws + pl.o_idxp) + p0, st));
+    }
     pa.M = M; pa.G = G; pa.kmap = h->d_kmapF;
     TIMED(h, CLS_MOMENTS, st, h->pl->moments(pa, pl.P, st));
     io.c0 = pa.c0; io.c1 = pa.c1;
@@ -622,11 +642,20 @@ extern "C" int mtp_compute(mtp_handle *h, int64_t N, const double *d_pos, const 
     pa.d4 = pl.atomic ? nullptr : d4; pa.F = pl.atomic ? d_F : nullptr;
     TIMED(h, CLS_PAIRGRAD, st, h->pl->pairgrad(pa, pl.P, pl.atomic, st, nullptr));
   }
+  if (pipe && pipe->rev_ready) CU(h, cudaStreamWaitEvent(st, pipe->rev_ready, 0));
   if (!pl.atomic) TIMED(h, CLS_OTHER, st, launch_gather((const long long *)d_off, d_rev, d4, (int)N, d_F, st));
   double *red = (double *)(ws + pl.o_red);
   CU(h, launch_reduce(Ei, N, 1, 1, d_E, red, st));
   if (d_virial) CU(h, launch_reduce(wpart, (long long)pl.n_chunks * pl.grid_chunk, 8, 6, d_virial, red, st));
   return MTP_OK;
+}
+
+extern "C" int mtp_compute(mtp_handle *h, int64_t N, const double *d_pos, const int32_t *d_type, const double *box,
+                           const int64_t *d_off, const int32_t *d_idx, const int8_t *d_shift, const int32_t *d_rev,
+                           int64_t nnz, double *d_E, double *d_Ei, double *d_F, double *d_virial, void *d_ws,
+                           size_t ws_bytes, void *stream) {
+  return compute_impl(h, N, d_pos, d_type, box, d_off, d_idx, d_shift, d_rev, nnz, d_E, d_Ei, d_F, d_virial, d_ws, ws_bytes,
+                      stream, nullptr);
 }
 
 extern "C" int mtp_grade(mtp_handle *h, int64_t N, const double *d_pos, const int32_t *d_type, const double *box,
@@ -704,22 +733,50 @@ extern "C" int mtp_compute_host(mtp_handle *h, int64_t N, const double *pos, con
     h->stage_bytes = o;
   }
   char *d = (char *)h->stage;
-  cudaStream_t st = 0;
+  // Two streams: the neighbour list (the bulk of the input: 11 B per pair) is copied chunk by chunk on the copy
+  // stream while the compute stream already evaluates the chunks that have arrived.  (Overlap needs pinned host
+  // buffers; with pageable memory the copies simply serialise.)
+  if (!h->s_copy) {
+    CU(h, cudaStreamCreateWithFlags(&h->s_copy, cudaStreamNonBlocking));
+    CU(h, cudaStreamCreateWithFlags(&h->s_comp, cudaStreamNonBlocking));
+  }
+  Plan pl;
+  rc = make_plan(h, N, nnz, 0, rev != nullptr, pl);
+  if (rc != MTP_OK) return fail(h, rc, "bad sizes");
+  while ((int)h->ev.size() < pl.n_chunks + 2) {
+    cudaEvent_t e = nullptr;
+    CU(h, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    h->ev.push_back(e);
+  }
+  cudaStream_t sc = h->s_copy, st = h->s_comp;
+  std::vector<long long> pair0(pl.n_chunks + 1, 0);
+  std::vector<cudaEvent_t> ready(h->ev.begin() + 2, h->ev.begin() + 2 + pl.n_chunks);
   if (N > 0) {
-    CU(h, cudaMemcpyAsync(d + o_pos, pos, (size_t)N * 24, cudaMemcpyHostToDevice, st));
-    CU(h, cudaMemcpyAsync(d + o_type, type, (size_t)N * 4, cudaMemcpyHostToDevice, st));
-    CU(h, cudaMemcpyAsync(d + o_off, off, (size_t)(N + 1) * 8, cudaMemcpyHostToDevice, st));
+    CU(h, cudaMemcpyAsync(d + o_pos, pos, (size_t)N * 24, cudaMemcpyHostToDevice, sc));
+    CU(h, cudaMemcpyAsync(d + o_type, type, (size_t)N * 4, cudaMemcpyHostToDevice, sc));
+    CU(h, cudaMemcpyAsync(d + o_off, off, (size_t)(N + 1) * 8, cudaMemcpyHostToDevice, sc));
   }
-  if (nnz > 0) {
-    CU(h, cudaMemcpyAsync(d + o_idx, idx, (size_t)nnz * 4, cudaMemcpyHostToDevice, st));
-    if (shift) CU(h, cudaMemcpyAsync(d + o_shift, shift, (size_t)nnz * 3, cudaMemcpyHostToDevice, st));
-    if (rev) CU(h, cudaMemcpyAsync(d + o_rev, rev, (size_t)nnz * 4, cudaMemcpyHostToDevice, st));
+  CU(h, cudaEventRecord(h->ev[0], sc));
+  for (int c = 0; c < pl.n_chunks; ++c) {
+    const long long p0 = off[(int64_t)c * pl.C], p1 = off[std::min<int64_t>(N, (int64_t)(c + 1) * pl.C)];
+    pair0[c] = p0; pair0[c + 1] = p1;
+    if (p1 > p0) {
+      CU(h, cudaMemcpyAsync(d + o_idx + 4 * p0, idx + p0, (size_t)(p1 - p0) * 4, cudaMemcpyHostToDevice, sc));
+      if (shift) CU(h, cudaMemcpyAsync(d + o_shift + 3 * p0, shift + 3 * p0, (size_t)(p1 - p0) * 3, cudaMemcpyHostToDevice, sc));
+    }
+    CU(h, cudaEventRecord(ready[c], sc));
   }
+  if (rev && nnz > 0) CU(h, cudaMemcpyAsync(d + o_rev, rev, (size_t)nnz * 4, cudaMemcpyHostToDevice, sc));
+  CU(h, cudaEventRecord(h->ev[1], sc));
+  CU(h, cudaStreamWaitEvent(st, h->ev[0], 0));
+  HostPipe pipe;
+  pipe.chunk_ready = &ready; pipe.chunk_pair0 = &pair0; pipe.rev_ready = h->ev[1];
   double *dE = (double *)(d + o_out), *dW = dE + 1, *dEi = dE + 7, *dF = dEi + N;
-  rc = mtp_compute(h, N, (double *)(d + o_pos), (int32_t *)(d + o_type), box, (int64_t *)(d + o_off),
-                   (int32_t *)(d + o_idx), shift ? (int8_t *)(d + o_shift) : nullptr,
-                   rev ? (int32_t *)(d + o_rev) : nullptr, nnz, dE, dEi, dF, dW, d + o_ws, wsb, st);
-  if (rc != MTP_OK) return rc;
+  rc = compute_impl(h, N, (double *)(d + o_pos), (int32_t *)(d + o_type), box, (int64_t *)(d + o_off),
+                    (int32_t *)(d + o_idx), shift ? (int8_t *)(d + o_shift) : nullptr,
+                    rev ? (int32_t *)(d + o_rev) : nullptr, nnz, dE, dEi, dF, dW, d + o_ws, wsb, st, N > 0 ? &pipe : nullptr);
+  if (rc != MTP_OK) { cudaStreamSynchronize(sc); cudaStreamSynchronize(st); return rc; }
+  if (N == 0) CU(h, cudaStreamWaitEvent(st, h->ev[1], 0));
   CU(h, cudaMemcpyAsync(E, dE, 8, cudaMemcpyDeviceToHost, st));
   if (virial) CU(h, cudaMemcpyAsync(virial, dW, 48, cudaMemcpyDeviceToHost, st));
   if (Ei && N > 0) CU(h, cudaMemcpyAsync(Ei, dEi, (size_t)N * 8, cudaMemcpyDeviceToHost, st));
