@@ -57,7 +57,7 @@ class ClockSampler:
         try:
             self.f = open(self.path, "w")
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
                                          stdout=self.f, stderr=subprocess.DEVNULL)
         except Exception:
             self.proc = None
@@ -140,7 +140,7 @@ def run_reference(args):
     except Exception:
         ctx = None
     w, table, cfg = build_workload(args.config, args.cells)
-    n_sample = args.ref_atoms
+    n_sample = args.ref_atoms or 1024          # x (steps + warmup): the whole run stays within a few minutes
     for _ in range(args.warmup):
         oracle_rate(w, n_sample)
     t = 0.0
@@ -230,7 +230,7 @@ def run_ours(args):
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
     hp = dict(pos=pin(w.pos), types=pin(w.types), off=pin(w.off), idx=pin(w.idx), shift=pin(w.shift), rev=pin(w.rev))
     hout = dict(E=pin(np.zeros(1)), Ei=pin(np.zeros(w.n_atoms)), F=pin(np.zeros((w.n_atoms, 3))), virial=pin(np.zeros(6)))
-    e2e_steps = max(1, min(args.steps, 3))
+    e2e_steps = max(1, min(args.steps, 10))
     pot.compute_host(hp["pos"], hp["types"], w.box, hp["off"], hp["idx"], hp["shift"], hp["rev"], out=hout)
     barrier()
     t0 = time.perf_counter()
@@ -286,7 +286,7 @@ def run_ours(args):
             lim = threadpool_limits(limits=1)
         except Exception:
             lim = None
-        rate, dt, k = oracle_rate(w, args.ref_atoms)
+        rate, dt, k = oracle_rate(w, args.ref_atoms or 8192)
         cpu = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": "first %d atoms of the workload (E_i, d_ij, force scatter), %.1f s" % (k, dt)}
 
@@ -320,7 +320,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="0-based index into BASELINE.json configs")
@@ -328,7 +328,8 @@ def main():
     ap.add_argument("--chunk", type=int, default=-1)
     ap.add_argument("--force-mode", type=int, default=-1)
     ap.add_argument("--grade", action="store_true", help="also run mtp_grade each step (config 4)")
-    ap.add_argument("--ref-atoms", type=int, default=8192, help="atoms per oracle sample (about 12 s of CPU work)")
+    ap.add_argument("--ref-atoms", type=int, default=None,
+                    help="atoms per oracle sample (default: 8192 = about 12 s for cpu_baseline, 1024 per step for --impl reference)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
