@@ -158,6 +158,10 @@ int mtp_debug_moments(mtp_handle *h, int64_t n_atoms, const double *d_pos,
  * count per kernel class since the last read; classes: 0 moments (K1), 1 tree (K2),
  * 2 pair gradient (K3), 3 force gather, 4 grade (K5).  Synchronises on the recorded events. */
 int mtp_profile_read(mtp_handle *h, double *ms /*[5]*/, int64_t *launches /*[5]*/);
+/* Host-only (no device needed): how mtp_create will evaluate the contraction table of *p (only the table
+ * fields are read).  out[8] = { partitioned (0/1), atoms per CTA of the whole table, cut rows, groups, ops of the
+ * top program, ops summed over the group programs, ops below the cut, smallest atoms per CTA over the groups }. */
+int mtp_table_plan(const mtp_params *p, int64_t *out);
 /* Number of kernels this library has launched since load (bench.py gpu_launches). */
 int64_t mtp_launch_count(void);
 /* fp64 FMA throughput microbenchmark: runs `iters` dependent-chain DFMA batches on every

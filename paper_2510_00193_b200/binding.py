@@ -37,7 +37,7 @@ class MtpParams(C.Structure):
 EXPORTS = ["mtp_enumerate", "mtp_table_free", "mtp_create", "mtp_destroy", "mtp_last_error",
            "mtp_set_option", "mtp_get_option", "mtp_workspace_bytes", "mtp_compute", "mtp_grade",
            "mtp_compute_host", "mtp_debug_moments", "mtp_launch_count", "mtp_peak_dfma",
-           "mtp_cost_model", "mtp_profile_read"]
+           "mtp_cost_model", "mtp_profile_read", "mtp_table_plan"]
 
 
 def _build():
@@ -52,8 +52,11 @@ def _load():
     if not os.path.exists(LIB_PATH):
         _build()
     lib = C.CDLL(LIB_PATH)
-    if not all(hasattr(lib, name) for name in EXPORTS):
-        raise ImportError("%s is stale (missing exports): run `python paper_2510_00193_b200/build.py`" % LIB_PATH)
+    if not all(hasattr(lib, name) for name in EXPORTS):      # stale build: rebuild once, then insist
+        _build()
+        lib = C.CDLL(LIB_PATH)
+        if not all(hasattr(lib, name) for name in EXPORTS):
+            raise ImportError("%s is stale (missing exports): run `python paper_2510_00193_b200/build.py`" % LIB_PATH)
     vp, i64, dbl = C.c_void_p, C.c_int64, C.c_double
     lib.mtp_enumerate.argtypes = [C.c_int32, C.POINTER(MtpParams)]
     lib.mtp_table_free.argtypes = [C.POINTER(MtpParams)]
@@ -76,6 +79,7 @@ def _load():
     lib.mtp_peak_dfma.argtypes = [i64, vp, C.POINTER(dbl), vp]
     lib.mtp_cost_model.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl)]
     lib.mtp_profile_read.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
+    lib.mtp_table_plan.argtypes = [C.POINTER(MtpParams), C.POINTER(i64)]
     return lib
 
 
@@ -108,6 +112,22 @@ class Table:
             self.basis_desc_off = np.ctypeslib.as_array(p.basis_desc_off, (p.n_basis + 1,)).copy()
         finally:
             _lib.mtp_table_free(C.byref(p))
+
+    def plan(self):
+        """mtp_table_plan: how mtp_create will evaluate this table (host-only diagnostic)."""
+        basic = np.ascontiguousarray(self.basic, dtype=np.int32)
+        prod = np.ascontiguousarray(self.prod, dtype=np.int32)
+        bn = np.ascontiguousarray(self.basis_node, dtype=np.int32)
+        p = MtpParams()
+        p.n_basic, p.basic, p.n_nodes = basic.shape[0], basic.ctypes.data_as(_I32P), int(self.n_nodes)
+        p.n_prod, p.prod = prod.shape[0], prod.ctypes.data_as(_I32P)
+        p.n_basis, p.basis_node = bn.shape[0], bn.ctypes.data_as(_I32P)
+        out = (C.c_int64 * 8)()
+        rc = _lib.mtp_table_plan(C.byref(p), out)
+        if rc != OK:
+            raise MtpError(rc, "mtp_table_plan")
+        keys = ["partitioned", "atoms_per_cta", "cut_rows", "groups", "top_ops", "group_ops", "ops_below_cut", "group_atoms_per_cta"]
+        return dict(zip(keys, [int(x) for x in out]))
 
     def describe(self, alpha: int):
         return list(self.basis_desc[self.basis_desc_off[alpha]:self.basis_desc_off[alpha + 1]])

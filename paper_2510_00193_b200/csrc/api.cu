@@ -257,6 +257,46 @@ extern "C" void mtp_destroy(mtp_handle *h) {
   delete h;
 }
 
+// The partition mtp_create uses for a table whose monolithic evaluation gets fewer than 32 atoms per CTA:
+// budgets = shared-memory slots per atom that leave room for 64 (else 32) atoms per CTA beside the energy partials.
+static bool decide_partition(const mtp_params *p, TreePartition &part) {
+  const char *penv = getenv("MTP_TREE_PARTITION");
+  if (penv && penv[0] == '0') return false;
+  bool ok = tree_partition(p->n_basic, p->n_nodes, p->n_prod, p->prod, p->n_basis, p->basis_node, 430, part);
+  if (!ok || part.groups.size() > 24)
+    ok = tree_partition(p->n_basic, p->n_nodes, p->n_prod, p->prod, p->n_basis, p->basis_node, 870, part);
+  return ok;
+}
+
+// Host-only diagnostic (no device needed): how mtp_create would evaluate this table.
+extern "C" int mtp_table_plan(const mtp_params *p, int64_t *out) {
+  if (!p || !out || p->n_basic < 1 || p->n_nodes < p->n_basic || p->n_prod < 0 || (p->n_prod && !p->prod) || !p->basis_node)
+    return MTP_EINVAL;
+  for (int q = 0; q < 8; ++q) out[q] = 0;
+  int nv = 0, na = 0, AL = 0, AR = 1;
+  tree_count_slots(p->n_basic, p->n_nodes, p->n_prod, p->prod, true, &nv, &na);
+  tree_pick_shape(nv, na, 0, &AL, &AR);
+  out[1] = (int64_t)AL * AR;
+  if (AL >= 32) return MTP_OK;
+  TreePartition part;
+  if (!decide_partition(p, part)) return MTP_OK;
+  out[0] = 1; out[2] = (int64_t)part.cut_node.size(); out[3] = (int64_t)part.groups.size(); out[4] = part.top.n_prod();
+  std::vector<char> seen(part.cut_node.size(), 0);
+  int64_t min_atoms = 1 << 30;
+  for (auto &g : part.groups) {
+    out[5] += g.table.n_prod();
+    for (int r : g.cut_row) { if (r < 0 || r >= (int)seen.size() || seen[r]) return MTP_EINVAL; seen[r] = 1; }
+    tree_count_slots(g.table.n_basic, g.table.n_nodes, g.table.n_prod(), g.table.prod.data(), true, &nv, &na, g.cut_local.data(),
+                     (int)g.cut_local.size());
+    tree_pick_shape(nv, na, 0, &AL, &AR);
+    min_atoms = std::min<int64_t>(min_atoms, (int64_t)AL * AR);
+  }
+  for (size_t r = 0; r < seen.size(); ++r) if (!seen[r] && part.cut_node[r] >= p->n_basic) return MTP_EINVAL;
+  out[6] = (int64_t)p->n_prod - part.top.n_prod();
+  out[7] = min_atoms;
+  return MTP_OK;
+}
+
 extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
   if (!out || !p) return fail(nullptr, MTP_EINVAL, "null argument");
   *out = nullptr;
@@ -302,12 +342,9 @@ extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
     tree_pick_shape(whole.slots[1][0], whole.slots[1][1], 0, &AL, &AR);
     // Too few atoms per CTA (lev_max >= 20): cut the table into a top program and group programs that each fit
     // 64 (else 32) atoms per CTA.  Budgets = shared-memory slots per atom left beside the energy partials.
-    const char *penv = getenv("MTP_TREE_PARTITION");
-    if (AL < 32 && !(penv && penv[0] == '0')) {
+    {
       TreePartition part;
-      bool ok = tree_partition(p->n_basic, p->n_nodes, p->n_prod, p->prod, p->n_basis, p->basis_node, 430, part);
-      if (!ok || part.groups.size() > 24)
-        ok = tree_partition(p->n_basic, p->n_nodes, p->n_prod, p->prod, p->n_basis, p->basis_node, 870, part);
+      const bool ok = AL < 32 && decide_partition(p, part);
       if (ok) {
         h->partitioned = true;
         h->n_cut_rows = (int)part.cut_node.size();

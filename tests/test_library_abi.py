@@ -63,3 +63,19 @@ def test_no_device_means_error_not_fallback(lib):
     with pytest.raises(lib.MtpError) as e:
         lib.Potential(t, 1, 8, 2.0, 5.0, np.zeros((1, 1, t.n_mu, 8)), np.zeros(1), np.zeros(t.n_basis))
     assert e.value.code == lib.ECUDA
+
+
+@pytest.mark.parametrize("lev,want_part", [(10, 0), (16, 0), (20, 1), (24, 1)])
+def test_table_plan_partitions_only_large_tables(lib, lev, want_part):
+    """Host logic of the K2 partition (csrc/tree_partition.cpp): small tables run whole with 64 atoms per CTA; large
+    ones are cut, every intermediate cut node lands in exactly one group (checked inside mtp_table_plan), all groups fit
+    at least 32 atoms per CTA, and the duplicated work stays moderate."""
+    plan = lib.Table(lev).plan()
+    assert plan["partitioned"] == want_part
+    if not want_part:
+        assert plan["atoms_per_cta"] == 64
+        return
+    assert plan["atoms_per_cta"] < 32 and plan["group_atoms_per_cta"] >= 32
+    assert 1 <= plan["groups"] <= 24 and plan["cut_rows"] > plan["groups"]
+    assert plan["top_ops"] + plan["ops_below_cut"] == lib.Table(lev).n_prod
+    assert plan["ops_below_cut"] <= plan["group_ops"] <= 1.5 * plan["ops_below_cut"]
