@@ -309,3 +309,18 @@ def test_error_codes_for_bad_tables_and_small_workspace(lib, torch):
                               p(d["rev"]), nnz, p(out[0]), p(out[1]), p(out[2]), p(out[3]), p(ws), ws.numel(), C.c_void_p(0))
     assert rc == lib.ESIZE
     pot.close()
+
+
+def test_level28_partitioned_tree_interpreted(lib, torch, monkeypatch):
+    """Level 28 (9 739 basis functions): one atom's node values exceed shared memory, so the table only runs
+    partitioned (132 group programs + top program).  Interpreter path (code generation off keeps create fast)."""
+    monkeypatch.setenv("MTP_TREE_CODEGEN", "0")
+    lev, n_mu = 28, 7
+    assert lib.Table(lev).plan()["partitioned"] == 1
+    w = cluster_workload(lev, n_mu, 33, 8, 2, r_list=5.0)
+    opot = oracle_pot(w)
+    ref = omtp.evaluate(opot, w.pos, w.types, w.box, w.off, w.idx, w.shift)
+    got, pot, _ = run_gpu(lib, torch, w)
+    assert pot.get_option(lib.INFO_TREE_KERNELS) == 0
+    check(w, ref, got, opot)
+    pot.close()
