@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -399,7 +400,8 @@ extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
   // the programs of a partitioned table are specialised in parallel (NVRTC takes seconds per program)
   {
     const char *env = getenv("MTP_TREE_CODEGEN");
-    std::vector<std::thread> workers;
+    struct Job { mtp_handle::Prog *pg; int AL, AR, key; };
+    std::vector<Job> jobs;
     for (size_t q = h->partitioned ? 1 : 0; h->partitioned && h->codegen && !(env && env[0] == '0') && q < h->progs.size(); ++q) {
       mtp_handle::Prog *pg = &h->progs[q];
       int AL = 0, AR = 1;
@@ -407,18 +409,26 @@ extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
       if (AL != 32 || 3LL * pg->n_prod() > 60000) continue;
       const int key = AL * 8 + AR * 2 + 1;
       pg->cubin[key];                          // created here: the workers only assign to existing entries
-      workers.emplace_back([pg, AL, AR, key]() {
+      jobs.push_back(Job{pg, AL, AR, key});
+    }
+    std::atomic<size_t> next{0};
+    auto work = [&]() {
+      for (size_t i = next.fetch_add(1); i < jobs.size(); i = next.fetch_add(1)) {
+        const Job &j = jobs[i];
         TreeSched sc;
         const char *terr = "";
-        const bool group = pg->is_group();
-        if (tree_compile(pg->n_basic, pg->n_nodes, pg->n_prod(), pg->prod.data(), pg->n_basis, pg->basis_node.data(),
-                         pg->xi.data(), AL * AR, tree_row_lanes(AL), true, sc, &terr, group ? pg->basic_map.data() : nullptr,
-                         group ? pg->cut_local.data() : nullptr, (int)pg->cut_local.size()) != MTP_OK) return;
-        if (tree_jit_smem_bytes(sc.n_val, sc.n_adj, AR, tree_threads(AL)) > 225 * 1024) return;
+        const bool group = j.pg->is_group();
+        if (tree_compile(j.pg->n_basic, j.pg->n_nodes, j.pg->n_prod(), j.pg->prod.data(), j.pg->n_basis, j.pg->basis_node.data(),
+                         j.pg->xi.data(), j.AL * j.AR, tree_row_lanes(j.AL), true, sc, &terr, group ? j.pg->basic_map.data() : nullptr,
+                         group ? j.pg->cut_local.data() : nullptr, (int)j.pg->cut_local.size()) != MTP_OK) continue;
+        if (tree_jit_smem_bytes(sc.n_val, sc.n_adj, j.AR, tree_threads(j.AL)) > 225 * 1024) continue;
         std::string why;
-        pg->cubin[key] = tree_jit_compile(sc, AL, AR, &why);
-      });
-    }
+        j.pg->cubin[j.key] = tree_jit_compile(sc, j.AL, j.AR, &why);
+      }
+    };
+    std::vector<std::thread> workers;
+    const unsigned hw = std::max(1u, std::thread::hardware_concurrency());
+    for (unsigned t = 0; t < std::min<unsigned>(std::min(hw, 16u), (unsigned)jobs.size()); ++t) workers.emplace_back(work);
     for (auto &w : workers) w.join();
     for (auto &pg : h->progs)                  // drop failed compilations: get_tree then decides on its own
       for (auto it = pg.cubin.begin(); it != pg.cubin.end();) it = it->second.empty() ? pg.cubin.erase(it) : std::next(it);
