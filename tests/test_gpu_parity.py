@@ -170,6 +170,7 @@ def test_host_path_matches_device_path(lib, torch):
     pot.close()
 
 
+@pytest.mark.codegen
 def test_specialised_tree_kernel_is_bit_identical_to_the_interpreter(lib, torch):
     """MTP_OPT_TREE_CODEGEN: the NVRTC-specialised K2 keeps the interpreter's arithmetic order."""
     w = make_workload(3, n_basis_of(16), cells=18)            # 23 328 atoms: the AL = 32, AR = 2 shape
@@ -184,6 +185,7 @@ def test_specialised_tree_kernel_is_bit_identical_to_the_interpreter(lib, torch)
     print("specialised tree kernels in use:", used)
 
 
+@pytest.mark.codegen
 def test_large_launch_configuration_on_sampled_atoms(lib, torch):
     """The launch configuration bench.py times (config 4 structure, thread-parallel pair kernels, 64-atom
     tree CTAs, specialised K2, several chunks): E_i, F_k on sampled atoms against the oracle, sum F = 0."""
@@ -229,6 +231,7 @@ def _check_sampled(w, got, n_sample, seed):
     assert np.all(np.abs(got["F"].sum(axis=0)) <= 1e-9 * np.abs(got["F"]).sum())
 
 
+@pytest.mark.codegen
 def test_full_size_config4_sampled(lib, torch):
     """BASELINE.json configs[3] at full size (1,048,576 atoms, level 16), default options = what bench.py times."""
     w = make_workload(3, n_basis_of(16))
@@ -238,6 +241,7 @@ def test_full_size_config4_sampled(lib, torch):
     _check_sampled(w, got, 4, 11)
 
 
+@pytest.mark.codegen
 def test_full_size_config3_sampled(lib, torch):
     """BASELINE.json configs[2] at full size (54,000 atoms, 2 species, level 20)."""
     w = make_workload(2, n_basis_of(20))
@@ -247,6 +251,7 @@ def test_full_size_config3_sampled(lib, torch):
     _check_sampled(w, got, 2, 12)
 
 
+@pytest.mark.codegen
 def test_full_size_config5_sampled_energy_and_grades(lib, torch):
     """BASELINE.json configs[4] at full size (250,000 atoms, level 24): E_i, B and both grade modes on sampled atoms."""
     nb = n_basis_of(24)
@@ -311,10 +316,9 @@ def test_error_codes_for_bad_tables_and_small_workspace(lib, torch):
     pot.close()
 
 
-def test_level28_partitioned_tree_interpreted(lib, torch, monkeypatch):
+def test_level28_partitioned_tree_interpreted(lib, torch):
     """Level 28 (9 739 basis functions): one atom's node values exceed shared memory, so the table only runs
     partitioned (132 group programs + top program).  Interpreter path (code generation off keeps create fast)."""
-    monkeypatch.setenv("MTP_TREE_CODEGEN", "0")
     lev, n_mu = 28, 7
     assert lib.Table(lev).plan()["partitioned"] == 1
     w = cluster_workload(lev, n_mu, 33, 8, 2, r_list=5.0)
