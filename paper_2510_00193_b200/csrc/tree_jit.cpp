@@ -96,6 +96,13 @@ struct TreeArgs {
 #define E(OA, OB) { const double2 X = LD(s0 + OA), Y = LD(vc + OB); ax = fma(X.x, Y.x, ax); ay = fma(X.y, Y.y, ay); }
 #define G0(M) { tx = __dmul_rn(M, ax); ty = __dmul_rn(M, ay); }
 #define GC(M) { tx = fma(M, ax, tx); ty = fma(M, ay, ty); }
+// exact shortcuts: a first factor that is the constant 1 (adj slot 0), a multiplier 1, a row that is the only
+// contribution to an adjoint whose initial value I is known here
+#define Y0(OB) { const double2 Y = LD(vc + OB); ax = Y.x; ay = Y.y; }
+#define Y1(OB) { const double2 Y = LD(vc + OB); ax += Y.x; ay += Y.y; }
+#define G1() { tx = ax; ty = ay; }
+#define RS(D) { *(double2 *)(ac + D) = make_double2(tx, ty); }
+#define RI(D, I) { *(double2 *)(ac + D) = make_double2(I + tx, I + ty); }
 #define RV(D) { *(double2 *)(vw + D) = make_double2(tx, ty); }
 #define RL(S) { ex = fma(S, tx, ex); ey = fma(S, ty, ey); }
 #define RA(D) { double2 o = LD(ac + D); o.x += tx; o.y += ty; *(double2 *)(ac + D) = o; }
@@ -111,6 +118,11 @@ struct TreeArgs {
 #define E(OA, OB) { ax = fma(LD(s0 + OA), LD(vc + OB), ax); }
 #define G0(M) { tx = __dmul_rn(M, ax); }
 #define GC(M) { tx = fma(M, ax, tx); }
+#define Y0(OB) { ax = LD(vc + OB); }
+#define Y1(OB) { ax += LD(vc + OB); }
+#define G1() { tx = ax; }
+#define RS(D) { *(double *)(ac + D) = tx; }
+#define RI(D, I) { *(double *)(ac + D) = I + tx; }
 #define RV(D) { *(double *)(vw + D) = tx; }
 #define RL(S) { ex = fma(S, tx, ex); }
 #define RA(D) { *(double *)(ac + D) += tx; }
@@ -216,9 +228,11 @@ void replace_all(std::string &s, const std::string &key, const std::string &val)
 }
 
 // straight-line source of one pass: per wave a switch over the row-lane, then the CTA barrier
+// adj_init (backward pass of a whole table only): initial adjoints by slot, for the store-instead-of-add rows
 std::string gen_pass(const std::vector<TreeTerm> &prog, const std::vector<int32_t> &wave, int R, bool bwd,
-                     const std::vector<double> &leaf_seed, int A) {
+                     const std::vector<double> &leaf_seed, int A, const std::vector<double> *adj_init = nullptr) {
   std::string out;
+  std::vector<char> added(adj_init ? adj_init->size() : 0, 0);   // adjoint slots a row has already been added to
   out.reserve(prog.size() * 24);
   char buf[160];
   const unsigned row = (unsigned)A * 8u;
@@ -234,11 +248,13 @@ std::string gen_pass(const std::vector<TreeTerm> &prog, const std::vector<int32_
       bool acc_open = false, tot_open = false;      // does acc / tot hold a partial sum?
       for (int s = wave[w]; s <= last; ++s) {
         const TreeTerm &t = prog[(size_t)s * R + l];
-        snprintf(buf, sizeof buf, "%s(%u,%u)", acc_open ? "E" : "E0", t.a & ~7u, t.b & kTreeBMask);
+        if (bwd && (t.a & ~7u) == 0) snprintf(buf, sizeof buf, "%s(%u)", acc_open ? "Y1" : "Y0", t.b & kTreeBMask);
+        else snprintf(buf, sizeof buf, "%s(%u,%u)", acc_open ? "E" : "E0", t.a & ~7u, t.b & kTreeBMask);
         out += buf;
         acc_open = true;
         if (t.a & kTreeGroup) {
-          snprintf(buf, sizeof buf, "%s(%a)", tot_open ? "GC" : "G0", t.mult);
+          if (!tot_open && t.mult == 1.0) snprintf(buf, sizeof buf, "G1()");
+          else snprintf(buf, sizeof buf, "%s(%a)", tot_open ? "GC" : "G0", t.mult);
           out += buf;
           acc_open = false; tot_open = true;
           if (t.a & kTreeRow) {
@@ -249,6 +265,11 @@ std::string gen_pass(const std::vector<TreeTerm> &prog, const std::vector<int32_
             } else {
               if (t.a & kTreeAlt) snprintf(buf, sizeof buf, "RG(%u)", d);
               else if (t.b & kTreeAcc) snprintf(buf, sizeof buf, "RV(%u)", d * row);     // partial sum of a split row
+              else if (adj_init && d < added.size() && !added[d]) {
+                added[d] = 1;
+                if ((*adj_init)[d] == 0.0) snprintf(buf, sizeof buf, "RS(%u)", d * row);
+                else snprintf(buf, sizeof buf, "RI(%u,%a)", d * row, (*adj_init)[d]);
+              }
               else snprintf(buf, sizeof buf, "RA(%u)", d * row);
             }
             out += buf;
@@ -297,7 +318,7 @@ std::vector<char> tree_jit_compile(const TreeSched &sc, int AL, int AR, std::str
   replace_all(src, "@NT@", std::to_string(NT));
   replace_all(src, "@GRP@", sc.mload_k.empty() ? "0" : "1");
   replace_all(src, "@FWD@", gen_pass(sc.fprog, sc.fwave, R, false, sc.leaf_seed, AL * AR));
-  replace_all(src, "@BWD@", gen_pass(sc.bprog, sc.bwave, R, true, sc.leaf_seed, AL * AR));
+  replace_all(src, "@BWD@", gen_pass(sc.bprog, sc.bwave, R, true, sc.leaf_seed, AL * AR, sc.mload_k.empty() ? &sc.adj_init : nullptr));
   nvrtcProgram prog = nullptr;
   if (rt.CreateProgram(&prog, src.c_str(), "k_tree_gen.cu", 0, nullptr, nullptr) != 0) { *why = "nvrtcCreateProgram failed"; return cubin; }
   const char *opts[] = {"--gpu-architecture=sm_100a", "--std=c++17", "-lineinfo", "-default-device"};
