@@ -170,6 +170,33 @@ def test_host_path_matches_device_path(lib, torch):
     pot.close()
 
 
+def test_cuda_graph_replay_of_a_call_is_bit_identical(lib, torch):
+    """mtp_compute only enqueues on the caller's stream (include/mtp_b200.h): a captured call replays exactly."""
+    w = make_workload(1, n_basis_of(16), cells=4)
+    a, pot, d = run_gpu(lib, torch, w, opts={lib.OPT_FORCE_MODE: lib.FORCE_GATHER})
+    out = pot.compute(d["pos"], d["types"], w.box, d["off"], d["idx"], d["shift"], d["rev"])
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        pot.compute(d["pos"], d["types"], w.box, d["off"], d["idx"], d["shift"], d["rev"], out=out)
+    for v in out.values():
+        v.fill_(float("nan"))
+    g.replay()
+    torch.cuda.synchronize()
+    for k in ("E", "Ei", "F", "virial"):
+        assert np.array_equal(out[k].cpu().numpy(), a[k]), k
+    d["pos"].add_(0.01 * torch.randn_like(d["pos"]))      # same buffers, new coordinates: the graph follows the data
+    g.replay()
+    torch.cuda.synchronize()
+    b = {k: v.cpu().numpy().copy() for k, v in out.items()}
+    ref = pot.compute(d["pos"], d["types"], w.box, d["off"], d["idx"], d["shift"], d["rev"])
+    torch.cuda.synchronize()
+    for k in ("E", "Ei", "F", "virial"):
+        assert np.array_equal(ref[k].cpu().numpy(), b[k]), k
+    pot.close()
+
+
 @pytest.mark.codegen
 def test_specialised_tree_kernel_is_bit_identical_to_the_interpreter(lib, torch):
     """MTP_OPT_TREE_CODEGEN: the NVRTC-specialised K2 keeps the interpreter's arithmetic order."""
