@@ -94,7 +94,11 @@ const char *mtp_last_error(const mtp_handle *h); /* h may be NULL: last create e
 #define MTP_OPT_PROFILE 4       /* 1: record CUDA events around every kernel launch        */
 #define MTP_OPT_TREE_CODEGEN 5  /* 1 (default): specialise the contraction kernel for the table with NVRTC at
                                    first use when the table is short enough; 0: always interpret the table.
-                                   Same arithmetic order either way (bit-identical results).             */
+                                   Same arithmetic order either way (bit-identical results).
+                                   Environment, read when a table is specialised: MTP_TREE_CODEGEN=0 (as option 0),
+                                   MTP_TREE_FORM=shared (one code body per row shape + operand tables instead of
+                                   straight-line code; bit-identical, currently slower: DESIGN.md section 11),
+                                   MTP_TREE_DUMP=<path> (write the generated CUDA source there).         */
 #define MTP_INFO_TREE_KERNELS 100 /* mtp_get_option only: number of NVRTC-specialised contraction kernels in use */
 #define MTP_FORCE_GATHER 0      /* deterministic; keeps d_ij for all pairs (nnz x 32 B)  */
 #define MTP_FORCE_ATOMIC 1      /* fp64 atomic scatter; no per-pair scratch              */

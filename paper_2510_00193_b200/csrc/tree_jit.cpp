@@ -11,6 +11,7 @@
 #include <dlfcn.h>
 
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -82,6 +83,9 @@ struct TreeArgs {
   int g_accum;
   int write_energy;
 };
+// four table offsets with one 16-byte load through L1 (the tables are streamed once per atom group: global memory,
+// not the constant bank, whose cache is made for reuse -- measured 4.2 ms against 2.8 ms of the straight-line form)
+__device__ __forceinline__ uint4 LQ(const uint4 *p) { return __ldg(p); }
 #define AR @AR@
 #define GRP @GRP@        // 1: group sub-program of a partitioned tree (subset loads, per-atom seeds, G accumulates)
 #define NT @NT@
@@ -134,6 +138,7 @@ struct TreeArgs {
 #endif
 #endif
 
+@TABLES@
 extern "C" __global__ void __launch_bounds__(NT, 1) k_tree_gen(const TreeArgs a) {
   extern __shared__ __align__(16) char smraw[];
   double *val = (double *)smraw;
@@ -284,6 +289,173 @@ std::string gen_pass(const std::vector<TreeTerm> &prog, const std::vector<int32_
   }
   return out;
 }
+
+// Shape-shared form of one pass (MTP_TREE_FORM=shared).  Rows of the same shape (entries per group, which
+// multipliers are 1, how the row is disposed of) run ONE code body; what differs between them -- operand offsets,
+// destination, multipliers, seeds -- comes from tables emitted as initialised __device__ const arrays and read
+// through L1 (the constant bank was tried first: its cache is built for reuse, the tables are streamed).  A
+// row-lane walks its rows of a wave in schedule order and dispatches on the shape, so every row does exactly the
+// arithmetic of the straight-line form, in the same order (bit-identical), but the code is ~80 KB instead of
+// ~220 KB at level 16 and stays in the instruction cache.
+//   tables (prefix f / b): X_row[r] = {shape, first offset, first multiplier, 0}; X_beg[w * R + l] .. [w * R + l + 1] = rows of
+//   row-lane l in wave w; X_off = byte offsets / destinations / run lengths, rows and runs padded to 16 bytes and
+//   read four at a time; X_mul = multipliers, initial adjoints, leaf seeds.
+// Returns the code; appends the tables to *tables and their size in bytes to *table_bytes.
+constexpr int kRunLoop = 6;      // plain entries in a row of one group from which a run is looped
+std::string gen_pass_shared(const std::vector<TreeTerm> &prog, const std::vector<int32_t> &wave, int R, bool bwd,
+                            const std::vector<double> &leaf_seed, int A, const std::vector<double> *adj_init,
+                            const char *pfx, std::string *tables, size_t *table_bytes) {
+  std::vector<char> added(adj_init ? adj_init->size() : 0, 0);
+  const unsigned row = (unsigned)A * 8u;
+  std::vector<std::string> bodies;                 // code of shape i
+  std::vector<std::string> keys;                   // its key
+  std::vector<int> rows;                           // shape, off0, mul0 per row
+  std::vector<int> beg;                            // [n_waves * R + 1]
+  std::vector<unsigned> off;
+  std::vector<double> mul;
+  char buf[512];
+  const size_t n_waves = wave.size() - 1;
+  for (size_t w = 0; w < n_waves; ++w)
+    for (int l = 0; l < R; ++l) {
+      beg.push_back((int)rows.size() / 3);
+      auto pad4 = [&] { while (off.size() & 3) off.push_back(0); };   // rows and runs start on 16 bytes: offsets are read four at a time
+      pad4();
+      int last = -1;
+      for (int s = wave[w]; s < wave[w + 1]; ++s)
+        if (prog[(size_t)s * R + l].a & kTreeRow) last = s;
+      std::string key, body, seg;                 // seg: text of the current segment, whose offsets are loaded up front
+      int seg_id = 0;
+      auto tq = [&](int k) { char t[32]; snprintf(t, sizeof t, "a%d_%d.%c", seg_id, k >> 2, "xyzw"[k & 3]); return std::string(t); };
+      int off0 = (int)off.size(), mul0 = (int)mul.size();
+      bool acc_open = false, tot_open = false;
+      int tcur = off0;                              // where the body's T4 points (moves past each run loop)
+      auto close_seg = [&] {                        // declare the segment's offsets: one 16-byte constant load per four
+        const int nq = ((int)off.size() - tcur + 3) / 4;
+        for (int i = 0; i < nq; ++i) { char t[64]; snprintf(t, sizeof t, "const uint4 a%d_%d=LQ(T4+%d);", seg_id, i, i); body += t; }
+        body += seg;
+        seg.clear();
+        ++seg_id;
+      };
+      for (int s = wave[w]; s <= last; ++s) {
+        const int io = (int)off.size() - tcur;
+        auto is_y = [&](const TreeTerm &q) { return bwd && (q.a & ~7u) == 0; };
+        // a long run of plain entries inside one group becomes a loop with its length in the table, so that
+        // rows which differ only in such lengths share a body (the FMA chain keeps its order)
+        int run = 0;
+        for (int s2 = s; s2 <= last; ++s2) {
+          const TreeTerm &q = prog[(size_t)s2 * R + l];
+          if (is_y(q)) break;
+          ++run;
+          if (q.a & kTreeGroup) break;
+        }
+        if (!acc_open) run = 0;                     // a group's first entry opens the accumulator outside the loop
+        if (run >= kRunLoop) {
+          off.push_back((unsigned)run);
+          seg += "{int n=" + tq(io) + ";";
+          pad4();
+          const int qpos = ((int)off.size() - tcur) / 4;
+          close_seg();
+          snprintf(buf, sizeof buf, "const uint4*q=T4+%d;\n_Pragma(\"unroll 1\")\nfor(;n>=2;n-=2,++q){const uint4 v=LQ(q);E(v.x,v.y)E(v.z,v.w)}"
+                   "if(n){const uint4 v=LQ(q);E(v.x,v.y)++q;}T4=q;}", qpos);
+          body += buf;
+          key += 'F';
+          for (int s2 = s; s2 < s + run; ++s2) {
+            const TreeTerm &q = prog[(size_t)s2 * R + l];
+            off.push_back(q.a & ~7u); off.push_back(q.b & kTreeBMask);
+          }
+          pad4();
+          tcur = (int)off.size();
+          s += run - 1;
+        }
+        const TreeTerm &t = prog[(size_t)s * R + l];
+        if (run >= kRunLoop) {
+        } else if (is_y(t)) {
+          seg += std::string(acc_open ? "Y1(" : "Y0(") + tq(io) + ")";
+          off.push_back(t.b & kTreeBMask);
+          key += 'y';
+        } else {
+          seg += std::string(acc_open ? "E(" : "E0(") + tq(io) + "," + tq(io + 1) + ")";
+          off.push_back(t.a & ~7u); off.push_back(t.b & kTreeBMask);
+          key += 'e';
+        }
+        acc_open = true;
+        if (t.a & kTreeGroup) {
+          if (!tot_open && t.mult == 1.0) { snprintf(buf, sizeof buf, "G1()"); key += '1'; }
+          else {
+            snprintf(buf, sizeof buf, "%s(__ldg(U+%d))", tot_open ? "GC" : "G0", (int)mul.size() - mul0);
+            mul.push_back(t.mult);
+            key += 'g';
+          }
+          seg += buf;
+          acc_open = false; tot_open = true;
+          if (t.a & kTreeRow) {
+            const unsigned d = t.b >> kTreeDstShift;
+            const int id = (int)off.size() - tcur, im = (int)mul.size() - mul0;
+            if (!bwd) {
+              if (t.a & kTreeAlt) { snprintf(buf, sizeof buf, "RL(__ldg(U+%d))", im); mul.push_back(leaf_seed[d]); key += 'L'; }
+              else { snprintf(buf, sizeof buf, "RV(%s)", tq(id).c_str()); off.push_back(d * row); key += 'V'; }
+            } else {
+              if (t.a & kTreeAlt) { snprintf(buf, sizeof buf, "RG(%s)", tq(id).c_str()); off.push_back(d); key += 'G'; }
+              else if (t.b & kTreeAcc) { snprintf(buf, sizeof buf, "RV(%s)", tq(id).c_str()); off.push_back(d * row); key += 'V'; }
+              else if (adj_init && d < added.size() && !added[d]) {
+                added[d] = 1;
+                if ((*adj_init)[d] == 0.0) { snprintf(buf, sizeof buf, "RS(%s)", tq(id).c_str()); off.push_back(d * row); key += 'S'; }
+                else { snprintf(buf, sizeof buf, "RI(%s,__ldg(U+%d))", tq(id).c_str(), im); off.push_back(d * row); mul.push_back((*adj_init)[d]); key += 'I'; }
+              }
+              else { snprintf(buf, sizeof buf, "RA(%s)", tq(id).c_str()); off.push_back(d * row); key += 'A'; }
+            }
+            seg += buf;
+            close_seg();
+            tot_open = false;
+            seg_id = 0;
+            // the row is complete: find or add its shape
+            size_t sh = 0;
+            while (sh < keys.size() && keys[sh] != key) ++sh;
+            if (sh == keys.size()) { keys.push_back(key); bodies.push_back(body); }
+            rows.push_back((int)sh); rows.push_back(off0); rows.push_back(mul0);
+            key.clear(); body.clear();
+            pad4();
+            off0 = (int)off.size(); mul0 = (int)mul.size();
+            tcur = off0;
+          }
+        }
+      }
+    }
+  beg.push_back((int)rows.size() / 3);
+  // ---- tables
+  std::string &tb = *tables;
+  const std::string P = pfx;
+  tb += "__device__ const int4 " + P + "_row[] = {";
+  for (size_t r = 0; r < rows.size() / 3; ++r) { snprintf(buf, sizeof buf, "{%d,%d,%d,0},", rows[3 * r], rows[3 * r + 1], rows[3 * r + 2]); tb += buf; }
+  tb += "{0,0,0,0}};\n__device__ const int " + P + "_beg[] = {";
+  for (int b : beg) { snprintf(buf, sizeof buf, "%d,", b); tb += buf; }
+  tb += "0};\n__device__ const __align__(16) unsigned " + P + "_off[] = {";
+  for (unsigned o : off) { snprintf(buf, sizeof buf, "%u,", o); tb += buf; }
+  tb += "0};\n__device__ const double " + P + "_mul[] = {";
+  for (double m : mul) { snprintf(buf, sizeof buf, "%a,", m); tb += buf; }
+  tb += "0.0};\n";
+  *table_bytes += rows.size() / 3 * 16 + 16 + beg.size() * 4 + 4 + off.size() * 4 + 4 + mul.size() * 8 + 8;
+  // ---- code: one copy of every body per pass; the waves are a loop around the dispatch
+  std::string out;
+  snprintf(buf, sizeof buf, "      _Pragma(\"unroll 1\")\n      for (int w = 0; w < %zu; ++w) {\n", n_waves);
+  out += buf;
+  out += "      int r = __ldg(" + P + "_beg + w * R + rl); const int r1 = __ldg(" + P + "_beg + w * R + rl + 1);\n";
+  out += "      int4 rn = __ldg(" + P + "_row + r);\n";
+  out += "      for (; r < r1; ++r) {\n";
+  // the row record is fetched one row ahead (the table ends with a spare record); prefetching the lines of the
+  // other two streams a few rows ahead as well was measured and changed nothing
+  out += "        const int4 rr = rn; rn = __ldg(" + P + "_row + r + 1);\n";
+  out += "        const uint4 *T4 = (const uint4 *)(" + P + "_off + rr.y); const double *U = " + P + "_mul + rr.z;\n";
+  out += "        switch (rr.x) {\n";
+  for (size_t sh = 0; sh < keys.size(); ++sh) {
+    snprintf(buf, sizeof buf, "        case %zu: { ", sh);
+    out += buf;
+    out += bodies[sh];
+    out += " } break;\n";
+  }
+  out += "        default: break;\n        }\n      }\n      __syncthreads();\n      }\n";
+  return out;
+}
 }  // namespace
 
 // shared memory of the generated kernel: val + adj + energy partials [NT][AR]
@@ -317,8 +489,30 @@ std::vector<char> tree_jit_compile(const TreeSched &sc, int AL, int AR, std::str
   replace_all(src, "@AR@", std::to_string(AR));
   replace_all(src, "@NT@", std::to_string(NT));
   replace_all(src, "@GRP@", sc.mload_k.empty() ? "0" : "1");
-  replace_all(src, "@FWD@", gen_pass(sc.fprog, sc.fwave, R, false, sc.leaf_seed, AL * AR));
-  replace_all(src, "@BWD@", gen_pass(sc.bprog, sc.bwave, R, true, sc.leaf_seed, AL * AR, sc.mload_k.empty() ? &sc.adj_init : nullptr));
+  // Two forms of the generated code: straight-line (default) and shape-shared bodies with operand tables
+  // (MTP_TREE_FORM=shared; same arithmetic, bit-identical).  Measured at config 4: 2.82 ms against 4.08 ms -- the
+  // shared form cures the instruction-fetch stall but pays for it in table-load latency and barrier imbalance
+  // (DESIGN.md section 11), so it stays an option until that is fixed.
+  std::string tables;
+  size_t table_bytes = 0;
+  const char *form = getenv("MTP_TREE_FORM");
+  std::string fwd, bwd;
+  if (form && form[0] == 's') {
+    fwd = gen_pass_shared(sc.fprog, sc.fwave, R, false, sc.leaf_seed, AL * AR, nullptr, "f", &tables, &table_bytes);
+    bwd = gen_pass_shared(sc.bprog, sc.bwave, R, true, sc.leaf_seed, AL * AR, sc.mload_k.empty() ? &sc.adj_init : nullptr, "b",
+                          &tables, &table_bytes);
+  }
+  if (table_bytes == 0 || table_bytes > 60 * 1024) {      // larger tables: not measured, keep the straight-line form
+    tables.clear();
+    fwd = gen_pass(sc.fprog, sc.fwave, R, false, sc.leaf_seed, AL * AR);
+    bwd = gen_pass(sc.bprog, sc.bwave, R, true, sc.leaf_seed, AL * AR, sc.mload_k.empty() ? &sc.adj_init : nullptr);
+  }
+  replace_all(src, "@TABLES@", tables);
+  replace_all(src, "@FWD@", fwd);
+  replace_all(src, "@BWD@", bwd);
+  if (const char *dump = getenv("MTP_TREE_DUMP")) {      // debugging aid: the generated source of the last compiled program
+    if (FILE *f = fopen(dump, "w")) { fputs(src.c_str(), f); fclose(f); }
+  }
   nvrtcProgram prog = nullptr;
   if (rt.CreateProgram(&prog, src.c_str(), "k_tree_gen.cu", 0, nullptr, nullptr) != 0) { *why = "nvrtcCreateProgram failed"; return cubin; }
   const char *opts[] = {"--gpu-architecture=sm_100a", "--std=c++17", "-lineinfo", "-default-device"};

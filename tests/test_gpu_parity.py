@@ -198,8 +198,11 @@ def test_cuda_graph_replay_of_a_call_is_bit_identical(lib, torch):
 
 
 @pytest.mark.codegen
-def test_specialised_tree_kernel_is_bit_identical_to_the_interpreter(lib, torch):
-    """MTP_OPT_TREE_CODEGEN: the NVRTC-specialised K2 keeps the interpreter's arithmetic order."""
+@pytest.mark.parametrize("form", ["line", "shared"])
+def test_specialised_tree_kernel_is_bit_identical_to_the_interpreter(lib, torch, form, monkeypatch):
+    """MTP_OPT_TREE_CODEGEN: the NVRTC-specialised K2 keeps the interpreter's arithmetic order, in both forms of
+    the generated code (straight-line, and MTP_TREE_FORM=shared: one body per row shape + operand tables)."""
+    monkeypatch.setenv("MTP_TREE_FORM", form)
     w = make_workload(3, n_basis_of(16), cells=18)            # 23 328 atoms: the AL = 32, AR = 2 shape
     a, pot, d = run_gpu(lib, torch, w, opts={lib.OPT_TREE_CODEGEN: 0, lib.OPT_VARIANT: lib.VARIANT_THREAD})
     assert pot.get_option(lib.INFO_TREE_KERNELS) == 0
