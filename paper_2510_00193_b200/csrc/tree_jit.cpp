@@ -234,12 +234,17 @@ void replace_all(std::string &s, const std::string &key, const std::string &val)
 
 // straight-line source of one pass: per wave a switch over the row-lane, then the CTA barrier
 // adj_init (backward pass of a whole table only): initial adjoints by slot, for the store-instead-of-add rows
+// runs: when given, a run of >= kLineRun plain entries inside one group is emitted as a loop over a table of operand
+// offsets (appended to *runs, emitted by the caller as the __device__ const array `l_off`) instead of 4 instructions
+// per entry: the long backward groups are a quarter of the straight-line code, which is what bounds the kernel.
+constexpr int kLineRun = 10;
 std::string gen_pass(const std::vector<TreeTerm> &prog, const std::vector<int32_t> &wave, int R, bool bwd,
-                     const std::vector<double> &leaf_seed, int A, const std::vector<double> *adj_init = nullptr) {
+                     const std::vector<double> &leaf_seed, int A, const std::vector<double> *adj_init = nullptr,
+                     std::vector<unsigned> *runs = nullptr) {
   std::string out;
   std::vector<char> added(adj_init ? adj_init->size() : 0, 0);   // adjoint slots a row has already been added to
   out.reserve(prog.size() * 24);
-  char buf[160];
+  char buf[400];
   const unsigned row = (unsigned)A * 8u;
   for (size_t w = 0; w + 1 < wave.size(); ++w) {
     out += "      switch (rl) {\n";
@@ -252,8 +257,29 @@ std::string gen_pass(const std::vector<TreeTerm> &prog, const std::vector<int32_
       out += buf;
       bool acc_open = false, tot_open = false;      // does acc / tot hold a partial sum?
       for (int s = wave[w]; s <= last; ++s) {
+        int run = 0;                                  // plain entries from here to the end of the group
+        if (runs && acc_open)
+          for (int s2 = s; s2 <= last; ++s2) {
+            const TreeTerm &q = prog[(size_t)s2 * R + l];
+            if (bwd && (q.a & ~7u) == 0) break;
+            ++run;
+            if (q.a & kTreeGroup) break;
+          }
+        if (run >= kLineRun) {
+          while (runs->size() & 3) runs->push_back(0);
+          snprintf(buf, sizeof buf, "{const uint4*q=(const uint4*)(l_off+%zu);int n=%d;\n_Pragma(\"unroll 1\")\n"
+                   "for(;n>=2;n-=2,++q){const uint4 v=LQ(q);E(v.x,v.y)E(v.z,v.w)}%s}",
+                   runs->size(), run, (run & 1) ? "{const uint4 v=LQ(q);E(v.x,v.y)}" : "");
+          out += buf;
+          for (int s2 = s; s2 < s + run; ++s2) {
+            const TreeTerm &q = prog[(size_t)s2 * R + l];
+            runs->push_back(q.a & ~7u); runs->push_back(q.b & kTreeBMask);
+          }
+          s += run - 1;
+        }
         const TreeTerm &t = prog[(size_t)s * R + l];
-        if (bwd && (t.a & ~7u) == 0) snprintf(buf, sizeof buf, "%s(%u)", acc_open ? "Y1" : "Y0", t.b & kTreeBMask);
+        if (run >= kLineRun) buf[0] = 0;
+        else if (bwd && (t.a & ~7u) == 0) snprintf(buf, sizeof buf, "%s(%u)", acc_open ? "Y1" : "Y0", t.b & kTreeBMask);
         else snprintf(buf, sizeof buf, "%s(%u,%u)", acc_open ? "E" : "E0", t.a & ~7u, t.b & kTreeBMask);
         out += buf;
         acc_open = true;
@@ -504,8 +530,16 @@ std::vector<char> tree_jit_compile(const TreeSched &sc, int AL, int AR, std::str
   }
   if (table_bytes == 0 || table_bytes > 60 * 1024) {      // larger tables: not measured, keep the straight-line form
     tables.clear();
-    fwd = gen_pass(sc.fprog, sc.fwave, R, false, sc.leaf_seed, AL * AR);
-    bwd = gen_pass(sc.bprog, sc.bwave, R, true, sc.leaf_seed, AL * AR, sc.mload_k.empty() ? &sc.adj_init : nullptr);
+    std::vector<unsigned> runs;                           // MTP_TREE_FORM=line: no run loops either (A/B measurements)
+    std::vector<unsigned> *rp = (form && form[0] == 'l') ? nullptr : &runs;
+    fwd = gen_pass(sc.fprog, sc.fwave, R, false, sc.leaf_seed, AL * AR, nullptr, rp);
+    bwd = gen_pass(sc.bprog, sc.bwave, R, true, sc.leaf_seed, AL * AR, sc.mload_k.empty() ? &sc.adj_init : nullptr, rp);
+    if (!runs.empty()) {
+      tables = "__device__ const __align__(16) unsigned l_off[] = {";
+      char t[16];
+      for (unsigned o : runs) { snprintf(t, sizeof t, "%u,", o); tables += t; }
+      tables += "0,0,0,0};\n";
+    }
   }
   replace_all(src, "@TABLES@", tables);
   replace_all(src, "@FWD@", fwd);
