@@ -98,6 +98,8 @@ const char *mtp_last_error(const mtp_handle *h); /* h may be NULL: last create e
                                    Environment, read when a table is specialised: MTP_TREE_CODEGEN=0 (as option 0),
                                    MTP_TREE_FORM=shared (one code body per row shape + operand tables instead of
                                    straight-line code; bit-identical, currently slower: DESIGN.md section 11),
+                                   MTP_TREE_FORM=line (no run loops: every entry as straight-line code),
+                                   MTP_TREE_RUN=<n> (shortest run of plain entries emitted as a loop, default 10),
                                    MTP_TREE_DUMP=<path> (write the generated CUDA source there).         */
 #define MTP_INFO_TREE_KERNELS 100 /* mtp_get_option only: number of NVRTC-specialised contraction kernels in use */
 #define MTP_FORCE_GATHER 0      /* deterministic; keeps d_ij for all pairs (nnz x 32 B)  */

@@ -238,10 +238,12 @@ void replace_all(std::string &s, const std::string &key, const std::string &val)
 // offsets (appended to *runs, emitted by the caller as the __device__ const array `l_off`) instead of 4 instructions
 // per entry: the long backward groups are a quarter of the straight-line code, which is what bounds the kernel.
 constexpr int kLineRun = 10;
+static int line_run() { const char *e = getenv("MTP_TREE_RUN"); const int v = e ? atoi(e) : 0; return v >= 3 ? v : kLineRun; }
 std::string gen_pass(const std::vector<TreeTerm> &prog, const std::vector<int32_t> &wave, int R, bool bwd,
                      const std::vector<double> &leaf_seed, int A, const std::vector<double> *adj_init = nullptr,
                      std::vector<unsigned> *runs = nullptr) {
   std::string out;
+  const int min_run = line_run();
   std::vector<char> added(adj_init ? adj_init->size() : 0, 0);   // adjoint slots a row has already been added to
   out.reserve(prog.size() * 24);
   char buf[400];
@@ -265,7 +267,7 @@ std::string gen_pass(const std::vector<TreeTerm> &prog, const std::vector<int32_
             ++run;
             if (q.a & kTreeGroup) break;
           }
-        if (run >= kLineRun) {
+        if (run >= min_run) {
           while (runs->size() & 3) runs->push_back(0);
           snprintf(buf, sizeof buf, "{const uint4*q=(const uint4*)(l_off+%zu);int n=%d;\n_Pragma(\"unroll 1\")\n"
                    "for(;n>=2;n-=2,++q){const uint4 v=LQ(q);E(v.x,v.y)E(v.z,v.w)}%s}",
@@ -278,7 +280,7 @@ std::string gen_pass(const std::vector<TreeTerm> &prog, const std::vector<int32_
           s += run - 1;
         }
         const TreeTerm &t = prog[(size_t)s * R + l];
-        if (run >= kLineRun) buf[0] = 0;
+        if (run >= min_run) buf[0] = 0;
         else if (bwd && (t.a & ~7u) == 0) snprintf(buf, sizeof buf, "%s(%u)", acc_open ? "Y1" : "Y0", t.b & kTreeBMask);
         else snprintf(buf, sizeof buf, "%s(%u,%u)", acc_open ? "E" : "E0", t.a & ~7u, t.b & kTreeBMask);
         out += buf;
