@@ -504,7 +504,7 @@ int make_plan(const mtp_handle *h, int64_t N, int64_t nnz, int want_grade, int h
   }
   if (C > N) C = std::max<int64_t>(N, 1);
   pl.C = C;
-  pl.ldm = (C + 31) / 32 * 32;
+  pl.ldm = (C + 63) / 64 * 64;            // whole 64-atom K2 groups: the generated kernel stores G rows unpredicated
   pl.n_chunks = N ? (int)((N + C - 1) / C) : 0;
   const int NS = h->pl->nsb * h->pl->nsc;
   if (h->variant == MTP_VARIANT_THREAD) pl.P = 1;

@@ -10,6 +10,7 @@
 #include <cuda_runtime.h>
 #include <dlfcn.h>
 
+#include <cstdint>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -110,11 +111,14 @@ __device__ __forceinline__ uint4 LQ(const uint4 *p) { return __ldg(p); }
 #define RV(D) { *(double2 *)(vw + D) = make_double2(tx, ty); }
 #define RL(S) { ex = fma(S, tx, ex); ey = fma(S, ty, ey); }
 #define RA(D) { double2 o = LD(ac + D); o.x += tx; o.y += ty; *(double2 *)(ac + D) = o; }
-#define RGA(K) { double *gp = Gcol + (long long)K * ldm; if (n_ok > 0) gp[0] += tx; if (n_ok > 1) gp[1] += ty; }   // later piece of a split row
+// rows of G: ldm is a multiple of 64 (api.cu make_plan) and a lane's two atoms sit on 16 bytes, so a row is one
+// unpredicated 16-byte store at a 32-bit index (the columns of atoms past the chunk's end are padding)
+#define GP(K) ((double2 *)(Gcol + (unsigned)(K) * ldm32))
+#define RGA(K) { double2 *gp = GP(K); double2 o = *gp; o.x += tx; o.y += ty; *gp = o; }   // later piece of a split row
 #if GRP
-#define RG(K) { double *gp = Gcol + (long long)K * ldm; if (n_ok > 0) gp[0] = ga ? gp[0] + tx : tx; if (n_ok > 1) gp[1] = ga ? gp[1] + ty : ty; }
+#define RG(K) { double2 *gp = GP(K); double2 o = make_double2(tx, ty); if (ga) { const double2 p = *gp; o.x = p.x + tx; o.y = p.y + ty; } *gp = o; }
 #else
-#define RG(K) { if (n_ok > 0) Gcol[(long long)K * ldm] = tx; if (n_ok > 1) Gcol[(long long)K * ldm + 1] = ty; }
+#define RG(K) { *GP(K) = make_double2(tx, ty); }
 #endif
 #else
 #define LD(p) (*(const double *)(p))
@@ -149,6 +153,7 @@ extern "C" __global__ void __launch_bounds__(NT, 1) k_tree_gen(const TreeArgs a)
   char *vw = smraw + al * AR * 8;
   char *ac = (char *)adj + al * AR * 8;
   const long long ldm = a.ldm;
+  const unsigned ldm32 = (unsigned)a.ldm; (void)ldm32;
   const int n_groups = (a.c1 - a.c0 + A - 1) / A;
   for (int g = blockIdx.x; g < n_groups; g += gridDim.x) {
     const int atom0 = a.c0 + g * A + al * AR;
@@ -594,6 +599,7 @@ cudaError_t tree_jit_launch(const TreeJit *j, const TreeArgs &a, cudaStream_t st
   const int Aat = 32 * j->AR;
   const int groups = (a.c1 - a.c0 + Aat - 1) / Aat;
   if (groups <= 0) return cudaSuccess;
+  if (j->AR == 2 && ((a.ldm & 63) || ((uintptr_t)a.G & 15))) return cudaErrorMisalignedAddress;   // unpredicated G rows (RG)
   static int sms = 0;
   if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
   const size_t smem = tree_jit_smem_bytes(a.n_val, a.n_adj, j->AR, j->NT);
