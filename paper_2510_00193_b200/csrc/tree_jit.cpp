@@ -243,12 +243,26 @@ void replace_all(std::string &s, const std::string &key, const std::string &val)
 // offsets (appended to *runs, emitted by the caller as the __device__ const array `l_off`) instead of 4 instructions
 // per entry: the long backward groups are a quarter of the straight-line code, which is what bounds the kernel.
 constexpr int kLineRun = 10;
+constexpr size_t kMaxConstMul = 6000;      // doubles in the constant bank (48 of its 64 KB)
 static int line_run() { const char *e = getenv("MTP_TREE_RUN"); const int v = e ? atoi(e) : 0; return v >= 3 ? v : kLineRun; }
 std::string gen_pass(const std::vector<TreeTerm> &prog, const std::vector<int32_t> &wave, int R, bool bwd,
                      const std::vector<double> &leaf_seed, int A, const std::vector<double> *adj_init = nullptr,
-                     std::vector<unsigned> *runs = nullptr) {
+                     std::vector<unsigned> *runs = nullptr, std::vector<double> *cmul = nullptr) {
   std::string out;
   const int min_run = line_run();
+  // multipliers and seeds: as operands from the constant bank (`cm[i]`, no instruction of their own) while the
+  // bank has room, else as literals (two moves each)
+  auto mref = [&](double v) {
+    char t[40];
+    if (cmul) {
+      size_t i = 0;
+      while (i < cmul->size() && memcmp(&(*cmul)[i], &v, 8) != 0) ++i;
+      if (i == cmul->size() && cmul->size() < kMaxConstMul) cmul->push_back(v);
+      if (i < cmul->size()) { snprintf(t, sizeof t, "cm[%zu]", i); return std::string(t); }
+    }
+    snprintf(t, sizeof t, "%a", v);
+    return std::string(t);
+  };
   std::vector<char> added(adj_init ? adj_init->size() : 0, 0);   // adjoint slots a row has already been added to
   out.reserve(prog.size() * 24);
   char buf[400];
@@ -292,13 +306,13 @@ std::string gen_pass(const std::vector<TreeTerm> &prog, const std::vector<int32_
         acc_open = true;
         if (t.a & kTreeGroup) {
           if (!tot_open && t.mult == 1.0) snprintf(buf, sizeof buf, "G1()");
-          else snprintf(buf, sizeof buf, "%s(%a)", tot_open ? "GC" : "G0", t.mult);
+          else snprintf(buf, sizeof buf, "%s(%s)", tot_open ? "GC" : "G0", mref(t.mult).c_str());
           out += buf;
           acc_open = false; tot_open = true;
           if (t.a & kTreeRow) {
             const unsigned d = t.b >> kTreeDstShift;
             if (!bwd) {
-              if (t.a & kTreeAlt) snprintf(buf, sizeof buf, "RL(%a)", leaf_seed[d]);
+              if (t.a & kTreeAlt) snprintf(buf, sizeof buf, "RL(%s)", mref(leaf_seed[d]).c_str());
               else snprintf(buf, sizeof buf, "RV(%u)", d * row);
             } else {
               if (t.a & kTreeAlt) snprintf(buf, sizeof buf, "RG(%u)", d);
@@ -306,7 +320,7 @@ std::string gen_pass(const std::vector<TreeTerm> &prog, const std::vector<int32_
               else if (adj_init && d < added.size() && !added[d]) {
                 added[d] = 1;
                 if ((*adj_init)[d] == 0.0) snprintf(buf, sizeof buf, "RS(%u)", d * row);
-                else snprintf(buf, sizeof buf, "RI(%u,%a)", d * row, (*adj_init)[d]);
+                else snprintf(buf, sizeof buf, "RI(%u,%s)", d * row, mref((*adj_init)[d]).c_str());
               }
               else snprintf(buf, sizeof buf, "RA(%u)", d * row);
             }
@@ -539,10 +553,18 @@ std::vector<char> tree_jit_compile(const TreeSched &sc, int AL, int AR, std::str
     tables.clear();
     std::vector<unsigned> runs;                           // MTP_TREE_FORM=line: no run loops either (A/B measurements)
     std::vector<unsigned> *rp = (form && form[0] == 'l') ? nullptr : &runs;
-    fwd = gen_pass(sc.fprog, sc.fwave, R, false, sc.leaf_seed, AL * AR, nullptr, rp);
-    bwd = gen_pass(sc.bprog, sc.bwave, R, true, sc.leaf_seed, AL * AR, sc.mload_k.empty() ? &sc.adj_init : nullptr, rp);
+    std::vector<double> cmul;
+    std::vector<double> *cp = (form && form[0] == 'l') ? nullptr : &cmul;
+    fwd = gen_pass(sc.fprog, sc.fwave, R, false, sc.leaf_seed, AL * AR, nullptr, rp, cp);
+    bwd = gen_pass(sc.bprog, sc.bwave, R, true, sc.leaf_seed, AL * AR, sc.mload_k.empty() ? &sc.adj_init : nullptr, rp, cp);
+    if (!cmul.empty()) {
+      tables += "__constant__ double cm[] = {";
+      char t[40];
+      for (double m : cmul) { snprintf(t, sizeof t, "%a,", m); tables += t; }
+      tables += "0.0};\n";
+    }
     if (!runs.empty()) {
-      tables = "__device__ const __align__(16) unsigned l_off[] = {";
+      tables += "__device__ const __align__(16) unsigned l_off[] = {";
       char t[16];
       for (unsigned o : runs) { snprintf(t, sizeof t, "%u,", o); tables += t; }
       tables += "0,0,0,0};\n";
