@@ -243,7 +243,7 @@ void replace_all(std::string &s, const std::string &key, const std::string &val)
 // offsets (appended to *runs, emitted by the caller as the __device__ const array `l_off`) instead of 4 instructions
 // per entry: the long backward groups are a quarter of the straight-line code, which is what bounds the kernel.
 constexpr int kLineRun = 10;
-constexpr size_t kMaxConstMul = 6000;      // doubles in the constant bank (48 of its 64 KB)
+constexpr size_t kMaxConstMul = 1024;      // doubles in the constant bank: 8 KB, what its cache holds (6000 cost 11 % at level 24)
 static int line_run() { const char *e = getenv("MTP_TREE_RUN"); const int v = e ? atoi(e) : 0; return v >= 3 ? v : kLineRun; }
 std::string gen_pass(const std::vector<TreeTerm> &prog, const std::vector<int32_t> &wave, int R, bool bwd,
                      const std::vector<double> &leaf_seed, int A, const std::vector<double> *adj_init = nullptr,
@@ -552,11 +552,21 @@ std::vector<char> tree_jit_compile(const TreeSched &sc, int AL, int AR, std::str
   if (table_bytes == 0 || table_bytes > 60 * 1024) {      // larger tables: not measured, keep the straight-line form
     tables.clear();
     std::vector<unsigned> runs;                           // MTP_TREE_FORM=line: no run loops either (A/B measurements)
-    std::vector<unsigned> *rp = (form && form[0] == 'l') ? nullptr : &runs;
+    // run loops for whole tables only: in the group programs of a partitioned table (level 24) they cost more in
+    // serial latency than they save in fetch (tree 58.8 -> 61.2 ms even when limited to programs with few runs)
+    std::vector<unsigned> *rp = ((form && form[0] == 'l') || (!sc.mload_k.empty() && !getenv("MTP_TREE_RUN"))) ? nullptr : &runs;
     std::vector<double> cmul;
     std::vector<double> *cp = (form && form[0] == 'l') ? nullptr : &cmul;
     fwd = gen_pass(sc.fprog, sc.fwave, R, false, sc.leaf_seed, AL * AR, nullptr, rp, cp);
     bwd = gen_pass(sc.bprog, sc.bwave, R, true, sc.leaf_seed, AL * AR, sc.mload_k.empty() ? &sc.adj_init : nullptr, rp, cp);
+    // A loop iteration is a serial chain (table load -> address -> shared loads -> FMA): where most of a program
+    // sits in long runs (the group programs of level 24: tree 58.8 -> 64.8 ms with loops) the loops themselves
+    // become the critical path, so they are used only while the runs are a minority of the entries
+    if (rp && !getenv("MTP_TREE_RUN") && (double)runs.size() / 2 > 0.4 * 3.0 * (double)sc.n_prod) {
+      runs.clear(); cmul.clear();
+      fwd = gen_pass(sc.fprog, sc.fwave, R, false, sc.leaf_seed, AL * AR, nullptr, nullptr, cp);
+      bwd = gen_pass(sc.bprog, sc.bwave, R, true, sc.leaf_seed, AL * AR, sc.mload_k.empty() ? &sc.adj_init : nullptr, nullptr, cp);
+    }
     if (!cmul.empty()) {
       tables += "__constant__ double cm[] = {";
       char t[40];
