@@ -79,10 +79,11 @@ typedef struct {
 int mtp_enumerate(int32_t lev_max, mtp_params *out);
 void mtp_table_free(mtp_params *table);
 
-/* Create / destroy.  Validates the table, compiles it into the kernels' schedules (large tables are first cut
- * into a top program and group programs that fit shared memory; short programs are additionally specialised
- * with NVRTC when libnvrtc is present -- seconds of one-time work) and copies c, xi0, xi and the schedules to
- * the current CUDA device. */
+/* Create / destroy.  Validates the table (MTP_EINVAL for indices out of range, a node read before its last write,
+ * negative multiplicities), turns it into register programs for the contraction kernels (tables whose working set
+ * exceeds an SM's registers + shared memory are first cut into a top program and group programs) and compiles them
+ * with NVRTC -- seconds of one-time work --, and copies c, xi0, xi to the current CUDA device.  Without libnvrtc
+ * the generic table interpreter is set up instead and mtp_last_error(handle) says why. */
 int mtp_create(mtp_handle **out, const mtp_params *p);
 void mtp_destroy(mtp_handle *h);
 const char *mtp_last_error(const mtp_handle *h); /* h may be NULL: last create error     */
@@ -92,16 +93,18 @@ const char *mtp_last_error(const mtp_handle *h); /* h may be NULL: last create e
 #define MTP_OPT_FORCE_MODE 2    /* MTP_FORCE_GATHER (needs d_rev) | MTP_FORCE_ATOMIC       */
 #define MTP_OPT_VARIANT 3       /* MTP_VARIANT_AUTO | _THREAD | _BLOCK                     */
 #define MTP_OPT_PROFILE 4       /* 1: record CUDA events around every kernel launch        */
-#define MTP_OPT_TREE_CODEGEN 5  /* 1 (default): specialise the contraction kernel for the table with NVRTC at
-                                   first use when the table is short enough; 0: always interpret the table.
-                                   Same arithmetic order either way (bit-identical results).
-                                   Environment, read when a table is specialised: MTP_TREE_CODEGEN=0 (as option 0),
-                                   MTP_TREE_FORM=shared (one code body per row shape + operand tables instead of
-                                   straight-line code; bit-identical, currently slower: DESIGN.md section 11),
-                                   MTP_TREE_FORM=line (no run loops: every entry as straight-line code),
-                                   MTP_TREE_RUN=<n> (shortest run of plain entries emitted as a loop, default 10),
-                                   MTP_TREE_DUMP=<path> (write the generated CUDA source there).         */
-#define MTP_INFO_TREE_KERNELS 100 /* mtp_get_option only: number of NVRTC-specialised contraction kernels in use */
+#define MTP_OPT_TREE_CODEGEN 5  /* 1 (default): run the contraction kernels specialised for the table (one register
+                                   program per table, generated and compiled with NVRTC at mtp_create);
+                                   0: interpret the table with the generic kernel (also what runs when libnvrtc is
+                                   absent -- mtp_last_error then says so after mtp_create).  Setting 1 fails with
+                                   MTP_EUNSUP when the specialised kernels could not be built.  The two forms sum
+                                   in different orders: results agree to rounding, not bit for bit.          */
+#define MTP_INFO_TREE_KERNELS 100  /* mtp_get_option only: NVRTC-specialised contraction kernels loaded (0: interpreter) */
+#define MTP_INFO_TREE_PROGRAMS 101 /* mtp_get_option only: tables they were built from (1: whole table; else the top
+                                      program + the group programs of the partition); kernels = 2 x programs        */
+#define MTP_INFO_INPUT_ERRORS 102  /* mtp_get_option only, SYNCHRONISES the device: neighbour-list entries rejected
+                                      since the last read (image shift outside {-1,0,1}^3 or index outside [0,N));
+                                      such pairs are dropped, so a non-zero count means the results are not valid   */
 #define MTP_FORCE_GATHER 0      /* deterministic; keeps d_ij for all pairs (nnz x 32 B)  */
 #define MTP_FORCE_ATOMIC 1      /* fp64 atomic scatter; no per-pair scratch              */
 #define MTP_FORCE_AUTO 2        /* default: gather when d_rev is given, else atomic      */
@@ -121,7 +124,8 @@ int mtp_workspace_bytes(const mtp_handle *h, int64_t n_atoms, int64_t nnz, int w
  *   d_pos   [N][3] f64      d_type [N] i32 in [0,S)
  *   box     [9] HOST, rows = lattice vectors
  *   d_off   [N+1] i64       d_idx [nnz] i32  (entries with r >= R_cut contribute nothing)
- *   d_shift [nnz][3] i8 image shifts, or NULL = minimum image (needs heights > 2 R_cut)
+ *   d_shift [nnz][3] i8 image shifts, each component in {-1,0,1} (the kernels pack index and image into one word;
+ *           other values are rejected, see MTP_INFO_INPUT_ERRORS), or NULL = minimum image (needs heights > 2 R_cut)
  *   d_rev   [nnz] i32 position of the reverse pair, required in MTP_FORCE_GATHER mode
  *   d_E [1], d_Ei [N] or NULL, d_F [N][3], d_virial [6] = xx,yy,zz,xy,xz,yz (eV) or NULL
  *   d_ws / ws_bytes: scratch of at least mtp_workspace_bytes(...). */
@@ -155,7 +159,8 @@ int mtp_compute_host(mtp_handle *h, int64_t n_atoms, const double *pos, const in
 
 /* Diagnostics (parity bring-up and roofline denominators; not part of the hot path). */
 /* Runs K1 + K2 as one chunk and exports the moments M and adjoints G = dE_i/dM, both laid
- * out [n_basic][n_atoms] (component-major), and optionally B [n_atoms][n_basis]. */
+ * out [n_basic][n_atoms] (component-major), and optionally B [n_atoms][n_basis].  Workspace: the size
+ * mtp_workspace_bytes reports with want_grade = 1 and chunk_atoms >= n_atoms. */
 int mtp_debug_moments(mtp_handle *h, int64_t n_atoms, const double *d_pos,
                       const int32_t *d_type, const double *box, const int64_t *d_off,
                       const int32_t *d_idx, const int8_t *d_shift, double *d_M, double *d_G,
@@ -164,16 +169,23 @@ int mtp_debug_moments(mtp_handle *h, int64_t n_atoms, const double *d_pos,
  * count per kernel class since the last read; classes: 0 moments (K1), 1 tree (K2),
  * 2 pair gradient (K3), 3 force gather, 4 grade (K5).  Synchronises on the recorded events. */
 int mtp_profile_read(mtp_handle *h, double *ms /*[5]*/, int64_t *launches /*[5]*/);
-/* Host-only (no device needed): how mtp_create will evaluate the contraction table of *p (only the table
- * fields are read).  out[8] = { partitioned (0/1), atoms per CTA of the whole table, cut rows, groups, ops of the
- * top program, ops summed over the group programs, ops below the cut, smallest atoms per CTA over the groups }. */
+/* Host-only (no device needed): how mtp_create will evaluate the contraction table of *p with the specialised
+ * kernels (only the table fields are read).  out[8] = { partitioned (0/1), threads (= atoms) per SM of the slowest
+ * program, cut rows, groups, ops of the top program, ops summed over the group programs, ops below the cut, same as
+ * out[1] }. */
 int mtp_table_plan(const mtp_params *p, int64_t *out);
+/* Host-only: the register program of the whole table (kind 0: energy + adjoint, 1: basis values) as data, so that a
+ * test can emulate it: prog[cap][7] int32 = op, d, a, b, c, k, x (csrc/tree_codegen.h K2Op), consts[ccap] doubles,
+ * info[4] = { instructions, constants, registers, shared-memory slots }.  Only the table fields and xi are read. */
+int mtp_k2_program(const mtp_params *p, int kind, int32_t *prog, int64_t cap, double *consts, int64_t ccap,
+                   int64_t *info);
 /* Number of kernels this library has launched since load (bench.py gpu_launches). */
 int64_t mtp_launch_count(void);
 /* fp64 FMA throughput microbenchmark: runs `iters` dependent-chain DFMA batches on every
  * SM and returns the useful flop count; time it with CUDA events on `cuda_stream`. */
 int mtp_peak_dfma(int64_t iters, double *d_sink, double *out_flops, void *cuda_stream);
-/* static facts for reporting: flops per pair / per atom of the compiled schedules */
+/* Algorithmic flops for the roofline report (FMA = 2, each quantity once; formulas in DESIGN.md section 6):
+ * flop_per_pair[2] = { K1 moments, K3 pair derivative }, K2 per atom, K5 per atom. */
 int mtp_cost_model(const mtp_handle *h, double *flop_per_pair, double *flop_per_atom_tree,
                    double *flop_per_atom_grade);
 

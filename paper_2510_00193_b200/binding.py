@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libmtp_b200.so")
 
 OK, EINVAL, ESIZE, EBOX, ECUDA, EUNSUP, ENOMEM = 0, -1, -2, -3, -4, -5, -6
 OPT_CHUNK_ATOMS, OPT_FORCE_MODE, OPT_VARIANT, OPT_PROFILE, OPT_TREE_CODEGEN = 1, 2, 3, 4, 5
-INFO_TREE_KERNELS = 100
+INFO_TREE_KERNELS, INFO_TREE_PROGRAMS, INFO_INPUT_ERRORS = 100, 101, 102
 FORCE_GATHER, FORCE_ATOMIC, FORCE_AUTO = 0, 1, 2
 VARIANT_AUTO, VARIANT_THREAD, VARIANT_BLOCK = 0, 1, 2
 
@@ -37,7 +37,7 @@ class MtpParams(C.Structure):
 EXPORTS = ["mtp_enumerate", "mtp_table_free", "mtp_create", "mtp_destroy", "mtp_last_error",
            "mtp_set_option", "mtp_get_option", "mtp_workspace_bytes", "mtp_compute", "mtp_grade",
            "mtp_compute_host", "mtp_debug_moments", "mtp_launch_count", "mtp_peak_dfma",
-           "mtp_cost_model", "mtp_profile_read", "mtp_table_plan"]
+           "mtp_cost_model", "mtp_profile_read", "mtp_table_plan", "mtp_k2_program"]
 
 
 def _build():
@@ -80,6 +80,7 @@ def _load():
     lib.mtp_cost_model.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl)]
     lib.mtp_profile_read.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
     lib.mtp_table_plan.argtypes = [C.POINTER(MtpParams), C.POINTER(i64)]
+    lib.mtp_k2_program.argtypes = [C.POINTER(MtpParams), C.c_int, vp, i64, vp, i64, C.POINTER(i64)]
     return lib
 
 
@@ -126,8 +127,32 @@ class Table:
         rc = _lib.mtp_table_plan(C.byref(p), out)
         if rc != OK:
             raise MtpError(rc, "mtp_table_plan")
-        keys = ["partitioned", "atoms_per_cta", "cut_rows", "groups", "top_ops", "group_ops", "ops_below_cut", "group_atoms_per_cta"]
+        keys = ["partitioned", "threads_per_sm", "cut_rows", "groups", "top_ops", "group_ops", "ops_below_cut", "_"]
         return dict(zip(keys, [int(x) for x in out]))
+
+    def k2_program(self, xi, kind=0):
+        """mtp_k2_program: the register program of the whole table as data (host-only), for emulation in the tests.
+        Returns dict(prog[n][7] int32, consts[m] f64, n_regs, n_slots)."""
+        basic = np.ascontiguousarray(self.basic, dtype=np.int32)
+        prod = np.ascontiguousarray(self.prod, dtype=np.int32)
+        bn = np.ascontiguousarray(self.basis_node, dtype=np.int32)
+        xi = np.ascontiguousarray(xi, dtype=np.float64)
+        p = MtpParams()
+        p.n_basic, p.basic, p.n_nodes = basic.shape[0], basic.ctypes.data_as(_I32P), int(self.n_nodes)
+        p.n_prod, p.prod = prod.shape[0], prod.ctypes.data_as(_I32P)
+        p.n_basis, p.basis_node = bn.shape[0], bn.ctypes.data_as(_I32P)
+        p.xi = xi.ctypes.data_as(C.POINTER(C.c_double))
+        info = (C.c_int64 * 4)()
+        rc = _lib.mtp_k2_program(C.byref(p), int(kind), None, 0, None, 0, info)
+        if rc != OK:
+            raise MtpError(rc, "mtp_k2_program")
+        prog = np.zeros((int(info[0]), 7), np.int32)
+        consts = np.zeros(max(int(info[1]), 1), np.float64)
+        rc = _lib.mtp_k2_program(C.byref(p), int(kind), C.c_void_p(prog.ctypes.data), prog.shape[0],
+                                 C.c_void_p(consts.ctypes.data), consts.shape[0], info)
+        if rc != OK:
+            raise MtpError(rc, "mtp_k2_program")
+        return dict(prog=prog, consts=consts[:int(info[1])], n_regs=int(info[2]), n_slots=int(info[3]))
 
     def describe(self, alpha: int):
         return list(self.basis_desc[self.basis_desc_off[alpha]:self.basis_desc_off[alpha + 1]])
@@ -204,9 +229,13 @@ class Potential:
         return int(out.value)
 
     def cost_model(self):
-        a, b, c = C.c_double(), C.c_double(), C.c_double()
-        self._check(_lib.mtp_cost_model(self._h, C.byref(a), C.byref(b), C.byref(c)))
-        return dict(flop_per_pair=a.value, flop_per_atom_tree=b.value, flop_per_atom_grade=c.value)
+        """mtp_cost_model: algorithmic flops per pair (K1, K3) and per atom (K2, K5)."""
+        a, b, c = (C.c_double * 2)(), C.c_double(), C.c_double()
+        self._check(_lib.mtp_cost_model(self._h, a, C.byref(b), C.byref(c)))
+        return dict(flop_per_pair_k1=a[0], flop_per_pair_k3=a[1], flop_per_atom_tree=b.value, flop_per_atom_grade=c.value)
+
+    def last_error(self):
+        return _lib.mtp_last_error(self._h).decode()
 
     def profile_read(self):
         """dict class -> (ms, launches) since the last read (needs OPT_PROFILE = 1)."""
@@ -269,7 +298,7 @@ class Potential:
         B = torch.empty((n, self.n_basis), dtype=torch.float64, device=dev)
         saved = self.get_option(OPT_CHUNK_ATOMS)
         self.set_option(OPT_CHUNK_ATOMS, max(n, 1))
-        ws = self._workspace(self.workspace_bytes(n, 0), dev)
+        ws = self._workspace(self.workspace_bytes(n, 0, True), dev)
         self.set_option(OPT_CHUNK_ATOMS, saved)
         boxh = (C.c_double * 9)(*[float(x) for x in np.asarray(box, dtype=np.float64).reshape(9)])
         self._check(_lib.mtp_debug_moments(self._h, n, _ptr(pos), _ptr(types), boxh, _ptr(off), _ptr(idx),

@@ -43,6 +43,7 @@ struct mtp_handle {
   int crow = 0;
   double *d_coef = nullptr, *d_xi = nullptr, *d_xi0 = nullptr;
   int *d_kmapF = nullptr, *d_kmapB = nullptr, *d_basis_node = nullptr;
+  int *d_flag = nullptr;                       // device counter of rejected input pairs (MTP_INFO_INPUT_ERRORS)
   // K2 schedules, one per atom-lane count AL (compiled on first use; the large-N one at create)
   struct TreeDev {
     TreeSched sched;
@@ -51,8 +52,6 @@ struct mtp_handle {
     int *d_eseed_slot = nullptr, *d_basis_slot = nullptr;
     double *d_adj_init = nullptr, *d_gseed_val = nullptr, *d_leaf_seed = nullptr, *d_eseed_val = nullptr;
     int *d_mload_k = nullptr, *d_cut_row = nullptr, *d_cut_vslot = nullptr, *d_cut_aslot = nullptr;
-    TreeJit *jit = nullptr;                    // specialised kernel (tree_jit.cpp), null = interpreter
-    std::string jit_note;
   };
   // A table the K2 kernels can run: the whole table, or -- when that leaves too few atoms per CTA -- the top
   // program and the group programs of its partition (tree_partition.cpp).  Host copies feed the compilations.
@@ -63,13 +62,27 @@ struct mtp_handle {
     std::vector<int32_t> basic_map, cut_local, cut_row;   // group programs only
     int slots[2][2] = {{0, 0}, {0, 0}};        // [elide][n_val, n_adj]
     std::map<int, TreeDev> trees;              // key: AL * 8 + AR * 2 + elide
-    std::map<int, std::vector<char>> cubin;    // same key: kernels compiled ahead in parallel at create
     int n_prod() const { return (int)(prod.size() / 4); }
     bool is_group() const { return !cut_local.empty(); }
   };
   int codegen = 1;                             // MTP_OPT_TREE_CODEGEN
+  // ---- K2, interpreter form (tree_kernel.cu): built on first use, i.e. only when the specialised kernels are
+  // switched off or unavailable
+  bool interp_ready = false;
   std::vector<Prog> progs;                     // [0] whole table; partitioned: [1] top, [2..] groups
   bool partitioned = false;
+  // ---- K2, specialised form (tree_codegen.cpp + tree_jit.cpp): one register program per table, compiled at create
+  struct JProg {
+    K2Table table;
+    K2Gen gen[2];                              // [K2_EF], [K2_VALUES]
+    K2Kernel *kern[2] = {nullptr, nullptr};
+  };
+  std::vector<JProg> jprogs;                   // [0] whole table or top program; [1..] group programs
+  bool jit_ready = false, jit_partitioned = false;
+  std::string jit_note;                        // why the specialised kernels are not in use
+  int n_jit_kernels = 0;
+  // the table as given (host copy) and what both forms share of a partition
+  K2Table whole;
   int n_cut_rows = 0;                          // rows of the cut-value arrays S / dE/dS
   int *d_gmap = nullptr;                       // [n_basic] cut row of a packed moment that is a cut node itself, else -1
   long long n_prod = 0;
@@ -172,8 +185,8 @@ static void build_kmaps(const PairLevel &pl, int n_basic, const int32_t *basic, 
   }
 }
 
-// K2 schedule of one program for a CTA shape (AL, AR) and leaf elision on/off: compiled from the host copy
-// of its table and uploaded on first use
+// K2 interpreter schedule of one program for a CTA shape (AL, AR) and leaf elision on/off: compiled from the host
+// copy of its table and uploaded on first use
 static int get_tree(mtp_handle *h, mtp_handle::Prog &pg, int AL, int AR, bool elide, const mtp_handle::TreeDev **out) {
   if (AL <= 0) return fail(h, MTP_EUNSUP, "contraction tree does not fit in shared memory");
   const int key = AL * 8 + AR * 2 + (elide ? 1 : 0);
@@ -182,25 +195,10 @@ static int get_tree(mtp_handle *h, mtp_handle::Prog &pg, int AL, int AR, bool el
   mtp_handle::TreeDev td;
   const char *terr = "";
   const bool group = pg.is_group();
-  auto compile = [&](int R) {
-    return tree_compile(pg.n_basic, pg.n_nodes, pg.n_prod(), pg.prod.data(), pg.n_basis, pg.basis_node.data(), pg.xi.data(),
-                        AL * AR, R, elide, td.sched, &terr, group ? pg.basic_map.data() : nullptr,
+  int rc = tree_compile(pg.n_basic, pg.n_nodes, pg.n_prod(), pg.prod.data(), pg.n_basis, pg.basis_node.data(), pg.xi.data(),
+                        AL * AR, tree_row_lanes(AL), elide, td.sched, &terr, group ? pg.basic_map.data() : nullptr,
                         group ? pg.cut_local.data() : nullptr, (int)pg.cut_local.size());
-  };
-  int rc = compile(tree_row_lanes(AL));
   if (rc != MTP_OK) return fail(h, rc, terr);
-  // The kernel specialised for this table (tree_jit.cpp) runs the same schedule as the interpreter (so the two
-  // are bit-identical); built when the table is short enough to be worth compiling and the shape has 32
-  // atom-lanes.  (Measured with 4 / 8 / 16 / 32 row-lane warps: 3.81 / 2.96 / 2.99 / 3.32 ms at config 4 --
-  // the generated code is bound by instruction-fetch bandwidth, i.e. by its size, not by per-warp latency.)
-  const char *env = getenv("MTP_TREE_CODEGEN");
-  if (h->codegen && !(env && env[0] == '0') && AL == 32 && 3LL * pg.n_prod() <= 60000 &&
-      tree_jit_smem_bytes(td.sched.n_val, td.sched.n_adj, AR, tree_threads(AL)) <= 225 * 1024)
-  {
-    auto pre = pg.cubin.find(key);
-    if (pre != pg.cubin.end()) { td.jit = tree_jit_load(pre->second, AR, td.sched.R * AL, &td.jit_note); pg.cubin.erase(pre); }
-    else td.jit = tree_jit_build(td.sched, AL, AR, &td.jit_note);
-  }
   cudaError_t e = cudaSuccess;
   auto up = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
   const TreeSched &sc = td.sched;
@@ -249,7 +247,7 @@ extern "C" void mtp_destroy(mtp_handle *h) {
   if (!h) return;
   for (auto &s : h->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
   for (auto e : h->pool) cudaEventDestroy(e);
-  for (auto &pg : h->progs) for (auto &kv : pg.trees) tree_jit_destroy(kv.second.jit);
+  for (auto &jp : h->jprogs) for (auto *k : jp.kern) k2_jit_destroy(k);
   for (void *p : h->to_free) cudaFree(p);
   if (h->stage) cudaFree(h->stage);
   for (auto e : h->ev) cudaEventDestroy(e);
@@ -258,43 +256,243 @@ extern "C" void mtp_destroy(mtp_handle *h) {
   delete h;
 }
 
-// The partition mtp_create uses for a table whose monolithic evaluation gets fewer than 32 atoms per CTA:
-// budgets = shared-memory slots per atom that leave room for 64 (else 32) atoms per CTA beside the energy partials.
-static bool decide_partition(const mtp_params *p, TreePartition &part) {
-  const char *penv = getenv("MTP_TREE_PARTITION");
-  if (penv && penv[0] == '0') return false;
-  bool ok = tree_partition(p->n_basic, p->n_nodes, p->n_prod, p->prod, p->n_basis, p->basis_node, 430, part);
+// ---- K2 set-up ------------------------------------------------------------------------------
+// Interpreter form: a table whose monolithic evaluation gets fewer than 32 atoms per CTA is cut into a top program
+// and group programs (tree_partition.cpp); budgets = shared-memory slots per atom that leave room for 64 (else 32)
+// atoms per CTA beside the energy partials.
+static bool interp_partition(const K2Table &t, TreePartition &part) {
+  const int nb = (int)t.basis_node.size();
+  bool ok = tree_partition(t.n_basic, t.n_nodes, t.n_prod(), t.prod.data(), nb, t.basis_node.data(), 430, part);
   if (!ok || part.groups.size() > 24)
-    ok = tree_partition(p->n_basic, p->n_nodes, p->n_prod, p->prod, p->n_basis, p->basis_node, 870, part);
+    ok = tree_partition(t.n_basic, t.n_nodes, t.n_prod(), t.prod.data(), nb, t.basis_node.data(), 870, part);
   return ok;
 }
 
-// Host-only diagnostic (no device needed): how mtp_create would evaluate this table.
-extern "C" int mtp_table_plan(const mtp_params *p, int64_t *out) {
-  if (!p || !out || p->n_basic < 1 || p->n_nodes < p->n_basic || p->n_prod < 0 || (p->n_prod && !p->prod) || !p->basis_node)
-    return MTP_EINVAL;
-  for (int q = 0; q < 8; ++q) out[q] = 0;
-  int nv = 0, na = 0, AL = 0, AR = 1;
-  tree_count_slots(p->n_basic, p->n_nodes, p->n_prod, p->prod, true, &nv, &na);
-  tree_pick_shape(nv, na, 0, &AL, &AR);
-  out[1] = (int64_t)AL * AR;
-  if (AL >= 32) return MTP_OK;
+static void prog_slots(mtp_handle::Prog &g) {
+  for (int el = 0; el < 2; ++el)
+    tree_count_slots(g.n_basic, g.n_nodes, g.n_prod(), g.prod.data(), el != 0, &g.slots[el][0], &g.slots[el][1],
+                     g.cut_local.data(), (int)g.cut_local.size());
+}
+
+static int upload_gmap(mtp_handle *h, const TreePartition &part) {
+  if (h->d_gmap) return MTP_OK;
+  std::vector<int> gmap(h->n_basic, -1);
+  for (size_t q = 0; q < part.cut_basic_k.size(); ++q) gmap[part.cut_basic_k[q]] = part.cut_basic_row[q];
+  if (upload(h, &h->d_gmap, gmap.data(), gmap.size()) != cudaSuccess) return fail(h, MTP_ECUDA, "cut map upload");
+  return MTP_OK;
+}
+
+static int ensure_interp(mtp_handle *h) {
+  if (h->interp_ready) return MTP_OK;
+  const K2Table &t = h->whole;
+  h->progs.clear();
+  h->progs.emplace_back();
+  {
+    mtp_handle::Prog &whole = h->progs.back();
+    whole.n_basic = t.n_basic; whole.n_nodes = t.n_nodes; whole.n_basis = h->n_basis;
+    whole.prod = t.prod; whole.basis_node = t.basis_node; whole.xi = t.xi;
+    prog_slots(whole);
+  }
+  int AL = 0, AR = 1;
+  tree_pick_shape(h->progs[0].slots[1][0], h->progs[0].slots[1][1], 0, &AL, &AR);
   TreePartition part;
-  if (!decide_partition(p, part)) return MTP_OK;
-  out[0] = 1; out[2] = (int64_t)part.cut_node.size(); out[3] = (int64_t)part.groups.size(); out[4] = part.top.n_prod();
-  std::vector<char> seen(part.cut_node.size(), 0);
-  int64_t min_atoms = 1 << 30;
-  for (auto &g : part.groups) {
+  if (AL < 32 && interp_partition(t, part)) {
+    h->partitioned = true;
+    h->n_cut_rows = (int)part.cut_node.size();
+    h->progs.emplace_back();
+    {
+      mtp_handle::Prog &top = h->progs.back();
+      top.n_basic = part.top.n_basic; top.n_nodes = part.top.n_nodes; top.n_basis = h->n_basis;
+      top.prod = part.top.prod; top.basis_node = part.top.basis_node; top.xi = t.xi;
+      prog_slots(top);
+    }
+    for (auto &g : part.groups) {
+      h->progs.emplace_back();
+      mtp_handle::Prog &pg = h->progs.back();
+      pg.n_basic = g.table.n_basic; pg.n_nodes = g.table.n_nodes; pg.n_basis = 0;
+      pg.prod = g.table.prod; pg.basic_map = g.basic_map; pg.cut_local = g.cut_local; pg.cut_row = g.cut_row;
+      prog_slots(pg);
+    }
+    int rc = upload_gmap(h, part);
+    if (rc != MTP_OK) return rc;
+  }
+  for (size_t q = h->partitioned ? 1 : 0; q < h->progs.size(); ++q)
+    for (int el = 0; el < 2; ++el) {
+      tree_pick_shape(h->progs[q].slots[el][0], h->progs[q].slots[el][1], 0, &AL, &AR);
+      if (AL == 0)
+        return fail(h, MTP_EUNSUP, "contraction tree does not fit in shared memory (one atom's node values and adjoints > 225 KB)");
+    }
+  // build the large-system schedules now, so that errors surface here
+  for (size_t q = h->partitioned ? 1 : 0; q < h->progs.size(); ++q) {
+    const mtp_handle::TreeDev *td = nullptr;
+    tree_pick_shape(h->progs[q].slots[1][0], h->progs[q].slots[1][1], 0, &AL, &AR);
+    int rc = get_tree(h, h->progs[q], AL, AR, true, &td);
+    if (rc != MTP_OK) return rc;
+  }
+  h->interp_ready = true;
+  return MTP_OK;
+}
+
+// Specialised form.  A table whose register program needs more private shared memory than one 128-thread CTA per SM
+// can have (kK2SlotsMax slots per thread) is cut below its product layer like for the interpreter; the group budget
+// is chosen among a few by the estimated cost: arithmetic instructions of all programs, weighted by how few threads
+// per SM their slot counts allow.
+namespace {
+struct JitPlan {
+  bool partitioned = false;
+  TreePartition part;
+  std::vector<K2Table> tables;          // [0] whole or top, then groups
+  double cost = 0.0;
+  int min_threads = 0;                  // smallest threads-per-SM over the programs
+};
+double slots_penalty(int n_slots) {
+  int threads = 0, ctas = 0;
+  k2_shape(n_slots, &threads, &ctas);
+  if (threads == 0) return 1e9;
+  const int per_sm = threads * ctas;
+  return per_sm >= 256 ? 1.0 : (per_sm >= 128 ? 1.5 : (per_sm >= 64 ? 3.0 : 6.0));
+}
+int threads_per_sm(int n_slots) { int t = 0, c = 0; k2_shape(n_slots, &t, &c); return t * c; }
+
+K2Table group_table(const TreeGroup &g) {
+  K2Table kt;
+  kt.n_basic = g.table.n_basic; kt.n_nodes = g.table.n_nodes; kt.prod = g.table.prod; kt.in_row = g.basic_map;
+  kt.cut_node = g.cut_local; kt.cut_row = g.cut_row;
+  return kt;
+}
+
+// 0 or a negative code; err receives a message
+int plan_jit(const K2Table &whole, JitPlan &best, std::string *err) {
+  K2Gen g;
+  int rc = k2_generate(whole, K2_EF, kK2Window, kK2Lookahead, g, err);
+  if (rc != MTP_OK) return rc;
+  best = JitPlan();
+  if (g.n_slots <= kK2SlotsMax) {
+    best.tables.push_back(whole);
+    best.cost = (double)g.n_arith * slots_penalty(g.n_slots);
+    best.min_threads = threads_per_sm(g.n_slots);
+    return MTP_OK;
+  }
+  bool have = false;
+  static const int budgets[] = {430, 600, 870, 1300, 2000};
+  for (int budget : budgets) {
+    JitPlan p;
+    if (!tree_partition(whole.n_basic, whole.n_nodes, whole.n_prod(), whole.prod.data(), (int)whole.basis_node.size(),
+                        whole.basis_node.data(), budget, p.part)) continue;
+    p.partitioned = true;
+    K2Table top;
+    top.n_basic = p.part.top.n_basic; top.n_nodes = p.part.top.n_nodes; top.prod = p.part.top.prod;
+    top.basis_node = p.part.top.basis_node; top.xi = whole.xi;
+    p.tables.push_back(std::move(top));
+    for (auto &gr : p.part.groups) p.tables.push_back(group_table(gr));
+    bool ok = true;
+    p.min_threads = 1 << 30;
+    for (size_t q = 0; q < p.tables.size() && ok; ++q) {
+      const int kinds = q == 0 ? 1 : 2;                 // groups run K2_VALUES and K2_EF in every evaluation
+      for (int k = 0; k < kinds && ok; ++k) {
+        K2Gen gq;
+        std::string e2;
+        if (k2_generate(p.tables[q], (K2Kind)k, kK2Window, kK2Lookahead, gq, &e2) != MTP_OK) { ok = false; break; }
+        const double pen = slots_penalty(gq.n_slots);
+        if (pen >= 1e9) { ok = false; break; }
+        p.cost += (double)gq.n_arith * pen;
+        p.min_threads = std::min(p.min_threads, threads_per_sm(gq.n_slots));
+      }
+    }
+    if (!ok) continue;
+    if (!have || p.cost < best.cost) { best = std::move(p); have = true; }
+  }
+  if (!have) { *err = "contraction table: no partition fits the specialised kernels"; return MTP_EUNSUP; }
+  long long ops = 0;
+  for (auto &t : best.tables) ops += t.n_prod();
+  if (ops > kK2MaxOps) {                 // level 28: 350 000 ops in 130 programs -- minutes of NVRTC time
+    *err = "contraction table too large to specialise (" + std::to_string(ops) + " ops after partitioning): interpreted";
+    return MTP_EUNSUP;
+  }
+  return MTP_OK;
+}
+}  // namespace
+
+// Generates, compiles (in parallel: NVRTC takes about a second per thousand table ops) and loads the specialised kernels.
+// On failure the handle stays usable through the interpreter; jit_note says why.
+static int ensure_jit(mtp_handle *h) {
+  if (h->jit_ready) return MTP_OK;
+  std::string why;
+  if (!k2_jit_available(&why)) { h->jit_note = why; return MTP_EUNSUP; }
+  JitPlan plan;
+  int rc = plan_jit(h->whole, plan, &why);
+  if (rc != MTP_OK) { h->jit_note = why; return rc; }
+  h->jprogs.clear();
+  h->jprogs.resize(plan.tables.size());
+  for (size_t q = 0; q < plan.tables.size(); ++q) h->jprogs[q].table = std::move(plan.tables[q]);
+  h->jit_partitioned = plan.partitioned;
+  if (plan.partitioned) {
+    h->n_cut_rows = (int)plan.part.cut_node.size();
+    rc = upload_gmap(h, plan.part);
+    if (rc != MTP_OK) { h->jit_note = h->err; return rc; }
+  }
+  struct Job { mtp_handle::JProg *jp; int kind; std::vector<char> cubin; std::string why; int rc = 0; };
+  std::vector<Job> jobs;
+  for (auto &jp : h->jprogs)
+    for (int k = 0; k < 2; ++k) jobs.push_back(Job{&jp, k, {}, "", 0});
+  std::atomic<size_t> next{0};
+  auto work = [&]() {
+    for (size_t i = next.fetch_add(1); i < jobs.size(); i = next.fetch_add(1)) {
+      Job &j = jobs[i];
+      j.rc = k2_generate(j.jp->table, (K2Kind)j.kind, kK2Window, kK2Lookahead, j.jp->gen[j.kind], &j.why);
+      if (j.rc != MTP_OK) continue;
+      j.cubin = k2_jit_compile(j.jp->gen[j.kind], &j.why);
+      if (j.cubin.empty()) j.rc = MTP_ECUDA;
+      j.jp->gen[j.kind].body.clear(); j.jp->gen[j.kind].body.shrink_to_fit();      // the source is not needed any more
+    }
+  };
+  std::vector<std::thread> workers;
+  const unsigned hw = std::max(1u, std::thread::hardware_concurrency());
+  for (unsigned t = 0; t < std::min<unsigned>(std::min(hw, 32u), (unsigned)jobs.size()); ++t) workers.emplace_back(work);
+  for (auto &w : workers) w.join();
+  for (auto &j : jobs) {
+    if (j.rc == MTP_OK) {
+      j.jp->kern[j.kind] = k2_jit_load(j.cubin, j.jp->gen[j.kind].n_slots, &j.why);
+      if (!j.jp->kern[j.kind]) j.rc = MTP_ECUDA;
+    }
+    if (j.rc != MTP_OK) {
+      h->jit_note = j.why;
+      for (auto &jp : h->jprogs) for (auto *&k : jp.kern) { k2_jit_destroy(k); k = nullptr; }
+      h->jprogs.clear();
+      return j.rc;
+    }
+  }
+  h->n_jit_kernels = (int)jobs.size();
+  h->jit_ready = true;
+  return MTP_OK;
+}
+
+// Host-only diagnostic (no device needed): how mtp_create would evaluate this table with the specialised kernels.
+extern "C" int mtp_table_plan(const mtp_params *p, int64_t *out) {
+  if (!p || !out) return MTP_EINVAL;
+  const char *verr = "";
+  if (k2_validate(p->n_basic, p->n_nodes, p->n_prod, p->prod, p->n_basis, p->basis_node, &verr) != MTP_OK) return MTP_EINVAL;
+  for (int q = 0; q < 8; ++q) out[q] = 0;
+  K2Table whole;
+  whole.n_basic = p->n_basic; whole.n_nodes = p->n_nodes; whole.prod.assign(p->prod, p->prod + 4 * (size_t)p->n_prod);
+  whole.basis_node.assign(p->basis_node, p->basis_node + p->n_basis);
+  whole.xi.assign((size_t)p->n_basis, 1.0);            // the plan does not depend on the weights (all taken non-zero)
+  JitPlan plan;
+  std::string err;
+  int rc = plan_jit(whole, plan, &err);
+  if (rc != MTP_OK) return rc;
+  out[0] = plan.partitioned ? 1 : 0;
+  out[1] = plan.min_threads;
+  if (!plan.partitioned) return MTP_OK;
+  out[2] = (int64_t)plan.part.cut_node.size(); out[3] = (int64_t)plan.part.groups.size(); out[4] = plan.part.top.n_prod();
+  std::vector<char> seen(plan.part.cut_node.size(), 0);
+  for (auto &g : plan.part.groups) {
     out[5] += g.table.n_prod();
     for (int r : g.cut_row) { if (r < 0 || r >= (int)seen.size() || seen[r]) return MTP_EINVAL; seen[r] = 1; }
-    tree_count_slots(g.table.n_basic, g.table.n_nodes, g.table.n_prod(), g.table.prod.data(), true, &nv, &na, g.cut_local.data(),
-                     (int)g.cut_local.size());
-    tree_pick_shape(nv, na, 0, &AL, &AR);
-    min_atoms = std::min<int64_t>(min_atoms, (int64_t)AL * AR);
   }
-  for (size_t r = 0; r < seen.size(); ++r) if (!seen[r] && part.cut_node[r] >= p->n_basic) return MTP_EINVAL;
-  out[6] = (int64_t)p->n_prod - part.top.n_prod();
-  out[7] = min_atoms;
+  for (size_t r = 0; r < seen.size(); ++r) if (!seen[r] && plan.part.cut_node[r] >= p->n_basic) return MTP_EINVAL;
+  out[6] = (int64_t)p->n_prod - plan.part.top.n_prod();
+  out[7] = plan.min_threads;
   return MTP_OK;
 }
 
@@ -306,6 +504,11 @@ extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
       p->n_nodes < p->n_basic || p->n_prod < 0 || p->n_basis < 1 || !p->basic || (p->n_prod && !p->prod) ||
       !p->basis_node || !p->c || !p->xi0 || !p->xi)
     return fail(nullptr, MTP_EINVAL, "mtp_params: bad sizes or null arrays");
+  {                                   // the table is validated before anything walks it
+    const char *verr = "";
+    int rc = k2_validate(p->n_basic, p->n_nodes, p->n_prod, p->prod, p->n_basis, p->basis_node, &verr);
+    if (rc != MTP_OK) return fail(nullptr, rc, verr);
+  }
   int dev_count = 0;
   if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0)
     return fail(nullptr, MTP_ECUDA, "no CUDA device: this library has no CPU fallback");
@@ -326,62 +529,19 @@ extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
   h->n_nodes = p->n_nodes; h->n_basis = p->n_basis; h->lev_max = p->lev_max; h->r_min = p->r_min; h->r_cut = p->r_cut;
   h->pl = pair_level(li);
   h->n_prod = p->n_prod;
-  {
-    auto slots_of = [](mtp_handle::Prog &g) {
-      for (int el = 0; el < 2; ++el)
-        tree_count_slots(g.n_basic, g.n_nodes, g.n_prod(), g.prod.data(), el != 0, &g.slots[el][0], &g.slots[el][1],
-                         g.cut_local.data(), (int)g.cut_local.size());
-    };
-    h->progs.emplace_back();
-    mtp_handle::Prog &whole = h->progs.back();
-    whole.n_basic = p->n_basic; whole.n_nodes = p->n_nodes; whole.n_basis = p->n_basis;
-    whole.prod.assign(p->prod, p->prod + 4 * (size_t)p->n_prod);
-    whole.basis_node.assign(p->basis_node, p->basis_node + p->n_basis);
-    whole.xi.assign(p->xi, p->xi + p->n_basis);
-    slots_of(whole);
-    int AL = 0, AR = 1;
-    tree_pick_shape(whole.slots[1][0], whole.slots[1][1], 0, &AL, &AR);
-    // Too few atoms per CTA (lev_max >= 20): cut the table into a top program and group programs that each fit
-    // 64 (else 32) atoms per CTA.  Budgets = shared-memory slots per atom left beside the energy partials.
-    {
-      TreePartition part;
-      const bool ok = AL < 32 && decide_partition(p, part);
-      if (ok) {
-        h->partitioned = true;
-        h->n_cut_rows = (int)part.cut_node.size();
-        h->progs.emplace_back();
-        {
-          mtp_handle::Prog &top = h->progs.back();
-          top.n_basic = part.top.n_basic; top.n_nodes = part.top.n_nodes; top.n_basis = p->n_basis;
-          top.prod = part.top.prod; top.basis_node = part.top.basis_node;
-          top.xi.assign(p->xi, p->xi + p->n_basis);
-          slots_of(top);
-        }
-        for (auto &g : part.groups) {
-          h->progs.emplace_back();
-          mtp_handle::Prog &pg = h->progs.back();
-          pg.n_basic = g.table.n_basic; pg.n_nodes = g.table.n_nodes; pg.n_basis = 0;
-          pg.prod = g.table.prod; pg.basic_map = g.basic_map; pg.cut_local = g.cut_local; pg.cut_row = g.cut_row;
-          slots_of(pg);
-        }
-        std::vector<int> gmap(p->n_basic, -1);
-        for (size_t q = 0; q < part.cut_basic_k.size(); ++q) gmap[part.cut_basic_k[q]] = part.cut_basic_row[q];
-        if (upload(h, &h->d_gmap, gmap.data(), gmap.size()) != cudaSuccess) { mtp_destroy(h); return fail(nullptr, MTP_ECUDA, "mtp_create upload"); }
-      }
-    }
-    for (size_t q = h->partitioned ? 1 : 0; q < h->progs.size(); ++q)
-      for (int el = 0; el < 2; ++el) {
-        tree_pick_shape(h->progs[q].slots[el][0], h->progs[q].slots[el][1], 0, &AL, &AR);
-        if (AL == 0) {
-          mtp_destroy(h);
-          return fail(nullptr, MTP_EUNSUP, "contraction tree does not fit in shared memory (one atom's node values and adjoints > 225 KB)");
-        }
-      }
-  }
+  h->whole.n_basic = p->n_basic; h->whole.n_nodes = p->n_nodes;
+  h->whole.prod.assign(p->prod, p->prod + 4 * (size_t)p->n_prod);
+  h->whole.basis_node.assign(p->basis_node, p->basis_node + p->n_basis);
+  h->whole.xi.assign(p->xi, p->xi + p->n_basis);
   // radial coefficients: blocks (z_i, z_j) laid out [beta][NMUP], NMUP = the level's n_mu rounded up to even
   // (16-byte pairs); +2 doubles per block spread the blocks over the banks
   const int nmu_lev = rt_nmu(h->pl->lev), nmup = (nmu_lev + 1) & ~1;
   h->crow = nmup * h->nb + 2;
+  // K1 / K3 stage the coefficients of every species pair in shared memory next to their pair tiles
+  if ((size_t)h->S * h->S * h->crow * 8 + h->pl->smem_fixed > 227 * 1024) {
+    delete h;
+    return fail(nullptr, MTP_EUNSUP, "n_species^2 x n_radial_basis x n_radial_funcs coefficients do not fit in shared memory beside the pair tiles");
+  }
   std::vector<double> coef((size_t)h->S * h->S * h->crow, 0.0);
   for (int r = 0; r < h->S * h->S; ++r)
     for (int m = 0; m < h->nmu && m < nmu_lev; ++m)
@@ -396,50 +556,16 @@ extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
   up(upload(h, &h->d_kmapF, kf.data(), kf.size()));
   up(upload(h, &h->d_kmapB, kb.data(), kb.size()));
   up(upload(h, &h->d_basis_node, p->basis_node, (size_t)p->n_basis));
+  up(upload(h, &h->d_flag, (const int *)nullptr, 0));
+  if (e == cudaSuccess) e = cudaMemset(h->d_flag, 0, sizeof(int));
   if (e != cudaSuccess) { int r = cuda_fail(nullptr, e, "mtp_create upload"); mtp_destroy(h); return r; }
-  // the programs of a partitioned table are specialised in parallel (NVRTC takes seconds per program)
-  {
-    const char *env = getenv("MTP_TREE_CODEGEN");
-    struct Job { mtp_handle::Prog *pg; int AL, AR, key; };
-    std::vector<Job> jobs;
-    for (size_t q = h->partitioned ? 1 : 0; h->partitioned && h->codegen && !(env && env[0] == '0') && q < h->progs.size(); ++q) {
-      mtp_handle::Prog *pg = &h->progs[q];
-      int AL = 0, AR = 1;
-      tree_pick_shape(pg->slots[1][0], pg->slots[1][1], 0, &AL, &AR);
-      if (AL != 32 || 3LL * pg->n_prod() > 60000) continue;
-      const int key = AL * 8 + AR * 2 + 1;
-      pg->cubin[key];                          // created here: the workers only assign to existing entries
-      jobs.push_back(Job{pg, AL, AR, key});
-    }
-    std::atomic<size_t> next{0};
-    auto work = [&]() {
-      for (size_t i = next.fetch_add(1); i < jobs.size(); i = next.fetch_add(1)) {
-        const Job &j = jobs[i];
-        TreeSched sc;
-        const char *terr = "";
-        const bool group = j.pg->is_group();
-        if (tree_compile(j.pg->n_basic, j.pg->n_nodes, j.pg->n_prod(), j.pg->prod.data(), j.pg->n_basis, j.pg->basis_node.data(),
-                         j.pg->xi.data(), j.AL * j.AR, tree_row_lanes(j.AL), true, sc, &terr, group ? j.pg->basic_map.data() : nullptr,
-                         group ? j.pg->cut_local.data() : nullptr, (int)j.pg->cut_local.size()) != MTP_OK) continue;
-        if (tree_jit_smem_bytes(sc.n_val, sc.n_adj, j.AR, tree_threads(j.AL)) > 225 * 1024) continue;
-        std::string why;
-        j.pg->cubin[j.key] = tree_jit_compile(sc, j.AL, j.AR, &why);
-      }
-    };
-    std::vector<std::thread> workers;
-    const unsigned hw = std::max(1u, std::thread::hardware_concurrency());
-    for (unsigned t = 0; t < std::min<unsigned>(std::min(hw, 16u), (unsigned)jobs.size()); ++t) workers.emplace_back(work);
-    for (auto &w : workers) w.join();
-    for (auto &pg : h->progs)                  // drop failed compilations: get_tree then decides on its own
-      for (auto it = pg.cubin.begin(); it != pg.cubin.end();) it = it->second.empty() ? pg.cubin.erase(it) : std::next(it);
-  }
-  // validate the table(s) and build the large-system schedules now, so that errors surface at create
-  for (size_t q = h->partitioned ? 1 : 0; q < h->progs.size(); ++q) {
-    const mtp_handle::TreeDev *td = nullptr;
-    int AL = 0, AR = 1;
-    tree_pick_shape(h->progs[q].slots[1][0], h->progs[q].slots[1][1], 0, &AL, &AR);
-    int rc = get_tree(h, h->progs[q], AL, AR, true, &td);
+  // K2: the specialised kernels; when they cannot be had (no NVRTC, ...) the reason is kept for mtp_last_error and
+  // the interpreter is set up instead.  A table neither form can run fails here.
+  int rc = ensure_jit(h);
+  if (rc != MTP_OK) {
+    rc = ensure_interp(h);
     if (rc != MTP_OK) { g_create_error = h->err; mtp_destroy(h); return rc; }
+    h->err = "specialised contraction kernels not in use: " + h->jit_note;
   }
   *out = h;
   return MTP_OK;
@@ -453,12 +579,8 @@ extern "C" int mtp_set_option(mtp_handle *h, int key, int64_t v) {
     case MTP_OPT_VARIANT: if (v < 0 || v > 2) return fail(h, MTP_EINVAL, "bad variant"); h->variant = (int)v; return MTP_OK;
     case MTP_OPT_PROFILE: h->profile = v != 0; return MTP_OK;
     case MTP_OPT_TREE_CODEGEN:
-      if (h->codegen != (v != 0)) {          // schedules are cached with or without their specialised kernel
-        for (auto &pg : h->progs) {
-          for (auto &kv : pg.trees) { tree_jit_destroy(kv.second.jit); kv.second.jit = nullptr; }
-          pg.trees.clear();                  // device arrays stay owned by the handle (to_free)
-        }
-      }
+      if (v != 0 && !h->jit_ready) return fail(h, MTP_EUNSUP, "specialised contraction kernels not available: " + h->jit_note);
+      if (v == 0) { int rc = ensure_interp(h); if (rc != MTP_OK) return rc; }
       h->codegen = v != 0; return MTP_OK;
   }
   return fail(h, MTP_EINVAL, "unknown option");
@@ -470,11 +592,14 @@ extern "C" int mtp_get_option(const mtp_handle *h, int key, int64_t *v) {
     case MTP_OPT_FORCE_MODE: *v = h->force_mode; return MTP_OK;
     case MTP_OPT_VARIANT: *v = h->variant; return MTP_OK;
     case MTP_OPT_PROFILE: *v = h->profile; return MTP_OK;
-    case MTP_OPT_TREE_CODEGEN: *v = h->codegen; return MTP_OK;
-    case MTP_INFO_TREE_KERNELS: {             // specialised K2 kernels in use
-      int n = 0;
-      for (auto &pg : h->progs) for (auto &kv : pg.trees) n += kv.second.jit != nullptr;
-      *v = n; return MTP_OK;
+    case MTP_OPT_TREE_CODEGEN: *v = h->codegen && h->jit_ready; return MTP_OK;
+    case MTP_INFO_TREE_KERNELS: *v = h->jit_ready ? h->n_jit_kernels : 0; return MTP_OK;      // specialised K2 kernels loaded
+    case MTP_INFO_TREE_PROGRAMS: *v = h->jit_ready ? (int64_t)h->jprogs.size() : 0; return MTP_OK;
+    case MTP_INFO_INPUT_ERRORS: {             // synchronises: pairs the packing kernel rejected since the last read
+      int flag = 0;
+      if (cudaMemcpy(&flag, h->d_flag, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess) return MTP_ECUDA;
+      if (flag) cudaMemset(h->d_flag, 0, sizeof(int));
+      *v = flag; return MTP_OK;
     }
   }
   return MTP_EINVAL;
@@ -483,9 +608,9 @@ extern "C" int mtp_get_option(const mtp_handle *h, int key, int64_t *v) {
 // ---- chunk scheduler / workspace plan ---------------------------------------------------
 namespace {
 struct Plan {
-  int64_t N = 0, nnz = 0, C = 0, ldm = 0;
+  int64_t N = 0, nnz = 0, C = 0, cols = 0;      // cols: C rounded up to whole tiles of 128 atoms (kTile)
   int n_chunks = 0, P = 1, atomic = 0, grid_chunk = 0, AL = 0, AR = 1, elide = 1;
-  size_t o_pos4 = 0, o_Ei = 0, o_M = 0, o_G = 0, o_wpart = 0, o_d4 = 0, o_B = 0, o_part = 0, o_red = 0, o_idxp = 0, o_S = 0, o_Sbar = 0, total = 0;
+  size_t o_pos4 = 0, o_Ei = 0, o_M = 0, o_G = 0, o_wpart = 0, o_d4 = 0, o_B = 0, o_red = 0, o_idxp = 0, o_S = 0, o_Sbar = 0, total = 0;
 };
 size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
@@ -504,31 +629,30 @@ int make_plan(const mtp_handle *h, int64_t N, int64_t nnz, int want_grade, int h
   }
   if (C > N) C = std::max<int64_t>(N, 1);
   pl.C = C;
-  pl.ldm = (C + 63) / 64 * 64;            // whole 64-atom K2 groups: the generated kernel stores G rows unpredicated
+  pl.cols = (C + kTile - 1) / kTile * kTile;
   pl.n_chunks = N ? (int)((N + C - 1) / C) : 0;
   const int NS = h->pl->nsb * h->pl->nsc;
   if (h->variant == MTP_VARIANT_THREAD) pl.P = 1;
   else if (h->variant == MTP_VARIANT_BLOCK) pl.P = h->pl->p_small;
   else pl.P = (N * NS >= 2LL * 148 * 256) ? 1 : h->pl->p_small;   // fill the SMs' register files
   pl.elide = want_grade ? 0 : 1;           // grades need every B_alpha stored
-  tree_pick_shape(h->progs[0].slots[pl.elide][0], h->progs[0].slots[pl.elide][1], N, &pl.AL, &pl.AR);
+  if (h->interp_ready) tree_pick_shape(h->progs[0].slots[pl.elide][0], h->progs[0].slots[pl.elide][1], N, &pl.AL, &pl.AR);
   pl.atomic = h->force_mode == MTP_FORCE_ATOMIC || (h->force_mode == MTP_FORCE_AUTO && !has_rev);
   pl.grid_chunk = h->pl->pairgrad_grid((int)C, pl.P);
   size_t o = 0;
   pl.o_pos4 = o; o = align_up(o + (size_t)N * 32);
   pl.o_Ei = o; o = align_up(o + (size_t)N * 8);
-  pl.o_M = o; o = align_up(o + (size_t)h->n_basic * pl.ldm * 8);
-  pl.o_G = o; o = align_up(o + (size_t)h->n_basic * pl.ldm * 8);
+  pl.o_M = o; o = align_up(o + (size_t)h->n_basic * pl.cols * 8);
+  pl.o_G = o; o = align_up(o + (size_t)h->n_basic * pl.cols * 8);
   pl.o_red = o; o = align_up(o + 256 * 8 * 8);
-  if (h->partitioned) {                      // cut values and their adjoints of one chunk (tree_partition.cpp)
-    pl.o_S = o; o = align_up(o + (size_t)h->n_cut_rows * pl.ldm * 8);
-    pl.o_Sbar = o; o = align_up(o + (size_t)h->n_cut_rows * pl.ldm * 8);
+  if (h->n_cut_rows > 0) {                   // cut values and their adjoints of one chunk (tree_partition.cpp)
+    pl.o_S = o; o = align_up(o + (size_t)h->n_cut_rows * pl.cols * 8);
+    pl.o_Sbar = o; o = align_up(o + (size_t)h->n_cut_rows * pl.cols * 8);
   }
   pl.o_idxp = o; o = align_up(o + (size_t)nnz * 4);          // packed neighbour words (used when shifts are given)
   pl.o_wpart = o; o = align_up(o + (size_t)std::max(1, pl.n_chunks) * pl.grid_chunk * 64);
   pl.o_d4 = o; if (!want_grade && !pl.atomic) o = align_up(o + (size_t)nnz * 32);
-  pl.o_B = o; if (want_grade) o = align_up(o + (size_t)C * h->n_basis * 8);
-  pl.o_part = o; if (want_grade) o = align_up(o + (size_t)64 * h->n_basis * 8);
+  pl.o_B = o; if (want_grade) o = align_up(o + (size_t)pl.cols * h->n_basis * 8);      // tiled Bt of one chunk
   pl.total = o;
   return MTP_OK;
 }
@@ -564,13 +688,16 @@ void fill_pair_args(const mtp_handle *h, PairArgs &pa, const double *pos4, const
   pa.M = nullptr; pa.G = nullptr; pa.d4 = nullptr; pa.F = nullptr; pa.wpart = nullptr; pa.kmap = nullptr;
 }
 
-// One K2 launch of program pg over the chunk [c0, c1).
+// One chunk of K2 work: B_alpha / E_i (forward) and, when want_adj, G = dE_i/dM.  B != null: every basis value of
+// the chunk is exported as the tiled Bt (no leaf elision).  All arrays are chunk-relative and tiled (kTile).
 struct K2Io {
-  const double *pos4; const double *M; double *G; long long ldm; double *Ei; double *B;
+  const double *pos4; const double *M; double *G; double *Ei; double *B;
   int c0, c1; int want_adj; int64_t N; double *S; double *Sbar;
 };
-int launch_prog(mtp_handle *h, mtp_handle::Prog &pg, const K2Io &io, bool elide, const double *M, double *G, int want_adj,
-                double *S, const double *Sbar, int g_accum, int write_energy, double *B, cudaStream_t st) {
+
+// interpreter: one launch of program pg
+int launch_prog(mtp_handle *h, mtp_handle::Prog &pg, const K2Io &io, bool elide, const double *M, double *G, int n_rows,
+                int want_adj, double *S, const double *Sbar, int g_accum, int write_energy, double *B, cudaStream_t st) {
   int AL = 0, AR = 1;
   tree_pick_shape(pg.slots[elide][0], pg.slots[elide][1], io.N, &AL, &AR);
   const mtp_handle::TreeDev *td = nullptr;
@@ -588,32 +715,63 @@ int launch_prog(mtp_handle *h, mtp_handle::Prog &pg, const K2Io &io, bool elide,
   ta.gseed_k = td->d_gseed_k; ta.gseed_val = td->d_gseed_val; ta.n_gseed = (int)sc.gseed_k.size();
   ta.gzero_k = td->d_gzero_k; ta.n_gzero = (int)sc.gzero_k.size();
   ta.n_val = sc.n_val; ta.n_adj = sc.n_adj; ta.n_basic = pg.n_basic; ta.n_basis = pg.n_basis;
-  ta.M = M; ta.G = G; ta.ldm = io.ldm; ta.Ei = io.Ei; ta.B = B; ta.c0 = io.c0; ta.c1 = io.c1; ta.want_adj = want_adj;
+  ta.M = M; ta.G = G; ta.n_rows = n_rows; ta.n_cut_rows = h->n_cut_rows;
+  ta.Ei = io.Ei; ta.B = B; ta.c0 = io.c0; ta.c1 = io.c1; ta.want_adj = want_adj;
   ta.mload_k = td->d_mload_k; ta.cut_row = td->d_cut_row; ta.cut_vslot = td->d_cut_vslot; ta.cut_aslot = td->d_cut_aslot;
   ta.n_cut = (int)pg.cut_local.size();
   ta.S = S; ta.Sbar = Sbar; ta.g_accum = g_accum; ta.write_energy = write_energy;
-  TIMED(h, CLS_TREE, st, (td->jit ? tree_jit_launch(td->jit, ta, st) : launch_tree(ta, AL, AR, st)));
+  TIMED(h, CLS_TREE, st, launch_tree(ta, AL, AR, st));
   return MTP_OK;
 }
 
-// K2 over one chunk: B_alpha / E_i (forward) and, when io.want_adj, G = dE_i/dM.  io.B != null keeps every basis
-// value (no leaf elision).  A partitioned table runs its group programs forward, the top program, and the
-// group programs again forward + backward seeded with the top program's adjoints (tree_partition.cpp).
-int run_k2(mtp_handle *h, const K2Io &io, cudaStream_t st) {
+// A partitioned table runs its group programs forward, the top program, and the group programs again forward +
+// backward seeded with the top program's adjoints (tree_partition.cpp).
+int run_k2_interp(mtp_handle *h, const K2Io &io, cudaStream_t st) {
+  int rc = ensure_interp(h);
+  if (rc != MTP_OK) return rc;
   const bool elide = io.B == nullptr;
   if (!h->partitioned)
-    return launch_prog(h, h->progs[0], io, elide, io.M, io.G, io.want_adj, nullptr, nullptr, 0, 1, io.B, st);
-  int rc = MTP_OK;
-  CU(h, launch_scopy(io.S, io.ldm, h->n_basic, io.c1 - io.c0, h->d_gmap, io.M, st));
+    return launch_prog(h, h->progs[0], io, elide, io.M, io.G, h->n_basic, io.want_adj, nullptr, nullptr, 0, 1, io.B, st);
+  CU(h, launch_scopy(io.S, h->n_cut_rows, h->n_basic, io.c1 - io.c0, h->d_gmap, io.M, st));
   for (size_t q = 2; q < h->progs.size() && rc == MTP_OK; ++q)
-    rc = launch_prog(h, h->progs[q], io, true, io.M, nullptr, 0, io.S, nullptr, 0, 0, nullptr, st);
+    rc = launch_prog(h, h->progs[q], io, true, io.M, nullptr, h->n_basic, 0, io.S, nullptr, 0, 0, nullptr, st);
   if (rc != MTP_OK) return rc;
-  rc = launch_prog(h, h->progs[1], io, elide, io.S, io.Sbar, io.want_adj, nullptr, nullptr, 0, 1, io.B, st);
+  rc = launch_prog(h, h->progs[1], io, elide, io.S, io.Sbar, h->n_cut_rows, io.want_adj, nullptr, nullptr, 0, 1, io.B, st);
   if (rc != MTP_OK || !io.want_adj) return rc;
-  CU(h, launch_ginit(io.G, io.ldm, h->n_basic, io.c1 - io.c0, h->d_gmap, io.Sbar, st));
+  CU(h, launch_ginit(io.G, h->n_cut_rows, h->n_basic, io.c1 - io.c0, h->d_gmap, io.Sbar, st));
   for (size_t q = 2; q < h->progs.size() && rc == MTP_OK; ++q)
-    rc = launch_prog(h, h->progs[q], io, true, io.M, io.G, 1, nullptr, io.Sbar, 1, 0, nullptr, st);
+    rc = launch_prog(h, h->progs[q], io, true, io.M, io.G, h->n_basic, 1, nullptr, io.Sbar, 1, 0, nullptr, st);
   return rc;
+}
+
+// specialised kernels: K2_VALUES exports (B or the cut values), K2_EF does energy + adjoint
+int run_k2_jit(mtp_handle *h, const K2Io &io, cudaStream_t st) {
+  K2Args ka;
+  ka.in = io.M; ka.out = io.G; ka.sbar = nullptr; ka.sout = nullptr; ka.bt = io.B; ka.Ei = io.Ei;
+  ka.xi0 = h->d_xi0; ka.pos4 = io.pos4;
+  ka.n_io = h->n_basic; ka.n_cut = h->n_cut_rows; ka.n_bt = h->n_basis; ka.c0 = io.c0; ka.n = io.c1 - io.c0;
+  const bool want_ef = io.want_adj || !io.B;
+  if (!h->jit_partitioned) {
+    if (io.B) TIMED(h, CLS_TREE, st, k2_jit_launch(h->jprogs[0].kern[K2_VALUES], ka, st));
+    if (want_ef) TIMED(h, CLS_TREE, st, k2_jit_launch(h->jprogs[0].kern[K2_EF], ka, st));
+    return MTP_OK;
+  }
+  CU(h, launch_scopy(io.S, h->n_cut_rows, h->n_basic, io.c1 - io.c0, h->d_gmap, io.M, st));
+  ka.sout = io.S;
+  for (size_t q = 1; q < h->jprogs.size(); ++q) TIMED(h, CLS_TREE, st, k2_jit_launch(h->jprogs[q].kern[K2_VALUES], ka, st));
+  K2Args kt = ka;                              // top program: inputs = cut values, adjoints = dE/dS
+  kt.in = io.S; kt.out = io.Sbar; kt.n_io = h->n_cut_rows; kt.sout = nullptr;
+  if (io.B) TIMED(h, CLS_TREE, st, k2_jit_launch(h->jprogs[0].kern[K2_VALUES], kt, st));
+  if (want_ef) TIMED(h, CLS_TREE, st, k2_jit_launch(h->jprogs[0].kern[K2_EF], kt, st));
+  if (!io.want_adj) return MTP_OK;
+  CU(h, launch_ginit(io.G, h->n_cut_rows, h->n_basic, io.c1 - io.c0, h->d_gmap, io.Sbar, st));
+  ka.sout = nullptr; ka.sbar = io.Sbar;
+  for (size_t q = 1; q < h->jprogs.size(); ++q) TIMED(h, CLS_TREE, st, k2_jit_launch(h->jprogs[q].kern[K2_EF], ka, st));
+  return MTP_OK;
+}
+
+int run_k2(mtp_handle *h, const K2Io &io, cudaStream_t st) {
+  return (h->codegen && h->jit_ready) ? run_k2_jit(h, io, st) : run_k2_interp(h, io, st);
 }
 }  // namespace
 
@@ -666,19 +824,19 @@ static int compute_impl(mtp_handle *h, int64_t N, const double *d_pos, const int
   if (pl.atomic) CU(h, launch_zero(d_F, 3 * N, st));
   const int32_t *idxp = d_idx;
   if (d_shift && nnz > 0) {
-    if (!pipe) CU(h, launch_pack_pairs(d_idx, (const signed char *)d_shift, nnz, (int *)(ws + pl.o_idxp), st));
+    if (!pipe) CU(h, launch_pack_pairs(d_idx, (const signed char *)d_shift, nnz, N, (int *)(ws + pl.o_idxp), h->d_flag, st));
     idxp = (const int32_t *)(ws + pl.o_idxp);
   }
   fill_pair_args(h, pa, pos4, d_off, idxp, d_shift);
-  pa.ldm = pl.ldm;
-  K2Io io{pos4, M, G, pl.ldm, Ei, nullptr, 0, 0, 1, N, (double *)(ws + pl.o_S), (double *)(ws + pl.o_Sbar)};
+  pa.n_rows = h->n_basic;
+  K2Io io{pos4, M, G, Ei, nullptr, 0, 0, 1, N, (double *)(ws + pl.o_S), (double *)(ws + pl.o_Sbar)};
   for (int c = 0; c < pl.n_chunks; ++c) {
     pa.c0 = (int)(c * pl.C); pa.c1 = (int)std::min<int64_t>(N, (c + 1) * pl.C);
     if (pipe) {                                  // this chunk's pairs have just arrived: pack their neighbour words
       CU(h, cudaStreamWaitEvent(st, (*pipe->chunk_ready)[c], 0));
       const long long p0 = (*pipe->chunk_pair0)[c], p1 = (*pipe->chunk_pair0)[c + 1];
       if (d_shift && p1 > p0)
-        CU(h, launch_pack_pairs(d_idx + p0, (const signed char *)d_shift + 3 * p0, p1 - p0, (int *)(ws + pl.o_idxp) + p0, st));
+        CU(h, launch_pack_pairs(d_idx + p0, (const signed char *)d_shift + 3 * p0, p1 - p0, N, (int *)(ws + pl.o_idxp) + p0, h->d_flag, st));
     }
     pa.M = M; pa.G = G; pa.kmap = h->d_kmapF;
     TIMED(h, CLS_MOMENTS, st, h->pl->moments(pa, pl.P, st));
@@ -726,33 +884,31 @@ extern "C" int mtp_grade(mtp_handle *h, int64_t N, const double *d_pos, const in
   if (rc != MTP_OK) return rc;
   char *ws = (char *)d_ws + base;
   double *pos4 = (double *)(ws + pl.o_pos4), *Ei = (double *)(ws + pl.o_Ei), *M = (double *)(ws + pl.o_M);
-  double *G = (double *)(ws + pl.o_G), *Bc = (double *)(ws + pl.o_B), *part = (double *)(ws + pl.o_part);
+  double *G = (double *)(ws + pl.o_G), *Bt = (double *)(ws + pl.o_B);      // Bt: tiled [tiles][n_basis][128] of one chunk
   double *Bsum = d_Bsum ? d_Bsum : (double *)(ws + pl.total);
   if (mode != 0 || d_Bsum) CU(h, launch_zero(Bsum, h->n_basis, st));
   if (N > 0) {
     CU(h, launch_pack(d_pos, d_type, (int)N, pos4, st));
     const int32_t *idxp = d_idx;
     if (d_shift && nnz > 0) {
-      CU(h, launch_pack_pairs(d_idx, (const signed char *)d_shift, nnz, (int *)(ws + pl.o_idxp), st));
+      CU(h, launch_pack_pairs(d_idx, (const signed char *)d_shift, nnz, N, (int *)(ws + pl.o_idxp), h->d_flag, st));
       idxp = (const int32_t *)(ws + pl.o_idxp);
     }
     fill_pair_args(h, pa, pos4, d_off, idxp, d_shift);
-    pa.ldm = pl.ldm;
-    K2Io io{pos4, M, G, pl.ldm, Ei, nullptr, 0, 0, 0, N, (double *)(ws + pl.o_S), (double *)(ws + pl.o_Sbar)};
+    pa.n_rows = h->n_basic;
+    K2Io io{pos4, M, G, Ei, nullptr, 0, 0, 0, N, (double *)(ws + pl.o_S), (double *)(ws + pl.o_Sbar)};
     for (int c = 0; c < pl.n_chunks; ++c) {
       pa.c0 = (int)(c * pl.C); pa.c1 = (int)std::min<int64_t>(N, (c + 1) * pl.C);
       pa.M = M; pa.kmap = h->d_kmapF;
       TIMED(h, CLS_MOMENTS, st, h->pl->moments(pa, pl.P, st));
       io.c0 = pa.c0; io.c1 = pa.c1;
-      // B rows are indexed by absolute atom: point the kernel at a base shifted by -c0 rows
-      double *Brows = d_B ? d_B : Bc - (size_t)pa.c0 * h->n_basis;
-      io.B = Brows;
+      io.B = Bt;
       rc = run_k2(h, io, st);
       if (rc != MTP_OK) return rc;
-      const double *Bchunk = Brows + (size_t)pa.c0 * h->n_basis;
       const int64_t nc = pa.c1 - pa.c0;
-      if (mode != 1) TIMED(h, CLS_GRADE, st, launch_grade(Bchunk, d_Ainv, nc, h->n_basis, d_gamma_atom + pa.c0, st));
-      if (mode != 0 || d_Bsum) CU(h, launch_colsum(Bchunk, nc, h->n_basis, Bsum, part, st));
+      if (mode != 1) TIMED(h, CLS_GRADE, st, launch_grade(Bt, d_Ainv, nc, h->n_basis, d_gamma_atom + pa.c0, st));
+      if (mode != 0 || d_Bsum) CU(h, launch_colsum(Bt, nc, h->n_basis, Bsum, st));
+      if (d_B) CU(h, launch_untile(Bt, h->n_basis, nc, d_B + (size_t)pa.c0 * h->n_basis, h->n_basis, 1, st));   // [atom][alpha] for the caller
     }
   }
   if (mode != 0) CU(h, launch_grade_cfg(Bsum, d_Ainv, h->n_basis, nullptr, d_gamma_cfg, st));
@@ -841,16 +997,17 @@ extern "C" int mtp_debug_moments(mtp_handle *h, int64_t N, const double *d_pos, 
   const int64_t saved = h->chunk_atoms;
   h->chunk_atoms = N;                       // single chunk so that M, G hold every atom
   Plan pl;
-  int rc = make_plan(h, N, 0, 0, 0, pl);
+  int rc = make_plan(h, N, 0, 1, 0, pl);    // sized like a grade call: the plan then has room for the tiled B
   h->chunk_atoms = saved;
   if (rc != MTP_OK) return rc;
   const size_t base = align_up((size_t)(uintptr_t)d_ws) - (size_t)(uintptr_t)d_ws;
-  if (!d_ws || ws_bytes < pl.total + base) return fail(h, MTP_ESIZE, "workspace too small");
+  if (!d_ws || ws_bytes < pl.total + base) return fail(h, MTP_ESIZE, "workspace too small (size it with want_grade = 1)");
   PairArgs pa;
   rc = box_setup(h, box, d_shift == nullptr, h->r_cut, pa);
   if (rc != MTP_OK) return rc;
   char *ws = (char *)d_ws + base;
   double *pos4 = (double *)(ws + pl.o_pos4), *Ei = (double *)(ws + pl.o_Ei), *M = (double *)(ws + pl.o_M), *G = (double *)(ws + pl.o_G);
+  double *Bt = (double *)(ws + pl.o_B);
   CU(h, launch_pack(d_pos, d_type, (int)N, pos4, st));
   int *tmp_idxp = nullptr;                  // diagnostics only: this entry point has no nnz argument
   if (d_shift) {
@@ -858,25 +1015,24 @@ extern "C" int mtp_debug_moments(mtp_handle *h, int64_t N, const double *d_pos, 
     CU(h, cudaMemcpyAsync(&nnz, d_off + N, 8, cudaMemcpyDeviceToHost, st));
     CU(h, cudaStreamSynchronize(st));
     CU(h, cudaMalloc((void **)&tmp_idxp, (size_t)std::max<long long>(nnz, 1) * 4));
-    cudaError_t e = launch_pack_pairs(d_idx, (const signed char *)d_shift, nnz, tmp_idxp, st);
+    cudaError_t e = launch_pack_pairs(d_idx, (const signed char *)d_shift, nnz, N, tmp_idxp, h->d_flag, st);
     if (e != cudaSuccess) { cudaFree(tmp_idxp); return cuda_fail(h, e, "launch_pack_pairs"); }
   }
   fill_pair_args(h, pa, pos4, d_off, tmp_idxp ? tmp_idxp : d_idx, d_shift);
-  pa.ldm = pl.ldm; pa.c0 = 0; pa.c1 = (int)N; pa.M = M; pa.kmap = h->d_kmapF;
+  pa.n_rows = h->n_basic; pa.c0 = 0; pa.c1 = (int)N; pa.M = M; pa.kmap = h->d_kmapF;
   {
     cudaError_t e = h->pl->moments(pa, pl.P, st);
     if (tmp_idxp) { cudaStreamSynchronize(st); cudaFree(tmp_idxp); }
     if (e != cudaSuccess) return cuda_fail(h, e, "moments");
   }
-  // B is exported, so every basis value is stored (no leaf elision).  When the caller does not want B the
-  // scratch chunk of the workspace cannot be assumed (this entry point sizes it without grades): require d_B.
-  if (!d_B) return fail(h, MTP_EINVAL, "mtp_debug_moments: d_B is required");
-  K2Io io{pos4, M, G, pl.ldm, Ei, d_B, 0, (int)N, 1, N, (double *)(ws + pl.o_S), (double *)(ws + pl.o_Sbar)};
+  // B is exported, so every basis value is stored (no leaf elision)
+  K2Io io{pos4, M, G, Ei, Bt, 0, (int)N, 1, N, (double *)(ws + pl.o_S), (double *)(ws + pl.o_Sbar)};
   rc = run_k2(h, io, st);
   if (rc != MTP_OK) return rc;
-  // outputs are [n_basic][N] (component-major), the kernels' own layout
-  if (d_M) CU(h, cudaMemcpy2DAsync(d_M, (size_t)N * 8, M, (size_t)pl.ldm * 8, (size_t)N * 8, h->n_basic, cudaMemcpyDeviceToDevice, st));
-  if (d_G) CU(h, cudaMemcpy2DAsync(d_G, (size_t)N * 8, G, (size_t)pl.ldm * 8, (size_t)N * 8, h->n_basic, cudaMemcpyDeviceToDevice, st));
+  // outputs: M, G as [n_basic][N] (component-major), B as [N][n_basis]
+  if (d_M) CU(h, launch_untile(M, h->n_basic, N, d_M, N, 0, st));
+  if (d_G) CU(h, launch_untile(G, h->n_basic, N, d_G, N, 0, st));
+  if (d_B) CU(h, launch_untile(Bt, h->n_basis, N, d_B, h->n_basis, 1, st));
   return MTP_OK;
 }
 
@@ -885,21 +1041,44 @@ extern "C" int mtp_peak_dfma(int64_t iters, double *d_sink, double *out_flops, v
   return launch_peak_dfma(iters, d_sink, out_flops, (cudaStream_t)stream) == cudaSuccess ? MTP_OK : MTP_ECUDA;
 }
 
-// Useful flops (FMA = 2, MUL/ADD = 1), each quantity counted once -- DESIGN.md "Roofline".
-//   per pair : geometry + rsqrt (12) + Chebyshev T_b, T'_b (2*3 per b) + f, f' (2*2 n_beta n_mu)
-//              + monomials (1 per packed monomial of rank <= nu_max) + moments (2 n_basic)
-//              + pair derivative (value+gradient of sum_mu f_mu P_mu: 8 n_basic)
-//   per atom : tree forward 3/op, adjoint 6/op, energy 2 n_basis;  grade 2 n_basis^2
+// Useful flops (FMA = 2), every quantity counted once, recomputation not counted -- DESIGN.md section 6:
+//   K1 per pair  30 + 16 n_mu + 2 C(nu_max + 3, 3) + 2 n_basic      (geometry, radial functions, monomials, moments)
+//   K3 per pair  30 + 16 n_mu + 8 n_basic                            (radial derivatives, value + gradient of sum_mu f_mu P_mu)
+//   K2 per atom  6 n_prod + 2 n_basis                                (forward 2 / op, adjoint 4 / op, energy)
+//   K5 per atom  2 n_basis^2
+// flop_per_pair[0] = K1, [1] = K3.
 extern "C" int mtp_cost_model(const mtp_handle *h, double *flop_per_pair, double *flop_per_atom_tree,
                               double *flop_per_atom_grade) {
   if (!h) return MTP_EINVAL;
-  int numax = 0;
-  for (int k = 0; k < h->n_basic; ++k) (void)k;
-  // highest rank present in the table
-  numax = rt_numax(h->pl->lev, 0);
+  const int numax = rt_numax(h->pl->lev, 0);
   const double monos = (numax + 1.0) * (numax + 2.0) * (numax + 3.0) / 6.0;
-  if (flop_per_pair) *flop_per_pair = 12.0 + 6.0 * h->nb + 4.0 * h->nb * h->nmu + monos + 10.0 * h->n_basic;
-  if (flop_per_atom_tree) *flop_per_atom_tree = 9.0 * (double)h->n_prod + 2.0 * h->n_basis;
+  if (flop_per_pair) {
+    flop_per_pair[0] = 30.0 + 16.0 * h->nmu + 2.0 * monos + 2.0 * h->n_basic;
+    flop_per_pair[1] = 30.0 + 16.0 * h->nmu + 8.0 * h->n_basic;
+  }
+  if (flop_per_atom_tree) *flop_per_atom_tree = 6.0 * (double)h->n_prod + 2.0 * h->n_basis;
   if (flop_per_atom_grade) *flop_per_atom_grade = 2.0 * (double)h->n_basis * h->n_basis;
+  return MTP_OK;
+}
+
+// Host-only: the register program mtp_create would run for this table (whole table only; kind 0 = energy + adjoint,
+// 1 = basis values), for emulation in the tests.  prog receives up to cap instructions of 7 int32 each
+// (op, d, a, b, c, k, x -- tree_codegen.h), consts up to ccap doubles; info = {instructions, constants, registers, slots}.
+extern "C" int mtp_k2_program(const mtp_params *p, int kind, int32_t *prog, int64_t cap, double *consts, int64_t ccap,
+                              int64_t *info) {
+  if (!p || !info || kind < 0 || kind > 1 || !p->xi) return MTP_EINVAL;
+  K2Table whole;
+  const char *verr = "";
+  if (k2_validate(p->n_basic, p->n_nodes, p->n_prod, p->prod, p->n_basis, p->basis_node, &verr) != MTP_OK) return MTP_EINVAL;
+  whole.n_basic = p->n_basic; whole.n_nodes = p->n_nodes; whole.prod.assign(p->prod, p->prod + 4 * (size_t)p->n_prod);
+  whole.basis_node.assign(p->basis_node, p->basis_node + p->n_basis);
+  whole.xi.assign(p->xi, p->xi + p->n_basis);
+  K2Gen g;
+  std::string err;
+  int rc = k2_generate(whole, (K2Kind)kind, kK2Window, kK2Lookahead, g, &err);
+  if (rc != MTP_OK) { g_create_error = err; return rc; }
+  info[0] = (int64_t)g.prog.size(); info[1] = (int64_t)g.consts.size(); info[2] = g.n_regs; info[3] = g.n_slots;
+  if (prog && cap >= (int64_t)g.prog.size()) std::memcpy(prog, g.prog.data(), g.prog.size() * sizeof(K2Inst));
+  if (consts && ccap >= (int64_t)g.consts.size() && !g.consts.empty()) std::memcpy(consts, g.consts.data(), g.consts.size() * 8);
   return MTP_OK;
 }

@@ -12,7 +12,7 @@
 namespace mtpb {
 
 constexpr int GBM = 128, GBN = 64, GBK = 16;
-constexpr int GLDA = GBK + 4, GLDB = GBN + 4;   // strides = 4 mod 16 doubles: the mma fragment loads are conflict-free
+constexpr int GLDA = GBM + 8, GLDB = GBN + 4;   // strides = 8 / 4 mod 16 doubles: the mma fragment loads are conflict-free
 
 // One fp64 tensor-core MMA (the only fp64 MMA on sm_100: legacy mma.sync, no tcgen05 kind): D(8x8) += A(8x4) B(4x8).
 // Fragments: lane l holds A[l/4][l%4], B[l%4][l/4], C[l/4][2(l%4) + {0,1}].  Measured 37.1 TFLOP/s = the DFMA
@@ -22,9 +22,11 @@ __device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b)
 }
 
 // CTA tile 128 atoms x 64 columns, 8 warps (4 x 2), warp tile 32 x 32 = 4 x 4 MMA tiles.
-__global__ void __launch_bounds__(256) k_grade(const double *__restrict__ B, const double *__restrict__ Ainv,
+// B arrives as the tiled Bt [tile of 128 atoms][nb][128] the K2 kernels write (kTile = GBM): a CTA's A tile is one
+// contiguous run of 128 atoms per k, kept k-major in shared memory.
+__global__ void __launch_bounds__(256) k_grade(const double *__restrict__ Bt, const double *__restrict__ Ainv,
                                                long long n, int nb, double *__restrict__ gamma) {
-  __shared__ __align__(16) double As[GBM][GLDA];     // B rows of the tile, [atom][k]
+  __shared__ __align__(16) double As[GBK][GLDA];     // B values of the tile, [k][atom]
   __shared__ __align__(16) double Bs[GBK][GLDB];     // Ainv rows of the tile, [k][column]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm = (warp & 3) * 32, wn = (warp >> 2) * 32;
@@ -36,14 +38,14 @@ __global__ void __launch_bounds__(256) k_grade(const double *__restrict__ B, con
   for (int i = 0; i < 4; ++i)
 #pragma unroll
     for (int j = 0; j < 4; ++j) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
-  const int arow = tid >> 1, ak = (tid & 1) * 8;        // A tile: 128 rows x 16 k
+  const int arow = tid & 127, ak = (tid >> 7) * 8;      // A tile: 16 k x 128 atoms, consecutive threads = consecutive atoms
+  const double *Btile = Bt + (size_t)blockIdx.y * nb * GBM;
   const int bk = tid >> 4, bc = (tid & 15) * 4;         // Ainv tile: 16 k x 64 cols
   for (int k0 = 0; k0 < nb; k0 += GBK) {
     {
       const long long row = m0 + arow;
-      const double *src = B + row * nb + k0 + ak;
 #pragma unroll
-      for (int j = 0; j < 8; ++j) As[arow][ak + j] = (row < n && k0 + ak + j < nb) ? src[j] : 0.0;
+      for (int j = 0; j < 8; ++j) As[ak + j][arow] = (row < n && k0 + ak + j < nb) ? Btile[(size_t)(k0 + ak + j) * GBM + arow] : 0.0;
       const int kr = k0 + bk;
       const double *s2 = Ainv + (long long)kr * nb + n0 + bc;
 #pragma unroll
@@ -54,7 +56,7 @@ __global__ void __launch_bounds__(256) k_grade(const double *__restrict__ B, con
     for (int kk = 0; kk < GBK; kk += 4) {
       double a[4], b[4];
 #pragma unroll
-      for (int i = 0; i < 4; ++i) a[i] = As[wm + 8 * i + fr][kk + fc];
+      for (int i = 0; i < 4; ++i) a[i] = As[kk + fc][wm + 8 * i + fr];
 #pragma unroll
       for (int j = 0; j < 4; ++j) b[j] = Bs[kk + fc][wn + 8 * j + fr];
 #pragma unroll
@@ -91,12 +93,13 @@ __global__ void k_grade_cfg(const double *__restrict__ Bsum, const double *__res
     atomicMax(reinterpret_cast<unsigned long long *>(gamma_cfg), (unsigned long long)__double_as_longlong(m));
 }
 
-cudaError_t launch_grade(const double *B, const double *Ainv, long long n, int nb, double *gamma, cudaStream_t st) {
+cudaError_t launch_grade(const double *Bt, const double *Ainv, long long n, int nb, double *gamma, cudaStream_t st) {
   if (n <= 0) return cudaSuccess;
   cudaError_t e = launch_zero(gamma, n, st);
   if (e != cudaSuccess) return e;
   dim3 g((nb + GBN - 1) / GBN, (unsigned)((n + GBM - 1) / GBM));
-  k_grade<<<g, 256, 0, st>>>(B, Ainv, n, nb, gamma);
+  static_assert(GBM == kTile, "the CTA tile is one tile of the Bt layout");
+  k_grade<<<g, 256, 0, st>>>(Bt, Ainv, n, nb, gamma);
   count_launch();
   return cudaGetLastError();
 }

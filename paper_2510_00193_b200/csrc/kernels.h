@@ -7,6 +7,7 @@
 
 #include "pair_kernels_args.h"
 #include "tree.h"
+#include "tree_codegen.h"
 
 namespace mtpb {
 
@@ -27,17 +28,18 @@ struct TreeArgs {
   const int *gseed_k; const double *gseed_val; int n_gseed;   // packed moments that are basis functions
   const int *gzero_k; int n_gzero;         // packed moments no op reads
   const double *pos4;
-  const double *M; double *G; long long ldm;
+  const double *M; double *G; int n_rows;    // tiled [tiles][n_rows][128] (kTile); n_rows = rows of M and G
+  int n_cut_rows;                          // rows of the tiled S / Sbar arrays
   double *Ei;          // [N]
-  double *B;           // [N][n_basis] or null
+  double *B;           // tiled [tiles][n_basis][128] B_alpha of the chunk (column = atom - c0), or null
   int n_val, n_adj, n_basic, n_basis;
   int c0, c1;
   int want_adj;
   // sub-programs of a partitioned tree (tree_partition.cpp); all null / 0 / 1 for a whole table
   const int *mload_k;                      // [n_basic] row of M / G per local packed moment, or null = identity
   const int *cut_row, *cut_vslot, *cut_aslot; int n_cut;   // the group's cut nodes: row in S / Sbar, val slot, adj slot
-  double *S;                               // [n_cut_rows][ldm] cut values out (after the forward pass), or null
-  const double *Sbar;                      // [n_cut_rows][ldm] dE_i/d(cut) in (seeds of the backward pass), or null
+  double *S;                               // tiled [tiles][n_cut_rows][128] cut values out (after the forward pass), or null
+  const double *Sbar;                      // tiled, same shape: dE_i/d(cut) in (seeds of the backward pass), or null
   int g_accum;                             // 1: G[k] += (groups accumulate), 0: G[k] =
   int write_energy;                        // 0: group programs leave E_i alone
 };
@@ -46,18 +48,31 @@ int tree_threads(int AL);               // CTA size used with AL atom-lanes
 int tree_row_lanes(int AL);             // row-lanes R = threads / AL the schedule must be dealt for
 size_t tree_smem_bytes(int n_val, int n_adj, int AL, int AR);
 cudaError_t launch_tree(const TreeArgs &a, int AL, int AR, cudaStream_t st);
-// K2 specialised for one schedule with NVRTC (tree_jit.cpp); null when unavailable (reason in *why)
-struct TreeJit;
-TreeJit *tree_jit_build(const TreeSched &sc, int AL, int AR, std::string *why);
-std::vector<char> tree_jit_compile(const TreeSched &sc, int AL, int AR, std::string *why);   // host only, thread-safe
-TreeJit *tree_jit_load(const std::vector<char> &cubin, int AR, int NT, std::string *why);
-cudaError_t tree_jit_launch(const TreeJit *j, const TreeArgs &a, cudaStream_t st);
-void tree_jit_destroy(TreeJit *j);
-size_t tree_jit_smem_bytes(int n_val, int n_adj, int AR, int NT);
+// K2 specialised for one table with NVRTC (tree_codegen.cpp generates the register program, tree_jit.cpp compiles
+// and launches it).  All arrays tiled (kTile); one thread per atom.
+struct K2Args {
+  const double *in;        // [tiles][n_io][128] inputs: M (whole table, groups) or the cut values S (top program)
+  double *out;             // [tiles][n_io][128] dE_i/d(input): G or dE_i/dS
+  const double *sbar;      // [tiles][n_cut][128] seeds of a group program: dE_i/dS
+  double *sout;            // [tiles][n_cut][128] cut values a group program exports
+  double *bt;              // [tiles][n_bt][128] B_alpha (K2_VALUES of a whole table / top program)
+  double *Ei;              // [N]
+  const double *xi0; const double *pos4;
+  int n_io, n_cut, n_bt, c0, n;
+};
+struct K2Kernel;
+bool k2_jit_available(std::string *why);
+void k2_shape(int n_slots, int *threads, int *ctas_per_sm);   // threads = 0: does not fit
+std::string k2_source(const K2Gen &g);
+std::vector<char> k2_jit_compile(const K2Gen &g, std::string *why);   // host only, thread-safe
+K2Kernel *k2_jit_load(const std::vector<char> &cubin, int n_slots, std::string *why);
+cudaError_t k2_jit_launch(const K2Kernel *k, const K2Args &a, cudaStream_t st);
+void k2_jit_destroy(K2Kernel *k);
 
 // ---- K1 / K3: one entry per compiled level (pair_lev*.cu)
 struct PairLevel {
   int lev, nsb, nsc, nslot, p_small;
+  int smem_fixed;            // shared memory of a CTA besides the radial coefficients (bytes, largest variant)
   cudaError_t (*moments)(const PairArgs &a, int P, cudaStream_t st);
   cudaError_t (*pairgrad)(const PairArgs &a, int P, int atomic, cudaStream_t st, int *grid_out);
   int (*pairgrad_grid)(int n_atoms, int P);
@@ -69,22 +84,26 @@ cudaError_t launch_pack(const double *pos, const int *type, int n, double *pos4,
 cudaError_t launch_zero(double *p, long long n, cudaStream_t st);
 // G[k][:] = gmap[k] >= 0 ? Sbar[gmap[k]][:] : 0  (partitioned K2, before the group programs accumulate)
 // S[gmap[k]][:] = M[k][:] for the packed moments that are cut nodes themselves
-cudaError_t launch_scopy(double *S, long long ldm, int n_basic, int ncol, const int *gmap, const double *M, cudaStream_t st);
-cudaError_t launch_ginit(double *G, long long ldm, int n_basic, int ncol, const int *gmap, const double *Sbar,
+cudaError_t launch_scopy(double *S, int n_cut_rows, int n_basic, int ncol, const int *gmap, const double *M, cudaStream_t st);
+cudaError_t launch_ginit(double *G, int n_cut_rows, int n_basic, int ncol, const int *gmap, const double *Sbar,
                          cudaStream_t st);
-// out[p] = idx[p] | image_code(shift[p]) << 27
-cudaError_t launch_pack_pairs(const int *idx, const signed char *shift, long long nnz, int *out, cudaStream_t st);
+// dst[row][col] (leading dimension ld) = tiled src[tiles][rows][128], or the transpose dst[col][row] (ld = row length)
+cudaError_t launch_untile(const double *src, int rows, long long ncol, double *dst, long long ld, int transpose, cudaStream_t st);
+// out[p] = idx[p] | image_code(shift[p]) << 27; pairs with a shift outside {-1,0,1}^3 or an index outside [0, n_atoms)
+// are dropped and counted in *flag
+cudaError_t launch_pack_pairs(const int *idx, const signed char *shift, long long nnz, long long n_atoms, int *out, int *flag,
+                              cudaStream_t st);
 // F_k = sum_p d[p] - d[rev[p]] over row k (warp per atom, fixed order)
 cudaError_t launch_gather(const long long *off, const int *rev, const double *d4, int n, double *F, cudaStream_t st);
 // out[c] = sum_i in[i*stride + c] for c < ncomp <= 8, fixed order; scratch: 256 x 8 doubles (or null)
 cudaError_t launch_reduce(const double *in, long long n, int stride, int ncomp, double *out, double *scratch,
                           cudaStream_t st);
-// Bsum[b] = sum_i B[i][b]  (fixed order per column)
-cudaError_t launch_colsum(const double *B, long long n, int nb, double *Bsum, double *scratch, cudaStream_t st);
+// Bsum[b] += sum_i Bt[b][i] over the tiled Bt of a chunk (fixed order per row)
+cudaError_t launch_colsum(const double *Bt, long long n, int nb, double *Bsum, cudaStream_t st);
 
 // ---- K5 (grade_kernel.cu)
-// gamma[i] = max_k | sum_a B[i][a] Ainv[a][k] |
-cudaError_t launch_grade(const double *B, const double *Ainv, long long n, int nb, double *gamma, cudaStream_t st);
+// gamma[i] = max_k | sum_a B[i][a] Ainv[a][k] |, B given as the tiled Bt [tiles][nb][128]
+cudaError_t launch_grade(const double *Bt, const double *Ainv, long long n, int nb, double *gamma, cudaStream_t st);
 // gamma_cfg = max_k | sum_a Bsum[a] Ainv[a][k] |
 cudaError_t launch_grade_cfg(const double *Bsum, const double *Ainv, int nb, double *scratch, double *gamma_cfg,
                              cudaStream_t st);

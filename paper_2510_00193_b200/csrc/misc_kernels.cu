@@ -24,32 +24,46 @@ __global__ void k_pack(const double *__restrict__ pos, const int *__restrict__ t
 }
 
 // packed neighbour word j | code << 27 (pair_kernels.cuh): one 4-byte load per pair in K1 / K3 instead of
-// an index and three shift bytes, and the shift vector becomes a table lookup
+// an index and three shift bytes, and the shift vector becomes a table lookup.  The word has room for shifts in
+// {-1,0,1}^3 and indices below 2^27 only: anything else (and j outside [0, n_atoms)) is counted in *flag
+// (MTP_INFO_INPUT_ERRORS) and the pair is dropped (word -1) instead of aliasing to another image or atom.
 __global__ void k_pack_pairs(const int *__restrict__ idx, const signed char *__restrict__ shift, long long nnz,
-                             int *__restrict__ out) {
+                             long long n_atoms, int *__restrict__ out, int *__restrict__ flag) {
   const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= nnz) return;
-  const int code = shift_code(shift[3 * p], shift[3 * p + 1], shift[3 * p + 2]);
-  out[p] = idx[p] | (code << kIdxBits);
+  const int s0 = shift[3 * p], s1 = shift[3 * p + 1], s2 = shift[3 * p + 2], j = idx[p];
+  const bool ok = s0 >= -1 && s0 <= 1 && s1 >= -1 && s1 <= 1 && s2 >= -1 && s2 <= 1 && j >= 0 && j < n_atoms;
+  if (!ok) { atomicAdd(flag, 1); out[p] = -1; return; }
+  out[p] = (int)((unsigned)j | ((unsigned)shift_code(s0, s1, s2) << kIdxBits));
 }
 
 // G of a partitioned table before the group programs accumulate into it: dE_i/d(cut) for the packed moments
 // that are cut nodes themselves (gmap[k] = their cut row), 0 for the others
-__global__ void k_ginit(double *__restrict__ G, long long ldm, int n_basic, int ncol, const int *__restrict__ gmap,
+__global__ void k_ginit(double *__restrict__ G, int n_cut_rows, int n_basic, int ncol, const int *__restrict__ gmap,
                         const double *__restrict__ Sbar) {
   const int col = blockIdx.x * blockDim.x + threadIdx.x, k = blockIdx.y;
   if (col >= ncol || k >= n_basic) return;
   const int r = gmap[k];
-  G[(long long)k * ldm + col] = r >= 0 ? Sbar[(long long)r * ldm + col] : 0.0;
+  G[tiled_index(n_basic, k, col)] = r >= 0 ? Sbar[tiled_index(n_cut_rows, r, col)] : 0.0;
 }
 
 // cut values of the packed moments that are cut nodes themselves: S[gmap[k]][:] = M[k][:]
-__global__ void k_scopy(double *__restrict__ S, long long ldm, int n_basic, int ncol, const int *__restrict__ gmap,
+__global__ void k_scopy(double *__restrict__ S, int n_cut_rows, int n_basic, int ncol, const int *__restrict__ gmap,
                         const double *__restrict__ M) {
   const int col = blockIdx.x * blockDim.x + threadIdx.x, k = blockIdx.y;
   if (col >= ncol || k >= n_basic) return;
   const int r = gmap[k];
-  if (r >= 0) S[(long long)r * ldm + col] = M[(long long)k * ldm + col];
+  if (r >= 0) S[tiled_index(n_cut_rows, r, col)] = M[tiled_index(n_basic, k, col)];
+}
+
+// tiled [tiles][rows][128] -> row-major dst[row * ld + col], or its transpose dst[col * ld + row]
+__global__ void k_untile(const double *__restrict__ src, int rows, long long ncol, double *__restrict__ dst, long long ld,
+                         int transpose) {
+  const long long col = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const int row = blockIdx.y;
+  if (col >= ncol || row >= rows) return;
+  const double v = src[tiled_index(rows, row, col)];
+  if (transpose) dst[col * ld + row] = v; else dst[(long long)row * ld + col] = v;
 }
 
 __global__ void k_zero(double *p, long long n) {
@@ -110,21 +124,16 @@ __global__ void __launch_bounds__(1024) k_reduce_rows(const double *__restrict__
   }
 }
 
-// partial[s][b] = sum_{i = s, s+ns, ...} B[i][b]
-__global__ void k_colsum_part(const double *__restrict__ B, long long n, int nb, double *__restrict__ part) {
-  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+// Bsum[b] += sum_i Bt[b][i] over the tiled Bt of a chunk: one warp per b, lanes stride the atoms, xor-shuffle tree
+// (fixed order -> bit-reproducible); accumulates across chunks in launch order
+__global__ void __launch_bounds__(256) k_colsum(const double *__restrict__ Bt, long long n, int nb, double *__restrict__ Bsum) {
+  const int b = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (b >= nb) return;
   double acc = 0.0;
-  for (long long i = blockIdx.y; i < n; i += gridDim.y) acc += B[i * nb + b];
-  part[(size_t)blockIdx.y * nb + b] = acc;
-}
-// Bsum[b] += sum_s partial[s][b]   (accumulates across chunks in launch order)
-__global__ void k_colsum_final(const double *__restrict__ part, int ns, int nb, double *__restrict__ Bsum) {
-  const int b = blockIdx.x * blockDim.x + threadIdx.x;
-  if (b >= nb) return;
-  double acc = 0.0;
-  for (int s = 0; s < ns; ++s) acc += part[(size_t)s * nb + b];
-  Bsum[b] += acc;
+  for (long long i = lane; i < n; i += 32) acc += Bt[tiled_index(nb, b, i)];
+#pragma unroll
+  for (int o = 16; o >= 1; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  if (lane == 0) Bsum[b] += acc;
 }
 
 cudaError_t launch_pack(const double *pos, const int *type, int n, double *pos4, cudaStream_t st) {
@@ -133,22 +142,29 @@ cudaError_t launch_pack(const double *pos, const int *type, int n, double *pos4,
   count_launch();
   return cudaGetLastError();
 }
-cudaError_t launch_pack_pairs(const int *idx, const signed char *shift, long long nnz, int *out, cudaStream_t st) {
+cudaError_t launch_pack_pairs(const int *idx, const signed char *shift, long long nnz, long long n_atoms, int *out, int *flag,
+                              cudaStream_t st) {
   if (nnz <= 0) return cudaSuccess;
-  k_pack_pairs<<<(unsigned)((nnz + 255) / 256), 256, 0, st>>>(idx, shift, nnz, out);
+  k_pack_pairs<<<(unsigned)((nnz + 255) / 256), 256, 0, st>>>(idx, shift, nnz, n_atoms, out, flag);
   count_launch();
   return cudaGetLastError();
 }
-cudaError_t launch_ginit(double *G, long long ldm, int n_basic, int ncol, const int *gmap, const double *Sbar,
+cudaError_t launch_untile(const double *src, int rows, long long ncol, double *dst, long long ld, int transpose, cudaStream_t st) {
+  if (ncol <= 0 || rows <= 0) return cudaSuccess;
+  k_untile<<<dim3((unsigned)((ncol + 127) / 128), rows), 128, 0, st>>>(src, rows, ncol, dst, ld, transpose);
+  count_launch();
+  return cudaGetLastError();
+}
+cudaError_t launch_ginit(double *G, int n_cut_rows, int n_basic, int ncol, const int *gmap, const double *Sbar,
                          cudaStream_t st) {
   if (ncol <= 0 || n_basic <= 0) return cudaSuccess;
-  k_ginit<<<dim3((ncol + 255) / 256, n_basic), 256, 0, st>>>(G, ldm, n_basic, ncol, gmap, Sbar);
+  k_ginit<<<dim3((ncol + 255) / 256, n_basic), 256, 0, st>>>(G, n_cut_rows, n_basic, ncol, gmap, Sbar);
   count_launch();
   return cudaGetLastError();
 }
-cudaError_t launch_scopy(double *S, long long ldm, int n_basic, int ncol, const int *gmap, const double *M, cudaStream_t st) {
+cudaError_t launch_scopy(double *S, int n_cut_rows, int n_basic, int ncol, const int *gmap, const double *M, cudaStream_t st) {
   if (ncol <= 0 || n_basic <= 0) return cudaSuccess;
-  k_scopy<<<dim3((ncol + 255) / 256, n_basic), 256, 0, st>>>(S, ldm, n_basic, ncol, gmap, M);
+  k_scopy<<<dim3((ncol + 255) / 256, n_basic), 256, 0, st>>>(S, n_cut_rows, n_basic, ncol, gmap, M);
   count_launch();
   return cudaGetLastError();
 }
@@ -177,13 +193,9 @@ cudaError_t launch_reduce(const double *in, long long n, int stride, int ncomp, 
   count_launch();
   return cudaGetLastError();
 }
-cudaError_t launch_colsum(const double *B, long long n, int nb, double *Bsum, double *scratch, cudaStream_t st) {
+cudaError_t launch_colsum(const double *Bt, long long n, int nb, double *Bsum, cudaStream_t st) {
   if (n <= 0) return cudaSuccess;
-  const int ns = 64;
-  dim3 g((nb + 127) / 128, ns);
-  k_colsum_part<<<g, 128, 0, st>>>(B, n, nb, scratch);
-  count_launch();
-  k_colsum_final<<<(nb + 127) / 128, 128, 0, st>>>(scratch, ns, nb, Bsum);
+  k_colsum<<<(nb + 7) / 8, 256, 0, st>>>(Bt, n, nb, Bsum);
   count_launch();
   return cudaGetLastError();
 }

@@ -3,6 +3,17 @@
 
 namespace mtpb {
 
+// Per-atom arrays of a chunk (M, G, S, dE/dS, B) are tiled: [tile of 128 atoms][row][128].  A thread that owns one
+// atom then finds all rows at a fixed 1 KB stride from one base pointer (immediate offsets in the generated K2
+// kernels), and 16 or 32 consecutive atoms of one row are still one contiguous segment for K1 / K3.
+constexpr int kTile = 128;
+#ifdef __CUDACC__
+__host__ __device__
+#endif
+inline unsigned long long tiled_index(int n_rows, int row, long long col) {
+  return ((unsigned long long)(col >> 7) * (unsigned long long)n_rows + (unsigned long long)row) * 128ull + (unsigned long long)(col & 127);
+}
+
 struct PairArgs {
   const double *pos4;        // [N][4] x, y, z, species (as double)
   const long long *off;      // [N+1]
@@ -10,12 +21,12 @@ struct PairArgs {
                              // else 1 + the index of the image shift in {-1,0,1}^3 order with 0,0,0 moved to the front
   const double *coef;        // [S*S][crow] radial coefficients, block = (z_i*S + z_j), [beta][NMUP]
   const int *kmap;           // [NS][NSLOT] slot -> packed component of the table, or -1
-  double *M;                 // K1 out: [n_basic][ldm], column = atom - c0
-  const double *G;           // K3 in : [n_basic][ldm]
+  double *M;                 // K1 out: tiled [tiles][n_rows][128], column = atom - c0 (kTile)
+  const double *G;           // K3 in : same layout
   double *d4;                // K3 out (gather mode): [nnz][4], or null
   double *F;                 // K3 out (atomic mode): [N][3], or null
   double *wpart;             // K3 out: [gridDim.x][8] virial partials
-  long long ldm;
+  int n_rows;                // rows of M / G (n_basic)
   int c0, c1;                // atom range of this chunk
   int n_species, nb, crow;
   int minimg;

@@ -57,8 +57,12 @@ struct PairLevelImpl {
     return atomic ? pairgrad_p<PS, true>(a, n, st) : pairgrad_p<PS, false>(a, n, st);
   }
   static int pairgrad_grid(int n_atoms, int P) { return P == 1 ? grid_for<1>(n_atoms) : grid_for<PS>(n_atoms); }
+  static constexpr int max2(int a, int b) { return a > b ? a : b; }
   static PairLevel record() {
-    return PairLevel{LEV, NSB, NSC, Sl::NSLOT, PS, &moments, &pairgrad, &pairgrad_grid};
+    constexpr int tile = max2(max2(Tile<LEV, NSB, NSC, 1>::WARP1, Tile<LEV, NSB, NSC, 1>::WARP3),
+                              max2(Tile<LEV, NSB, NSC, PS>::WARP1, Tile<LEV, NSB, NSC, PS>::WARP3));
+    const int fixed = 8 * (kShiftLut + ((Sl::NS * Sl::NSLOT + 3) / 4) * 2 + kWarps * tile);
+    return PairLevel{LEV, NSB, NSC, Sl::NSLOT, PS, fixed, &moments, &pairgrad, &pairgrad_grid};
   }
 };
 

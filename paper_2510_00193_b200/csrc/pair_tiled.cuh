@@ -206,11 +206,11 @@ __global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB1) k_moments_
   }
   if (act && part == 0) {
     const int *km = kmsm + slice * NSLOT;
-    double *Mc = a.M + (atom - a.c0);
+    double *Mc = a.M + tiled_index(a.n_rows, 0, atom - a.c0);
 #pragma unroll
     for (int s = 0; s < NSLOT; ++s) {
       const int k = km[s];
-      if (k >= 0) Mc[(long long)k * a.ldm] = acc[s];
+      if (k >= 0) Mc[k * kTile] = acc[s];
     }
   }
 }
@@ -242,11 +242,11 @@ __global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB3) k_pairgrad
   int n_nb = 0;
   if (act) {
     const int *km = kmsm + slice * NSLOT;
-    const double *Gc = a.G + (atom - a.c0);
+    const double *Gc = a.G + tiled_index(a.n_rows, 0, atom - a.c0);
 #pragma unroll
     for (int s = 0; s < NSLOT; ++s) {
       const int k = km[s];
-      g[s] = k >= 0 ? Gc[(long long)k * a.ldm] : 0.0;
+      g[s] = k >= 0 ? Gc[k * kTile] : 0.0;
     }
     load_pos4(a.pos4, atom, xi, yi, zi, ti);
     beg = a.off[atom];

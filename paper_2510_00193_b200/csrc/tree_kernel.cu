@@ -40,7 +40,7 @@ template <int AL, int AR, int R, bool BWD, bool PS>
 __device__ __forceinline__ void run_pass(const int4 *__restrict__ prog, const int *__restrict__ wave, int n_waves,
                                          int rl, const char *__restrict__ val, char *adj, char *valw,
                                          const double *__restrict__ leaf_seed, Vec<AR> &e,
-                                         double *__restrict__ Gcol, long long ldm, int n_ok, bool g_accum) {
+                                         double *__restrict__ Gcol, int n_ok, bool g_accum) {
   constexpr int BL = kTreePrefetch;            // block: entries between two wave-boundary checks
   constexpr int NB = PS ? 1 : 4;               // blocks in the queue: 4 entries ahead from shared memory, 16 from L2
   constexpr int PF = BL * NB;
@@ -91,7 +91,7 @@ __device__ __forceinline__ void run_pass(const int4 *__restrict__ prog, const in
 #pragma unroll
               for (int r = 0; r < AR; ++r)
                 if (r < n_ok) {
-                  double *gp = Gcol + (long long)d * ldm + r;
+                  double *gp = Gcol + d * kTile + r;
                   *gp = g_accum ? *gp + tot.v[r] : tot.v[r];
                 }
             } else if (t.y & (int)kTreeAcc) {          // piece of a split row: partial sum into a spare val slot
@@ -145,7 +145,7 @@ __global__ void __launch_bounds__(NT) k_tree(const TreeArgs a) {
     for (int k = rl; k < a.n_basic; k += R) {
       Vec<AR> m;
 #pragma unroll
-      for (int r = 0; r < AR; ++r) m.v[r] = r < n_ok ? a.M[(long long)(a.mload_k ? a.mload_k[k] : k) * a.ldm + col + r] : 0.0;
+      for (int r = 0; r < AR; ++r) m.v[r] = r < n_ok ? a.M[tiled_index(a.n_rows, a.mload_k ? a.mload_k[k] : k, col + r)] : 0.0;
       sts<AR>(const_cast<char *>(valc) + (size_t)k * A * 8, m);
     }
     if (a.want_adj)
@@ -160,7 +160,7 @@ __global__ void __launch_bounds__(NT) k_tree(const TreeArgs a) {
       for (int q = rl; q < a.n_cut; q += R) {
         Vec<AR> s;
 #pragma unroll
-        for (int r = 0; r < AR; ++r) s.v[r] = r < n_ok ? a.Sbar[(long long)a.cut_row[q] * a.ldm + col + r] : 0.0;
+        for (int r = 0; r < AR; ++r) s.v[r] = r < n_ok ? a.Sbar[tiled_index(a.n_cut_rows, a.cut_row[q], col + r)] : 0.0;
         sts<AR>(adjc + (size_t)a.cut_aslot[q] * A * 8, s);
       }
     }
@@ -169,7 +169,7 @@ __global__ void __launch_bounds__(NT) k_tree(const TreeArgs a) {
 #pragma unroll
     for (int r = 0; r < AR; ++r) e.v[r] = 0.0;
     run_pass<AL, AR, R, false, PS>(fprog, fw, a.nfw, rl, valc, nullptr, const_cast<char *>(valc), a.leaf_seed, e, nullptr,
-                                   0, n_ok, false);
+                                   n_ok, false);
     // ---- energy (stored basis nodes here, elided leaves were added inside the waves) and basis values
     {
       for (int q = rl; q < a.n_eseed; q += R) {
@@ -180,11 +180,11 @@ __global__ void __launch_bounds__(NT) k_tree(const TreeArgs a) {
       }
 #pragma unroll
       for (int r = 0; r < AR; ++r) esm[(rl * A) + al * AR + r] = e.v[r];
-      if (a.B) {        // B[atom][b]: consecutive threads write consecutive b of one atom
+      if (a.B) {        // tiled Bt[b][column]: consecutive threads write consecutive atoms of one b
         const int na = min(A, a.c1 - (a.c0 + g * A));
         for (int i = threadIdx.x; i < na * a.n_basis; i += NT) {
-          const int at = i / a.n_basis, b = i - at * a.n_basis;
-          a.B[(long long)(a.c0 + g * A + at) * a.n_basis + b] = val[a.basis_slot[b] * A + at];
+          const int b = i / na, at = i - b * na;
+          a.B[tiled_index(a.n_basis, b, g * A + at)] = val[a.basis_slot[b] * A + at];
         }
       }
       __syncthreads();
@@ -193,7 +193,7 @@ __global__ void __launch_bounds__(NT) k_tree(const TreeArgs a) {
           const Vec<AR> v = lds<AR>(valc + (size_t)a.cut_vslot[q] * A * 8);
 #pragma unroll
           for (int r = 0; r < AR; ++r)
-            if (r < n_ok) a.S[(long long)a.cut_row[q] * a.ldm + col + r] = v.v[r];
+            if (r < n_ok) a.S[tiled_index(a.n_cut_rows, a.cut_row[q], col + r)] = v.v[r];
         }
       if (rl == 0 && a.write_energy) {           // fixed-order reduction over the R row-lanes
 #pragma unroll
@@ -208,18 +208,18 @@ __global__ void __launch_bounds__(NT) k_tree(const TreeArgs a) {
       }
     }
     if (!a.want_adj) continue;
-    double *Gcol = a.G + col;
+    double *Gcol = a.G + tiled_index(a.n_rows, 0, col);     // a lane's AR atoms are consecutive columns of one tile
     for (int q = rl; q < a.n_gzero; q += R)
 #pragma unroll
       for (int r = 0; r < AR; ++r)
-        if (r < n_ok) Gcol[(long long)a.gzero_k[q] * a.ldm + r] = 0.0;
-    run_pass<AL, AR, R, true, PS>(bprog, bw, a.nbw, rl, valc, adjc, const_cast<char *>(valc), nullptr, e, Gcol, a.ldm, n_ok, a.g_accum != 0);
+        if (r < n_ok) Gcol[a.gzero_k[q] * kTile + r] = 0.0;
+    run_pass<AL, AR, R, true, PS>(bprog, bw, a.nbw, rl, valc, adjc, const_cast<char *>(valc), nullptr, e, Gcol, n_ok, a.g_accum != 0);
     __syncthreads();
     // packed moments that are basis functions themselves (M_{mu,0}): G += xi
     for (int q = rl; q < a.n_gseed; q += R)
 #pragma unroll
       for (int r = 0; r < AR; ++r)
-        if (r < n_ok) Gcol[(long long)a.gseed_k[q] * a.ldm + r] += a.gseed_val[q];
+        if (r < n_ok) Gcol[a.gseed_k[q] * kTile + r] += a.gseed_val[q];
   }
 }
 

@@ -10,7 +10,6 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
-    config.addinivalue_line("markers", "codegen: runs with the NVRTC-specialised contraction kernel enabled")
 
 
 @pytest.fixture(scope="session")
@@ -18,13 +17,3 @@ def lib():
     """The C-ABI binding; GPU tests fail loudly if the extension is missing."""
     import paper_2510_00193_b200 as m
     return m
-
-
-@pytest.fixture(autouse=True)
-def _codegen_off_unless_asked(request, monkeypatch):
-    """NVRTC specialisation of the contraction kernel costs seconds per potential: GPU tests run the interpreted
-    kernel (bit-identical by construction and by test) unless they are marked `codegen`."""
-    if request.node.get_closest_marker("codegen") is None:
-        monkeypatch.setenv("MTP_TREE_CODEGEN", "0")
-    else:
-        monkeypatch.delenv("MTP_TREE_CODEGEN", raising=False)

@@ -21,10 +21,25 @@ def torch():
     return t
 
 
-def run_gpu(lib, torch, w, pot=None, opts=None):
+def assert_specialised(lib, pot):
+    """The contraction kernels that ran are the NVRTC-specialised ones (the product path), not the interpreter:
+    two kernels (energy + adjoint, values) per program, and the handle reports no fallback."""
+    n_prog = pot.get_option(lib.INFO_TREE_PROGRAMS)
+    assert n_prog >= 1 and pot.get_option(lib.INFO_TREE_KERNELS) == 2 * n_prog, pot.last_error()
+    assert pot.get_option(lib.OPT_TREE_CODEGEN) == 1
+    return n_prog
+
+
+def run_gpu(lib, torch, w, pot=None, opts=None, interp=False):
+    """One mtp_compute through the C ABI.  interp: the table interpreter instead of the specialised kernels."""
     pot = gpu_pot(lib, w) if pot is None else pot
     for k, v in (opts or {}).items():
         pot.set_option(k, v)
+    if interp:
+        pot.set_option(lib.OPT_TREE_CODEGEN, 0)
+        assert pot.get_option(lib.OPT_TREE_CODEGEN) == 0
+    else:
+        assert_specialised(lib, pot)
     d = to_dev(w, torch)
     out = pot.compute(d["pos"], d["types"], w.box, d["off"], d["idx"], d["shift"], d["rev"])
     torch.cuda.synchronize()
@@ -55,6 +70,9 @@ def test_energy_force_virial_parity(lib, torch, ci, cells):
             got, pot, _ = run_gpu(lib, torch, w, opts={lib.OPT_VARIANT: variant, lib.OPT_FORCE_MODE: mode})
             check(w, ref, got, opot)
             pot.close()
+    got, pot, _ = run_gpu(lib, torch, w, interp=True)          # the fallback form of K2 against the oracle as well
+    check(w, ref, got, opot)
+    pot.close()
 
 
 def test_chunked_equals_unchunked_and_gather_is_deterministic(lib, torch):
@@ -91,6 +109,11 @@ def test_ragged_cluster_with_skin_and_short_pairs(lib, torch, lev, n_mu, n):
     opot = oracle_pot(w)
     ref = omtp.evaluate(opot, w.pos, w.types, w.box, w.off, w.idx, w.shift)
     got, pot, _ = run_gpu(lib, torch, w)
+    if lev >= 20:
+        assert pot.get_option(lib.INFO_TREE_PROGRAMS) > 1          # partitioned: top program + group programs
+    check(w, ref, got, opot)
+    pot.close()
+    got, pot, _ = run_gpu(lib, torch, w, interp=True)
     check(w, ref, got, opot)
     pot.close()
 
@@ -197,25 +220,20 @@ def test_cuda_graph_replay_of_a_call_is_bit_identical(lib, torch):
     pot.close()
 
 
-@pytest.mark.codegen
-@pytest.mark.parametrize("form", ["line", "shared"])
-def test_specialised_tree_kernel_is_bit_identical_to_the_interpreter(lib, torch, form, monkeypatch):
-    """MTP_OPT_TREE_CODEGEN: the NVRTC-specialised K2 keeps the interpreter's arithmetic order, in both forms of
-    the generated code (straight-line, and MTP_TREE_FORM=shared: one body per row shape + operand tables)."""
-    monkeypatch.setenv("MTP_TREE_FORM", form)
-    w = make_workload(3, n_basis_of(16), cells=18)            # 23 328 atoms: the AL = 32, AR = 2 shape
-    a, pot, d = run_gpu(lib, torch, w, opts={lib.OPT_TREE_CODEGEN: 0, lib.OPT_VARIANT: lib.VARIANT_THREAD})
-    assert pot.get_option(lib.INFO_TREE_KERNELS) == 0
+def test_specialised_and_interpreted_tree_kernels_agree(lib, torch):
+    """MTP_OPT_TREE_CODEGEN: the two forms of K2 sum in different orders, so they agree to rounding (relative to the
+    magnitude of the summed terms), not bit for bit; each is compared with the oracle elsewhere."""
+    w = make_workload(3, n_basis_of(16), cells=18)            # 23 328 atoms, 3 species, level 16
+    a, pot, d = run_gpu(lib, torch, w, opts={lib.OPT_VARIANT: lib.VARIANT_THREAD}, interp=True)
     pot.close()
-    b, pot, _ = run_gpu(lib, torch, w, opts={lib.OPT_TREE_CODEGEN: 1, lib.OPT_VARIANT: lib.VARIANT_THREAD})
-    used = pot.get_option(lib.INFO_TREE_KERNELS)
+    b, pot, _ = run_gpu(lib, torch, w, opts={lib.OPT_VARIANT: lib.VARIANT_THREAD})
     pot.close()
-    for k in ("Ei", "F", "virial", "E"):
-        assert np.array_equal(a[k], b[k]), k
-    print("specialised tree kernels in use:", used)
+    sE = np.maximum(1.0, np.abs(a["Ei"]))
+    assert np.all(np.abs(a["Ei"] - b["Ei"]) <= 1e-12 * sE.max())
+    assert np.all(np.abs(a["F"] - b["F"]) <= 1e-11 * np.abs(a["F"]).max())
+    assert np.allclose(a["virial"], b["virial"], rtol=0, atol=1e-11 * np.abs(a["virial"]).max())
 
 
-@pytest.mark.codegen
 def test_large_launch_configuration_on_sampled_atoms(lib, torch):
     """The launch configuration bench.py times (config 4 structure, thread-parallel pair kernels, 64-atom
     tree CTAs, specialised K2, several chunks): E_i, F_k on sampled atoms against the oracle, sum F = 0."""
@@ -261,7 +279,6 @@ def _check_sampled(w, got, n_sample, seed):
     assert np.all(np.abs(got["F"].sum(axis=0)) <= 1e-9 * np.abs(got["F"]).sum())
 
 
-@pytest.mark.codegen
 def test_full_size_config4_sampled(lib, torch):
     """BASELINE.json configs[3] at full size (1,048,576 atoms, level 16), default options = what bench.py times."""
     w = make_workload(3, n_basis_of(16))
@@ -271,7 +288,6 @@ def test_full_size_config4_sampled(lib, torch):
     _check_sampled(w, got, 4, 11)
 
 
-@pytest.mark.codegen
 def test_full_size_config3_sampled(lib, torch):
     """BASELINE.json configs[2] at full size (54,000 atoms, 2 species, level 20)."""
     w = make_workload(2, n_basis_of(20))
@@ -281,7 +297,6 @@ def test_full_size_config3_sampled(lib, torch):
     _check_sampled(w, got, 2, 12)
 
 
-@pytest.mark.codegen
 def test_full_size_config5_sampled_energy_and_grades(lib, torch):
     """BASELINE.json configs[4] at full size (250,000 atoms, level 24): E_i, B and both grade modes on sampled atoms."""
     nb = n_basis_of(24)
