@@ -171,8 +171,8 @@ int mtp_debug_moments(mtp_handle *h, int64_t n_atoms, const double *d_pos,
 int mtp_profile_read(mtp_handle *h, double *ms /*[5]*/, int64_t *launches /*[5]*/);
 /* Host-only (no device needed): how mtp_create will evaluate the contraction table of *p with the specialised
  * kernels (only the table fields are read).  out[8] = { partitioned (0/1), threads (= atoms) per SM of the slowest
- * program, cut rows, groups, ops of the top program, ops summed over the group programs, ops below the cut, same as
- * out[1] }. */
+ * program, cut rows, groups, ops of the top program, ops summed over the group programs, ops below the cut,
+ * specialised (0: more than 120 000 ops after partitioning -- such a table is interpreted) }. */
 int mtp_table_plan(const mtp_params *p, int64_t *out);
 /* Host-only: the register program of the whole table (kind 0: energy + adjoint, 1: basis values) as data, so that a
  * test can emulate it: prog[cap][7] int32 = op, d, a, b, c, k, x (csrc/tree_codegen.h K2Op), consts[ccap] doubles,

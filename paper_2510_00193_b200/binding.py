@@ -127,7 +127,7 @@ class Table:
         rc = _lib.mtp_table_plan(C.byref(p), out)
         if rc != OK:
             raise MtpError(rc, "mtp_table_plan")
-        keys = ["partitioned", "threads_per_sm", "cut_rows", "groups", "top_ops", "group_ops", "ops_below_cut", "_"]
+        keys = ["partitioned", "threads_per_sm", "cut_rows", "groups", "top_ops", "group_ops", "ops_below_cut", "specialised"]
         return dict(zip(keys, [int(x) for x in out]))
 
     def k2_program(self, xi, kind=0):

@@ -9,6 +9,8 @@
 #include <cstdlib>
 #include <cstring>
 #include <map>
+#include <memory>
+#include <mutex>
 #include <string>
 #include <thread>
 #include <tuple>
@@ -362,7 +364,7 @@ K2Table group_table(const TreeGroup &g) {
 }
 
 // 0 or a negative code; err receives a message
-int plan_jit(const K2Table &whole, JitPlan &best, std::string *err) {
+int plan_jit(const K2Table &whole, JitPlan &best, std::string *err, bool *too_large = nullptr) {
   K2Gen g;
   int rc = k2_generate(whole, K2_EF, kK2Window, kK2Lookahead, g, err);
   if (rc != MTP_OK) return rc;
@@ -374,8 +376,9 @@ int plan_jit(const K2Table &whole, JitPlan &best, std::string *err) {
     return MTP_OK;
   }
   bool have = false;
-  static const int budgets[] = {430, 600, 870, 1300, 2000};
+  static const int budgets[] = {430, 600, 870};
   for (int budget : budgets) {
+    if (getenv("XBUDGET") && atoi(getenv("XBUDGET")) != budget) continue;
     JitPlan p;
     if (!tree_partition(whole.n_basic, whole.n_nodes, whole.n_prod(), whole.prod.data(), (int)whole.basis_node.size(),
                         whole.basis_node.data(), budget, p.part)) continue;
@@ -405,11 +408,36 @@ int plan_jit(const K2Table &whole, JitPlan &best, std::string *err) {
   if (!have) { *err = "contraction table: no partition fits the specialised kernels"; return MTP_EUNSUP; }
   long long ops = 0;
   for (auto &t : best.tables) ops += t.n_prod();
-  if (ops > kK2MaxOps) {                 // level 28: 350 000 ops in 130 programs -- minutes of NVRTC time
+  if (too_large) *too_large = ops > kK2MaxOps;
+  if (ops > kK2MaxOps && !too_large) {   // level 28: 350 000 ops in 130 programs -- minutes of NVRTC time
     *err = "contraction table too large to specialise (" + std::to_string(ops) + " ops after partitioning): interpreted";
     return MTP_EUNSUP;
   }
   return MTP_OK;
+}
+}  // namespace
+
+// Compiled kernels are kept for the life of the process, keyed by what the program text depends on (the table and
+// its role, not the weights): a second potential with the same table costs no NVRTC time.
+namespace {
+struct CubinCache {
+  std::mutex mu;
+  std::map<std::pair<uint64_t, uint64_t>, std::shared_ptr<const std::vector<char>>> map;
+};
+CubinCache &cubin_cache() { static CubinCache c; return c; }
+std::pair<uint64_t, uint64_t> program_key(const K2Table &t, int kind, int window, int lookahead) {
+  uint64_t h1 = 1469598103934665603ull, h2 = 0x9e3779b97f4a7c15ull;
+  auto mix = [&](int64_t v) {
+    h1 = (h1 ^ (uint64_t)v) * 1099511628211ull;
+    h2 = (h2 + (uint64_t)v) * 0xff51afd7ed558ccdull; h2 ^= h2 >> 33;
+  };
+  mix(kind); mix(window); mix(lookahead); mix(t.n_basic); mix(t.n_nodes);
+  mix((int64_t)t.prod.size()); for (int32_t v : t.prod) mix(v);
+  mix((int64_t)t.in_row.size()); for (int32_t v : t.in_row) mix(v);
+  mix((int64_t)t.basis_node.size()); for (int32_t v : t.basis_node) mix(v);
+  mix((int64_t)t.cut_node.size()); for (int32_t v : t.cut_node) mix(v);
+  for (int32_t v : t.cut_row) mix(v);
+  return {h1, h2};
 }
 }  // namespace
 
@@ -431,18 +459,30 @@ static int ensure_jit(mtp_handle *h) {
     rc = upload_gmap(h, plan.part);
     if (rc != MTP_OK) { h->jit_note = h->err; return rc; }
   }
-  struct Job { mtp_handle::JProg *jp; int kind; std::vector<char> cubin; std::string why; int rc = 0; };
+  struct Job { mtp_handle::JProg *jp; int kind; std::shared_ptr<const std::vector<char>> cubin; std::string why; int rc = 0; };
   std::vector<Job> jobs;
   for (auto &jp : h->jprogs)
-    for (int k = 0; k < 2; ++k) jobs.push_back(Job{&jp, k, {}, "", 0});
+    for (int k = 0; k < 2; ++k) jobs.push_back(Job{&jp, k, nullptr, "", 0});
   std::atomic<size_t> next{0};
+  const int window = getenv("XW") ? atoi(getenv("XW")) : kK2Window, lookahead = getenv("XD") ? atoi(getenv("XD")) : kK2Lookahead;
   auto work = [&]() {
     for (size_t i = next.fetch_add(1); i < jobs.size(); i = next.fetch_add(1)) {
       Job &j = jobs[i];
-      j.rc = k2_generate(j.jp->table, (K2Kind)j.kind, kK2Window, kK2Lookahead, j.jp->gen[j.kind], &j.why);
+      j.rc = k2_generate(j.jp->table, (K2Kind)j.kind, window, lookahead, j.jp->gen[j.kind], &j.why);
       if (j.rc != MTP_OK) continue;
-      j.cubin = k2_jit_compile(j.jp->gen[j.kind], &j.why);
-      if (j.cubin.empty()) j.rc = MTP_ECUDA;
+      const auto key = program_key(j.jp->table, j.kind, window, lookahead);
+      {
+        std::lock_guard<std::mutex> lk(cubin_cache().mu);
+        auto it = cubin_cache().map.find(key);
+        if (it != cubin_cache().map.end()) j.cubin = it->second;
+      }
+      if (!j.cubin) {
+        auto bin = std::make_shared<std::vector<char>>(k2_jit_compile(j.jp->gen[j.kind], &j.why));
+        if (bin->empty()) { j.rc = MTP_ECUDA; continue; }
+        std::lock_guard<std::mutex> lk(cubin_cache().mu);
+        cubin_cache().map[key] = bin;
+        j.cubin = bin;
+      }
       j.jp->gen[j.kind].body.clear(); j.jp->gen[j.kind].body.shrink_to_fit();      // the source is not needed any more
     }
   };
@@ -452,7 +492,7 @@ static int ensure_jit(mtp_handle *h) {
   for (auto &w : workers) w.join();
   for (auto &j : jobs) {
     if (j.rc == MTP_OK) {
-      j.jp->kern[j.kind] = k2_jit_load(j.cubin, j.jp->gen[j.kind].n_slots, &j.why);
+      j.jp->kern[j.kind] = k2_jit_load(*j.cubin, j.jp->gen[j.kind].n_slots, j.jp->gen[j.kind].consts, &j.why);
       if (!j.jp->kern[j.kind]) j.rc = MTP_ECUDA;
     }
     if (j.rc != MTP_OK) {
@@ -479,10 +519,12 @@ extern "C" int mtp_table_plan(const mtp_params *p, int64_t *out) {
   whole.xi.assign((size_t)p->n_basis, 1.0);            // the plan does not depend on the weights (all taken non-zero)
   JitPlan plan;
   std::string err;
-  int rc = plan_jit(whole, plan, &err);
+  bool too_large = false;
+  int rc = plan_jit(whole, plan, &err, &too_large);
   if (rc != MTP_OK) return rc;
   out[0] = plan.partitioned ? 1 : 0;
   out[1] = plan.min_threads;
+  out[7] = too_large ? 0 : 1;
   if (!plan.partitioned) return MTP_OK;
   out[2] = (int64_t)plan.part.cut_node.size(); out[3] = (int64_t)plan.part.groups.size(); out[4] = plan.part.top.n_prod();
   std::vector<char> seen(plan.part.cut_node.size(), 0);
@@ -492,7 +534,6 @@ extern "C" int mtp_table_plan(const mtp_params *p, int64_t *out) {
   }
   for (size_t r = 0; r < seen.size(); ++r) if (!seen[r] && plan.part.cut_node[r] >= p->n_basic) return MTP_EINVAL;
   out[6] = (int64_t)p->n_prod - plan.part.top.n_prod();
-  out[7] = plan.min_threads;
   return MTP_OK;
 }
 

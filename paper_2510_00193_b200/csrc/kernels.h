@@ -59,13 +59,14 @@ struct K2Args {
   double *Ei;              // [N]
   const double *xi0; const double *pos4;
   int n_io, n_cut, n_bt, c0, n;
+  const double *cmx;       // constants beyond the kernel's constant bank (set by k2_jit_launch)
 };
 struct K2Kernel;
 bool k2_jit_available(std::string *why);
 void k2_shape(int n_slots, int *threads, int *ctas_per_sm);   // threads = 0: does not fit
 std::string k2_source(const K2Gen &g);
 std::vector<char> k2_jit_compile(const K2Gen &g, std::string *why);   // host only, thread-safe
-K2Kernel *k2_jit_load(const std::vector<char> &cubin, int n_slots, std::string *why);
+K2Kernel *k2_jit_load(const std::vector<char> &cubin, int n_slots, const std::vector<double> &consts, std::string *why);
 cudaError_t k2_jit_launch(const K2Kernel *k, const K2Args &a, cudaStream_t st);
 void k2_jit_destroy(K2Kernel *k);
 

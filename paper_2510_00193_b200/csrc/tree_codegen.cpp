@@ -55,7 +55,7 @@ struct Builder {
   const int N, nb;
   const bool group;
   std::vector<VInst> v;
-  std::vector<double> consts;
+  std::vector<std::pair<int, int>> const_desc;
   std::map<uint64_t, int> cidx;
   int n_values;                            // VAL(n) = n, ADJ(n) = N + n, temporaries from 2N
   std::vector<Row> rows;
@@ -70,13 +70,14 @@ struct Builder {
   int ADJ(int n) const { return N + n; }
   int temp() { return n_values++; }
   int in_row(int k) const { return t.in_row.empty() ? k : t.in_row[k]; }
-  int konst(double x) {
-    uint64_t bits;
-    std::memcpy(&bits, &x, 8);
-    auto it = cidx.find(bits);
+  // constants are kept symbolically, mult * seed(node) (node = -1: the number mult itself), so that the program
+  // text does not depend on the weights xi: one compiled kernel serves every potential with this table
+  int konst(int node, int mult) {
+    const uint64_t key = ((uint64_t)(uint32_t)(node + 1) << 32) | (uint32_t)mult;
+    auto it = cidx.find(key);
     if (it != cidx.end()) return it->second;
-    consts.push_back(x);
-    return cidx[bits] = (int)consts.size() - 1;
+    const_desc.push_back({node, mult});
+    return cidx[key] = (int)const_desc.size() - 1;
   }
   void emit(int op, int d, int a = -1, int b = -1, int c = -1, int k = -1, int x = -1) { v.push_back(VInst{op, d, a, b, c, k, x}); }
 
@@ -106,7 +107,7 @@ struct Builder {
   void classify() {
     seed.assign(N, 0.0); seeded.assign(N, 0); is_cut.assign(N, 0); is_basis.assign(N, 0); cut_row_of.assign(N, -1);
     for (size_t a = 0; a < t.basis_node.size(); ++a) { seed[t.basis_node[a]] += t.xi[a]; is_basis[t.basis_node[a]] = 1; }
-    for (int n = 0; n < N; ++n) seeded[n] = is_basis[n] && seed[n] != 0.0;
+    for (int n = 0; n < N; ++n) seeded[n] = is_basis[n];              // whatever the value of its weight: see konst()
     for (size_t q = 0; q < t.cut_node.size(); ++q) { is_cut[t.cut_node[q]] = 1; cut_row_of[t.cut_node[q]] = t.cut_row[q]; }
     // a node is needed when it can reach an output: E_i (seeded), an exported basis value, or a cut node
     needed.assign(N, 0); read_needed.assign(N, 0);
@@ -143,14 +144,14 @@ struct Builder {
         else emit(P_FMA, acc, VAL(ab.first), VAL(ab.second), acc);
         first = false;
       }
-      if (energy_leaf) { emit(P_ENERGY, -1, acc, -1, -1, konst(seed[d] * m)); any_energy = true; }
+      if (energy_leaf) { emit(P_ENERGY, -1, acc, -1, -1, konst(d, m)); any_energy = true; }
       else if (direct) have = true;
-      else if (!have) { emit(P_MULK, VAL(d), acc, -1, -1, konst((double)m)); have = true; }
+      else if (!have) { emit(P_MULK, VAL(d), acc, -1, -1, konst(-1, m)); have = true; }
       else if (m == 1) emit(P_ADD, VAL(d), acc, -1, VAL(d));
-      else emit(P_FMAK, VAL(d), acc, -1, VAL(d), konst((double)m));
+      else emit(P_FMAK, VAL(d), acc, -1, VAL(d), konst(-1, m));
     }
     if (energy_leaf) return;
-    if (kind == K2_EF && !group && seeded[d]) { emit(P_ENERGY, -1, VAL(d), -1, -1, konst(seed[d])); any_energy = true; }
+    if (kind == K2_EF && !group && seeded[d]) { emit(P_ENERGY, -1, VAL(d), -1, -1, konst(d, 1)); any_energy = true; }
     if (kind == K2_VALUES) {
       if (group && is_cut[d]) emit(P_STS_OUT, -1, VAL(d), -1, -1, -1, cut_row_of[d]);
       if (!group && is_basis[d])
@@ -166,7 +167,7 @@ struct Builder {
       bool have = true;
       if (x < nb && group) emit(P_LDOUT, ax, -1, -1, -1, -1, in_row(x));          // running sum over the groups
       else if (is_cut[x]) emit(P_LDSEED, ax, -1, -1, -1, -1, cut_row_of[x]);
-      else if (!group && seeded[x]) emit(P_CONST, ax, -1, -1, -1, konst(seed[x]));
+      else if (!group && seeded[x]) emit(P_CONST, ax, -1, -1, -1, konst(x, 1));
       else have = false;
       if (!have) {
         if (sv >= 0) emit(P_MUL, ax, sv, VAL(other));
@@ -195,9 +196,9 @@ struct Builder {
     for (auto &g : row.groups) {
       const int m = g.first;
       int sv = -1, sk = -1;
-      if (leaf) sk = konst(seed[d] * m);
+      if (leaf) sk = konst(d, m);
       else if (m == 1) sv = ADJ(d);
-      else { sv = temp(); emit(P_MULK, sv, ADJ(d), -1, -1, konst((double)m)); }
+      else { sv = temp(); emit(P_MULK, sv, ADJ(d), -1, -1, konst(-1, m)); }
       for (auto &ab : g.second) {
         contribute(ab.first, ab.second, sv, sk, ready);
         contribute(ab.second, ab.first, sv, sk, ready);
@@ -210,7 +211,7 @@ struct Builder {
     classify();
     // packed inputs that are outputs themselves
     for (int k = 0; k < nb; ++k) {
-      if (kind == K2_EF && !group && seeded[k]) { emit(P_ENERGY, -1, VAL(k), -1, -1, konst(seed[k])); any_energy = true; }
+      if (kind == K2_EF && !group && seeded[k]) { emit(P_ENERGY, -1, VAL(k), -1, -1, konst(k, 1)); any_energy = true; }
       if (kind == K2_VALUES && !group && is_basis[k])
         for (size_t a = 0; a < t.basis_node.size(); ++a) if (t.basis_node[a] == k) emit(P_STB, -1, VAL(k), -1, -1, -1, (int)a);
     }
@@ -231,7 +232,7 @@ struct Builder {
       for (int k = 0; k < nb; ++k)
         if (!adj_init[k]) {                // a packed input no needed row reads: its adjoint is its own seed
           const int tv = temp();
-          emit(P_CONST, tv, -1, -1, -1, konst(seeded[k] ? seed[k] : 0.0));
+          emit(P_CONST, tv, -1, -1, -1, (seeded[k] ? konst(k, 1) : konst(-1, 0)));
           emit(P_STOUT, -1, tv, -1, -1, -1, in_row(k));
         }
   }
@@ -392,24 +393,29 @@ struct Allocator {
 
 void emit_source(const Builder &B, K2Gen &g) {
   // multipliers and seeds: operands from the constant bank while it has room (8 KB, what its cache holds), else literals
-  constexpr size_t kMaxConst = 1024;
+  constexpr size_t kMaxConst = (size_t)kK2ConstBank;
   std::string &s = g.source;
   s.clear();
   s.reserve(g.prog.size() * 20 + 4096);
   char buf[160];
   auto K = [&](int k) {
     char t[48];
-    if ((size_t)k < kMaxConst) snprintf(t, sizeof t, "cm[%d]", k);
-    else snprintf(t, sizeof t, "%a", g.consts[k]);
+    // the multinomial multipliers 2, 3, 6, ... are immediate operands of DFMA / DMUL (their low word is zero); what
+    // depends on the weights comes from the constant bank, filled when the kernel is loaded (K2Gen::consts), and
+    // beyond its size from a table in global memory
+    if (g.const_node[k] < 0) snprintf(t, sizeof t, "%d.0", g.const_mult[k]);
+    else if ((size_t)k < kMaxConst) snprintf(t, sizeof t, "cm[%d]", k);
+    else snprintf(t, sizeof t, "__ldg(a.cmx+%d)", k);
     return std::string(t);
   };
-  if (!g.consts.empty()) {
-    s += "__constant__ double cm[] = {";
-    for (size_t k = 0; k < g.consts.size() && k < kMaxConst; ++k) { snprintf(buf, sizeof buf, "%a,", g.consts[k]); s += buf; }
-    s += "0.0};\n";
-  }
+  snprintf(buf, sizeof buf, "__constant__ double cm[%zu];\n", std::min(kMaxConst, std::max<size_t>(g.const_node.size(), 1)));
+  s += buf;
   snprintf(buf, sizeof buf, "#define K2_SLOTS %d\n#define K2_ENERGY %d\n", g.n_slots, g.writes_energy ? 1 : 0);
   s += buf;
+  // what the CTA asks L2 for when it starts: the whole input block of its tile for a whole table or top program
+  // (one bulk prefetch: config 4 tree time 0.68 -> 0.62 ms); nothing for a group program, which reads a subset of the
+  // rows -- a prefetch per row was measured and costs more than it hides (level 24: tree 17.0 -> 19.0 ms)
+  s += B.t.in_row.empty() ? "#define K2_PREFETCH PFALL();\n" : "#define K2_PREFETCH\n";
   std::string &b = g.body;
   b.clear();
   b.reserve(g.prog.size() * 20 + 4096);
@@ -443,6 +449,14 @@ void emit_source(const Builder &B, K2Gen &g) {
 
 }  // namespace
 
+void k2_constants(const K2Table &t, K2Gen &g) {
+  std::vector<double> seed(t.n_nodes, 0.0);
+  for (size_t a = 0; a < t.basis_node.size(); ++a) seed[t.basis_node[a]] += t.xi[a];
+  g.consts.resize(g.const_node.size());
+  for (size_t k = 0; k < g.const_node.size(); ++k)
+    g.consts[k] = g.const_node[k] < 0 ? (double)g.const_mult[k] : (double)g.const_mult[k] * seed[g.const_node[k]];
+}
+
 int k2_generate(const K2Table &t, K2Kind kind, int window, int lookahead, K2Gen &out, std::string *err) {
   out = K2Gen();
   const char *verr = "";
@@ -456,7 +470,9 @@ int k2_generate(const K2Table &t, K2Kind kind, int window, int lookahead, K2Gen 
   b.build();
   out.writes_energy = b.any_energy || (kind == K2_EF && !t.is_group());
   Allocator a(b, window, lookahead, out);
-  out.consts = b.consts;
+  out.const_node.clear(); out.const_mult.clear();
+  for (auto &cd : b.const_desc) { out.const_node.push_back(cd.first); out.const_mult.push_back(cd.second); }
+  k2_constants(t, out);
   rc = a.run(err);
   if (rc != MTP_OK) return rc;
   emit_source(b, out);

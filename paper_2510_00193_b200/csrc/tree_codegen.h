@@ -62,7 +62,8 @@ struct K2Inst { int32_t op, d, a, b, c, k, x; };
 
 struct K2Gen {
   std::vector<K2Inst> prog;
-  std::vector<double> consts;
+  std::vector<double> consts;             // values of the constants for this table's weights xi
+  std::vector<int32_t> const_node, const_mult;   // what they are: mult * (sum of xi on node), node = -1: the number mult
   int n_regs = 0;        // window size W
   int n_slots = 0;       // shared-memory slots per thread
   bool writes_energy = false;
@@ -79,9 +80,13 @@ int k2_validate(int n_basic, int n_nodes, int n_prod, const int32_t *prod, int n
 // reloaded.  Returns 0 or a negative MTP_E* code.
 int k2_generate(const K2Table &t, K2Kind kind, int window, int lookahead, K2Gen &out, std::string *err);
 
+// (re)computes g.consts from the table's weights: the program itself does not depend on them
+void k2_constants(const K2Table &t, K2Gen &g);
+
+constexpr int kK2ConstBank = 4096;      // doubles of the kernel's constant bank; further constants come from global memory
 constexpr int kK2Threads = 128;         // shared-memory column stride (threads per CTA the slots are laid out for)
-constexpr int kK2Window = 100;
-constexpr int kK2Lookahead = 6;
+constexpr int kK2Window = 108;          // measured at config 4: 100 / 108 doubles -> tree 0.62 / 0.60 ms per step (255 registers, no spills)
+constexpr int kK2Lookahead = 2;
 constexpr int kK2SlotsTwoCtas = 110;    // <= this many slots: two 128-thread CTAs per SM; up to kK2SlotsMax: one
 constexpr int kK2SlotsMax = 226;
 constexpr long long kK2MaxOps = 120000;  // table ops (after partitioning) above which a table is interpreted, not specialised

@@ -12,6 +12,7 @@
 #include <cuda_runtime.h>
 #include <dlfcn.h>
 
+#include <algorithm>
 #include <cstdint>
 #include <cstdio>
 #include <cstdlib>
@@ -69,6 +70,7 @@ struct K2Args {
   const double *in; double *out; const double *sbar; double *sout; double *bt; double *Ei;
   const double *xi0; const double *pos4;
   int n_io, n_cut, n_bt, c0, n;
+  const double *cmx;
 };
 @PRE@
 #define T @T@
@@ -78,6 +80,7 @@ template <int OFF> __device__ __forceinline__ double ldgl(const double *p) { dou
 template <int OFF> __device__ __forceinline__ void stgl(double *p, double v) { asm volatile("st.global.f64 [%0+%1], %2;" :: "l"(p), "n"(OFF), "d"(v)); }
 template <int OFF> __device__ __forceinline__ double lds(unsigned a) { double v; asm volatile("ld.shared.f64 %0, [%1+%2];" : "=d"(v) : "r"(a), "n"(OFF)); return v; }
 template <int OFF> __device__ __forceinline__ void sts(unsigned a, double v) { asm volatile("st.shared.f64 [%0+%1], %2;" :: "r"(a), "n"(OFF), "d"(v)); }
+#define PFALL() asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(IN), "r"(a.n_io * 1024) : "memory")
 #define LI(x) ldnc<(x) * 1024>(IN)
 #define LR(x) ldvol<(x) * 1024>(IN)
 #define LB(x) ldnc<(x) * 1024>(SBAR)
@@ -98,6 +101,10 @@ extern "C" __global__ void __launch_bounds__(T, @MINB@) k2(const K2Args a) {
   const double *SBAR = a.sbar + tile * a.n_cut + lane; (void)SBAR;
   double *SOUT = a.sout + tile * a.n_cut + lane; (void)SOUT;
   double *BT = a.bt + tile * a.n_bt + lane; (void)BT;
+  // Whoever starts a tile asks L2 for what the tile's threads will read row by row over their whole run
+  // (K2_PREFETCH: one bulk prefetch of the input block): without it every first touch of a row pays the HBM
+  // latency with only 8 warps per SM to hide it
+  if (lane == 0) { K2_PREFETCH }
   double e = 0.0; (void)e;
 @BODY@
 #if K2_ENERGY
@@ -174,16 +181,18 @@ struct K2Kernel {
   cudaKernel_t kernel = nullptr;
   int threads = 128;
   size_t smem = 0;
+  double *cmx = nullptr;        // constants beyond the constant bank
 };
 
 void k2_jit_destroy(K2Kernel *k) {
   if (!k) return;
   if (k->lib) cudaLibraryUnload(k->lib);
+  if (k->cmx) cudaFree(k->cmx);
   delete k;
 }
 
 // Device half: load a compiled program.
-K2Kernel *k2_jit_load(const std::vector<char> &cubin, int n_slots, std::string *why) {
+K2Kernel *k2_jit_load(const std::vector<char> &cubin, int n_slots, const std::vector<double> &consts, std::string *why) {
   if (cubin.empty()) return nullptr;
   K2Kernel *k = new K2Kernel();
   int minb = 1;
@@ -193,6 +202,18 @@ K2Kernel *k2_jit_load(const std::vector<char> &cubin, int n_slots, std::string *
   if (e == cudaSuccess) e = cudaLibraryGetKernel(&k->kernel, k->lib, "k2");
   if (e == cudaSuccess && k->smem > 48 * 1024)
     e = cudaFuncSetAttribute((const void *)k->kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k->smem);
+  if (e == cudaSuccess && !consts.empty()) {           // the weights-dependent constants: bank first, overflow in global memory
+    void *cm = nullptr;
+    size_t bytes = 0;
+    e = cudaLibraryGetGlobal(&cm, &bytes, k->lib, "cm");
+    const size_t nbank = std::min(consts.size(), (size_t)kK2ConstBank);
+    if (e == cudaSuccess && bytes < nbank * 8) e = cudaErrorInvalidValue;
+    if (e == cudaSuccess) e = cudaMemcpy(cm, consts.data(), nbank * 8, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && consts.size() > (size_t)kK2ConstBank) {
+      e = cudaMalloc((void **)&k->cmx, consts.size() * 8);
+      if (e == cudaSuccess) e = cudaMemcpy(k->cmx, consts.data(), consts.size() * 8, cudaMemcpyHostToDevice);
+    }
+  }
   if (e != cudaSuccess) {
     *why = std::string("loading the generated kernel failed: ") + cudaGetErrorString(e);
     cudaGetLastError();
@@ -206,6 +227,7 @@ cudaError_t k2_jit_launch(const K2Kernel *k, const K2Args &a, cudaStream_t st) {
   if (a.n <= 0) return cudaSuccess;
   const int grid = (a.n + k->threads - 1) / k->threads;
   K2Args args = a;
+  args.cmx = k->cmx;
   void *params[] = {&args};
   cudaError_t e = cudaLaunchKernel((const void *)k->kernel, dim3(grid), dim3(k->threads), params, k->smem, st);
   count_launch();

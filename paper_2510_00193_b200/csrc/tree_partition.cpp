@@ -98,7 +98,7 @@ bool tree_partition(int n_basic, int n_nodes, int n_prod, const int32_t *prod, i
     std::vector<char> in(n_nodes, 0);
     for (int n : clo[seed]) in[n] = 1;
     int cur_slots = slots_of(in, n_basic, n_nodes);
-    if (cur_slots > budget_slots) return false;                           // one closure alone does not fit
+    // (a closure that alone exceeds the budget becomes a group of its own: whether it fits is the caller's question)
     std::vector<int> members{seed};
     left[seed] = 0; --n_left;
     while (true) {

@@ -28,7 +28,8 @@ struct TreePartition {
   std::vector<TreeGroup> groups;
 };
 
-// false: the table has no product layer to cut at, or one closure alone exceeds the budget
+// false: the table has no product layer to cut at.  A cut node whose closure alone exceeds the budget gets a group
+// of its own.
 bool tree_partition(int n_basic, int n_nodes, int n_prod, const int32_t *prod, int n_basis, const int32_t *basis_node,
                     int budget_slots, TreePartition &out);
 

@@ -363,13 +363,15 @@ def test_error_codes_for_bad_tables_and_small_workspace(lib, torch):
 
 def test_level28_partitioned_tree_interpreted(lib, torch):
     """Level 28 (9 739 basis functions): one atom's node values exceed shared memory, so the table only runs
-    partitioned (132 group programs + top program).  Interpreter path (code generation off keeps create fast)."""
+    partitioned (132 group programs + top program), and with 350 000 table ops it is above the size mtp_create
+    specialises: the interpreter runs, and the handle says so."""
     lev, n_mu = 28, 7
-    assert lib.Table(lev).plan()["partitioned"] == 1
+    plan = lib.Table(lev).plan()
+    assert plan["partitioned"] == 1 and plan["specialised"] == 0
     w = cluster_workload(lev, n_mu, 33, 8, 2, r_list=5.0)
     opot = oracle_pot(w)
     ref = omtp.evaluate(opot, w.pos, w.types, w.box, w.off, w.idx, w.shift)
-    got, pot, _ = run_gpu(lib, torch, w)
-    assert pot.get_option(lib.INFO_TREE_KERNELS) == 0
+    got, pot, _ = run_gpu(lib, torch, w, interp=True)
+    assert pot.get_option(lib.INFO_TREE_KERNELS) == 0 and "too large to specialise" in pot.last_error()
     check(w, ref, got, opot)
     pot.close()
