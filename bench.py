@@ -1,11 +1,12 @@
 #!/usr/bin/env python
 """bench.py -- MTP energy+force atom-evaluations/s on one B200 (or N replicas, weak scaling).
 
-A "step" is one pass of the whole hot path (rows a1-a8, a10 of SURVEY.md 8(a)) over the
-BASELINE.json configs[3] workload: 1,048,576 atoms, 3 species, FCC 64^3, level 16, fp64,
-chunked evaluation.  `value` is device-resident throughput (CUDA events), `e2e` the same
-metric through mtp_compute_host with pinned HOST buffers (H2D + D2H inside the timed region).
-`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample.
+A "step" is one pass of the whole hot path (rows a1-a8, a10 of SURVEY.md 8(a)) over one BASELINE.json
+workload; the default is configs[3], the one the metric is quoted on: 1,048,576 atoms, 3 species, FCC 64^3,
+level 16, fp64, chunked evaluation.  `value` is device-resident throughput (CUDA events), `e2e` the same metric
+through mtp_compute_host with pinned HOST buffers (H2D + D2H inside the timed region).  `--impl reference`
+times the CPU oracle (oracle/, as it stands) on a bounded sample, on all host cores; it does not load the
+CUDA library.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
                   [--config I] [--cells C] [--grade]        (the last three: profiling aids)
@@ -14,11 +15,12 @@ from __future__ import annotations
 
 import argparse
 import json
+import multiprocessing
 import os
+import socket
 import subprocess
 import sys
 import tempfile
-import threading
 import time
 
 import numpy as np
@@ -27,18 +29,22 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 LEVELS = [10, 16, 20, 16, 24]
-METRIC = "MTP energy+force atom-evals/s at ~1M atoms lev16 fp64"
+HEADLINE = 3                         # 0-based index of the configuration BASELINE.json's metric is quoted on
 UNIT = "atom-evals/s"
 
 
-def survey_flops(lev, n_mu, n_basic, n_prod, n_basis, nu_max):
-    """Useful flops (FMA = 2): F_pair = 60 + 32 n_mu + 2 C(nu_max+3,3) + 10 n_basic,
-    split K1 (moments) / K3 (pair derivative); tree 6 n_prod + 2 n_basis per atom."""
-    mono = (nu_max + 1) * (nu_max + 2) * (nu_max + 3) // 6
-    k1 = 30 + 16 * n_mu + 2 * mono + 2 * n_basic
-    k3 = 30 + 16 * n_mu + 8 * n_basic
-    tree = 6 * n_prod + 2 * n_basis
-    return dict(k1_per_pair=k1, k3_per_pair=k3, tree_per_atom=tree)
+def metric_name(config, w):
+    """BASELINE.json's metric string for the configuration it is quoted on; the other configs say what they are."""
+    if config == HEADLINE and w.n_atoms == 1048576:
+        return "MTP energy+force atom-evals/s at ~1M atoms lev16 fp64"
+    return "MTP energy+force atom-evals/s at %d atoms lev%d fp64" % (w.n_atoms, w.lev_max)
+
+
+def flops_per_step(cost, w):
+    """Algorithmic flops of one step per kernel class (FMA = 2, each quantity once; formulas: DESIGN.md section 6,
+    numbers from mtp_cost_model)."""
+    return {"moments": cost["flop_per_pair_k1"] * w.nnz, "pairgrad": cost["flop_per_pair_k3"] * w.nnz,
+            "tree": cost["flop_per_atom_tree"] * w.n_atoms}
 
 
 class ClockSampler:
@@ -108,25 +114,104 @@ def whole_job_rate(n_atoms_per_rank, steps, seconds_local, world, dist, device):
     return world * n_atoms_per_rank * steps / max_over_ranks(seconds_local, dist, device)
 
 
-def build_workload(config, cells, seed_shift=0):
+def build_workload(config, cells, n_basis, seed_shift=0):
+    """The seeded synthetic workload (workloads/ holds no method arithmetic).  n_basis comes from the caller's own
+    basis enumeration: the CUDA library's for our arm, the oracle's for the reference arm."""
     from workloads import make_workload, CONFIGS
-    import paper_2510_00193_b200 as lib
-    table = lib.Table(LEVELS[config])
     from workloads.lattice import BASE_SEED
-    w = make_workload(config, table.n_basis, cells=cells, with_ainv=None,
-                      seed=BASE_SEED + config + 1000 * seed_shift)
-    return w, table, CONFIGS[config]
+    w = make_workload(config, n_basis, cells=cells, with_ainv=None, seed=BASE_SEED + config + 1000 * seed_shift)
+    return w, CONFIGS[config]
 
 
-def oracle_rate(w, n_sample, want_grad=True):
-    """atom-evals/s of the CPU oracle on the first n_sample atoms of the workload."""
+def config_dict(w, cfg, world):
+    """What the workload is -- the same dictionary in both arms."""
+    return {"workload": cfg["name"], "n_atoms": w.n_atoms, "nnz": w.nnz, "lev_max": w.lev_max, "n_species": w.n_species,
+            "n_basis": int(w.xi.shape[0]),
+            "l2": "inputs larger than L2 (neighbour list %.0f MB + per-pair scratch), no flush" % (w.nnz * 11 / 1e6),
+            "parallelism": "replicas x%d" % world}
+
+
+# ---------------------------------------------------------------- the oracle, timed on the host cores
+_ORACLE = {}
+
+
+def _oracle_worker(rng):
     from oracle import mtp as omtp
-    pot = omtp.Potential(w.lev_max, w.n_mu, w.n_beta, w.r_min, w.r_cut, w.c, w.xi0, w.xi)
-    atoms = range(min(n_sample, w.n_atoms))
-    t0 = time.perf_counter()
-    omtp.evaluate(pot, w.pos, w.types, w.box, w.off, w.idx, w.shift, atoms=atoms, want_grad=want_grad)
-    dt = time.perf_counter() - t0
-    return len(atoms) / dt, dt, len(atoms)
+    w, pot = _ORACLE["w"], _ORACLE["pot"]
+    omtp.evaluate(pot, w.pos, w.types, w.box, w.off, w.idx, w.shift, atoms=range(rng[0], rng[1]), want_grad=True)
+    return rng[1] - rng[0]
+
+
+def host_cores():
+    try:
+        return max(1, len(os.sched_getaffinity(0)))
+    except Exception:
+        return max(1, os.cpu_count() or 1)
+
+
+class OraclePool:
+    """The oracle as it stands (oracle/mtp.py evaluate: E_i, d_ij, force scatter per atom), one single-threaded
+    process per host core over contiguous atom ranges of the same workload.  Forked before CUDA is touched."""
+
+    def __init__(self, w, cores):
+        from oracle import mtp as omtp
+        try:
+            from threadpoolctl import threadpool_limits
+            threadpool_limits(limits=1)
+        except Exception:
+            pass
+        _ORACLE["w"] = w
+        _ORACLE["pot"] = omtp.Potential(w.lev_max, w.n_mu, w.n_beta, w.r_min, w.r_cut, w.c, w.xi0, w.xi)
+        self.cores = cores
+        self.pool = multiprocessing.get_context("fork").Pool(cores) if cores > 1 else None
+
+    def rate(self, w, atoms_per_core):
+        n = min(w.n_atoms, atoms_per_core * self.cores)
+        per = (n + self.cores - 1) // self.cores
+        ranges = [(lo, min(n, lo + per)) for lo in range(0, n, per)]
+        t0 = time.perf_counter()
+        done = sum(self.pool.map(_oracle_worker, ranges)) if self.pool else sum(_oracle_worker(r) for r in ranges)
+        dt = time.perf_counter() - t0
+        return done / dt, dt, done
+
+    def close(self):
+        if self.pool:
+            self.pool.close()
+            self.pool.join()
+
+
+def run_reference(args):
+    """--impl reference: the oracle timed on the host cores; each step is a bounded sample.  Loads nothing of the
+    CUDA library: n_basis is the oracle's own enumeration."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from oracle import basis as obasis
+    n_basis = len(obasis.basis_functions(LEVELS[args.config]))
+    w, cfg = build_workload(args.config, args.cells, n_basis)
+    cores = host_cores()
+    pool = OraclePool(w, cores)
+    per_core = args.ref_atoms or 1024           # x (steps + warmup): the whole run stays within a few minutes
+    for _ in range(args.warmup):
+        pool.rate(w, max(64, per_core // 8))
+    t = 0.0
+    n = 0
+    for _ in range(args.steps):
+        _, dt, k = pool.rate(w, per_core)
+        t += dt
+        n += k
+    pool.close()
+    value = n / t
+    sample = "first %d atoms of the workload per step (E_i, d_ij, force scatter), %d processes" % (n // max(args.steps, 1), cores)
+    line = {
+        "impl": "reference", "metric": metric_name(args.config, w), "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / max(args.steps, 1),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": config_dict(w, cfg, 1),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
 
 
 def graph_replay(torch, lib, pot, step, out, calls=100):
@@ -155,48 +240,37 @@ def graph_replay(torch, lib, pot, step, out, calls=100):
     return e0.elapsed_time(e1) / calls
 
 
-def run_reference(args):
-    """--impl reference: the oracle timed on host cores; each step is a bounded sample."""
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
-        return
+def load_traffic(workload, kernel):
+    """dram bytes per launch of `kernel` from the committed ncu capture of THIS workload (profiles/traffic.json,
+    keyed by workload name), else None: the number is not measurable without ncu."""
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
     try:
-        from threadpoolctl import threadpool_limits
-        ctx = threadpool_limits(limits=1)
+        return json.load(open(tpath)).get(workload, {}).get(kernel)
     except Exception:
-        ctx = None
-    w, table, cfg = build_workload(args.config, args.cells)
-    n_sample = args.ref_atoms or 1024          # x (steps + warmup): the whole run stays within a few minutes
-    for _ in range(args.warmup):
-        oracle_rate(w, n_sample)
-    t = 0.0
-    n = 0
-    for _ in range(args.steps):
-        r, dt, k = oracle_rate(w, n_sample)
-        t += dt
-        n += k
-    value = n / t
-    line = {
-        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg["name"], "n_atoms": w.n_atoms, "nnz": w.nnz, "lev_max": w.lev_max,
-                   "n_species": w.n_species},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
-                         "sample": "first %d atoms of the workload per step, E_i + d_ij + force scatter" % n_sample},
-        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-        "gpu_launches": 0,
-    }
-    print(json.dumps(line), flush=True)
+        return None
 
 
 def run_ours(args):
-    import torch
-    import paper_2510_00193_b200 as lib
-
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+
+    import paper_2510_00193_b200 as lib           # raises if libmtp_b200.so is missing: there is no fallback
+    table = lib.Table(LEVELS[args.config])
+    w, cfg = build_workload(args.config, args.cells, table.n_basis, seed_shift=rank)
+
+    # ---- CPU baseline first (processes are forked before this process touches CUDA): the oracle on a bounded
+    # sample of the same workload, all host cores
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        cores = host_cores()
+        pool = OraclePool(w, cores)
+        rate, dt, k = pool.rate(w, args.ref_atoms or 8192)
+        pool.close()
+        cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": "first %d atoms of the workload (E_i, d_ij, force scatter), %d processes, %.1f s" % (k, cores, dt)}
+
+    import torch
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
     torch.cuda.set_device(local)
@@ -207,7 +281,6 @@ def run_ours(args):
         dist = dist_
         dist.init_process_group("nccl", device_id=dev)
 
-    w, table, cfg = build_workload(args.config, args.cells, seed_shift=rank)
     pot = lib.Potential(table, w.n_species, w.n_beta, w.r_min, w.r_cut, w.c, w.xi0, w.xi)
     if args.chunk >= 0:
         pot.set_option(lib.OPT_CHUNK_ATOMS, args.chunk)
@@ -280,16 +353,14 @@ def run_ours(args):
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (fp64 ALU bound; DESIGN.md "Roofline")
-    nu_max = int(table.basic[:, 1:].sum(axis=1).max())
-    fl = survey_flops(w.lev_max, w.n_mu, table.n_basic, table.n_prod, table.n_basis, nu_max)
-    per_step = {"moments": fl["k1_per_pair"] * w.nnz, "pairgrad": fl["k3_per_pair"] * w.nnz,
-                "tree": fl["tree_per_atom"] * w.n_atoms}
+    # ---- roofline of the dominant kernel (fp64 ALU bound; DESIGN.md section 6)
+    per_step = flops_per_step(pot.cost_model(), w)
     timed = {k: prof[k] for k in ("moments", "tree", "pairgrad")}
     dom = max(timed, key=lambda k: timed[k][0])
     dom_ms, dom_n = timed[dom]
     sms = torch.cuda.get_device_properties(dev).multi_processor_count
-    peak_tf = sms * 64 * 2 * 1.965e9 / 1e12          # 64 fp64 FMA / clk / SM at clocks.max.sm
+    sm_ghz = (clocks.get("sm_max_mhz") or 1965.0) / 1e3
+    peak_tf = sms * 64 * 2 * sm_ghz * 1e9 / 1e12       # 64 fp64 FMA / clk / SM at clocks.max.sm
     achieved_tf = per_step[dom] * args.steps / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
     step_tf = sum(per_step.values()) * args.steps / (ms * 1e-3) / 1e12
     # measured DFMA throughput of this box (own microbenchmark, reported beside the derived peak)
@@ -302,42 +373,25 @@ def run_ours(args):
     a1.record()
     torch.cuda.synchronize()
     measured_tf = pk / (a0.elapsed_time(a1) * 1e-3) / 1e12
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath):
-        try:
-            traffic = json.load(open(tpath)).get(dom)
-        except Exception:
-            traffic = None
-
-    # ---- CPU baseline: the oracle on a bounded sample of the same workload
-    cpu = None
-    if world == 1 and not args.no_cpu_baseline:
-        try:
-            from threadpoolctl import threadpool_limits
-            lim = threadpool_limits(limits=1)
-        except Exception:
-            lim = None
-        rate, dt, k = oracle_rate(w, args.ref_atoms or 8192)
-        cpu = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": "first %d atoms of the workload (E_i, d_ij, force scatter), %.1f s" % (k, dt)}
+    ws_bytes = pot.workspace_bytes(w.n_atoms, w.nnz)
 
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "metric": metric_name(args.config, w), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg["name"], "n_atoms": w.n_atoms, "nnz": w.nnz, "lev_max": w.lev_max,
-                   "n_species": w.n_species, "n_basis": table.n_basis, "chunk_atoms": pot.get_option(lib.OPT_CHUNK_ATOMS),
-                   "force_mode": pot.get_option(lib.OPT_FORCE_MODE), "grade": bool(Ainv is not None),
-                   "l2": "inputs larger than L2 (neighbour list %.0f MB + per-pair scratch), no flush" % (w.nnz * 11 / 1e6),
-                   "parallelism": "replicas x%d" % world},
+        "config": config_dict(w, cfg, world),
+        "run": {"chunk_atoms": pot.get_option(lib.OPT_CHUNK_ATOMS), "force_mode": pot.get_option(lib.OPT_FORCE_MODE),
+                "grade": bool(Ainv is not None), "tree_kernels": pot.get_option(lib.INFO_TREE_KERNELS),
+                "tree_programs": pot.get_option(lib.INFO_TREE_PROGRAMS), "tree_note": pot.last_error(),
+                "workspace_bytes": int(ws_bytes)},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                 "steps": e2e_steps},
         "gpu_launches": int(launches),
         "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                     "frac": achieved_tf / peak_tf, "traffic": traffic,
-                     "peak_source": "derived: %d SMs x 64 fp64 FMA/clk x 2 x 1.965 GHz; measured DFMA microbenchmark %.1f TF/s" % (sms, measured_tf),
+                     "frac": achieved_tf / peak_tf, "traffic": load_traffic(cfg["name"], dom),
+                     "peak_source": "derived: %d SMs x 64 fp64 FMA/clk x 2 x %.3f GHz (clocks.max.sm); MEASURED_PEAKS.json has no fp64 entry; "
+                                    "own DFMA microbenchmark in this run %.1f TF/s" % (sms, sm_ghz, measured_tf),
                      "flops_per_launch": per_step[dom] / max(dom_n / args.steps, 1), "launches": dom_n,
                      "avg_launch_ms": dom_ms / max(dom_n, 1),
                      "step_achieved": step_tf, "step_frac": step_tf / peak_tf,
@@ -351,23 +405,35 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def spawn_ranks(args):
+    """`python bench.py --gpus N` outside torchrun: re-run this script as N ranks of one node."""
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=3, help="0-based index into BASELINE.json configs")
+    ap.add_argument("--config", type=int, default=HEADLINE, help="0-based index into BASELINE.json configs")
     ap.add_argument("--cells", type=int, default=None, help="override the lattice repeat (scaled-down instance)")
     ap.add_argument("--chunk", type=int, default=-1)
     ap.add_argument("--force-mode", type=int, default=-1)
     ap.add_argument("--grade", action="store_true", help="also run mtp_grade each step (config 4)")
     ap.add_argument("--ref-atoms", type=int, default=None,
-                    help="atoms per oracle sample (default: 8192 = about 12 s for cpu_baseline, 1024 per step for --impl reference)")
+                    help="atoms per core of an oracle sample (default: 8192 for cpu_baseline, 1024 per step for --impl reference)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(args)
     else:
         run_ours(args)
 

@@ -249,13 +249,14 @@ def grade_configuration(B, Ainv):
 
 
 # ---------------------------------------------------------------- own neighbour search
-def brute_force_neighbours(pos, box, r_cut):
+def brute_force_neighbours(pos, box, r_cut, rows=None):
     """The oracle's own O(27 N^2) search (north_star: 'brute-force neighbor search on
-    small inputs'); returns CSR (off, idx, shift), rows ordered by (j, shift)."""
+    small inputs'); returns CSR (off, idx, shift), rows ordered by (j, shift).
+    `rows`: only these centre atoms (the CSR then has len(rows) rows, in that order)."""
     pos = np.asarray(pos, dtype=np.float64)
     n = pos.shape[0]
     off, idx, sh = [0], [], []
-    for i in range(n):
+    for i in (range(n) if rows is None else rows):
         row = []
         for j in range(n):
             for sx in (-1, 0, 1):

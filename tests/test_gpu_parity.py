@@ -75,6 +75,81 @@ def test_energy_force_virial_parity(lib, torch, ci, cells):
     pot.close()
 
 
+def test_config1_meets_the_absolute_tolerances_as_written(lib, torch):
+    """BASELINE.json configs[0] (128 atoms, level 10) at full size against north_star's numbers read literally:
+    |dE_i| <= 1e-10 eV, |dF| <= 1e-9 eV/A, virial relative 1e-10 (at level 10 the magnitudes
+    still allow it)."""
+    w = make_workload(0, n_basis_of(10))
+    assert w.n_atoms == 128
+    opot = oracle_pot(w)
+    ref = omtp.evaluate(opot, w.pos, w.types, w.box, w.off, w.idx, w.shift)
+    got, pot, _ = run_gpu(lib, torch, w)
+    pot.close()
+    assert np.abs(got["Ei"] - ref["E_i"]).max() <= 1e-10
+    assert np.abs(got["F"] - ref["F"]).max() <= 1e-9
+    W6 = omtp.virial6(ref["W"])
+    assert np.abs(got["virial"] - W6).max() <= 1e-10 * np.abs(W6).max()
+
+
+def test_config2_full_size_energy_force_virial(lib, torch):
+    """BASELINE.json configs[1] at its stated size (2 000 atoms, level 16): every E_i, F_k and the virial."""
+    w = make_workload(1, n_basis_of(16))
+    assert w.n_atoms == 2000
+    opot = oracle_pot(w)
+    ref = omtp.evaluate(opot, w.pos, w.types, w.box, w.off, w.idx, w.shift)
+    got, pot, _ = run_gpu(lib, torch, w)
+    check(w, ref, got, opot)
+    pot.close()
+
+
+def sheared_workload(lev, n_mu, seed, n, S):
+    """Triclinic periodic box (rows = lattice vectors, all heights > 2 R_cut) with random atoms."""
+    rng = np.random.default_rng(seed)
+    box = np.array([[12.5, 0.0, 0.0], [3.1, 12.0, 0.0], [-2.2, 1.7, 11.6]])
+    pos = rng.uniform(0, 1, (n, 3)) @ box
+    types = rng.integers(0, S, n).astype(np.int32)
+    off, idx, sh = omtp.brute_force_neighbours(pos, box, 5.0)
+    nb = n_basis_of(lev)
+    return Workload(name="sheared", lev_max=lev, n_mu=n_mu, n_beta=8, r_min=2.0, r_cut=5.0, n_species=S,
+                    box=box, pos=pos, types=types, c=rng.uniform(-0.1, 0.1, (S, S, n_mu, 8)),
+                    xi0=rng.uniform(-0.1, 0.1, S), xi=rng.uniform(-0.1, 0.1, nb), off=off, idx=idx,
+                    shift=sh, rev=reverse_index(off, idx, sh))
+
+
+@pytest.mark.parametrize("lev,n_mu", [(10, 3), (16, 4)])
+def test_triclinic_box_with_shifts_and_with_minimum_image(lib, torch, lev, n_mu):
+    """A sheared box reaches the CUDA path: the image-shift table s.H and the inverse-box columns of the minimum
+    image (csrc/api.cu box_setup, csrc/pair_kernels.cuh pair_vector) against the oracle, both ways."""
+    w = sheared_workload(lev, n_mu, 41, 30, 2)
+    assert np.abs(w.shift).max() == 1
+    opot = oracle_pot(w)
+    ref = omtp.evaluate(opot, w.pos, w.types, w.box, w.off, w.idx, w.shift)
+    got, pot, d = run_gpu(lib, torch, w)
+    check(w, ref, got, opot)
+    out = pot.compute(d["pos"], d["types"], w.box, d["off"], d["idx"], None, d["rev"])       # minimum image
+    torch.cuda.synchronize()
+    check(w, ref, {k: v.cpu().numpy() for k, v in out.items()}, opot)
+    pot.close()
+
+
+def test_rejected_neighbour_entries_are_counted(lib, torch):
+    """include/mtp_b200.h: image shifts outside {-1,0,1}^3 (and indices outside [0, N)) do not fit the packed
+    neighbour word; they are dropped and reported through MTP_INFO_INPUT_ERRORS instead of aliasing silently."""
+    w = make_workload(0, n_basis_of(10))
+    pot = gpu_pot(lib, w)
+    d = to_dev(w, torch)
+    assert pot.get_option(lib.INFO_INPUT_ERRORS) == 0
+    pot.compute(d["pos"], d["types"], w.box, d["off"], d["idx"], d["shift"], d["rev"])
+    assert pot.get_option(lib.INFO_INPUT_ERRORS) == 0
+    bad = d["shift"].clone()
+    bad[5, 0] = 2
+    bad[77, 2] = -3
+    pot.compute(d["pos"], d["types"], w.box, d["off"], d["idx"], bad, d["rev"])
+    assert pot.get_option(lib.INFO_INPUT_ERRORS) == 2
+    assert pot.get_option(lib.INFO_INPUT_ERRORS) == 0          # reading resets the counter
+    pot.close()
+
+
 def test_chunked_equals_unchunked_and_gather_is_deterministic(lib, torch):
     w = make_workload(1, n_basis_of(16), cells=5)
     a, pot, d = run_gpu(lib, torch, w, opts={lib.OPT_FORCE_MODE: lib.FORCE_GATHER})
@@ -292,6 +367,7 @@ def test_full_size_config3_sampled(lib, torch):
     """BASELINE.json configs[2] at full size (54,000 atoms, 2 species, level 20)."""
     w = make_workload(2, n_basis_of(20))
     got, pot, _ = run_gpu(lib, torch, w)
+    assert assert_specialised(lib, pot) == lib.Table(20).plan()["groups"] + 1
     pot.close()
     assert w.n_atoms == 54000
     _check_sampled(w, got, 2, 12)
@@ -318,8 +394,12 @@ def test_full_size_config5_sampled_energy_and_grades(lib, torch):
         sE = max(1.0, np.abs(ref["B"][k] * w.xi).sum())
         assert abs(Ei[k] - ref["E_i"][k]) <= TOL_E * sE
         assert ga[k] == pytest.approx(want[q], rel=TOL_G)
-    F = out["F"].cpu().numpy()
-    assert np.all(np.abs(F.sum(axis=0)) <= 1e-9 * np.abs(F).sum())
+    n_prog = assert_specialised(lib, pot)
+    assert n_prog == lib.Table(24).plan()["groups"] + 1        # top program + every group program, all specialised
+    # forces through the partitioned, specialised K2 (group programs seeded with dE/dS, G accumulated over the
+    # groups) and K3: F_k of sampled atoms against the oracle, which evaluates them and all their neighbours
+    got = {"Ei": Ei, "F": out["F"].cpu().numpy()}
+    _check_sampled(w, got, 2, 13)
     # configuration mode: property that holds at any size -- gamma_cfg = max_k |Bsum . Ainv[:, k]| of the returned Bsum
     Bsum = g["Bsum"].cpu().numpy()
     assert g["gamma_cfg"].cpu().numpy()[0] == pytest.approx(np.abs(Bsum @ w.Ainv).max(), rel=TOL_G)

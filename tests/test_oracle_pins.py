@@ -11,7 +11,7 @@ import pytest
 from numpy.polynomial import chebyshev as npcheb
 
 from oracle import basis, mtp
-from workloads import random_cluster
+from workloads import random_cluster, make_workload, neighbor_list_bruteforce, reverse_index
 
 R_MIN, R_CUT, NB = 2.0, 5.0, 8
 N_MU = {6: 2, 8: 2, 10: 3, 12: 3, 14: 4, 16: 4, 20: 5, 24: 6}
@@ -96,7 +96,7 @@ def test_single_radial_function_is_cutoff_parabola():
 
 
 # ---------------------------------------------------------------- pin 1: one neighbour
-@pytest.mark.parametrize("lev", [10, 16, 20])
+@pytest.mark.parametrize("lev", [10, 16, 20, 24])
 def test_single_neighbour_closed_form(lev):
     """M_{mu,nu} = f_mu(r) r^{(x)nu}  =>  B_alpha = prod_v f_{mu_v}(r) * r^{sum nu}."""
     pot = make_pot(lev, S=2)
@@ -144,7 +144,7 @@ def dot_form(pot, zi, rv, zj, func):
     return total
 
 
-@pytest.mark.parametrize("lev,nn", [(10, 4), (12, 4), (16, 3)])
+@pytest.mark.parametrize("lev,nn", [(10, 4), (12, 4), (16, 3), (20, 3), (24, 2)])
 def test_vertex_assignment_brute_force(lev, nn):
     pot = make_pot(lev, S=2, seed=11)
     rng = np.random.default_rng(3)
@@ -168,10 +168,10 @@ def total_energy(pot, pos, types, box, r_list=None, dtype=np.float64):
     return mtp.evaluate(pot, pos, types, box, off, idx, sh, dtype=dtype), (off, idx, sh)
 
 
-@pytest.mark.parametrize("lev", [10, 16])
+@pytest.mark.parametrize("lev", [10, 16, 20, 24])
 def test_forces_sum_to_zero_and_match_finite_differences(lev):
     pot = make_pot(lev, S=2)
-    pos, types, box = small_config(n=12 if lev == 16 else 14)
+    pos, types, box = small_config(n={10: 14, 16: 12, 20: 10, 24: 8}[lev])
     out, _ = total_energy(pot, pos, types, box)
     scale = np.abs(out["F"]).max()
     assert np.abs(out["F"].sum(axis=0)).max() <= 1e-11 * scale
@@ -315,3 +315,90 @@ def test_long_double_arbiter_agrees():
     sE = np.abs(o80["E_i"]).max()
     assert float(np.abs(o64["E_i"] - o80["E_i"]).max()) < 1e-12 * float(sE)
     assert float(np.abs(o64["F"] - o80["F"]).max()) < 1e-11 * float(np.abs(o80["F"]).max())
+
+
+# ---------------------------------------------------------------- step 1: pair vectors and neighbour lists
+def _sheared_box():
+    """A triclinic box (rows = lattice vectors) whose three heights all exceed 2 R_cut."""
+    box = np.array([[12.5, 0.0, 0.0], [3.1, 12.0, 0.0], [-2.2, 1.7, 11.6]])
+    vol = abs(np.linalg.det(box))
+    heights = [vol / np.linalg.norm(np.cross(box[(k + 1) % 3], box[(k + 2) % 3])) for k in range(3)]
+    assert min(heights) > 2 * R_CUT
+    return box
+
+
+@pytest.mark.parametrize("triclinic", [False, True])
+def test_minimum_image_branch_equals_explicit_shifts(triclinic):
+    """pair_vectors(shift=None) (G17: minimum image, legal when every box height exceeds 2 R_cut) must give exactly
+    the vectors of the explicit-shift branch for every listed pair, in an orthorhombic and in a sheared box."""
+    rng = np.random.default_rng(17)
+    if triclinic:
+        box = _sheared_box()
+        pos = rng.uniform(0, 1, (26, 3)) @ box
+    else:
+        pos, _, box = random_cluster(9, 24, 11.0)
+    off, idx, sh = mtp.brute_force_neighbours(pos, box, R_CUT)
+    assert idx.shape[0] > 50 and np.abs(sh).max() == 1          # pairs through the periodic boundary are present
+    for i in range(pos.shape[0]):
+        js_a, rv_a = mtp.pair_vectors(i, pos, box, off, idx, sh)
+        js_b, rv_b = mtp.pair_vectors(i, pos, box, off, idx, None)
+        assert np.array_equal(js_a, js_b)
+        assert np.allclose(rv_a, rv_b, rtol=0, atol=1e-12)
+        assert np.all(np.linalg.norm(rv_a, axis=1) < R_CUT)
+    # and the brute-force list itself: every pair within R_cut of the 27 images is listed exactly once, nothing else
+    n = pos.shape[0]
+    count = 0
+    for i in range(n):
+        for j in range(n):
+            for s in itertools.product((-1, 0, 1), repeat=3):
+                if i == j and s == (0, 0, 0):
+                    continue
+                v = pos[j] - pos[i] + np.array(s) @ box
+                count += bool(v @ v < R_CUT * R_CUT)
+    assert count == idx.shape[0]
+
+
+def test_sheared_box_energy_is_rotation_invariant_and_forces_match_fd():
+    """The triclinic path of the oracle (shift . box with a non-diagonal box) against invariance and finite differences."""
+    pot = make_pot(10, S=2)
+    rng = np.random.default_rng(23)
+    box = _sheared_box()
+    pos = rng.uniform(0, 1, (16, 3)) @ box
+    types = rng.integers(0, 2, 16).astype(np.int32)
+    out, (off, idx, sh) = total_energy(pot, pos, types, box)
+    out_mi = mtp.evaluate(pot, pos, types, box, off, idx, None)
+    assert np.allclose(out_mi["E_i"], out["E_i"], rtol=1e-13) and np.allclose(out_mi["F"], out["F"], rtol=0, atol=1e-12 * np.abs(out["F"]).max())
+    q, _ = np.linalg.qr(rng.standard_normal((3, 3)))
+    out2, _ = total_energy(pot, pos @ q.T, types, box @ q.T)
+    assert np.allclose(out2["E_i"], out["E_i"], rtol=0, atol=1e-11 * np.abs(out["E_i"]).max())
+    h = 1e-5
+    for (k, a) in [(2, 0), (9, 2)]:
+        p = pos.copy(); p[k, a] += h
+        ep, _ = total_energy(pot, p, types, box)
+        p = pos.copy(); p[k, a] -= h
+        em, _ = total_energy(pot, p, types, box)
+        assert -(ep["E"] - em["E"]) / (2 * h) == pytest.approx(out["F"][k, a], rel=2e-6, abs=2e-7 * np.abs(out["F"]).max())
+
+
+@pytest.mark.parametrize("ci", [0, 1])
+def test_three_neighbour_list_builders_agree(ci):
+    """BASELINE.json configs[0] and configs[1] at full size: the lattice-stencil list the workloads use (both arms
+    consume it) equals the vectorised brute-force 27-image search bit for bit (off, idx, shift), and the oracle's
+    own pure-Python brute force equals both (every row at 128 atoms, sampled rows at 2 000 atoms); the reverse index
+    is an involution that maps (i, j, s) to (j, i, -s)."""
+    w = make_workload(ci, 1, with_rev=True)
+    assert w.n_atoms == (128, 2000)[ci]
+    off, idx, sh = neighbor_list_bruteforce(w.pos, w.box, R_CUT)
+    assert np.array_equal(off, w.off) and np.array_equal(idx, w.idx) and np.array_equal(sh, w.shift)
+    rows = list(range(w.n_atoms)) if ci == 0 else [0, 1, 77, 512, 999, 1203, 1998, 1999]
+    o_off, o_idx, o_sh = mtp.brute_force_neighbours(w.pos, w.box, R_CUT, rows=rows)
+    for q, i in enumerate(rows):
+        a, b = w.off[i], w.off[i + 1]
+        assert np.array_equal(o_idx[o_off[q]:o_off[q + 1]], w.idx[a:b])
+        assert np.array_equal(o_sh[o_off[q]:o_off[q + 1]], w.shift[a:b])
+    rev = w.rev
+    i_of = np.repeat(np.arange(w.n_atoms), np.diff(w.off))
+    assert np.array_equal(rev[rev], np.arange(w.nnz))
+    assert np.array_equal(w.idx[rev], i_of) and np.array_equal(i_of[rev], w.idx)
+    assert np.array_equal(w.shift[rev], -w.shift)
+    assert np.array_equal(reverse_index(w.off, w.idx, w.shift), rev)
