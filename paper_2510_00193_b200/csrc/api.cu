@@ -44,7 +44,7 @@ struct mtp_handle {
   const PairLevel *pl = nullptr;
   int crow = 0;
   double *d_coef = nullptr, *d_xi = nullptr, *d_xi0 = nullptr;
-  int *d_kmapF = nullptr, *d_kmapB = nullptr, *d_basis_node = nullptr;
+  int *d_kmapF = nullptr, *d_kmapB = nullptr, *d_kmapS = nullptr, *d_basis_node = nullptr;
   int *d_flag = nullptr;                       // device counter of rejected input pairs (MTP_INFO_INPUT_ERRORS)
   // K2 schedules, one per atom-lane count AL (compiled on first use; the large-N one at create)
   struct TreeDev {
@@ -579,7 +579,7 @@ extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
   const int nmu_lev = rt_nmu(h->pl->lev), nmup = (nmu_lev + 1) & ~1;
   h->crow = nmup * h->nb + 2;
   // K1 / K3 stage the coefficients of every species pair in shared memory next to their pair tiles
-  if ((size_t)h->S * h->S * h->crow * 8 + h->pl->smem_fixed > 227 * 1024) {
+  if ((size_t)h->S * h->S * h->crow * 8 + std::max(h->pl->smem_fixed, h->pl->smem_fixed_s) > 227 * 1024) {
     delete h;
     return fail(nullptr, MTP_EUNSUP, "n_species^2 x n_radial_basis x n_radial_funcs coefficients do not fit in shared memory beside the pair tiles");
   }
@@ -596,6 +596,11 @@ extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
   up(upload(h, &h->d_xi0, p->xi0, (size_t)p->n_species));
   up(upload(h, &h->d_kmapF, kf.data(), kf.size()));
   up(upload(h, &h->d_kmapB, kb.data(), kb.size()));
+  if (h->pl->nsl > 0) {                   // slot map of the sliced (large-system) pair kernels
+    std::vector<int> ks((size_t)h->pl->nsl * h->pl->nslot_s, -1);
+    h->pl->kmap_s(p->n_basic, p->basic, ks.data());
+    up(upload(h, &h->d_kmapS, ks.data(), ks.size()));
+  }
   up(upload(h, &h->d_basis_node, p->basis_node, (size_t)p->n_basis));
   up(upload(h, &h->d_flag, (const int *)nullptr, 0));
   if (e == cudaSuccess) e = cudaMemset(h->d_flag, 0, sizeof(int));
@@ -650,7 +655,7 @@ extern "C" int mtp_get_option(const mtp_handle *h, int key, int64_t *v) {
 namespace {
 struct Plan {
   int64_t N = 0, nnz = 0, C = 0, cols = 0;      // cols: C rounded up to whole tiles of 128 atoms (kTile)
-  int n_chunks = 0, P = 1, atomic = 0, grid_chunk = 0, AL = 0, AR = 1, elide = 1;
+  int n_chunks = 0, P = 1, sliced = 0, atomic = 0, grid_chunk = 0, AL = 0, AR = 1, elide = 1;
   size_t o_pos4 = 0, o_Ei = 0, o_M = 0, o_G = 0, o_wpart = 0, o_d4 = 0, o_B = 0, o_red = 0, o_idxp = 0, o_S = 0, o_Sbar = 0, total = 0;
 };
 size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -676,10 +681,13 @@ int make_plan(const mtp_handle *h, int64_t N, int64_t nnz, int want_grade, int h
   if (h->variant == MTP_VARIANT_THREAD) pl.P = 1;
   else if (h->variant == MTP_VARIANT_BLOCK) pl.P = h->pl->p_small;
   else pl.P = (N * NS >= 2LL * 148 * 256) ? 1 : h->pl->p_small;   // fill the SMs' register files
+  // PAPER.md:35 regimes: the thread-parallel mapping of a level that has the sliced kernels (pair_sliced.cuh: 32 atoms
+  // per CTA, components across the warps) is those; the block-parallel one splits an atom's neighbours over lanes
+  pl.sliced = pl.P == 1 && h->pl->nsl > 0 && h->d_kmapS != nullptr;
   pl.elide = want_grade ? 0 : 1;           // grades need every B_alpha stored
   if (h->interp_ready) tree_pick_shape(h->progs[0].slots[pl.elide][0], h->progs[0].slots[pl.elide][1], N, &pl.AL, &pl.AR);
   pl.atomic = h->force_mode == MTP_FORCE_ATOMIC || (h->force_mode == MTP_FORCE_AUTO && !has_rev);
-  pl.grid_chunk = h->pl->pairgrad_grid((int)C, pl.P);
+  pl.grid_chunk = pl.sliced ? h->pl->pairgrad_grid_s((int)C) : h->pl->pairgrad_grid((int)C, pl.P);
   size_t o = 0;
   pl.o_pos4 = o; o = align_up(o + (size_t)N * 32);
   pl.o_Ei = o; o = align_up(o + (size_t)N * 8);
@@ -879,14 +887,14 @@ static int compute_impl(mtp_handle *h, int64_t N, const double *d_pos, const int
       if (d_shift && p1 > p0)
         CU(h, launch_pack_pairs(d_idx + p0, (const signed char *)d_shift + 3 * p0, p1 - p0, N, (int *)(ws + pl.o_idxp) + p0, h->d_flag, st));
     }
-    pa.M = M; pa.G = G; pa.kmap = h->d_kmapF;
-    TIMED(h, CLS_MOMENTS, st, h->pl->moments(pa, pl.P, st));
+    pa.M = M; pa.G = G; pa.kmap = pl.sliced ? h->d_kmapS : h->d_kmapF;
+    TIMED(h, CLS_MOMENTS, st, (pl.sliced ? h->pl->moments_s(pa, st) : h->pl->moments(pa, pl.P, st)));
     io.c0 = pa.c0; io.c1 = pa.c1;
     rc = run_k2(h, io, st);
     if (rc != MTP_OK) return rc;
-    pa.kmap = h->d_kmapB; pa.wpart = wpart + (size_t)c * pl.grid_chunk * 8;
+    pa.kmap = pl.sliced ? h->d_kmapS : h->d_kmapB; pa.wpart = wpart + (size_t)c * pl.grid_chunk * 8;
     pa.d4 = pl.atomic ? nullptr : d4; pa.F = pl.atomic ? d_F : nullptr;
-    TIMED(h, CLS_PAIRGRAD, st, h->pl->pairgrad(pa, pl.P, pl.atomic, st, nullptr));
+    TIMED(h, CLS_PAIRGRAD, st, (pl.sliced ? h->pl->pairgrad_s(pa, pl.atomic, st) : h->pl->pairgrad(pa, pl.P, pl.atomic, st, nullptr)));
   }
   if (pipe && pipe->rev_ready) CU(h, cudaStreamWaitEvent(st, pipe->rev_ready, 0));
   if (!pl.atomic) TIMED(h, CLS_OTHER, st, launch_gather((const long long *)d_off, d_rev, d4, (int)N, d_F, st));
@@ -940,8 +948,8 @@ extern "C" int mtp_grade(mtp_handle *h, int64_t N, const double *d_pos, const in
     K2Io io{pos4, M, G, Ei, nullptr, 0, 0, 0, N, (double *)(ws + pl.o_S), (double *)(ws + pl.o_Sbar)};
     for (int c = 0; c < pl.n_chunks; ++c) {
       pa.c0 = (int)(c * pl.C); pa.c1 = (int)std::min<int64_t>(N, (c + 1) * pl.C);
-      pa.M = M; pa.kmap = h->d_kmapF;
-      TIMED(h, CLS_MOMENTS, st, h->pl->moments(pa, pl.P, st));
+      pa.M = M; pa.kmap = pl.sliced ? h->d_kmapS : h->d_kmapF;
+      TIMED(h, CLS_MOMENTS, st, (pl.sliced ? h->pl->moments_s(pa, st) : h->pl->moments(pa, pl.P, st)));
       io.c0 = pa.c0; io.c1 = pa.c1;
       io.B = Bt;
       rc = run_k2(h, io, st);
@@ -1060,9 +1068,9 @@ extern "C" int mtp_debug_moments(mtp_handle *h, int64_t N, const double *d_pos, 
     if (e != cudaSuccess) { cudaFree(tmp_idxp); return cuda_fail(h, e, "launch_pack_pairs"); }
   }
   fill_pair_args(h, pa, pos4, d_off, tmp_idxp ? tmp_idxp : d_idx, d_shift);
-  pa.n_rows = h->n_basic; pa.c0 = 0; pa.c1 = (int)N; pa.M = M; pa.kmap = h->d_kmapF;
+  pa.n_rows = h->n_basic; pa.c0 = 0; pa.c1 = (int)N; pa.M = M; pa.kmap = pl.sliced ? h->d_kmapS : h->d_kmapF;
   {
-    cudaError_t e = h->pl->moments(pa, pl.P, st);
+    cudaError_t e = pl.sliced ? h->pl->moments_s(pa, st) : h->pl->moments(pa, pl.P, st);
     if (tmp_idxp) { cudaStreamSynchronize(st); cudaFree(tmp_idxp); }
     if (e != cudaSuccess) return cuda_fail(h, e, "moments");
   }

@@ -77,6 +77,12 @@ struct PairLevel {
   cudaError_t (*moments)(const PairArgs &a, int P, cudaStream_t st);
   cudaError_t (*pairgrad)(const PairArgs &a, int P, int atomic, cudaStream_t st, int *grid_out);
   int (*pairgrad_grid)(int n_atoms, int P);
+  // large-system kernels with the components dealt to the warps of a CTA (pair_sliced.cuh); nsl = 0: the level has none
+  int nsl, nslot_s, smem_fixed_s;
+  cudaError_t (*moments_s)(const PairArgs &a, cudaStream_t st);
+  cudaError_t (*pairgrad_s)(const PairArgs &a, int atomic, cudaStream_t st);
+  int (*pairgrad_grid_s)(int n_atoms);
+  void (*kmap_s)(int n_basic, const int *basic, int *out);     // [nsl][nslot_s] slot -> packed component or -1
 };
 const PairLevel *pair_level(int index);   // index into kLevels
 

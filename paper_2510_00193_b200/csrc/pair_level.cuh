@@ -4,10 +4,65 @@
 #pragma once
 #include "kernels.h"
 #include "pair_tiled.cuh"
+#include "pair_sliced.cuh"
 
 namespace mtpb {
 
-template <int LEV, int NSB, int NSC, int PS>
+// the sliced (large-system) kernels of a level; NSL = 0: none
+template <int LEV, int NSL>
+struct SlicedImpl {
+  using Sl = Slicing<LEV, NSL>;
+  using Tl = STile<LEV, NSL>;
+  static size_t coef_doubles(const PairArgs &a) {
+    return (size_t)(a.n_species * a.n_species * a.crow) + kShiftLut + (size_t)((NSL * Sl::NSLOT + 3) / 4) * 2;
+  }
+  template <class K>
+  static cudaError_t prep(K kernel, size_t smem) {
+    return smem > 48 * 1024 ? cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) : cudaSuccess;
+  }
+  static int grid(int n_atoms) { return (n_atoms + 31) / 32; }
+  static cudaError_t moments(const PairArgs &a, cudaStream_t st) {
+    const int n = a.c1 - a.c0;
+    if (n <= 0) return cudaSuccess;
+    const size_t smem = 8 * (coef_doubles(a) + (size_t)Tl::CTA1);
+    cudaError_t e = a.nb == 8 ? prep(k_moments_s<LEV, NSL, 8>, smem) : prep(k_moments_s<LEV, NSL, 0>, smem);
+    if (e != cudaSuccess) return e;
+    if (a.nb == 8) k_moments_s<LEV, NSL, 8><<<grid(n), 32 * NSL, smem, st>>>(a);
+    else k_moments_s<LEV, NSL, 0><<<grid(n), 32 * NSL, smem, st>>>(a);
+    count_launch();
+    return cudaGetLastError();
+  }
+  template <bool ATOMIC>
+  static cudaError_t pairgrad_a(const PairArgs &a, int n, cudaStream_t st) {
+    const size_t smem = 8 * (coef_doubles(a) + (size_t)Tl::CTA3);
+    cudaError_t e = a.nb == 8 ? prep(k_pairgrad_s<LEV, NSL, ATOMIC, 8>, smem) : prep(k_pairgrad_s<LEV, NSL, ATOMIC, 0>, smem);
+    if (e != cudaSuccess) return e;
+    if (a.nb == 8) k_pairgrad_s<LEV, NSL, ATOMIC, 8><<<grid(n), 32 * NSL, smem, st>>>(a);
+    else k_pairgrad_s<LEV, NSL, ATOMIC, 0><<<grid(n), 32 * NSL, smem, st>>>(a);
+    count_launch();
+    return cudaGetLastError();
+  }
+  static cudaError_t pairgrad(const PairArgs &a, int atomic, cudaStream_t st) {
+    const int n = a.c1 - a.c0;
+    if (n <= 0) return cudaSuccess;
+    return atomic ? pairgrad_a<true>(a, n, st) : pairgrad_a<false>(a, n, st);
+  }
+  static void kmap(int n_basic, const int *basic, int *out) { sliced_kmap<LEV, NSL>(n_basic, basic, out); }
+  static void fill(PairLevel &r) {
+    r.nsl = NSL; r.nslot_s = Sl::NSLOT;
+    r.smem_fixed_s = 8 * (kShiftLut + ((NSL * Sl::NSLOT + 3) / 4) * 2 + (Tl::CTA3 > Tl::CTA1 ? Tl::CTA3 : Tl::CTA1));
+    r.moments_s = &moments; r.pairgrad_s = &pairgrad; r.pairgrad_grid_s = &grid; r.kmap_s = &kmap;
+  }
+};
+template <int LEV>
+struct SlicedImpl<LEV, 0> {
+  static void fill(PairLevel &r) {
+    r.nsl = 0; r.nslot_s = 0; r.smem_fixed_s = 0;
+    r.moments_s = nullptr; r.pairgrad_s = nullptr; r.pairgrad_grid_s = nullptr; r.kmap_s = nullptr;
+  }
+};
+
+template <int LEV, int NSB, int NSC, int PS, int NSL = 0>
 struct PairLevelImpl {
   using Sl = Slices<LEV, NSB, NSC>;
   static constexpr int kWarps = 4;                      // 128 threads per CTA
@@ -62,7 +117,9 @@ struct PairLevelImpl {
     constexpr int tile = max2(max2(Tile<LEV, NSB, NSC, 1>::WARP1, Tile<LEV, NSB, NSC, 1>::WARP3),
                               max2(Tile<LEV, NSB, NSC, PS>::WARP1, Tile<LEV, NSB, NSC, PS>::WARP3));
     const int fixed = 8 * (kShiftLut + ((Sl::NS * Sl::NSLOT + 3) / 4) * 2 + kWarps * tile);
-    return PairLevel{LEV, NSB, NSC, Sl::NSLOT, PS, fixed, &moments, &pairgrad, &pairgrad_grid};
+    PairLevel r{LEV, NSB, NSC, Sl::NSLOT, PS, fixed, &moments, &pairgrad, &pairgrad_grid, 0, 0, 0, nullptr, nullptr, nullptr, nullptr};
+    SlicedImpl<LEV, NSL>::fill(r);
+    return r;
   }
 };
 
