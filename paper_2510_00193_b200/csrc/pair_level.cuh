@@ -18,7 +18,8 @@ struct SlicedImpl {
   }
   template <class K>
   static cudaError_t prep(K kernel, size_t smem) {
-    return smem > 48 * 1024 ? cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) : cudaSuccess;
+    // the kernels also hold a little static shared memory: opt in well below the 48 KB default limit
+    return smem > 40 * 1024 ? cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) : cudaSuccess;
   }
   static int grid(int n_atoms) { return (n_atoms + 31) / 32; }
   static cudaError_t moments(const PairArgs &a, cudaStream_t st) {

@@ -100,7 +100,8 @@ struct STile {
   static constexpr int TILE1 = TN * KS1, TILE3 = TN * KS3;          // doubles
   static constexpr int DKS = 4 * 32 + KPAD;                         // dpart: [slice][k] blocks of [4][32] doubles
   static constexpr int DPART = NSL * TN * DKS;
-  static constexpr int STAGE = 2 * NT * 4 + (3 * NT + 1) / 2;       // two position buffers (32 B per thread) + three word buffers
+  static constexpr int STAGE = 2 * NT * 4 + (3 * NT + 1) / 2 + 32 * 4;   // two position buffers (32 B per thread), three word buffers,
+                                                                         // the 32 centre-atom records (x, y, z, species)
   static constexpr int CTA1 = 2 * TILE1 + STAGE, CTA3 = 2 * TILE3 + DPART + STAGE;       // the tile is double-buffered
   // CTAs per SM the register allocation aims at: 128 registers per thread while a slice has <= 40 components
   static constexpr int MINB = Slicing<LEV, NSL>::NSLOT <= 40 ? (512 / NT > 0 ? 512 / NT : 1) : 1;
@@ -295,15 +296,21 @@ __global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB) k_moments_s(c
   const int atom0 = a.c0 + blockIdx.x * 32;
   // phase A role: pair (pa, pk) = neighbour pk of the tile of atom pa
   const int pa = threadIdx.x / TN, pk = threadIdx.x % TN;
-  double xi = 0, yi = 0, zi = 0, ti = 0;
   long long beg = 0;
   int n_nb = 0;
   if (atom0 + pa < a.c1) {
-    load_pos4(a.pos4, atom0 + pa, xi, yi, zi, ti);
     beg = a.off[atom0 + pa];
     n_nb = (int)(a.off[atom0 + pa + 1] - beg);
   }
-  const int zi_s = (int)ti;
+  // the centre atoms' records live in shared memory: phase A reads its atom's (a broadcast) instead of holding
+  // x, y, z, species in registers across phase B
+  double *ctr = reinterpret_cast<double *>(wst - threadIdx.x + 3 * NT + (NT & 1));
+  if (threadIdx.x < 32) {
+    double cx = 0, cy = 0, cz = 0, ct = 0;
+    if (atom0 + threadIdx.x < a.c1) load_pos4(a.pos4, atom0 + threadIdx.x, cx, cy, cz, ct);
+    ctr[4 * threadIdx.x] = cx; ctr[4 * threadIdx.x + 1] = cy; ctr[4 * threadIdx.x + 2] = cz; ctr[4 * threadIdx.x + 3] = ct;
+  }
+  __syncthreads();
   // phase B role: lane = atom; every warp sees the same 32 atoms, so the row-length maximum is a warp reduction
   int nb_lane = 0;
   if (atom0 + lane < a.c1) nb_lane = (int)(a.off[atom0 + lane + 1] - a.off[atom0 + lane]);
@@ -329,7 +336,8 @@ __global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB) k_moments_s(c
     stage_word1(a, beg, n_nb, t0 + 2 * TN + pk, wst + NT * wnn);
     commit_copies();
     wb = wn; pb ^= 1;
-    stage_pair_fields<NMU, false, NB>(a, csm, slut, w, rec, NT, xi, yi, zi, zi_s, rc2, dst + pk * KS + pa);
+    const double2 c0 = *reinterpret_cast<const double2 *>(ctr + 4 * pa), c1 = *reinterpret_cast<const double2 *>(ctr + 4 * pa + 2);
+    stage_pair_fields<NMU, false, NB>(a, csm, slut, w, rec, NT, c0.x, c0.y, c1.x, (int)c1.y, rc2, dst + pk * KS + pa);
   };
   if (n_max > 0) phase_a(0, tile);
   __syncthreads();
@@ -372,15 +380,19 @@ __global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB) k_pairgrad_s(
   const int lane = threadIdx.x & 31, slice = threadIdx.x >> 5;
   const int atom0 = a.c0 + blockIdx.x * 32;
   const int pa = threadIdx.x / TN, pk = threadIdx.x % TN;
-  double xi = 0, yi = 0, zi = 0, ti = 0;
   long long beg = 0;
   int n_nb = 0;
   if (atom0 + pa < a.c1) {
-    load_pos4(a.pos4, atom0 + pa, xi, yi, zi, ti);
     beg = a.off[atom0 + pa];
     n_nb = (int)(a.off[atom0 + pa + 1] - beg);
   }
-  const int zi_s = (int)ti;
+  double *ctr = reinterpret_cast<double *>(wst - threadIdx.x + 3 * NT + (NT & 1));      // centre-atom records, as in K1
+  if (threadIdx.x < 32) {
+    double cx = 0, cy = 0, cz = 0, ct = 0;
+    if (atom0 + threadIdx.x < a.c1) load_pos4(a.pos4, atom0 + threadIdx.x, cx, cy, cz, ct);
+    ctr[4 * threadIdx.x] = cx; ctr[4 * threadIdx.x + 1] = cy; ctr[4 * threadIdx.x + 2] = cz; ctr[4 * threadIdx.x + 3] = ct;
+  }
+  __syncthreads();
   int nb_lane = 0;
   double g[NSLOT];
   if (atom0 + lane < a.c1) {
@@ -416,7 +428,8 @@ __global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB) k_pairgrad_s(
     stage_word1(a, beg, n_nb, t0 + 2 * TN + pk, wst + NT * wnn);
     commit_copies();
     wb = wn; pb ^= 1;
-    stage_pair_fields<NMU, true, NB>(a, csm, slut, w, rec, NT, xi, yi, zi, zi_s, rc2, dst + pk * KS + pa);
+    const double2 c0 = *reinterpret_cast<const double2 *>(ctr + 4 * pa), c1 = *reinterpret_cast<const double2 *>(ctr + 4 * pa + 2);
+    stage_pair_fields<NMU, true, NB>(a, csm, slut, w, rec, NT, c0.x, c0.y, c1.x, (int)c1.y, rc2, dst + pk * KS + pa);
     return w;
   };
   if (n_max > 0) w_cur = phase_a(0, tile);
