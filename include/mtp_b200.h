@@ -93,6 +93,11 @@ const char *mtp_last_error(const mtp_handle *h); /* h may be NULL: last create e
 #define MTP_OPT_FORCE_MODE 2    /* MTP_FORCE_GATHER (needs d_rev) | MTP_FORCE_ATOMIC       */
 #define MTP_OPT_VARIANT 3       /* MTP_VARIANT_AUTO | _THREAD | _BLOCK                     */
 #define MTP_OPT_PROFILE 4       /* 1: record CUDA events around every kernel launch        */
+#define MTP_OPT_CHUNK_PAIRS 6    /* upper bound of the neighbour-list entries of any one chunk: what the per-pair scratch
+                                   (packed neighbour words 4 B + d_ij records 32 B per pair) is sized for.  0 = automatic:
+                                   1.25 x nnz x chunk_atoms / N + 4096, right for lattice-like inputs; a chunk with more
+                                   pairs is counted in MTP_INFO_SCRATCH_OVERFLOW and its excess pairs are dropped.  With a
+                                   single chunk the scratch always holds all nnz pairs.                       */
 #define MTP_OPT_TREE_CODEGEN 5  /* 1 (default): run the contraction kernels specialised for the table (one register
                                    program per table, generated and compiled with NVRTC at mtp_create);
                                    0: interpret the table with the generic kernel (also what runs when libnvrtc is
@@ -105,7 +110,10 @@ const char *mtp_last_error(const mtp_handle *h); /* h may be NULL: last create e
 #define MTP_INFO_INPUT_ERRORS 102  /* mtp_get_option only, SYNCHRONISES the device: neighbour-list entries rejected
                                       since the last read (image shift outside {-1,0,1}^3 or index outside [0,N));
                                       such pairs are dropped, so a non-zero count means the results are not valid   */
-#define MTP_FORCE_GATHER 0      /* deterministic; keeps d_ij for all pairs (nnz x 32 B)  */
+#define MTP_INFO_SCRATCH_OVERFLOW 103 /* mtp_get_option only, SYNCHRONISES: pairs that did not fit the per-pair scratch of their
+                                      chunk since the last read (see MTP_OPT_CHUNK_PAIRS); non-zero = results not valid */
+#define MTP_FORCE_GATHER 0      /* deterministic: d_ij kept for one chunk at a time, forces assembled chunk by chunk in
+                                   fixed order over the reverse-neighbour index (bit-reproducible run to run)    */
 #define MTP_FORCE_ATOMIC 1      /* fp64 atomic scatter; no per-pair scratch              */
 #define MTP_FORCE_AUTO 2        /* default: gather when d_rev is given, else atomic      */
 #define MTP_VARIANT_AUTO 0

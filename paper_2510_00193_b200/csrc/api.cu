@@ -45,7 +45,9 @@ struct mtp_handle {
   int crow = 0;
   double *d_coef = nullptr, *d_xi = nullptr, *d_xi0 = nullptr;
   int *d_kmapF = nullptr, *d_kmapB = nullptr, *d_kmapS = nullptr, *d_basis_node = nullptr;
-  int *d_flag = nullptr;                       // device counter of rejected input pairs (MTP_INFO_INPUT_ERRORS)
+  int *d_flag = nullptr;                       // device counters: [0] rejected input pairs (MTP_INFO_INPUT_ERRORS), [1] pairs beyond the
+                                               // per-pair scratch of a chunk (MTP_INFO_SCRATCH_OVERFLOW)
+  int64_t chunk_pairs = 0;                     // MTP_OPT_CHUNK_PAIRS
   // K2 schedules, one per atom-lane count AL (compiled on first use; the large-N one at create)
   struct TreeDev {
     TreeSched sched;
@@ -602,8 +604,10 @@ extern "C" int mtp_create(mtp_handle **out, const mtp_params *p) {
     up(upload(h, &h->d_kmapS, ks.data(), ks.size()));
   }
   up(upload(h, &h->d_basis_node, p->basis_node, (size_t)p->n_basis));
-  up(upload(h, &h->d_flag, (const int *)nullptr, 0));
-  if (e == cudaSuccess) e = cudaMemset(h->d_flag, 0, sizeof(int));
+  {
+    const int zero2[2] = {0, 0};
+    up(upload(h, &h->d_flag, zero2, 2));
+  }
   if (e != cudaSuccess) { int r = cuda_fail(nullptr, e, "mtp_create upload"); mtp_destroy(h); return r; }
   // K2: the specialised kernels; when they cannot be had (no NVRTC, ...) the reason is kept for mtp_last_error and
   // the interpreter is set up instead.  A table neither form can run fails here.
@@ -624,6 +628,7 @@ extern "C" int mtp_set_option(mtp_handle *h, int key, int64_t v) {
     case MTP_OPT_FORCE_MODE: if (v < 0 || v > 2) return fail(h, MTP_EINVAL, "bad force mode"); h->force_mode = (int)v; return MTP_OK;
     case MTP_OPT_VARIANT: if (v < 0 || v > 2) return fail(h, MTP_EINVAL, "bad variant"); h->variant = (int)v; return MTP_OK;
     case MTP_OPT_PROFILE: h->profile = v != 0; return MTP_OK;
+    case MTP_OPT_CHUNK_PAIRS: if (v < 0) return fail(h, MTP_EINVAL, "chunk_pairs < 0"); h->chunk_pairs = v; return MTP_OK;
     case MTP_OPT_TREE_CODEGEN:
       if (v != 0 && !h->jit_ready) return fail(h, MTP_EUNSUP, "specialised contraction kernels not available: " + h->jit_note);
       if (v == 0) { int rc = ensure_interp(h); if (rc != MTP_OK) return rc; }
@@ -641,10 +646,13 @@ extern "C" int mtp_get_option(const mtp_handle *h, int key, int64_t *v) {
     case MTP_OPT_TREE_CODEGEN: *v = h->codegen && h->jit_ready; return MTP_OK;
     case MTP_INFO_TREE_KERNELS: *v = h->jit_ready ? h->n_jit_kernels : 0; return MTP_OK;      // specialised K2 kernels loaded
     case MTP_INFO_TREE_PROGRAMS: *v = h->jit_ready ? (int64_t)h->jprogs.size() : 0; return MTP_OK;
-    case MTP_INFO_INPUT_ERRORS: {             // synchronises: pairs the packing kernel rejected since the last read
+    case MTP_OPT_CHUNK_PAIRS: *v = h->chunk_pairs; return MTP_OK;
+    case MTP_INFO_INPUT_ERRORS:               // synchronises: pairs the packing kernel rejected since the last read
+    case MTP_INFO_SCRATCH_OVERFLOW: {         // synchronises: pairs that did not fit a chunk's per-pair scratch
+      const int q = key == MTP_INFO_INPUT_ERRORS ? 0 : 1;
       int flag = 0;
-      if (cudaMemcpy(&flag, h->d_flag, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess) return MTP_ECUDA;
-      if (flag) cudaMemset(h->d_flag, 0, sizeof(int));
+      if (cudaMemcpy(&flag, h->d_flag + q, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess) return MTP_ECUDA;
+      if (flag) cudaMemset(h->d_flag + q, 0, sizeof(int));
       *v = flag; return MTP_OK;
     }
   }
@@ -656,11 +664,12 @@ namespace {
 struct Plan {
   int64_t N = 0, nnz = 0, C = 0, cols = 0;      // cols: C rounded up to whole tiles of 128 atoms (kTile)
   int n_chunks = 0, P = 1, sliced = 0, atomic = 0, grid_chunk = 0, AL = 0, AR = 1, elide = 1;
-  size_t o_pos4 = 0, o_Ei = 0, o_M = 0, o_G = 0, o_wpart = 0, o_d4 = 0, o_B = 0, o_red = 0, o_idxp = 0, o_S = 0, o_Sbar = 0, total = 0;
+  int64_t cap = 0;                              // pairs of one chunk the per-pair scratch (packed words, d4) holds
+  size_t o_pos4 = 0, o_Ei = 0, o_M = 0, o_G = 0, o_wpart = 0, o_d4 = 0, o_B = 0, o_red = 0, o_idxp = 0, o_S = 0, o_Sbar = 0, o_jr = 0, total = 0;
 };
 size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
-int make_plan(const mtp_handle *h, int64_t N, int64_t nnz, int want_grade, int has_rev, Plan &pl) {
+int make_plan(const mtp_handle *h, int64_t N, int64_t nnz, int want_grade, int has_rev, Plan &pl, int64_t cap_exact = -1) {
   if (N < 0 || nnz < 0) return MTP_EINVAL;
   if (N > (1LL << 27)) return MTP_EUNSUP;      // neighbour words carry 27 index bits (pair_kernels.cuh)
   pl.N = N; pl.nnz = nnz;
@@ -698,9 +707,18 @@ int make_plan(const mtp_handle *h, int64_t N, int64_t nnz, int want_grade, int h
     pl.o_S = o; o = align_up(o + (size_t)h->n_cut_rows * pl.cols * 8);
     pl.o_Sbar = o; o = align_up(o + (size_t)h->n_cut_rows * pl.cols * 8);
   }
-  pl.o_idxp = o; o = align_up(o + (size_t)nnz * 4);          // packed neighbour words (used when shifts are given)
+  // a10 (north_star "a chunk scheduler that bounds per-pair scratch"): packed neighbour words and d_ij
+  // records exist for one chunk at a time.  The pair count of a chunk is known only on the device, so the buffers are
+  // sized for MTP_OPT_CHUNK_PAIRS when set, else for 1.25 x the mean pairs per chunk + 4096 (lattice-like inputs; a
+  // chunk that does not fit is counted in MTP_INFO_SCRATCH_OVERFLOW); a single chunk gets exactly nnz.
+  if (pl.n_chunks <= 1) pl.cap = nnz;
+  else if (cap_exact >= 0) pl.cap = cap_exact;
+  else if (h->chunk_pairs > 0) pl.cap = std::min<int64_t>(nnz, h->chunk_pairs);
+  else pl.cap = std::min<int64_t>(nnz, (int64_t)(1.25 * (double)nnz * (double)C / (double)std::max<int64_t>(N, 1)) + 4096);
+  pl.o_idxp = o; o = align_up(o + (size_t)pl.cap * 4);        // packed neighbour words (used when shifts are given)
+  pl.o_jr = o; o = align_up(o + kTouchWords * sizeof(unsigned));      // touch bitmap of the current chunk
   pl.o_wpart = o; o = align_up(o + (size_t)std::max(1, pl.n_chunks) * pl.grid_chunk * 64);
-  pl.o_d4 = o; if (!want_grade && !pl.atomic) o = align_up(o + (size_t)nnz * 32);
+  pl.o_d4 = o; if (!want_grade && !pl.atomic) o = align_up(o + (size_t)pl.cap * 32);
   pl.o_B = o; if (want_grade) o = align_up(o + (size_t)pl.cols * h->n_basis * 8);      // tiled Bt of one chunk
   pl.total = o;
   return MTP_OK;
@@ -735,6 +753,7 @@ void fill_pair_args(const mtp_handle *h, PairArgs &pa, const double *pos4, const
   pa.coef = h->d_coef; pa.n_species = h->S; pa.nb = h->nb; pa.crow = h->crow;
   pa.minimg = shift ? 0 : 1; pa.r_min = h->r_min; pa.r_cut = h->r_cut;
   pa.M = nullptr; pa.G = nullptr; pa.d4 = nullptr; pa.F = nullptr; pa.wpart = nullptr; pa.kmap = nullptr;
+  pa.d4_cap = 0; pa.flag = h->d_flag; pa.idx_rel = 0; pa.idx_cap = 1LL << 62;
 }
 
 // One chunk of K2 work: B_alpha / E_i (forward) and, when want_adj, G = dE_i/dM.  B != null: every basis value of
@@ -845,14 +864,14 @@ struct HostPipe {
 static int compute_impl(mtp_handle *h, int64_t N, const double *d_pos, const int32_t *d_type, const double *box,
                         const int64_t *d_off, const int32_t *d_idx, const int8_t *d_shift, const int32_t *d_rev,
                         int64_t nnz, double *d_E, double *d_Ei, double *d_F, double *d_virial, void *d_ws,
-                        size_t ws_bytes, void *stream, const HostPipe *pipe) {
+                        size_t ws_bytes, void *stream, const HostPipe *pipe, int64_t cap_exact = -1) {
   if (!h) return MTP_EINVAL;
   if (!box || !d_E || (N > 0 && (!d_pos || !d_type || !d_off || !d_F)) || (nnz > 0 && !d_idx))
     return fail(h, MTP_EINVAL, "mtp_compute: null argument");
   if (h->force_mode == MTP_FORCE_GATHER && !d_rev && nnz > 0) return fail(h, MTP_EINVAL, "gather mode needs d_rev");
   cudaStream_t st = (cudaStream_t)stream;
   Plan pl;
-  int rc = make_plan(h, N, nnz, 0, d_rev != nullptr, pl);
+  int rc = make_plan(h, N, nnz, 0, d_rev != nullptr, pl, cap_exact);
   if (rc != MTP_OK) return fail(h, rc, "bad sizes");
   const size_t base = align_up((size_t)(uintptr_t)d_ws) - (size_t)(uintptr_t)d_ws;
   if (N > 0 && (!d_ws || ws_bytes < pl.total + base)) return fail(h, MTP_ESIZE, "workspace too small");
@@ -870,34 +889,36 @@ static int compute_impl(mtp_handle *h, int64_t N, const double *d_pos, const int
   double *d4 = (double *)(ws + pl.o_d4);
   CU(h, launch_pack(d_pos, d_type, (int)N, pos4, st));
   CU(h, launch_zero(wpart, (long long)pl.n_chunks * pl.grid_chunk * 8, st));
-  if (pl.atomic) CU(h, launch_zero(d_F, 3 * N, st));
-  const int32_t *idxp = d_idx;
-  if (d_shift && nnz > 0) {
-    if (!pipe) CU(h, launch_pack_pairs(d_idx, (const signed char *)d_shift, nnz, N, (int *)(ws + pl.o_idxp), h->d_flag, st));
-    idxp = (const int32_t *)(ws + pl.o_idxp);
-  }
-  fill_pair_args(h, pa, pos4, d_off, idxp, d_shift);
+  CU(h, launch_zero(d_F, 3 * N, st));            // both force modes accumulate: atomics, or chunk by chunk in fixed order
+  int *idxp = (int *)(ws + pl.o_idxp);
+  unsigned *jrange = (unsigned *)(ws + pl.o_jr);
+  fill_pair_args(h, pa, pos4, d_off, d_shift ? idxp : d_idx, d_shift);
   pa.n_rows = h->n_basic;
+  pa.idx_rel = d_shift ? 1 : 0;                  // packed words exist for the current chunk only
+  pa.idx_cap = d_shift ? pl.cap : nnz;
+  pa.d4_cap = pl.cap;
   K2Io io{pos4, M, G, Ei, nullptr, 0, 0, 1, N, (double *)(ws + pl.o_S), (double *)(ws + pl.o_Sbar)};
+  bool rev_waited = false;
   for (int c = 0; c < pl.n_chunks; ++c) {
     pa.c0 = (int)(c * pl.C); pa.c1 = (int)std::min<int64_t>(N, (c + 1) * pl.C);
-    if (pipe) {                                  // this chunk's pairs have just arrived: pack their neighbour words
-      CU(h, cudaStreamWaitEvent(st, (*pipe->chunk_ready)[c], 0));
-      const long long p0 = (*pipe->chunk_pair0)[c], p1 = (*pipe->chunk_pair0)[c + 1];
-      if (d_shift && p1 > p0)
-        CU(h, launch_pack_pairs(d_idx + p0, (const signed char *)d_shift + 3 * p0, p1 - p0, N, (int *)(ws + pl.o_idxp) + p0, h->d_flag, st));
-    }
+    if (pipe) CU(h, cudaStreamWaitEvent(st, (*pipe->chunk_ready)[c], 0));      // this chunk's pairs have arrived
+    // the chunk's neighbour words (validated, index + image code in 4 bytes) and the range of atoms it touches
+    if (nnz > 0)
+      CU(h, launch_pack_pairs_chunk((const long long *)d_off, pa.c0, pa.c1, d_idx, (const signed char *)d_shift, N, pl.cap,
+                                    d_shift ? idxp : nullptr, h->d_flag, jrange, st));
     pa.M = M; pa.G = G; pa.kmap = pl.sliced ? h->d_kmapS : h->d_kmapF;
     TIMED(h, CLS_MOMENTS, st, (pl.sliced ? h->pl->moments_s(pa, st) : h->pl->moments(pa, pl.P, st)));
     io.c0 = pa.c0; io.c1 = pa.c1;
     rc = run_k2(h, io, st);
     if (rc != MTP_OK) return rc;
     pa.kmap = pl.sliced ? h->d_kmapS : h->d_kmapB; pa.wpart = wpart + (size_t)c * pl.grid_chunk * 8;
-    pa.d4 = pl.atomic ? nullptr : d4; pa.F = pl.atomic ? d_F : nullptr;
+    pa.d4 = pl.atomic ? nullptr : d4; pa.F = d_F;
     TIMED(h, CLS_PAIRGRAD, st, (pl.sliced ? h->pl->pairgrad_s(pa, pl.atomic, st) : h->pl->pairgrad(pa, pl.P, pl.atomic, st, nullptr)));
+    if (!pl.atomic && nnz > 0) {                 // a8: this chunk's share of every F_k it touches, chunks in stream order
+      if (pipe && pipe->rev_ready && !rev_waited) { CU(h, cudaStreamWaitEvent(st, pipe->rev_ready, 0)); rev_waited = true; }
+      TIMED(h, CLS_OTHER, st, launch_gather_chunk((const long long *)d_off, d_idx, d_rev, d4, pl.cap, pa.c0, pa.c1, (int)N, jrange, d_F, st));
+    }
   }
-  if (pipe && pipe->rev_ready) CU(h, cudaStreamWaitEvent(st, pipe->rev_ready, 0));
-  if (!pl.atomic) TIMED(h, CLS_OTHER, st, launch_gather((const long long *)d_off, d_rev, d4, (int)N, d_F, st));
   double *red = (double *)(ws + pl.o_red);
   CU(h, launch_reduce(Ei, N, 1, 1, d_E, red, st));
   if (d_virial) CU(h, launch_reduce(wpart, (long long)pl.n_chunks * pl.grid_chunk, 8, 6, d_virial, red, st));
@@ -938,16 +959,18 @@ extern "C" int mtp_grade(mtp_handle *h, int64_t N, const double *d_pos, const in
   if (mode != 0 || d_Bsum) CU(h, launch_zero(Bsum, h->n_basis, st));
   if (N > 0) {
     CU(h, launch_pack(d_pos, d_type, (int)N, pos4, st));
-    const int32_t *idxp = d_idx;
-    if (d_shift && nnz > 0) {
-      CU(h, launch_pack_pairs(d_idx, (const signed char *)d_shift, nnz, N, (int *)(ws + pl.o_idxp), h->d_flag, st));
-      idxp = (const int32_t *)(ws + pl.o_idxp);
-    }
-    fill_pair_args(h, pa, pos4, d_off, idxp, d_shift);
+    int *idxp = (int *)(ws + pl.o_idxp);
+    unsigned *jrange = (unsigned *)(ws + pl.o_jr);
+    fill_pair_args(h, pa, pos4, d_off, d_shift ? idxp : d_idx, d_shift);
     pa.n_rows = h->n_basic;
+    pa.idx_rel = d_shift ? 1 : 0;
+    pa.idx_cap = d_shift ? pl.cap : nnz;
     K2Io io{pos4, M, G, Ei, nullptr, 0, 0, 0, N, (double *)(ws + pl.o_S), (double *)(ws + pl.o_Sbar)};
     for (int c = 0; c < pl.n_chunks; ++c) {
       pa.c0 = (int)(c * pl.C); pa.c1 = (int)std::min<int64_t>(N, (c + 1) * pl.C);
+      if (nnz > 0)
+        CU(h, launch_pack_pairs_chunk((const long long *)d_off, pa.c0, pa.c1, d_idx, (const signed char *)d_shift, N, pl.cap,
+                                      d_shift ? idxp : nullptr, h->d_flag, jrange, st));
       pa.M = M; pa.kmap = pl.sliced ? h->d_kmapS : h->d_kmapF;
       TIMED(h, CLS_MOMENTS, st, (pl.sliced ? h->pl->moments_s(pa, st) : h->pl->moments(pa, pl.P, st)));
       io.c0 = pa.c0; io.c1 = pa.c1;
@@ -970,9 +993,16 @@ extern "C" int mtp_compute_host(mtp_handle *h, int64_t N, const double *pos, con
                                 int64_t nnz, double *E, double *Ei, double *F, double *virial) {
   if (!h) return MTP_EINVAL;
   if (!box || !E || (N > 0 && (!pos || !type || !off || !F)) || (nnz > 0 && !idx)) return fail(h, MTP_EINVAL, "mtp_compute_host: null argument");
-  size_t wsb = 0;
-  int rc = mtp_workspace_bytes(h, N, nnz, 0, &wsb);
-  if (rc != MTP_OK) return rc;
+  // the CSR offsets are on the host here: the per-pair scratch is sized for the largest chunk exactly
+  Plan pl;
+  int rc = make_plan(h, N, nnz, 0, rev != nullptr, pl);
+  if (rc != MTP_OK) return fail(h, rc, "bad sizes");
+  int64_t cap = 0;
+  for (int c = 0; c < pl.n_chunks; ++c)
+    cap = std::max<int64_t>(cap, off[std::min<int64_t>(N, (int64_t)(c + 1) * pl.C)] - off[(int64_t)c * pl.C]);
+  rc = make_plan(h, N, nnz, 0, rev != nullptr, pl, cap);
+  if (rc != MTP_OK) return fail(h, rc, "bad sizes");
+  const size_t wsb = pl.total + 512;
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
   const size_t o_pos = take((size_t)N * 24), o_type = take((size_t)N * 4), o_off = take((size_t)(N + 1) * 8);
@@ -992,9 +1022,6 @@ extern "C" int mtp_compute_host(mtp_handle *h, int64_t N, const double *pos, con
     CU(h, cudaStreamCreateWithFlags(&h->s_copy, cudaStreamNonBlocking));
     CU(h, cudaStreamCreateWithFlags(&h->s_comp, cudaStreamNonBlocking));
   }
-  Plan pl;
-  rc = make_plan(h, N, nnz, 0, rev != nullptr, pl);
-  if (rc != MTP_OK) return fail(h, rc, "bad sizes");
   while ((int)h->ev.size() < pl.n_chunks + 2) {
     cudaEvent_t e = nullptr;
     CU(h, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
@@ -1017,16 +1044,19 @@ extern "C" int mtp_compute_host(mtp_handle *h, int64_t N, const double *pos, con
       if (shift) CU(h, cudaMemcpyAsync(d + o_shift + 3 * p0, shift + 3 * p0, (size_t)(p1 - p0) * 3, cudaMemcpyHostToDevice, sc));
     }
     CU(h, cudaEventRecord(ready[c], sc));
+    if (c == 0) {      // the reverse index is needed by the first chunk's force assembly: it travels while chunk 0 is evaluated
+      if (rev && nnz > 0) CU(h, cudaMemcpyAsync(d + o_rev, rev, (size_t)nnz * 4, cudaMemcpyHostToDevice, sc));
+      CU(h, cudaEventRecord(h->ev[1], sc));
+    }
   }
-  if (rev && nnz > 0) CU(h, cudaMemcpyAsync(d + o_rev, rev, (size_t)nnz * 4, cudaMemcpyHostToDevice, sc));
-  CU(h, cudaEventRecord(h->ev[1], sc));
+  if (pl.n_chunks == 0) CU(h, cudaEventRecord(h->ev[1], sc));
   CU(h, cudaStreamWaitEvent(st, h->ev[0], 0));
   HostPipe pipe;
   pipe.chunk_ready = &ready; pipe.chunk_pair0 = &pair0; pipe.rev_ready = h->ev[1];
   double *dE = (double *)(d + o_out), *dW = dE + 1, *dEi = dE + 7, *dF = dEi + N;
   rc = compute_impl(h, N, (double *)(d + o_pos), (int32_t *)(d + o_type), box, (int64_t *)(d + o_off),
                     (int32_t *)(d + o_idx), shift ? (int8_t *)(d + o_shift) : nullptr,
-                    rev ? (int32_t *)(d + o_rev) : nullptr, nnz, dE, dEi, dF, dW, d + o_ws, wsb, st, N > 0 ? &pipe : nullptr);
+                    rev ? (int32_t *)(d + o_rev) : nullptr, nnz, dE, dEi, dF, dW, d + o_ws, wsb, st, N > 0 ? &pipe : nullptr, cap);
   if (rc != MTP_OK) { cudaStreamSynchronize(sc); cudaStreamSynchronize(st); return rc; }
   if (N == 0) CU(h, cudaStreamWaitEvent(st, h->ev[1], 0));
   CU(h, cudaMemcpyAsync(E, dE, 8, cudaMemcpyDeviceToHost, st));
@@ -1064,10 +1094,12 @@ extern "C" int mtp_debug_moments(mtp_handle *h, int64_t N, const double *d_pos, 
     CU(h, cudaMemcpyAsync(&nnz, d_off + N, 8, cudaMemcpyDeviceToHost, st));
     CU(h, cudaStreamSynchronize(st));
     CU(h, cudaMalloc((void **)&tmp_idxp, (size_t)std::max<long long>(nnz, 1) * 4));
-    cudaError_t e = launch_pack_pairs(d_idx, (const signed char *)d_shift, nnz, N, tmp_idxp, h->d_flag, st);
-    if (e != cudaSuccess) { cudaFree(tmp_idxp); return cuda_fail(h, e, "launch_pack_pairs"); }
+    cudaError_t e = launch_pack_pairs_chunk((const long long *)d_off, 0, (int)N, d_idx, (const signed char *)d_shift, N, nnz, tmp_idxp,
+                                            h->d_flag, (unsigned *)(ws + pl.o_jr), st);
+    if (e != cudaSuccess) { cudaFree(tmp_idxp); return cuda_fail(h, e, "launch_pack_pairs_chunk"); }
   }
   fill_pair_args(h, pa, pos4, d_off, tmp_idxp ? tmp_idxp : d_idx, d_shift);
+  pa.idx_rel = 0;                            // one chunk starting at atom 0: relative = absolute
   pa.n_rows = h->n_basic; pa.c0 = 0; pa.c1 = (int)N; pa.M = M; pa.kmap = pl.sliced ? h->d_kmapS : h->d_kmapF;
   {
     cudaError_t e = pl.sliced ? h->pl->moments_s(pa, st) : h->pl->moments(pa, pl.P, st);

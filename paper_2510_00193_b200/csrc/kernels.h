@@ -96,12 +96,16 @@ cudaError_t launch_ginit(double *G, int n_cut_rows, int n_basic, int ncol, const
                          cudaStream_t st);
 // dst[row][col] (leading dimension ld) = tiled src[tiles][rows][128], or the transpose dst[col][row] (ld = row length)
 cudaError_t launch_untile(const double *src, int rows, long long ncol, double *dst, long long ld, int transpose, cudaStream_t st);
-// out[p] = idx[p] | image_code(shift[p]) << 27; pairs with a shift outside {-1,0,1}^3 or an index outside [0, n_atoms)
-// are dropped and counted in *flag
-cudaError_t launch_pack_pairs(const int *idx, const signed char *shift, long long nnz, long long n_atoms, int *out, int *flag,
-                              cudaStream_t st);
-// F_k = sum_p d[p] - d[rev[p]] over row k (warp per atom, fixed order)
-cudaError_t launch_gather(const long long *off, const int *rev, const double *d4, int n, double *F, cudaStream_t st);
+// the pairs [off[c0], off[c1]) of one chunk: packed words (or plain indices when shift == null; out may be null) into
+// out[p - off[c0]], at most cap; touch = bitmap of kTouchWords x 32 bits marking the blocks of 2^touch_shift(n_atoms)
+// atoms that hold a neighbour of the chunk
+constexpr int kTouchWords = 512;
+inline int touch_shift(long long n_atoms) { int s = 6; while ((n_atoms >> s) >= kTouchWords * 32) ++s; return s; }
+cudaError_t launch_pack_pairs_chunk(const long long *off, int c0, int c1, const int *idx, const signed char *shift, long long n_atoms,
+                                    long long cap, int *out, int *flag, unsigned *touch, cudaStream_t st);
+// F_k -= sum over the neighbours j in the chunk of d4[rev], for every atom k of a touched block
+cudaError_t launch_gather_chunk(const long long *off, const int *idx, const int *rev, const double *d4, long long d4_cap, int c0,
+                                int c1, int n_atoms, const unsigned *touch, double *F, cudaStream_t st);
 // out[c] = sum_i in[i*stride + c] for c < ncomp <= 8, fixed order; scratch: 256 x 8 doubles (or null)
 cudaError_t launch_reduce(const double *in, long long n, int stride, int ncomp, double *out, double *scratch,
                           cudaStream_t st);

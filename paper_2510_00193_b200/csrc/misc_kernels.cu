@@ -2,6 +2,7 @@
 // gather over the reverse-neighbour index (a8), fixed-order reductions of E, virial and B.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <atomic>
 
 #include "kernels.h"
@@ -23,18 +24,54 @@ __global__ void k_pack(const double *__restrict__ pos, const int *__restrict__ t
   o[1] = make_double2(pos[3 * (size_t)i + 2], (double)type[i]);
 }
 
-// packed neighbour word j | code << 27 (pair_kernels.cuh): one 4-byte load per pair in K1 / K3 instead of
-// an index and three shift bytes, and the shift vector becomes a table lookup.  The word has room for shifts in
-// {-1,0,1}^3 and indices below 2^27 only: anything else (and j outside [0, n_atoms)) is counted in *flag
-// (MTP_INFO_INPUT_ERRORS) and the pair is dropped (word -1) instead of aliasing to another image or atom.
-__global__ void k_pack_pairs(const int *__restrict__ idx, const signed char *__restrict__ shift, long long nnz,
-                             long long n_atoms, int *__restrict__ out, int *__restrict__ flag) {
-  const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (p >= nnz) return;
-  const int s0 = shift[3 * p], s1 = shift[3 * p + 1], s2 = shift[3 * p + 2], j = idx[p];
-  const bool ok = s0 >= -1 && s0 <= 1 && s1 >= -1 && s1 <= 1 && s2 >= -1 && s2 <= 1 && j >= 0 && j < n_atoms;
-  if (!ok) { atomicAdd(flag, 1); out[p] = -1; return; }
-  out[p] = (int)((unsigned)j | ((unsigned)shift_code(s0, s1, s2) << kIdxBits));
+// Packed neighbour word j | code << 27 (pair_kernels.cuh): one 4-byte load per pair in K1 / K3 instead of an index and
+// three shift bytes, and the shift vector becomes a table lookup.  The word has room for shifts in {-1,0,1}^3 and
+// indices below 2^27 only: anything else (and j outside [0, n_atoms)) is counted in flag[0] (MTP_INFO_INPUT_ERRORS) and
+// the pair is dropped (word -1) instead of aliasing to another image or atom.
+// k_pack_pairs_chunk does this for the pairs of one chunk of atoms [c0, c1): out[p - off[c0]] for p in [off[c0], off[c1]), at most cap
+// of them (the excess is counted in flag[1]).  The pair range is read on the device: no host synchronisation.
+// Bit (j >> tshift) of the touch bitmap (kTouchWords x 32 bits, tshift chosen so that all atoms fit) is set for every
+// neighbour j of the chunk: the force assembly walks only blocks of rows that hold a neighbour in the chunk.
+__global__ void __launch_bounds__(256) k_pack_pairs_chunk(const long long *__restrict__ off, int c0, int c1, const int *__restrict__ idx,
+                                                          const signed char *__restrict__ shift, long long n_atoms, long long cap,
+                                                          int *__restrict__ out, int *__restrict__ flag, unsigned *__restrict__ touch,
+                                                          int tshift) {
+  __shared__ unsigned bits[kTouchWords];             // this block's share of the touch bitmap: merged into the global one at the end
+  for (int i = threadIdx.x; i < kTouchWords; i += blockDim.x) bits[i] = 0u;
+  __syncthreads();
+  const long long p0 = off[c0], n = off[c1] - p0;
+  for (long long q0 = (long long)blockIdx.x * (4 * blockDim.x) + threadIdx.x; q0 < n; q0 += (long long)gridDim.x * (4 * blockDim.x)) {
+  // four pairs per thread, a block stride apart: the loads of all four are in flight together
+  int j[4], s0[4], s1[4], s2[4];
+#pragma unroll
+  for (int u = 0; u < 4; ++u) {
+    const long long q = q0 + (long long)u * blockDim.x;
+    j[u] = -1; s0[u] = s1[u] = s2[u] = 0;
+    if (q < n) {
+      j[u] = idx[p0 + q];
+      if (shift) { s0[u] = shift[3 * (p0 + q)]; s1[u] = shift[3 * (p0 + q) + 1]; s2[u] = shift[3 * (p0 + q) + 2]; }
+    }
+  }
+#pragma unroll
+  for (int u = 0; u < 4; ++u) {
+    const long long q = q0 + (long long)u * blockDim.x;
+    if (q >= n) continue;
+    const bool ok = j[u] >= 0 && j[u] < n_atoms && s0[u] >= -1 && s0[u] <= 1 && s1[u] >= -1 && s1[u] <= 1 && s2[u] >= -1 && s2[u] <= 1;
+    int word = -1;
+    if (!ok) atomicAdd(flag, 1);
+    else {
+      word = shift ? (int)((unsigned)j[u] | ((unsigned)shift_code(s0[u], s1[u], s2[u]) << kIdxBits)) : j[u];
+      const int b = j[u] >> tshift;
+      atomicOr(&bits[b >> 5], 1u << (b & 31));
+    }
+    if (out) {
+      if (q < cap) out[q] = word;
+      else atomicAdd(flag + 1, 1);
+    }
+  }
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < kTouchWords; i += blockDim.x) if (bits[i]) atomicOr(touch + i, bits[i]);
 }
 
 // G of a partitioned table before the group programs accumulate into it: dE_i/d(cut) for the packed moments
@@ -71,28 +108,45 @@ __global__ void k_zero(double *p, long long n) {
   if (i < n) p[i] = 0.0;
 }
 
-// a8 gather: F_k = sum_{p in row k} ( d[p] - d[rev[p]] ); one warp per atom, lanes over the
-// row, xor-shuffle tree -> the summation order is fixed, the result bit-reproducible (G19).
-__global__ void __launch_bounds__(256) k_gather(const long long *__restrict__ off, const int *__restrict__ rev,
-                                                const double *__restrict__ d4, int n, double *__restrict__ F) {
-  const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-  if (warp >= n) return;
-  const long long beg = off[warp], end = off[warp + 1];
-  double fx = 0, fy = 0, fz = 0;
+// a8 with bounded per-pair scratch (SURVEY.md 8(a) note on a8 + a10, design (ii)): the pair kernel of the chunk
+// [c0, c1) has written d4[p - off[c0]] for the chunk's pairs and added each atom's own sum to F; here every atom k
+// with a neighbour j in the chunk subtracts d_jk, found through rev.  One warp per atom, lanes over the row,
+// xor-shuffle tree, one read-modify-write of F_k per chunk: the chunks come in stream order, so the sum has a fixed
+// order and is bit-reproducible (G19).  Blocks of 2^tshift rows without a neighbour in the chunk (touch bitmap
+// written by k_pack_pairs_chunk) are skipped without reading their rows.
+__global__ void __launch_bounds__(256) k_gather_chunk(const long long *__restrict__ off, const int *__restrict__ idx,
+                                                      const int *__restrict__ rev, const double *__restrict__ d4, long long d4_cap,
+                                                      int c0, int c1, int n_atoms, const unsigned *__restrict__ touch, int tshift,
+                                                      double *__restrict__ F) {
+  const int lane = threadIdx.x & 31;
+  const bool all = c0 == 0 && c1 == n_atoms;       // a single chunk: every neighbour is in it, the index test is not needed
+  const long long p0 = off[c0];
   const double2 *d = reinterpret_cast<const double2 *>(d4);
-  for (long long p = beg + lane; p < end; p += 32) {
-    const long long q = rev[p];
-    const double2 a0 = d[2 * p], a1 = d[2 * p + 1];
-    const double2 b0 = __ldg(d + 2 * q), b1 = __ldg(d + 2 * q + 1);
-    fx += a0.x - b0.x; fy += a0.y - b0.y; fz += a1.x - b1.x;
-  }
+  for (int k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; k < n_atoms; k += (gridDim.x * blockDim.x) >> 5) {
+    if (!((touch[(k >> tshift) >> 5] >> ((k >> tshift) & 31)) & 1u)) continue;
+    const long long beg = off[k], end = off[k + 1];
+    double fx = 0, fy = 0, fz = 0;
+    bool any = false;
+    for (long long p = beg + lane; p < end; p += 32) {
+      const int j = all ? c0 : idx[p];
+      if (j >= c0 && j < c1) {
+        const long long q = rev[p] - p0;
+        if (q >= 0 && q < d4_cap) {
+          const double2 b0 = __ldg(d + 2 * q), b1 = __ldg(d + 2 * q + 1);
+          fx -= b0.x; fy -= b0.y; fz -= b1.x;
+        }
+        any = true;
+      }
+    }
+    any = __any_sync(0xffffffffu, any);
 #pragma unroll
-  for (int o = 16; o >= 1; o >>= 1) {
-    fx += __shfl_xor_sync(0xffffffffu, fx, o);
-    fy += __shfl_xor_sync(0xffffffffu, fy, o);
-    fz += __shfl_xor_sync(0xffffffffu, fz, o);
+    for (int o = 16; o >= 1; o >>= 1) {
+      fx += __shfl_xor_sync(0xffffffffu, fx, o);
+      fy += __shfl_xor_sync(0xffffffffu, fy, o);
+      fz += __shfl_xor_sync(0xffffffffu, fz, o);
+    }
+    if (lane == 0 && any) { F[3 * (size_t)k] += fx; F[3 * (size_t)k + 1] += fy; F[3 * (size_t)k + 2] += fz; }
   }
-  if (lane == 0) { F[3 * (size_t)warp] = fx; F[3 * (size_t)warp + 1] = fy; F[3 * (size_t)warp + 2] = fz; }
 }
 
 // out[blockIdx.x][c] = sum over this block's share of i of in[i*stride + c], c < ncomp <= 8.
@@ -142,13 +196,6 @@ cudaError_t launch_pack(const double *pos, const int *type, int n, double *pos4,
   count_launch();
   return cudaGetLastError();
 }
-cudaError_t launch_pack_pairs(const int *idx, const signed char *shift, long long nnz, long long n_atoms, int *out, int *flag,
-                              cudaStream_t st) {
-  if (nnz <= 0) return cudaSuccess;
-  k_pack_pairs<<<(unsigned)((nnz + 255) / 256), 256, 0, st>>>(idx, shift, nnz, n_atoms, out, flag);
-  count_launch();
-  return cudaGetLastError();
-}
 cudaError_t launch_untile(const double *src, int rows, long long ncol, double *dst, long long ld, int transpose, cudaStream_t st) {
   if (ncol <= 0 || rows <= 0) return cudaSuccess;
   k_untile<<<dim3((unsigned)((ncol + 127) / 128), rows), 128, 0, st>>>(src, rows, ncol, dst, ld, transpose);
@@ -174,16 +221,27 @@ cudaError_t launch_zero(double *p, long long n, cudaStream_t st) {
   count_launch();
   return cudaGetLastError();
 }
-cudaError_t launch_gather(const long long *off, const int *rev, const double *d4, int n, double *F,
-                          cudaStream_t st) {
-  if (n <= 0) return cudaSuccess;
-  k_gather<<<(n + 7) / 8, 256, 0, st>>>(off, rev, d4, n, F);
+cudaError_t launch_pack_pairs_chunk(const long long *off, int c0, int c1, const int *idx, const signed char *shift, long long n_atoms,
+                                    long long cap, int *out, int *flag, unsigned *touch, cudaStream_t st) {
+  if (c1 <= c0) return cudaSuccess;
+  cudaError_t e = cudaMemsetAsync(touch, 0, kTouchWords * sizeof(unsigned), st);
+  if (e != cudaSuccess) return e;
+  // the pair count of the chunk lives on the device: a persistent grid strides over it
+  const long long blocks = std::min<long long>(148 * 8, std::max<long long>(1, (cap + 1023) / 1024));
+  k_pack_pairs_chunk<<<(unsigned)blocks, 256, 0, st>>>(off, c0, c1, idx, shift, n_atoms, cap, out, flag, touch, touch_shift(n_atoms));
+  count_launch();
+  return cudaGetLastError();
+}
+cudaError_t launch_gather_chunk(const long long *off, const int *idx, const int *rev, const double *d4, long long d4_cap, int c0,
+                                int c1, int n_atoms, const unsigned *touch, double *F, cudaStream_t st) {
+  if (c1 <= c0) return cudaSuccess;
+  k_gather_chunk<<<148 * 8, 256, 0, st>>>(off, idx, rev, d4, d4_cap, c0, c1, n_atoms, touch, touch_shift(n_atoms), F);
   count_launch();
   return cudaGetLastError();
 }
 cudaError_t launch_reduce(const double *in, long long n, int stride, int ncomp, double *out, double *scratch,
                           cudaStream_t st) {
-  if (n > 64 * 1024 && scratch) {
+  if (n > 4 * 1024 && scratch) {          // one block alone is latency-bound: 82 us for the 32 768 virial partials of config 4
     k_reduce_rows<<<kReduceBlocks, 1024, 0, st>>>(in, n, stride, ncomp, scratch);
     count_launch();
     k_reduce_rows<<<1, 1024, 0, st>>>(scratch, kReduceBlocks, 8, ncomp, out);

@@ -23,8 +23,13 @@ struct PairArgs {
   const int *kmap;           // [NS][NSLOT] slot -> packed component of the table, or -1
   double *M;                 // K1 out: tiled [tiles][n_rows][128], column = atom - c0 (kTile)
   const double *G;           // K3 in : same layout
-  double *d4;                // K3 out (gather mode): [nnz][4], or null
-  double *F;                 // K3 out (atomic mode): [N][3], or null
+  double *d4;                // K3 out (gather mode): [d4_cap][4] records of THIS CHUNK's pairs (index p - off[c0]), or null
+  long long d4_cap;          // pairs the chunk's d4 buffer holds; a chunk with more sets flag[1] and drops the excess
+  int *flag;                 // device error counters: [0] rejected input pairs, [1] per-pair scratch overflow
+  int idx_rel;               // 1: idx holds this chunk's pairs only (index p - off[c0]); 0: the whole list
+  long long idx_cap;         // entries idx holds (pairs beyond are treated as absent: their chunk overflowed the scratch)
+  double *F;                 // K3 out: [N][3]; atomic mode: every pair is scattered with fp64 atomics; gather mode: F_i += the sum of
+                             // the atom's own pairs (the reaction terms come from k_gather_chunk)
   double *wpart;             // K3 out: [gridDim.x][8] virial partials
   int n_rows;                // rows of M / G (n_basic)
   int c0, c1;                // atom range of this chunk

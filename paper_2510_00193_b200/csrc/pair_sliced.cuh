@@ -103,13 +103,16 @@ struct STile {
   static constexpr int STAGE = 2 * NT * 4 + (3 * NT + 1) / 2 + 32 * 4;   // two position buffers (32 B per thread), three word buffers,
                                                                          // the 32 centre-atom records (x, y, z, species)
   static constexpr int CTA1 = 2 * TILE1 + STAGE, CTA3 = 2 * TILE3 + DPART + STAGE;       // the tile is double-buffered
-  // CTAs per SM the register allocation aims at: 128 registers per thread while a slice has <= 40 components
-  static constexpr int MINB = Slicing<LEV, NSL>::NSLOT <= 40 ? (512 / NT > 0 ? 512 / NT : 1) : 1;
+  // CTAs per SM the register allocation aims at while a slice has <= 40 components: K1 128 registers per thread
+  // (16 warps per SM); K3 168 (12 warps): with 128 its force / virial accumulators spill (measured at config 4:
+  // K1 1.53 / 1.70 ms and K3 2.97 / 2.71 ms per step with 16 / 12 warps)
+  static constexpr int MINB1 = Slicing<LEV, NSL>::NSLOT <= 40 ? (512 / NT > 0 ? 512 / NT : 1) : 1;
+  static constexpr int MINB3 = Slicing<LEV, NSL>::NSLOT <= 40 ? (384 / NT > 0 ? 384 / NT : 1) : 1;
 };
 
 // cp.async staging of one pair per thread (the scheme of pair_tiled.cuh with one slot per thread)
 __device__ __forceinline__ void stage_word1(const PairArgs &a, long long beg, int n_nb, int k, int *slot) {
-  if (k < n_nb) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(slot)), "l"(a.idx + beg + k));
+  if (k < n_nb && beg + k < a.idx_cap) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(slot)), "l"(a.idx + beg + k));
   else *slot = -1;
 }
 __device__ __forceinline__ void stage_pos1(const PairArgs &a, int w, double *slot, int nt) {
@@ -280,7 +283,7 @@ __device__ __forceinline__ void k3_dispatch(int slice, const double *g, const do
 
 // ------------------------------------------------------------------------------ K1
 template <int LEV, int NSL, int NB>
-__global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB) k_moments_s(const PairArgs a) {
+__global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB1) k_moments_s(const PairArgs a) {
   using St = Stair<LEV>;
   using Sl = Slicing<LEV, NSL>;
   using Tl = STile<LEV, NSL>;
@@ -301,6 +304,7 @@ __global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB) k_moments_s(c
   if (atom0 + pa < a.c1) {
     beg = a.off[atom0 + pa];
     n_nb = (int)(a.off[atom0 + pa + 1] - beg);
+    if (a.idx_rel) beg -= a.off[a.c0];           // the neighbour words of this chunk start at 0
   }
   // the centre atoms' records live in shared memory: phase A reads its atom's (a broadcast) instead of holding
   // x, y, z, species in registers across phase B
@@ -364,7 +368,7 @@ __global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB) k_moments_s(c
 
 // ------------------------------------------------------------------------------ K3
 template <int LEV, int NSL, bool ATOMIC, int NB>
-__global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB) k_pairgrad_s(const PairArgs a) {
+__global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB3) k_pairgrad_s(const PairArgs a) {
   using St = Stair<LEV>;
   using Sl = Slicing<LEV, NSL>;
   using Tl = STile<LEV, NSL>;
@@ -380,11 +384,13 @@ __global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB) k_pairgrad_s(
   const int lane = threadIdx.x & 31, slice = threadIdx.x >> 5;
   const int atom0 = a.c0 + blockIdx.x * 32;
   const int pa = threadIdx.x / TN, pk = threadIdx.x % TN;
-  long long beg = 0;
+  long long beg = 0, dbeg = 0;
   int n_nb = 0;
   if (atom0 + pa < a.c1) {
     beg = a.off[atom0 + pa];
     n_nb = (int)(a.off[atom0 + pa + 1] - beg);
+    dbeg = beg - a.off[a.c0];                    // d4 holds this chunk's pairs only
+    if (a.idx_rel) beg = dbeg;
   }
   double *ctr = reinterpret_cast<double *>(wst - threadIdx.x + 3 * NT + (NT & 1));      // centre-atom records, as in K1
   if (threadIdx.x < 32) {
@@ -470,9 +476,12 @@ __global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB) k_pairgrad_s(
           }
           Fx += dx; Fy += dy; Fz += dz;
         } else {
-          double2 *o = reinterpret_cast<double2 *>(a.d4) + 2 * (size_t)(beg + k);
-          o[0] = make_double2(dx, dy);
-          o[1] = make_double2(dz, 0.0);
+          if (dbeg + k < a.d4_cap) {
+            double2 *o = reinterpret_cast<double2 *>(a.d4) + 2 * (size_t)(dbeg + k);
+            o[0] = make_double2(dx, dy);
+            o[1] = make_double2(dz, 0.0);
+            Fx += dx; Fy += dy; Fz += dz;          // the atom's own pairs are summed here, in fixed order
+          } else atomicAdd(a.flag + 1, 1);
         }
         W[0] = fma(-x, dx, W[0]); W[1] = fma(-y, dy, W[1]); W[2] = fma(-z, dz, W[2]);
         W[3] = fma(-x, dy, W[3]); W[4] = fma(-x, dz, W[4]); W[5] = fma(-y, dz, W[5]);
@@ -482,7 +491,7 @@ __global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB) k_pairgrad_s(
     buf ^= 1;
     __syncthreads();
   }
-  if (ATOMIC) {
+  {
 #pragma unroll
     for (int o = 1; o < TN; o <<= 1) {                             // the TN threads of an atom are consecutive lanes
       Fx += __shfl_xor_sync(0xffffffffu, Fx, o);
@@ -490,9 +499,9 @@ __global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB) k_pairgrad_s(
       Fz += __shfl_xor_sync(0xffffffffu, Fz, o);
     }
     if (atom0 + pa < a.c1 && pk == 0) {
-      atomicAdd(a.F + 3 * (size_t)(atom0 + pa), Fx);
-      atomicAdd(a.F + 3 * (size_t)(atom0 + pa) + 1, Fy);
-      atomicAdd(a.F + 3 * (size_t)(atom0 + pa) + 2, Fz);
+      double *Fo = a.F + 3 * (size_t)(atom0 + pa);
+      if (ATOMIC) { atomicAdd(Fo, Fx); atomicAdd(Fo + 1, Fy); atomicAdd(Fo + 2, Fz); }
+      else { Fo[0] += Fx; Fo[1] += Fy; Fo[2] += Fz; }              // one thread per atom, chunks in stream order: deterministic
     }
   }
   // virial partial of this block, fixed reduction order (deterministic)

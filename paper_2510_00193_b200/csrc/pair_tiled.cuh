@@ -46,7 +46,7 @@ __device__ __forceinline__ void stage_words(const PairArgs &a, long long beg, in
   const unsigned s0 = (unsigned)__cvta_generic_to_shared(slots);
 #pragma unroll
   for (int u = 0; u < 4; ++u) {
-    if (k0 + u < n_nb) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(s0 + 4 * u), "l"(a.idx + beg + k0 + u));
+    if (k0 + u < n_nb && beg + k0 + u < a.idx_cap) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(s0 + 4 * u), "l"(a.idx + beg + k0 + u));
     else slots[u] = -1;
   }
 }
@@ -130,6 +130,7 @@ __global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB1) k_moments_
     load_pos4(a.pos4, atom, xi, yi, zi, ti);
     beg = a.off[atom];
     n_nb = (int)(a.off[atom + 1] - beg);
+    if (a.idx_rel) beg -= a.off[a.c0];           // the neighbour words of this chunk start at 0
   }
   const int zi_s = (int)ti;
   const double rc2 = a.r_cut * a.r_cut;
@@ -238,7 +239,7 @@ __global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB3) k_pairgrad
   const bool act = atom < a.c1;
   double g[NSLOT];
   double xi = 0, yi = 0, zi = 0, ti = 0;
-  long long beg = 0;
+  long long beg = 0, dbeg = 0;
   int n_nb = 0;
   if (act) {
     const int *km = kmsm + slice * NSLOT;
@@ -251,6 +252,8 @@ __global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB3) k_pairgrad
     load_pos4(a.pos4, atom, xi, yi, zi, ti);
     beg = a.off[atom];
     n_nb = (int)(a.off[atom + 1] - beg);
+    dbeg = beg - a.off[a.c0];                    // d4 holds this chunk's pairs only
+    if (a.idx_rel) beg = dbeg;
   } else {
 #pragma unroll
     for (int s = 0; s < NSLOT; ++s) g[s] = 0.0;
@@ -365,7 +368,7 @@ __global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB3) k_pairgrad
         const double2 *xy = reinterpret_cast<const double2 *>(mine + kl * PD);
         const double2 p0 = xy[0], p1 = xy[1];
         const double x = p0.x, y = p0.y, z = p1.x;
-        const long long p = beg + k;
+        const long long p = dbeg + k;
         if (ATOMIC) {
           if (dx != 0.0 || dy != 0.0 || dz != 0.0) {
             const int j = (u == 0 ? jc4.x : (u == 1 ? jc4.y : (u == 2 ? jc4.z : jc4.w))) & kIdxMask;
@@ -375,16 +378,19 @@ __global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB3) k_pairgrad
           }
           Fx += dx; Fy += dy; Fz += dz;
         } else {
-          double2 *o = reinterpret_cast<double2 *>(a.d4) + 2 * (size_t)p;
-          o[0] = make_double2(dx, dy);
-          o[1] = make_double2(dz, 0.0);
+          if (p < a.d4_cap) {
+            double2 *o = reinterpret_cast<double2 *>(a.d4) + 2 * (size_t)p;
+            o[0] = make_double2(dx, dy);
+            o[1] = make_double2(dz, 0.0);
+            Fx += dx; Fy += dy; Fz += dz;          // the atom's own pairs are summed here, in fixed order
+          } else atomicAdd(a.flag + 1, 1);
         }
         W[0] = fma(-x, dx, W[0]); W[1] = fma(-y, dy, W[1]); W[2] = fma(-z, dz, W[2]);
         W[3] = fma(-x, dy, W[3]); W[4] = fma(-x, dz, W[4]); W[5] = fma(-y, dz, W[5]);
       }
     }
   }
-  if (ATOMIC) {
+  {
 #pragma unroll
     for (int o = 1; o < LPA; o <<= 1) {
       Fx += __shfl_xor_sync(0xffffffffu, Fx, o);
@@ -392,9 +398,9 @@ __global__ void __launch_bounds__(128, Tile<LEV, NSB, NSC, P>::MINB3) k_pairgrad
       Fz += __shfl_xor_sync(0xffffffffu, Fz, o);
     }
     if (act && q == 0) {
-      atomicAdd(a.F + 3 * (size_t)atom, Fx);
-      atomicAdd(a.F + 3 * (size_t)atom + 1, Fy);
-      atomicAdd(a.F + 3 * (size_t)atom + 2, Fz);
+      double *Fo = a.F + 3 * (size_t)atom;
+      if (ATOMIC) { atomicAdd(Fo, Fx); atomicAdd(Fo + 1, Fy); atomicAdd(Fo + 2, Fz); }
+      else { Fo[0] += Fx; Fo[1] += Fy; Fo[2] += Fz; }              // one thread per atom, chunks in stream order: deterministic
     }
   }
   // virial partial of this block, fixed reduction order (deterministic)

@@ -150,6 +150,26 @@ def test_rejected_neighbour_entries_are_counted(lib, torch):
     pot.close()
 
 
+def test_per_pair_scratch_is_bounded_by_the_chunk(lib, torch):
+    """a10 (north_star 'a chunk scheduler that bounds per-pair scratch'): with the paper's example
+    chunk of 32 768 atoms the workspace of config 4 (1 048 576 atoms, 47.2 M pairs) stays below 200 MB in the
+    deterministic force mode (d_ij for all pairs would be 1.5 GB); a chunk with more pairs than the scratch was sized
+    for is reported, not silently wrong."""
+    w = make_workload(1, n_basis_of(16), cells=5)
+    pot = gpu_pot(lib, w)
+    pot.set_option(lib.OPT_FORCE_MODE, lib.FORCE_GATHER)
+    pot.set_option(lib.OPT_CHUNK_ATOMS, 32768)
+    assert pot.workspace_bytes(1048576, 47194874) < 200e6
+    pot.set_option(lib.OPT_CHUNK_ATOMS, 0)
+    assert pot.workspace_bytes(1048576, 47194874) < 1.3e9        # automatic chunks (262 144 atoms): a quarter of the pairs
+    d = to_dev(w, torch)
+    pot.set_option(lib.OPT_CHUNK_ATOMS, 64)
+    pot.set_option(lib.OPT_CHUNK_PAIRS, 100)                      # far too small for 64 atoms x ~54 neighbours
+    pot.compute(d["pos"], d["types"], w.box, d["off"], d["idx"], d["shift"], d["rev"])
+    assert pot.get_option(lib.INFO_SCRATCH_OVERFLOW) > 0
+    pot.close()
+
+
 def test_chunked_equals_unchunked_and_gather_is_deterministic(lib, torch):
     w = make_workload(1, n_basis_of(16), cells=5)
     a, pot, d = run_gpu(lib, torch, w, opts={lib.OPT_FORCE_MODE: lib.FORCE_GATHER})
@@ -157,8 +177,14 @@ def test_chunked_equals_unchunked_and_gather_is_deterministic(lib, torch):
     assert np.array_equal(a["F"], b["F"]) and np.array_equal(a["Ei"], b["Ei"]) and np.array_equal(a["virial"], b["virial"])
     c, _, _ = run_gpu(lib, torch, w, pot=pot, opts={lib.OPT_CHUNK_ATOMS: 77})   # ragged last chunk
     assert np.array_equal(a["Ei"], c["Ei"])
-    assert np.array_equal(a["F"], c["F"])          # gather: same per-pair values, same order
+    # forces are assembled chunk by chunk in stream order (per-pair scratch exists for one chunk at a time): same
+    # per-pair values, another summation order -> equal to rounding, and bit-identical from run to run
+    assert np.allclose(a["F"], c["F"], rtol=0, atol=1e-13 * np.abs(a["F"]).max())
     assert np.allclose(a["virial"], c["virial"], rtol=1e-12)
+    c2, _, _ = run_gpu(lib, torch, w, pot=pot)
+    assert np.array_equal(c["F"], c2["F"]) and np.array_equal(c["virial"], c2["virial"])
+    assert pot.get_option(lib.INFO_SCRATCH_OVERFLOW) == 0 and pot.get_option(lib.INFO_INPUT_ERRORS) == 0
+    pot.set_option(lib.OPT_CHUNK_ATOMS, 0)
     # minimum image instead of explicit shifts gives the same pairs here (box > 2 R_cut)
     out = pot.compute(d["pos"], d["types"], w.box, d["off"], d["idx"], None, d["rev"])
     torch.cuda.synchronize()
