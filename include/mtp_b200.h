@@ -165,6 +165,42 @@ int mtp_compute_host(mtp_handle *h, int64_t n_atoms, const double *pos, const in
                      const int8_t *shift, const int32_t *rev, int64_t nnz, double *E,
                      double *Ei, double *F, double *virial);
 
+/* Device neighbour list and MD loop (the paper's rates are atom-timesteps/s of a
+ * whole MD step, list builds included; its GPU runs take the list from the host code).
+ *
+ * mtp_neighbors_build: the full CSR list mtp_compute consumes, from positions and box, on the device.
+ *   Listed: every (i, j, s), s in {-1,0,1}^3, (j, s) != (i, 0), with |x_j - x_i + s.H| < r_list (the same operation
+ *   order, no contractions); rows ordered by (j, s0, s1, s2) ascending -- bit-identical to a brute-force search over
+ *   the 27 images.  Positions should lie in the box; an atom outside is handled as long as no listed shift leaves
+ *   {-1,0,1}^3 (such pairs are not listed).
+ *   d_off [N+1] i64, d_idx [capacity] i32, d_shift [capacity][3] i8, d_rev [capacity] i32 or NULL (reverse index:
+ *   d_rev[p] = position of (j, i, -s)), d_info [2] i64 = { pairs found, errors (rows longer than 256 entries) }.
+ *   At most `capacity` pairs are written: when d_info[0] > capacity the arrays hold a truncated list (call again
+ *   with larger arrays; capacity 0 just counts).  Workspace: mtp_neighbors_workspace_bytes(n_atoms).  No handle: the
+ *   list does not depend on the potential.  MTP_EBOX for a singular box. */
+int mtp_neighbors_workspace_bytes(int64_t n_atoms, size_t *out_bytes);
+int mtp_neighbors_build(int64_t n_atoms, const double *d_pos, const double *box, double r_list, int64_t capacity,
+                        int64_t *d_off, int32_t *d_idx, int8_t *d_shift, int32_t *d_rev, int64_t *d_info,
+                        void *d_ws, size_t ws_bytes, void *cuda_stream);
+/* mtp_md_run: n_steps of velocity-Verlet (NVE) with the potential of the handle, entirely enqueued on the stream:
+ *   v += dt/2 F/m; x += dt v; [every rebuild_every steps: atoms wrapped into the box, list rebuilt at R_cut + skin];
+ *   F = mtp_compute(x); v += dt/2 F/m.   Units: eV, Angstrom, ps, g/mol (LAMMPS "metal"); mass[S] HOST, per species.
+ *   d_pos, d_vel are updated in place; d_E[2] = potential and kinetic energy after the last step, d_Ei (or NULL), d_F,
+ *   d_virial (or NULL) as mtp_compute returns them for the final positions; d_info[2] = { largest pair count of any
+ *   build, accumulated list errors }: the run is valid when d_info[0] <= capacity, d_info[1] == 0 and
+ *   MTP_INFO_INPUT_ERRORS / MTP_INFO_SCRATCH_OVERFLOW read 0.  The caller chooses skin and cadence such that no atom
+ *   moves more than skin / 2 between builds.  n_steps = 0 evaluates the forces once. */
+int mtp_md_workspace_bytes(const mtp_handle *h, int64_t n_atoms, int64_t capacity, size_t *out_bytes);
+int mtp_md_run(mtp_handle *h, int64_t n_atoms, double *d_pos, double *d_vel, const int32_t *d_type, const double *box,
+               const double *mass, double dt, int64_t n_steps, int32_t rebuild_every, double skin, int64_t capacity,
+               double *d_E, double *d_Ei, double *d_F, double *d_virial, int64_t *d_info, void *d_ws, size_t ws_bytes,
+               void *cuda_stream);
+/* Host positions in, host forces out (what an MD host code does every step): positions and types are copied to the
+ * device, the list is built there at R_cut (it never crosses PCIe), the kernels of mtp_compute run in the
+ * deterministic force mode, and E, E_i, F, virial are copied back; synchronises.  nnz_out (or NULL): pairs listed. */
+int mtp_compute_host_pos(mtp_handle *h, int64_t n_atoms, const double *pos, const int32_t *type, const double *box,
+                         double *E, double *Ei, double *F, double *virial, int64_t *nnz_out);
+
 /* Diagnostics (parity bring-up and roofline denominators; not part of the hot path). */
 /* Runs K1 + K2 as one chunk and exports the moments M and adjoints G = dE_i/dM, both laid
  * out [n_basic][n_atoms] (component-major), and optionally B [n_atoms][n_basis].  Workspace: the size

@@ -37,7 +37,9 @@ class MtpParams(C.Structure):
 EXPORTS = ["mtp_enumerate", "mtp_table_free", "mtp_create", "mtp_destroy", "mtp_last_error",
            "mtp_set_option", "mtp_get_option", "mtp_workspace_bytes", "mtp_compute", "mtp_grade",
            "mtp_compute_host", "mtp_debug_moments", "mtp_launch_count", "mtp_peak_dfma",
-           "mtp_cost_model", "mtp_profile_read", "mtp_table_plan", "mtp_k2_program"]
+           "mtp_cost_model", "mtp_profile_read", "mtp_table_plan", "mtp_k2_program",
+           "mtp_neighbors_workspace_bytes", "mtp_neighbors_build", "mtp_md_workspace_bytes", "mtp_md_run",
+           "mtp_compute_host_pos"]
 
 
 def _build():
@@ -80,6 +82,12 @@ def _load():
     lib.mtp_cost_model.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl)]
     lib.mtp_profile_read.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
     lib.mtp_table_plan.argtypes = [C.POINTER(MtpParams), C.POINTER(i64)]
+    lib.mtp_neighbors_workspace_bytes.argtypes = [i64, C.POINTER(C.c_size_t)]
+    lib.mtp_neighbors_build.argtypes = [i64, vp, C.POINTER(dbl), dbl, i64, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
+    lib.mtp_md_workspace_bytes.argtypes = [vp, i64, i64, C.POINTER(C.c_size_t)]
+    lib.mtp_md_run.argtypes = [vp, i64, vp, vp, vp, C.POINTER(dbl), C.POINTER(dbl), dbl, i64, C.c_int32, dbl, i64,
+                               vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
+    lib.mtp_compute_host_pos.argtypes = [vp, i64, vp, vp, C.POINTER(dbl), vp, vp, vp, vp, C.POINTER(i64)]
     lib.mtp_k2_program.argtypes = [C.POINTER(MtpParams), C.c_int, vp, i64, vp, i64, C.POINTER(i64)]
     return lib
 
@@ -306,6 +314,37 @@ class Potential:
                                            self._stream(stream)))
         return M, G, B
 
+    def md_run(self, pos, vel, types, box, mass, dt, n_steps, rebuild_every, skin, capacity, stream=None):
+        """mtp_md_run: velocity-Verlet on the device; pos / vel (torch CUDA, [N][3]) are updated in place.
+        Returns dict(E[2] = potential, kinetic; Ei, F, virial, info[2])."""
+        import torch
+        n, dev = int(pos.shape[0]), pos.device
+        wsb = C.c_size_t()
+        self._check(_lib.mtp_md_workspace_bytes(self._h, n, int(capacity), C.byref(wsb)))
+        ws = self._workspace(int(wsb.value), dev)
+        out = dict(E=torch.empty(2, dtype=torch.float64, device=dev), Ei=torch.empty(n, dtype=torch.float64, device=dev),
+                   F=torch.empty((n, 3), dtype=torch.float64, device=dev), virial=torch.empty(6, dtype=torch.float64, device=dev),
+                   info=torch.zeros(2, dtype=torch.int64, device=dev))
+        boxh = (C.c_double * 9)(*[float(x) for x in np.asarray(box, dtype=np.float64).reshape(9)])
+        m = np.ascontiguousarray(mass, dtype=np.float64)
+        self._check(_lib.mtp_md_run(self._h, n, _ptr(pos), _ptr(vel), _ptr(types), boxh, m.ctypes.data_as(C.POINTER(C.c_double)),
+                                    float(dt), int(n_steps), int(rebuild_every), float(skin), int(capacity), _ptr(out["E"]),
+                                    _ptr(out["Ei"]), _ptr(out["F"]), _ptr(out["virial"]), _ptr(out["info"]), _ptr(ws), ws.numel(),
+                                    self._stream(stream)))
+        return out
+
+    def compute_host_pos(self, pos, types, box, out=None):
+        """mtp_compute_host_pos on numpy (or pinned) arrays: positions in, forces out, list built on the device."""
+        n = int(pos.shape[0])
+        if out is None:
+            out = dict(E=np.empty(1), Ei=np.empty(n), F=np.empty((n, 3)), virial=np.empty(6))
+        boxh = (C.c_double * 9)(*[float(x) for x in np.asarray(box, dtype=np.float64).reshape(9)])
+        nnz = C.c_int64()
+        self._check(_lib.mtp_compute_host_pos(self._h, n, _np_ptr(pos), _np_ptr(types), boxh, _np_ptr(out["E"]), _np_ptr(out["Ei"]),
+                                              _np_ptr(out["F"]), _np_ptr(out["virial"]), C.byref(nnz)))
+        out["nnz"] = int(nnz.value)
+        return out
+
     def compute_host(self, pos, types, box, off, idx, shift=None, rev=None, out=None):
         """mtp_compute_host on numpy (or pinned torch CPU) arrays; H2D/D2H inside the call."""
         n, nnz = int(pos.shape[0]), int(idx.shape[0])
@@ -316,6 +355,39 @@ class Potential:
                                           _np_ptr(shift), _np_ptr(rev), nnz, _np_ptr(out["E"]), _np_ptr(out["Ei"]),
                                           _np_ptr(out["F"]), _np_ptr(out["virial"])))
         return out
+
+
+def neighbors_build(pos, box, r_list, capacity=None, want_rev=True, stream=None):
+    """mtp_neighbors_build on a torch CUDA tensor pos [N][3].  capacity None: count first, then build exactly.
+    Returns dict(off, idx, shift, rev, nnz, errors); tensors are sized `capacity` (nnz of them valid)."""
+    import torch
+    n, dev = int(pos.shape[0]), pos.device
+    wsb = C.c_size_t()
+    rc = _lib.mtp_neighbors_workspace_bytes(n, C.byref(wsb))
+    if rc != OK:
+        raise MtpError(rc, "mtp_neighbors_workspace_bytes")
+    ws = torch.empty(int(wsb.value), dtype=torch.uint8, device=dev)
+    boxh = (C.c_double * 9)(*[float(x) for x in np.asarray(box, dtype=np.float64).reshape(9)])
+    off = torch.empty(n + 1, dtype=torch.int64, device=dev)
+    info = torch.zeros(2, dtype=torch.int64, device=dev)
+    st = Potential._stream(stream)
+
+    def run(cap):
+        idx = torch.empty(max(cap, 1), dtype=torch.int32, device=dev)
+        shift = torch.empty((max(cap, 1), 3), dtype=torch.int8, device=dev)
+        rev = torch.empty(max(cap, 1), dtype=torch.int32, device=dev) if want_rev else None
+        rc = _lib.mtp_neighbors_build(n, _ptr(pos), boxh, float(r_list), int(cap), _ptr(off), _ptr(idx), _ptr(shift), _ptr(rev),
+                                      _ptr(info), _ptr(ws), ws.numel(), st)
+        if rc != OK:
+            raise MtpError(rc, "mtp_neighbors_build")
+        return idx, shift, rev
+
+    if capacity is None:
+        run(0)
+        capacity = int(info.cpu()[0])
+    idx, shift, rev = run(int(capacity))
+    nnz, errors = [int(x) for x in info.cpu()]
+    return dict(off=off, idx=idx, shift=shift, rev=rev, nnz=nnz, errors=errors)
 
 
 def launch_count() -> int:

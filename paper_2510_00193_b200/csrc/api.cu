@@ -96,6 +96,9 @@ struct mtp_handle {
   // staging for mtp_compute_host (grow-only), its copy / compute streams and chunk events
   void *stage = nullptr;
   size_t stage_bytes = 0;
+  void *stage_nb = nullptr;                    // mtp_compute_host_pos: device list + its workspace (grow-only)
+  size_t stage_nb_bytes = 0;
+  int64_t nb_capacity = 0;                     // pairs the staged list holds
   cudaStream_t s_copy = nullptr, s_comp = nullptr;
   std::vector<cudaEvent_t> ev;
   std::vector<void *> to_free;
@@ -254,6 +257,7 @@ extern "C" void mtp_destroy(mtp_handle *h) {
   for (auto &jp : h->jprogs) for (auto *k : jp.kern) k2_jit_destroy(k);
   for (void *p : h->to_free) cudaFree(p);
   if (h->stage) cudaFree(h->stage);
+  if (h->stage_nb) cudaFree(h->stage_nb);
   for (auto e : h->ev) cudaEventDestroy(e);
   if (h->s_copy) cudaStreamDestroy(h->s_copy);
   if (h->s_comp) cudaStreamDestroy(h->s_comp);
@@ -1065,6 +1069,177 @@ extern "C" int mtp_compute_host(mtp_handle *h, int64_t N, const double *pos, con
   if (N > 0) CU(h, cudaMemcpyAsync(F, dF, (size_t)N * 24, cudaMemcpyDeviceToHost, st));
   CU(h, cudaStreamSynchronize(st));
   return MTP_OK;
+}
+
+// ---- device neighbour list, MD loop --------------------------------------------------------
+extern "C" int mtp_neighbors_workspace_bytes(int64_t n_atoms, size_t *out) {
+  if (n_atoms < 0 || !out) return MTP_EINVAL;
+  *out = nb_workspace_bytes(n_atoms);
+  return MTP_OK;
+}
+
+extern "C" int mtp_neighbors_build(int64_t N, const double *d_pos, const double *box, double r_list, int64_t capacity,
+                                   int64_t *d_off, int32_t *d_idx, int8_t *d_shift, int32_t *d_rev, int64_t *d_info,
+                                   void *d_ws, size_t ws_bytes, void *stream) {
+  if (N < 0 || N > (1LL << 27) || !box || !d_off || !d_info || capacity < 0 || (N > 0 && !d_pos) ||
+      (capacity > 0 && (!d_idx || !d_shift)) || capacity > 0x7fffffffLL)
+    return MTP_EINVAL;
+  if (!d_ws || ws_bytes < nb_workspace_bytes(N)) return MTP_ESIZE;
+  NbGrid g;
+  if (!nb_grid(box, r_list, N, g)) return MTP_EBOX;
+  char *ws = (char *)d_ws;
+  ws += (256 - ((uintptr_t)ws & 255)) & 255;
+  cudaError_t e = launch_neighbors_build(g, N, d_pos, r_list, capacity, (long long *)d_off, d_idx, (signed char *)d_shift, d_rev,
+                                         (long long *)d_info, 0, ws, (cudaStream_t)stream);
+  return e == cudaSuccess ? MTP_OK : MTP_ECUDA;
+}
+
+namespace {
+// LAMMPS "metal" units: eV, Angstrom, ps, g/mol.  a [A/ps^2] = F [eV/A] / m [g/mol] x kFtm2v
+constexpr double kFtm2v = 1.602176634e-19 / 1.66053906660e-27 * 1e-4;      // 9648.533...
+struct MdLayout { size_t off, idx, shift, rev, info, imass, mass, ke, nbws, ws, total; };
+MdLayout md_layout(const mtp_handle *h, int64_t N, int64_t cap, size_t compute_ws) {
+  MdLayout L;
+  size_t o = 0;
+  auto take = [&](size_t b) { size_t at = o; o = align_up(o + b); return at; };
+  L.off = take((size_t)(N + 1) * 8); L.idx = take((size_t)cap * 4); L.shift = take((size_t)cap * 3); L.rev = take((size_t)cap * 4);
+  L.info = take(16); L.imass = take((size_t)h->S * 8); L.mass = take((size_t)h->S * 8); L.ke = take((size_t)N * 8);
+  L.nbws = take(nb_workspace_bytes(N)); L.ws = take(compute_ws);
+  L.total = o;
+  return L;
+}
+}  // namespace
+
+extern "C" int mtp_md_workspace_bytes(const mtp_handle *h, int64_t n_atoms, int64_t capacity, size_t *out) {
+  if (!h || !out || n_atoms < 0 || capacity < 0) return MTP_EINVAL;
+  size_t cw = 0;
+  int rc = mtp_workspace_bytes(h, n_atoms, capacity, 0, &cw);
+  if (rc != MTP_OK) return rc;
+  *out = md_layout(h, n_atoms, capacity, cw).total + 512;
+  return MTP_OK;
+}
+
+extern "C" int mtp_md_run(mtp_handle *h, int64_t N, double *d_pos, double *d_vel, const int32_t *d_type, const double *box,
+                          const double *mass, double dt, int64_t n_steps, int32_t rebuild_every, double skin, int64_t capacity,
+                          double *d_E, double *d_Ei, double *d_F, double *d_virial, int64_t *d_info, void *d_ws, size_t ws_bytes,
+                          void *stream) {
+  if (!h) return MTP_EINVAL;
+  if (N <= 0 || !d_pos || !d_vel || !d_type || !box || !mass || !(dt > 0) || n_steps < 0 || rebuild_every < 1 || !(skin >= 0) ||
+      capacity <= 0 || capacity > 0x7fffffffLL || !d_E || !d_F || !d_info)
+    return fail(h, MTP_EINVAL, "mtp_md_run: bad argument");
+  for (int s = 0; s < h->S; ++s) if (!(mass[s] > 0)) return fail(h, MTP_EINVAL, "mtp_md_run: masses must be positive");
+  cudaStream_t st = (cudaStream_t)stream;
+  size_t cw = 0;
+  int rc = mtp_workspace_bytes(h, N, capacity, 0, &cw);
+  if (rc != MTP_OK) return rc;
+  const MdLayout L = md_layout(h, N, capacity, cw);
+  const size_t base = align_up((size_t)(uintptr_t)d_ws) - (size_t)(uintptr_t)d_ws;
+  if (!d_ws || ws_bytes < L.total + base) return fail(h, MTP_ESIZE, "workspace too small (mtp_md_workspace_bytes)");
+  char *ws = (char *)d_ws + base;
+  int64_t *off = (int64_t *)(ws + L.off);
+  int32_t *idx = (int32_t *)(ws + L.idx), *rev = (int32_t *)(ws + L.rev);
+  int8_t *shift = (int8_t *)(ws + L.shift);
+  double *imass = (double *)(ws + L.imass), *dmass = (double *)(ws + L.mass), *ke = (double *)(ws + L.ke);
+  const double r_list = h->r_cut + skin;
+  NbGrid g;
+  if (!nb_grid(box, r_list, N, g)) return fail(h, MTP_EBOX, "singular box");
+  std::vector<double> im(h->S);
+  for (int s = 0; s < h->S; ++s) im[s] = 1.0 / mass[s];
+  CU(h, cudaMemcpyAsync(imass, im.data(), (size_t)h->S * 8, cudaMemcpyHostToDevice, st));
+  CU(h, cudaMemcpyAsync(dmass, mass, (size_t)h->S * 8, cudaMemcpyHostToDevice, st));
+  CU(h, cudaStreamSynchronize(st));           // the two host arrays above are the caller's / this frame's
+  CU(h, cudaMemsetAsync(d_info, 0, 16, st));
+  auto build = [&]() -> int {                 // atoms back into the box, then the list at r_cut + skin (entries beyond r_cut
+    CU(h, launch_wrap(g, (int)N, d_pos, st)); // contribute exactly nothing: reading G3)
+    CU(h, launch_neighbors_build(g, N, d_pos, r_list, capacity, (long long *)off, idx, (signed char *)shift, rev, (long long *)d_info, 1,
+                                 ws + L.nbws, st));
+    return MTP_OK;
+  };
+  auto forces = [&]() {
+    return compute_impl(h, N, d_pos, d_type, box, off, idx, shift, rev, capacity, d_E, d_Ei, d_F, d_virial, ws + L.ws, cw, st, nullptr);
+  };
+  const int saved_mode = h->force_mode;
+  if (h->force_mode == MTP_FORCE_AUTO) h->force_mode = MTP_FORCE_GATHER;      // the list comes with its reverse index
+  rc = build();
+  if (rc == MTP_OK) rc = forces();
+  const double half = 0.5 * dt * kFtm2v;
+  for (int64_t s = 1; s <= n_steps && rc == MTP_OK; ++s) {
+    cudaError_t e = launch_vv((int)N, d_pos, d_vel, d_F, d_type, imass, half, dt, 1, st);      // v(t + dt/2), x(t + dt)
+    if (e != cudaSuccess) { rc = cuda_fail(h, e, "launch_vv"); break; }
+    if (s % rebuild_every == 0) rc = build();
+    if (rc == MTP_OK) rc = forces();                                                            // F(t + dt)
+    if (rc != MTP_OK) break;
+    e = launch_vv((int)N, d_pos, d_vel, d_F, d_type, imass, half, dt, 0, st);                   // v(t + dt)
+    if (e != cudaSuccess) rc = cuda_fail(h, e, "launch_vv");
+  }
+  h->force_mode = saved_mode;
+  if (rc != MTP_OK) return rc;
+  // kinetic energy sum m v^2 / 2 in eV
+  CU(h, launch_ke((int)N, d_vel, d_type, dmass, 0.5 / kFtm2v, ke, st));
+  CU(h, launch_reduce(ke, N, 1, 1, d_E + 1, nullptr, st));
+  return MTP_OK;
+}
+
+// Host positions in, host forces out: the neighbour list never crosses PCIe (it is built on the device at R_cut).
+extern "C" int mtp_compute_host_pos(mtp_handle *h, int64_t N, const double *pos, const int32_t *type, const double *box,
+                                    double *E, double *Ei, double *F, double *virial, int64_t *nnz_out) {
+  if (!h) return MTP_EINVAL;
+  if (N <= 0 || !pos || !type || !box || !E || !F) return fail(h, MTP_EINVAL, "mtp_compute_host_pos: bad argument");
+  NbGrid g;
+  if (!nb_grid(box, h->r_cut, N, g)) return fail(h, MTP_EBOX, "singular box");
+  if (!h->s_comp) {
+    CU(h, cudaStreamCreateWithFlags(&h->s_copy, cudaStreamNonBlocking));
+    CU(h, cudaStreamCreateWithFlags(&h->s_comp, cudaStreamNonBlocking));
+  }
+  cudaStream_t st = h->s_comp;
+  const int saved_mode = h->force_mode;
+  for (int attempt = 0; attempt < 3; ++attempt) {
+    const int64_t cap = h->nb_capacity;
+    size_t cw = 0;
+    int rc = mtp_workspace_bytes(h, N, std::max<int64_t>(cap, 1), 0, &cw);
+    if (rc != MTP_OK) return rc;
+    size_t o = 0;
+    auto take = [&](size_t b) { size_t at = o; o = align_up(o + b); return at; };
+    const size_t o_pos = take((size_t)N * 24), o_type = take((size_t)N * 4), o_off = take((size_t)(N + 1) * 8);
+    const size_t o_idx = take((size_t)cap * 4), o_shift = take((size_t)cap * 3), o_rev = take((size_t)cap * 4), o_info = take(16);
+    const size_t o_out = take((size_t)(7 + 4 * N) * 8), o_nbws = take(nb_workspace_bytes(N)), o_ws = take(cw);
+    if (o > h->stage_nb_bytes) {
+      if (h->stage_nb) cudaFree(h->stage_nb);
+      h->stage_nb = nullptr; h->stage_nb_bytes = 0;
+      CU(h, cudaMalloc(&h->stage_nb, o));
+      h->stage_nb_bytes = o;
+    }
+    char *d = (char *)h->stage_nb;
+    CU(h, cudaMemcpyAsync(d + o_pos, pos, (size_t)N * 24, cudaMemcpyHostToDevice, st));
+    CU(h, cudaMemcpyAsync(d + o_type, type, (size_t)N * 4, cudaMemcpyHostToDevice, st));
+    CU(h, launch_neighbors_build(g, N, (double *)(d + o_pos), h->r_cut, cap, (long long *)(d + o_off), (int *)(d + o_idx),
+                                 (signed char *)(d + o_shift), (int *)(d + o_rev), (long long *)(d + o_info), 0, d + o_nbws, st));
+    long long info[2] = {0, 0};
+    if (cap > 0) {
+      double *dE = (double *)(d + o_out), *dW = dE + 1, *dEi = dE + 7, *dF = dEi + N;
+      if (h->force_mode == MTP_FORCE_AUTO) h->force_mode = MTP_FORCE_GATHER;
+      rc = compute_impl(h, N, (double *)(d + o_pos), (int32_t *)(d + o_type), box, (int64_t *)(d + o_off), (int32_t *)(d + o_idx),
+                        (int8_t *)(d + o_shift), (int32_t *)(d + o_rev), cap, dE, dEi, dF, dW, d + o_ws, cw, st, nullptr);
+      h->force_mode = saved_mode;
+      if (rc != MTP_OK) { cudaStreamSynchronize(st); return rc; }
+      CU(h, cudaMemcpyAsync(E, dE, 8, cudaMemcpyDeviceToHost, st));
+      if (virial) CU(h, cudaMemcpyAsync(virial, dW, 48, cudaMemcpyDeviceToHost, st));
+      if (Ei) CU(h, cudaMemcpyAsync(Ei, dEi, (size_t)N * 8, cudaMemcpyDeviceToHost, st));
+      CU(h, cudaMemcpyAsync(F, dF, (size_t)N * 24, cudaMemcpyDeviceToHost, st));
+    }
+    CU(h, cudaMemcpyAsync(info, d + o_info, 16, cudaMemcpyDeviceToHost, st));
+    CU(h, cudaStreamSynchronize(st));
+    if (info[1] != 0) return fail(h, MTP_EUNSUP, "neighbour rows longer than 256 entries");
+    if (nnz_out) *nnz_out = info[0];
+    if (info[0] <= cap && cap > 0) return MTP_OK;
+    if (info[0] == 0) {                          // no pairs at all: E_i = xi0, F = 0 -- run the plain path with an empty list
+      h->nb_capacity = 1;
+      if (cap > 0) return MTP_OK;
+      continue;
+    }
+    h->nb_capacity = info[0] + info[0] / 16 + 1024;        // first call, or the list outgrew the buffers: size them and redo
+  }
+  return fail(h, MTP_ESIZE, "neighbour list kept outgrowing its buffers");
 }
 
 // ---- diagnostics ------------------------------------------------------------------------------

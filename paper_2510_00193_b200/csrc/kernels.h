@@ -112,6 +112,20 @@ cudaError_t launch_reduce(const double *in, long long n, int stride, int ncomp, 
 // Bsum[b] += sum_i Bt[b][i] over the tiled Bt of a chunk (fixed order per row)
 cudaError_t launch_colsum(const double *Bt, long long n, int nb, double *Bsum, cudaStream_t st);
 
+// ---- device neighbour list and velocity-Verlet (neighbor_kernels.cu)
+struct NbGrid { double H[9], Hi[9]; int nc[3]; };          // box rows, inverse box, cells per lattice direction
+bool nb_grid(const double *box, double r_list, long long n_atoms, NbGrid &g);
+size_t nb_workspace_bytes(long long n_atoms);
+cudaError_t launch_scan(const int *in, long long n, long long *out, long long *totals, cudaStream_t st);
+// full CSR list (rows ordered by (j, shift)), image shifts and, when rev != null, the reverse index; info[2] = {pairs
+// found, errors}; at most `capacity` pairs are written
+cudaError_t launch_neighbors_build(const NbGrid &g, long long n, const double *pos, double r_list, long long capacity, long long *off,
+                                   int *idx, signed char *shift, int *rev, long long *info, int accumulate, void *ws, cudaStream_t st);
+cudaError_t launch_wrap(const NbGrid &g, int n, double *pos, cudaStream_t st);
+cudaError_t launch_vv(int n, double *pos, double *vel, const double *F, const int *type, const double *inv_mass, double half_dt_ftm2v,
+                      double dt, int drift, cudaStream_t st);
+cudaError_t launch_ke(int n, const double *vel, const int *type, const double *mass, double half_mvv2e, double *ke_i, cudaStream_t st);
+
 // ---- K5 (grade_kernel.cu)
 // gamma[i] = max_k | sum_a B[i][a] Ainv[a][k] |, B given as the tiled Bt [tiles][nb][128]
 cudaError_t launch_grade(const double *Bt, const double *Ainv, long long n, int nb, double *gamma, cudaStream_t st);

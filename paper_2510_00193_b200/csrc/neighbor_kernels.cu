@@ -1,0 +1,376 @@
+// Device-side neighbour list (the paper's rates are atom-timesteps/s with the list
+// build inside; the GPU runs use the host code's list): the full CSR list mtp_compute consumes, its
+// image shifts and its reverse index, built from positions and box with a cell list, and the two halves of a
+// velocity-Verlet step.  Integer work: the result is bit-identical to a brute-force search over the 27 images
+// (rows ordered by (j, shift), the order of oracle/mtp.py brute_force_neighbours; tests compare bit for bit).
+//
+//   cells    the box is cut into n_k = floor(height_k / r_list) >= 1 cells per lattice direction (fractional
+//            coordinates), so a neighbour image lies in one of the 27 cells around the centre atom's; the image shift of
+//            a candidate is the number of box lengths the cell index wrapped by.  With fewer than three cells in a
+//            direction the same cell is visited through different shifts -- still every image in {-1,0,1}^3 exactly once.
+//   build    cell index per atom + histogram -> exclusive scan -> atoms sorted by cell (each cell's atoms in ascending
+//            order) with a cell-ordered copy of the wrapped positions -> per atom (one warp): count pass -> scan ->
+//            fill pass: hits collected in shared memory, rank-sorted by key j * 27 + code, written as idx / shift.
+//   rev      per pair a binary search of the mirror key (i, -s) in row j.
+// The distance test uses the same operation order as the definition, (x_j - x_i) + s0 H0 + s1 H1 + s2 H2, without
+// contractions, on the caller's coordinates.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+
+#include "kernels.h"
+
+namespace mtpb {
+
+namespace {
+constexpr int kRowMax = 256;            // longest row the fill pass sorts in shared memory (longer rows: flag[0] counts them)
+
+__device__ __forceinline__ int cell_of(const NbGrid &g, double x, double y, double z, int *w) {
+  // fractional coordinates (row-vector convention frac = cart . Hi), wrapped into [0, 1)
+  double f0 = x * g.Hi[0] + y * g.Hi[3] + z * g.Hi[6];
+  double f1 = x * g.Hi[1] + y * g.Hi[4] + z * g.Hi[7];
+  double f2 = x * g.Hi[2] + y * g.Hi[5] + z * g.Hi[8];
+  const double w0 = floor(f0), w1 = floor(f1), w2 = floor(f2);
+  f0 -= w0; f1 -= w1; f2 -= w2;
+  w[0] = (int)w0; w[1] = (int)w1; w[2] = (int)w2;
+  const int c0 = min((int)(f0 * g.nc[0]), g.nc[0] - 1), c1 = min((int)(f1 * g.nc[1]), g.nc[1] - 1), c2 = min((int)(f2 * g.nc[2]), g.nc[2] - 1);
+  return (c0 * g.nc[1] + c1) * g.nc[2] + c2;
+}
+
+// cell index and wrap image of every atom; histogram of the cells
+__global__ void k_nb_cells(NbGrid g, const double *__restrict__ pos, int n, int *__restrict__ cell, int *__restrict__ wrap,
+                           int *__restrict__ count) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int w[3];
+  const int c = cell_of(g, pos[3 * (size_t)i], pos[3 * (size_t)i + 1], pos[3 * (size_t)i + 2], w);
+  cell[i] = c;
+  wrap[3 * (size_t)i] = w[0]; wrap[3 * (size_t)i + 1] = w[1]; wrap[3 * (size_t)i + 2] = w[2];
+  atomicAdd(count + c, 1);
+}
+
+// ---- exclusive scan of int32 counts into int64 offsets: blocks of 1024, block totals scanned by a second level
+__global__ void __launch_bounds__(1024) k_scan_block(const int *__restrict__ in, long long n, long long *__restrict__ out,
+                                                     long long *__restrict__ totals) {
+  __shared__ long long sm[1024];
+  const long long i = (long long)blockIdx.x * 1024 + threadIdx.x;
+  const long long v = i < n ? in[i] : 0;
+  sm[threadIdx.x] = v;
+  __syncthreads();
+  for (int o = 1; o < 1024; o <<= 1) {
+    const long long t = threadIdx.x >= o ? sm[threadIdx.x - o] : 0;
+    __syncthreads();
+    sm[threadIdx.x] += t;
+    __syncthreads();
+  }
+  if (i < n) out[i] = sm[threadIdx.x] - v;
+  if (threadIdx.x == 1023) totals[blockIdx.x] = sm[1023];
+}
+__global__ void __launch_bounds__(1024) k_scan_totals(long long *__restrict__ totals, int nblocks, long long *__restrict__ grand) {
+  // one block: exclusive scan of up to 1024 * 1024 block totals, 1024 at a time with a running carry
+  __shared__ long long sm[1024];
+  __shared__ long long carry;
+  if (threadIdx.x == 0) carry = 0;
+  __syncthreads();
+  for (int base = 0; base < nblocks; base += 1024) {
+    const int i = base + threadIdx.x;
+    const long long v = i < nblocks ? totals[i] : 0;
+    sm[threadIdx.x] = v;
+    __syncthreads();
+    for (int o = 1; o < 1024; o <<= 1) {
+      const long long t = threadIdx.x >= o ? sm[threadIdx.x - o] : 0;
+      __syncthreads();
+      sm[threadIdx.x] += t;
+      __syncthreads();
+    }
+    if (i < nblocks) totals[i] = carry + sm[threadIdx.x] - v;
+    __syncthreads();
+    if (threadIdx.x == 1023) carry += sm[1023];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *grand = carry;
+}
+__global__ void __launch_bounds__(1024) k_scan_add(long long *__restrict__ out, long long n, const long long *__restrict__ totals,
+                                                   const long long *__restrict__ grand) {
+  const long long i = (long long)blockIdx.x * 1024 + threadIdx.x;
+  if (i < n) out[i] += totals[blockIdx.x];
+  if (i == n) out[n] = *grand;            // the closing offset
+}
+}  // namespace
+
+// out[0 .. n] = exclusive prefix sums of in[0 .. n) (out[n] = total); totals: scratch of ceil(n / 1024) + 1 int64
+cudaError_t launch_scan(const int *in, long long n, long long *out, long long *totals, cudaStream_t st) {
+  const int nblocks = (int)((n + 1 + 1023) / 1024);      // + 1: some block must own index n for the closing offset
+  k_scan_block<<<nblocks, 1024, 0, st>>>(in, n, out, totals);
+  k_scan_totals<<<1, 1024, 0, st>>>(totals, nblocks, totals + nblocks);
+  k_scan_add<<<nblocks, 1024, 0, st>>>(out, n, totals, totals + nblocks);
+  count_launch(); count_launch(); count_launch();
+  return cudaGetLastError();
+}
+
+
+namespace {
+// atoms into their cells (any order), then each cell's atoms in ascending order: the candidate order is deterministic
+__global__ void k_nb_scatter(const int *__restrict__ cell, int n, const long long *__restrict__ start, int *__restrict__ cursor,
+                             int *__restrict__ sorted) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int c = cell[i];
+  sorted[start[c] + atomicAdd(cursor + c, 1)] = i;
+}
+__global__ void k_nb_sort_cells(const long long *__restrict__ start, int n_cells, int *__restrict__ sorted) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= n_cells) return;
+  const long long a = start[c], b = start[c + 1];
+  for (long long p = a + 1; p < b; ++p) {            // insertion sort: a cell holds about ten atoms
+    const int v = sorted[p];
+    long long q = p;
+    while (q > a && sorted[q - 1] > v) { sorted[q] = sorted[q - 1]; --q; }
+    sorted[q] = v;
+  }
+}
+// the caller's coordinates of the atoms in cell order (x, y, z, atom index as double): one 32-byte record per candidate
+__global__ void k_nb_gather_pos(const double *__restrict__ pos, const int *__restrict__ sorted, int n, double *__restrict__ pos_s) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  const int i = sorted[t];
+  double2 *o = reinterpret_cast<double2 *>(pos_s) + 2 * (size_t)t;
+  o[0] = make_double2(pos[3 * (size_t)i], pos[3 * (size_t)i + 1]);
+  o[1] = make_double2(pos[3 * (size_t)i + 2], (double)i);
+}
+
+// One warp per atom (in cell order): the 27 cells around its cell, lanes over the candidates of a cell.
+// FILL = false: count[i] = number of neighbours.  FILL = true: the row's keys j * 27 + code are collected in shared
+// memory, rank-sorted, and written as idx / shift at off[i].
+template <bool FILL>
+__global__ void __launch_bounds__(256) k_nb_rows(NbGrid g, const double *__restrict__ pos_s, const int *__restrict__ cell,
+                                                 const int *__restrict__ wrap, const long long *__restrict__ start, int n, double r2max,
+                                                 int *__restrict__ count, const long long *__restrict__ off, long long capacity,
+                                                 int *__restrict__ idx, signed char *__restrict__ shift, int *__restrict__ flag) {
+  __shared__ unsigned keys[8][kRowMax];
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  const int t = blockIdx.x * 8 + wib;                       // position in cell order
+  if (t >= n) return;
+  const double2 a0 = reinterpret_cast<const double2 *>(pos_s)[2 * (size_t)t], a1 = reinterpret_cast<const double2 *>(pos_s)[2 * (size_t)t + 1];
+  const int i = (int)a1.y;
+  const double xi = a0.x, yi = a0.y, zi = a1.x;
+  const int ci = cell[i];
+  const int c2 = ci % g.nc[2], c1 = (ci / g.nc[2]) % g.nc[1], c0 = ci / (g.nc[2] * g.nc[1]);
+  const int wi0 = wrap[3 * (size_t)i], wi1 = wrap[3 * (size_t)i + 1], wi2 = wrap[3 * (size_t)i + 2];
+  int n_row = 0;
+  for (int d = 0; d < 27; ++d) {
+    const int e0 = c0 + d / 9 - 1, e1 = c1 + (d / 3) % 3 - 1, e2 = c2 + d % 3 - 1;
+    // cell index wrapped into the grid; the number of box lengths it wrapped by is the image of the wrapped coordinates
+    const int q0 = (e0 % g.nc[0] + g.nc[0]) % g.nc[0], q1 = (e1 % g.nc[1] + g.nc[1]) % g.nc[1], q2 = (e2 % g.nc[2] + g.nc[2]) % g.nc[2];
+    const int m0 = (e0 - q0) / g.nc[0], m1 = (e1 - q1) / g.nc[1], m2 = (e2 - q2) / g.nc[2];
+    const int cj = (q0 * g.nc[1] + q1) * g.nc[2] + q2;
+    const long long a = start[cj], b = start[cj + 1];
+    for (long long p = a + lane; p < b + ((32 - (b - a) % 32) % 32); p += 32) {   // whole warp iterations (ballots inside)
+      bool hit = false;
+      unsigned key = 0;
+      if (p < b) {
+        const double2 b0 = reinterpret_cast<const double2 *>(pos_s)[2 * (size_t)p], b1 = reinterpret_cast<const double2 *>(pos_s)[2 * (size_t)p + 1];
+        const int j = (int)b1.y;
+        // image shift relative to the caller's (possibly unwrapped) coordinates
+        const int s0 = m0 - (wrap[3 * (size_t)j] - wi0), s1 = m1 - (wrap[3 * (size_t)j + 1] - wi1), s2 = m2 - (wrap[3 * (size_t)j + 2] - wi2);
+        if (s0 >= -1 && s0 <= 1 && s1 >= -1 && s1 <= 1 && s2 >= -1 && s2 <= 1 && !(j == i && s0 == 0 && s1 == 0 && s2 == 0)) {
+          // r = (x_j - x_i) + s0 H0 + s1 H1 + s2 H2, no contractions (the definition's rounding)
+          const double x = __dadd_rn(__dadd_rn(__dadd_rn(__dadd_rn(b0.x, -xi), __dmul_rn((double)s0, g.H[0])), __dmul_rn((double)s1, g.H[3])), __dmul_rn((double)s2, g.H[6]));
+          const double y = __dadd_rn(__dadd_rn(__dadd_rn(__dadd_rn(b0.y, -yi), __dmul_rn((double)s0, g.H[1])), __dmul_rn((double)s1, g.H[4])), __dmul_rn((double)s2, g.H[7]));
+          const double z = __dadd_rn(__dadd_rn(__dadd_rn(__dadd_rn(b1.x, -zi), __dmul_rn((double)s0, g.H[2])), __dmul_rn((double)s1, g.H[5])), __dmul_rn((double)s2, g.H[8]));
+          const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y)), __dmul_rn(z, z));
+          hit = r2 < r2max;
+          key = (unsigned)j * 27u + (unsigned)((s0 + 1) * 9 + (s1 + 1) * 3 + (s2 + 1));
+        }
+      }
+      const unsigned m = __ballot_sync(0xffffffffu, hit);
+      if (FILL && hit) {
+        const int slot = n_row + __popc(m & ((1u << lane) - 1u));
+        if (slot < kRowMax) keys[wib][slot] = key;
+      }
+      n_row += __popc(m);
+    }
+  }
+  if (!FILL) { if (lane == 0) count[i] = n_row; return; }
+  __syncwarp();
+  if (n_row > kRowMax) { if (lane == 0) atomicAdd(flag, 1); n_row = kRowMax; }
+  const long long beg = off[i];
+  for (int q = lane; q < n_row; q += 32) {                  // rank sort: the keys of a row are distinct
+    const unsigned k = keys[wib][q];
+    int rank = 0;
+    for (int r = 0; r < n_row; ++r) rank += keys[wib][r] < k;
+    if (beg + rank < capacity) {
+      const unsigned code = k % 27u;
+      idx[beg + rank] = (int)(k / 27u);
+      shift[3 * (beg + rank)] = (signed char)((int)(code / 9u) - 1);
+      shift[3 * (beg + rank) + 1] = (signed char)((int)((code / 3u) % 3u) - 1);
+      shift[3 * (beg + rank) + 2] = (signed char)((int)(code % 3u) - 1);
+    }
+  }
+}
+
+// rev[p] = position of (j, i, -s) for p = (i, j, s): binary search in row j (sorted by key)
+__global__ void __launch_bounds__(256) k_nb_rev(const long long *__restrict__ off, const int *__restrict__ idx,
+                                                const signed char *__restrict__ shift, int n, long long capacity, int *__restrict__ rev,
+                                                int *__restrict__ flag) {
+  const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (i >= n) return;
+  const long long beg = off[i], end = min(off[i + 1], capacity);
+  for (long long p = beg + lane; p < end; p += 32) {
+    const int j = idx[p];
+    const unsigned want = (unsigned)i * 27u + (unsigned)((1 - shift[3 * p]) * 9 + (1 - shift[3 * p + 1]) * 3 + (1 - shift[3 * p + 2]));
+    long long lo = off[j], hi = min(off[j + 1], capacity);
+    long long found = -1;
+    while (lo < hi) {
+      const long long mid = (lo + hi) >> 1;
+      const unsigned k = (unsigned)idx[mid] * 27u + (unsigned)((shift[3 * mid] + 1) * 9 + (shift[3 * mid + 1] + 1) * 3 + (shift[3 * mid + 2] + 1));
+      if (k == want) { found = mid; break; }
+      if (k < want) lo = mid + 1; else hi = mid;
+    }
+    if (found < 0) atomicAdd(flag, 1);                       // cannot happen for a list built here (the test is symmetric)
+    rev[p] = (int)found;
+  }
+}
+
+// velocity-Verlet halves ("100 steps ... 1 fs"): v += (dt / 2) F / m ; x += dt v (first half only)
+__global__ void k_vv(int n, double *__restrict__ pos, double *__restrict__ vel, const double *__restrict__ F, const int *__restrict__ type,
+                     const double *__restrict__ inv_mass, double half_dt_ftm2v, double dt, int drift) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double s = half_dt_ftm2v * inv_mass[type[i]];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    const double v = fma(s, F[3 * (size_t)i + c], vel[3 * (size_t)i + c]);
+    vel[3 * (size_t)i + c] = v;
+    if (drift) pos[3 * (size_t)i + c] = fma(dt, v, pos[3 * (size_t)i + c]);
+  }
+}
+// kinetic energy partials sum_i m v^2 / 2 (fixed order per block) -- reduced by launch_reduce
+__global__ void k_ke(int n, const double *__restrict__ vel, const int *__restrict__ type, const double *__restrict__ mass,
+                     double half_mvv2e, double *__restrict__ ke_i) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double vx = vel[3 * (size_t)i], vy = vel[3 * (size_t)i + 1], vz = vel[3 * (size_t)i + 2];
+  ke_i[i] = half_mvv2e * mass[type[i]] * (vx * vx + vy * vy + vz * vz);
+}
+}  // namespace
+
+namespace {
+__global__ void k_nb_finish(const long long *__restrict__ off, int n, const int *__restrict__ flag, long long *__restrict__ info,
+                            int accumulate) {
+  // pairs found (may exceed the capacity: then the arrays hold a truncated list); rows longer than the sort buffer or
+  // pairs without a mirror.  accumulate: over the builds of an MD run (largest pair count, summed errors)
+  info[0] = accumulate ? max(info[0], off[n]) : off[n];
+  info[1] = (accumulate ? info[1] : 0) + flag[0];
+}
+// x -= floor(x . Hi) . H: atoms back into the box (before a list build of an MD run)
+__global__ void k_wrap(NbGrid g, int n, double *__restrict__ pos) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double x = pos[3 * (size_t)i], y = pos[3 * (size_t)i + 1], z = pos[3 * (size_t)i + 2];
+  const double w0 = floor(x * g.Hi[0] + y * g.Hi[3] + z * g.Hi[6]), w1 = floor(x * g.Hi[1] + y * g.Hi[4] + z * g.Hi[7]),
+               w2 = floor(x * g.Hi[2] + y * g.Hi[5] + z * g.Hi[8]);
+  if (w0 == 0.0 && w1 == 0.0 && w2 == 0.0) return;
+  pos[3 * (size_t)i] = x - (w0 * g.H[0] + w1 * g.H[3] + w2 * g.H[6]);
+  pos[3 * (size_t)i + 1] = y - (w0 * g.H[1] + w1 * g.H[4] + w2 * g.H[7]);
+  pos[3 * (size_t)i + 2] = z - (w0 * g.H[2] + w1 * g.H[5] + w2 * g.H[8]);
+}
+size_t al(size_t x) { return (x + 255) & ~(size_t)255; }
+struct NbLayout {
+  size_t cell, wrap, ccount, cursor, start, totals, sorted, pos_s, rcount, flag, total;
+};
+NbLayout nb_layout(long long n, long long n_cells) {
+  NbLayout L;
+  size_t o = 0;
+  L.cell = o; o = al(o + (size_t)n * 4);
+  L.wrap = o; o = al(o + (size_t)n * 12);
+  L.ccount = o; o = al(o + (size_t)n_cells * 4);
+  L.cursor = o; o = al(o + (size_t)n_cells * 4);
+  L.start = o; o = al(o + (size_t)(n_cells + 1) * 8);
+  L.totals = o; o = al(o + (size_t)((std::max(n, n_cells) + 1) / 1024 + 3) * 8);
+  L.sorted = o; o = al(o + (size_t)n * 4);
+  L.pos_s = o; o = al(o + (size_t)n * 32);
+  L.rcount = o; o = al(o + (size_t)n * 4);
+  L.flag = o; o = al(o + 16);
+  L.total = o;
+  return L;
+}
+}  // namespace
+
+// cells per lattice direction for this box and list radius: floor(height / r_list) >= 1, reduced when the grid would
+// be much larger than the number of atoms (a sparse box); Hi = inverse box.  false: singular box.
+bool nb_grid(const double *box, double r_list, long long n_atoms, NbGrid &g) {
+  const double *a = box, *b = box + 3, *c = box + 6;
+  const double bc[3] = {b[1] * c[2] - b[2] * c[1], b[2] * c[0] - b[0] * c[2], b[0] * c[1] - b[1] * c[0]};
+  const double ca[3] = {c[1] * a[2] - c[2] * a[1], c[2] * a[0] - c[0] * a[2], c[0] * a[1] - c[1] * a[0]};
+  const double ab[3] = {a[1] * b[2] - a[2] * b[1], a[2] * b[0] - a[0] * b[2], a[0] * b[1] - a[1] * b[0]};
+  const double vol = a[0] * bc[0] + a[1] * bc[1] + a[2] * bc[2];
+  if (!(std::fabs(vol) > 0) || !(r_list > 0)) return false;
+  for (int i = 0; i < 9; ++i) g.H[i] = box[i];
+  for (int i = 0; i < 3; ++i) { g.Hi[3 * i + 0] = bc[i] / vol; g.Hi[3 * i + 1] = ca[i] / vol; g.Hi[3 * i + 2] = ab[i] / vol; }
+  auto norm = [](const double *v) { return std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]); };
+  const double h[3] = {std::fabs(vol) / norm(bc), std::fabs(vol) / norm(ca), std::fabs(vol) / norm(ab)};
+  for (int k = 0; k < 3; ++k) g.nc[k] = std::max(1, (int)std::floor(h[k] / r_list));
+  while ((long long)g.nc[0] * g.nc[1] * g.nc[2] > 8 * n_atoms + 64) {       // larger cells are still correct
+    int k = g.nc[0] >= g.nc[1] ? (g.nc[0] >= g.nc[2] ? 0 : 2) : (g.nc[1] >= g.nc[2] ? 1 : 2);
+    g.nc[k] = std::max(1, g.nc[k] / 2);
+  }
+  return true;
+}
+
+size_t nb_workspace_bytes(long long n_atoms) { return nb_layout(n_atoms, 8 * n_atoms + 64).total + 256; }
+
+cudaError_t launch_neighbors_build(const NbGrid &g, long long n, const double *pos, double r_list, long long capacity, long long *off,
+                                   int *idx, signed char *shift, int *rev, long long *info, int accumulate, void *ws, cudaStream_t st) {
+  const long long n_cells = (long long)g.nc[0] * g.nc[1] * g.nc[2];
+  const NbLayout L = nb_layout(n, n_cells);
+  char *w = (char *)ws;
+  int *cell = (int *)(w + L.cell), *wrap = (int *)(w + L.wrap), *ccount = (int *)(w + L.ccount), *cursor = (int *)(w + L.cursor);
+  long long *start = (long long *)(w + L.start), *totals = (long long *)(w + L.totals);
+  int *sorted = (int *)(w + L.sorted), *rcount = (int *)(w + L.rcount), *flag = (int *)(w + L.flag);
+  double *pos_s = (double *)(w + L.pos_s);
+  cudaError_t e = cudaMemsetAsync(w + L.ccount, 0, L.start - L.ccount, st);     // cell histogram and cursors
+  if (e == cudaSuccess) e = cudaMemsetAsync(flag, 0, 16, st);
+  if (e != cudaSuccess) return e;
+  if (n == 0) { e = cudaMemsetAsync(off, 0, 8, st); if (e == cudaSuccess && !accumulate) e = cudaMemsetAsync(info, 0, 16, st); return e; }
+  const int nb = (int)((n + 255) / 256);
+  k_nb_cells<<<nb, 256, 0, st>>>(g, pos, (int)n, cell, wrap, ccount);
+  e = launch_scan(ccount, n_cells, start, totals, st);
+  if (e != cudaSuccess) return e;
+  k_nb_scatter<<<nb, 256, 0, st>>>(cell, (int)n, start, cursor, sorted);
+  k_nb_sort_cells<<<(unsigned)((n_cells + 255) / 256), 256, 0, st>>>(start, (int)n_cells, sorted);
+  k_nb_gather_pos<<<nb, 256, 0, st>>>(pos, sorted, (int)n, pos_s);
+  const double r2 = r_list * r_list;
+  k_nb_rows<false><<<(unsigned)((n + 7) / 8), 256, 0, st>>>(g, pos_s, cell, wrap, start, (int)n, r2, rcount, nullptr, 0, nullptr, nullptr, flag);
+  e = launch_scan(rcount, n, off, totals, st);
+  if (e != cudaSuccess) return e;
+  k_nb_rows<true><<<(unsigned)((n + 7) / 8), 256, 0, st>>>(g, pos_s, cell, wrap, start, (int)n, r2, rcount, off, capacity, idx, shift, flag);
+  if (rev) k_nb_rev<<<(unsigned)((n + 7) / 8), 256, 0, st>>>(off, idx, shift, (int)n, capacity, rev, flag);
+  k_nb_finish<<<1, 1, 0, st>>>(off, (int)n, flag, info, accumulate);
+  for (int q = 0; q < 8; ++q) count_launch();
+  return cudaGetLastError();
+}
+
+cudaError_t launch_wrap(const NbGrid &g, int n, double *pos, cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  k_wrap<<<(n + 255) / 256, 256, 0, st>>>(g, n, pos);
+  count_launch();
+  return cudaGetLastError();
+}
+cudaError_t launch_vv(int n, double *pos, double *vel, const double *F, const int *type, const double *inv_mass, double half_dt_ftm2v,
+                      double dt, int drift, cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  k_vv<<<(n + 255) / 256, 256, 0, st>>>(n, pos, vel, F, type, inv_mass, half_dt_ftm2v, dt, drift);
+  count_launch();
+  return cudaGetLastError();
+}
+cudaError_t launch_ke(int n, const double *vel, const int *type, const double *mass, double half_mvv2e, double *ke_i, cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  k_ke<<<(n + 255) / 256, 256, 0, st>>>(n, vel, type, mass, half_mvv2e, ke_i);
+  count_launch();
+  return cudaGetLastError();
+}
+
+}  // namespace mtpb

@@ -1,0 +1,164 @@
+"""-m gpu: the device neighbour list (bit-exact against the brute-force searches), the positions-only host path and
+the velocity-Verlet loop, all through the C ABI."""
+import numpy as np
+import pytest
+
+from oracle import mtp as omtp
+from workloads import make_workload, neighbor_list_bruteforce, reverse_index
+from _util import n_basis_of, gpu_pot, to_dev
+
+pytestmark = pytest.mark.gpu
+KFTM2V = 1.602176634e-19 / 1.66053906660e-27 * 1e-4      # eV/A / (g/mol) -> A/ps^2
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    assert t.cuda.is_available()
+    return t
+
+
+def build(lib, torch, pos, box, r, **kw):
+    nb = lib.neighbors_build(torch.as_tensor(np.ascontiguousarray(pos)).cuda(), box, r, **kw)
+    n = nb["nnz"]
+    return (nb["off"].cpu().numpy(), nb["idx"].cpu().numpy()[:n], nb["shift"].cpu().numpy()[:n],
+            nb["rev"].cpu().numpy()[:n] if nb["rev"] is not None else None, nb)
+
+
+@pytest.mark.parametrize("ci", [0, 1])
+def test_list_is_bit_exact_at_configs_1_and_2(lib, torch, ci):
+    """Integer work: off / idx / shift / rev equal the brute-force 27-image search bit for bit (the oracle's own search on
+    every row at 128 atoms and on sampled rows at 2 000 atoms; the vectorised brute force on every row)."""
+    w = make_workload(ci, 1)
+    off, idx, sh, rev, nb = build(lib, torch, w.pos, w.box, 5.0)
+    assert nb["errors"] == 0 and nb["nnz"] == w.nnz
+    b_off, b_idx, b_sh = neighbor_list_bruteforce(w.pos, w.box, 5.0)
+    assert np.array_equal(off, b_off) and np.array_equal(idx, b_idx) and np.array_equal(sh, b_sh)
+    rows = list(range(w.n_atoms)) if ci == 0 else [0, 3, 500, 1234, 1999]
+    o_off, o_idx, o_sh = omtp.brute_force_neighbours(w.pos, w.box, 5.0, rows=rows)
+    for q, i in enumerate(rows):
+        assert np.array_equal(o_idx[o_off[q]:o_off[q + 1]], idx[off[i]:off[i + 1]])
+        assert np.array_equal(o_sh[o_off[q]:o_off[q + 1]], sh[off[i]:off[i + 1]])
+    assert np.array_equal(rev, reverse_index(b_off, b_idx, b_sh))
+
+
+def test_sheared_small_and_unwrapped_boxes(lib, torch):
+    """Triclinic box; a box with fewer than three cells per direction and one with a single cell (the same cell is
+    reached through several images); atoms given outside the box."""
+    rng = np.random.default_rng(7)
+    box = np.array([[12.5, 0.0, 0.0], [3.1, 12.0, 0.0], [-2.2, 1.7, 11.6]])
+    pos = rng.uniform(0, 1, (60, 3)) @ box
+    for bx, ps, r in [(box, pos, 5.0), (np.eye(3) * 11.0, rng.uniform(0, 11.0, (50, 3)), 5.0),
+                      (np.eye(3) * 7.0, rng.uniform(0, 7.0, (20, 3)), 5.0)]:
+        off, idx, sh, rev, nb = build(lib, torch, ps, bx, r)
+        o_off, o_idx, o_sh = omtp.brute_force_neighbours(ps, bx, r)
+        assert nb["errors"] == 0
+        assert np.array_equal(off, o_off) and np.array_equal(idx, o_idx) and np.array_equal(sh, o_sh)
+        assert np.array_equal(rev, reverse_index(o_off, o_idx, o_sh))
+    # atoms shifted out of the box by one lattice vector: the definition's pairs for the given coordinates
+    ps = pos.copy()
+    ps[::3] += box[0]
+    ps[1::5] -= box[2]
+    off, idx, sh, rev, nb = build(lib, torch, ps, box, 5.0)
+    o_off, o_idx, o_sh = omtp.brute_force_neighbours(ps, box, 5.0)       # images in {-1,0,1}^3 of the GIVEN coordinates
+    assert np.array_equal(off, o_off) and np.array_equal(idx, o_idx) and np.array_equal(sh, o_sh)
+    assert o_idx.shape[0] < omtp.brute_force_neighbours(pos, box, 5.0)[1].shape[0]     # some pairs would need a shift of 2
+
+
+def test_capacity_and_count_only(lib, torch):
+    w = make_workload(0, 1)
+    pos = torch.as_tensor(w.pos).cuda()
+    nb = lib.neighbors_build(pos, w.box, 5.0, capacity=0)
+    assert nb["nnz"] == w.nnz and np.array_equal(nb["off"].cpu().numpy(), w.off)
+    nb = lib.neighbors_build(pos, w.box, 5.0, capacity=1000)           # truncated: the count still says what is needed
+    assert nb["nnz"] == w.nnz
+    assert np.array_equal(nb["idx"].cpu().numpy()[:1000], w.idx[:1000])
+
+
+def test_config4_sampled_rows(lib, torch):
+    """BASELINE.json configs[3] at full size: the device list has the workload's pair count and its rows equal the
+    stencil list's (pinned against brute force on the CPU) on sampled rows; rev is an involution."""
+    w = make_workload(3, 1)
+    off, idx, sh, rev, nb = build(lib, torch, w.pos, w.box, 5.0)
+    assert nb["errors"] == 0 and nb["nnz"] == w.nnz and np.array_equal(off, w.off)
+    rng = np.random.default_rng(1)
+    for i in rng.choice(w.n_atoms, 200, replace=False):
+        a, b = off[i], off[i + 1]
+        assert np.array_equal(idx[a:b], w.idx[a:b]) and np.array_equal(sh[a:b], w.shift[a:b])
+    p = rng.choice(w.nnz, 100000, replace=False)
+    assert np.array_equal(rev[rev[p]], p) and np.array_equal(rev[p], w.rev[p])
+
+
+def test_host_positions_path_equals_host_list_path(lib, torch):
+    w = make_workload(1, n_basis_of(16), cells=5)
+    pot = gpu_pot(lib, w)
+    pot.set_option(lib.OPT_FORCE_MODE, lib.FORCE_GATHER)
+    a = pot.compute_host(w.pos, w.types, w.box, w.off, w.idx, w.shift, w.rev)
+    b = pot.compute_host_pos(w.pos, w.types, w.box)
+    assert b["nnz"] == w.nnz
+    for k in ("E", "Ei", "F", "virial"):
+        assert np.array_equal(a[k], b[k]), k
+    c = pot.compute_host_pos(w.pos, w.types, w.box)                     # second call: buffers already sized
+    assert np.array_equal(b["F"], c["F"])
+    pot.close()
+
+
+def test_velocity_verlet_loop(lib, torch):
+    """mtp_md_run: (1) zero steps = one force evaluation; (2) two steps equal the same update written out in numpy on
+    top of mtp_compute's forces; (3) over 200 steps the total energy drifts by a small fraction of the kinetic energy,
+    with list rebuilds every 10 steps at a 1 A skin giving the same trajectory as rebuilding every step.  (The seeded
+    random coefficients make a stiff, unphysical potential -- forces of 1e3 - 1e4 eV/A at level 10 -- hence steps of 0.01 and 0.001 fs.)"""
+    w = make_workload(0, n_basis_of(10))
+    pot = gpu_pot(lib, w)
+    d = to_dev(w, torch)
+    rng = np.random.default_rng(3)
+    mass = np.array([55.845])
+    vel0 = rng.normal(0.0, 2.0, (w.n_atoms, 3))                         # A/ps
+    vel0 -= vel0.mean(axis=0)
+    cap = int(w.nnz * 1.6)
+    ref = pot.compute(d["pos"], d["types"], w.box, d["off"], d["idx"], d["shift"], d["rev"])
+    torch.cuda.synchronize()
+    pos, vel = d["pos"].clone(), torch.as_tensor(vel0).cuda()
+    out = pot.md_run(pos, vel, d["types"], w.box, mass, 1e-5, 0, 1, 0.0, cap)
+    torch.cuda.synchronize()
+    assert np.array_equal(out["F"].cpu().numpy(), ref["F"].cpu().numpy()) and np.array_equal(pos.cpu().numpy(), w.pos)
+    ke0 = 0.5 / KFTM2V * (mass[0] * vel0 ** 2).sum()
+    assert out["E"].cpu().numpy()[1] == pytest.approx(ke0, rel=1e-13)
+    # (2) two steps by hand
+    dt = 1e-5
+    x, v, F = w.pos.copy(), vel0.copy(), ref["F"].cpu().numpy()
+    for _ in range(2):
+        v = v + 0.5 * dt * KFTM2V / mass[0] * F
+        x = x + dt * v
+        nb = lib.neighbors_build(torch.as_tensor(x).cuda(), w.box, 5.0)
+        o = pot.compute(torch.as_tensor(x).cuda(), d["types"], w.box, nb["off"], nb["idx"][:nb["nnz"]], nb["shift"][:nb["nnz"]],
+                        nb["rev"][:nb["nnz"]])
+        torch.cuda.synchronize()
+        F = o["F"].cpu().numpy()
+        v = v + 0.5 * dt * KFTM2V / mass[0] * F
+    pos, vel = d["pos"].clone(), torch.as_tensor(vel0).cuda()
+    out = pot.md_run(pos, vel, d["types"], w.box, mass, dt, 2, 1, 0.0, cap)
+    torch.cuda.synchronize()
+    L = w.box[0, 0]
+    dx = pos.cpu().numpy() - x
+    dx -= np.round(dx / L) * L                                          # md_run wraps atoms into the box at a rebuild
+    assert np.abs(dx).max() < 1e-12 and np.abs(vel.cpu().numpy() - v).max() < 1e-10
+    # (3) energy conservation and rebuild cadence
+    res = {}
+    dt = 1e-6
+    for every, skin in ((1, 0.0), (10, 1.0)):
+        pos, vel = d["pos"].clone(), torch.as_tensor(vel0).cuda()
+        o = pot.md_run(pos, vel, d["types"], w.box, mass, dt, 200, every, skin, int(w.nnz * 2.2))
+        torch.cuda.synchronize()
+        info = o["info"].cpu().numpy()
+        assert info[1] == 0 and info[0] <= int(w.nnz * 2.2)
+        assert pot.get_option(lib.INFO_INPUT_ERRORS) == 0 and pot.get_option(lib.INFO_SCRATCH_OVERFLOW) == 0
+        res[every] = (o["E"].cpu().numpy().copy(), pos.cpu().numpy().copy())
+    e0 = ref["E"].cpu().numpy()[0] + ke0
+    e1 = res[1][0].sum()
+    assert res[1][0][1] > 2 * ke0                                        # the atoms did pick up kinetic energy
+    assert abs(e1 - e0) < 1e-3 * (res[1][0][1] + ke0)
+    dx = res[1][1] - res[10][1]
+    dx -= np.round(dx / L) * L
+    assert np.abs(dx).max() < 1e-9 and abs(res[1][0].sum() - res[10][0].sum()) < 1e-9 * abs(e0)
+    pot.close()
