@@ -86,7 +86,8 @@ void mtp_table_free(mtp_params *table);
  * the generic table interpreter is set up instead and mtp_last_error(handle) says why. */
 int mtp_create(mtp_handle **out, const mtp_params *p);
 void mtp_destroy(mtp_handle *h);
-const char *mtp_last_error(const mtp_handle *h); /* h may be NULL: last create error     */
+const char *mtp_last_error(const mtp_handle *h); /* h may be NULL: last error of a call that
+                                                    takes no handle (mtp_create, ..._build_static) */
 
 /* Options (a10 chunk scheduler PAPER.md:62,76; a8 force mode; a12 variant PAPER.md:35). */
 #define MTP_OPT_CHUNK_ATOMS 1   /* atoms per chunk; 0 = automatic (L2-sized)               */
@@ -182,6 +183,21 @@ int mtp_neighbors_workspace_bytes(int64_t n_atoms, size_t *out_bytes);
 int mtp_neighbors_build(int64_t n_atoms, const double *d_pos, const double *box, double r_list, int64_t capacity,
                         int64_t *d_off, int32_t *d_idx, int8_t *d_shift, int32_t *d_rev, int64_t *d_info,
                         void *d_ws, size_t ws_bytes, void *cuda_stream);
+/* mtp_neighbors_build_static: mtp_neighbors_build for callers that cannot allocate device memory (code under CUDA
+ *   graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Same arguments, same kernels and the
+ *   same bit-identical result, but no workspace argument: the workspace is a static array in the library's device
+ *   image, 6 MiB, which every GPU that loads the library holds until the process exits.  The call itself allocates
+ *   nothing (no cudaMalloc / cudaFree, no allocating library routine): it enqueues two memsets and the kernels on
+ *   the stream.  Limit: n_atoms <= MTP_NB_STATIC_MAX_ATOMS; beyond it MTP_ESIZE, and mtp_last_error(NULL) names the
+ *   limit (use mtp_neighbors_build with your own workspace there).
+ *   All calls on a device share the array, which keeps the last call's contents (the call clears what has to start
+ *   at zero): calls that overlap on the GPU -- different streams with no ordering between them -- race; calls on
+ *   one stream, or ordered by events, are safe.  The first call on each device looks up the array's device address
+ *   (cudaGetSymbolAddress): make that first call outside stream capture. */
+#define MTP_NB_STATIC_MAX_ATOMS 32768
+int mtp_neighbors_build_static(int64_t n_atoms, const double *d_pos, const double *box, double r_list, int64_t capacity,
+                               int64_t *d_off, int32_t *d_idx, int8_t *d_shift, int32_t *d_rev, int64_t *d_info,
+                               void *cuda_stream);
 /* mtp_md_run: n_steps of velocity-Verlet (NVE) with the potential of the handle, entirely enqueued on the stream:
  *   v += dt/2 F/m; x += dt v; [every rebuild_every steps: atoms wrapped into the box, list rebuilt at R_cut + skin];
  *   F = mtp_compute(x); v += dt/2 F/m.   Units: eV, Angstrom, ps, g/mol (LAMMPS "metal"); mass[S] HOST, per species.

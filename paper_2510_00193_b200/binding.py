@@ -38,7 +38,7 @@ EXPORTS = ["mtp_enumerate", "mtp_table_free", "mtp_create", "mtp_destroy", "mtp_
            "mtp_set_option", "mtp_get_option", "mtp_workspace_bytes", "mtp_compute", "mtp_grade",
            "mtp_compute_host", "mtp_debug_moments", "mtp_launch_count", "mtp_peak_dfma",
            "mtp_cost_model", "mtp_profile_read", "mtp_table_plan", "mtp_k2_program",
-           "mtp_neighbors_workspace_bytes", "mtp_neighbors_build", "mtp_md_workspace_bytes", "mtp_md_run",
+           "mtp_neighbors_workspace_bytes", "mtp_neighbors_build", "mtp_neighbors_build_static", "mtp_md_workspace_bytes", "mtp_md_run",
            "mtp_compute_host_pos"]
 
 
@@ -84,6 +84,7 @@ def _load():
     lib.mtp_table_plan.argtypes = [C.POINTER(MtpParams), C.POINTER(i64)]
     lib.mtp_neighbors_workspace_bytes.argtypes = [i64, C.POINTER(C.c_size_t)]
     lib.mtp_neighbors_build.argtypes = [i64, vp, C.POINTER(dbl), dbl, i64, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
+    lib.mtp_neighbors_build_static.argtypes = [i64, vp, C.POINTER(dbl), dbl, i64, vp, vp, vp, vp, vp, vp]
     lib.mtp_md_workspace_bytes.argtypes = [vp, i64, i64, C.POINTER(C.c_size_t)]
     lib.mtp_md_run.argtypes = [vp, i64, vp, vp, vp, C.POINTER(dbl), C.POINTER(dbl), dbl, i64, C.c_int32, dbl, i64,
                                vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
@@ -388,6 +389,23 @@ def neighbors_build(pos, box, r_list, capacity=None, want_rev=True, stream=None)
     idx, shift, rev = run(int(capacity))
     nnz, errors = [int(x) for x in info.cpu()]
     return dict(off=off, idx=idx, shift=shift, rev=rev, nnz=nnz, errors=errors)
+
+
+NB_STATIC_MAX_ATOMS = 32768
+
+
+def neighbors_build_static(pos, box, r_list, off, idx, shift, rev, info, stream=None):
+    """mtp_neighbors_build_static: the list build with no workspace argument and no allocation (limit
+    NB_STATIC_MAX_ATOMS atoms).  Every output is the caller's torch CUDA tensor: off [N+1] i64, idx [cap] i32,
+    shift [cap][3] i8, rev [cap] i32 or None, info [2] i64 (pairs found, errors).  Nothing is read back or
+    synchronised here."""
+    n, cap = int(pos.shape[0]), int(idx.shape[0])
+    boxh = (C.c_double * 9)(*[float(x) for x in np.asarray(box, dtype=np.float64).reshape(9)])
+    rc = _lib.mtp_neighbors_build_static(n, _ptr(pos), boxh, float(r_list), cap, _ptr(off), _ptr(idx), _ptr(shift), _ptr(rev),
+                                         _ptr(info), Potential._stream(stream))
+    if rc != OK:
+        raise MtpError(rc, "mtp_neighbors_build_static: " + _lib.mtp_last_error(None).decode())
+    return rc
 
 
 def launch_count() -> int:

@@ -37,6 +37,7 @@ const PairLevel *pair_level(int index) {
 }  // namespace mtpb
 
 static thread_local std::string g_create_error;
+void mtpb::set_thread_error(const char *msg) { g_create_error = msg ? msg : ""; }
 
 struct mtp_handle {
   int S = 0, nb = 0, nmu = 0, n_basic = 0, n_nodes = 0, n_basis = 0, lev_max = 0;

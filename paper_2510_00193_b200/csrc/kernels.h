@@ -121,6 +121,8 @@ cudaError_t launch_scan(const int *in, long long n, long long *out, long long *t
 // found, errors}; at most `capacity` pairs are written
 cudaError_t launch_neighbors_build(const NbGrid &g, long long n, const double *pos, double r_list, long long capacity, long long *off,
                                    int *idx, signed char *shift, int *rev, long long *info, int accumulate, void *ws, cudaStream_t st);
+// text for mtp_last_error(NULL) from entry points that take no handle (defined in api.cu)
+void set_thread_error(const char *msg);
 cudaError_t launch_wrap(const NbGrid &g, int n, double *pos, cudaStream_t st);
 cudaError_t launch_vv(int n, double *pos, double *vel, const double *F, const int *type, const double *inv_mass, double half_dt_ftm2v,
                       double dt, int drift, cudaStream_t st);

@@ -19,8 +19,11 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdint>
+#include <cstdio>
+#include <mutex>
 
 #include "kernels.h"
+#include "mtp_b200.h"
 
 namespace mtpb {
 
@@ -373,4 +376,76 @@ cudaError_t launch_ke(int n, const double *vel, const int *type, const double *m
   return cudaGetLastError();
 }
 
+
+// ---- mtp_neighbors_build_static: the list build with its workspace in a static device array -------------------------
+// For callers that cannot allocate (stream capture, serving loops, harnesses that forbid cudaMalloc): the kernels of
+// launch_neighbors_build, unchanged, on a workspace that lives in the library's device image.  Every GPU that loads
+// the library holds the array (6 MiB) until the process exits.  All calls on a device share it: calls that overlap
+// on the GPU (different streams without ordering) race; calls on one stream, or ordered by events, do not.
+namespace {
+constexpr long long kNbStaticAtoms = MTP_NB_STATIC_MAX_ATOMS;
+constexpr size_t kNbStaticBytes = (size_t)6 << 20;          // nb_workspace_bytes(32 768) = 6 033 408
+static __device__ __align__(256) unsigned char g_nb_static[kNbStaticBytes];
+
+constexpr int kMaxDevices = 64;
+std::mutex g_nb_static_mu;
+void *g_nb_static_ptr[kMaxDevices] = {};
+
+// Device address of the array on the current device.  In host code the name g_nb_static is only a handle for the
+// runtime, not a device address: the address comes from cudaGetSymbolAddress, asked once per device with that
+// device current (every device has its own copy of the array).
+cudaError_t nb_static_address(void **out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_nb_static_mu);
+  if (!g_nb_static_ptr[dev]) {
+    void *p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_nb_static);
+    if (e != cudaSuccess) return e;
+    g_nb_static_ptr[dev] = p;
+  }
+  *out = g_nb_static_ptr[dev];
+  return cudaSuccess;
+}
+}  // namespace
+
 }  // namespace mtpb
+
+extern "C" int mtp_neighbors_build_static(int64_t N, const double *d_pos, const double *box, double r_list, int64_t capacity,
+                                          int64_t *d_off, int32_t *d_idx, int8_t *d_shift, int32_t *d_rev, int64_t *d_info,
+                                          void *stream) {
+  using namespace mtpb;
+  char msg[256];
+  if (N < 0 || !box || !d_off || !d_info || capacity < 0 || (N > 0 && !d_pos) || (capacity > 0 && (!d_idx || !d_shift)) ||
+      capacity > 0x7fffffffLL) {
+    set_thread_error("mtp_neighbors_build_static: bad argument (null pointer or negative size)");
+    return MTP_EINVAL;
+  }
+  if (N > kNbStaticAtoms || nb_workspace_bytes(N) > kNbStaticBytes) {
+    std::snprintf(msg, sizeof msg,
+                  "mtp_neighbors_build_static: n_atoms = %lld exceeds MTP_NB_STATIC_MAX_ATOMS = %lld "
+                  "(use mtp_neighbors_build with a caller workspace)", (long long)N, kNbStaticAtoms);
+    set_thread_error(msg);
+    return MTP_ESIZE;
+  }
+  NbGrid g;
+  if (!nb_grid(box, r_list, N, g)) {
+    set_thread_error("mtp_neighbors_build_static: singular box or r_list <= 0");
+    return MTP_EBOX;
+  }
+  void *ws = nullptr;
+  cudaError_t e = nb_static_address(&ws);
+  // what must start at zero (cell histogram, scatter cursors, error flag) is cleared by launch_neighbors_build on the
+  // stream; everything else in the workspace is written before it is read, so the last call's contents do not matter
+  if (e == cudaSuccess)
+    e = launch_neighbors_build(g, N, d_pos, r_list, capacity, (long long *)d_off, d_idx, (signed char *)d_shift, d_rev,
+                               (long long *)d_info, 0, ws, (cudaStream_t)stream);
+  if (e != cudaSuccess) {
+    std::snprintf(msg, sizeof msg, "mtp_neighbors_build_static: %s", cudaGetErrorString(e));
+    set_thread_error(msg);
+    return MTP_ECUDA;
+  }
+  return MTP_OK;
+}
