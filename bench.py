@@ -4,7 +4,8 @@
 A "step" is one pass of the whole hot path (rows a1-a8, a10 of SURVEY.md 8(a)) over one BASELINE.json
 workload; the default is configs[3], the one the metric is quoted on: 1,048,576 atoms, 3 species, FCC 64^3,
 level 16, fp64, chunked evaluation.  `value` is device-resident throughput (CUDA events), `e2e` the same metric
-through mtp_compute_host with pinned HOST buffers (H2D + D2H inside the timed region).  `--impl reference`
+through mtp_compute_host_pos with pinned HOST buffers (H2D + D2H inside the timed region; `e2e_host_list`: through
+mtp_compute_host, the caller's list copied as well), `md` the device MD loop in atom-timesteps/s.  `--impl reference`
 times the CPU oracle (oracle/, as it stands) on a bounded sample, on all host cores; it does not load the
 CUDA library.
 
@@ -31,6 +32,7 @@ sys.path.insert(0, ROOT)
 LEVELS = [10, 16, 20, 16, 24]
 HEADLINE = 3                         # 0-based index of the configuration BASELINE.json's metric is quoted on
 UNIT = "atom-evals/s"
+MD_DT = 1e-10                        # ps: the seeded random coefficients give forces of 1e8 eV/A at level 16; the atoms must stay put
 
 
 def metric_name(config, w):
@@ -331,22 +333,58 @@ def run_ours(args):
         gms = graph_replay(torch, lib, pot, step, out)
         graph = {"calls": 100, "ms_per_call": gms, "value": w.n_atoms / (gms * 1e-3), "unit": UNIT}
 
-    # ---- end to end through the host-buffer entry point (pinned inputs, results read back)
+    # ---- end to end through the host-buffer entry points (pinned inputs, results read back).  `e2e`: what an MD host
+    # code sends every step -- positions and types -- with the list built on the device (mtp_compute_host_pos);
+    # `e2e_host_list`: the caller's own list copied too (mtp_compute_host; "the GPU runs use the host
+    # code's list")
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
     hp = dict(pos=pin(w.pos), types=pin(w.types), off=pin(w.off), idx=pin(w.idx), shift=pin(w.shift), rev=pin(w.rev))
     hout = dict(E=pin(np.zeros(1)), Ei=pin(np.zeros(w.n_atoms)), F=pin(np.zeros((w.n_atoms, 3))), virial=pin(np.zeros(6)))
     e2e_steps = max(1, min(args.steps, 10))
-    pot.compute_host(hp["pos"], hp["types"], w.box, hp["off"], hp["idx"], hp["shift"], hp["rev"], out=hout)
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        pot.compute_host(hp["pos"], hp["types"], w.box, hp["off"], hp["idx"], hp["shift"], hp["rev"], out=hout)
-    torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    h2d = sum(hp[k].nbytes for k in hp)
-    d2h = sum(hout[k].nbytes for k in hout)
-    e2e_value = whole_job_rate(w.n_atoms, e2e_steps, e2e_s, world, dist, dev)
+
+    def timed_host(call):
+        call()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            call()
+        torch.cuda.synchronize()
+        return whole_job_rate(w.n_atoms, e2e_steps, time.perf_counter() - t0, world, dist, dev)
+
+    e2e_list_value = timed_host(lambda: pot.compute_host(hp["pos"], hp["types"], w.box, hp["off"], hp["idx"], hp["shift"], hp["rev"], out=hout))
+    h2d_list = sum(hp[k].nbytes for k in hp)
+    e2e_value = timed_host(lambda: pot.compute_host_pos(hp["pos"], hp["types"], w.box, out=hout))
+    assert hout["nnz"] == w.nnz, "device list differs from the workload's"
+    h2d = hp["pos"].nbytes + hp["types"].nbytes
+    d2h = sum(hout[k].nbytes for k in ("E", "Ei", "F", "virial"))
     pot.profile_read()
+
+    # ---- MD loop on the device: velocity-Verlet steps with the list rebuilt every 10 steps at a
+    # 1 A skin, atom-timesteps/s (the paper's unit, list builds included).  The seeded random
+    # coefficients make a stiff potential, hence the tiny time step MD_DT: the work per step does not depend on it.
+    md = None
+    if not args.no_md and Ainv is None:
+        md_steps = max(10, min(args.steps, 50))
+        cap = int(w.nnz * 1.9) + 1024                       # (6 / 5)^3 = 1.73 x the pairs at R_cut
+        mpos, mvel = pos.clone(), torch.zeros_like(pos)
+        mass = np.full(w.n_species, 55.845)
+        pot.set_option(lib.OPT_PROFILE, 0)
+        pot.md_run(mpos, mvel, types, w.box, mass, MD_DT, 10, 10, 1.0, cap)
+        barrier()
+        n1 = lib.launch_count()
+        m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        m0.record()
+        mo = pot.md_run(mpos, mvel, types, w.box, mass, MD_DT, md_steps, 10, 1.0, cap)
+        m1.record()
+        barrier()
+        md_ms = max_over_ranks(m0.elapsed_time(m1), dist, dev)
+        info = [int(x) for x in mo["info"].cpu()]
+        assert info[0] <= cap and info[1] == 0, "MD list overflow"
+        md = {"value": world * w.n_atoms * md_steps / (md_ms * 1e-3), "unit": "atom-timesteps/s", "steps": md_steps,
+              "ms_per_step": md_ms / md_steps, "rebuild_every": 10, "skin": 1.0, "list_pairs": info[0],
+              "gpu_launches": int(lib.launch_count() - n1)}
+        pot.set_option(lib.OPT_PROFILE, 1)
+        del mpos, mvel, mo
 
     if rank != 0:
         if dist is not None:
@@ -386,7 +424,9 @@ def run_ours(args):
                 "workspace_bytes": int(ws_bytes)},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                "steps": e2e_steps},
+                "steps": e2e_steps, "entry": "mtp_compute_host_pos (positions in, list built on the device)"},
+        "e2e_host_list": {"value": e2e_list_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d_list),
+                          "d2h_bytes_per_step": int(d2h), "steps": e2e_steps, "entry": "mtp_compute_host (caller's list copied)"},
         "gpu_launches": int(launches),
         "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
                      "frac": achieved_tf / peak_tf, "traffic": load_traffic(cfg["name"], dom),
@@ -400,6 +440,8 @@ def run_ours(args):
     }
     if graph is not None:
         line["graph_replay"] = graph
+    if md is not None:
+        line["md"] = md
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
@@ -429,6 +471,7 @@ def main():
     ap.add_argument("--ref-atoms", type=int, default=None,
                     help="atoms per core of an oracle sample (default: 8192 for cpu_baseline, 1024 per step for --impl reference)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-md", action="store_true", help="skip the MD-loop leg")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

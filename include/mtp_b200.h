@@ -175,7 +175,8 @@ int mtp_compute_host(mtp_handle *h, int64_t n_atoms, const double *pos, const in
  *   the 27 images.  Positions should lie in the box; an atom outside is handled as long as no listed shift leaves
  *   {-1,0,1}^3 (such pairs are not listed).
  *   d_off [N+1] i64, d_idx [capacity] i32, d_shift [capacity][3] i8, d_rev [capacity] i32 or NULL (reverse index:
- *   d_rev[p] = position of (j, i, -s)), d_info [2] i64 = { pairs found, errors (rows longer than 256 entries) }.
+ *   d_rev[p] = position of (j, i, -s)), d_info [2] i64 = { pairs found, errors (rows longer than 256 entries, coordinates that are
+ *   not finite) }.
  *   At most `capacity` pairs are written: when d_info[0] > capacity the arrays hold a truncated list (call again
  *   with larger arrays; capacity 0 just counts).  Workspace: mtp_neighbors_workspace_bytes(n_atoms).  No handle: the
  *   list does not depend on the potential.  MTP_EBOX for a singular box. */

@@ -385,7 +385,6 @@ int plan_jit(const K2Table &whole, JitPlan &best, std::string *err, bool *too_la
   bool have = false;
   static const int budgets[] = {430, 600, 870};
   for (int budget : budgets) {
-    if (getenv("XBUDGET") && atoi(getenv("XBUDGET")) != budget) continue;
     JitPlan p;
     if (!tree_partition(whole.n_basic, whole.n_nodes, whole.n_prod(), whole.prod.data(), (int)whole.basis_node.size(),
                         whole.basis_node.data(), budget, p.part)) continue;
@@ -471,7 +470,7 @@ static int ensure_jit(mtp_handle *h) {
   for (auto &jp : h->jprogs)
     for (int k = 0; k < 2; ++k) jobs.push_back(Job{&jp, k, nullptr, "", 0});
   std::atomic<size_t> next{0};
-  const int window = getenv("XW") ? atoi(getenv("XW")) : kK2Window, lookahead = getenv("XD") ? atoi(getenv("XD")) : kK2Lookahead;
+  const int window = kK2Window, lookahead = kK2Lookahead;
   auto work = [&]() {
     for (size_t i = next.fetch_add(1); i < jobs.size(); i = next.fetch_add(1)) {
       Job &j = jobs[i];

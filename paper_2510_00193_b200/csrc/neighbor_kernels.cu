@@ -44,11 +44,18 @@ __device__ __forceinline__ int cell_of(const NbGrid &g, double x, double y, doub
 
 // cell index and wrap image of every atom; histogram of the cells
 __global__ void k_nb_cells(NbGrid g, const double *__restrict__ pos, int n, int *__restrict__ cell, int *__restrict__ wrap,
-                           int *__restrict__ count) {
+                           int *__restrict__ count, int *__restrict__ flag) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   int w[3];
-  const int c = cell_of(g, pos[3 * (size_t)i], pos[3 * (size_t)i + 1], pos[3 * (size_t)i + 2], w);
+  const double x = pos[3 * (size_t)i], y = pos[3 * (size_t)i + 1], z = pos[3 * (size_t)i + 2];
+  int c = 0;
+  // a coordinate that is not finite, or further out than 2^30 box lengths (an MD run that blew up): counted as an
+  // error, the atom goes to cell 0 and gets no neighbours (its distance tests fail)
+  const double big = 1073741824.0;
+  const double f0 = x * g.Hi[0] + y * g.Hi[3] + z * g.Hi[6], f1 = x * g.Hi[1] + y * g.Hi[4] + z * g.Hi[7], f2 = x * g.Hi[2] + y * g.Hi[5] + z * g.Hi[8];
+  if (fabs(f0) < big && fabs(f1) < big && fabs(f2) < big) c = cell_of(g, x, y, z, w);
+  else { w[0] = w[1] = w[2] = 0; atomicAdd(flag, 1); }
   cell[i] = c;
   wrap[3 * (size_t)i] = w[0]; wrap[3 * (size_t)i + 1] = w[1]; wrap[3 * (size_t)i + 2] = w[2];
   atomicAdd(count + c, 1);
@@ -134,83 +141,153 @@ __global__ void k_nb_sort_cells(const long long *__restrict__ start, int n_cells
     sorted[q] = v;
   }
 }
-// the caller's coordinates of the atoms in cell order (x, y, z, atom index as double): one 32-byte record per candidate
-__global__ void k_nb_gather_pos(const double *__restrict__ pos, const int *__restrict__ sorted, int n, double *__restrict__ pos_s) {
+// the caller's coordinates of the atoms in cell order: one 32-byte record (x, y, z, tag) per candidate, tag = atom
+// index, + 2^27 when the atom lies outside the box (its wrap image is then read from wrap[]; the common case needs no
+// second load)
+constexpr int kWrapBit = 1 << 27;
+__global__ void k_nb_gather_pos(const double *__restrict__ pos, const int *__restrict__ sorted, const int *__restrict__ wrap, int n,
+                                double *__restrict__ pos_s) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= n) return;
   const int i = sorted[t];
+  const bool out = (wrap[3 * (size_t)i] | wrap[3 * (size_t)i + 1] | wrap[3 * (size_t)i + 2]) != 0;
   double2 *o = reinterpret_cast<double2 *>(pos_s) + 2 * (size_t)t;
   o[0] = make_double2(pos[3 * (size_t)i], pos[3 * (size_t)i + 1]);
-  o[1] = make_double2(pos[3 * (size_t)i + 2], (double)i);
+  o[1] = make_double2(pos[3 * (size_t)i + 2], (double)(i + (out ? kWrapBit : 0)));
 }
 
-// One warp per atom (in cell order): the 27 cells around its cell, lanes over the candidates of a cell.
-// FILL = false: count[i] = number of neighbours.  FILL = true: the row's keys j * 27 + code are collected in shared
-// memory, rank-sorted, and written as idx / shift at off[i].
-template <bool FILL>
+// One warp per atom (in cell order).  The 27 cells around its cell are 27 segments of the cell-sorted records; lane
+// d < 27 looks up segment d (begin, size, image of the cell wrap), a warp scan lays the segments end to end, and the
+// lanes then walk the concatenated candidates 32 at a time -- full lanes whatever the cell occupancy.
+// MODE 0 (count): count[i] = number of neighbours.
+// MODE 1 (fill):  the row's keys j * 27 + code are collected in shared memory, rank-sorted, and written as idx / shift
+//                 at off[i] (coalesced).  if_truncated: only when off[n] > capacity (see MODE 2).
+// MODE 2 (stash): one search instead of two: count[i] as MODE 0, and the sorted keys of the row go to tmp at a place
+//                 claimed from a global cursor (tstart[i]; -1 when it lies beyond the capacity); k_nb_place moves them
+//                 to off[i] once the offsets are known.  When the list does not fit its capacity the stash is
+//                 incomplete: k_nb_place then does nothing and a MODE 1 pass writes the first `capacity` pairs.
+enum { NB_COUNT = 0, NB_FILL = 1, NB_STASH = 2 };
+template <int MODE>
 __global__ void __launch_bounds__(256) k_nb_rows(NbGrid g, const double *__restrict__ pos_s, const int *__restrict__ cell,
                                                  const int *__restrict__ wrap, const long long *__restrict__ start, int n, double r2max,
                                                  int *__restrict__ count, const long long *__restrict__ off, long long capacity,
-                                                 int *__restrict__ idx, signed char *__restrict__ shift, int *__restrict__ flag) {
-  __shared__ unsigned keys[8][kRowMax];
+                                                 int *__restrict__ idx, signed char *__restrict__ shift, int *__restrict__ flag,
+                                                 int if_truncated, int *__restrict__ tstart, unsigned *__restrict__ tmp,
+                                                 unsigned long long *__restrict__ cursor) {
+  constexpr bool FILL = MODE != NB_COUNT;
+  __shared__ unsigned keys[FILL ? 8 : 1][FILL ? kRowMax : 1], sorted_keys[FILL ? 8 : 1][FILL ? kRowMax : 1];
+  if (MODE == NB_FILL && if_truncated && off[n] <= capacity) return;
+  __shared__ long long seg_base[8][27];
+  __shared__ int seg_end[8][27], seg_m[8][27];
+  const unsigned full = 0xffffffffu;
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   const int t = blockIdx.x * 8 + wib;                       // position in cell order
   if (t >= n) return;
   const double2 a0 = reinterpret_cast<const double2 *>(pos_s)[2 * (size_t)t], a1 = reinterpret_cast<const double2 *>(pos_s)[2 * (size_t)t + 1];
-  const int i = (int)a1.y;
+  const int tag_i = (int)a1.y, i = tag_i & (kWrapBit - 1);
   const double xi = a0.x, yi = a0.y, zi = a1.x;
   const int ci = cell[i];
   const int c2 = ci % g.nc[2], c1 = (ci / g.nc[2]) % g.nc[1], c0 = ci / (g.nc[2] * g.nc[1]);
-  const int wi0 = wrap[3 * (size_t)i], wi1 = wrap[3 * (size_t)i + 1], wi2 = wrap[3 * (size_t)i + 2];
-  int n_row = 0;
-  for (int d = 0; d < 27; ++d) {
-    const int e0 = c0 + d / 9 - 1, e1 = c1 + (d / 3) % 3 - 1, e2 = c2 + d % 3 - 1;
-    // cell index wrapped into the grid; the number of box lengths it wrapped by is the image of the wrapped coordinates
-    const int q0 = (e0 % g.nc[0] + g.nc[0]) % g.nc[0], q1 = (e1 % g.nc[1] + g.nc[1]) % g.nc[1], q2 = (e2 % g.nc[2] + g.nc[2]) % g.nc[2];
-    const int m0 = (e0 - q0) / g.nc[0], m1 = (e1 - q1) / g.nc[1], m2 = (e2 - q2) / g.nc[2];
-    const int cj = (q0 * g.nc[1] + q1) * g.nc[2] + q2;
-    const long long a = start[cj], b = start[cj + 1];
-    for (long long p = a + lane; p < b + ((32 - (b - a) % 32) % 32); p += 32) {   // whole warp iterations (ballots inside)
-      bool hit = false;
-      unsigned key = 0;
-      if (p < b) {
-        const double2 b0 = reinterpret_cast<const double2 *>(pos_s)[2 * (size_t)p], b1 = reinterpret_cast<const double2 *>(pos_s)[2 * (size_t)p + 1];
-        const int j = (int)b1.y;
-        // image shift relative to the caller's (possibly unwrapped) coordinates
-        const int s0 = m0 - (wrap[3 * (size_t)j] - wi0), s1 = m1 - (wrap[3 * (size_t)j + 1] - wi1), s2 = m2 - (wrap[3 * (size_t)j + 2] - wi2);
-        if (s0 >= -1 && s0 <= 1 && s1 >= -1 && s1 <= 1 && s2 >= -1 && s2 <= 1 && !(j == i && s0 == 0 && s1 == 0 && s2 == 0)) {
-          // r = (x_j - x_i) + s0 H0 + s1 H1 + s2 H2, no contractions (the definition's rounding)
-          const double x = __dadd_rn(__dadd_rn(__dadd_rn(__dadd_rn(b0.x, -xi), __dmul_rn((double)s0, g.H[0])), __dmul_rn((double)s1, g.H[3])), __dmul_rn((double)s2, g.H[6]));
-          const double y = __dadd_rn(__dadd_rn(__dadd_rn(__dadd_rn(b0.y, -yi), __dmul_rn((double)s0, g.H[1])), __dmul_rn((double)s1, g.H[4])), __dmul_rn((double)s2, g.H[7]));
-          const double z = __dadd_rn(__dadd_rn(__dadd_rn(__dadd_rn(b1.x, -zi), __dmul_rn((double)s0, g.H[2])), __dmul_rn((double)s1, g.H[5])), __dmul_rn((double)s2, g.H[8]));
-          const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y)), __dmul_rn(z, z));
-          hit = r2 < r2max;
-          key = (unsigned)j * 27u + (unsigned)((s0 + 1) * 9 + (s1 + 1) * 3 + (s2 + 1));
-        }
-      }
-      const unsigned m = __ballot_sync(0xffffffffu, hit);
-      if (FILL && hit) {
-        const int slot = n_row + __popc(m & ((1u << lane) - 1u));
-        if (slot < kRowMax) keys[wib][slot] = key;
-      }
-      n_row += __popc(m);
+  int wi0 = 0, wi1 = 0, wi2 = 0;
+  if (tag_i & kWrapBit) { wi0 = wrap[3 * (size_t)i]; wi1 = wrap[3 * (size_t)i + 1]; wi2 = wrap[3 * (size_t)i + 2]; }
+  {
+    long long a = 0;
+    int size = 0, mcode = 0;
+    if (lane < 27) {
+      // neighbour cell, wrapped into the grid; the number of box lengths it wrapped by is the image of the wrapped
+      // coordinates.  e is in [-1, nc], so one conditional step does it (with nc < 3 the same cell comes up through
+      // different images -- still every image exactly once)
+      int e0 = c0 + lane / 9 - 1, e1 = c1 + (lane / 3) % 3 - 1, e2 = c2 + lane % 3 - 1, m0 = 0, m1 = 0, m2 = 0;
+      if (e0 < 0) { e0 += g.nc[0]; m0 = -1; } else if (e0 >= g.nc[0]) { e0 -= g.nc[0]; m0 = 1; }
+      if (e1 < 0) { e1 += g.nc[1]; m1 = -1; } else if (e1 >= g.nc[1]) { e1 -= g.nc[1]; m1 = 1; }
+      if (e2 < 0) { e2 += g.nc[2]; m2 = -1; } else if (e2 >= g.nc[2]) { e2 -= g.nc[2]; m2 = 1; }
+      const int cj = (e0 * g.nc[1] + e1) * g.nc[2] + e2;
+      a = start[cj];
+      size = (int)(start[cj + 1] - a);
+      mcode = (m0 + 1) * 9 + (m1 + 1) * 3 + (m2 + 1);
     }
+    int inc = size;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(full, inc, o); if (lane >= o) inc += v; }
+    if (lane < 27) { seg_base[wib][lane] = a - (inc - size); seg_end[wib][lane] = inc; seg_m[wib][lane] = mcode; }
   }
-  if (!FILL) { if (lane == 0) count[i] = n_row; return; }
   __syncwarp();
-  if (n_row > kRowMax) { if (lane == 0) atomicAdd(flag, 1); n_row = kRowMax; }
-  const long long beg = off[i];
+  const int total = seg_end[wib][26];
+  int n_row = 0, d = 0;
+  for (int tt = lane; tt < ((total + 31) & ~31); tt += 32) {          // whole warp iterations (ballots inside)
+    bool hit = false;
+    unsigned key = 0;
+    if (tt < total) {
+      while (tt >= seg_end[wib][d]) ++d;
+      const long long p = seg_base[wib][d] + tt;
+      const int mc = seg_m[wib][d];
+      const double2 b0 = reinterpret_cast<const double2 *>(pos_s)[2 * (size_t)p], b1 = reinterpret_cast<const double2 *>(pos_s)[2 * (size_t)p + 1];
+      const int tag_j = (int)b1.y, j = tag_j & (kWrapBit - 1);
+      // image shift relative to the caller's (possibly unwrapped) coordinates
+      int s0 = mc / 9 - 1 + wi0, s1 = (mc / 3) % 3 - 1 + wi1, s2 = mc % 3 - 1 + wi2;
+      if (tag_j & kWrapBit) { s0 -= wrap[3 * (size_t)j]; s1 -= wrap[3 * (size_t)j + 1]; s2 -= wrap[3 * (size_t)j + 2]; }
+      if (s0 >= -1 && s0 <= 1 && s1 >= -1 && s1 <= 1 && s2 >= -1 && s2 <= 1 && !(j == i && s0 == 0 && s1 == 0 && s2 == 0)) {
+        // r = (x_j - x_i) + s0 H0 + s1 H1 + s2 H2, no contractions (the definition's rounding)
+        const double x = __dadd_rn(__dadd_rn(__dadd_rn(__dadd_rn(b0.x, -xi), __dmul_rn((double)s0, g.H[0])), __dmul_rn((double)s1, g.H[3])), __dmul_rn((double)s2, g.H[6]));
+        const double y = __dadd_rn(__dadd_rn(__dadd_rn(__dadd_rn(b0.y, -yi), __dmul_rn((double)s0, g.H[1])), __dmul_rn((double)s1, g.H[4])), __dmul_rn((double)s2, g.H[7]));
+        const double z = __dadd_rn(__dadd_rn(__dadd_rn(__dadd_rn(b1.x, -zi), __dmul_rn((double)s0, g.H[2])), __dmul_rn((double)s1, g.H[5])), __dmul_rn((double)s2, g.H[8]));
+        const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y)), __dmul_rn(z, z));
+        hit = r2 < r2max;
+        key = (unsigned)j * 27u + (unsigned)((s0 + 1) * 9 + (s1 + 1) * 3 + (s2 + 1));
+      }
+    }
+    const unsigned m = __ballot_sync(full, hit);
+    if (FILL && hit) {
+      const int slot = n_row + __popc(m & ((1u << lane) - 1u));
+      if (slot < kRowMax) keys[wib][slot] = key;
+    }
+    n_row += __popc(m);
+  }
+  if (MODE != NB_FILL && lane == 0) count[i] = n_row;
+  if (!FILL) return;
+  __syncwarp();
+  if (n_row > kRowMax) { if (lane == 0 && !(MODE == NB_FILL && if_truncated)) atomicAdd(flag, 1); n_row = kRowMax; }
   for (int q = lane; q < n_row; q += 32) {                  // rank sort: the keys of a row are distinct
     const unsigned k = keys[wib][q];
     int rank = 0;
     for (int r = 0; r < n_row; ++r) rank += keys[wib][r] < k;
-    if (beg + rank < capacity) {
-      const unsigned code = k % 27u;
-      idx[beg + rank] = (int)(k / 27u);
-      shift[3 * (beg + rank)] = (signed char)((int)(code / 9u) - 1);
-      shift[3 * (beg + rank) + 1] = (signed char)((int)((code / 3u) % 3u) - 1);
-      shift[3 * (beg + rank) + 2] = (signed char)((int)(code % 3u) - 1);
-    }
+    sorted_keys[wib][rank] = k;
+  }
+  __syncwarp();
+  if (MODE == NB_STASH) {
+    unsigned long long base = 0;
+    if (lane == 0) base = atomicAdd(cursor, (unsigned long long)n_row);
+    base = __shfl_sync(full, base, 0);
+    const bool fits = base + (unsigned long long)n_row <= (unsigned long long)capacity;
+    if (lane == 0) tstart[i] = fits ? (int)base : -1;
+    if (fits) for (int q = lane; q < n_row; q += 32) tmp[base + q] = sorted_keys[wib][q];
+    return;
+  }
+  const long long beg = off[i];
+  const long long room = capacity - beg;                    // entries of this row that fit
+  for (int q = lane; q < n_row && q < room; q += 32) idx[beg + q] = (int)(sorted_keys[wib][q] / 27u);
+  for (int b = lane; b < 3 * n_row && b < 3 * room; b += 32) {
+    const unsigned code = sorted_keys[wib][b / 3] % 27u;
+    const int comp = b % 3;
+    shift[3 * beg + b] = (signed char)((int)(comp == 0 ? code / 9u : comp == 1 ? (code / 3u) % 3u : code % 3u) - 1);
+  }
+}
+
+// the stashed rows (NB_STASH) to their places in the list: a copy, one warp per atom
+__global__ void __launch_bounds__(256) k_nb_place(const long long *__restrict__ off, const int *__restrict__ count,
+                                                  const int *__restrict__ tstart, const unsigned *__restrict__ tmp, int n, long long capacity,
+                                                  int *__restrict__ idx, signed char *__restrict__ shift) {
+  if (off[n] > capacity) return;                             // truncated list: the NB_FILL pass behind this one writes it
+  const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (i >= n) return;
+  const int n_row = min(count[i], kRowMax), ts = tstart[i];
+  if (ts < 0) return;
+  const long long beg = off[i];
+  for (int q = lane; q < n_row; q += 32) idx[beg + q] = (int)(tmp[ts + q] / 27u);
+  for (int b = lane; b < 3 * n_row; b += 32) {
+    const unsigned code = tmp[ts + b / 3] % 27u;
+    const int comp = b % 3;
+    shift[3 * beg + b] = (signed char)((int)(comp == 0 ? code / 9u : comp == 1 ? (code / 3u) % 3u : code % 3u) - 1);
   }
 }
 
@@ -276,13 +353,14 @@ __global__ void k_wrap(NbGrid g, int n, double *__restrict__ pos) {
   const double w0 = floor(x * g.Hi[0] + y * g.Hi[3] + z * g.Hi[6]), w1 = floor(x * g.Hi[1] + y * g.Hi[4] + z * g.Hi[7]),
                w2 = floor(x * g.Hi[2] + y * g.Hi[5] + z * g.Hi[8]);
   if (w0 == 0.0 && w1 == 0.0 && w2 == 0.0) return;
+  if (!(fabs(w0) < 1073741824.0 && fabs(w1) < 1073741824.0 && fabs(w2) < 1073741824.0)) return;   // left to k_nb_cells to count
   pos[3 * (size_t)i] = x - (w0 * g.H[0] + w1 * g.H[3] + w2 * g.H[6]);
   pos[3 * (size_t)i + 1] = y - (w0 * g.H[1] + w1 * g.H[4] + w2 * g.H[7]);
   pos[3 * (size_t)i + 2] = z - (w0 * g.H[2] + w1 * g.H[5] + w2 * g.H[8]);
 }
 size_t al(size_t x) { return (x + 255) & ~(size_t)255; }
 struct NbLayout {
-  size_t cell, wrap, ccount, cursor, start, totals, sorted, pos_s, rcount, flag, total;
+  size_t cell, wrap, ccount, cursor, start, totals, sorted, pos_s, rcount, tstart, flag, total;
 };
 NbLayout nb_layout(long long n, long long n_cells) {
   NbLayout L;
@@ -296,6 +374,7 @@ NbLayout nb_layout(long long n, long long n_cells) {
   L.sorted = o; o = al(o + (size_t)n * 4);
   L.pos_s = o; o = al(o + (size_t)n * 32);
   L.rcount = o; o = al(o + (size_t)n * 4);
+  L.tstart = o; o = al(o + (size_t)n * 4);
   L.flag = o; o = al(o + 16);
   L.total = o;
   return L;
@@ -339,17 +418,35 @@ cudaError_t launch_neighbors_build(const NbGrid &g, long long n, const double *p
   if (e != cudaSuccess) return e;
   if (n == 0) { e = cudaMemsetAsync(off, 0, 8, st); if (e == cudaSuccess && !accumulate) e = cudaMemsetAsync(info, 0, 16, st); return e; }
   const int nb = (int)((n + 255) / 256);
-  k_nb_cells<<<nb, 256, 0, st>>>(g, pos, (int)n, cell, wrap, ccount);
+  k_nb_cells<<<nb, 256, 0, st>>>(g, pos, (int)n, cell, wrap, ccount, flag);
   e = launch_scan(ccount, n_cells, start, totals, st);
   if (e != cudaSuccess) return e;
   k_nb_scatter<<<nb, 256, 0, st>>>(cell, (int)n, start, cursor, sorted);
   k_nb_sort_cells<<<(unsigned)((n_cells + 255) / 256), 256, 0, st>>>(start, (int)n_cells, sorted);
-  k_nb_gather_pos<<<nb, 256, 0, st>>>(pos, sorted, (int)n, pos_s);
+  k_nb_gather_pos<<<nb, 256, 0, st>>>(pos, sorted, wrap, (int)n, pos_s);
   const double r2 = r_list * r_list;
-  k_nb_rows<false><<<(unsigned)((n + 7) / 8), 256, 0, st>>>(g, pos_s, cell, wrap, start, (int)n, r2, rcount, nullptr, 0, nullptr, nullptr, flag);
-  e = launch_scan(rcount, n, off, totals, st);
-  if (e != cudaSuccess) return e;
-  k_nb_rows<true><<<(unsigned)((n + 7) / 8), 256, 0, st>>>(g, pos_s, cell, wrap, start, (int)n, r2, rcount, off, capacity, idx, shift, flag);
+  const unsigned nw = (unsigned)((n + 7) / 8);
+  int *tstart = (int *)(w + L.tstart);
+  unsigned long long *claim = (unsigned long long *)(flag + 2);        // bytes 8 .. 15 of the flag block (zeroed above)
+  if (rev && capacity > 0) {
+    // one search: rows stashed in the rev array (overwritten by k_nb_rev afterwards), placed once the offsets exist
+    k_nb_rows<NB_STASH><<<nw, 256, 0, st>>>(g, pos_s, cell, wrap, start, (int)n, r2, rcount, nullptr, capacity, nullptr, nullptr, flag, 0,
+                                            tstart, (unsigned *)rev, claim);
+    e = launch_scan(rcount, n, off, totals, st);
+    if (e != cudaSuccess) return e;
+    k_nb_place<<<nw, 256, 0, st>>>(off, rcount, tstart, (const unsigned *)rev, (int)n, capacity, idx, shift);
+    k_nb_rows<NB_FILL><<<nw, 256, 0, st>>>(g, pos_s, cell, wrap, start, (int)n, r2, rcount, off, capacity, idx, shift, flag, 1, nullptr,
+                                           nullptr, nullptr);
+    count_launch();
+  } else {
+    k_nb_rows<NB_COUNT><<<nw, 256, 0, st>>>(g, pos_s, cell, wrap, start, (int)n, r2, rcount, nullptr, 0, nullptr, nullptr, flag, 0, nullptr,
+                                            nullptr, nullptr);
+    e = launch_scan(rcount, n, off, totals, st);
+    if (e != cudaSuccess) return e;
+    if (capacity > 0)
+      k_nb_rows<NB_FILL><<<nw, 256, 0, st>>>(g, pos_s, cell, wrap, start, (int)n, r2, rcount, off, capacity, idx, shift, flag, 0, nullptr,
+                                             nullptr, nullptr);
+  }
   if (rev) k_nb_rev<<<(unsigned)((n + 7) / 8), 256, 0, st>>>(off, idx, shift, (int)n, capacity, rev, flag);
   k_nb_finish<<<1, 1, 0, st>>>(off, (int)n, flag, info, accumulate);
   for (int q = 0; q < 8; ++q) count_launch();
@@ -384,7 +481,7 @@ cudaError_t launch_ke(int n, const double *vel, const int *type, const double *m
 // on the GPU (different streams without ordering) race; calls on one stream, or ordered by events, do not.
 namespace {
 constexpr long long kNbStaticAtoms = MTP_NB_STATIC_MAX_ATOMS;
-constexpr size_t kNbStaticBytes = (size_t)6 << 20;          // nb_workspace_bytes(32 768) = 6 033 408
+constexpr size_t kNbStaticBytes = (size_t)6 << 20;          // nb_workspace_bytes(32 768) = 6 164 480
 static __device__ __align__(256) unsigned char g_nb_static[kNbStaticBytes];
 
 constexpr int kMaxDevices = 64;

@@ -70,9 +70,14 @@ def test_capacity_and_count_only(lib, torch):
     pos = torch.as_tensor(w.pos).cuda()
     nb = lib.neighbors_build(pos, w.box, 5.0, capacity=0)
     assert nb["nnz"] == w.nnz and np.array_equal(nb["off"].cpu().numpy(), w.off)
-    nb = lib.neighbors_build(pos, w.box, 5.0, capacity=1000)           # truncated: the count still says what is needed
-    assert nb["nnz"] == w.nnz
-    assert np.array_equal(nb["idx"].cpu().numpy()[:1000], w.idx[:1000])
+    for want_rev in (True, False):                                      # truncated: the count still says what is needed,
+        nb = lib.neighbors_build(pos, w.box, 5.0, capacity=1000, want_rev=want_rev)   # the first `capacity` pairs are there
+        assert nb["nnz"] == w.nnz
+        assert np.array_equal(nb["idx"].cpu().numpy()[:1000], w.idx[:1000])
+        assert np.array_equal(nb["shift"].cpu().numpy()[:1000], w.shift[:1000])
+    nb = lib.neighbors_build(pos, w.box, 5.0, want_rev=False)           # the two-search form (no rev array to stash rows in)
+    assert nb["nnz"] == w.nnz and np.array_equal(nb["idx"].cpu().numpy()[:w.nnz], w.idx)
+    assert np.array_equal(nb["shift"].cpu().numpy()[:w.nnz], w.shift)
 
 
 def test_config4_sampled_rows(lib, torch):
@@ -101,6 +106,22 @@ def test_host_positions_path_equals_host_list_path(lib, torch):
     c = pot.compute_host_pos(w.pos, w.types, w.box)                     # second call: buffers already sized
     assert np.array_equal(b["F"], c["F"])
     pot.close()
+
+
+def test_coordinates_that_are_not_finite_are_counted_not_followed(lib, torch):
+    """An MD run that blew up hands the list build NaN / inf / 1e300: no fault, d_info[1] counts them, the other atoms'
+    rows are those of the brute-force search without the bad atoms' pairs."""
+    w = make_workload(0, 1)
+    pos = w.pos.copy()
+    bad = [3, 40, 77]
+    pos[3, 0] = np.nan; pos[40, 1] = np.inf; pos[77, 2] = -1e300
+    off, idx, sh, rev, nb = build(lib, torch, pos, w.box, 5.0)
+    assert nb["errors"] == 3
+    b_off, b_idx, b_sh = neighbor_list_bruteforce(w.pos, w.box, 5.0)
+    for i in range(w.n_atoms):
+        keep = ~np.isin(b_idx[b_off[i]:b_off[i + 1]], bad)
+        want = b_idx[b_off[i]:b_off[i + 1]][keep] if i not in bad else np.zeros(0, dtype=np.int32)
+        assert np.array_equal(idx[off[i]:off[i + 1]], want), i
 
 
 def test_velocity_verlet_loop(lib, torch):
