@@ -42,11 +42,11 @@ def metric_name(config, w):
     return "MTP energy+force atom-evals/s at %d atoms lev%d fp64" % (w.n_atoms, w.lev_max)
 
 
-def flops_per_step(cost, w):
+def flops_per_step(cost, n_pairs, n_atoms):
     """Algorithmic flops of one step per kernel class (FMA = 2, each quantity once; formulas: DESIGN.md section 6,
-    numbers from mtp_cost_model)."""
-    return {"moments": cost["flop_per_pair_k1"] * w.nnz, "pairgrad": cost["flop_per_pair_k3"] * w.nnz,
-            "tree": cost["flop_per_atom_tree"] * w.n_atoms}
+    numbers from mtp_cost_model) for the pairs and atoms this rank evaluates."""
+    return {"moments": cost["flop_per_pair_k1"] * n_pairs, "pairgrad": cost["flop_per_pair_k3"] * n_pairs,
+            "tree": cost["flop_per_atom_tree"] * n_atoms}
 
 
 class ClockSampler:
@@ -125,12 +125,12 @@ def build_workload(config, cells, n_basis, seed_shift=0):
     return w, CONFIGS[config]
 
 
-def config_dict(w, cfg, world):
+def config_dict(w, cfg, world, sharded=False):
     """What the workload is -- the same dictionary in both arms."""
     return {"workload": cfg["name"], "n_atoms": w.n_atoms, "nnz": w.nnz, "lev_max": w.lev_max, "n_species": w.n_species,
             "n_basis": int(w.xi.shape[0]),
             "l2": "inputs larger than L2 (neighbour list %.0f MB + per-pair scratch), no flush" % (w.nnz * 11 / 1e6),
-            "parallelism": "replicas x%d" % world}
+            "parallelism": ("atom ranges x%d, all-reduce of F" if sharded else "replicas x%d") % world}
 
 
 # ---------------------------------------------------------------- the oracle, timed on the host cores
@@ -259,7 +259,9 @@ def run_ours(args):
 
     import paper_2510_00193_b200 as lib           # raises if libmtp_b200.so is missing: there is no fallback
     table = lib.Table(LEVELS[args.config])
-    w, cfg = build_workload(args.config, args.cells, table.n_basis, seed_shift=rank)
+    # replicas (default, weak scaling): every rank its own seeded system; --sharded (strong scaling): one system, the
+    # atoms cut into contiguous ranges, one all-reduce of the partial forces per step (paper_2510_00193_b200/sharded.py)
+    w, cfg = build_workload(args.config, args.cells, table.n_basis, seed_shift=0 if args.sharded else rank)
 
     # ---- CPU baseline first (processes are forked before this process touches CUDA): the oracle on a bounded
     # sample of the same workload, all host cores
@@ -294,7 +296,18 @@ def run_ours(args):
     shift, rev = t(w.shift, torch.int8), t(w.rev, torch.int32)
     Ainv = t(w.Ainv, torch.float64) if (args.grade and w.Ainv is not None) else None
 
+    if args.sharded:
+        from paper_2510_00193_b200 import sharded
+        lo, hi = sharded.balanced_row_range(w.off, rank, world)
+        off_w, idx_w, shift_w = (t(a, dt) for a, dt in zip(sharded.window_list(w.off, w.idx, w.shift, lo, hi),
+                                                           (torch.int64, torch.int32, torch.int8)))
+
     def step(out=None):
+        if args.sharded:
+            o = pot.compute_rows(pos, types, w.box, lo, hi, off_w, idx_w, shift_w, out=out)
+            if dist is not None:
+                sharded.all_reduce_sum(dist, o["F"], o["E"], o["virial"])
+            return o
         o = pot.compute(pos, types, w.box, off, idx, shift, rev, out=out)
         if Ainv is not None:
             pot.grade(pos, types, w.box, off, idx, Ainv, shift, mode=2)
@@ -325,11 +338,12 @@ def run_ours(args):
     ms = e0.elapsed_time(e1)
     prof = pot.profile_read()
     ms = max_over_ranks(ms, dist, dev)
-    value = whole_job_rate(w.n_atoms, args.steps, ms * 1e-3, world, None, dev)
+    # replicas: every rank evaluated its own n_atoms; sharded: the ranks evaluated one system together
+    value = whole_job_rate(w.n_atoms, args.steps, ms * 1e-3, 1 if args.sharded else world, None, dev)
 
     # ---- small systems: the same call replayed from a CUDA graph (launch overhead removed)
     graph = None
-    if w.n_atoms <= 16384 and Ainv is None and world == 1:
+    if w.n_atoms <= 16384 and Ainv is None and world == 1 and not args.sharded:
         gms = graph_replay(torch, lib, pot, step, out)
         graph = {"calls": 100, "ms_per_call": gms, "value": w.n_atoms / (gms * 1e-3), "unit": UNIT}
 
@@ -351,6 +365,8 @@ def run_ours(args):
         torch.cuda.synchronize()
         return whole_job_rate(w.n_atoms, e2e_steps, time.perf_counter() - t0, world, dist, dev)
 
+
+    # (the host entry points and the MD loop evaluate a whole system per rank: these legs are replicas in either mode)
     e2e_list_value = timed_host(lambda: pot.compute_host(hp["pos"], hp["types"], w.box, hp["off"], hp["idx"], hp["shift"], hp["rev"], out=hout))
     h2d_list = sum(hp[k].nbytes for k in hp)
     e2e_value = timed_host(lambda: pot.compute_host_pos(hp["pos"], hp["types"], w.box, out=hout))
@@ -392,7 +408,8 @@ def run_ours(args):
         return
 
     # ---- roofline of the dominant kernel (fp64 ALU bound)
-    per_step = flops_per_step(pot.cost_model(), w)
+    per_step = flops_per_step(pot.cost_model(), int(w.off[hi] - w.off[lo]), hi - lo) if args.sharded else \
+        flops_per_step(pot.cost_model(), w.nnz, w.n_atoms)
     timed = {k: prof[k] for k in ("moments", "tree", "pairgrad")}
     dom = max(timed, key=lambda k: timed[k][0])
     dom_ms, dom_n = timed[dom]
@@ -415,9 +432,9 @@ def run_ours(args):
 
     line = {
         "metric": metric_name(args.config, w), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": config_dict(w, cfg, world),
+        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "scaling": "strong" if args.sharded else "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": config_dict(w, cfg, world, args.sharded),
         "run": {"chunk_atoms": pot.get_option(lib.OPT_CHUNK_ATOMS), "force_mode": pot.get_option(lib.OPT_FORCE_MODE),
                 "grade": bool(Ainv is not None), "tree_kernels": pot.get_option(lib.INFO_TREE_KERNELS),
                 "tree_programs": pot.get_option(lib.INFO_TREE_PROGRAMS), "tree_note": pot.last_error(),
@@ -472,6 +489,8 @@ def main():
                     help="atoms per core of an oracle sample (default: 8192 for cpu_baseline, 1024 per step for --impl reference)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-md", action="store_true", help="skip the MD-loop leg")
+    ap.add_argument("--sharded", action="store_true",
+                    help="N > 1: one system cut into atom ranges with an all-reduce of F per step (strong scaling) instead of replicas")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

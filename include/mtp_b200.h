@@ -166,6 +166,32 @@ int mtp_compute_host(mtp_handle *h, int64_t n_atoms, const double *pos, const in
                      const int8_t *shift, const int32_t *rev, int64_t nnz, double *E,
                      double *Ei, double *F, double *virial);
 
+/* One rank's share of a sharded evaluation ("full node" runs): the atoms are
+ * cut into contiguous ranges, positions and types are replicated, and every rank holds the CSR rows of its own range
+ * only.  mtp_compute_rows evaluates the rows [row_lo, row_hi) of an n_atoms system:
+ *   d_off [row_hi - row_lo + 1] the window's own CSR (d_off[0] = 0), d_idx / d_shift [nnz] its pairs, d_idx holding
+ *   GLOBAL atom indices; d_pos / d_type cover all n_atoms.
+ *   d_F [n_atoms][3]: zeroed, then F_i += d_ij and F_j -= d_ij for the window's pairs (fp64 atomics: a window has no
+ *   reverse pairs to gather, so MTP_FORCE_GATHER is refused) -- the rank's PARTIAL force on every atom;
+ *   d_Ei [n_atoms] or NULL: entries [row_lo, row_hi) are written; d_E, d_virial: the window's partial sums.
+ *   Summing d_F, d_E, d_virial over the ranks (one all-reduce of 3 n_atoms + 7 doubles) gives mtp_compute's result
+ *   to rounding (the summation order differs).  Workspace: mtp_rows_workspace_bytes(h, n_atoms, n_rows, nnz, 0).
+ * mtp_grade_rows: neighbourhood grades of the window (d_gamma_atom [n_atoms], entries of the window written; no
+ *   exchange needed) and the window's sum of basis values d_Bsum [n_basis]; the configuration grade follows from the
+ *   all-reduced sum through mtp_grade_cfg_from_sum (the GEMV of mtp_grade's mode 1).  Workspace: want_grade = 1. */
+int mtp_rows_workspace_bytes(const mtp_handle *h, int64_t n_atoms, int64_t n_rows, int64_t nnz, int want_grade,
+                             size_t *out_bytes);
+int mtp_compute_rows(mtp_handle *h, int64_t n_atoms, const double *d_pos, const int32_t *d_type, const double *box,
+                     int64_t row_lo, int64_t row_hi, const int64_t *d_off, const int32_t *d_idx, const int8_t *d_shift,
+                     int64_t nnz, double *d_E, double *d_Ei, double *d_F, double *d_virial, void *d_ws, size_t ws_bytes,
+                     void *cuda_stream);
+int mtp_grade_rows(mtp_handle *h, int64_t n_atoms, const double *d_pos, const int32_t *d_type, const double *box,
+                   int64_t row_lo, int64_t row_hi, const int64_t *d_off, const int32_t *d_idx, const int8_t *d_shift,
+                   int64_t nnz, const double *d_Ainv, double *d_gamma_atom, double *d_Bsum, void *d_ws, size_t ws_bytes,
+                   void *cuda_stream);
+int mtp_grade_cfg_from_sum(mtp_handle *h, const double *d_Bsum, const double *d_Ainv, double *d_gamma_cfg,
+                           void *cuda_stream);
+
 /* Device neighbour list and MD loop (the paper's rates are atom-timesteps/s of a
  * whole MD step, list builds included; its GPU runs take the list from the host code).
  *

@@ -38,7 +38,8 @@ EXPORTS = ["mtp_enumerate", "mtp_table_free", "mtp_create", "mtp_destroy", "mtp_
            "mtp_set_option", "mtp_get_option", "mtp_workspace_bytes", "mtp_compute", "mtp_grade",
            "mtp_compute_host", "mtp_debug_moments", "mtp_launch_count", "mtp_peak_dfma",
            "mtp_cost_model", "mtp_profile_read", "mtp_table_plan", "mtp_k2_program",
-           "mtp_neighbors_workspace_bytes", "mtp_neighbors_build", "mtp_neighbors_build_static", "mtp_md_workspace_bytes", "mtp_md_run",
+           "mtp_neighbors_workspace_bytes", "mtp_neighbors_build", "mtp_neighbors_build_static",
+           "mtp_rows_workspace_bytes", "mtp_compute_rows", "mtp_grade_rows", "mtp_grade_cfg_from_sum", "mtp_md_workspace_bytes", "mtp_md_run",
            "mtp_compute_host_pos"]
 
 
@@ -84,6 +85,10 @@ def _load():
     lib.mtp_table_plan.argtypes = [C.POINTER(MtpParams), C.POINTER(i64)]
     lib.mtp_neighbors_workspace_bytes.argtypes = [i64, C.POINTER(C.c_size_t)]
     lib.mtp_neighbors_build.argtypes = [i64, vp, C.POINTER(dbl), dbl, i64, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
+    lib.mtp_rows_workspace_bytes.argtypes = [vp, i64, i64, i64, C.c_int, C.POINTER(C.c_size_t)]
+    lib.mtp_compute_rows.argtypes = [vp, i64, vp, vp, C.POINTER(dbl), i64, i64, vp, vp, vp, i64, vp, vp, vp, vp, vp, C.c_size_t, vp]
+    lib.mtp_grade_rows.argtypes = [vp, i64, vp, vp, C.POINTER(dbl), i64, i64, vp, vp, vp, i64, vp, vp, vp, vp, C.c_size_t, vp]
+    lib.mtp_grade_cfg_from_sum.argtypes = [vp, vp, vp, vp, vp]
     lib.mtp_neighbors_build_static.argtypes = [i64, vp, C.POINTER(dbl), dbl, i64, vp, vp, vp, vp, vp, vp]
     lib.mtp_md_workspace_bytes.argtypes = [vp, i64, i64, C.POINTER(C.c_size_t)]
     lib.mtp_md_run.argtypes = [vp, i64, vp, vp, vp, C.POINTER(dbl), C.POINTER(dbl), dbl, i64, C.c_int32, dbl, i64,
@@ -297,6 +302,43 @@ class Potential:
                                    _ptr(Ainv), int(mode), _ptr(out["gamma_atom"]), _ptr(out["gamma_cfg"]),
                                    _ptr(out["Bsum"]), _ptr(out["B"]), _ptr(ws), ws.numel(), self._stream(stream)))
         return out
+
+    def compute_rows(self, pos, types, box, row_lo, row_hi, off, idx, shift=None, out=None, stream=None):
+        """mtp_compute_rows: the rows [row_lo, row_hi) of the system (off = the window's own CSR, idx global).
+        Returns dict(E[1], Ei[N], F[N,3], virial[6]) -- PARTIAL sums, to be added over the ranks."""
+        import torch
+        n, nnz, dev = int(pos.shape[0]), int(idx.shape[0]), pos.device
+        if out is None:
+            out = dict(E=torch.empty(1, dtype=torch.float64, device=dev), Ei=torch.zeros(n, dtype=torch.float64, device=dev),
+                       F=torch.empty((n, 3), dtype=torch.float64, device=dev), virial=torch.empty(6, dtype=torch.float64, device=dev))
+        wsb = C.c_size_t()
+        self._check(_lib.mtp_rows_workspace_bytes(self._h, n, int(row_hi - row_lo), nnz, 0, C.byref(wsb)))
+        ws = self._workspace(int(wsb.value), dev)
+        boxh = (C.c_double * 9)(*[float(x) for x in np.asarray(box, dtype=np.float64).reshape(9)])
+        self._check(_lib.mtp_compute_rows(self._h, n, _ptr(pos), _ptr(types), boxh, int(row_lo), int(row_hi), _ptr(off), _ptr(idx),
+                                          _ptr(shift), nnz, _ptr(out["E"]), _ptr(out.get("Ei")), _ptr(out["F"]), _ptr(out["virial"]),
+                                          _ptr(ws), ws.numel(), self._stream(stream)))
+        return out
+
+    def grade_rows(self, pos, types, box, row_lo, row_hi, off, idx, Ainv, shift=None, stream=None):
+        """mtp_grade_rows: dict(gamma_atom[N] (window entries written), Bsum[n_basis] = the window's sum of B)."""
+        import torch
+        n, nnz, dev = int(pos.shape[0]), int(idx.shape[0]), pos.device
+        out = dict(gamma_atom=torch.zeros(n, dtype=torch.float64, device=dev), Bsum=torch.empty(self.n_basis, dtype=torch.float64, device=dev))
+        wsb = C.c_size_t()
+        self._check(_lib.mtp_rows_workspace_bytes(self._h, n, int(row_hi - row_lo), nnz, 1, C.byref(wsb)))
+        ws = self._workspace(int(wsb.value), dev)
+        boxh = (C.c_double * 9)(*[float(x) for x in np.asarray(box, dtype=np.float64).reshape(9)])
+        self._check(_lib.mtp_grade_rows(self._h, n, _ptr(pos), _ptr(types), boxh, int(row_lo), int(row_hi), _ptr(off), _ptr(idx),
+                                        _ptr(shift), nnz, _ptr(Ainv), _ptr(out["gamma_atom"]), _ptr(out["Bsum"]), _ptr(ws), ws.numel(),
+                                        self._stream(stream)))
+        return out
+
+    def grade_cfg_from_sum(self, Bsum, Ainv, stream=None):
+        import torch
+        g = torch.empty(1, dtype=torch.float64, device=Bsum.device)
+        self._check(_lib.mtp_grade_cfg_from_sum(self._h, _ptr(Bsum), _ptr(Ainv), _ptr(g), self._stream(stream)))
+        return g
 
     def debug_moments(self, pos, types, box, off, idx, shift=None, stream=None):
         """M, G as [n_basic][N] and B [N][n_basis] from one K1+K2 pass."""

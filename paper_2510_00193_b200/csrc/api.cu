@@ -673,9 +673,13 @@ struct Plan {
 };
 size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
-int make_plan(const mtp_handle *h, int64_t N, int64_t nnz, int want_grade, int has_rev, Plan &pl, int64_t cap_exact = -1) {
-  if (N < 0 || nnz < 0) return MTP_EINVAL;
-  if (N > (1LL << 27)) return MTP_EUNSUP;      // neighbour words carry 27 index bits (pair_kernels.cuh)
+// rows: atoms whose rows are evaluated (a window of the N atoms: mtp_compute_rows), -1 = all of them.  pos4 / Ei cover
+// all N atoms, chunks and per-chunk scratch only the window.
+int make_plan(const mtp_handle *h, int64_t n_all, int64_t nnz, int want_grade, int has_rev, Plan &pl, int64_t cap_exact = -1,
+              int64_t rows = -1) {
+  if (n_all < 0 || nnz < 0 || rows > n_all) return MTP_EINVAL;
+  if (n_all > (1LL << 27)) return MTP_EUNSUP;      // neighbour words carry 27 index bits (pair_kernels.cuh)
+  const int64_t N = rows < 0 ? n_all : rows;
   pl.N = N; pl.nnz = nnz;
   int64_t C = h->chunk_atoms;
   if (C <= 0) {   // automatic: many waves per launch (no tail), M + G scratch (16 B x n_basic per atom) <= 1 GB
@@ -702,8 +706,8 @@ int make_plan(const mtp_handle *h, int64_t N, int64_t nnz, int want_grade, int h
   pl.atomic = h->force_mode == MTP_FORCE_ATOMIC || (h->force_mode == MTP_FORCE_AUTO && !has_rev);
   pl.grid_chunk = pl.sliced ? h->pl->pairgrad_grid_s((int)C) : h->pl->pairgrad_grid((int)C, pl.P);
   size_t o = 0;
-  pl.o_pos4 = o; o = align_up(o + (size_t)N * 32);
-  pl.o_Ei = o; o = align_up(o + (size_t)N * 8);
+  pl.o_pos4 = o; o = align_up(o + (size_t)n_all * 32);
+  pl.o_Ei = o; o = align_up(o + (size_t)n_all * 8);
   pl.o_M = o; o = align_up(o + (size_t)h->n_basic * pl.cols * 8);
   pl.o_G = o; o = align_up(o + (size_t)h->n_basic * pl.cols * 8);
   pl.o_red = o; o = align_up(o + 256 * 8 * 8);
@@ -868,15 +872,23 @@ struct HostPipe {
 static int compute_impl(mtp_handle *h, int64_t N, const double *d_pos, const int32_t *d_type, const double *box,
                         const int64_t *d_off, const int32_t *d_idx, const int8_t *d_shift, const int32_t *d_rev,
                         int64_t nnz, double *d_E, double *d_Ei, double *d_F, double *d_virial, void *d_ws,
-                        size_t ws_bytes, void *stream, const HostPipe *pipe, int64_t cap_exact = -1) {
+                        size_t ws_bytes, void *stream, const HostPipe *pipe, int64_t cap_exact = -1, int64_t row_lo = 0,
+                        int64_t row_hi = -1) {
+  // [row_lo, row_hi): the atoms whose rows this call evaluates (mtp_compute_rows; d_off then is the window's own CSR,
+  // d_off[0] = 0); the default is all of them
   if (!h) return MTP_EINVAL;
   if (!box || !d_E || (N > 0 && (!d_pos || !d_type || !d_off || !d_F)) || (nnz > 0 && !d_idx))
     return fail(h, MTP_EINVAL, "mtp_compute: null argument");
   if (h->force_mode == MTP_FORCE_GATHER && !d_rev && nnz > 0) return fail(h, MTP_EINVAL, "gather mode needs d_rev");
   cudaStream_t st = (cudaStream_t)stream;
+  const bool window = row_hi >= 0;
+  if (!window) { row_lo = 0; row_hi = N; }
+  if (row_lo < 0 || row_hi < row_lo || row_hi > N) return fail(h, MTP_EINVAL, "row window outside [0, n_atoms]");
+  d_off -= row_lo;                               // the kernels index offsets by atom
   Plan pl;
-  int rc = make_plan(h, N, nnz, 0, d_rev != nullptr, pl, cap_exact);
+  int rc = make_plan(h, N, nnz, 0, d_rev != nullptr, pl, cap_exact, window ? row_hi - row_lo : -1);
   if (rc != MTP_OK) return fail(h, rc, "bad sizes");
+  if (window && !pl.atomic) return fail(h, MTP_EINVAL, "a row window has no reverse pairs to gather: MTP_FORCE_ATOMIC or MTP_FORCE_AUTO");
   const size_t base = align_up((size_t)(uintptr_t)d_ws) - (size_t)(uintptr_t)d_ws;
   if (N > 0 && (!d_ws || ws_bytes < pl.total + base)) return fail(h, MTP_ESIZE, "workspace too small");
   PairArgs pa;
@@ -904,7 +916,7 @@ static int compute_impl(mtp_handle *h, int64_t N, const double *d_pos, const int
   K2Io io{pos4, M, G, Ei, nullptr, 0, 0, 1, N, (double *)(ws + pl.o_S), (double *)(ws + pl.o_Sbar)};
   bool rev_waited = false;
   for (int c = 0; c < pl.n_chunks; ++c) {
-    pa.c0 = (int)(c * pl.C); pa.c1 = (int)std::min<int64_t>(N, (c + 1) * pl.C);
+    pa.c0 = (int)(row_lo + c * pl.C); pa.c1 = (int)std::min<int64_t>(row_hi, row_lo + (c + 1) * pl.C);
     if (pipe) CU(h, cudaStreamWaitEvent(st, (*pipe->chunk_ready)[c], 0));      // this chunk's pairs have arrived
     // the chunk's neighbour words (validated, index + image code in 4 bytes) and the range of atoms it touches
     if (nnz > 0)
@@ -924,7 +936,8 @@ static int compute_impl(mtp_handle *h, int64_t N, const double *d_pos, const int
     }
   }
   double *red = (double *)(ws + pl.o_red);
-  CU(h, launch_reduce(Ei, N, 1, 1, d_E, red, st));
+  if (row_hi > row_lo) CU(h, launch_reduce(Ei + row_lo, row_hi - row_lo, 1, 1, d_E, red, st));
+  else CU(h, launch_zero(d_E, 1, st));
   if (d_virial) CU(h, launch_reduce(wpart, (long long)pl.n_chunks * pl.grid_chunk, 8, 6, d_virial, red, st));
   return MTP_OK;
 }
@@ -937,17 +950,22 @@ extern "C" int mtp_compute(mtp_handle *h, int64_t N, const double *d_pos, const 
                       stream, nullptr);
 }
 
-extern "C" int mtp_grade(mtp_handle *h, int64_t N, const double *d_pos, const int32_t *d_type, const double *box,
-                         const int64_t *d_off, const int32_t *d_idx, const int8_t *d_shift, int64_t nnz,
-                         const double *d_Ainv, int mode, double *d_gamma_atom, double *d_gamma_cfg, double *d_Bsum,
-                         double *d_B, void *d_ws, size_t ws_bytes, void *stream) {
+static int grade_impl(mtp_handle *h, int64_t N, const double *d_pos, const int32_t *d_type, const double *box,
+                      const int64_t *d_off, const int32_t *d_idx, const int8_t *d_shift, int64_t nnz,
+                      const double *d_Ainv, int mode, double *d_gamma_atom, double *d_gamma_cfg, double *d_Bsum,
+                      double *d_B, void *d_ws, size_t ws_bytes, void *stream, int64_t row_lo = 0, int64_t row_hi = -1) {
+  // [row_lo, row_hi): as in compute_impl; gamma_atom and B stay indexed by atom
   if (!h) return MTP_EINVAL;
+  const bool window = row_hi >= 0;
+  if (!window) { row_lo = 0; row_hi = N; }
+  if (row_lo < 0 || row_hi < row_lo || row_hi > N) return fail(h, MTP_EINVAL, "row window outside [0, n_atoms]");
+  if (d_off) d_off -= row_lo;
   if (!box || !d_Ainv || mode < 0 || mode > 2 || (N > 0 && (!d_pos || !d_type || !d_off)) || (nnz > 0 && !d_idx) ||
       (mode != 1 && N > 0 && !d_gamma_atom) || (mode != 0 && !d_gamma_cfg))
     return fail(h, MTP_EINVAL, "mtp_grade: null or inconsistent argument");
   cudaStream_t st = (cudaStream_t)stream;
   Plan pl;
-  int rc = make_plan(h, N, nnz, 1, 0, pl);
+  int rc = make_plan(h, N, nnz, 1, 0, pl, -1, window ? row_hi - row_lo : -1);
   if (rc != MTP_OK) return fail(h, rc, "bad sizes");
   const size_t base = align_up((size_t)(uintptr_t)d_ws) - (size_t)(uintptr_t)d_ws;
   // one extra n_basis vector at the end holds sum_i B when the caller does not want it
@@ -971,7 +989,7 @@ extern "C" int mtp_grade(mtp_handle *h, int64_t N, const double *d_pos, const in
     pa.idx_cap = d_shift ? pl.cap : nnz;
     K2Io io{pos4, M, G, Ei, nullptr, 0, 0, 0, N, (double *)(ws + pl.o_S), (double *)(ws + pl.o_Sbar)};
     for (int c = 0; c < pl.n_chunks; ++c) {
-      pa.c0 = (int)(c * pl.C); pa.c1 = (int)std::min<int64_t>(N, (c + 1) * pl.C);
+      pa.c0 = (int)(row_lo + c * pl.C); pa.c1 = (int)std::min<int64_t>(row_hi, row_lo + (c + 1) * pl.C);
       if (nnz > 0)
         CU(h, launch_pack_pairs_chunk((const long long *)d_off, pa.c0, pa.c1, d_idx, (const signed char *)d_shift, N, pl.cap,
                                       d_shift ? idxp : nullptr, h->d_flag, jrange, st));
@@ -988,6 +1006,56 @@ extern "C" int mtp_grade(mtp_handle *h, int64_t N, const double *d_pos, const in
     }
   }
   if (mode != 0) CU(h, launch_grade_cfg(Bsum, d_Ainv, h->n_basis, nullptr, d_gamma_cfg, st));
+  return MTP_OK;
+}
+
+extern "C" int mtp_grade(mtp_handle *h, int64_t N, const double *d_pos, const int32_t *d_type, const double *box,
+                         const int64_t *d_off, const int32_t *d_idx, const int8_t *d_shift, int64_t nnz,
+                         const double *d_Ainv, int mode, double *d_gamma_atom, double *d_gamma_cfg, double *d_Bsum,
+                         double *d_B, void *d_ws, size_t ws_bytes, void *stream) {
+  return grade_impl(h, N, d_pos, d_type, box, d_off, d_idx, d_shift, nnz, d_Ainv, mode, d_gamma_atom, d_gamma_cfg, d_Bsum, d_B,
+                    d_ws, ws_bytes, stream);
+}
+
+// ---- one rank's share of a sharded evaluation ----------------------------------------
+extern "C" int mtp_rows_workspace_bytes(const mtp_handle *h, int64_t n_atoms, int64_t n_rows, int64_t nnz, int want_grade,
+                                        size_t *out) {
+  if (!h || !out || n_rows < 0) return MTP_EINVAL;
+  Plan pl;
+  int rc = make_plan(h, n_atoms, nnz, want_grade, /*has_rev=*/0, pl, -1, n_rows);
+  if (rc != MTP_OK) return rc;
+  *out = pl.total + 512 + (want_grade ? align_up((size_t)h->n_basis * 8) : 0);
+  return MTP_OK;
+}
+
+extern "C" int mtp_compute_rows(mtp_handle *h, int64_t N, const double *d_pos, const int32_t *d_type, const double *box,
+                                int64_t row_lo, int64_t row_hi, const int64_t *d_off, const int32_t *d_idx, const int8_t *d_shift,
+                                int64_t nnz, double *d_E, double *d_Ei, double *d_F, double *d_virial, void *d_ws,
+                                size_t ws_bytes, void *stream) {
+  if (!h) return MTP_EINVAL;
+  if (row_lo < 0 || row_hi < row_lo) return fail(h, MTP_EINVAL, "row window outside [0, n_atoms]");
+  const int saved = h->force_mode;
+  if (saved == MTP_FORCE_AUTO) h->force_mode = MTP_FORCE_ATOMIC;
+  int rc = compute_impl(h, N, d_pos, d_type, box, d_off, d_idx, d_shift, nullptr, nnz, d_E, d_Ei, d_F, d_virial, d_ws, ws_bytes,
+                        stream, nullptr, -1, row_lo, row_hi);
+  h->force_mode = saved;
+  return rc;
+}
+
+extern "C" int mtp_grade_rows(mtp_handle *h, int64_t N, const double *d_pos, const int32_t *d_type, const double *box,
+                              int64_t row_lo, int64_t row_hi, const int64_t *d_off, const int32_t *d_idx, const int8_t *d_shift,
+                              int64_t nnz, const double *d_Ainv, double *d_gamma_atom, double *d_Bsum, void *d_ws, size_t ws_bytes,
+                              void *stream) {
+  if (!h) return MTP_EINVAL;
+  if (row_lo < 0 || row_hi < row_lo || !d_Bsum) return fail(h, MTP_EINVAL, "mtp_grade_rows: bad argument");
+  return grade_impl(h, N, d_pos, d_type, box, d_off, d_idx, d_shift, nnz, d_Ainv, 0, d_gamma_atom, nullptr, d_Bsum, nullptr, d_ws,
+                    ws_bytes, stream, row_lo, row_hi);
+}
+
+extern "C" int mtp_grade_cfg_from_sum(mtp_handle *h, const double *d_Bsum, const double *d_Ainv, double *d_gamma_cfg, void *stream) {
+  if (!h) return MTP_EINVAL;
+  if (!d_Bsum || !d_Ainv || !d_gamma_cfg) return fail(h, MTP_EINVAL, "mtp_grade_cfg_from_sum: null argument");
+  CU(h, launch_grade_cfg(d_Bsum, d_Ainv, h->n_basis, nullptr, d_gamma_cfg, (cudaStream_t)stream));
   return MTP_OK;
 }
 
