@@ -238,6 +238,31 @@ int mtp_md_run(mtp_handle *h, int64_t n_atoms, double *d_pos, double *d_vel, con
                const double *mass, double dt, int64_t n_steps, int32_t rebuild_every, double skin, int64_t capacity,
                double *d_E, double *d_Ei, double *d_F, double *d_virial, int64_t *d_info, void *d_ws, size_t ws_bytes,
                void *cuda_stream);
+/* Active-learning policy around the grade: mtp_md_run with the extrapolation grade
+ * evaluated on the initial configuration and after every grade_every-th step ("every X timesteps"; 1 = the
+ * MLIP-3 style of PAPER.md:106).  mode 0: the largest neighbourhood grade max_i gamma_i (reduced on the device,
+ * order independent); mode 1: the configuration grade.  A grade above select_threshold keeps the configuration: its
+ * positions go to d_selected[k] (device, [max_selected][N][3], or NULL) and its step and grade to sel_step[k],
+ * sel_grade[k] (HOST, [max_selected]) until max_selected are kept.  A grade above break_threshold ends the run after
+ * that step ("the simulation is immediately terminated").  The decision is taken on the host: every
+ * grade evaluation ends with an 8-byte read and a stream synchronisation; between evaluations the loop only enqueues.
+ *   d_Ainv [n_basis][n_basis]; d_gamma_atom [N] or NULL: the neighbourhood grades of the last evaluation (mode 0);
+ *   out [4] HOST = { steps done, configurations kept, grade evaluations, 1 when stopped at the break threshold };
+ *   max_grade [1] HOST or NULL: the largest grade seen.  Everything else as mtp_md_run.
+ * Training / MaxVol selection of the active set stays outside: A^-1 is an input. */
+typedef struct mtp_al_policy {
+  int32_t grade_every;       /* >= 1 */
+  int32_t mode;              /* 0 neighbourhood, 1 configuration */
+  double select_threshold;
+  double break_threshold;
+  int32_t max_selected;      /* >= 0 */
+} mtp_al_policy;
+int mtp_md_al_workspace_bytes(const mtp_handle *h, int64_t n_atoms, int64_t capacity, size_t *out_bytes);
+int mtp_md_run_al(mtp_handle *h, int64_t n_atoms, double *d_pos, double *d_vel, const int32_t *d_type, const double *box,
+                  const double *mass, double dt, int64_t n_steps, int32_t rebuild_every, double skin, int64_t capacity,
+                  const double *d_Ainv, const mtp_al_policy *policy, double *d_E, double *d_Ei, double *d_F,
+                  double *d_virial, int64_t *d_info, double *d_gamma_atom, double *d_selected, int64_t *sel_step,
+                  double *sel_grade, int64_t *out, double *max_grade, void *d_ws, size_t ws_bytes, void *cuda_stream);
 /* Host positions in, host forces out (what an MD host code does every step): positions and types are copied to the
  * device, the list is built there at R_cut (it never crosses PCIe), the kernels of mtp_compute run in the
  * deterministic force mode, and E, E_i, F, virial are copied back; synchronises.  nnz_out (or NULL): pairs listed. */

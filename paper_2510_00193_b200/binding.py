@@ -34,12 +34,18 @@ class MtpParams(C.Structure):
     ]
 
 
+class AlPolicy(C.Structure):
+    """mtp_al_policy of include/mtp_b200.h"""
+    _fields_ = [("grade_every", C.c_int32), ("mode", C.c_int32), ("select_threshold", C.c_double),
+                ("break_threshold", C.c_double), ("max_selected", C.c_int32)]
+
+
 EXPORTS = ["mtp_enumerate", "mtp_table_free", "mtp_create", "mtp_destroy", "mtp_last_error",
            "mtp_set_option", "mtp_get_option", "mtp_workspace_bytes", "mtp_compute", "mtp_grade",
            "mtp_compute_host", "mtp_debug_moments", "mtp_launch_count", "mtp_peak_dfma",
            "mtp_cost_model", "mtp_profile_read", "mtp_table_plan", "mtp_k2_program",
            "mtp_neighbors_workspace_bytes", "mtp_neighbors_build", "mtp_neighbors_build_static",
-           "mtp_rows_workspace_bytes", "mtp_compute_rows", "mtp_grade_rows", "mtp_grade_cfg_from_sum", "mtp_md_workspace_bytes", "mtp_md_run",
+           "mtp_md_al_workspace_bytes", "mtp_md_run_al", "mtp_rows_workspace_bytes", "mtp_compute_rows", "mtp_grade_rows", "mtp_grade_cfg_from_sum", "mtp_md_workspace_bytes", "mtp_md_run",
            "mtp_compute_host_pos"]
 
 
@@ -85,6 +91,10 @@ def _load():
     lib.mtp_table_plan.argtypes = [C.POINTER(MtpParams), C.POINTER(i64)]
     lib.mtp_neighbors_workspace_bytes.argtypes = [i64, C.POINTER(C.c_size_t)]
     lib.mtp_neighbors_build.argtypes = [i64, vp, C.POINTER(dbl), dbl, i64, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
+    lib.mtp_md_al_workspace_bytes.argtypes = [vp, i64, i64, C.POINTER(C.c_size_t)]
+    lib.mtp_md_run_al.argtypes = [vp, i64, vp, vp, vp, C.POINTER(dbl), C.POINTER(dbl), dbl, i64, C.c_int32, dbl, i64, vp,
+                                  C.POINTER(AlPolicy), vp, vp, vp, vp, vp, vp, vp, C.POINTER(i64), C.POINTER(dbl), C.POINTER(i64),
+                                  C.POINTER(dbl), vp, C.c_size_t, vp]
     lib.mtp_rows_workspace_bytes.argtypes = [vp, i64, i64, i64, C.c_int, C.POINTER(C.c_size_t)]
     lib.mtp_compute_rows.argtypes = [vp, i64, vp, vp, C.POINTER(dbl), i64, i64, vp, vp, vp, i64, vp, vp, vp, vp, vp, C.c_size_t, vp]
     lib.mtp_grade_rows.argtypes = [vp, i64, vp, vp, C.POINTER(dbl), i64, i64, vp, vp, vp, i64, vp, vp, vp, vp, C.c_size_t, vp]
@@ -374,6 +384,36 @@ class Potential:
                                     float(dt), int(n_steps), int(rebuild_every), float(skin), int(capacity), _ptr(out["E"]),
                                     _ptr(out["Ei"]), _ptr(out["F"]), _ptr(out["virial"]), _ptr(out["info"]), _ptr(ws), ws.numel(),
                                     self._stream(stream)))
+        return out
+
+    def md_run_al(self, pos, vel, types, box, mass, dt, n_steps, rebuild_every, skin, capacity, Ainv, grade_every, mode,
+                  select_threshold, break_threshold, max_selected, stream=None):
+        """mtp_md_run_al: the MD loop with the grade policy.  Returns md_run's dict plus gamma_atom[N], selected
+        [n_kept][N][3] (device), sel_step / sel_grade (lists), steps_done, n_evaluations, stopped, max_grade."""
+        import torch
+        n, dev = int(pos.shape[0]), pos.device
+        wsb = C.c_size_t()
+        self._check(_lib.mtp_md_al_workspace_bytes(self._h, n, int(capacity), C.byref(wsb)))
+        ws = self._workspace(int(wsb.value), dev)
+        out = dict(E=torch.empty(2, dtype=torch.float64, device=dev), Ei=torch.empty(n, dtype=torch.float64, device=dev),
+                   F=torch.empty((n, 3), dtype=torch.float64, device=dev), virial=torch.empty(6, dtype=torch.float64, device=dev),
+                   info=torch.zeros(2, dtype=torch.int64, device=dev), gamma_atom=torch.zeros(n, dtype=torch.float64, device=dev))
+        sel = torch.empty((max(int(max_selected), 1), n, 3), dtype=torch.float64, device=dev)
+        pol = AlPolicy(int(grade_every), int(mode), float(select_threshold), float(break_threshold), int(max_selected))
+        sel_step = (C.c_int64 * max(int(max_selected), 1))()
+        sel_grade = (C.c_double * max(int(max_selected), 1))()
+        res = (C.c_int64 * 4)()
+        mx = C.c_double()
+        boxh = (C.c_double * 9)(*[float(x) for x in np.asarray(box, dtype=np.float64).reshape(9)])
+        m = np.ascontiguousarray(mass, dtype=np.float64)
+        self._check(_lib.mtp_md_run_al(self._h, n, _ptr(pos), _ptr(vel), _ptr(types), boxh, m.ctypes.data_as(C.POINTER(C.c_double)),
+                                       float(dt), int(n_steps), int(rebuild_every), float(skin), int(capacity), _ptr(Ainv),
+                                       C.byref(pol), _ptr(out["E"]), _ptr(out["Ei"]), _ptr(out["F"]), _ptr(out["virial"]),
+                                       _ptr(out["info"]), _ptr(out["gamma_atom"]), _ptr(sel), sel_step, sel_grade, res, C.byref(mx),
+                                       _ptr(ws), ws.numel(), self._stream(stream)))
+        k = int(res[1])
+        out.update(selected=sel[:k], sel_step=[int(sel_step[i]) for i in range(k)], sel_grade=[float(sel_grade[i]) for i in range(k)],
+                   steps_done=int(res[0]), n_evaluations=int(res[2]), stopped=bool(res[3]), max_grade=float(mx.value))
         return out
 
     def compute_host_pos(self, pos, types, box, out=None):

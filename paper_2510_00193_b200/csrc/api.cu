@@ -1165,13 +1165,14 @@ extern "C" int mtp_neighbors_build(int64_t N, const double *d_pos, const double 
 namespace {
 // LAMMPS "metal" units: eV, Angstrom, ps, g/mol.  a [A/ps^2] = F [eV/A] / m [g/mol] x kFtm2v
 constexpr double kFtm2v = 1.602176634e-19 / 1.66053906660e-27 * 1e-4;      // 9648.533...
-struct MdLayout { size_t off, idx, shift, rev, info, imass, mass, ke, nbws, ws, total; };
-MdLayout md_layout(const mtp_handle *h, int64_t N, int64_t cap, size_t compute_ws) {
+struct MdLayout { size_t off, idx, shift, rev, info, imass, mass, ke, gamma, gmax, nbws, ws, total; };
+MdLayout md_layout(const mtp_handle *h, int64_t N, int64_t cap, size_t compute_ws, bool policy = false) {
   MdLayout L;
   size_t o = 0;
   auto take = [&](size_t b) { size_t at = o; o = align_up(o + b); return at; };
   L.off = take((size_t)(N + 1) * 8); L.idx = take((size_t)cap * 4); L.shift = take((size_t)cap * 3); L.rev = take((size_t)cap * 4);
   L.info = take(16); L.imass = take((size_t)h->S * 8); L.mass = take((size_t)h->S * 8); L.ke = take((size_t)N * 8);
+  L.gamma = take(policy ? (size_t)N * 8 : 0); L.gmax = take(policy ? 8 : 0);
   L.nbws = take(nb_workspace_bytes(N)); L.ws = take(compute_ws);
   L.total = o;
   return L;
@@ -1187,20 +1188,36 @@ extern "C" int mtp_md_workspace_bytes(const mtp_handle *h, int64_t n_atoms, int6
   return MTP_OK;
 }
 
-extern "C" int mtp_md_run(mtp_handle *h, int64_t N, double *d_pos, double *d_vel, const int32_t *d_type, const double *box,
-                          const double *mass, double dt, int64_t n_steps, int32_t rebuild_every, double skin, int64_t capacity,
-                          double *d_E, double *d_Ei, double *d_F, double *d_virial, int64_t *d_info, void *d_ws, size_t ws_bytes,
-                          void *stream) {
+namespace {
+// what the active-learning policy needs on top of the plain loop (mtp_md_run_al)
+struct MdPolicy {
+  const mtp_al_policy *p = nullptr;
+  const double *d_Ainv = nullptr;
+  double *d_gamma_atom = nullptr;          // [N] or nullptr (then a workspace array)
+  double *d_selected = nullptr;            // [max_selected][N][3] or nullptr
+  int64_t *sel_step = nullptr;             // host [max_selected]
+  double *sel_grade = nullptr;             // host [max_selected]
+  int64_t *out = nullptr;                  // host [4]: steps done, configurations selected, grade evaluations, 1 = stopped at the break threshold
+  double *max_grade = nullptr;             // host [1]: largest grade seen
+};
+
+int md_impl(mtp_handle *h, int64_t N, double *d_pos, double *d_vel, const int32_t *d_type, const double *box, const double *mass,
+            double dt, int64_t n_steps, int32_t rebuild_every, double skin, int64_t capacity, double *d_E, double *d_Ei, double *d_F,
+            double *d_virial, int64_t *d_info, void *d_ws, size_t ws_bytes, void *stream, const MdPolicy *al) {
   if (!h) return MTP_EINVAL;
   if (N <= 0 || !d_pos || !d_vel || !d_type || !box || !mass || !(dt > 0) || n_steps < 0 || rebuild_every < 1 || !(skin >= 0) ||
       capacity <= 0 || capacity > 0x7fffffffLL || !d_E || !d_F || !d_info)
     return fail(h, MTP_EINVAL, "mtp_md_run: bad argument");
+  if (al && (!al->p || !al->d_Ainv || !al->out || al->p->grade_every < 1 || al->p->mode < 0 || al->p->mode > 1 || al->p->max_selected < 0 ||
+             (al->p->max_selected > 0 && (!al->sel_step || !al->sel_grade))))
+    return fail(h, MTP_EINVAL, "mtp_md_run_al: bad policy argument");
   for (int s = 0; s < h->S; ++s) if (!(mass[s] > 0)) return fail(h, MTP_EINVAL, "mtp_md_run: masses must be positive");
   cudaStream_t st = (cudaStream_t)stream;
-  size_t cw = 0;
+  size_t cw = 0, gw = 0;
   int rc = mtp_workspace_bytes(h, N, capacity, 0, &cw);
+  if (rc == MTP_OK && al) rc = mtp_workspace_bytes(h, N, capacity, 1, &gw);
   if (rc != MTP_OK) return rc;
-  const MdLayout L = md_layout(h, N, capacity, cw);
+  const MdLayout L = md_layout(h, N, capacity, std::max(cw, gw), al != nullptr);
   const size_t base = align_up((size_t)(uintptr_t)d_ws) - (size_t)(uintptr_t)d_ws;
   if (!d_ws || ws_bytes < L.total + base) return fail(h, MTP_ESIZE, "workspace too small (mtp_md_workspace_bytes)");
   char *ws = (char *)d_ws + base;
@@ -1226,26 +1243,90 @@ extern "C" int mtp_md_run(mtp_handle *h, int64_t N, double *d_pos, double *d_vel
   auto forces = [&]() {
     return compute_impl(h, N, d_pos, d_type, box, off, idx, shift, rev, capacity, d_E, d_Ei, d_F, d_virial, ws + L.ws, cw, st, nullptr);
   };
+  // grades every X steps; above the selection threshold the configuration is kept, above the break
+  // threshold the run stops.  The decision is the host's, so each evaluation ends with a 8-byte read and a
+  // synchronisation.  0 = go on, 1 = stop, < 0 = error.
+  int64_t n_sel = 0, n_eval = 0;
+  double seen_max = 0.0;
+  auto policy = [&](int64_t step) -> int {
+    double *gamma = al->d_gamma_atom ? al->d_gamma_atom : (double *)(ws + L.gamma);
+    double *gmax = (double *)(ws + L.gmax);
+    int r = grade_impl(h, N, d_pos, d_type, box, off, idx, shift, capacity, al->d_Ainv, al->p->mode == 0 ? 0 : 1, gamma, gmax,
+                       nullptr, nullptr, ws + L.ws, std::max(cw, gw), st);
+    if (r != MTP_OK) return r;
+    if (al->p->mode == 0) CU(h, launch_max_nonneg(gamma, N, gmax, st));       // neighbourhood mode: the largest per-atom grade
+    double m = 0.0;
+    CU(h, cudaMemcpyAsync(&m, gmax, 8, cudaMemcpyDeviceToHost, st));
+    CU(h, cudaStreamSynchronize(st));
+    ++n_eval;
+    seen_max = std::max(seen_max, m);
+    if (m > al->p->select_threshold && n_sel < al->p->max_selected) {
+      if (al->d_selected) CU(h, cudaMemcpyAsync(al->d_selected + (size_t)n_sel * 3 * N, d_pos, (size_t)N * 24, cudaMemcpyDeviceToDevice, st));
+      al->sel_step[n_sel] = step; al->sel_grade[n_sel] = m;
+      ++n_sel;
+    }
+    return m > al->p->break_threshold ? 1 : 0;
+  };
   const int saved_mode = h->force_mode;
   if (h->force_mode == MTP_FORCE_AUTO) h->force_mode = MTP_FORCE_GATHER;      // the list comes with its reverse index
   rc = build();
   if (rc == MTP_OK) rc = forces();
+  int64_t done = 0;
+  int stop = 0;
+  if (rc == MTP_OK && al) { stop = policy(0); if (stop < 0) rc = stop; }
   const double half = 0.5 * dt * kFtm2v;
-  for (int64_t s = 1; s <= n_steps && rc == MTP_OK; ++s) {
+  for (int64_t s = 1; s <= n_steps && rc == MTP_OK && stop == 0; ++s) {
     cudaError_t e = launch_vv((int)N, d_pos, d_vel, d_F, d_type, imass, half, dt, 1, st);      // v(t + dt/2), x(t + dt)
     if (e != cudaSuccess) { rc = cuda_fail(h, e, "launch_vv"); break; }
     if (s % rebuild_every == 0) rc = build();
     if (rc == MTP_OK) rc = forces();                                                            // F(t + dt)
     if (rc != MTP_OK) break;
     e = launch_vv((int)N, d_pos, d_vel, d_F, d_type, imass, half, dt, 0, st);                   // v(t + dt)
-    if (e != cudaSuccess) rc = cuda_fail(h, e, "launch_vv");
+    if (e != cudaSuccess) { rc = cuda_fail(h, e, "launch_vv"); break; }
+    done = s;
+    if (al && s % al->p->grade_every == 0) { stop = policy(s); if (stop < 0) rc = stop; }
   }
   h->force_mode = saved_mode;
   if (rc != MTP_OK) return rc;
   // kinetic energy sum m v^2 / 2 in eV
   CU(h, launch_ke((int)N, d_vel, d_type, dmass, 0.5 / kFtm2v, ke, st));
   CU(h, launch_reduce(ke, N, 1, 1, d_E + 1, nullptr, st));
+  if (al) {
+    al->out[0] = done; al->out[1] = n_sel; al->out[2] = n_eval; al->out[3] = stop > 0 ? 1 : 0;
+    if (al->max_grade) *al->max_grade = seen_max;
+  }
   return MTP_OK;
+}
+}  // namespace
+
+extern "C" int mtp_md_run(mtp_handle *h, int64_t N, double *d_pos, double *d_vel, const int32_t *d_type, const double *box,
+                          const double *mass, double dt, int64_t n_steps, int32_t rebuild_every, double skin, int64_t capacity,
+                          double *d_E, double *d_Ei, double *d_F, double *d_virial, int64_t *d_info, void *d_ws, size_t ws_bytes,
+                          void *stream) {
+  return md_impl(h, N, d_pos, d_vel, d_type, box, mass, dt, n_steps, rebuild_every, skin, capacity, d_E, d_Ei, d_F, d_virial, d_info,
+                 d_ws, ws_bytes, stream, nullptr);
+}
+
+extern "C" int mtp_md_al_workspace_bytes(const mtp_handle *h, int64_t n_atoms, int64_t capacity, size_t *out) {
+  if (!h || !out || n_atoms < 0 || capacity < 0) return MTP_EINVAL;
+  size_t cw = 0, gw = 0;
+  int rc = mtp_workspace_bytes(h, n_atoms, capacity, 0, &cw);
+  if (rc == MTP_OK) rc = mtp_workspace_bytes(h, n_atoms, capacity, 1, &gw);
+  if (rc != MTP_OK) return rc;
+  *out = md_layout(h, n_atoms, capacity, std::max(cw, gw), true).total + 512;
+  return MTP_OK;
+}
+
+extern "C" int mtp_md_run_al(mtp_handle *h, int64_t N, double *d_pos, double *d_vel, const int32_t *d_type, const double *box,
+                             const double *mass, double dt, int64_t n_steps, int32_t rebuild_every, double skin, int64_t capacity,
+                             const double *d_Ainv, const mtp_al_policy *policy, double *d_E, double *d_Ei, double *d_F,
+                             double *d_virial, int64_t *d_info, double *d_gamma_atom, double *d_selected, int64_t *sel_step,
+                             double *sel_grade, int64_t *out, double *max_grade, void *d_ws, size_t ws_bytes, void *stream) {
+  MdPolicy al;
+  al.p = policy; al.d_Ainv = d_Ainv; al.d_gamma_atom = d_gamma_atom; al.d_selected = d_selected; al.sel_step = sel_step;
+  al.sel_grade = sel_grade; al.out = out; al.max_grade = max_grade;
+  return md_impl(h, N, d_pos, d_vel, d_type, box, mass, dt, n_steps, rebuild_every, skin, capacity, d_E, d_Ei, d_F, d_virial, d_info,
+                 d_ws, ws_bytes, stream, &al);
 }
 
 // Host positions in, host forces out: the neighbour list never crosses PCIe (it is built on the device at R_cut).

@@ -7,6 +7,8 @@
 // maximum across column tiles is an integer atomicMax (order independent -> deterministic).
 #include <cuda_runtime.h>
 
+#include <algorithm>
+
 #include "kernels.h"
 
 namespace mtpb {
@@ -110,6 +112,24 @@ cudaError_t launch_grade_cfg(const double *Bsum, const double *Ainv, int nb, dou
   cudaError_t e = launch_zero(gamma_cfg, 1, st);
   if (e != cudaSuccess) return e;
   k_grade_cfg<<<(nb + 127) / 128, 128, 0, st>>>(Bsum, Ainv, nb, gamma_cfg);
+  count_launch();
+  return cudaGetLastError();
+}
+
+// maximum of n non-negative doubles (the neighbourhood grades of a configuration): integer atomicMax on the bit
+// pattern, order independent -> deterministic
+__global__ void k_max_nonneg(const double *__restrict__ x, long long n, double *__restrict__ out) {
+  double m = 0.0;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) m = fmax(m, x[i]);
+#pragma unroll
+  for (int o = 16; o >= 1; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0 && m > 0.0) atomicMax(reinterpret_cast<unsigned long long *>(out), (unsigned long long)__double_as_longlong(m));
+}
+cudaError_t launch_max_nonneg(const double *x, long long n, double *out, cudaStream_t st) {
+  cudaError_t e = launch_zero(out, 1, st);
+  if (e != cudaSuccess || n <= 0) return e;
+  const int blocks = (int)std::min<long long>((n + 255) / 256, 148 * 8);
+  k_max_nonneg<<<blocks, 256, 0, st>>>(x, n, out);
   count_launch();
   return cudaGetLastError();
 }

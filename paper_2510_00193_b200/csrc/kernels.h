@@ -132,6 +132,7 @@ cudaError_t launch_ke(int n, const double *vel, const int *type, const double *m
 // gamma[i] = max_k | sum_a B[i][a] Ainv[a][k] |, B given as the tiled Bt [tiles][nb][128]
 cudaError_t launch_grade(const double *Bt, const double *Ainv, long long n, int nb, double *gamma, cudaStream_t st);
 // gamma_cfg = max_k | sum_a Bsum[a] Ainv[a][k] |
+cudaError_t launch_max_nonneg(const double *x, long long n, double *out, cudaStream_t st);
 cudaError_t launch_grade_cfg(const double *Bsum, const double *Ainv, int nb, double *scratch, double *gamma_cfg,
                              cudaStream_t st);
 // fp64 FMA throughput microbenchmark

@@ -183,3 +183,53 @@ def test_velocity_verlet_loop(lib, torch):
     dx -= np.round(dx / L) * L
     assert np.abs(dx).max() < 1e-9 and abs(res[1][0].sum() - res[10][0].sum()) < 1e-9 * abs(e0)
     pot.close()
+
+
+def test_md_loop_with_grade_policy(lib, torch):
+    """mtp_md_run_al: grades on the initial configuration and after every 5th step.
+    Expected values come from the pieces already tested: the trajectory of mtp_md_run stopped at the same steps, the
+    grades of mtp_grade on it.  Checked: the per-evaluation maximum (device reduction) bit for bit, which steps are
+    kept and their positions, the break."""
+    w = make_workload(0, n_basis_of(10), with_ainv=True)
+    pot = gpu_pot(lib, w)
+    d = to_dev(w, torch)
+    Ainv = torch.as_tensor(w.Ainv).cuda()
+    rng = np.random.default_rng(5)
+    mass = np.array([55.845])
+    vel0 = rng.normal(0.0, 2.0, (w.n_atoms, 3))
+    cap, dt, every, skin, X, steps = int(w.nnz * 2.2), 1e-6, 10, 1.0, 5, 20
+    # reference: run to step s with the plain loop, then grade that configuration on that list
+    want = {}
+    for s in range(0, steps + 1, X):
+        pos, vel = d["pos"].clone(), torch.as_tensor(vel0).cuda()
+        pot.md_run(pos, vel, d["types"], w.box, mass, dt, s, every, skin, cap)
+        # the list the loop holds at step s: built at the last multiple of `every` (positions wrapped there)
+        p2, v2 = d["pos"].clone(), torch.as_tensor(vel0).cuda()
+        pot.md_run(p2, v2, d["types"], w.box, mass, dt, (s // every) * every, every, skin, cap)
+        nb = lib.neighbors_build(p2, w.box, 5.0 + skin)
+        n = nb["nnz"]
+        g = pot.grade(pos, d["types"], w.box, nb["off"], nb["idx"][:n], Ainv, nb["shift"][:n], mode=2)
+        torch.cuda.synchronize()
+        want[s] = (pos.cpu().numpy(), float(g["gamma_atom"].max()), float(g["gamma_cfg"][0]), g["gamma_atom"].cpu().numpy())
+    for mode in (0, 1):
+        grades = [want[s][1 + mode] for s in sorted(want)]
+        thr = 0.5 * (min(grades) + max(grades))
+        assert min(grades) < thr < max(grades)
+        pos, vel = d["pos"].clone(), torch.as_tensor(vel0).cuda()
+        o = pot.md_run_al(pos, vel, d["types"], w.box, mass, dt, steps, every, skin, cap, Ainv, X, mode, thr, 1e300, 16)
+        torch.cuda.synchronize()
+        keep = [s for s in sorted(want) if want[s][1 + mode] > thr]
+        assert o["steps_done"] == steps and not o["stopped"] and o["n_evaluations"] == steps // X + 1
+        assert o["sel_step"] == keep and o["sel_grade"] == [want[s][1 + mode] for s in keep]
+        assert o["max_grade"] == max(grades)
+        for k, s in enumerate(keep):
+            assert np.array_equal(o["selected"][k].cpu().numpy(), want[s][0])
+        if mode == 0:
+            assert np.array_equal(o["gamma_atom"].cpu().numpy(), want[steps][3])
+        assert np.array_equal(pos.cpu().numpy(), want[steps][0])
+        # at most two kept; break at the first evaluation above the threshold
+        pos, vel = d["pos"].clone(), torch.as_tensor(vel0).cuda()
+        o = pot.md_run_al(pos, vel, d["types"], w.box, mass, dt, steps, every, skin, cap, Ainv, X, mode, -1.0, thr, 2)
+        assert o["stopped"] and o["steps_done"] == keep[0] and o["sel_step"] == [0, X][:o["n_evaluations"]][:2]
+        assert np.array_equal(pos.cpu().numpy(), want[keep[0]][0])
+    pot.close()
