@@ -216,29 +216,18 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
-def graph_replay(torch, lib, pot, step, out, calls=100):
-    """small configurations additionally as a CUDA-graph replay of `calls` whole calls, which takes
-    the per-launch host overhead out of the number.  The call is captured once (the library only enqueues on the
-    given stream: no allocation, no synchronisation) and the graph replayed back to back; ms per call."""
-    pot.set_option(lib.OPT_PROFILE, 0)            # timing events of the profile cannot be read back from a graph
-    side = torch.cuda.Stream()
-    side.wait_stream(torch.cuda.current_stream())
-    with torch.cuda.stream(side):
-        step(out)
-    torch.cuda.current_stream().wait_stream(side)
-    g = torch.cuda.CUDAGraph()
-    with torch.cuda.graph(g, stream=side):
-        step(out)
+def graph_replay(torch, pot, graph, calls=100):
+    """small configurations additionally through the library's own CUDA graph of the call
+    (mtp_graph_capture / mtp_graph_launch: one launch per evaluation, the per-kernel launch overhead gone); ms per call."""
     for _ in range(3):
-        g.replay()
+        graph.launch()
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for _ in range(calls):
-        g.replay()
+        graph.launch()
     e1.record()
     torch.cuda.synchronize()
-    pot.set_option(lib.OPT_PROFILE, 1)
     return e0.elapsed_time(e1) / calls
 
 
@@ -344,8 +333,12 @@ def run_ours(args):
     # ---- small systems: the same call replayed from a CUDA graph (launch overhead removed)
     graph = None
     if w.n_atoms <= 16384 and Ainv is None and world == 1 and not args.sharded:
-        gms = graph_replay(torch, lib, pot, step, out)
-        graph = {"calls": 100, "ms_per_call": gms, "value": w.n_atoms / (gms * 1e-3), "unit": UNIT}
+        cg, gout = pot.graph(pos, types, w.box, off, idx, shift, rev)
+        gms = graph_replay(torch, pot, cg)
+        assert torch.equal(gout["F"], out["F"]), "graph launch differs from mtp_compute"
+        cg.close()
+        graph = {"calls": 100, "ms_per_call": gms, "value": w.n_atoms / (gms * 1e-3), "unit": UNIT,
+                 "entry": "mtp_graph_capture / mtp_graph_launch"}
 
     # ---- end to end through the host-buffer entry points (pinned inputs, results read back).  `e2e`: what an MD host
     # code sends every step -- positions and types -- with the list built on the device (mtp_compute_host_pos);

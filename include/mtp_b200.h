@@ -166,6 +166,21 @@ int mtp_compute_host(mtp_handle *h, int64_t n_atoms, const double *pos, const in
                      const int8_t *shift, const int32_t *rev, int64_t nnz, double *E,
                      double *Ei, double *F, double *virial);
 
+/* Small systems (the "small" GPU variant): one mtp_compute call captured as a CUDA graph and
+ * replayed with one launch, which takes the per-kernel launch overhead (a dozen launches of a few microseconds) out of
+ * a call that computes for tens of microseconds.  mtp_graph_capture records the call with exactly these buffers --
+ * nothing runs yet; mtp_graph_launch enqueues the whole evaluation on the stream: it reads whatever the buffers hold
+ * at that time (new coordinates, a list rebuilt in place with the same nnz) and is bit-identical to mtp_compute on
+ * the same inputs.  The buffers, the workspace and the handle must outlive the graph; the options of the handle are
+ * those at capture time.  Graph launches that overlap on the GPU share the workspace and race. */
+typedef struct mtp_graph mtp_graph;
+int mtp_graph_capture(mtp_handle *h, int64_t n_atoms, const double *d_pos, const int32_t *d_type, const double *box,
+                      const int64_t *d_off, const int32_t *d_idx, const int8_t *d_shift, const int32_t *d_rev,
+                      int64_t nnz, double *d_E, double *d_Ei, double *d_F, double *d_virial, void *d_ws, size_t ws_bytes,
+                      mtp_graph **out);
+int mtp_graph_launch(mtp_graph *g, void *cuda_stream);
+int mtp_graph_destroy(mtp_graph *g);
+
 /* One rank's share of a sharded evaluation ("full node" runs): the atoms are
  * cut into contiguous ranges, positions and types are replicated, and every rank holds the CSR rows of its own range
  * only.  mtp_compute_rows evaluates the rows [row_lo, row_hi) of an n_atoms system:

@@ -45,7 +45,7 @@ EXPORTS = ["mtp_enumerate", "mtp_table_free", "mtp_create", "mtp_destroy", "mtp_
            "mtp_compute_host", "mtp_debug_moments", "mtp_launch_count", "mtp_peak_dfma",
            "mtp_cost_model", "mtp_profile_read", "mtp_table_plan", "mtp_k2_program",
            "mtp_neighbors_workspace_bytes", "mtp_neighbors_build", "mtp_neighbors_build_static",
-           "mtp_md_al_workspace_bytes", "mtp_md_run_al", "mtp_rows_workspace_bytes", "mtp_compute_rows", "mtp_grade_rows", "mtp_grade_cfg_from_sum", "mtp_md_workspace_bytes", "mtp_md_run",
+           "mtp_md_al_workspace_bytes", "mtp_md_run_al", "mtp_graph_capture", "mtp_graph_launch", "mtp_graph_destroy", "mtp_rows_workspace_bytes", "mtp_compute_rows", "mtp_grade_rows", "mtp_grade_cfg_from_sum", "mtp_md_workspace_bytes", "mtp_md_run",
            "mtp_compute_host_pos"]
 
 
@@ -91,6 +91,9 @@ def _load():
     lib.mtp_table_plan.argtypes = [C.POINTER(MtpParams), C.POINTER(i64)]
     lib.mtp_neighbors_workspace_bytes.argtypes = [i64, C.POINTER(C.c_size_t)]
     lib.mtp_neighbors_build.argtypes = [i64, vp, C.POINTER(dbl), dbl, i64, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
+    lib.mtp_graph_capture.argtypes = [vp, i64, vp, vp, C.POINTER(dbl), vp, vp, vp, vp, i64, vp, vp, vp, vp, vp, C.c_size_t, C.POINTER(vp)]
+    lib.mtp_graph_launch.argtypes = [vp, vp]
+    lib.mtp_graph_destroy.argtypes = [vp]
     lib.mtp_md_al_workspace_bytes.argtypes = [vp, i64, i64, C.POINTER(C.c_size_t)]
     lib.mtp_md_run_al.argtypes = [vp, i64, vp, vp, vp, C.POINTER(dbl), C.POINTER(dbl), dbl, i64, C.c_int32, dbl, i64, vp,
                                   C.POINTER(AlPolicy), vp, vp, vp, vp, vp, vp, vp, C.POINTER(i64), C.POINTER(dbl), C.POINTER(i64),
@@ -299,6 +302,21 @@ class Potential:
                                      _ptr(out["virial"]), _ptr(ws), ws.numel(), self._stream(stream)))
         return out
 
+    def graph(self, pos, types, box, off, idx, shift=None, rev=None):
+        """mtp_graph_capture of one compute call on these tensors.  Returns (ComputeGraph, out dict); graph.launch()
+        re-evaluates from whatever the tensors hold.  The graph keeps its own workspace and references to the tensors."""
+        import torch
+        n, nnz, dev = int(pos.shape[0]), int(idx.shape[0]), pos.device
+        out = dict(E=torch.empty(1, dtype=torch.float64, device=dev), Ei=torch.empty(n, dtype=torch.float64, device=dev),
+                   F=torch.empty((n, 3), dtype=torch.float64, device=dev), virial=torch.empty(6, dtype=torch.float64, device=dev))
+        ws = torch.empty(self.workspace_bytes(n, nnz), dtype=torch.uint8, device=dev)
+        boxh = (C.c_double * 9)(*[float(x) for x in np.asarray(box, dtype=np.float64).reshape(9)])
+        g = C.c_void_p()
+        self._check(_lib.mtp_graph_capture(self._h, n, _ptr(pos), _ptr(types), boxh, _ptr(off), _ptr(idx), _ptr(shift), _ptr(rev),
+                                           nnz, _ptr(out["E"]), _ptr(out["Ei"]), _ptr(out["F"]), _ptr(out["virial"]), _ptr(ws),
+                                           ws.numel(), C.byref(g)))
+        return ComputeGraph(self, g, (pos, types, off, idx, shift, rev, ws, out)), out
+
     def grade(self, pos, types, box, off, idx, Ainv, shift=None, mode=2, want_B=False, stream=None):
         import torch
         n, nnz, dev = int(pos.shape[0]), int(idx.shape[0]), pos.device
@@ -438,6 +456,29 @@ class Potential:
                                           _np_ptr(shift), _np_ptr(rev), nnz, _np_ptr(out["E"]), _np_ptr(out["Ei"]),
                                           _np_ptr(out["F"]), _np_ptr(out["virial"])))
         return out
+
+
+class ComputeGraph:
+    """An mtp_graph: one captured mtp_compute call."""
+
+    def __init__(self, pot, g, keep):
+        self._pot, self._g, self._keep = pot, g, keep
+
+    def launch(self, stream=None):
+        rc = _lib.mtp_graph_launch(self._g, Potential._stream(stream))
+        if rc != OK:
+            raise MtpError(rc, "mtp_graph_launch")
+
+    def close(self):
+        if self._g:
+            _lib.mtp_graph_destroy(self._g)
+            self._g = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 def neighbors_build(pos, box, r_list, capacity=None, want_rev=True, stream=None):

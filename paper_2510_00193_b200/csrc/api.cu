@@ -3,6 +3,8 @@
 // mtp_compute / mtp_grade.  No CPU fallback: every numeric step runs in the CUDA kernels.
 #include <cuda_runtime.h>
 
+#include <new>
+
 #include <algorithm>
 #include <atomic>
 #include <cmath>
@@ -1015,6 +1017,60 @@ extern "C" int mtp_grade(mtp_handle *h, int64_t N, const double *d_pos, const in
                          double *d_B, void *d_ws, size_t ws_bytes, void *stream) {
   return grade_impl(h, N, d_pos, d_type, box, d_off, d_idx, d_shift, nnz, d_Ainv, mode, d_gamma_atom, d_gamma_cfg, d_Bsum, d_B,
                     d_ws, ws_bytes, stream);
+}
+
+// ---- small systems: the whole call as one CUDA graph (the small-system variant exists because a
+// handful of launches of a few microseconds each dominate below ~10^4 atoms) ---------------------------------------
+struct mtp_graph {
+  cudaGraph_t graph = nullptr;
+  cudaGraphExec_t exec = nullptr;
+  mtp_handle *h = nullptr;
+};
+
+extern "C" int mtp_graph_capture(mtp_handle *h, int64_t N, const double *d_pos, const int32_t *d_type, const double *box,
+                                 const int64_t *d_off, const int32_t *d_idx, const int8_t *d_shift, const int32_t *d_rev,
+                                 int64_t nnz, double *d_E, double *d_Ei, double *d_F, double *d_virial, void *d_ws,
+                                 size_t ws_bytes, mtp_graph **out) {
+  if (!h) return MTP_EINVAL;
+  if (!out) return fail(h, MTP_EINVAL, "mtp_graph_capture: null argument");
+  *out = nullptr;
+  cudaStream_t st = nullptr;
+  CU(h, cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+  const int saved_profile = h->profile;
+  h->profile = 0;                              // timing events cannot be read back from a graph
+  cudaError_t e = cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal);
+  int rc = MTP_OK;
+  cudaGraph_t graph = nullptr;
+  if (e == cudaSuccess) {
+    rc = compute_impl(h, N, d_pos, d_type, box, d_off, d_idx, d_shift, d_rev, nnz, d_E, d_Ei, d_F, d_virial, d_ws, ws_bytes, st, nullptr);
+    e = cudaStreamEndCapture(st, &graph);      // also ends a capture the call invalidated
+  }
+  h->profile = saved_profile;
+  cudaStreamDestroy(st);
+  if (rc != MTP_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+  if (e != cudaSuccess || !graph) { cudaGetLastError(); return cuda_fail(h, e, "mtp_graph_capture"); }
+  mtp_graph *g = new (std::nothrow) mtp_graph;
+  if (!g) { cudaGraphDestroy(graph); return fail(h, MTP_ENOMEM, "out of host memory"); }
+  g->graph = graph; g->h = h;
+  e = cudaGraphInstantiate(&g->exec, graph, 0);
+  if (e != cudaSuccess) { cudaGraphDestroy(graph); delete g; return cuda_fail(h, e, "cudaGraphInstantiate"); }
+  *out = g;
+  return MTP_OK;
+}
+
+extern "C" int mtp_graph_launch(mtp_graph *g, void *stream) {
+  if (!g || !g->exec) return MTP_EINVAL;
+  cudaError_t e = cudaGraphLaunch(g->exec, (cudaStream_t)stream);
+  if (e != cudaSuccess) return cuda_fail(g->h, e, "cudaGraphLaunch");
+  return MTP_OK;
+}
+
+extern "C" int mtp_graph_destroy(mtp_graph *g) {
+  if (!g) return MTP_OK;
+  if (g->exec) cudaGraphExecDestroy(g->exec);
+  if (g->graph) cudaGraphDestroy(g->graph);
+  delete g;
+  return MTP_OK;
 }
 
 // ---- one rank's share of a sharded evaluation ----------------------------------------

@@ -321,6 +321,38 @@ def test_cuda_graph_replay_of_a_call_is_bit_identical(lib, torch):
     pot.close()
 
 
+def test_graph_behind_the_abi_is_bit_identical_and_follows_the_data(lib, torch):
+    """mtp_graph_capture / mtp_graph_launch: the small-system path (one launch per evaluation).  Capture runs nothing;
+    a launch equals mtp_compute bit for bit, also after the coordinates changed in place, on any stream."""
+    for ci, cells in ((0, None), (1, 4)):
+        w = make_workload(ci, n_basis_of([10, 16][ci]), cells=cells)
+        a, pot, d = run_gpu(lib, torch, w, opts={lib.OPT_FORCE_MODE: lib.FORCE_GATHER})
+        pot.set_option(lib.OPT_PROFILE, 1)                             # capture has to switch the timing events off itself
+        n0 = lib.launch_count()
+        g, out = pot.graph(d["pos"], d["types"], w.box, d["off"], d["idx"], d["shift"], d["rev"])
+        assert pot.get_option(lib.OPT_PROFILE) == 1
+        for v in out.values():
+            v.fill_(float("nan"))
+        torch.cuda.synchronize()
+        assert np.isnan(out["F"].cpu().numpy()).all()                  # nothing ran at capture
+        g.launch()
+        torch.cuda.synchronize()
+        for k in ("E", "Ei", "F", "virial"):
+            assert np.array_equal(out[k].cpu().numpy(), a[k]), k
+        d["pos"].add_(0.01 * torch.randn_like(d["pos"]))
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        g.launch(stream=side)
+        g.launch(stream=side)
+        side.synchronize()
+        ref = pot.compute(d["pos"], d["types"], w.box, d["off"], d["idx"], d["shift"], d["rev"])
+        torch.cuda.synchronize()
+        for k in ("E", "Ei", "F", "virial"):
+            assert np.array_equal(ref[k].cpu().numpy(), out[k].cpu().numpy()), k
+        g.close()
+        pot.close()
+
+
 def test_specialised_and_interpreted_tree_kernels_agree(lib, torch):
     """MTP_OPT_TREE_CODEGEN: the two forms of K2 sum in different orders, so they agree to rounding (relative to the
     magnitude of the summed terms), not bit for bit; each is compared with the oracle elsewhere."""
