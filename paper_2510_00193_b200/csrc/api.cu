@@ -761,7 +761,7 @@ void fill_pair_args(const mtp_handle *h, PairArgs &pa, const double *pos4, const
                     const int8_t *shift) {
   pa.pos4 = pos4; pa.off = (const long long *)off; pa.idx = idx;
   pa.coef = h->d_coef; pa.n_species = h->S; pa.nb = h->nb; pa.crow = h->crow;
-  pa.minimg = shift ? 0 : 1; pa.r_min = h->r_min; pa.r_cut = h->r_cut;
+  pa.minimg = shift ? 0 : 1; pa.r_min = h->r_min; pa.r_cut = h->r_cut; pa.inv_width = 1.0 / (h->r_cut - h->r_min);
   pa.M = nullptr; pa.G = nullptr; pa.d4 = nullptr; pa.F = nullptr; pa.wpart = nullptr; pa.kmap = nullptr;
   pa.d4_cap = 0; pa.flag = h->d_flag; pa.idx_rel = 0; pa.idx_cap = 1LL << 62;
 }

@@ -28,11 +28,11 @@ __device__ __forceinline__ void pow_fixed(double y, double &p, double &dp) {
 // size (8 in every BASELINE config), NB = 0: run-time nb.
 template <int NMU, bool DERIV, int NB>
 __device__ __forceinline__ void radial(const double *__restrict__ crow, int nb_rt, double r, double r_min,
-                                       double r_cut, double *f, double *df) {
+                                       double r_cut, double inv_width, double *f, double *df) {
   constexpr int NMUP = (NMU + 1) & ~1;
   const int nb = NB > 0 ? NB : nb_rt;
-  const double sx = 2.0 / (r_cut - r_min);
-  const double xi = (2.0 * r - r_min - r_cut) / (r_cut - r_min);
+  const double sx = 2.0 * inv_width;                     // inv_width = 1 / (R_cut - R_min), from the host
+  const double xi = (2.0 * r - r_min - r_cut) * inv_width;
   double s[NMUP], ds[NMUP];
 #pragma unroll
   for (int m = 0; m < NMUP; ++m) { s[m] = 0.0; ds[m] = 0.0; }

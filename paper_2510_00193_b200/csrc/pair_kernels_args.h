@@ -37,6 +37,7 @@ struct PairArgs {
   int minimg;
   double H[9], Hi[9];        // box rows, inverse (columns of Hi map cartesian -> fractional)
   double r_min, r_cut;
+  double inv_width;            // 1 / (R_cut - R_min): the Chebyshev argument by a multiplication, not a division per pair
 };
 
 }  // namespace mtpb

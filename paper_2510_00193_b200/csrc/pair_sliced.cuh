@@ -23,6 +23,13 @@
 #include "pair_kernels.cuh"
 #include "pair_tiled.cuh"
 
+#ifndef K3_UNROLL_WIDE
+#define K3_UNROLL_WIDE 1
+#endif
+#ifndef K3_UNROLL_NARROW
+#define K3_UNROLL_NARROW 4
+#endif
+
 namespace mtpb {
 
 // ---- columns (mu, a) of a level's staircase, in (mu asc, a asc) order
@@ -106,6 +113,11 @@ struct STile {
   // CTAs per SM the register allocation aims at while a slice has <= 40 components: K1 128 registers per thread
   // (16 warps per SM); K3 168 (12 warps): with 128 its force / virial accumulators spill (measured at config 4:
   // K1 1.53 / 1.70 ms and K3 2.97 / 2.71 ms per step with 16 / 12 warps)
+  // K3's neighbour loop unrolled over a whole tile interleaves independent neighbours (what hides the DFMA latency
+  // with 3 warps per scheduler), but the code of all slices has to stay in the instruction cache: level 20 / 24 with
+  // 8 neighbours unrolled is 137 / 225 KB of code (no_instruction 8.5 stall cycles per issue at config 3), with
+  // UNR3 neighbours per trip it fits
+  static constexpr int UNR3 = TN <= 4 ? K3_UNROLL_NARROW : K3_UNROLL_WIDE;
   static constexpr int MINB1 = Slicing<LEV, NSL>::NSLOT <= 40 ? (512 / NT > 0 ? 512 / NT : 1) : 1;
   static constexpr int MINB3 = Slicing<LEV, NSL>::NSLOT <= 40 ? (384 / NT > 0 ? 384 / NT : 1) : 1;
 };
@@ -140,8 +152,12 @@ __device__ __forceinline__ void stage_pair_fields(const PairArgs &a, const doubl
     const double r2 = gx * gx + gy * gy + gz * gz;
     if (r2 < rc2) {
       x = gx; y = gy; z = gz;
-      const double r = r2 * rsqrt(r2);
-      radial<NMU, DERIV, NB>(csm + (zi_s * a.n_species + (int)p1.y) * a.crow, a.nb, r, a.r_min, a.r_cut, f, df);
+      const double rinv = r2 > 0.0 ? rsqrt(r2) : 0.0;
+      radial<NMU, DERIV, NB>(csm + (zi_s * a.n_species + (int)p1.y) * a.crow, a.nb, r2 * rinv, a.r_min, a.r_cut, a.inv_width, f, df);
+      if (DERIV) {                        // K3 needs f'_mu / r (d_ij = sum f_mu grad P_mu + (sum f'_mu P_mu) r_ij / r): folded in here
+#pragma unroll
+        for (int m = 0; m < NMU; ++m) df[m] *= rinv;
+      }
     }
   }
   out[0] = x; out[32] = y; out[64] = z;
@@ -445,6 +461,7 @@ __global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB3) k_pairgrad_s
     const double *cur = tile + buf * Tl::TILE3;
     // ---- phase B (lane = atom, warp = slice)
     const int kend = min(TN, n_max - t0);
+#pragma unroll(Tl::UNR3)
     for (int k = 0; k < kend; ++k) {
       double rs = 0.0, dx = 0.0, dy = 0.0, dz = 0.0;
       k3_dispatch<LEV, NSL>(slice, g, cur + k * KS + lane, rs, dx, dy, dz);
@@ -464,9 +481,7 @@ __global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB3) k_pairgrad_s
         }
         const double *r = cur + pk * KS + pa;
         const double x = r[0], y = r[32], z = r[64];
-        const double r2 = x * x + y * y + z * z;
-        const double q = r2 > 0.0 ? rs * rsqrt(r2) : 0.0;
-        dx = fma(q, x, dx); dy = fma(q, y, dy); dz = fma(q, z, dz);
+        dx = fma(rs, x, dx); dy = fma(rs, y, dy); dz = fma(rs, z, dz);      // rs = sum_mu (f'_mu / r) P_mu: phase A stored f' / r
         if (ATOMIC) {
           if (dx != 0.0 || dy != 0.0 || dz != 0.0) {
             const int j = w_cur & kIdxMask;

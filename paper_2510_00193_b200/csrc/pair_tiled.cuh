@@ -89,7 +89,7 @@ __device__ __forceinline__ void stage_pair(const PairArgs &a, const double *__re
   if (g.zj >= 0 && r2 < rc2) {
     x = g.x; y = g.y; z = g.z;
     const double r = r2 * rsqrt(r2);
-    radial<NMU, DERIV, NB>(csm + (zi_s * a.n_species + g.zj) * a.crow, a.nb, r, a.r_min, a.r_cut, f, df);
+    radial<NMU, DERIV, NB>(csm + (zi_s * a.n_species + g.zj) * a.crow, a.nb, r, a.r_min, a.r_cut, a.inv_width, f, df);
   }
   double2 *o = reinterpret_cast<double2 *>(out);
   double buf[PD];
