@@ -2,6 +2,8 @@
 // gather over the reverse-neighbour index (a8), fixed-order reductions of E, virial and B.
 #include <cuda_runtime.h>
 
+#include <cstdint>
+
 #include <algorithm>
 #include <atomic>
 
@@ -35,40 +37,66 @@ __global__ void k_pack(const double *__restrict__ pos, const int *__restrict__ t
 __global__ void __launch_bounds__(256) k_pack_pairs_chunk(const long long *__restrict__ off, int c0, int c1, const int *__restrict__ idx,
                                                           const signed char *__restrict__ shift, long long n_atoms, long long cap,
                                                           int *__restrict__ out, int *__restrict__ flag, unsigned *__restrict__ touch,
-                                                          int tshift) {
+                                                          int tshift, int vec) {
   __shared__ unsigned bits[kTouchWords];             // this block's share of the touch bitmap: merged into the global one at the end
   for (int i = threadIdx.x; i < kTouchWords; i += blockDim.x) bits[i] = 0u;
   __syncthreads();
   const long long p0 = off[c0], n = off[c1] - p0;
-  for (long long q0 = (long long)blockIdx.x * (4 * blockDim.x) + threadIdx.x; q0 < n; q0 += (long long)gridDim.x * (4 * blockDim.x)) {
-  // four pairs per thread, a block stride apart: the loads of all four are in flight together
-  int j[4], s0[4], s1[4], s2[4];
+  // four CONSECUTIVE pairs per thread, at absolute positions 4 g .. 4 g + 3: the indices come as one 16-byte load and
+  // the twelve shift bytes as three 4-byte loads (the arrays are 16-byte aligned: checked by the launcher, which
+  // otherwise asks for the scalar loads)
+  const long long g0 = p0 >> 2, g1 = (p0 + n + 3) >> 2;
+  for (long long g = g0 + (long long)blockIdx.x * blockDim.x + threadIdx.x; g < g1; g += (long long)gridDim.x * blockDim.x) {
+    int j[4];
+    unsigned sw[3] = {0u, 0u, 0u};
+    const long long a = 4 * g;
+    if (vec && a >= p0 && a + 4 <= p0 + n) {
+      const int4 v = *reinterpret_cast<const int4 *>(idx + a);
+      j[0] = v.x; j[1] = v.y; j[2] = v.z; j[3] = v.w;
+      if (shift) {
+        const unsigned *sp = reinterpret_cast<const unsigned *>(shift + 3 * a);
+        sw[0] = sp[0]; sw[1] = sp[1]; sw[2] = sp[2];
+      }
+    } else {
 #pragma unroll
-  for (int u = 0; u < 4; ++u) {
-    const long long q = q0 + (long long)u * blockDim.x;
-    j[u] = -1; s0[u] = s1[u] = s2[u] = 0;
-    if (q < n) {
-      j[u] = idx[p0 + q];
-      if (shift) { s0[u] = shift[3 * (p0 + q)]; s1[u] = shift[3 * (p0 + q) + 1]; s2[u] = shift[3 * (p0 + q) + 2]; }
-    }
-  }
+      for (int u = 0; u < 4; ++u) {
+        const long long p = a + u;
+        j[u] = -1;
+        if (p >= p0 && p < p0 + n) {
+          j[u] = idx[p];
+          if (shift) {
 #pragma unroll
-  for (int u = 0; u < 4; ++u) {
-    const long long q = q0 + (long long)u * blockDim.x;
-    if (q >= n) continue;
-    const bool ok = j[u] >= 0 && j[u] < n_atoms && s0[u] >= -1 && s0[u] <= 1 && s1[u] >= -1 && s1[u] <= 1 && s2[u] >= -1 && s2[u] <= 1;
-    int word = -1;
-    if (!ok) atomicAdd(flag, 1);
-    else {
-      word = shift ? (int)((unsigned)j[u] | ((unsigned)shift_code(s0[u], s1[u], s2[u]) << kIdxBits)) : j[u];
-      const int b = j[u] >> tshift;
-      atomicOr(&bits[b >> 5], 1u << (b & 31));
+            for (int c = 0; c < 3; ++c) {
+              const int byte = 3 * u + c;
+              sw[byte >> 2] |= (unsigned)(unsigned char)shift[3 * p + c] << (8 * (byte & 3));
+            }
+          }
+        }
+      }
     }
-    if (out) {
-      if (q < cap) out[q] = word;
-      else atomicAdd(flag + 1, 1);
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const long long q = a + u - p0;
+      if (q < 0 || q >= n) continue;
+      int sv[3];
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        const int byte = 3 * u + c;
+        sv[c] = (int)(signed char)((sw[byte >> 2] >> (8 * (byte & 3))) & 0xffu);
+      }
+      const bool ok = j[u] >= 0 && j[u] < n_atoms && sv[0] >= -1 && sv[0] <= 1 && sv[1] >= -1 && sv[1] <= 1 && sv[2] >= -1 && sv[2] <= 1;
+      int word = -1;
+      if (!ok) atomicAdd(flag, 1);
+      else {
+        word = shift ? (int)((unsigned)j[u] | ((unsigned)shift_code(sv[0], sv[1], sv[2]) << kIdxBits)) : j[u];
+        const int b = j[u] >> tshift;
+        atomicOr(&bits[b >> 5], 1u << (b & 31));
+      }
+      if (out) {
+        if (q < cap) out[q] = word;
+        else atomicAdd(flag + 1, 1);
+      }
     }
-  }
   }
   __syncthreads();
   for (int i = threadIdx.x; i < kTouchWords; i += blockDim.x) if (bits[i]) atomicOr(touch + i, bits[i]);
@@ -119,8 +147,8 @@ __global__ void __launch_bounds__(256) k_gather_chunk(const long long *__restric
                                                       int c0, int c1, int n_atoms, const unsigned *__restrict__ touch, int tshift,
                                                       double *__restrict__ F) {
   const int lane = threadIdx.x & 31;
-  const bool all = c0 == 0 && c1 == n_atoms;       // a single chunk: every neighbour is in it, the index test is not needed
-  const long long p0 = off[c0];
+  // the mirror pair of p lies in this chunk exactly when rev[p] falls into the chunk's pair range: idx is not read
+  const long long p0 = off[c0], np = off[c1] - p0;
   const double2 *d = reinterpret_cast<const double2 *>(d4);
   for (int k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; k < n_atoms; k += (gridDim.x * blockDim.x) >> 5) {
     if (!((touch[(k >> tshift) >> 5] >> ((k >> tshift) & 31)) & 1u)) continue;
@@ -128,10 +156,9 @@ __global__ void __launch_bounds__(256) k_gather_chunk(const long long *__restric
     double fx = 0, fy = 0, fz = 0;
     bool any = false;
     for (long long p = beg + lane; p < end; p += 32) {
-      const int j = all ? c0 : idx[p];
-      if (j >= c0 && j < c1) {
-        const long long q = rev[p] - p0;
-        if (q >= 0 && q < d4_cap) {
+      const long long q = rev[p] - p0;
+      if (q >= 0 && q < np) {
+        if (q < d4_cap) {
           const double2 b0 = __ldg(d + 2 * q), b1 = __ldg(d + 2 * q + 1);
           fx -= b0.x; fy -= b0.y; fz -= b1.x;
         }
@@ -228,7 +255,8 @@ cudaError_t launch_pack_pairs_chunk(const long long *off, int c0, int c1, const 
   if (e != cudaSuccess) return e;
   // the pair count of the chunk lives on the device: a persistent grid strides over it
   const long long blocks = std::min<long long>(148 * 8, std::max<long long>(1, (cap + 1023) / 1024));
-  k_pack_pairs_chunk<<<(unsigned)blocks, 256, 0, st>>>(off, c0, c1, idx, shift, n_atoms, cap, out, flag, touch, touch_shift(n_atoms));
+  const int vec = (((uintptr_t)idx & 15) == 0 && ((uintptr_t)shift & 3) == 0) ? 1 : 0;
+  k_pack_pairs_chunk<<<(unsigned)blocks, 256, 0, st>>>(off, c0, c1, idx, shift, n_atoms, cap, out, flag, touch, touch_shift(n_atoms), vec);
   count_launch();
   return cudaGetLastError();
 }

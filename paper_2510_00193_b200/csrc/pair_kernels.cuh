@@ -43,9 +43,13 @@ __device__ __forceinline__ void radial(const double *__restrict__ crow, int nb_r
 #pragma unroll
     for (int m = 0; m < NMUP; m += 2) {
       const double2 c = c2[(b * NMUP + m) >> 1];
-      s[m] = fma(c.x, tm, s[m]);
-      s[m + 1] = fma(c.y, tm, s[m + 1]);
-      if (DERIV) { ds[m] = fma(c.x, dtm, ds[m]); ds[m + 1] = fma(c.y, dtm, ds[m + 1]); }
+      // T_0 = 1, T_0' = 0, T_1' = 1 written out (same values, no multiplications by 0 and 1 on the fp64 pipe)
+      if (b == 0) { s[m] = c.x; s[m + 1] = c.y; }
+      else { s[m] = fma(c.x, tm, s[m]); s[m + 1] = fma(c.y, tm, s[m + 1]); }
+      if (DERIV) {
+        if (b == 1) { ds[m] = c.x; ds[m + 1] = c.y; }
+        else if (b > 1) { ds[m] = fma(c.x, dtm, ds[m]); ds[m + 1] = fma(c.y, dtm, ds[m + 1]); }
+      }
     }
     const double tn = fma(2.0 * xi, t, -tm);
     if (DERIV) { const double dtn = fma(2.0 * xi, dt, fma(2.0, t, -dtm)); dtm = dt; dt = dtn; }

@@ -473,9 +473,10 @@ __global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB3) k_pairgrad_s
     {
       const int k = t0 + pk;
       if (k < n_nb && pk < kend) {
-        double rs = 0.0, dx = 0.0, dy = 0.0, dz = 0.0;
+        const double *o0 = dpart + pk * DKS + pa;
+        double rs = o0[0], dx = o0[32], dy = o0[64], dz = o0[96];
 #pragma unroll
-        for (int s = 0; s < NSL; ++s) {                            // fixed order over the slices: bit-reproducible
+        for (int s = 1; s < NSL; ++s) {                            // fixed order over the slices: bit-reproducible
           const double *o = dpart + (s * TN + pk) * DKS + pa;
           rs += o[0]; dx += o[32]; dy += o[64]; dz += o[96];
         }

@@ -353,6 +353,23 @@ def test_graph_behind_the_abi_is_bit_identical_and_follows_the_data(lib, torch):
         pot.close()
 
 
+def test_unaligned_list_arrays_take_the_scalar_loads(lib, torch):
+    """The pair packer reads indices 16 bytes and shifts 4 bytes at a time when the arrays are aligned; list arrays that
+    start at an odd element (a view into a larger buffer) go through the scalar loads: same result bit for bit."""
+    w = make_workload(1, n_basis_of(16), cells=4)
+    a, pot, d = run_gpu(lib, torch, w, opts={lib.OPT_FORCE_MODE: lib.FORCE_GATHER, lib.OPT_CHUNK_ATOMS: 40})
+    idx = torch.empty(w.nnz + 3, dtype=torch.int32, device="cuda")[3:]
+    shift = torch.empty((w.nnz * 3 + 1,), dtype=torch.int8, device="cuda")[1:].view(w.nnz, 3)
+    assert idx.data_ptr() % 16 != 0 and shift.data_ptr() % 4 != 0
+    idx.copy_(d["idx"]); shift.copy_(d["shift"])
+    b = pot.compute(d["pos"], d["types"], w.box, d["off"], idx, shift, d["rev"])
+    torch.cuda.synchronize()
+    for k in ("E", "Ei", "F", "virial"):
+        assert np.array_equal(b[k].cpu().numpy(), a[k]), k
+    assert pot.get_option(lib.INFO_INPUT_ERRORS) == 0
+    pot.close()
+
+
 def test_specialised_and_interpreted_tree_kernels_agree(lib, torch):
     """MTP_OPT_TREE_CODEGEN: the two forms of K2 sum in different orders, so they agree to rounding (relative to the
     magnitude of the summed terms), not bit for bit; each is compared with the oracle elsewhere."""
