@@ -94,6 +94,13 @@ const char *mtp_last_error(const mtp_handle *h); /* h may be NULL: last error of
 #define MTP_OPT_FORCE_MODE 2    /* MTP_FORCE_GATHER (needs d_rev) | MTP_FORCE_ATOMIC       */
 #define MTP_OPT_VARIANT 3       /* MTP_VARIANT_AUTO | _THREAD | _BLOCK                     */
 #define MTP_OPT_PROFILE 4       /* 1: record CUDA events around every kernel launch        */
+#define MTP_OPT_SKIN_LIST 7     /* 1: the list carries a skin (pairs beyond R_cut; reading G3: they contribute exactly
+                                   nothing).  The large-system kernels then first compact every row to its entries within
+                                   R_cut (one extra position gather per listed pair) and loop over those only: with a 1 A
+                                   skin at R_cut = 5 A that is 1 / 1.73 of the work.  E_i is bit-identical to the default
+                                   (0), which multiplies such pairs by zero; forces and virial agree to rounding (their
+                                   summation order follows the position in the row) and stay deterministic in gather
+                                   mode.  mtp_md_run sets it for skin > 0. */
 #define MTP_OPT_CHUNK_PAIRS 6    /* upper bound of the neighbour-list entries of any one chunk: what the per-pair scratch
                                    (packed neighbour words 4 B + d_ij records 32 B per pair) is sized for.  0 = automatic:
                                    1.25 x nnz x chunk_atoms / N + 4096, right for lattice-like inputs; a chunk with more

@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmtp_b200.so")
 
 OK, EINVAL, ESIZE, EBOX, ECUDA, EUNSUP, ENOMEM = 0, -1, -2, -3, -4, -5, -6
-OPT_CHUNK_ATOMS, OPT_FORCE_MODE, OPT_VARIANT, OPT_PROFILE, OPT_TREE_CODEGEN, OPT_CHUNK_PAIRS = 1, 2, 3, 4, 5, 6
+OPT_CHUNK_ATOMS, OPT_FORCE_MODE, OPT_VARIANT, OPT_PROFILE, OPT_TREE_CODEGEN, OPT_CHUNK_PAIRS, OPT_SKIN_LIST = 1, 2, 3, 4, 5, 6, 7
 INFO_TREE_KERNELS, INFO_TREE_PROGRAMS, INFO_INPUT_ERRORS, INFO_SCRATCH_OVERFLOW = 100, 101, 102, 103
 FORCE_GATHER, FORCE_ATOMIC, FORCE_AUTO = 0, 1, 2
 VARIANT_AUTO, VARIANT_THREAD, VARIANT_BLOCK = 0, 1, 2

@@ -107,6 +107,7 @@ struct mtp_handle {
   std::vector<void *> to_free;
   // per-kernel-class device timing (MTP_OPT_PROFILE): event pairs recorded around each launch
   int profile = 0;
+  int skin_list = 0;                            // MTP_OPT_SKIN_LIST: the caller's list carries pairs beyond R_cut
   struct Span { cudaEvent_t a, b; int cls; };
   std::vector<Span> spans;
   std::vector<cudaEvent_t> pool;
@@ -634,6 +635,7 @@ extern "C" int mtp_set_option(mtp_handle *h, int key, int64_t v) {
     case MTP_OPT_FORCE_MODE: if (v < 0 || v > 2) return fail(h, MTP_EINVAL, "bad force mode"); h->force_mode = (int)v; return MTP_OK;
     case MTP_OPT_VARIANT: if (v < 0 || v > 2) return fail(h, MTP_EINVAL, "bad variant"); h->variant = (int)v; return MTP_OK;
     case MTP_OPT_PROFILE: h->profile = v != 0; return MTP_OK;
+    case MTP_OPT_SKIN_LIST: h->skin_list = v != 0; return MTP_OK;
     case MTP_OPT_CHUNK_PAIRS: if (v < 0) return fail(h, MTP_EINVAL, "chunk_pairs < 0"); h->chunk_pairs = v; return MTP_OK;
     case MTP_OPT_TREE_CODEGEN:
       if (v != 0 && !h->jit_ready) return fail(h, MTP_EUNSUP, "specialised contraction kernels not available: " + h->jit_note);
@@ -649,6 +651,7 @@ extern "C" int mtp_get_option(const mtp_handle *h, int key, int64_t *v) {
     case MTP_OPT_FORCE_MODE: *v = h->force_mode; return MTP_OK;
     case MTP_OPT_VARIANT: *v = h->variant; return MTP_OK;
     case MTP_OPT_PROFILE: *v = h->profile; return MTP_OK;
+    case MTP_OPT_SKIN_LIST: *v = h->skin_list; return MTP_OK;
     case MTP_OPT_TREE_CODEGEN: *v = h->codegen && h->jit_ready; return MTP_OK;
     case MTP_INFO_TREE_KERNELS: *v = h->jit_ready ? h->n_jit_kernels : 0; return MTP_OK;      // specialised K2 kernels loaded
     case MTP_INFO_TREE_PROGRAMS: *v = h->jit_ready ? (int64_t)h->jprogs.size() : 0; return MTP_OK;
@@ -671,7 +674,7 @@ struct Plan {
   int64_t N = 0, nnz = 0, C = 0, cols = 0;      // cols: C rounded up to whole tiles of 128 atoms (kTile)
   int n_chunks = 0, P = 1, sliced = 0, atomic = 0, grid_chunk = 0, AL = 0, AR = 1, elide = 1;
   int64_t cap = 0;                              // pairs of one chunk the per-pair scratch (packed words, d4) holds
-  size_t o_pos4 = 0, o_Ei = 0, o_M = 0, o_G = 0, o_wpart = 0, o_d4 = 0, o_B = 0, o_red = 0, o_idxp = 0, o_S = 0, o_Sbar = 0, o_jr = 0, total = 0;
+  size_t o_pos4 = 0, o_Ei = 0, o_M = 0, o_G = 0, o_wpart = 0, o_d4 = 0, o_B = 0, o_red = 0, o_idxp = 0, o_S = 0, o_Sbar = 0, o_jr = 0, o_korig = 0, o_cnt = 0, total = 0;
 };
 size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
@@ -726,6 +729,8 @@ int make_plan(const mtp_handle *h, int64_t n_all, int64_t nnz, int want_grade, i
   else if (h->chunk_pairs > 0) pl.cap = std::min<int64_t>(nnz, h->chunk_pairs);
   else pl.cap = std::min<int64_t>(nnz, (int64_t)(1.25 * (double)nnz * (double)C / (double)std::max<int64_t>(N, 1)) + 4096);
   pl.o_idxp = o; o = align_up(o + (size_t)pl.cap * 4);        // packed neighbour words (used when shifts are given)
+  pl.o_korig = o; o = align_up(o + (pl.sliced ? (size_t)pl.cap * 2 : 0));      // live rows (MTP_OPT_SKIN_LIST): CSR position of
+  pl.o_cnt = o; o = align_up(o + (pl.sliced ? (size_t)pl.cols * 4 : 0));       // a compacted entry, live entries per atom
   pl.o_jr = o; o = align_up(o + kTouchWords * sizeof(unsigned));      // touch bitmap of the current chunk
   pl.o_wpart = o; o = align_up(o + (size_t)std::max(1, pl.n_chunks) * pl.grid_chunk * 64);
   pl.o_d4 = o; if (!want_grade && !pl.atomic) o = align_up(o + (size_t)pl.cap * 32);
@@ -763,7 +768,7 @@ void fill_pair_args(const mtp_handle *h, PairArgs &pa, const double *pos4, const
   pa.coef = h->d_coef; pa.n_species = h->S; pa.nb = h->nb; pa.crow = h->crow;
   pa.minimg = shift ? 0 : 1; pa.r_min = h->r_min; pa.r_cut = h->r_cut; pa.inv_width = 1.0 / (h->r_cut - h->r_min);
   pa.M = nullptr; pa.G = nullptr; pa.d4 = nullptr; pa.F = nullptr; pa.wpart = nullptr; pa.kmap = nullptr;
-  pa.d4_cap = 0; pa.flag = h->d_flag; pa.idx_rel = 0; pa.idx_cap = 1LL << 62;
+  pa.d4_cap = 0; pa.flag = h->d_flag; pa.idx_rel = 0; pa.idx_cap = 1LL << 62; pa.cnt = nullptr; pa.korig = nullptr;
 }
 
 // One chunk of K2 work: B_alpha / E_i (forward) and, when want_adj, G = dE_i/dM.  B != null: every basis value of
@@ -910,10 +915,14 @@ static int compute_impl(mtp_handle *h, int64_t N, const double *d_pos, const int
   CU(h, launch_zero(d_F, 3 * N, st));            // both force modes accumulate: atomics, or chunk by chunk in fixed order
   int *idxp = (int *)(ws + pl.o_idxp);
   unsigned *jrange = (unsigned *)(ws + pl.o_jr);
-  fill_pair_args(h, pa, pos4, d_off, d_shift ? idxp : d_idx, d_shift);
+  // MTP_OPT_SKIN_LIST (large-system kernels only): rows compacted to the entries within R_cut, chunk by chunk
+  const bool live = h->skin_list && pl.sliced && nnz > 0;
+  unsigned short *korig = (unsigned short *)(ws + pl.o_korig);
+  int *cnt = (int *)(ws + pl.o_cnt);
+  fill_pair_args(h, pa, pos4, d_off, (d_shift || live) ? idxp : d_idx, d_shift);
   pa.n_rows = h->n_basic;
-  pa.idx_rel = d_shift ? 1 : 0;                  // packed words exist for the current chunk only
-  pa.idx_cap = d_shift ? pl.cap : nnz;
+  pa.idx_rel = (d_shift || live) ? 1 : 0;        // packed words exist for the current chunk only
+  pa.idx_cap = (d_shift || live) ? pl.cap : nnz;
   pa.d4_cap = pl.cap;
   K2Io io{pos4, M, G, Ei, nullptr, 0, 0, 1, N, (double *)(ws + pl.o_S), (double *)(ws + pl.o_Sbar)};
   bool rev_waited = false;
@@ -921,9 +930,12 @@ static int compute_impl(mtp_handle *h, int64_t N, const double *d_pos, const int
     pa.c0 = (int)(row_lo + c * pl.C); pa.c1 = (int)std::min<int64_t>(row_hi, row_lo + (c + 1) * pl.C);
     if (pipe) CU(h, cudaStreamWaitEvent(st, (*pipe->chunk_ready)[c], 0));      // this chunk's pairs have arrived
     // the chunk's neighbour words (validated, index + image code in 4 bytes) and the range of atoms it touches
-    if (nnz > 0)
+    if (live)
+      CU(h, launch_pack_rows_live(pa, d_idx, (const signed char *)d_shift, N, pl.cap, idxp, korig, cnt, pl.atomic ? nullptr : d4, jrange, st));
+    else if (nnz > 0)
       CU(h, launch_pack_pairs_chunk((const long long *)d_off, pa.c0, pa.c1, d_idx, (const signed char *)d_shift, N, pl.cap,
                                     d_shift ? idxp : nullptr, h->d_flag, jrange, st));
+    pa.cnt = live ? cnt : nullptr; pa.korig = live ? korig : nullptr;
     pa.M = M; pa.G = G; pa.kmap = pl.sliced ? h->d_kmapS : h->d_kmapF;
     TIMED(h, CLS_MOMENTS, st, (pl.sliced ? h->pl->moments_s(pa, st) : h->pl->moments(pa, pl.P, st)));
     io.c0 = pa.c0; io.c1 = pa.c1;
@@ -1323,8 +1335,9 @@ int md_impl(mtp_handle *h, int64_t N, double *d_pos, double *d_vel, const int32_
     }
     return m > al->p->break_threshold ? 1 : 0;
   };
-  const int saved_mode = h->force_mode;
+  const int saved_mode = h->force_mode, saved_skin = h->skin_list;
   if (h->force_mode == MTP_FORCE_AUTO) h->force_mode = MTP_FORCE_GATHER;      // the list comes with its reverse index
+  if (skin > 0) h->skin_list = 1;                                             // pairs between R_cut and R_cut + skin are skipped, not multiplied by 0
   rc = build();
   if (rc == MTP_OK) rc = forces();
   int64_t done = 0;
@@ -1342,7 +1355,7 @@ int md_impl(mtp_handle *h, int64_t N, double *d_pos, double *d_vel, const int32_
     done = s;
     if (al && s % al->p->grade_every == 0) { stop = policy(s); if (stop < 0) rc = stop; }
   }
-  h->force_mode = saved_mode;
+  h->force_mode = saved_mode; h->skin_list = saved_skin;
   if (rc != MTP_OK) return rc;
   // kinetic energy sum m v^2 / 2 in eV
   CU(h, launch_ke((int)N, d_vel, d_type, dmass, 0.5 / kFtm2v, ke, st));

@@ -103,6 +103,9 @@ constexpr int kTouchWords = 512;
 inline int touch_shift(long long n_atoms) { int s = 6; while ((n_atoms >> s) >= kTouchWords * 32) ++s; return s; }
 cudaError_t launch_pack_pairs_chunk(const long long *off, int c0, int c1, const int *idx, const signed char *shift, long long n_atoms,
                                     long long cap, int *out, int *flag, unsigned *touch, cudaStream_t st);
+// the same for a list with a skin (MTP_OPT_SKIN_LIST): rows compacted to the entries within R_cut (misc_kernels.cu)
+cudaError_t launch_pack_rows_live(const PairArgs &a, const int *idx, const signed char *shift, long long n_atoms, long long cap, int *out,
+                                  unsigned short *korig, int *cnt, double *d4, unsigned *touch, cudaStream_t st);
 // F_k -= sum over the neighbours j in the chunk of d4[rev], for every atom k of a touched block
 cudaError_t launch_gather_chunk(const long long *off, const int *idx, const int *rev, const double *d4, long long d4_cap, int c0,
                                 int c1, int n_atoms, const unsigned *touch, double *F, cudaStream_t st);

@@ -102,6 +102,79 @@ __global__ void __launch_bounds__(256) k_pack_pairs_chunk(const long long *__res
   for (int i = threadIdx.x; i < kTouchWords; i += blockDim.x) if (bits[i]) atomicOr(touch + i, bits[i]);
 }
 
+// Live rows (MTP_OPT_SKIN_LIST; reading G3: listed pairs with r >= R_cut contribute exactly nothing): the packer of a
+// list that carries a skin.  One warp per atom of the chunk: the row's entries within R_cut are moved to the front of
+// the row's stretch of the word array (order kept), cnt[atom - c0] says how many, korig[] keeps each one's position
+// in the CSR row (K3 writes the d4 record there, so the reverse gather is unchanged), and the d4 records of the
+// dropped entries are zeroed here.  The distance is pair_vector's, the test K1 / K3 make themselves: an entry dropped
+// here is one they would have multiplied by zero.  K1 / K3 then loop over cnt instead of the CSR row length -- with a
+// 1 A skin at R_cut = 5 A that is 1 / 1.73 of the pairs.
+__global__ void __launch_bounds__(256) k_pack_rows_live(const PairArgs a, const int *__restrict__ idx, const signed char *__restrict__ shift,
+                                                        long long n_atoms, long long cap, int *__restrict__ out,
+                                                        unsigned short *__restrict__ korig, int *__restrict__ cnt, double *__restrict__ d4,
+                                                        unsigned *__restrict__ touch, int tshift) {
+  __shared__ unsigned bits[kTouchWords];
+  __shared__ __align__(16) double slut[kShiftLut];
+  for (int i = threadIdx.x; i < kTouchWords; i += blockDim.x) bits[i] = 0u;
+  if (threadIdx.x < 27) {
+    const int q = (threadIdx.x + 13) % 27;                  // code -> position in the {-1,0,1}^3 list (as stage_coef)
+    const double s0 = q / 9 - 1, s1 = (q / 3) % 3 - 1, s2 = q % 3 - 1;
+    slut[4 * threadIdx.x] = s0 * a.H[0] + s1 * a.H[3] + s2 * a.H[6];
+    slut[4 * threadIdx.x + 1] = s0 * a.H[1] + s1 * a.H[4] + s2 * a.H[7];
+    slut[4 * threadIdx.x + 2] = s0 * a.H[2] + s1 * a.H[5] + s2 * a.H[8];
+    slut[4 * threadIdx.x + 3] = 0.0;
+  }
+  __syncthreads();
+  const int lane = threadIdx.x & 31;
+  const long long p0 = a.off[a.c0];
+  const double rc2 = a.r_cut * a.r_cut;
+  for (int i = a.c0 + ((blockIdx.x * blockDim.x + threadIdx.x) >> 5); i < a.c1; i += (gridDim.x * blockDim.x) >> 5) {
+    const long long beg = a.off[i], rb = beg - p0;
+    const int n = (int)min(a.off[i + 1] - beg, 65535LL);     // korig is 16 bits wide; longer rows are counted as errors below
+    if (lane == 0 && a.off[i + 1] - beg > 65535LL) atomicAdd(a.flag, 1);
+    double xi, yi, zi, ti;
+    load_pos4(a.pos4, i, xi, yi, zi, ti);
+    int live = 0;
+    for (int base = 0; base < n; base += 32) {
+      const int k = base + lane;
+      bool keep = false;
+      int word = -1, j = 0;
+      const bool here = k < n && rb + k < cap;
+      if (k < n && rb + k >= cap) atomicAdd(a.flag + 1, 1);
+      if (here) {
+        j = idx[beg + k];
+        int s0 = 0, s1 = 0, s2 = 0;
+        if (shift) { s0 = shift[3 * (beg + k)]; s1 = shift[3 * (beg + k) + 1]; s2 = shift[3 * (beg + k) + 2]; }
+        const bool ok = j >= 0 && j < n_atoms && s0 >= -1 && s0 <= 1 && s1 >= -1 && s1 <= 1 && s2 >= -1 && s2 <= 1;
+        if (!ok) atomicAdd(a.flag, 1);
+        else {
+          const int code = shift ? shift_code(s0, s1, s2) : 0;
+          double xj, yj, zj, tj, x, y, z;
+          load_pos4(a.pos4, j, xj, yj, zj, tj);
+          pair_vector(a, slut, code, xi, yi, zi, xj, yj, zj, x, y, z);
+          keep = x * x + y * y + z * z < rc2;
+          word = (int)((unsigned)j | ((unsigned)code << kIdxBits));
+        }
+      }
+      const unsigned m = __ballot_sync(0xffffffffu, keep);
+      if (keep) {
+        const int pos = live + __popc(m & ((1u << lane) - 1u));
+        out[rb + pos] = word;
+        korig[rb + pos] = (unsigned short)k;
+        const int b = j >> tshift;
+        atomicOr(&bits[b >> 5], 1u << (b & 31));
+      } else if (here && d4) {
+        double2 *o = reinterpret_cast<double2 *>(d4) + 2 * (size_t)(rb + k);
+        o[0] = make_double2(0.0, 0.0); o[1] = make_double2(0.0, 0.0);
+      }
+      live += __popc(m);
+    }
+    if (lane == 0) cnt[i - a.c0] = live;
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < kTouchWords; i += blockDim.x) if (bits[i]) atomicOr(touch + i, bits[i]);
+}
+
 // G of a partitioned table before the group programs accumulate into it: dE_i/d(cut) for the packed moments
 // that are cut nodes themselves (gmap[k] = their cut row), 0 for the others
 __global__ void k_ginit(double *__restrict__ G, int n_cut_rows, int n_basic, int ncol, const int *__restrict__ gmap,
@@ -257,6 +330,16 @@ cudaError_t launch_pack_pairs_chunk(const long long *off, int c0, int c1, const 
   const long long blocks = std::min<long long>(148 * 8, std::max<long long>(1, (cap + 1023) / 1024));
   const int vec = (((uintptr_t)idx & 15) == 0 && ((uintptr_t)shift & 3) == 0) ? 1 : 0;
   k_pack_pairs_chunk<<<(unsigned)blocks, 256, 0, st>>>(off, c0, c1, idx, shift, n_atoms, cap, out, flag, touch, touch_shift(n_atoms), vec);
+  count_launch();
+  return cudaGetLastError();
+}
+cudaError_t launch_pack_rows_live(const PairArgs &a, const int *idx, const signed char *shift, long long n_atoms, long long cap, int *out,
+                                  unsigned short *korig, int *cnt, double *d4, unsigned *touch, cudaStream_t st) {
+  if (a.c1 <= a.c0) return cudaSuccess;
+  cudaError_t e = cudaMemsetAsync(touch, 0, kTouchWords * sizeof(unsigned), st);
+  if (e != cudaSuccess) return e;
+  const int blocks = (int)std::min<long long>(148 * 8, ((long long)(a.c1 - a.c0) + 7) / 8);
+  k_pack_rows_live<<<blocks, 256, 0, st>>>(a, idx, shift, n_atoms, cap, out, korig, cnt, d4, touch, touch_shift(n_atoms));
   count_launch();
   return cudaGetLastError();
 }

@@ -26,6 +26,9 @@ struct PairArgs {
   double *d4;                // K3 out (gather mode): [d4_cap][4] records of THIS CHUNK's pairs (index p - off[c0]), or null
   long long d4_cap;          // pairs the chunk's d4 buffer holds; a chunk with more sets flag[1] and drops the excess
   int *flag;                 // device error counters: [0] rejected input pairs, [1] per-pair scratch overflow
+  const int *cnt;            // live rows (MTP_OPT_SKIN_LIST): cnt[atom - c0] = entries of the atom's row within R_cut, moved to the
+                             // front of the row by k_pack_rows_live; null: the CSR row lengths
+  const unsigned short *korig;   // live rows: position in the CSR row of the entry at a compacted position (d4 keeps CSR positions)
   int idx_rel;               // 1: idx holds this chunk's pairs only (index p - off[c0]); 0: the whole list
   long long idx_cap;         // entries idx holds (pairs beyond are treated as absent: their chunk overflowed the scratch)
   double *F;                 // K3 out: [N][3]; atomic mode: every pair is scattered with fp64 atomics; gather mode: F_i += the sum of

@@ -319,7 +319,7 @@ __global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB1) k_moments_s(
   int n_nb = 0;
   if (atom0 + pa < a.c1) {
     beg = a.off[atom0 + pa];
-    n_nb = (int)(a.off[atom0 + pa + 1] - beg);
+    n_nb = a.cnt ? a.cnt[atom0 + pa - a.c0] : (int)(a.off[atom0 + pa + 1] - beg);
     if (a.idx_rel) beg -= a.off[a.c0];           // the neighbour words of this chunk start at 0
   }
   // the centre atoms' records live in shared memory: phase A reads its atom's (a broadcast) instead of holding
@@ -333,7 +333,7 @@ __global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB1) k_moments_s(
   __syncthreads();
   // phase B role: lane = atom; every warp sees the same 32 atoms, so the row-length maximum is a warp reduction
   int nb_lane = 0;
-  if (atom0 + lane < a.c1) nb_lane = (int)(a.off[atom0 + lane + 1] - a.off[atom0 + lane]);
+  if (atom0 + lane < a.c1) nb_lane = a.cnt ? a.cnt[atom0 + lane - a.c0] : (int)(a.off[atom0 + lane + 1] - a.off[atom0 + lane]);
   const int n_max = __reduce_max_sync(0xffffffffu, nb_lane);
   const double rc2 = a.r_cut * a.r_cut;
   double acc[NSLOT];
@@ -404,7 +404,7 @@ __global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB3) k_pairgrad_s
   int n_nb = 0;
   if (atom0 + pa < a.c1) {
     beg = a.off[atom0 + pa];
-    n_nb = (int)(a.off[atom0 + pa + 1] - beg);
+    n_nb = a.cnt ? a.cnt[atom0 + pa - a.c0] : (int)(a.off[atom0 + pa + 1] - beg);
     dbeg = beg - a.off[a.c0];                    // d4 holds this chunk's pairs only
     if (a.idx_rel) beg = dbeg;
   }
@@ -418,7 +418,7 @@ __global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB3) k_pairgrad_s
   int nb_lane = 0;
   double g[NSLOT];
   if (atom0 + lane < a.c1) {
-    nb_lane = (int)(a.off[atom0 + lane + 1] - a.off[atom0 + lane]);
+    nb_lane = a.cnt ? a.cnt[atom0 + lane - a.c0] : (int)(a.off[atom0 + lane + 1] - a.off[atom0 + lane]);
     const int *km = kmsm + slice * NSLOT;
     const double *Gc = a.G + tiled_index(a.n_rows, 0, atom0 + lane - a.c0);
 #pragma unroll
@@ -492,8 +492,9 @@ __global__ void __launch_bounds__(32 * NSL, STile<LEV, NSL>::MINB3) k_pairgrad_s
           }
           Fx += dx; Fy += dy; Fz += dz;
         } else {
-          if (dbeg + k < a.d4_cap) {
-            double2 *o = reinterpret_cast<double2 *>(a.d4) + 2 * (size_t)(dbeg + k);
+          const long long kd = dbeg + (a.korig ? (int)a.korig[dbeg + k] : k);      // live rows: the record keeps its CSR position
+          if (kd < a.d4_cap) {
+            double2 *o = reinterpret_cast<double2 *>(a.d4) + 2 * (size_t)kd;
             o[0] = make_double2(dx, dy);
             o[1] = make_double2(dz, 0.0);
             Fx += dx; Fy += dy; Fz += dz;          // the atom's own pairs are summed here, in fixed order

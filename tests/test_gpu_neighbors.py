@@ -233,3 +233,43 @@ def test_md_loop_with_grade_policy(lib, torch):
         assert o["stopped"] and o["steps_done"] == keep[0] and o["sel_step"] == [0, X][:o["n_evaluations"]][:2]
         assert np.array_equal(pos.cpu().numpy(), want[keep[0]][0])
     pot.close()
+
+
+def test_skin_list_rows_are_compacted_not_multiplied_by_zero(lib, torch):
+    """MTP_OPT_SKIN_LIST: a list built at R_cut + 1 A through the large-system kernels, with the rows compacted to the
+    entries within R_cut, equals the same list evaluated with the skin pairs multiplied by zero, and the list built at
+    R_cut itself: E_i bit for bit (the kept entries come in the same order, and adding zeros changes no sum); forces and
+    virial to rounding (an atom's own pairs are summed by TN threads according to their position in the row, which the
+    dropped entries shift).  Several chunks, explicit shifts and minimum image, both force modes."""
+    w = make_workload(3, n_basis_of(16), cells=8)
+    pot = gpu_pot(lib, w)
+    pot.set_option(lib.OPT_VARIANT, lib.VARIANT_THREAD)
+    pot.set_option(lib.OPT_CHUNK_ATOMS, 600)
+    pos, types = torch.as_tensor(w.pos).cuda(), torch.as_tensor(w.types).cuda()
+    exact, skin = lib.neighbors_build(pos, w.box, 5.0), lib.neighbors_build(pos, w.box, 6.0)
+    assert skin["nnz"] > 1.5 * exact["nnz"]
+
+    def run(nb, live, mode, with_shift=True):
+        pot.set_option(lib.OPT_SKIN_LIST, live)
+        pot.set_option(lib.OPT_FORCE_MODE, mode)
+        n = nb["nnz"]
+        o = pot.compute(pos, types, w.box, nb["off"], nb["idx"][:n], nb["shift"][:n] if with_shift else None, nb["rev"][:n])
+        torch.cuda.synchronize()
+        assert pot.get_option(lib.INFO_INPUT_ERRORS) == 0 and pot.get_option(lib.INFO_SCRATCH_OVERFLOW) == 0
+        return {k: v.cpu().numpy() for k, v in o.items()}
+
+    for with_shift in (True, False):
+        ref = run(exact, 0, lib.FORCE_GATHER, with_shift)
+        zero = run(skin, 0, lib.FORCE_GATHER, with_shift)
+        live = run(skin, 1, lib.FORCE_GATHER, with_shift)
+        for k in ("E", "Ei"):
+            assert np.array_equal(live[k], zero[k]) and np.array_equal(live[k], ref[k]), (k, with_shift)
+        for k in ("F", "virial"):
+            scale = np.abs(ref[k]).max()
+            assert np.abs(live[k] - ref[k]).max() <= 1e-12 * scale and np.abs(zero[k] - ref[k]).max() <= 1e-12 * scale, (k, with_shift)
+        again = run(skin, 1, lib.FORCE_GATHER, with_shift)
+        assert np.array_equal(again["F"], live["F"])                      # still deterministic
+        atom = run(skin, 1, lib.FORCE_ATOMIC, with_shift)
+        assert np.array_equal(atom["Ei"], ref["Ei"])
+        assert np.abs(atom["F"] - ref["F"]).max() <= 1e-12 * np.abs(ref["F"]).max()
+    pot.close()
