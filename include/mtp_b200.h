@@ -90,7 +90,9 @@ const char *mtp_last_error(const mtp_handle *h); /* h may be NULL: last error of
                                                     takes no handle (mtp_create, ..._build_static) */
 
 /* Options (a10 chunk scheduler PAPER.md:62,76; a8 force mode; a12 variant PAPER.md:35). */
-#define MTP_OPT_CHUNK_ATOMS 1   /* atoms per chunk; 0 = automatic (L2-sized)               */
+#define MTP_OPT_CHUNK_ATOMS 1   /* atoms per chunk ("chunksize"); 0 = automatic: as few equal chunks as
+                                   2^20 atoms per chunk and 4 GB of per-atom scratch allow (config 4: one chunk, 4.0 GB
+                                   of workspace); smaller chunks trade speed for memory (32 768 atoms: 179 MB)     */
 #define MTP_OPT_FORCE_MODE 2    /* MTP_FORCE_GATHER (needs d_rev) | MTP_FORCE_ATOMIC       */
 #define MTP_OPT_VARIANT 3       /* MTP_VARIANT_AUTO | _THREAD | _BLOCK                     */
 #define MTP_OPT_PROFILE 4       /* 1: record CUDA events around every kernel launch        */

@@ -687,8 +687,12 @@ int make_plan(const mtp_handle *h, int64_t n_all, int64_t nnz, int want_grade, i
   const int64_t N = rows < 0 ? n_all : rows;
   pl.N = N; pl.nnz = nnz;
   int64_t C = h->chunk_atoms;
-  if (C <= 0) {   // automatic: many waves per launch (no tail), M + G scratch (16 B x n_basic per atom) <= 1 GB
-    C = std::min<int64_t>(262144, (1LL << 30) / (16LL * h->n_basic));
+  if (C <= 0) {
+    // automatic: as few chunks as a budget of 4 GB for M + G (16 B x n_basic per atom) and 2^20 atoms allows -- every chunk
+    // pays its own launches, tails and a walk of the rows it touches in the reverse gather (config 4, one B200: 4 / 2 /
+    // 1 chunks -> 5.64 / 5.41 / 5.28 ms per step at 1.2 / 2.3 / 4.0 GB of workspace, 2 % of the 180 GB).  Callers
+    // short of memory set MTP_OPT_CHUNK_ATOMS: 32 768 atoms -> 179 MB.
+    C = std::min<int64_t>(1 << 20, (4LL << 30) / (16LL * h->n_basic));
     C = std::max<int64_t>(1024, C / 1024 * 1024);
     if (N > C) {  // equal chunks: no small last chunk
       const int64_t nc = (N + C - 1) / C;
@@ -1133,6 +1137,16 @@ extern "C" int mtp_compute_host(mtp_handle *h, int64_t N, const double *pos, con
                                 int64_t nnz, double *E, double *Ei, double *F, double *virial) {
   if (!h) return MTP_EINVAL;
   if (!box || !E || (N > 0 && (!pos || !type || !off || !F)) || (nnz > 0 && !idx)) return fail(h, MTP_EINVAL, "mtp_compute_host: null argument");
+  // Chunks are the unit of the copy / compute pipeline here (the list of chunk c + 1 crosses PCIe while chunk c is
+  // evaluated), so the automatic choice is at most 2^18 atoms instead of as few chunks as possible
+  struct ChunkGuard {
+    mtp_handle *h; int64_t saved;
+    ~ChunkGuard() { h->chunk_atoms = saved; }
+  } guard{h, h->chunk_atoms};
+  if (h->chunk_atoms <= 0 && N > (1 << 18)) {
+    const int64_t nc = (N + (1 << 18) - 1) >> 18;
+    h->chunk_atoms = ((N + nc - 1) / nc + 31) / 32 * 32;
+  }
   // the CSR offsets are on the host here: the per-pair scratch is sized for the largest chunk exactly
   Plan pl;
   int rc = make_plan(h, N, nnz, 0, rev != nullptr, pl);

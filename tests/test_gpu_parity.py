@@ -160,8 +160,10 @@ def test_per_pair_scratch_is_bounded_by_the_chunk(lib, torch):
     pot.set_option(lib.OPT_FORCE_MODE, lib.FORCE_GATHER)
     pot.set_option(lib.OPT_CHUNK_ATOMS, 32768)
     assert pot.workspace_bytes(1048576, 47194874) < 200e6
+    pot.set_option(lib.OPT_CHUNK_ATOMS, 262144)
+    assert pot.workspace_bytes(1048576, 47194874) < 1.3e9        # four chunks: a quarter of the pairs
     pot.set_option(lib.OPT_CHUNK_ATOMS, 0)
-    assert pot.workspace_bytes(1048576, 47194874) < 1.3e9        # automatic chunks (262 144 atoms): a quarter of the pairs
+    assert pot.workspace_bytes(1048576, 47194874) < 4.2e9        # automatic: one chunk within the 4 GB budget for M + G
     d = to_dev(w, torch)
     pot.set_option(lib.OPT_CHUNK_ATOMS, 64)
     pot.set_option(lib.OPT_CHUNK_PAIRS, 100)                      # far too small for 64 atoms x ~54 neighbours
