@@ -300,15 +300,18 @@ __global__ void __launch_bounds__(256) k_nb_rev(const long long *__restrict__ of
   const long long beg = off[i], end = min(off[i + 1], capacity);
   for (long long p = beg + lane; p < end; p += 32) {
     const int j = idx[p];
-    const unsigned want = (unsigned)i * 27u + (unsigned)((1 - shift[3 * p]) * 9 + (1 - shift[3 * p + 1]) * 3 + (1 - shift[3 * p + 2]));
+    // row j is sorted by (neighbour, shift): binary search on the neighbour index alone (one 4-byte load per probe), then
+    // the few entries with that neighbour (one per image) are compared by shift
+    const int w0 = -shift[3 * p], w1 = -shift[3 * p + 1], w2 = -shift[3 * p + 2];
     long long lo = off[j], hi = min(off[j + 1], capacity);
-    long long found = -1;
+    const long long end_j = hi;
     while (lo < hi) {
       const long long mid = (lo + hi) >> 1;
-      const unsigned k = (unsigned)idx[mid] * 27u + (unsigned)((shift[3 * mid] + 1) * 9 + (shift[3 * mid + 1] + 1) * 3 + (shift[3 * mid + 2] + 1));
-      if (k == want) { found = mid; break; }
-      if (k < want) lo = mid + 1; else hi = mid;
+      if (idx[mid] < i) lo = mid + 1; else hi = mid;
     }
+    long long found = -1;
+    for (long long q = lo; q < end_j && idx[q] == i; ++q)
+      if (shift[3 * q] == w0 && shift[3 * q + 1] == w1 && shift[3 * q + 2] == w2) { found = q; break; }
     if (found < 0) atomicAdd(flag, 1);                       // cannot happen for a list built here (the test is symmetric)
     rev[p] = (int)found;
   }
