@@ -129,7 +129,8 @@ def config_dict(w, cfg, world, sharded=False):
     """What the workload is -- the same dictionary in both arms."""
     return {"workload": cfg["name"], "n_atoms": w.n_atoms, "nnz": w.nnz, "lev_max": w.lev_max, "n_species": w.n_species,
             "n_basis": int(w.xi.shape[0]),
-            "l2": "inputs larger than L2 (neighbour list %.0f MB + per-pair scratch), no flush" % (w.nnz * 11 / 1e6),
+            "l2": ("inputs larger than L2 (neighbour list %.0f MB + per-pair scratch), no flush" % (w.nnz * 11 / 1e6)) if w.nnz * 43 > 126e6
+                  else "inputs and scratch fit in the 126 MB L2 and are not flushed: L2-warm steady state, as between the steps of an MD run",
             "parallelism": ("atom ranges x%d, all-reduce of F" if sharded else "replicas x%d") % world}
 
 
