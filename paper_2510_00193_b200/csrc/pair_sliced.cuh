@@ -119,7 +119,7 @@ struct STile {
   // UNR3 neighbours per trip it fits
   static constexpr int UNR3 = TN <= 4 ? K3_UNROLL_NARROW : K3_UNROLL_WIDE;
   static constexpr int MINB1 = Slicing<LEV, NSL>::NSLOT <= 40 ? (512 / NT > 0 ? 512 / NT : 1) : 1;
-  static constexpr int MINB3 = Slicing<LEV, NSL>::NSLOT <= 40 ? (K3_THREADS_PER_SM / NT > 0 ? K3_THREADS_PER_SM / NT : 1) : 1;
+  static constexpr int MINB3 = Slicing<LEV, NSL>::NSLOT <= 40 ? (384 / NT > 0 ? 384 / NT : 1) : 1;
 };
 
 // cp.async staging of one pair per thread (the scheme of pair_tiled.cuh with one slot per thread)
