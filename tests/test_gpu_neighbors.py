@@ -273,3 +273,33 @@ def test_skin_list_rows_are_compacted_not_multiplied_by_zero(lib, torch):
         assert np.array_equal(atom["Ei"], ref["Ei"])
         assert np.abs(atom["F"] - ref["F"]).max() <= 1e-12 * np.abs(ref["F"]).max()
     pot.close()
+
+
+def test_list_and_md_edge_cases(lib, torch):
+    """One atom (its own images only), two atoms out of range (no pairs at all), an atom count that is not a multiple
+    of anything, a zero-step MD call on a system without pairs."""
+    box = np.eye(3) * 12.0
+    one = np.array([[1.0, 2.0, 3.0]])
+    off, idx, sh, rev, nb = build(lib, torch, one, box, 5.0)
+    assert nb["nnz"] == 0 and off.tolist() == [0, 0] and nb["errors"] == 0
+    off, idx, sh, rev, nb = build(lib, torch, one, np.eye(3) * 4.0, 5.0)          # box smaller than the radius: 6 own images at 4 A
+    o_off, o_idx, o_sh = omtp.brute_force_neighbours(one, np.eye(3) * 4.0, 5.0)
+    assert nb["nnz"] == o_off[-1] == 6 and np.array_equal(sh, o_sh) and np.array_equal(rev, reverse_index(o_off, o_idx, o_sh))
+    two = np.array([[1.0, 1.0, 1.0], [7.0, 7.0, 7.0]])
+    off, idx, sh, rev, nb = build(lib, torch, two, box, 5.0)
+    assert nb["nnz"] == 0 and off.tolist() == [0, 0, 0]
+    rng = np.random.default_rng(2)
+    pos = rng.uniform(0, 12.0, (37, 3))
+    off, idx, sh, rev, nb = build(lib, torch, pos, box, 5.0)
+    o_off, o_idx, o_sh = omtp.brute_force_neighbours(pos, box, 5.0)
+    assert np.array_equal(off, o_off) and np.array_equal(idx, o_idx) and np.array_equal(sh, o_sh)
+    # MD on the pairless system: E = sum xi0, F = 0, nothing moves without velocities
+    w = make_workload(0, n_basis_of(10))
+    pot = gpu_pot(lib, w)
+    p, v, t = torch.as_tensor(two).cuda(), torch.zeros((2, 3), dtype=torch.float64, device="cuda"), torch.zeros(2, dtype=torch.int32, device="cuda")
+    o = pot.md_run(p, v, t, box, np.array([55.845]), 1e-3, 3, 1, 0.5, 16)
+    torch.cuda.synchronize()
+    assert o["info"].cpu().tolist() == [0, 0] and not o["F"].cpu().numpy().any()
+    assert float(o["E"][0]) == pytest.approx(2 * w.xi0[0]) and float(o["E"][1]) == 0.0
+    assert np.array_equal(p.cpu().numpy(), two)
+    pot.close()
