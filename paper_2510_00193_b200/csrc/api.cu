@@ -719,7 +719,7 @@ int make_plan(const mtp_handle *h, int64_t n_all, int64_t nnz, int want_grade, i
   pl.o_Ei = o; o = align_up(o + (size_t)n_all * 8);
   pl.o_M = o; o = align_up(o + (size_t)h->n_basic * pl.cols * 8);
   pl.o_G = o; o = align_up(o + (size_t)h->n_basic * pl.cols * 8);
-  pl.o_red = o; o = align_up(o + 256 * 8 * 8);
+  pl.o_red = o; o = align_up(o + 2 * 256 * 8 * 8);            // partial rows of the two final sums (launch_reduce_energy_virial)
   if (h->n_cut_rows > 0) {                   // cut values and their adjoints of one chunk (tree_partition.cpp)
     pl.o_S = o; o = align_up(o + (size_t)h->n_cut_rows * pl.cols * 8);
     pl.o_Sbar = o; o = align_up(o + (size_t)h->n_cut_rows * pl.cols * 8);
@@ -914,11 +914,11 @@ static int compute_impl(mtp_handle *h, int64_t N, const double *d_pos, const int
   double *pos4 = (double *)(ws + pl.o_pos4), *Ei = d_Ei ? d_Ei : (double *)(ws + pl.o_Ei);
   double *M = (double *)(ws + pl.o_M), *G = (double *)(ws + pl.o_G), *wpart = (double *)(ws + pl.o_wpart);
   double *d4 = (double *)(ws + pl.o_d4);
-  CU(h, launch_pack(d_pos, d_type, (int)N, pos4, st));
-  CU(h, launch_zero(wpart, (long long)pl.n_chunks * pl.grid_chunk * 8, st));
-  CU(h, launch_zero(d_F, 3 * N, st));            // both force modes accumulate: atomics, or chunk by chunk in fixed order
   int *idxp = (int *)(ws + pl.o_idxp);
   unsigned *jrange = (unsigned *)(ws + pl.o_jr);
+  // pos4, F = 0 (both force modes accumulate: atomics, or chunk by chunk in fixed order), virial partials = 0, the first
+  // chunk's touch bitmap = 0: one launch
+  CU(h, launch_prologue(d_pos, d_type, (int)N, pos4, d_F, wpart, (long long)pl.n_chunks * pl.grid_chunk * 8, jrange, st));
   // MTP_OPT_SKIN_LIST (large-system kernels only): rows compacted to the entries within R_cut, chunk by chunk
   const bool live = h->skin_list && pl.sliced && nnz > 0;
   unsigned short *korig = (unsigned short *)(ws + pl.o_korig);
@@ -935,10 +935,11 @@ static int compute_impl(mtp_handle *h, int64_t N, const double *d_pos, const int
     if (pipe) CU(h, cudaStreamWaitEvent(st, (*pipe->chunk_ready)[c], 0));      // this chunk's pairs have arrived
     // the chunk's neighbour words (validated, index + image code in 4 bytes) and the range of atoms it touches
     if (live)
-      CU(h, launch_pack_rows_live(pa, d_idx, (const signed char *)d_shift, N, pl.cap, idxp, korig, cnt, pl.atomic ? nullptr : d4, jrange, st));
+      CU(h, launch_pack_rows_live(pa, d_idx, (const signed char *)d_shift, N, pl.cap, idxp, korig, cnt, pl.atomic ? nullptr : d4, jrange, st,
+                                  c == 0));
     else if (nnz > 0)
       CU(h, launch_pack_pairs_chunk((const long long *)d_off, pa.c0, pa.c1, d_idx, (const signed char *)d_shift, N, pl.cap,
-                                    d_shift ? idxp : nullptr, h->d_flag, jrange, st));
+                                    d_shift ? idxp : nullptr, h->d_flag, jrange, st, c == 0));
     pa.cnt = live ? cnt : nullptr; pa.korig = live ? korig : nullptr;
     pa.M = M; pa.G = G; pa.kmap = pl.sliced ? h->d_kmapS : h->d_kmapF;
     TIMED(h, CLS_MOMENTS, st, (pl.sliced ? h->pl->moments_s(pa, st) : h->pl->moments(pa, pl.P, st)));
@@ -954,9 +955,8 @@ static int compute_impl(mtp_handle *h, int64_t N, const double *d_pos, const int
     }
   }
   double *red = (double *)(ws + pl.o_red);
-  if (row_hi > row_lo) CU(h, launch_reduce(Ei + row_lo, row_hi - row_lo, 1, 1, d_E, red, st));
-  else CU(h, launch_zero(d_E, 1, st));
-  if (d_virial) CU(h, launch_reduce(wpart, (long long)pl.n_chunks * pl.grid_chunk, 8, 6, d_virial, red, st));
+  // E = sum of the window's E_i (an empty window sums nothing: 0) and the virial from the block partials, in one launch
+  CU(h, launch_reduce_energy_virial(Ei + row_lo, row_hi - row_lo, d_E, wpart, (long long)pl.n_chunks * pl.grid_chunk, d_virial, red, st));
   return MTP_OK;
 }
 

@@ -89,6 +89,11 @@ const PairLevel *pair_level(int index);   // index into kLevels
 // ---- misc kernels (misc_kernels.cu)
 cudaError_t launch_pack(const double *pos, const int *type, int n, double *pos4, cudaStream_t st);
 cudaError_t launch_zero(double *p, long long n, cudaStream_t st);
+// pack + F = 0 + virial partials = 0 + touch bitmap = 0 in one launch; E and virial sums in one (two-level: two) launch
+cudaError_t launch_prologue(const double *pos, const int *type, int n, double *pos4, double *F, double *wpart, long long n_wpart,
+                            unsigned *touch, cudaStream_t st);
+cudaError_t launch_reduce_energy_virial(const double *Ei, long long n, double *E, const double *wpart, long long n_w, double *virial,
+                                        double *scratch, cudaStream_t st);
 // G[k][:] = gmap[k] >= 0 ? Sbar[gmap[k]][:] : 0  (partitioned K2, before the group programs accumulate)
 // S[gmap[k]][:] = M[k][:] for the packed moments that are cut nodes themselves
 cudaError_t launch_scopy(double *S, int n_cut_rows, int n_basic, int ncol, const int *gmap, const double *M, cudaStream_t st);
@@ -102,10 +107,10 @@ cudaError_t launch_untile(const double *src, int rows, long long ncol, double *d
 constexpr int kTouchWords = 512;
 inline int touch_shift(long long n_atoms) { int s = 6; while ((n_atoms >> s) >= kTouchWords * 32) ++s; return s; }
 cudaError_t launch_pack_pairs_chunk(const long long *off, int c0, int c1, const int *idx, const signed char *shift, long long n_atoms,
-                                    long long cap, int *out, int *flag, unsigned *touch, cudaStream_t st);
+                                    long long cap, int *out, int *flag, unsigned *touch, cudaStream_t st, bool touch_is_zero = false);
 // the same for a list with a skin (MTP_OPT_SKIN_LIST): rows compacted to the entries within R_cut (misc_kernels.cu)
 cudaError_t launch_pack_rows_live(const PairArgs &a, const int *idx, const signed char *shift, long long n_atoms, long long cap, int *out,
-                                  unsigned short *korig, int *cnt, double *d4, unsigned *touch, cudaStream_t st);
+                                  unsigned short *korig, int *cnt, double *d4, unsigned *touch, cudaStream_t st, bool touch_is_zero = false);
 // F_k -= sum over the neighbours j in the chunk of d4[rev], for every atom k of a touched block
 cudaError_t launch_gather_chunk(const long long *off, const int *idx, const int *rev, const double *d4, long long d4_cap, int c0,
                                 int c1, int n_atoms, const unsigned *touch, double *F, cudaStream_t st);

@@ -204,6 +204,21 @@ __global__ void k_untile(const double *__restrict__ src, int rows, long long nco
   if (transpose) dst[col * ld + row] = v; else dst[(long long)row * ld + col] = v;
 }
 
+// Prologue of mtp_compute in one launch (small systems pay per launch): pos4 = (x, y, z, species), F = 0, the virial
+// partials = 0, the touch bitmap of the first chunk = 0
+__global__ void k_prologue(const double *__restrict__ pos, const int *__restrict__ type, int n, double *__restrict__ pos4,
+                           double *__restrict__ F, double *__restrict__ wpart, long long n_wpart, unsigned *__restrict__ touch) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) {
+    double2 *o = reinterpret_cast<double2 *>(pos4) + 2 * (size_t)i;
+    o[0] = make_double2(pos[3 * (size_t)i], pos[3 * (size_t)i + 1]);
+    o[1] = make_double2(pos[3 * (size_t)i + 2], (double)type[i]);
+    F[3 * (size_t)i] = 0.0; F[3 * (size_t)i + 1] = 0.0; F[3 * (size_t)i + 2] = 0.0;
+  }
+  if (i < n_wpart) wpart[i] = 0.0;
+  if (i < kTouchWords) touch[i] = 0u;
+}
+
 __global__ void k_zero(double *p, long long n) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) p[i] = 0.0;
@@ -315,6 +330,13 @@ cudaError_t launch_scopy(double *S, int n_cut_rows, int n_basic, int ncol, const
   count_launch();
   return cudaGetLastError();
 }
+cudaError_t launch_prologue(const double *pos, const int *type, int n, double *pos4, double *F, double *wpart, long long n_wpart,
+                            unsigned *touch, cudaStream_t st) {
+  const long long m = std::max<long long>(std::max<long long>(n, n_wpart), kTouchWords);
+  k_prologue<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(pos, type, n, pos4, F, wpart, n_wpart, touch);
+  count_launch();
+  return cudaGetLastError();
+}
 cudaError_t launch_zero(double *p, long long n, cudaStream_t st) {
   if (n <= 0) return cudaSuccess;
   k_zero<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p, n);
@@ -322,9 +344,9 @@ cudaError_t launch_zero(double *p, long long n, cudaStream_t st) {
   return cudaGetLastError();
 }
 cudaError_t launch_pack_pairs_chunk(const long long *off, int c0, int c1, const int *idx, const signed char *shift, long long n_atoms,
-                                    long long cap, int *out, int *flag, unsigned *touch, cudaStream_t st) {
+                                    long long cap, int *out, int *flag, unsigned *touch, cudaStream_t st, bool touch_is_zero) {
   if (c1 <= c0) return cudaSuccess;
-  cudaError_t e = cudaMemsetAsync(touch, 0, kTouchWords * sizeof(unsigned), st);
+  cudaError_t e = touch_is_zero ? cudaSuccess : cudaMemsetAsync(touch, 0, kTouchWords * sizeof(unsigned), st);
   if (e != cudaSuccess) return e;
   // the pair count of the chunk lives on the device: a persistent grid strides over it
   const long long blocks = std::min<long long>(148 * 8, std::max<long long>(1, (cap + 1023) / 1024));
@@ -334,9 +356,9 @@ cudaError_t launch_pack_pairs_chunk(const long long *off, int c0, int c1, const 
   return cudaGetLastError();
 }
 cudaError_t launch_pack_rows_live(const PairArgs &a, const int *idx, const signed char *shift, long long n_atoms, long long cap, int *out,
-                                  unsigned short *korig, int *cnt, double *d4, unsigned *touch, cudaStream_t st) {
+                                  unsigned short *korig, int *cnt, double *d4, unsigned *touch, cudaStream_t st, bool touch_is_zero) {
   if (a.c1 <= a.c0) return cudaSuccess;
-  cudaError_t e = cudaMemsetAsync(touch, 0, kTouchWords * sizeof(unsigned), st);
+  cudaError_t e = touch_is_zero ? cudaSuccess : cudaMemsetAsync(touch, 0, kTouchWords * sizeof(unsigned), st);
   if (e != cudaSuccess) return e;
   const int blocks = (int)std::min<long long>(148 * 8, ((long long)(a.c1 - a.c0) + 7) / 8);
   k_pack_rows_live<<<blocks, 256, 0, st>>>(a, idx, shift, n_atoms, cap, out, korig, cnt, d4, touch, touch_shift(n_atoms));
@@ -358,6 +380,54 @@ cudaError_t launch_reduce(const double *in, long long n, int stride, int ncomp, 
     k_reduce_rows<<<1, 1024, 0, st>>>(scratch, kReduceBlocks, 8, ncomp, out);
   } else {
     k_reduce_rows<<<1, 1024, 0, st>>>(in, n, stride, ncomp, out);
+  }
+  count_launch();
+  return cudaGetLastError();
+}
+// E = sum E_i and the six virial sums in the same launches: blockIdx.y selects the array (fixed order, as launch_reduce)
+__global__ void __launch_bounds__(1024) k_reduce_two(const double *__restrict__ in0, long long n0, int stride0, int ncomp0, double *__restrict__ out0,
+                                                     const double *__restrict__ in1, long long n1, int stride1, int ncomp1,
+                                                     double *__restrict__ out1) {
+  const bool second = blockIdx.y == 1;
+  const double *in = second ? in1 : in0;
+  const long long n = second ? n1 : n0;
+  const int stride = second ? stride1 : stride0, ncomp = second ? ncomp1 : ncomp0;
+  double *out = second ? out1 : out0;
+  __shared__ double sm[32][8];
+  double acc[8];
+#pragma unroll
+  for (int c = 0; c < 8; ++c) acc[c] = 0.0;
+  for (long long i = (long long)blockIdx.x * 1024 + threadIdx.x; i < n; i += 1024LL * gridDim.x)
+    for (int c = 0; c < ncomp; ++c) acc[c] += in[i * stride + c];
+#pragma unroll
+  for (int c = 0; c < 8; ++c) {
+    double v = acc[c];
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5][c] = v;
+  }
+  __syncthreads();
+  if (threadIdx.x < 8) {
+    double v = 0.0;
+    if (threadIdx.x < ncomp)
+      for (int w = 0; w < 32; ++w) v += sm[w][threadIdx.x];
+    if (gridDim.x > 1) out[(size_t)blockIdx.x * 8 + threadIdx.x] = v;
+    else if (threadIdx.x < ncomp) out[threadIdx.x] = v;
+  }
+}
+// E (from Ei [n]) and, when virial != null, the virial (from wpart [n_w][8]); scratch: 2 x kReduceBlocks x 8 doubles.
+// The same summation order as two launch_reduce calls.
+cudaError_t launch_reduce_energy_virial(const double *Ei, long long n, double *E, const double *wpart, long long n_w, double *virial,
+                                        double *scratch, cudaStream_t st) {
+  const dim3 two(1, virial ? 2 : 1);
+  if (std::max(n, virial ? n_w : 0) > 4 * 1024) {
+    // level 1 writes kReduceBlocks partial rows per array (an array shorter than the grid just leaves zeros), level 2 sums them
+    double *s0 = scratch, *s1 = scratch + kReduceBlocks * 8;
+    k_reduce_two<<<dim3(kReduceBlocks, two.y), 1024, 0, st>>>(Ei, n, 1, 1, s0, wpart, n_w, 8, 6, s1);
+    count_launch();
+    k_reduce_two<<<two, 1024, 0, st>>>(s0, kReduceBlocks, 8, 1, E, s1, kReduceBlocks, 8, 6, virial);
+  } else {
+    k_reduce_two<<<two, 1024, 0, st>>>(Ei, n, 1, 1, E, wpart, n_w, 8, 6, virial);
   }
   count_launch();
   return cudaGetLastError();
