@@ -194,13 +194,13 @@ def test_chunked_equals_unchunked_and_gather_is_deterministic(lib, torch):
     pot.close()
 
 
-def cluster_workload(lev, n_mu, seed, n, S, box_len=11.0, r_list=5.0):
+def cluster_workload(lev, n_mu, seed, n, S, box_len=11.0, r_list=5.0, n_beta=8):
     pos, types, box = random_cluster(seed, n, box_len, n_species=S)
     off, idx, sh = omtp.brute_force_neighbours(pos, box, r_list)
     rng = np.random.default_rng(seed + 1)
     nb = n_basis_of(lev)
-    return Workload(name="cluster", lev_max=lev, n_mu=n_mu, n_beta=8, r_min=2.0, r_cut=5.0, n_species=S,
-                    box=box, pos=pos, types=types, c=rng.uniform(-0.1, 0.1, (S, S, n_mu, 8)),
+    return Workload(name="cluster", lev_max=lev, n_mu=n_mu, n_beta=n_beta, r_min=2.0, r_cut=5.0, n_species=S,
+                    box=box, pos=pos, types=types, c=rng.uniform(-0.1, 0.1, (S, S, n_mu, n_beta)),
                     xi0=rng.uniform(-0.1, 0.1, S), xi=rng.uniform(-0.1, 0.1, nb), off=off, idx=idx,
                     shift=sh, rev=reverse_index(off, idx, sh))
 
@@ -219,6 +219,20 @@ def test_ragged_cluster_with_skin_and_short_pairs(lib, torch, lev, n_mu, n):
     got, pot, _ = run_gpu(lib, torch, w, interp=True)
     check(w, ref, got, opot)
     pot.close()
+
+
+@pytest.mark.parametrize("n_beta", [1, 2, 5, 12])
+def test_radial_basis_sizes_other_than_eight(lib, torch, n_beta):
+    """The BASELINE configurations all have 8 Chebyshev polynomials (a compile-time size in K1 / K3); any other size
+    takes the run-time loop.  Small-system kernels, then the large-system (sliced) kernels forced on the same cluster."""
+    w = cluster_workload(16, 4, 33, 36, 3, r_list=5.3, n_beta=n_beta)
+    opot = oracle_pot(w)
+    ref = omtp.evaluate(opot, w.pos, w.types, w.box, w.off, w.idx, w.shift)
+    for variant in (lib.VARIANT_AUTO, lib.VARIANT_THREAD):
+        for mode in (lib.FORCE_GATHER, lib.FORCE_ATOMIC):
+            got, pot, _ = run_gpu(lib, torch, w, opts={lib.OPT_VARIANT: variant, lib.OPT_FORCE_MODE: mode})
+            check(w, ref, got, opot)
+            pot.close()
 
 
 def test_level24_lattice_sample_and_grades(lib, torch):
