@@ -235,6 +235,20 @@ def test_radial_basis_sizes_other_than_eight(lib, torch, n_beta):
             pot.close()
 
 
+@pytest.mark.parametrize("S", [5, 8])
+def test_many_species(lib, torch, S):
+    """More species than any BASELINE configuration: S^2 coefficient blocks staged in shared memory (c[z_i][z_j] is not
+    symmetric: reading G6), small- and large-system kernels."""
+    w = cluster_workload(10, 3, 44 + S, 48, S, r_list=5.0)
+    assert len(set(w.types.tolist())) == S
+    opot = oracle_pot(w)
+    ref = omtp.evaluate(opot, w.pos, w.types, w.box, w.off, w.idx, w.shift)
+    for variant in (lib.VARIANT_AUTO, lib.VARIANT_THREAD):
+        got, pot, _ = run_gpu(lib, torch, w, opts={lib.OPT_VARIANT: variant})
+        check(w, ref, got, opot)
+        pot.close()
+
+
 def test_level24_lattice_sample_and_grades(lib, torch):
     """Config-5 shape at reduced size: B, E_i on sampled atoms; both grade modes."""
     nb = n_basis_of(24)
