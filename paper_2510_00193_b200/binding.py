@@ -458,6 +458,23 @@ class Potential:
         return out
 
 
+def dump_selected(path, run, types, box, append=True):
+    """The dump step of the grade policy ("the current configuration is written to the output file"): the
+    configurations md_run_al kept, as extended-XYZ text frames (species index, x, y, z per atom; lattice, step and
+    grade in the comment line).  The MLIP-3 .cfg format of the paper is not reproduced (its specification is not
+    available here).  Returns the number of frames written."""
+    box = np.asarray(box, dtype=np.float64).reshape(9)
+    types = np.asarray(types.cpu() if hasattr(types, "cpu") else types)
+    sel = run["selected"].cpu().numpy() if hasattr(run["selected"], "cpu") else np.asarray(run["selected"])
+    with open(path, "a" if append else "w") as f:
+        for k, (step, grade) in enumerate(zip(run["sel_step"], run["sel_grade"])):
+            f.write("%d\n" % sel.shape[1])
+            f.write('Lattice="%s" Properties=species:I:1:pos:R:3 step=%d grade=%.17g\n' % (" ".join("%.17g" % v for v in box), step, grade))
+            for t, (x, y, z) in zip(types, sel[k]):
+                f.write("%d %.17g %.17g %.17g\n" % (int(t), x, y, z))
+    return len(run["sel_step"])
+
+
 class ComputeGraph:
     """An mtp_graph: one captured mtp_compute call."""
 

@@ -224,6 +224,14 @@ def test_md_loop_with_grade_policy(lib, torch):
         assert o["max_grade"] == max(grades)
         for k, s in enumerate(keep):
             assert np.array_equal(o["selected"][k].cpu().numpy(), want[s][0])
+        if mode == 0:                                                    # the dump of the kept configurations reads back exactly
+            import os, tempfile
+            path = os.path.join(tempfile.mkdtemp(), "selected.xyz")
+            assert lib.dump_selected(path, o, d["types"], w.box) == len(keep)
+            lines = open(path).read().split("\n")
+            assert len(lines) == len(keep) * (w.n_atoms + 2) + 1 and ("step=%d " % keep[0]) in lines[1]
+            back = np.array([[float(v) for v in ln.split()[1:]] for ln in lines[2:2 + w.n_atoms]])
+            assert np.array_equal(back, want[keep[0]][0])
         if mode == 0:
             assert np.array_equal(o["gamma_atom"].cpu().numpy(), want[steps][3])
         assert np.array_equal(pos.cpu().numpy(), want[steps][0])
