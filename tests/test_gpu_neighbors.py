@@ -266,7 +266,8 @@ def test_skin_list_rows_are_compacted_not_multiplied_by_zero(lib, torch):
         assert pot.get_option(lib.INFO_INPUT_ERRORS) == 0 and pot.get_option(lib.INFO_SCRATCH_OVERFLOW) == 0
         return {k: v.cpu().numpy() for k, v in o.items()}
 
-    for with_shift in (True, False):
+    for with_shift, chunk in ((True, 600), (False, 600), (True, 0)):       # several chunks, and the automatic single chunk
+        pot.set_option(lib.OPT_CHUNK_ATOMS, chunk)
         ref = run(exact, 0, lib.FORCE_GATHER, with_shift)
         zero = run(skin, 0, lib.FORCE_GATHER, with_shift)
         live = run(skin, 1, lib.FORCE_GATHER, with_shift)
