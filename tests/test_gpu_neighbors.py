@@ -312,3 +312,31 @@ def test_list_and_md_edge_cases(lib, torch):
     assert float(o["E"][0]) == pytest.approx(2 * w.xi0[0]) and float(o["E"][1]) == 0.0
     assert np.array_equal(p.cpu().numpy(), two)
     pot.close()
+
+
+def test_md_loop_through_the_large_system_kernels(lib, torch):
+    """The MD loop on the sliced K1 / K3 (forced), where a list with a skin is compacted every step (MTP_OPT_SKIN_LIST):
+    the total energy is conserved to a small fraction of the kinetic energy gained, and rebuilding every 5 steps at a
+    1 A skin gives the trajectory of rebuilding every step at no skin."""
+    w = make_workload(3, n_basis_of(16), cells=12)
+    pot = gpu_pot(lib, w)
+    pot.set_option(lib.OPT_VARIANT, lib.VARIANT_THREAD)
+    pos0, types = torch.as_tensor(w.pos).cuda(), torch.as_tensor(w.types).cuda()
+    mass = np.full(w.n_species, 55.845)
+    cap = int(w.nnz * 1.9) + 1024
+    res = {}
+    for every, skin in ((1, 0.0), (5, 1.0)):
+        pos, vel = pos0.clone(), torch.zeros_like(pos0)
+        e0 = pot.md_run(pos, vel, types, w.box, mass, 2e-9, 0, every, skin, cap)["E"].cpu().numpy().sum()
+        o = pot.md_run(pos, vel, types, w.box, mass, 2e-9, 40, every, skin, cap)
+        torch.cuda.synchronize()
+        E = o["E"].cpu().numpy()
+        assert o["info"].cpu().tolist()[1] == 0 and o["info"].cpu().tolist()[0] <= cap
+        assert pot.get_option(lib.INFO_INPUT_ERRORS) == 0 and pot.get_option(lib.INFO_SCRATCH_OVERFLOW) == 0
+        assert E[1] > 0 and abs(E.sum() - e0) < 1e-4 * E[1]
+        res[every] = pos.cpu().numpy()
+    d = res[1] - res[5]
+    L = w.box[0, 0]
+    d -= np.round(d / L) * L
+    assert np.abs(d).max() < 1e-10
+    pot.close()
