@@ -32,7 +32,7 @@ sys.path.insert(0, ROOT)
 LEVELS = [10, 16, 20, 16, 24]
 HEADLINE = 3                         # 0-based index of the configuration BASELINE.json's metric is quoted on
 UNIT = "atom-evals/s"
-MD_DT = 1e-10                        # ps: the seeded random coefficients give forces of 1e8 eV/A at level 16; the atoms must stay put
+MD_DT = 1e-10                        # ps, upper bound of the MD leg's time step (it is reduced further where the forces ask for it)
 
 
 def metric_name(config, w):
@@ -378,20 +378,24 @@ def run_ours(args):
         cap = int(w.nnz * 1.9) + 1024                       # (6 / 5)^3 = 1.73 x the pairs at R_cut
         mpos, mvel = pos.clone(), torch.zeros_like(pos)
         mass = np.full(w.n_species, 55.845)
+        # the atoms must stay put over the 10 + md_steps steps (forces reach 1e8 eV/A at level 16 and far more at level
+        # 24 with the seeded coefficients): a step such that the largest acceleration moves an atom by < 1e-3 A in total
+        a_max = 9648.533 * float(out["F"].abs().max().item()) / mass[0]
+        md_dt = min(MD_DT, (2e-3 / max(a_max, 1e-300)) ** 0.5 / (10 + md_steps))
         pot.set_option(lib.OPT_PROFILE, 0)
-        pot.md_run(mpos, mvel, types, w.box, mass, MD_DT, 10, 10, 1.0, cap)
+        pot.md_run(mpos, mvel, types, w.box, mass, md_dt, 10, 10, 1.0, cap)
         barrier()
         n1 = lib.launch_count()
         m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         m0.record()
-        mo = pot.md_run(mpos, mvel, types, w.box, mass, MD_DT, md_steps, 10, 1.0, cap)
+        mo = pot.md_run(mpos, mvel, types, w.box, mass, md_dt, md_steps, 10, 1.0, cap)
         m1.record()
         barrier()
         md_ms = max_over_ranks(m0.elapsed_time(m1), dist, dev)
         info = [int(x) for x in mo["info"].cpu()]
         assert info[0] <= cap and info[1] == 0, "MD list overflow"
         md = {"value": world * w.n_atoms * md_steps / (md_ms * 1e-3), "unit": "atom-timesteps/s", "steps": md_steps,
-              "ms_per_step": md_ms / md_steps, "rebuild_every": 10, "skin": 1.0, "list_pairs": info[0],
+              "ms_per_step": md_ms / md_steps, "rebuild_every": 10, "skin": 1.0, "dt_ps": md_dt, "list_pairs": info[0],
               "gpu_launches": int(lib.launch_count() - n1)}
         pot.set_option(lib.OPT_PROFILE, 1)
         del mpos, mvel, mo
