@@ -409,6 +409,9 @@ def run_ours(args):
     per_step = flops_per_step(pot.cost_model(), int(w.off[hi] - w.off[lo]), hi - lo) if args.sharded else \
         flops_per_step(pot.cost_model(), w.nnz, w.n_atoms)
     timed = {k: prof[k] for k in ("moments", "tree", "pairgrad")}
+    if Ainv is not None:                                   # --grade: K5's GEMM, 2 n_basis^2 flop per atom (fp64 mma.sync: the same peak)
+        per_step["grade"] = 2.0 * float(table.n_basis) ** 2 * (hi - lo if args.sharded else w.n_atoms)
+        timed["grade"] = prof["grade"]
     dom = max(timed, key=lambda k: timed[k][0])
     dom_ms, dom_n = timed[dom]
     sms = torch.cuda.get_device_properties(dev).multi_processor_count
