@@ -334,12 +334,15 @@ def run_ours(args):
     # ---- small systems: the same call replayed from a CUDA graph (launch overhead removed)
     graph = None
     if w.n_atoms <= 16384 and Ainv is None and world == 1 and not args.sharded:
-        cg, gout = pot.graph(pos, types, w.box, off, idx, shift, rev)
-        gms = graph_replay(torch, pot, cg)
-        assert torch.equal(gout["F"], out["F"]), "graph launch differs from mtp_compute"
-        cg.close()
-        graph = {"calls": 100, "ms_per_call": gms, "value": w.n_atoms / (gms * 1e-3), "unit": UNIT,
-                 "entry": "mtp_graph_capture / mtp_graph_launch"}
+        try:
+            cg, gout = pot.graph(pos, types, w.box, off, idx, shift, rev)
+            gms = graph_replay(torch, pot, cg)
+            assert torch.equal(gout["F"], out["F"]), "graph launch differs from mtp_compute"
+            cg.close()
+            graph = {"calls": 100, "ms_per_call": gms, "value": w.n_atoms / (gms * 1e-3), "unit": UNIT,
+                     "entry": "mtp_graph_capture / mtp_graph_launch"}
+        except Exception as exc:      # an auxiliary leg must not take the headline line with it
+            graph = {"error": "%s: %s" % (type(exc).__name__, exc)}
 
     # ---- end to end through the host-buffer entry points (pinned inputs, results read back).  `e2e`: what an MD host
     # code sends every step -- positions and types -- with the list built on the device (mtp_compute_host_pos);
@@ -374,31 +377,35 @@ def run_ours(args):
     # coefficients make a stiff potential, hence the tiny time step MD_DT: the work per step does not depend on it.
     md = None
     if not args.no_md and Ainv is None:
-        md_steps = max(10, min(args.steps, 50))
-        cap = int(w.nnz * 1.9) + 1024                       # (6 / 5)^3 = 1.73 x the pairs at R_cut
-        mpos, mvel = pos.clone(), torch.zeros_like(pos)
-        mass = np.full(w.n_species, 55.845)
-        # the atoms must stay put over the 10 + md_steps steps (forces reach 1e8 eV/A at level 16 and far more at level
-        # 24 with the seeded coefficients): a step such that the largest acceleration moves an atom by < 1e-3 A in total
-        a_max = 9648.533 * float(out["F"].abs().max().item()) / mass[0]
-        md_dt = min(MD_DT, (2e-3 / max(a_max, 1e-300)) ** 0.5 / (10 + md_steps))
-        pot.set_option(lib.OPT_PROFILE, 0)
-        pot.md_run(mpos, mvel, types, w.box, mass, md_dt, 10, 10, 1.0, cap)
-        barrier()
-        n1 = lib.launch_count()
-        m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        m0.record()
-        mo = pot.md_run(mpos, mvel, types, w.box, mass, md_dt, md_steps, 10, 1.0, cap)
-        m1.record()
-        barrier()
-        md_ms = max_over_ranks(m0.elapsed_time(m1), dist, dev)
-        info = [int(x) for x in mo["info"].cpu()]
-        assert info[0] <= cap and info[1] == 0, "MD list overflow"
-        md = {"value": world * w.n_atoms * md_steps / (md_ms * 1e-3), "unit": "atom-timesteps/s", "steps": md_steps,
-              "ms_per_step": md_ms / md_steps, "rebuild_every": 10, "skin": 1.0, "dt_ps": md_dt, "list_pairs": info[0],
-              "gpu_launches": int(lib.launch_count() - n1)}
-        pot.set_option(lib.OPT_PROFILE, 1)
-        del mpos, mvel, mo
+        try:
+            md_steps = max(10, min(args.steps, 50))
+            cap = int(w.nnz * 1.9) + 1024                       # (6 / 5)^3 = 1.73 x the pairs at R_cut
+            mpos, mvel = pos.clone(), torch.zeros_like(pos)
+            mass = np.full(w.n_species, 55.845)
+            # the atoms must stay put over the 10 + md_steps steps (forces reach 1e8 eV/A at level 16 and far more at level
+            # 24 with the seeded coefficients): a step such that the largest acceleration moves an atom by < 1e-3 A in total
+            a_max = 9648.533 * float(out["F"].abs().max().item()) / mass[0]
+            md_dt = min(MD_DT, (2e-3 / max(a_max, 1e-300)) ** 0.5 / (10 + md_steps))
+            pot.set_option(lib.OPT_PROFILE, 0)
+            pot.md_run(mpos, mvel, types, w.box, mass, md_dt, 10, 10, 1.0, cap)
+            barrier()
+            n1 = lib.launch_count()
+            m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            m0.record()
+            mo = pot.md_run(mpos, mvel, types, w.box, mass, md_dt, md_steps, 10, 1.0, cap)
+            m1.record()
+            barrier()
+            md_ms = max_over_ranks(m0.elapsed_time(m1), dist, dev)
+            info = [int(x) for x in mo["info"].cpu()]
+            assert info[0] <= cap and info[1] == 0, "MD list overflow"
+            md = {"value": world * w.n_atoms * md_steps / (md_ms * 1e-3), "unit": "atom-timesteps/s", "steps": md_steps,
+                  "ms_per_step": md_ms / md_steps, "rebuild_every": 10, "skin": 1.0, "dt_ps": md_dt, "list_pairs": info[0],
+                  "gpu_launches": int(lib.launch_count() - n1)}
+            pot.set_option(lib.OPT_PROFILE, 1)
+            del mpos, mvel, mo
+        except Exception as exc:      # an auxiliary leg must not take the headline line with it
+            md = {"error": "%s: %s" % (type(exc).__name__, exc)}
+            pot.set_option(lib.OPT_PROFILE, 1)
 
     if rank != 0:
         if dist is not None:
