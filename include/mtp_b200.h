@@ -22,6 +22,12 @@
  * return without synchronising the host.  Outputs are overwritten, never accumulated.
  * Return value: 0 on success, a negative MTP_E* code otherwise; nothing aborts or throws.
  * There is no CPU fallback: without a CUDA device mtp_create fails with MTP_ECUDA.
+ * Threads: a handle carries options, error text and (for the *_host* calls) staging buffers, so one
+ * handle serves one host thread at a time; different handles are independent (the compiled contraction
+ * kernels are shared through a process-wide cache behind a mutex).  Two calls that use the same workspace
+ * must be ordered on the device (same stream, or events).  Exceptions to "return without synchronising":
+ * mtp_compute_host, mtp_compute_host_pos, mtp_profile_read, mtp_md_run_al (once per grade evaluation) and
+ * the short copies of masses at the start of mtp_md_run.
  */
 #ifndef MTP_B200_H
 #define MTP_B200_H
